@@ -1,0 +1,385 @@
+"""Pins for oracle/wilson_oracle.py against what the paper and the mathematics fix.
+
+None of these tests re-types the oracle's formulas: each compares it with a printed value
+(tests/golden/paper_pins.txt), a closed form, an invariant, an exact identity or a brute-force
+evaluation that takes a different route.  All run on CPU (``-m "not gpu"``).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import wilson_oracle as wo
+from paper_2312_13051_b200 import workloads as wl
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _golden():
+    out = {}
+    with open(os.path.join(HERE, "golden", "paper_pins.txt")) as f:
+        for line in f:
+            line = line.split("#", 1)[0].strip()
+            if "=" in line:
+                k, v = line.split("=", 1)
+                out[k.strip()] = float(v)
+    return out
+
+
+GOLD = _golden()
+
+
+# ------------------------------------------------------------------ closed-form helpers (test side)
+def lower_band_vector(d):
+    """Closed-form lower eigenvector of d.sigma (E = -|d|), gauge irrelevant."""
+    dx, dy, dz = d
+    n = np.sqrt(dx * dx + dy * dy + dz * dz)
+    if dz <= 0:
+        v = np.array([dz - n, dx + 1j * dy])
+    else:  # avoid the cancellation / zero vector at d = (0,0,+|d|)
+        v = np.array([-(dx - 1j * dy), dz + n])
+    return v / np.linalg.norm(v)
+
+
+def qwz_d(kx, ky, M=1.5):
+    return np.array([np.sin(kx), np.sin(ky), np.cos(kx) + np.cos(ky) + M])
+
+
+# ------------------------------------------------------------------ SSH
+def test_ssh_berry_phase_quantized():
+    H, _ = wl.ssh_loop(1.0, 0.5, 50)
+    th, ab, _ = wo.wilson_loop(H, 1)
+    assert abs(wo.wrap_pi(th[0] - np.pi * GOLD["ssh_trivial_phase_over_pi"])) < 1e-12
+    H, _ = wl.ssh_loop(0.5, 1.0, 50)
+    th, ab, _ = wo.wilson_loop(H, 1)
+    assert abs(wo.wrap_pi(th[0] - np.pi * GOLD["ssh_topological_phase_over_pi"])) < 1e-12
+    # both bands: total phase = arg det W = 0 or 2 pi * integer, and the upper band mirrors it
+    th2, _, _ = wo.wilson_loop(H, 2)
+    assert abs(wo.wrap_pi(np.sum(th2))) < 1e-10
+
+
+def test_ssh_position_gauge_needs_closing_phase():
+    """R6: in the position gauge (r_B = 1/2) the loop phase is the periodic-gauge one shifted by
+    -2 pi * <r> = -pi/2 (chiral symmetry puts weight exactly 1/2 on sublattice B); without the
+    closing phase Phi the two dimerizations become indistinguishable."""
+    for (v, w), per in (((1.0, 0.5), 0.0), ((0.5, 1.0), np.pi)):
+        H, phi = wl.ssh_loop(v, w, 50, position_gauge=True)
+        th, _, _ = wo.wilson_loop(H, 1, close=phi)
+        assert abs(wo.wrap_pi(th[0] - (per - np.pi / 2))) < 1e-12
+    Ha, phi = wl.ssh_loop(1.0, 0.5, 50, position_gauge=True)
+    Hb, _ = wl.ssh_loop(0.5, 1.0, 50, position_gauge=True)
+    ta, _, _ = wo.wilson_loop(Ha, 1)
+    tb, _, _ = wo.wilson_loop(Hb, 1)
+    assert abs(wo.wrap_pi(ta[0] - tb[0])) < 1e-10  # a missing Phi is caught by the test above
+
+
+# ------------------------------------------------------------------ QWZ Eq. 4
+def test_qwz_chern_number_is_one_paper_value():
+    H = wl.qwz_grid(100, 100)
+    th, ab, mg = wo.wilson_surface(H[None], 1, direction=1)
+    assert wo.chern_number(th) == int(GOLD["qwz_eq4_chern"])
+    assert abs(-wo.winding(th) - 1.0) < 1e-12
+    assert mg.min() > 0.9
+    # trivial phase of the same model: M = 2.5 -> C = 0
+    th0, _, _ = wo.wilson_surface(wl.qwz_grid(40, 40, M=2.5)[None], 1, direction=1)
+    assert wo.chern_number(th0) == 0
+
+
+def test_qwz_chern_matches_berry_curvature_plaquette_sum():
+    """Independent route (Eq. 5, PAPER.md:69 with A = i<u|d_k u>, Eq. 1): lattice field strength
+    from closed-form eigenvectors, summed over plaquettes.  <u_k|u_{k+dk}> ~ 1 - i A dk, so the
+    counter-clockwise plaquette flux is -arg(prod of links)."""
+    n = 40
+    ks = 2 * np.pi * np.arange(n) / n
+    u = [[lower_band_vector(qwz_d(kx, ky)) for ky in ks] for kx in ks]
+    tot = 0.0
+    for i in range(n):
+        for j in range(n):
+            a, b = u[i][j], u[(i + 1) % n][j]
+            c, d = u[(i + 1) % n][(j + 1) % n], u[i][(j + 1) % n]
+            tot += -np.angle(np.vdot(a, b) * np.vdot(b, c) * np.vdot(c, d) * np.vdot(d, a))
+    C_curv = tot / (2 * np.pi)
+    assert abs(C_curv - round(C_curv)) < 1e-10
+    # Stokes with F_xy = d_x A_y - d_y A_x and a gauge periodic along the loop direction:
+    #   int F = -int dky d_ky (oint dkx A_x)  =>  flow of xbar_x(ky) (Eq. 6) = -C_curvature,
+    #   int F = +int dkx d_kx (oint dky A_y)  =>  flow of xbar_y(kx)         = +C_curvature.
+    # The paper quotes C = 1 from the kx-loop flow; Eq. 5 read literally has the
+    # opposite orientation (reading R15).  Both orientations are pinned here.
+    G = wl.qwz_grid(n, n)[None]
+    th, _, _ = wo.wilson_surface(G, 1, direction=1)   # loops along kx, flow in ky
+    assert wo.chern_number(th) == -int(round(C_curv)) == int(GOLD["qwz_eq4_chern"])
+    th, _, _ = wo.wilson_surface(G, 1, direction=0)   # loops along ky, flow in kx
+    assert wo.chern_number(th) == int(round(C_curv))
+
+
+def test_abelian_loop_equals_scalar_product_of_closed_form_vectors():
+    """m = 1: W = prod_j <u_j|u_{j+1}> is a scalar; u from the closed form, not from eigh."""
+    n1 = 37
+    for ky in (0.3, 2.1, 4.0):
+        Hl = np.array([wl.qwz_eq4(2 * np.pi * i / n1, ky) for i in range(n1)])
+        us = [lower_band_vector(qwz_d(2 * np.pi * i / n1, ky)) for i in range(n1)]
+        Wb = 1.0 + 0j
+        for j in range(n1):
+            Wb *= np.vdot(us[j], us[(j + 1) % n1])
+        th, ab, _ = wo.wilson_loop(Hl, 1)
+        assert abs(wo.wrap_pi(th[0] - np.angle(Wb))) < 1e-12
+        assert abs(ab[0] - abs(Wb)) < 1e-12
+
+
+def test_wilson_matrix_brute_force_index_loops():
+    """4x4 model, m = 2: the ordered product written out with explicit index sums, and
+    sum theta = arg det W = sum_j arg det M_j (mod 2 pi)."""
+    n1 = 9
+    Hl = np.array([wl.bhz4(2 * np.pi * i / n1, 0.7) for i in range(n1)])
+    frames, _ = wo.occupied_frames(Hl, 2)
+    W = wo.wilson_matrix(frames)
+    m = 2
+    acc = [[1.0 + 0j if a == b else 0j for b in range(m)] for a in range(m)]
+    detsum = 0.0
+    for j in range(n1):
+        A, B = frames[j], frames[(j + 1) % n1]
+        M = [[sum(np.conj(A[r, a]) * B[r, b] for r in range(4)) for b in range(m)] for a in range(m)]
+        detsum += np.angle(M[0][0] * M[1][1] - M[0][1] * M[1][0])
+        acc = [[sum(acc[a][c] * M[c][b] for c in range(m)) for b in range(m)] for a in range(m)]
+    assert np.allclose(np.array(acc), W, atol=1e-13)
+    th, _ = wo.eigenphases(W)
+    assert abs(wo.wrap_pi(np.sum(th) - detsum)) < 1e-11
+    # 2x2 closed form: lambda = tr/2 +- sqrt(tr^2/4 - det)
+    tr, det = W[0, 0] + W[1, 1], W[0, 0] * W[1, 1] - W[0, 1] * W[1, 0]
+    lam = np.array([tr / 2 + np.sqrt(tr * tr / 4 - det), tr / 2 - np.sqrt(tr * tr / 4 - det)])
+    assert wo.circ_sorted_distance(th, np.angle(lam)) < 1e-10
+
+
+def test_path_ordering_matters_and_direction_conjugates():
+    """Reversing the path conjugates the spectrum of W (W -> W^dagger up to similarity); a
+    scrambled order does not give the same phases (non-Abelian)."""
+    parts = wl.config5_parts(norb_spatial=4, delta=3.0)
+    n1 = 12
+    Hl = np.array([wl.assemble_config5(parts, 2 * np.pi * np.array([0.13, 0.41, l / n1]))
+                   for l in range(n1)])
+    frames, mg = wo.occupied_frames(Hl, 4)
+    assert mg > 0.2
+    th, _ = wo.eigenphases(wo.wilson_matrix(frames))
+    rev = [frames[0]] + frames[:0:-1]
+    thr, _ = wo.eigenphases(wo.wilson_matrix(rev))
+    assert wo.circ_sorted_distance(th, -thr) < 1e-10
+    perm = [frames[i] for i in (0, 2, 1, 3, 5, 4, 6, 7, 9, 8, 10, 11)]
+    thp, _ = wo.eigenphases(wo.wilson_matrix(perm))
+    assert wo.circ_sorted_distance(th, thp) > 1e-4
+
+
+# ------------------------------------------------------------------ gauge invariance, |lambda| -> 1
+def _random_unitary(rng, m):
+    Z = rng.standard_normal((m, m)) + 1j * rng.standard_normal((m, m))
+    Q, R = np.linalg.qr(Z)
+    return Q * (np.diag(R) / np.abs(np.diag(R)))
+
+
+def test_gauge_invariance_random_unitary_per_k():
+    rng = np.random.default_rng(7)
+    parts = wl.config5_parts(norb_spatial=8, delta=3.0)
+    n1 = 15
+    Hl = np.array([wl.assemble_config5(parts, 2 * np.pi * np.array([0.3, 0.8, l / n1]))
+                   for l in range(n1)])
+    frames, _ = wo.occupied_frames(Hl, 8)
+    th, ab = wo.eigenphases(wo.wilson_matrix(frames))
+    scr = [U @ _random_unitary(rng, 8) for U in frames]
+    th2, ab2 = wo.eigenphases(wo.wilson_matrix(scr))
+    assert wo.circ_sorted_distance(th, th2) < 1e-12
+    assert np.allclose(np.sort(ab), np.sort(ab2), atol=1e-12)
+
+
+def test_eigenvalue_modulus_tends_to_one_on_dense_grids():
+    dev = []
+    for n1 in (25, 100, 400):
+        Hl = np.array([wl.bhz4(2 * np.pi * i / n1, 1.1) for i in range(n1)])
+        _, ab, _ = wo.wilson_loop(Hl, 2)
+        assert np.all(ab <= 1 + 1e-12)
+        dev.append(1 - ab.min())
+    assert dev[0] > dev[1] > dev[2]
+    assert dev[2] < 0.02 and dev[1] / dev[2] > 3.0  # 1 - |lambda| = O(1/N1)
+
+
+# ------------------------------------------------------------------ eigenvalues (S1)
+def test_eigenvalues_closed_forms():
+    rng = np.random.default_rng(3)
+    for _ in range(5):
+        kx, ky = rng.uniform(0, 2 * np.pi, 2)
+        E, _ = wo.eigh_batched(wl.bhz4(kx, ky)[None])
+        e = np.sqrt(np.sin(kx) ** 2 + np.sin(ky) ** 2 + (1 - np.cos(kx) - np.cos(ky)) ** 2)
+        assert np.allclose(E[0], [-e, -e, e, e], atol=1e-13)
+        E, _ = wo.eigh_batched(wl.bbh(kx, ky, 0.5, 1.0)[None])
+        e = np.sqrt((0.5 + np.cos(kx)) ** 2 + np.sin(kx) ** 2 + (0.5 + np.cos(ky)) ** 2 + np.sin(ky) ** 2)
+        assert np.allclose(E[0], [-e, -e, e, e], atol=1e-13)
+
+
+def test_supercell_spectrum_is_folded_primitive_spectrum():
+    """Clean L x L supercell at twist (t1,t2): spectrum = union over n of the 4-band spectra at
+    k = 2 pi (t + n)/L (k = 2 pi n_x / L + theta_x / L)."""
+    L = 4
+    parts = wl.bhz_supercell_parts(L)
+    t1, t2 = 0.23, 0.61
+    E, U = wo.eigh_batched(wl.assemble_supercell(parts, t1, t2)[None])
+    ref = []
+    for nx in range(L):
+        for ny in range(L):
+            kx, ky = 2 * np.pi * (t1 + nx) / L, 2 * np.pi * (t2 + ny) / L
+            e = np.sqrt(np.sin(kx) ** 2 + np.sin(ky) ** 2 + (1 - np.cos(kx) - np.cos(ky)) ** 2)
+            ref += [-e, -e, e, e]
+    assert np.allclose(E[0], np.sort(ref), atol=1e-12)
+    H = wl.assemble_supercell(parts, t1, t2)
+    assert np.allclose(H, H.conj().T)
+    assert abs(np.trace(H).real - E[0].sum()) < 1e-10
+    assert np.linalg.norm(H @ U[0] - U[0] * E[0]) < 1e-12
+    # periodic gauge: H(t + 1) = H(t)
+    assert np.allclose(wl.assemble_supercell(parts, t1 + 1, t2), H)
+
+
+def test_zheev_agrees_with_zheevd_R14():
+    import scipy.linalg as sl
+    H = wl.assemble_supercell(wl.config3_parts(0, L=5), 0.3, 0.7)
+    E, _ = wo.eigh_batched(H[None])
+    Eev = sl.eigh(H, eigvals_only=True, driver="ev")
+    assert np.max(np.abs(E[0] - Eev)) < 1e-13 * np.linalg.norm(H, 2) * 10
+
+
+# ------------------------------------------------------------------ folding identity (large-m product)
+def test_supercell_folding_identity():
+    """Exact at finite N1.  Clean L x 1... here L x L supercell in the *position* gauge along x
+    with closing Phi = e^{-i 2 pi x / L}: {lambda^L} = eigenvalues of the primitive 4-band loop
+    with L N1 points at ky = 2 pi (t2 + n)/L, each repeated L times."""
+    L, n1 = 3, 7
+    parts = wl.bhz_supercell_parts(L)
+    t2 = 0.37
+    xs = np.repeat(np.arange(L), L * 4).astype(float)  # x coordinate of each orbital (site = L x + y)
+    lam_super = []
+    frames = []
+    for i in range(n1):
+        t1 = i / n1
+        Hper = wl.assemble_supercell(parts, t1, t2)
+        D = np.exp(1j * 2 * np.pi * t1 * xs / L)  # position gauge: H_pos = D^dagger H D
+        Hpos = (np.conj(D)[:, None] * Hper) * D[None, :]
+        E, V = np.linalg.eigh(Hpos)
+        frames.append(V[:, : 2 * L * L])
+    phi = np.exp(-1j * 2 * np.pi * xs / L)
+    W = wo.wilson_matrix(frames, close=phi)
+    lam_super = np.linalg.eigvals(W) ** L
+    lam_prim = []
+    for ny in range(L):
+        ky = 2 * np.pi * (t2 + ny) / L
+        Hl = np.array([wl.bhz4(2 * np.pi * i / (L * n1), ky) for i in range(L * n1)])
+        fr, _ = wo.occupied_frames(Hl, 2)
+        lam_prim += list(np.linalg.eigvals(wo.wilson_matrix(fr))) * L
+    lam_prim = np.array(lam_prim)
+    # optimal matching of two multisets of complex numbers
+    from scipy.optimize import linear_sum_assignment
+    cost = np.abs(lam_super[:, None] - lam_prim[None, :])
+    r, c = linear_sum_assignment(cost)
+    assert cost[r, c].max() < 1e-11
+
+
+# ------------------------------------------------------------------ spin-resolved (S6)
+def test_bhz_spin_resolved_windings_and_block_reduction():
+    n1, n2 = 60, 41
+    H = wl.config1_grid(n1, n2)
+    S = wl.bhz4_spin_z()
+    lo, hi, pso = wo.spin_resolved_surface(H[None], 2, 1, S)
+    assert np.allclose(np.abs(pso), GOLD["pso_abs_eigenvalue_no_soc"], atol=1e-12)  # [H,S]=0
+    w_lo, w_hi = wo.winding(lo), wo.winding(hi)
+    assert abs(abs(w_lo) - GOLD["bhz_sector_abs_winding"]) < 1e-10
+    assert abs(w_lo + w_hi - GOLD["bhz_total_winding"]) < 1e-10
+    th, _, _ = wo.wilson_surface(H[None], 2, 1)
+    assert abs(wo.winding(th) - GOLD["bhz_total_winding"]) < 1e-10
+    # R11: lower sector (S_z = -1) winds +1 => C_down = -1, C_up = +1, C_s = +1 (paper sign)
+    assert round(w_lo) == 1 and round(w_hi) == -1
+    # block reduction: spin-down block (indices 1,3) is -sin kx sx + sin ky sy + M sz etc.
+    for j in (0, 5, 17):
+        ky = 2 * np.pi * j / n2
+        for sgn, sector in ((-1.0, lo), (+1.0, hi)):
+            Hl = np.array([sgn * np.sin(2 * np.pi * i / n1) * wl.sx + np.sin(ky) * wl.sy
+                           + (1 - np.cos(2 * np.pi * i / n1) - np.cos(ky)) * wl.sz for i in range(n1)])
+            tb, _, _ = wo.wilson_loop(Hl, 1)
+            assert abs(wo.wrap_pi(tb[0] - sector[j, 0])) < 1e-10
+    # the union of the sector phases is the full spectrum when [H,S]=0
+    for j in range(n2):
+        assert wo.circ_sorted_distance(th[j], np.concatenate([lo[j], hi[j]])) < 1e-10
+
+
+def test_spin_resolved_with_spin_mixing_keeps_quantized_sector_windings():
+    """with spin-orbit coupling PSO eigenvalues leave +-1 but stay gapped."""
+    n1, n2 = 40, 31
+    H = wl.config1_grid(n1, n2)
+    mix = 0.3 * np.kron(wl.sy, wl.sx)  # anticommutes with neither mass term entirely; breaks S_z
+    H = H + mix
+    S = wl.bhz4_spin_z()
+    lo, hi, pso = wo.spin_resolved_surface(H[None], 2, 1, S)
+    assert np.abs(pso).min() < 1 - 1e-2 and np.abs(pso).min() > 0.2  # left +-1, still gapped
+    assert abs(abs(wo.winding(lo)) - 1) < 1e-9 and abs(wo.winding(lo) + wo.winding(hi)) < 1e-9
+
+
+# ------------------------------------------------------------------ nested (S5)
+@pytest.mark.parametrize("gamma,key", [(0.5, "bbh_nested_polarization_topological"),
+                                       (1.5, "bbh_nested_polarization_trivial")])
+def test_bbh_nested_polarization(gamma, key):
+    n = 40
+    H = wl.config2_grid(n, n, gamma=gamma)
+    for base in (0, 11):
+        for band in (0, 1):
+            th1, thn = wo.nested_wilson(H, 2, base=base, wb_lo=band, wb_hi=band + 1)
+            assert wo.nested_polarization(thn) == GOLD[key]
+            p = (-thn[0] / (2 * np.pi)) % 1.0
+            assert min(abs(p - GOLD[key]), abs(p - GOLD[key] - 1), abs(p - GOLD[key] + 1)) < 1e-9
+    # Wannier bands are gapped at 0 and 1/2 and symmetric about 0
+    nu = th1 / (2 * np.pi)
+    assert np.all(np.abs(nu) > 0.02) and np.all(np.abs(nu) < 0.48)
+    assert np.allclose(nu[:, 0], -nu[:, 1], atol=1e-10)
+
+
+def test_nested_first_level_matches_plain_surface():
+    H = wl.config2_grid(24, 20)
+    th1, _ = wo.nested_wilson(H, 2)
+    th, _, _ = wo.wilson_surface(H[None], 2, 1)
+    for j in range(20):
+        assert wo.circ_sorted_distance(th1[j], th[j]) < 1e-12
+
+
+# ------------------------------------------------------------------ comparator and invariants
+def test_comparator_handles_cut_and_degenerate_clusters():
+    a = np.array([-np.pi + 1e-12, 0.0, 0.0, 0.0, 1.0])
+    b = np.array([0.0, 0.0, 0.0, 1.0, np.pi - 1e-12])
+    assert wo.circ_sorted_distance(a, b) < 1e-11
+    assert abs(wo.circ_sorted_distance(np.array([0.1, 0.5]), np.array([0.1, 0.6])) - 0.1) < 1e-15
+
+
+def test_winding_counts_turns():
+    i = np.arange(50)
+    for w in (-2, -1, 0, 1, 3):
+        th = wo.wrap_pi(2 * np.pi * w * i / 50 + 0.3)[:, None]
+        assert abs(wo.winding(th) - w) < 1e-12
+
+
+# ------------------------------------------------------------------ workload sanity (harness asserts)
+def test_config5_gap_and_hermiticity():
+    parts = wl.config5_parts()
+    rng = np.random.default_rng(0)
+    gaps = []
+    for _ in range(40):
+        k = rng.uniform(0, 2 * np.pi, 3)
+        H = wl.assemble_config5(parts, k)
+        assert np.allclose(H, H.conj().T)
+        E = np.linalg.eigvalsh(H)
+        gaps.append(E[32] - E[31])
+    assert min(gaps) >= 0.2
+
+
+def test_config3_and_4_structure():
+    p3 = wl.config3_parts(0, L=4)
+    H = wl.assemble_supercell(p3, 0.1, 0.2)
+    assert np.allclose(H, H.conj().T)
+    on = wl.config4_onsite(20)
+    nz = [(x, y) for x in range(20) for y in range(20) if np.abs(on[x, y]).max() > 0]
+    assert len(nz) == 20
+    for x, y in nz:
+        assert np.allclose(np.abs(np.diag(on[x, y])), 0.3)
+    S = wl.supercell_spin_z(3)
+    assert S.shape == (36,) and set(S) == {1.0, -1.0}
