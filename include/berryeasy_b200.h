@@ -1,0 +1,161 @@
+/*
+ * berryeasy_b200.h -- C ABI of the B200-native Wilson-loop hot path of BerryEasy
+ * (A. C. Tyner, arXiv 2312.13051; citations "PAPER.md:<line>" refer to /root/reference/PAPER.md,
+ * "R<n>" to the readings listed in DESIGN.md).
+ *
+ * The library takes an already assembled grid of Bloch / supercell Hamiltonians H(k) and returns
+ * Wannier-centre-charge phases.  Every step runs in hand-written sm_100a CUDA kernels; there is
+ * no cuSOLVER / cuBLAS inside and no CPU fallback.
+ *
+ * Common conventions
+ * ------------------
+ *  - complex128 = interleaved (re, im) pairs of IEEE double, 16-byte aligned.
+ *  - A Hamiltonian is a dense row-major [N][N] complex128 array, Hermitian, full storage (only
+ *    the upper triangle H[r][c], c >= r, is read).
+ *  - H_grid layout: [batch][dims[0]]..[dims[ndim-1]][N][N], last grid axis fastest (be_grid).
+ *  - "d" prefixed pointers are DEVICE pointers, "h" prefixed pointers are HOST pointers.
+ *  - Ownership: the caller owns every data buffer; the library never frees them and keeps no
+ *    reference past the call.  be_ctx owns only scratch memory (allocated lazily with
+ *    cudaMallocAsync-free plain cudaMalloc, grown on demand, released by be_destroy).
+ *  - Asynchrony: device entry points enqueue all work on the context's stream and return; outputs
+ *    are valid once the caller synchronises that stream.  (Scratch growth may synchronise.)
+ *    *_host entry points are synchronous: they return after the host outputs are written.
+ *  - Errors: return value 0 = BE_OK; negative = argument / shape / alignment error detected on the
+ *    host before anything is enqueued; positive = CUDA runtime error (cudaError_t value).
+ *    Numerical trouble is never an error return: see d_info / d_mingap.
+ *  - Thread safety: one context per host thread; no global state.
+ *  - Phases are returned in radians, ascending, on the branch (-pi, pi] (R7).  The library's
+ *    W = prod_j U_j^dagger U_{j+1} is the Hermitian conjugate of the paper's product (Eq. 2,
+ *    PAPER.md:38), so the paper's WCC is xbar_n = -theta_n / 2 pi (mod 1) (R3).
+ */
+#ifndef BERRYEASY_B200_H
+#define BERRYEASY_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BE_OK                 0
+#define BE_ERR_NULL          -1   /* required pointer is NULL                                  */
+#define BE_ERR_SHAPE         -2   /* N, n_occ, dims, dir ... out of range                      */
+#define BE_ERR_ALIGN         -3   /* pointer not 16-byte (complex) / 8-byte (double) aligned   */
+#define BE_ERR_UNSUPPORTED   -4   /* valid request this build cannot serve (stated per call)   */
+#define BE_ERR_NOMEM         -5   /* scratch allocation failed                                 */
+
+typedef struct be_ctx be_ctx;   /* opaque; owns scratch only */
+
+typedef struct {
+  int     ndim;      /* number of grid axes after the batch axis, 1..3                          */
+  int64_t batch;     /* independent realizations, >= 1                                          */
+  int     dims[3];   /* points per grid axis; unused trailing entries ignored                   */
+  int     N;         /* orbitals: every H is [N][N]                                             */
+} be_grid;
+
+/* Create / destroy a context bound to a CUDA stream (cudaStream_t passed as void*; NULL = the
+ * legacy default stream).  The current CUDA device at creation time is used for all scratch. */
+int be_create(be_ctx** out, void* cuda_stream);
+int be_destroy(be_ctx* ctx);
+const char* be_strerror(int code);
+
+/* Upper bound, in bytes, on the scratch one call with these shapes allocates (informative; op:
+ * 0 = eigh, 1 = wilson loop, 2 = nested, 3 = spin resolved). */
+size_t be_workspace_bytes(const be_grid* grid, int n_occ, int op);
+
+/* Cap on the scratch used for per-chunk work buffers (default 48 GiB).  Work is processed in
+ * chunks of whole loops sized to stay under the cap. */
+int be_set_workspace_limit(be_ctx* ctx, size_t bytes);
+
+/* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */
+int64_t be_launch_count(const be_ctx* ctx);
+
+/*
+ * S1 -- batched Hermitian eigensolve ("exact diagonalization of a discretized
+ * Hamiltonian at many points in reciprocal space").
+ *   dH     [count][N][N] complex128, Hermitian, not modified.
+ *   dE     [count][N] double: all eigenvalues, ascending.
+ *   dU     [count][N][n_vec] complex128, may be NULL: U[c][r][v] = component r of the eigenvector of
+ *          the v-th lowest eigenvalue; columns orthonormal.  0 <= n_vec <= N.
+ *   d_info [count] int, may be NULL: 0 = converged; >0 = number of vectors whose inverse iteration
+ *          or Jacobi sweep limit did not meet its tolerance.
+ * Paths: N <= 8 cyclic one-sided Jacobi on the shifted matrix, one thread per matrix; otherwise
+ * blocked Householder tridiagonalization + bisection + inverse iteration + compact-WY
+ * back-transform, all matrices of the batch advanced in lock step.
+ */
+int be_eigh_batched(be_ctx* ctx, const void* dH, int64_t count, int N, int n_vec,
+                    double* dE, void* dU, int* d_info);
+
+/*
+ * S1-S4 -- hybrid Wannier-centre-charge surface (``WSurf``, Eq. 2
+ * Eq. 3): for every batch entry and every grid point of the axes other than
+ * ``dir`` one discretized, path-ordered Wilson loop along axis ``dir`` over the n_occ lowest bands
+ *     W = prod_{j=0}^{N1-1} U_j^dagger U_{j+1},   U_{N1} := diag(Phi) U_0,   theta = arg eig(W).
+ * No unitarization of links or of W (R4); exactly N1 = dims[dir] links, all points distinct (R5).
+ *   d_close  [N] complex128 unit-modulus Phi_alpha = exp(-i G.r_alpha) (R6), NULL = identity.
+ *   d_theta  [loops][n_occ] double, loops = batch * prod(dims other than dir), row-major over
+ *            (batch, remaining axes in order); ascending in (-pi, pi].
+ *   d_abs    same shape, |lambda_n| in the order of d_theta; may be NULL.
+ *   d_mingap [loops] double, min over the loop of E[n_occ]-E[n_occ-1] (+inf if n_occ == N);
+ *            a value <= 1e-8 ||H|| marks a loop without a spectral gap (R8); may be NULL.
+ */
+int be_wilson_loop(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_occ, int dir,
+                   const void* d_close, double* d_theta, double* d_abs, double* d_mingap);
+
+/*
+ * S5 -- nested Wilson loop (``WNWL``, Eq. 8; R9).
+ * grid->ndim >= 2.  For every point of axis dir2 (and every batch entry / remaining axis) the loop
+ * along dir1 is started at index ``base``; the right eigenvectors of W whose phases rank
+ * wb_lo..wb_hi-1 on the branch (theta_cut - 2 pi, theta_cut] span the Wannier-band subspace V_S
+ * (orthonormalized); w = U_base V_S; a second loop of w runs along dir2 (closing phase d_close2).
+ *   d_theta1       [batch][other][dims[dir2]][n_occ]: first-level phases, branch (-pi, pi].
+ *   d_theta_nested [batch][other][wb_hi-wb_lo]: nested phases; polarization p = -sum/2pi mod 1.
+ * This build: n_occ <= 2 uses closed-form eigenvectors; larger n_occ uses inverse iteration on
+ * W - lambda I and requires wb_hi - wb_lo <= 32.
+ */
+int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_occ,
+                     int dir1, int dir2, int base, int wb_lo, int wb_hi, double theta_cut,
+                     const void* d_close1, const void* d_close2,
+                     double* d_theta1, double* d_theta_nested);
+
+/*
+ * S6 -- spin-resolved Wilson loop (``WSpinSurf``): at every k the reduced
+ * projected spin operator U^dagger S U (the non-zero block of P S P) is
+ * diagonalized, S_red = V Sigma V^dagger (ascending); the occupied frame is rotated into the
+ * lower sector U V[:, :m_lo] and the upper sector U V[:, m_lo:] and each sector is looped (R10).
+ *   dS         S_is_diag = 1: [N] double (real diagonal);  0: [N][N] complex128 row-major.
+ *   m_lo       size of the lower sector; -1 = n_occ / 2.
+ *   d_theta_lo [loops][m_lo], d_theta_hi [loops][n_occ-m_lo] (either may be NULL).
+ *   d_pso      [loops][N1][n_occ] PSO eigenvalues ascending (``spin_spectrum``);
+ *              may be NULL.
+ */
+int be_spin_resolved_wilson(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_occ,
+                            int dir, const void* dS, int S_is_diag, int m_lo, const void* d_close,
+                            double* d_theta_lo, double* d_theta_hi, double* d_pso);
+
+/*
+ * S7 -- winding of Theta_i = sum_n theta_n over a closed transverse cycle (Eq. 6):
+ *   d_theta [n_cycles][n_points][m]  ->  d_wind [n_cycles] double,
+ *   wind = (1/2pi) sum_i wrap(Theta_{i+1} - Theta_i), indices cyclic.  Paper's C = -wind (R3).
+ */
+int be_winding(be_ctx* ctx, const double* d_theta, int64_t n_cycles, int n_points, int m,
+               double* d_wind);
+
+/*
+ * Host-buffer variants (end-to-end path): h* pointers are host memory (pinned recommended).  The
+ * grid is streamed to the device in chunks of whole loops, overlapped with compute on an internal
+ * copy stream; results are copied back before return.  Semantics as the device calls above.
+ * Requires dir == ndim-1 (loops contiguous in memory), else BE_ERR_UNSUPPORTED.
+ */
+int be_wilson_loop_host(be_ctx* ctx, const void* hH_grid, const be_grid* grid, int n_occ, int dir,
+                        const void* h_close, double* h_theta, double* h_abs, double* h_mingap);
+int be_spin_resolved_wilson_host(be_ctx* ctx, const void* hH_grid, const be_grid* grid, int n_occ,
+                                 int dir, const void* hS, int S_is_diag, int m_lo,
+                                 const void* h_close, double* h_theta_lo, double* h_theta_hi,
+                                 double* h_pso);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BERRYEASY_B200_H */

@@ -1,0 +1,172 @@
+// Shared declarations of the CUDA path: context, launch bookkeeping, complex helpers, the batched
+// ZGEMM interface and the internal stage entry points.  Nothing in here is used by oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <math.h>
+#include "../../include/berryeasy_b200.h"
+
+typedef double2 cplx;
+
+__host__ __device__ __forceinline__ cplx mkc(double r, double i) { cplx z; z.x = r; z.y = i; return z; }
+__host__ __device__ __forceinline__ cplx cadd(cplx a, cplx b) { return mkc(a.x + b.x, a.y + b.y); }
+__host__ __device__ __forceinline__ cplx csub(cplx a, cplx b) { return mkc(a.x - b.x, a.y - b.y); }
+__host__ __device__ __forceinline__ cplx cmul(cplx a, cplx b) { return mkc(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+// conj(a) * b
+__host__ __device__ __forceinline__ cplx cmulc(cplx a, cplx b) { return mkc(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x); }
+__host__ __device__ __forceinline__ cplx cconj(cplx a) { return mkc(a.x, -a.y); }
+__host__ __device__ __forceinline__ cplx cscale(double s, cplx a) { return mkc(s * a.x, s * a.y); }
+__host__ __device__ __forceinline__ double cabs2(cplx a) { return a.x * a.x + a.y * a.y; }
+__device__ __forceinline__ double cabs1(cplx a) { return fabs(a.x) + fabs(a.y); }
+__device__ __forceinline__ cplx cdiv(cplx a, cplx b) {
+  // Smith's algorithm
+  if (fabs(b.x) >= fabs(b.y)) {
+    double r = b.y / b.x, den = b.x + b.y * r;
+    return mkc((a.x + a.y * r) / den, (a.y - a.x * r) / den);
+  } else {
+    double r = b.x / b.y, den = b.x * r + b.y;
+    return mkc((a.x * r + a.y) / den, (a.y * r - a.x) / den);
+  }
+}
+// acc += a*b
+__device__ __forceinline__ void cfma(cplx& acc, cplx a, cplx b) {
+  acc.x = fma(a.x, b.x, acc.x); acc.x = fma(-a.y, b.y, acc.x);
+  acc.y = fma(a.x, b.y, acc.y); acc.y = fma(a.y, b.x, acc.y);
+}
+// acc += conj(a)*b
+__device__ __forceinline__ void cfmac(cplx& acc, cplx a, cplx b) {
+  acc.x = fma(a.x, b.x, acc.x); acc.x = fma(a.y, b.y, acc.x);
+  acc.y = fma(a.x, b.y, acc.y); acc.y = fma(-a.y, b.x, acc.y);
+}
+// acc -= a*b
+__device__ __forceinline__ void cfms(cplx& acc, cplx a, cplx b) {
+  acc.x = fma(-a.x, b.x, acc.x); acc.x = fma(a.y, b.y, acc.x);
+  acc.y = fma(-a.x, b.y, acc.y); acc.y = fma(-a.y, b.x, acc.y);
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ cplx warp_sum(cplx v) { return mkc(warp_sum(v.x), warp_sum(v.y)); }
+
+// Block-wide sum (all threads get the result).  ``red`` : shared scratch of >= 33 entries of T.
+template <typename T>
+__device__ __forceinline__ T block_sum(T v, T* red) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  v = warp_sum(v);
+  __syncthreads();
+  if (lane == 0) red[w] = v;
+  __syncthreads();
+  if (w == 0) {
+    T t = (lane < nw) ? red[lane] : T{};
+    t = warp_sum(t);
+    if (lane == 0) red[32] = t;
+  }
+  __syncthreads();
+  return red[32];
+}
+
+// ---------------------------------------------------------------------------------------------
+struct be_ctx {
+  cudaStream_t stream;
+  cudaStream_t copy_stream;   // host variants only
+  int device;
+  int sm_count;
+  size_t ws_limit;
+  int64_t launches;
+  // scratch arena (bump allocated per call, grown on demand)
+  char* arena;
+  size_t arena_bytes;
+  size_t arena_used;
+  int gemm_attr_set;
+};
+
+#define BE_CUDA(x) do { cudaError_t e__ = (x); if (e__ != cudaSuccess) return (int)e__; } while (0)
+#define BE_TRY(x) do { int r__ = (x); if (r__ != BE_OK) return r__; } while (0)
+
+// bump allocator on the context arena; pointers stay valid until arena_reset
+int  be_arena_reserve(be_ctx* ctx, size_t bytes);   // ensure capacity (may sync + realloc); resets
+void* be_arena_alloc(be_ctx* ctx, size_t bytes);    // 256-byte aligned; NULL when exhausted
+static inline size_t be_align256(size_t b) { return (b + 255) & ~(size_t)255; }
+
+// ---------------------------------------------------------------------------------------------
+// Batched complex GEMM on the FP64 tensor cores (DMMA.8x8x4), column-major operands:
+//   C[b] = alpha * op(A[b]) * op(B[b]) + beta * C[b]
+// op: 0 = N, 1 = T (transpose), 2 = C (conjugate transpose), 3 = J (conjugate, no transpose).
+// Batch b = o * inner + i;  X[b] = X + o * sXo + i * sXi (element strides).
+enum { BE_OP_N = 0, BE_OP_T = 1, BE_OP_C = 2, BE_OP_J = 3 };
+struct ZgemmParams {
+  int M, N, K;
+  const cplx* A; int lda; int64_t sAi, sAo;
+  const cplx* B; int ldb; int64_t sBi, sBo;
+  cplx* C; int ldc; int64_t sCi, sCo;
+  int inner; int64_t batch;
+  int ringB;          // B uses inner index (i + 1) % inner (next frame of the loop)
+  const cplx* phiB;   // with ringB: when i == phi_at, B(k, n) is multiplied by phiB[k] (opB = N)
+  int phi_at;         // inner index of the link that crosses the zone boundary (default inner-1)
+  cplx alpha, beta;
+  int lower;          // 1: skip tiles strictly above the diagonal (C lower triangle, tile granular)
+};
+int be_zgemm(be_ctx* ctx, int opA, int opB, const ZgemmParams& p);
+static inline ZgemmParams zgemm_simple(int M, int N, int K, const cplx* A, int lda, int64_t sA,
+                                       const cplx* B, int ldb, int64_t sB, cplx* C, int ldc,
+                                       int64_t sC, int64_t batch) {
+  ZgemmParams p;
+  p.M = M; p.N = N; p.K = K;
+  p.A = A; p.lda = lda; p.sAi = 0; p.sAo = sA;
+  p.B = B; p.ldb = ldb; p.sBi = 0; p.sBo = sB;
+  p.C = C; p.ldc = ldc; p.sCi = 0; p.sCo = sC;
+  p.inner = 1; p.batch = batch;
+  p.ringB = 0; p.phiB = nullptr; p.phi_at = -1;
+  p.alpha = mkc(1.0, 0.0); p.beta = mkc(0.0, 0.0); p.lower = 0;
+  return p;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Mapping (loop, j) -> matrix index inside H_grid for a loop direction ``dir`` (units: matrices).
+struct GridMap {
+  int ndim, dir, n1;
+  int shift;           // loop point j reads grid index (j + shift) % n1 along dir (nested: base)
+  int dims[3];
+  int64_t stride[3];
+  int64_t batch_stride;
+  int64_t loops;       // batch * prod(dims other than dir)
+};
+__host__ __device__ inline int64_t gridmap_index(const GridMap& g, int64_t loop, int j) {
+  int64_t idx = loop, off = 0;
+  for (int a = g.ndim - 1; a >= 0; --a) {
+    if (a == g.dir) continue;
+    int64_t i = idx % g.dims[a];
+    idx /= g.dims[a];
+    off += i * g.stride[a];
+  }
+  int jj = j + g.shift; if (jj >= g.n1) jj -= g.n1;
+  return off + idx * g.batch_stride + (int64_t)jj * g.stride[g.dir];
+}
+
+// ---------------------------------------------------------------------------------------------
+// Stage entry points (host functions enqueueing kernels on ctx->stream)
+
+// Frames-producing eigensolve for ``cnt`` matrices gathered from H via (loop0.., map):
+//   matrix c = (loop0 + c / map.n1, c % map.n1).  Outputs:
+//   E [cnt][N] ascending;  X [cnt][nv][N] column-major frames (X[c][v*N + r] = U[r][v]);
+//   info [cnt] or NULL.  Scratch comes from the context arena (caller reserved it).
+int be_eigh_frames(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt,
+                   int N, int nv, double* E, cplx* X, int* info);
+size_t be_eigh_scratch_bytes(int64_t cnt, int N, int nv);
+
+// eigenphases of ``cnt`` general complex m x m matrices W (column-major, stride m*m, destroyed):
+//   theta [cnt][m] ascending in (-pi, pi], absl [cnt][m] or NULL.
+int be_eigenphases(be_ctx* ctx, cplx* W, int64_t cnt, int m, double* theta, double* absl);
+size_t be_eigenphases_scratch_bytes(int64_t cnt, int m);
+int be_eigenvalues_general(be_ctx* ctx, cplx* W, int64_t cnt, int m, cplx* lam, int* fail);
+
+int be_eigh_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N,
+                  int nv, double* E, cplx* X, int* info);
+int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N,
+                  int nv, double* E, cplx* X, int* info);
+size_t be_eigh_large_scratch_bytes(int64_t cnt, int N, int nv);
+int be_frames_to_public(be_ctx* ctx, const cplx* X, cplx* U, int64_t cnt, int N, int nv);

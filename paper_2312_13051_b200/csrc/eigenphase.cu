@@ -1,0 +1,306 @@
+// S4 -- eigenphases theta_n = arg lambda_n(W) of the Wilson matrices (Eq. 2,
+// PAPER.md:127 Eq. 8 "Im Ln").  W is NOT unitary at finite Delta k and is not unitarized (R4), so
+// this is a general complex eigenvalue problem:
+//   m = 1, 2 : closed form, one thread per matrix
+//   m > 2    : Householder reduction to Hessenberg form, then explicit single-shift complex QR on
+//              the active window (eigenvalues only), one CTA per matrix, W resident in L2.
+// Output sorted ascending on the branch (-pi, pi] (R7) by a rank sort.
+#include "be_common.cuh"
+#include <float.h>
+
+namespace {
+
+__device__ __forceinline__ cplx csqrt_(cplx z) {
+  const double r = hypot(z.x, z.y);
+  if (r == 0.0) return mkc(0.0, 0.0);
+  double a = sqrt(0.5 * (r + fabs(z.x)));
+  double b = 0.5 * z.y / a;
+  if (z.x >= 0.0) return mkc(a, b);
+  return mkc(fabs(b), copysign(a, z.y));
+}
+
+// eigenvalues of [[a, b], [c, d]]
+__device__ __forceinline__ void eig2(cplx a, cplx b, cplx c, cplx d, cplx& l1, cplx& l2) {
+  const cplx h = mkc(0.5 * (a.x - d.x), 0.5 * (a.y - d.y));
+  const cplx disc = csqrt_(cadd(cmul(h, h), cmul(b, c)));
+  const cplx mid = mkc(0.5 * (a.x + d.x), 0.5 * (a.y + d.y));
+  // larger-modulus root first, the other from the determinant (avoids cancellation)
+  const cplx p = cadd(mid, disc), q = csub(mid, disc);
+  const cplx big = (cabs2(p) >= cabs2(q)) ? p : q;
+  const cplx det = csub(cmul(a, d), cmul(b, c));
+  l1 = big;
+  l2 = (cabs2(big) > 0.0) ? cdiv(det, big) : mkc(0.0, 0.0);
+}
+
+__global__ void k_eig_small(const cplx* __restrict__ W, int64_t cnt, int m, cplx* __restrict__ lam) {
+  const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (c >= cnt) return;
+  if (m == 1) { lam[c] = W[c]; return; }
+  const cplx* w = W + c * 4;   // column-major 2x2: w[0]=a, w[1]=c, w[2]=b, w[3]=d
+  cplx l1, l2;
+  eig2(w[0], w[2], w[1], w[3], l1, l2);
+  lam[c * 2] = l1; lam[c * 2 + 1] = l2;
+}
+
+// ------------------------------------------------------------------------------------------
+__global__ void k_hessenberg(cplx* __restrict__ W, int m) {
+  extern __shared__ cplx vsh[];   // v[m], y[m]
+  __shared__ double redd[33];
+  __shared__ cplx sh_alpha;
+  cplx* v = vsh; cplx* y = vsh + m;
+  cplx* H = W + blockIdx.x * (int64_t)m * m;
+  const int tid = threadIdx.x, nt = blockDim.x, warp = tid >> 5, lane = tid & 31, nw = nt >> 5;
+  for (int k = 0; k < m - 2; ++k) {
+    double ss = 0.0;
+    for (int r = k + 1 + tid; r < m; r += nt) {
+      const cplx x = H[r + (int64_t)k * m];
+      if (r == k + 1) sh_alpha = x; else ss += cabs2(x);
+    }
+    const double xn2 = block_sum(ss, redd);
+    const cplx alpha = sh_alpha;
+    if (xn2 == 0.0 && alpha.y == 0.0) { __syncthreads(); continue; }
+    const double beta = -copysign(sqrt(cabs2(alpha) + xn2), alpha.x);
+    const cplx tau = mkc((beta - alpha.x) / beta, -alpha.y / beta);
+    const cplx scale = cdiv(mkc(1.0, 0.0), mkc(alpha.x - beta, alpha.y));
+    for (int r = k + 1 + tid; r < m; r += nt) {
+      if (r == k + 1) { v[r] = mkc(1.0, 0.0); H[r + (int64_t)k * m] = mkc(beta, 0.0); }
+      else { v[r] = cmul(H[r + (int64_t)k * m], scale); H[r + (int64_t)k * m] = mkc(0.0, 0.0); }
+    }
+    __syncthreads();
+    // left: H[k+1:, j] -= conj(tau) v (v^H H[k+1:, j]),  j > k      (warp per column)
+    const cplx ctau = cconj(tau);
+    for (int j = k + 1 + warp; j < m; j += nw) {
+      cplx* col = H + (int64_t)j * m;
+      cplx dot = mkc(0.0, 0.0);
+      for (int r = k + 1 + lane; r < m; r += 32) cfmac(dot, v[r], col[r]);
+      dot = cmul(ctau, warp_sum(dot));
+      for (int r = k + 1 + lane; r < m; r += 32) cfms(col[r], v[r], dot);
+    }
+    __syncthreads();
+    // right: H[:, k+1:] -= tau (H[:, k+1:] v) v^H                    (thread per row)
+    for (int i = tid; i < m; i += nt) {
+      cplx acc = mkc(0.0, 0.0);
+      for (int j = k + 1; j < m; ++j) cfma(acc, H[i + (int64_t)j * m], v[j]);
+      acc = cmul(tau, acc);
+      for (int j = k + 1; j < m; ++j) {
+        cplx h = H[i + (int64_t)j * m];
+        cfms(h, acc, cconj(v[j]));
+        H[i + (int64_t)j * m] = h;
+      }
+    }
+    __syncthreads();
+  }
+  (void)y;
+}
+
+// Givens: c real, s complex with [c s; -conj(s) c] [a; b] = [r; 0]
+__device__ __forceinline__ void givens(cplx a, cplx b, double& c, cplx& s) {
+  const double nb2 = cabs2(b);
+  if (nb2 == 0.0) { c = 1.0; s = mkc(0.0, 0.0); return; }
+  const double na2 = cabs2(a);
+  if (na2 == 0.0) { c = 0.0; const double nb = sqrt(nb2); s = mkc(b.x / nb, -b.y / nb); return; }
+  const double na = sqrt(na2), nrm = sqrt(na2 + nb2);
+  c = na / nrm;
+  const cplx ph = mkc(a.x / na, a.y / na);          // a / |a|
+  s = cscale(1.0 / nrm, cmulc(b, ph));              // (a/|a|) conj(b) / nrm
+}
+
+constexpr int QR_MAXOWN = 8;   // columns / rows owned per thread: m <= 8 * blockDim
+
+// Explicit single-shift QR on the upper Hessenberg matrix H (column-major m x m), eigenvalues only.
+__global__ void k_hqr(cplx* __restrict__ W, int m, cplx* __restrict__ lam, int* __restrict__ fail) {
+  extern __shared__ double shq[];       // cs[m] (double), sn[m] (cplx)
+  double* cs = shq;
+  cplx* sn = (cplx*)(shq + ((m + 1) & ~1));
+  __shared__ int s_l;
+  __shared__ cplx s_sig;
+  __shared__ int redi[33];
+  cplx* H = W + blockIdx.x * (int64_t)m * m;
+  cplx* out = lam + blockIdx.x * (int64_t)m;
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const double eps = DBL_EPSILON;
+  int hi = m - 1, its = 0, nfail = 0;
+  while (hi >= 0) {
+    // ---- deflation scan: largest l in (0, hi] with negligible H[l][l-1], else 0
+    int best = 0;
+    for (int k = hi - tid; k >= 1; k -= nt) {
+      const double sub = cabs1(H[k + (int64_t)(k - 1) * m]);
+      double sd = cabs1(H[(k - 1) + (int64_t)(k - 1) * m]) + cabs1(H[k + (int64_t)k * m]);
+      if (sd == 0.0) sd = 1.0;
+      if (sub <= eps * sd) { best = k; break; }   // first hit going down is this thread's largest
+    }
+    // block max
+    for (int o = 16; o > 0; o >>= 1) best = max(best, __shfl_xor_sync(0xffffffffu, best, o));
+    __syncthreads();
+    if ((tid & 31) == 0) redi[tid >> 5] = best;
+    __syncthreads();
+    if (tid == 0) {
+      int b = 0;
+      for (int w = 0; w < (nt + 31) / 32; ++w) b = max(b, redi[w]);
+      s_l = b;
+      if (b < hi) {
+        if (b > 0) H[b + (int64_t)(b - 1) * m] = mkc(0.0, 0.0);
+        cplx sig;
+        if (its == 10 || its == 20 || its == 30) {
+          sig = H[hi + (int64_t)hi * m];
+          sig.x += 0.75 * cabs1(H[hi + (int64_t)(hi - 1) * m]);
+        } else {
+          const cplx a = H[(hi - 1) + (int64_t)(hi - 1) * m], bb = H[(hi - 1) + (int64_t)hi * m];
+          const cplx cc = H[hi + (int64_t)(hi - 1) * m], d = H[hi + (int64_t)hi * m];
+          cplx l1, l2;
+          eig2(a, bb, cc, d, l1, l2);
+          sig = (cabs2(csub(l1, d)) <= cabs2(csub(l2, d))) ? l1 : l2;
+        }
+        s_sig = sig;
+      }
+    }
+    __syncthreads();
+    const int l = s_l;
+    if (l == hi) {
+      if (tid == 0) out[hi] = H[hi + (int64_t)hi * m];
+      --hi; its = 0;
+      continue;
+    }
+    ++its;
+    if (its > 60) {   // give up on this eigenvalue: take the diagonal entry, flag it
+      if (tid == 0) out[hi] = H[hi + (int64_t)hi * m];
+      ++nfail; --hi; its = 0;
+      continue;
+    }
+    const cplx sig = s_sig;
+    // ---- left phase: R = Q^H (H - sig I); thread owns columns j = l + tid + q*nt
+    cplx carry[QR_MAXOWN];
+#pragma unroll
+    for (int q = 0; q < QR_MAXOWN; ++q) {
+      const int j = l + tid + q * nt;
+      if (j <= hi) {
+        cplx x = H[l + (int64_t)j * m];
+        if (j == l) x = csub(x, sig);
+        carry[q] = x;
+      }
+    }
+    for (int s = l; s < hi; ++s) {
+      {
+        const int rel = s - l;
+        if (rel % nt == tid) {
+          const int q = rel / nt;
+          cplx a = mkc(0.0, 0.0);
+#pragma unroll
+          for (int qq = 0; qq < QR_MAXOWN; ++qq) if (qq == q) a = carry[qq];
+          const cplx b = H[(s + 1) + (int64_t)s * m];
+          double c_; cplx s_;
+          givens(a, b, c_, s_);
+          cs[rel] = c_; sn[rel] = s_;
+        }
+      }
+      __syncthreads();
+      const double c_ = cs[s - l];
+      const cplx s_ = sn[s - l];
+#pragma unroll
+      for (int q = 0; q < QR_MAXOWN; ++q) {
+        const int j = l + tid + q * nt;
+        if (j >= s && j <= hi) {
+          const cplx x = carry[q];
+          cplx yv = H[(s + 1) + (int64_t)j * m];
+          if (j == s + 1) yv = csub(yv, sig);
+          // new row s: c x + s y ; new row s+1: -conj(s) x + c y
+          cplx top = cscale(c_, x); cfma(top, s_, yv);
+          cplx bot = cscale(c_, yv); cfms(bot, cconj(s_), x);
+          H[s + (int64_t)j * m] = top;
+          carry[q] = bot;
+        }
+      }
+    }
+#pragma unroll
+    for (int q = 0; q < QR_MAXOWN; ++q) {
+      const int j = l + tid + q * nt;
+      if (j == hi) H[hi + (int64_t)hi * m] = carry[q];
+    }
+    __syncthreads();
+    // ---- right phase: H = R Q + sig I; thread owns rows i = l + tid + q*nt, walks along the row
+    for (int i = l + tid; i <= hi; i += nt) {
+      const int sstart = (i - 1 > l) ? i - 1 : l;
+      cplx x = (sstart == i - 1) ? mkc(0.0, 0.0) : H[i + (int64_t)sstart * m];   // R[i][i-1] = 0
+      for (int s = sstart; s < hi; ++s) {
+        const double c_ = cs[s - l];
+        const cplx s_ = sn[s - l];
+        const cplx yv = H[i + (int64_t)(s + 1) * m];
+        // col s: c x + conj(s) y ; col s+1: -s x + c y
+        cplx ns = cscale(c_, x); cfma(ns, cconj(s_), yv);
+        cplx n1 = cscale(c_, yv); cfms(n1, s_, x);
+        if (s == i) ns = cadd(ns, sig);
+        H[i + (int64_t)s * m] = ns;
+        x = n1;
+      }
+      if (i == hi) x = cadd(x, sig);
+      H[i + (int64_t)hi * m] = x;
+    }
+    __syncthreads();
+  }
+  if (tid == 0 && fail) fail[blockIdx.x] = nfail;
+}
+
+// theta = arg(lambda) on (-pi, pi], rank sort ascending (ties by index), |lambda| carried along.
+__global__ void k_sort_phases(const cplx* __restrict__ lam, int m, double* __restrict__ theta,
+                              double* __restrict__ absl) {
+  extern __shared__ double th[];   // m
+  const int64_t c = blockIdx.x;
+  const cplx* l = lam + c * m;
+  for (int i = threadIdx.x; i < m; i += blockDim.x) {
+    double t = atan2(l[i].y, l[i].x);
+    if (t <= -M_PI) t = M_PI;
+    th[i] = t;
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < m; i += blockDim.x) {
+    const double t = th[i];
+    int rank = 0;
+    for (int j = 0; j < m; ++j) rank += (th[j] < t) || (th[j] == t && j < i);
+    theta[c * m + rank] = t;
+    if (absl) absl[c * m + rank] = hypot(l[i].x, l[i].y);
+  }
+}
+
+}  // namespace
+
+size_t be_eigenphases_scratch_bytes(int64_t cnt, int m) {
+  return be_align256((size_t)cnt * m * sizeof(cplx)) + be_align256((size_t)cnt * sizeof(int));
+}
+
+int be_eigenvalues_general(be_ctx* ctx, cplx* W, int64_t cnt, int m, cplx* lam, int* fail) {
+  cudaStream_t st = ctx->stream;
+  if (cnt <= 0) return BE_OK;
+  if (m <= 2) {
+    k_eig_small<<<(unsigned)((cnt + 127) / 128), 128, 0, st>>>(W, cnt, m, lam);
+    ctx->launches++;
+    return (int)cudaGetLastError();
+  }
+  int nt = ((m + 31) / 32) * 32;
+  if (nt > 256) nt = 256;
+  if (m > QR_MAXOWN * nt) return BE_ERR_UNSUPPORTED;
+  const size_t sh1 = 2 * (size_t)m * sizeof(cplx);
+  if (sh1 > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_hessenberg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh1));
+  k_hessenberg<<<(unsigned)cnt, nt, sh1, st>>>(W, m);
+  ctx->launches++;
+  BE_CUDA(cudaGetLastError());
+  const size_t sh2 = (size_t)((m + 1) & ~1) * sizeof(double) + (size_t)m * sizeof(cplx);
+  if (sh2 > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_hqr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh2));
+  k_hqr<<<(unsigned)cnt, nt, sh2, st>>>(W, m, lam, fail);
+  ctx->launches++;
+  return (int)cudaGetLastError();
+}
+
+int be_eigenphases(be_ctx* ctx, cplx* W, int64_t cnt, int m, double* theta, double* absl) {
+  if (cnt <= 0 || m <= 0) return BE_OK;
+  cplx* lam = (cplx*)be_arena_alloc(ctx, (size_t)cnt * m * sizeof(cplx));
+  int* fail = (int*)be_arena_alloc(ctx, (size_t)cnt * sizeof(int));
+  if (!lam || !fail) return BE_ERR_NOMEM;
+  BE_TRY(be_eigenvalues_general(ctx, W, cnt, m, lam, fail));
+  int nt = ((m + 31) / 32) * 32;
+  if (nt > 256) nt = 256;
+  const size_t sh = (size_t)m * sizeof(double);
+  if (sh > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_sort_phases, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
+  k_sort_phases<<<(unsigned)cnt, nt, sh, ctx->stream>>>(lam, m, theta, absl);
+  ctx->launches++;
+  return (int)cudaGetLastError();
+}

@@ -1,0 +1,201 @@
+// Batched complex128 GEMM on the FP64 tensor cores of sm_100a.
+//
+// tcgen05.mma has no f64 kind, so the FP64 tensor path on Blackwell is the warp-level
+// mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4) fed from shared memory with the accumulators in registers.
+// A complex product is four real DMMAs on split re/im operands: the interleaved complex128 input
+// is de-interleaved while it is staged into shared memory, where transposition and conjugation
+// are also applied (a sign flip), so every op(A), op(B) combination runs the same inner loop.
+//
+// Used for: the link overlaps M_j = U_j^dagger U_{j+1} (ring mode, closing phase Phi applied in
+// the loader; Eq. 2), the ordered Wilson product, the rank-2k
+// update of the blocked tridiagonalization, the compact-WY back-transform, U^dagger S U and the
+// sector rotations of the spin-resolved loop.
+//
+// Tile: 64 x 64 x 16 per CTA, 256 threads = 8 warps as 2 (M) x 4 (N), warp tile 32 x 16 =
+// 4 x 2 DMMA blocks, 32 DMMAs per 12 shared loads per k4 step.  Double-buffered shared memory,
+// global loads of tile t+1 are in flight while tile t is multiplied.
+#include "be_common.cuh"
+
+namespace {
+
+constexpr int TM = 64, TN = 64, TK = 16, LDS = 68;  // LDS % 16 == 4: conflict-free fragment loads
+constexpr int NTHREADS = 256;
+constexpr int SM_PLANE = TK * LDS;                   // doubles per plane
+constexpr int SM_STAGE = 4 * SM_PLANE;               // A_re, A_im, B_re, B_im
+constexpr size_t SM_BYTES = 2 * SM_STAGE * sizeof(double);
+
+__device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+template <int OPA, int OPB>
+__global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p, int tilesM, int tilesN) {
+  extern __shared__ double smem[];
+  const int tid = threadIdx.x;
+  const int64_t tiles = (int64_t)tilesM * tilesN;
+  const int64_t bidx = blockIdx.x;
+  const int64_t b = bidx / tiles;
+  const int t = (int)(bidx - b * tiles);
+  const int tm = t % tilesM, tn = t / tilesM;
+  if (p.lower && tn > tm) return;
+  const int64_t bo = b / p.inner;
+  const int bi = (int)(b - bo * p.inner);
+  const cplx* __restrict__ A = p.A + bo * p.sAo + (int64_t)bi * p.sAi;
+  int biB = bi;
+  bool wrap = false;
+  if (p.ringB) { biB = bi + 1; if (biB == p.inner) biB = 0; wrap = (bi == p.phi_at); }
+  const cplx* __restrict__ B = p.B + bo * p.sBo + (int64_t)biB * p.sBi;
+  cplx* __restrict__ C = p.C + bo * p.sCo + (int64_t)bi * p.sCi;
+  const cplx* __restrict__ phi = (wrap && p.phiB) ? p.phiB : nullptr;
+
+  const int m0 = tm * TM, n0 = tn * TN;
+  const int M = p.M, N = p.N, K = p.K;
+  const bool transA = (OPA == BE_OP_T || OPA == BE_OP_C), conjA = (OPA == BE_OP_C || OPA == BE_OP_J);
+  const bool transB = (OPB == BE_OP_T || OPB == BE_OP_C), conjB = (OPB == BE_OP_C || OPB == BE_OP_J);
+
+  // staging coordinates
+  int ai, ak, aqi, aqk;   // A tile element (i, k) = (ai + q*aqi, ak + q*aqk), q = 0..3
+  if (!transA) { ai = tid & 63; ak = tid >> 6; aqi = 0; aqk = 4; }
+  else         { ak = tid & 15; ai = tid >> 4; aqi = 16; aqk = 0; }
+  int bn, bk, bqn, bqk;
+  if (!transB) { bk = tid & 15; bn = tid >> 4; bqn = 16; bqk = 0; }
+  else         { bn = tid & 63; bk = tid >> 6; bqn = 0; bqk = 4; }
+
+  cplx ra[4], rb[4];
+  auto gload = [&](int k0) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int i = m0 + ai + q * aqi, k = k0 + ak + q * aqk;
+      cplx v = mkc(0.0, 0.0);
+      if (i < M && k < K) v = transA ? A[(int64_t)k + (int64_t)i * p.lda] : A[(int64_t)i + (int64_t)k * p.lda];
+      if (conjA) v.y = -v.y;
+      ra[q] = v;
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int n = n0 + bn + q * bqn, k = k0 + bk + q * bqk;
+      cplx v = mkc(0.0, 0.0);
+      if (n < N && k < K) {
+        v = transB ? B[(int64_t)n + (int64_t)k * p.ldb] : B[(int64_t)k + (int64_t)n * p.ldb];
+        if (phi) v = cmul(phi[k], v);
+      }
+      if (conjB) v.y = -v.y;
+      rb[q] = v;
+    }
+  };
+  auto sstore = [&](int stage) {
+    double* s = smem + stage * SM_STAGE;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int i = ai + q * aqi, k = ak + q * aqk;
+      s[k * LDS + i] = ra[q].x;
+      s[SM_PLANE + k * LDS + i] = ra[q].y;
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int n = bn + q * bqn, k = bk + q * bqk;
+      s[2 * SM_PLANE + k * LDS + n] = rb[q].x;
+      s[3 * SM_PLANE + k * LDS + n] = rb[q].y;
+    }
+  };
+
+  const int warp = tid >> 5, lane = tid & 31;
+  const int wm = warp & 1, wn = warp >> 1;
+  const int g = lane >> 2, tg = lane & 3;
+
+  double accr[4][2][2], acci[4][2][2];
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int c = 0; c < 2; ++c) { accr[a][c][0] = accr[a][c][1] = 0.0; acci[a][c][0] = acci[a][c][1] = 0.0; }
+
+  const int KT = (K + TK - 1) / TK;
+  gload(0);
+  sstore(0);
+  __syncthreads();
+  for (int kt = 0; kt < KT; ++kt) {
+    const int cur = kt & 1;
+    if (kt + 1 < KT) gload((kt + 1) * TK);
+    const double* s = smem + cur * SM_STAGE;
+#pragma unroll
+    for (int ks = 0; ks < 4; ++ks) {
+      const int k = ks * 4 + tg;
+      double ar[4], aim[4], br[2], bim[2];
+#pragma unroll
+      for (int mb = 0; mb < 4; ++mb) {
+        const int i = wm * 32 + mb * 8 + g;
+        ar[mb] = s[k * LDS + i];
+        aim[mb] = s[SM_PLANE + k * LDS + i];
+      }
+#pragma unroll
+      for (int nb = 0; nb < 2; ++nb) {
+        const int n = wn * 16 + nb * 8 + g;
+        br[nb] = s[2 * SM_PLANE + k * LDS + n];
+        bim[nb] = s[3 * SM_PLANE + k * LDS + n];
+      }
+#pragma unroll
+      for (int mb = 0; mb < 4; ++mb) {
+        const double nai = -aim[mb];
+#pragma unroll
+        for (int nb = 0; nb < 2; ++nb) {
+          dmma(accr[mb][nb][0], accr[mb][nb][1], ar[mb], br[nb]);
+          dmma(accr[mb][nb][0], accr[mb][nb][1], nai, bim[nb]);
+          dmma(acci[mb][nb][0], acci[mb][nb][1], ar[mb], bim[nb]);
+          dmma(acci[mb][nb][0], acci[mb][nb][1], aim[mb], br[nb]);
+        }
+      }
+    }
+    if (kt + 1 < KT) {
+      sstore(cur ^ 1);   // the other stage was last read before the previous barrier
+      __syncthreads();
+    }
+  }
+
+  const bool has_beta = (p.beta.x != 0.0 || p.beta.y != 0.0);
+#pragma unroll
+  for (int mb = 0; mb < 4; ++mb) {
+    const int row = m0 + wm * 32 + mb * 8 + g;
+    if (row >= M) continue;
+#pragma unroll
+    for (int nb = 0; nb < 2; ++nb) {
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const int col = n0 + wn * 16 + nb * 8 + 2 * tg + e;
+        if (col >= N) continue;
+        cplx v = cmul(p.alpha, mkc(accr[mb][nb][e], acci[mb][nb][e]));
+        cplx* dst = C + (int64_t)row + (int64_t)col * p.ldc;
+        if (has_beta) v = cadd(v, cmul(p.beta, *dst));
+        *dst = v;
+      }
+    }
+  }
+}
+
+template <int OPA, int OPB>
+int launch(be_ctx* ctx, const ZgemmParams& p) {
+  const int tilesM = (p.M + TM - 1) / TM, tilesN = (p.N + TN - 1) / TN;
+  const int64_t blocks = p.batch * tilesM * tilesN;
+  if (blocks <= 0) return BE_OK;
+  if (blocks > 0x7fffffffLL) return BE_ERR_SHAPE;
+  static bool attr_done = false;  // per instantiation; idempotent
+  if (!attr_done) {
+    BE_CUDA(cudaFuncSetAttribute(zgemm_kernel<OPA, OPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM_BYTES));
+    attr_done = true;
+  }
+  zgemm_kernel<OPA, OPB><<<(unsigned)blocks, NTHREADS, SM_BYTES, ctx->stream>>>(p, tilesM, tilesN);
+  ctx->launches++;
+  return (int)cudaGetLastError();
+}
+
+}  // namespace
+
+int be_zgemm(be_ctx* ctx, int opA, int opB, const ZgemmParams& p) {
+  if (p.M <= 0 || p.N <= 0 || p.batch <= 0) return BE_OK;
+  if (p.phiB && opB != BE_OP_N) return BE_ERR_UNSUPPORTED;
+#define CASE(a, b) if (opA == a && opB == b) return launch<a, b>(ctx, p);
+  CASE(BE_OP_N, BE_OP_N) CASE(BE_OP_N, BE_OP_C) CASE(BE_OP_C, BE_OP_N) CASE(BE_OP_N, BE_OP_T)
+  CASE(BE_OP_T, BE_OP_N) CASE(BE_OP_J, BE_OP_N) CASE(BE_OP_N, BE_OP_J) CASE(BE_OP_C, BE_OP_C) CASE(BE_OP_T, BE_OP_J)
+#undef CASE
+  return BE_ERR_UNSUPPORTED;
+}
