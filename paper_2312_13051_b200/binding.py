@@ -1,0 +1,246 @@
+"""Thin ctypes binding of the C-ABI library (include/berryeasy_b200.h).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels of
+``libberryeasy_b200.so``.  PyTorch supplies device memory and streams.  There is no CPU fallback:
+if the library is missing or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libberryeasy_b200.so")
+
+EXPORTS = [
+    "be_create", "be_destroy", "be_strerror", "be_workspace_bytes", "be_set_workspace_limit",
+    "be_launch_count", "be_eigh_batched", "be_wilson_loop", "be_nested_wilson",
+    "be_spin_resolved_wilson", "be_winding", "be_wilson_loop_host", "be_spin_resolved_wilson_host",
+]
+
+
+class BeGrid(C.Structure):
+    _fields_ = [("ndim", C.c_int), ("batch", C.c_int64), ("dims", C.c_int * 3), ("N", C.c_int)]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree shared library (built by ``python -m paper_2312_13051_b200.build``)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} not found: run `python -m paper_2312_13051_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i64, dbl, ci = C.c_void_p, C.c_int64, C.c_double, C.c_int
+    gp = C.POINTER(BeGrid)
+    lib.be_create.argtypes = [C.POINTER(vp), vp]
+    lib.be_destroy.argtypes = [vp]
+    lib.be_strerror.argtypes = [ci]
+    lib.be_strerror.restype = C.c_char_p
+    lib.be_workspace_bytes.argtypes = [gp, ci, ci]
+    lib.be_workspace_bytes.restype = C.c_size_t
+    lib.be_set_workspace_limit.argtypes = [vp, C.c_size_t]
+    lib.be_launch_count.argtypes = [vp]
+    lib.be_launch_count.restype = i64
+    lib.be_eigh_batched.argtypes = [vp, vp, i64, ci, ci, vp, vp, vp]
+    lib.be_wilson_loop.argtypes = [vp, vp, gp, ci, ci, vp, vp, vp, vp]
+    lib.be_nested_wilson.argtypes = [vp, vp, gp, ci, ci, ci, ci, ci, ci, dbl, vp, vp, vp, vp]
+    lib.be_spin_resolved_wilson.argtypes = [vp, vp, gp, ci, ci, vp, ci, ci, vp, vp, vp, vp]
+    lib.be_winding.argtypes = [vp, vp, i64, ci, ci, vp]
+    lib.be_wilson_loop_host.argtypes = [vp, vp, gp, ci, ci, vp, vp, vp, vp]
+    lib.be_spin_resolved_wilson_host.argtypes = [vp, vp, gp, ci, ci, vp, ci, ci, vp, vp, vp, vp]
+    _lib = lib
+    return lib
+
+
+class BerryEasyError(RuntimeError):
+    pass
+
+
+def _check(lib, rc):
+    if rc != 0:
+        raise BerryEasyError(f"berryeasy_b200 error {rc}: {lib.be_strerror(rc).decode()}")
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _dev(t, dtype, name):
+    if not t.is_cuda:
+        raise ValueError(f"{name} must be a CUDA tensor")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous {dtype}")
+    return t
+
+
+def _host(t, dtype, name):
+    if t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise ValueError(f"{name} must be a contiguous host tensor of {dtype}")
+    return t
+
+
+def _grid_of(H, grid_ndim):
+    if H.dim() != grid_ndim + 3:
+        raise ValueError("H_grid must be [batch][dims...][N][N]")
+    g = BeGrid()
+    g.ndim = grid_ndim
+    g.batch = H.shape[0]
+    for a in range(3):
+        g.dims[a] = H.shape[1 + a] if a < grid_ndim else 1
+    g.N = H.shape[-1]
+    if H.shape[-2] != H.shape[-1]:
+        raise ValueError("H must be square")
+    return g
+
+
+class Context:
+    """Owns a ``be_ctx`` bound to the current torch CUDA stream (or the one given)."""
+
+    def __init__(self, stream: "torch.cuda.Stream | None" = None, device=None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("berryeasy_b200 needs a CUDA device (no CPU fallback)")
+        self.lib = load_library()
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        with torch.cuda.device(self.device):
+            self.stream = stream if stream is not None else torch.cuda.current_stream()
+            h = C.c_void_p()
+            _check(self.lib, self.lib.be_create(C.byref(h), C.c_void_p(self.stream.cuda_stream)))
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.be_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_workspace_limit(self, nbytes: int):
+        _check(self.lib, self.lib.be_set_workspace_limit(self._h, nbytes))
+
+    def launch_count(self) -> int:
+        return int(self.lib.be_launch_count(self._h))
+
+    # ------------------------------------------------------------------ be_eigh_batched
+    def eigh_batched(self, H, n_vec=None, want_info=False):
+        """H [count][N][N] complex128 (device) -> E [count][N], U [count][N][n_vec] (or None)."""
+        _dev(H, torch.complex128, "H")
+        count, N = H.shape[0], H.shape[-1]
+        n_vec = N if n_vec is None else n_vec
+        E = torch.empty((count, N), dtype=torch.float64, device=H.device)
+        U = torch.empty((count, N, n_vec), dtype=torch.complex128, device=H.device) if n_vec > 0 else None
+        info = torch.empty((count,), dtype=torch.int32, device=H.device) if want_info else None
+        _check(self.lib, self.lib.be_eigh_batched(self._h, _ptr(H), count, N, n_vec, _ptr(E), _ptr(U), _ptr(info)))
+        return (E, U, info) if want_info else (E, U)
+
+    # ------------------------------------------------------------------ be_wilson_loop
+    def wilson_loop(self, H_grid, n_occ, direction, close=None, want_abs=True, want_mingap=True):
+        """H_grid [batch][dims...][N][N] -> theta [loops][n_occ], |lambda| or None, mingap or None."""
+        _dev(H_grid, torch.complex128, "H_grid")
+        nd = H_grid.dim() - 3
+        g = _grid_of(H_grid, nd)
+        loops = H_grid.shape[0]
+        for a in range(nd):
+            if a != direction:
+                loops *= H_grid.shape[1 + a]
+        dev = H_grid.device
+        theta = torch.empty((loops, n_occ), dtype=torch.float64, device=dev)
+        ab = torch.empty((loops, n_occ), dtype=torch.float64, device=dev) if want_abs else None
+        mg = torch.empty((loops,), dtype=torch.float64, device=dev) if want_mingap else None
+        if close is not None:
+            _dev(close, torch.complex128, "close")
+        _check(self.lib, self.lib.be_wilson_loop(self._h, _ptr(H_grid), C.byref(g), n_occ, direction,
+                                                 _ptr(close), _ptr(theta), _ptr(ab), _ptr(mg)))
+        return theta, ab, mg
+
+    # ------------------------------------------------------------------ be_spin_resolved_wilson
+    def spin_resolved_wilson(self, H_grid, n_occ, direction, S, m_lo=-1, close=None, want_pso=True):
+        """S: real diagonal [N] float64 or dense [N][N] complex128 (device)."""
+        _dev(H_grid, torch.complex128, "H_grid")
+        nd = H_grid.dim() - 3
+        g = _grid_of(H_grid, nd)
+        loops = H_grid.shape[0]
+        for a in range(nd):
+            if a != direction:
+                loops *= H_grid.shape[1 + a]
+        n1 = H_grid.shape[1 + direction]
+        is_diag = 1 if S.dim() == 1 else 0
+        _dev(S, torch.float64 if is_diag else torch.complex128, "S")
+        mlo = n_occ // 2 if m_lo < 0 else m_lo
+        dev = H_grid.device
+        lo = torch.empty((loops, mlo), dtype=torch.float64, device=dev)
+        hi = torch.empty((loops, n_occ - mlo), dtype=torch.float64, device=dev)
+        pso = torch.empty((loops, n1, n_occ), dtype=torch.float64, device=dev) if want_pso else None
+        _check(self.lib, self.lib.be_spin_resolved_wilson(self._h, _ptr(H_grid), C.byref(g), n_occ, direction,
+                                                          _ptr(S), is_diag, m_lo, _ptr(close),
+                                                          _ptr(lo), _ptr(hi), _ptr(pso)))
+        return lo, hi, pso
+
+    # ------------------------------------------------------------------ be_nested_wilson
+    def nested_wilson(self, H_grid, n_occ, dir1, dir2, base=0, wb_lo=0, wb_hi=1, theta_cut=None,
+                      close1=None, close2=None):
+        import math
+        _dev(H_grid, torch.complex128, "H_grid")
+        nd = H_grid.dim() - 3
+        g = _grid_of(H_grid, nd)
+        outer = H_grid.shape[0]
+        for a in range(nd):
+            if a not in (dir1, dir2):
+                outer *= H_grid.shape[1 + a]
+        n2 = H_grid.shape[1 + dir2]
+        dev = H_grid.device
+        th1 = torch.empty((outer, n2, n_occ), dtype=torch.float64, device=dev)
+        thn = torch.empty((outer, wb_hi - wb_lo), dtype=torch.float64, device=dev)
+        cut = math.pi if theta_cut is None else float(theta_cut)
+        _check(self.lib, self.lib.be_nested_wilson(self._h, _ptr(H_grid), C.byref(g), n_occ, dir1, dir2, base,
+                                                   wb_lo, wb_hi, cut, _ptr(close1), _ptr(close2),
+                                                   _ptr(th1), _ptr(thn)))
+        return th1, thn
+
+    # ------------------------------------------------------------------ be_winding
+    def winding(self, theta):
+        """theta [n_cycles][n_points][m] (device) -> wind [n_cycles]."""
+        _dev(theta, torch.float64, "theta")
+        nc, npnt, m = theta.shape
+        out = torch.empty((nc,), dtype=torch.float64, device=theta.device)
+        _check(self.lib, self.lib.be_winding(self._h, _ptr(theta), nc, npnt, m, _ptr(out)))
+        return out
+
+    # ------------------------------------------------------------------ host variants (end to end)
+    def wilson_loop_host(self, H_grid, n_occ, direction, close=None):
+        _host(H_grid, torch.complex128, "H_grid")
+        nd = H_grid.dim() - 3
+        g = _grid_of(H_grid, nd)
+        loops = H_grid.numel() // (H_grid.shape[-1] ** 2 * H_grid.shape[1 + direction])
+        theta = torch.empty((loops, n_occ), dtype=torch.float64).pin_memory()
+        ab = torch.empty((loops, n_occ), dtype=torch.float64).pin_memory()
+        mg = torch.empty((loops,), dtype=torch.float64).pin_memory()
+        _check(self.lib, self.lib.be_wilson_loop_host(self._h, _ptr(H_grid), C.byref(g), n_occ, direction,
+                                                      _ptr(close), _ptr(theta), _ptr(ab), _ptr(mg)))
+        return theta, ab, mg
+
+    def spin_resolved_wilson_host(self, H_grid, n_occ, direction, S, m_lo=-1, close=None, want_pso=True):
+        _host(H_grid, torch.complex128, "H_grid")
+        nd = H_grid.dim() - 3
+        g = _grid_of(H_grid, nd)
+        n1 = H_grid.shape[1 + direction]
+        loops = H_grid.numel() // (H_grid.shape[-1] ** 2 * n1)
+        is_diag = 1 if S.dim() == 1 else 0
+        mlo = n_occ // 2 if m_lo < 0 else m_lo
+        lo = torch.empty((loops, mlo), dtype=torch.float64).pin_memory()
+        hi = torch.empty((loops, n_occ - mlo), dtype=torch.float64).pin_memory()
+        pso = torch.empty((loops, n1, n_occ), dtype=torch.float64).pin_memory() if want_pso else None
+        _check(self.lib, self.lib.be_spin_resolved_wilson_host(self._h, _ptr(H_grid), C.byref(g), n_occ,
+                                                               direction, _ptr(S), is_diag, m_lo, _ptr(close),
+                                                               _ptr(lo), _ptr(hi), _ptr(pso)))
+        return lo, hi, pso

@@ -1,0 +1,166 @@
+// C-ABI entry points (include/berryeasy_b200.h): argument checks, scratch arena, chunking over
+// whole loops, sequencing of the stages.  All arithmetic is in the kernels of the other files.
+#include "be_common.cuh"
+#include <new>
+#include <vector>
+#include <string.h>
+
+// stage entry points defined in wilson.cu
+int be_mingap(be_ctx* ctx, const double* E, int N, int m, int n1, int64_t loops, double* out);
+int be_scale_rows(be_ctx* ctx, const cplx* X, const double* S, cplx* SX, int N, int64_t total);
+int be_winding_impl(be_ctx* ctx, const double* theta, int64_t n_cycles, int n_points, int m, double* wind);
+int be_nested_select_small(be_ctx* ctx, const cplx* W, int64_t cnt, int m, int wb_lo, int wb_hi,
+                           double cut, double* theta1, cplx* Vs);
+int be_chain_product(be_ctx* ctx, const cplx* F, int N, int m, int64_t outer, int n1,
+                     const cplx* d_close, int phi_at, cplx** Wout);
+
+// ---------------------------------------------------------------------------------------------
+// arena
+int be_arena_reserve(be_ctx* ctx, size_t bytes) {
+  ctx->arena_used = 0;
+  if (bytes <= ctx->arena_bytes) return BE_OK;
+  if (ctx->arena) {
+    BE_CUDA(cudaStreamSynchronize(ctx->stream));
+    BE_CUDA(cudaFree(ctx->arena));
+    ctx->arena = nullptr; ctx->arena_bytes = 0;
+  }
+  void* p = nullptr;
+  cudaError_t e = cudaMalloc(&p, bytes);
+  if (e != cudaSuccess) { cudaGetLastError(); return BE_ERR_NOMEM; }
+  ctx->arena = (char*)p; ctx->arena_bytes = bytes;
+  return BE_OK;
+}
+
+void* be_arena_alloc(be_ctx* ctx, size_t bytes) {
+  const size_t b = be_align256(bytes ? bytes : 1);
+  if (ctx->arena_used + b > ctx->arena_bytes) return nullptr;
+  void* p = ctx->arena + ctx->arena_used;
+  ctx->arena_used += b;
+  return p;
+}
+
+// ---------------------------------------------------------------------------------------------
+extern "C" int be_create(be_ctx** out, void* cuda_stream) {
+  if (!out) return BE_ERR_NULL;
+  be_ctx* c = new (std::nothrow) be_ctx;
+  if (!c) return BE_ERR_NOMEM;
+  memset(c, 0, sizeof(*c));
+  c->stream = (cudaStream_t)cuda_stream;
+  cudaError_t e = cudaGetDevice(&c->device);
+  if (e != cudaSuccess) { delete c; return (int)e; }
+  cudaDeviceProp prop;
+  e = cudaGetDeviceProperties(&prop, c->device);
+  if (e != cudaSuccess) { delete c; return (int)e; }
+  c->sm_count = prop.multiProcessorCount;
+  c->ws_limit = (size_t)64 << 30;
+  *out = c;
+  return BE_OK;
+}
+
+extern "C" int be_destroy(be_ctx* ctx) {
+  if (!ctx) return BE_ERR_NULL;
+  cudaStreamSynchronize(ctx->stream);
+  if (ctx->arena) cudaFree(ctx->arena);
+  if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+  delete ctx;
+  return BE_OK;
+}
+
+extern "C" const char* be_strerror(int code) {
+  switch (code) {
+    case BE_OK: return "ok";
+    case BE_ERR_NULL: return "required pointer is NULL";
+    case BE_ERR_SHAPE: return "shape / index argument out of range";
+    case BE_ERR_ALIGN: return "pointer not aligned";
+    case BE_ERR_UNSUPPORTED: return "request not supported by this build";
+    case BE_ERR_NOMEM: return "scratch allocation failed";
+    default: break;
+  }
+  if (code > 0) return cudaGetErrorString((cudaError_t)code);
+  return "unknown error";
+}
+
+extern "C" int be_set_workspace_limit(be_ctx* ctx, size_t bytes) {
+  if (!ctx) return BE_ERR_NULL;
+  if (bytes < ((size_t)64 << 20)) return BE_ERR_SHAPE;
+  ctx->ws_limit = bytes;
+  return BE_OK;
+}
+
+extern "C" int64_t be_launch_count(const be_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+// ---------------------------------------------------------------------------------------------
+size_t be_eigh_scratch_bytes(int64_t cnt, int N, int nv) {
+  if (N <= 8) return 256;
+  return be_eigh_large_scratch_bytes(cnt, N, nv) + 4096;
+}
+
+int be_eigh_frames(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt,
+                   int N, int nv, double* E, cplx* X, int* info) {
+  if (cnt <= 0) return BE_OK;
+  if (N <= 8) return be_eigh_small(ctx, H, map, loop0, cnt, N, nv, E, X, info);
+  const size_t mark = ctx->arena_used;
+  const int r = be_eigh_large(ctx, H, map, loop0, cnt, N, nv, E, X, info);
+  ctx->arena_used = mark;   // stage scratch is dead once its kernels are enqueued (stream order)
+  return r;
+}
+
+static inline bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
+
+static GridMap flat_map(int64_t count) {
+  GridMap m;
+  memset(&m, 0, sizeof(m));
+  m.ndim = 1; m.dir = 0; m.n1 = 1; m.shift = 0;
+  m.dims[0] = 1; m.stride[0] = 0; m.batch_stride = 1; m.loops = count;
+  return m;
+}
+
+extern "C" size_t be_workspace_bytes(const be_grid* g, int n_occ, int op) {
+  if (!g || g->ndim < 1 || g->ndim > 3) return 0;
+  int64_t pts = g->batch;
+  for (int a = 0; a < g->ndim; ++a) pts *= g->dims[a];
+  const int N = g->N, m = (op == 0) ? n_occ : n_occ;
+  size_t per = be_eigh_scratch_bytes(1, N, m) + (size_t)N * (m + 1) * 16 * 4 + (size_t)m * m * 16 * 6;
+  size_t tot = per * (size_t)pts;
+  const size_t cap = (size_t)64 << 30;
+  return tot < cap ? tot : cap;
+}
+
+// ---------------------------------------------------------------------------------------------
+extern "C" int be_eigh_batched(be_ctx* ctx, const void* dH, int64_t count, int N, int n_vec,
+                               double* dE, void* dU, int* d_info) {
+  if (!ctx || !dH || !dE) return BE_ERR_NULL;
+  if (count < 0 || N < 1 || n_vec < 0 || n_vec > N) return BE_ERR_SHAPE;
+  if (!aligned(dH, 16) || !aligned(dE, 8) || (dU && !aligned(dU, 16))) return BE_ERR_ALIGN;
+  if (count == 0) return BE_OK;
+  const int nv = dU ? n_vec : 0;
+  const size_t per = be_eigh_scratch_bytes(1, N, nv) + (size_t)N * (nv > 0 ? nv : 1) * sizeof(cplx) + 1024;
+  int64_t chunk = (int64_t)(ctx->ws_limit / per);
+  if (chunk < 1) chunk = 1;
+  if (chunk > count) chunk = count;
+  const int64_t nchunks = (count + chunk - 1) / chunk;
+  chunk = (count + nchunks - 1) / nchunks;
+  BE_TRY(be_arena_reserve(ctx, per * (size_t)chunk + (1 << 20)));
+  const GridMap map = flat_map(count);
+  for (int64_t c0 = 0; c0 < count; c0 += chunk) {
+    const int64_t cnt = (count - c0 < chunk) ? count - c0 : chunk;
+    ctx->arena_used = 0;
+    cplx* X = nullptr;
+    if (nv > 0) {
+      X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * nv * sizeof(cplx));
+      if (!X) return BE_ERR_NOMEM;
+    }
+    BE_TRY(be_eigh_frames(ctx, (const cplx*)dH, map, c0, cnt, N, nv, dE + c0 * N, X,
+                          d_info ? d_info + c0 : nullptr));
+    if (nv > 0) BE_TRY(be_frames_to_public(ctx, X, (cplx*)dU + c0 * (int64_t)N * nv, cnt, N, nv));
+  }
+  return BE_OK;
+}
+
+extern "C" int be_winding(be_ctx* ctx, const double* d_theta, int64_t n_cycles, int n_points, int m,
+                          double* d_wind) {
+  if (!ctx || !d_theta || !d_wind) return BE_ERR_NULL;
+  if (n_cycles < 0 || n_points < 1 || m < 1) return BE_ERR_SHAPE;
+  if (n_cycles == 0) return BE_OK;
+  return be_winding_impl(ctx, d_theta, n_cycles, n_points, m, d_wind);
+}

@@ -1,0 +1,130 @@
+// Host-buffer (end-to-end) variants: the grid is streamed host -> device in chunks of whole loops
+// on a copy stream, double buffered against the compute stream; results are copied back before
+// return.  Semantics are those of the device entry points (include/berryeasy_b200.h).
+#include "be_common.cuh"
+#include <string.h>
+
+size_t be_wilson_per_loop_bytes(int N, int m, int n1, int spin);
+
+namespace {
+
+struct DevBuf {
+  void* p = nullptr;
+  ~DevBuf() { if (p) cudaFree(p); }
+  int alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 16) == cudaSuccess ? BE_OK : BE_ERR_NOMEM; }
+};
+
+int host_run(be_ctx* ctx, const void* hH, const be_grid* grid, int n_occ, int dir, const void* hS,
+             int S_is_diag, int m_lo, bool spin, const void* h_close, double* h_a, double* h_b,
+             double* h_c) {
+  if (!ctx || !hH || !grid) return BE_ERR_NULL;
+  if (grid->ndim < 1 || grid->ndim > 3 || grid->batch < 1 || grid->N < 1) return BE_ERR_SHAPE;
+  if (dir != grid->ndim - 1) return BE_ERR_UNSUPPORTED;
+  if (n_occ < 1 || n_occ > grid->N) return BE_ERR_SHAPE;
+  const int N = grid->N, m = n_occ, n1 = grid->dims[dir];
+  int64_t loops = grid->batch;
+  for (int a = 0; a < grid->ndim - 1; ++a) loops *= grid->dims[a];
+  if (spin) {
+    if (!hS) return BE_ERR_NULL;
+    if (m_lo < 0) m_lo = m / 2;
+    if (m_lo > m) return BE_ERR_SHAPE;
+  } else if (!h_a) return BE_ERR_NULL;
+  if (!ctx->copy_stream) BE_CUDA(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+
+  const size_t per = be_wilson_per_loop_bytes(N, m, n1, spin ? 1 : 0);
+  const size_t loop_bytes = (size_t)n1 * N * N * sizeof(cplx);
+  // leave room for the two staging buffers next to the work arena
+  int64_t lc = (int64_t)(ctx->ws_limit / (per + 2 * loop_bytes));
+  if (lc < 1) lc = 1;
+  if (lc > loops) lc = loops;
+  const int64_t nchunks = (loops + lc - 1) / lc;
+  lc = (loops + nchunks - 1) / nchunks;
+
+  DevBuf stage[2], dS, dclose, da, db, dc;
+  BE_TRY(stage[0].alloc(loop_bytes * lc));
+  if (nchunks > 1) BE_TRY(stage[1].alloc(loop_bytes * lc));
+  const int mlo = spin ? m_lo : 0, mhi = spin ? m - m_lo : 0;
+  if (spin) {
+    const size_t sb = S_is_diag ? (size_t)N * sizeof(double) : (size_t)N * N * sizeof(cplx);
+    BE_TRY(dS.alloc(sb));
+    BE_CUDA(cudaMemcpyAsync(dS.p, hS, sb, cudaMemcpyHostToDevice, ctx->stream));
+    if (h_a) BE_TRY(da.alloc((size_t)loops * mlo * sizeof(double)));
+    if (h_b) BE_TRY(db.alloc((size_t)loops * mhi * sizeof(double)));
+    if (h_c) BE_TRY(dc.alloc((size_t)loops * n1 * m * sizeof(double)));
+  } else {
+    BE_TRY(da.alloc((size_t)loops * m * sizeof(double)));
+    if (h_b) BE_TRY(db.alloc((size_t)loops * m * sizeof(double)));
+    if (h_c) BE_TRY(dc.alloc((size_t)loops * sizeof(double)));
+  }
+  if (h_close) {
+    BE_TRY(dclose.alloc((size_t)N * sizeof(cplx)));
+    BE_CUDA(cudaMemcpyAsync(dclose.p, h_close, (size_t)N * sizeof(cplx), cudaMemcpyHostToDevice, ctx->stream));
+  }
+  cudaEvent_t copied[2], freed[2];
+  for (int i = 0; i < 2; ++i) {
+    BE_CUDA(cudaEventCreateWithFlags(&copied[i], cudaEventDisableTiming));
+    BE_CUDA(cudaEventCreateWithFlags(&freed[i], cudaEventDisableTiming));
+  }
+  int rc = BE_OK;
+  auto issue_copy = [&](int64_t ci) -> int {
+    const int b = (int)(ci & 1);
+    const int64_t l0 = ci * lc, nl = (loops - l0 < lc) ? loops - l0 : lc;
+    if (ci >= 2) BE_CUDA(cudaStreamWaitEvent(ctx->copy_stream, freed[b], 0));
+    BE_CUDA(cudaMemcpyAsync(stage[b].p, (const char*)hH + (size_t)l0 * loop_bytes, (size_t)nl * loop_bytes,
+                            cudaMemcpyHostToDevice, ctx->copy_stream));
+    BE_CUDA(cudaEventRecord(copied[b], ctx->copy_stream));
+    return BE_OK;
+  };
+  rc = issue_copy(0);
+  for (int64_t ci = 0; ci < nchunks && rc == BE_OK; ++ci) {
+    const int b = (int)(ci & 1);
+    const int64_t l0 = ci * lc, nl = (loops - l0 < lc) ? loops - l0 : lc;
+    if (ci + 1 < nchunks) { rc = issue_copy(ci + 1); if (rc != BE_OK) break; }
+    rc = (int)cudaStreamWaitEvent(ctx->stream, copied[b], 0);
+    if (rc != BE_OK) break;
+    be_grid g;
+    g.ndim = 1; g.batch = nl; g.dims[0] = n1; g.dims[1] = g.dims[2] = 1; g.N = N;
+    if (spin)
+      rc = be_spin_resolved_wilson(ctx, stage[b].p, &g, m, 0, dS.p, S_is_diag, m_lo, dclose.p,
+                                   da.p ? (double*)da.p + l0 * mlo : nullptr,
+                                   db.p && h_b ? (double*)db.p + l0 * mhi : nullptr,
+                                   dc.p && h_c ? (double*)dc.p + l0 * (int64_t)n1 * m : nullptr);
+    else
+      rc = be_wilson_loop(ctx, stage[b].p, &g, m, 0, dclose.p, (double*)da.p + l0 * m,
+                          h_b ? (double*)db.p + l0 * m : nullptr, h_c ? (double*)dc.p + l0 : nullptr);
+    if (rc != BE_OK) break;
+    rc = (int)cudaEventRecord(freed[b], ctx->stream);
+  }
+  if (rc == BE_OK) {
+    cudaStream_t st = ctx->stream;
+    if (spin) {
+      if (h_a && rc == BE_OK) rc = (int)cudaMemcpyAsync(h_a, da.p, (size_t)loops * mlo * sizeof(double), cudaMemcpyDeviceToHost, st);
+      if (h_b && rc == BE_OK) rc = (int)cudaMemcpyAsync(h_b, db.p, (size_t)loops * mhi * sizeof(double), cudaMemcpyDeviceToHost, st);
+      if (h_c && rc == BE_OK) rc = (int)cudaMemcpyAsync(h_c, dc.p, (size_t)loops * n1 * m * sizeof(double), cudaMemcpyDeviceToHost, st);
+    } else {
+      rc = (int)cudaMemcpyAsync(h_a, da.p, (size_t)loops * m * sizeof(double), cudaMemcpyDeviceToHost, st);
+      if (h_b && rc == BE_OK) rc = (int)cudaMemcpyAsync(h_b, db.p, (size_t)loops * m * sizeof(double), cudaMemcpyDeviceToHost, st);
+      if (h_c && rc == BE_OK) rc = (int)cudaMemcpyAsync(h_c, dc.p, (size_t)loops * sizeof(double), cudaMemcpyDeviceToHost, st);
+    }
+  }
+  cudaStreamSynchronize(ctx->copy_stream);
+  const cudaError_t se = cudaStreamSynchronize(ctx->stream);
+  if (rc == BE_OK && se != cudaSuccess) rc = (int)se;
+  for (int i = 0; i < 2; ++i) { cudaEventDestroy(copied[i]); cudaEventDestroy(freed[i]); }
+  return rc;
+}
+
+}  // namespace
+
+extern "C" int be_wilson_loop_host(be_ctx* ctx, const void* hH_grid, const be_grid* grid, int n_occ, int dir,
+                                   const void* h_close, double* h_theta, double* h_abs, double* h_mingap) {
+  return host_run(ctx, hH_grid, grid, n_occ, dir, nullptr, 0, 0, false, h_close, h_theta, h_abs, h_mingap);
+}
+
+extern "C" int be_spin_resolved_wilson_host(be_ctx* ctx, const void* hH_grid, const be_grid* grid, int n_occ,
+                                            int dir, const void* hS, int S_is_diag, int m_lo,
+                                            const void* h_close, double* h_theta_lo, double* h_theta_hi,
+                                            double* h_pso) {
+  return host_run(ctx, hH_grid, grid, n_occ, dir, hS, S_is_diag, m_lo, true, h_close, h_theta_lo,
+                  h_theta_hi, h_pso);
+}

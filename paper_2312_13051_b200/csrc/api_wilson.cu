@@ -1,0 +1,231 @@
+// be_wilson_loop / be_spin_resolved_wilson / be_nested_wilson and their host-buffer variants:
+// chunking over whole loops and stage sequencing.
+#include "be_common.cuh"
+#include <string.h>
+#include <vector>
+
+int be_mingap(be_ctx* ctx, const double* E, int N, int m, int n1, int64_t loops, double* out);
+int be_scale_rows(be_ctx* ctx, const cplx* X, const double* S, cplx* SX, int N, int64_t total);
+int be_nested_select_small(be_ctx* ctx, const cplx* W, int64_t cnt, int m, int wb_lo, int wb_hi,
+                           double cut, double* theta1, cplx* Vs);
+int be_chain_product(be_ctx* ctx, const cplx* F, int N, int m, int64_t outer, int n1,
+                     const cplx* d_close, int phi_at, cplx** Wout);
+
+static inline bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
+
+static int make_map(const be_grid* g, int dir, GridMap* out) {
+  if (!g) return BE_ERR_NULL;
+  if (g->ndim < 1 || g->ndim > 3 || g->batch < 1 || g->N < 1) return BE_ERR_SHAPE;
+  if (dir < 0 || dir >= g->ndim) return BE_ERR_SHAPE;
+  GridMap m;
+  memset(&m, 0, sizeof(m));
+  m.ndim = g->ndim; m.dir = dir; m.shift = 0;
+  int64_t st = 1, loops = g->batch;
+  for (int a = g->ndim - 1; a >= 0; --a) {
+    if (g->dims[a] < 1) return BE_ERR_SHAPE;
+    m.dims[a] = g->dims[a]; m.stride[a] = st; st *= g->dims[a];
+    if (a != dir) loops *= g->dims[a];
+  }
+  m.batch_stride = st; m.n1 = g->dims[dir]; m.loops = loops;
+  *out = m;
+  return BE_OK;
+}
+
+struct SpinArgs {
+  const void* dS; int S_is_diag; int m_lo;
+  double* theta_lo; double* theta_hi; double* pso;
+};
+
+// bytes of scratch one loop needs (upper bound), plain or spin-resolved
+static size_t per_loop_bytes(int N, int m, int n1, bool spin) {
+  const size_t fr = (size_t)N * m * sizeof(cplx);
+  size_t b = (size_t)n1 * (be_eigh_scratch_bytes(1, N, m) + fr + (size_t)N * sizeof(double) + 512);
+  const size_t mm = (size_t)m * m * sizeof(cplx);
+  b += (size_t)n1 * mm + 4 * mm + (size_t)m * 64 + 4096;           // links, products, eigenvalues
+  if (spin) {
+    b += (size_t)n1 * (fr /*SX*/ + 2 * mm /*S_red, V*/ + fr /*sector frames*/ + (size_t)m * 8 + 1024);
+    const size_t inner = (size_t)n1 * be_eigh_scratch_bytes(1, m, m);
+    const size_t outer = (size_t)n1 * be_eigh_scratch_bytes(1, N, m);
+    if (inner > outer) b += inner - outer;
+  }
+  return b;
+}
+
+// One pass over all loops of ``map`` (device H).  Plain loop when ``sp`` is NULL.
+static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, int m,
+                         const cplx* d_close, double* d_theta, double* d_abs, double* d_mingap,
+                         const SpinArgs* sp) {
+  const int n1 = map.n1;
+  const int64_t loops = map.loops;
+  const size_t per = per_loop_bytes(N, m, n1, sp != nullptr);
+  int64_t lc = (int64_t)(ctx->ws_limit / per);
+  if (lc < 1) lc = 1;
+  if (lc > loops) lc = loops;
+  const int64_t nchunks = (loops + lc - 1) / lc;
+  lc = (loops + nchunks - 1) / nchunks;
+  BE_TRY(be_arena_reserve(ctx, per * (size_t)lc + (4 << 20)));
+  const int mlo = sp ? sp->m_lo : 0, mhi = sp ? m - sp->m_lo : 0;
+  for (int64_t l0 = 0; l0 < loops; l0 += lc) {
+    const int64_t nl = (loops - l0 < lc) ? loops - l0 : lc;
+    const int64_t cnt = nl * n1;
+    ctx->arena_used = 0;
+    double* E = (double*)be_arena_alloc(ctx, (size_t)cnt * N * sizeof(double));
+    cplx* X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
+    if (!E || !X) return BE_ERR_NOMEM;
+    BE_TRY(be_eigh_frames(ctx, H, map, l0, cnt, N, m, E, X, nullptr));
+    if (d_mingap) BE_TRY(be_mingap(ctx, E, N, m, n1, nl, d_mingap + l0));
+    if (!sp) {
+      cplx* W = nullptr;
+      BE_TRY(be_chain_product(ctx, X, N, m, nl, n1, d_close, n1 - 1, &W));
+      BE_TRY(be_eigenphases(ctx, W, nl, m, d_theta + l0 * m, d_abs ? d_abs + l0 * m : nullptr));
+      continue;
+    }
+    // ---- spin-resolved: S_red = U^H S U, diagonalize, rotate into sectors
+    cplx* SX = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
+    cplx* Sred = (cplx*)be_arena_alloc(ctx, (size_t)cnt * m * m * sizeof(cplx));
+    cplx* V = (cplx*)be_arena_alloc(ctx, (size_t)cnt * m * m * sizeof(cplx));
+    double* sig = sp->pso ? sp->pso + l0 * (int64_t)n1 * m
+                          : (double*)be_arena_alloc(ctx, (size_t)cnt * m * sizeof(double));
+    if (!SX || !Sred || !V || !sig) return BE_ERR_NOMEM;
+    if (sp->S_is_diag) {
+      BE_TRY(be_scale_rows(ctx, X, (const double*)sp->dS, SX, N, cnt * (int64_t)N * m));
+    } else {
+      // row-major S read column-major is S^T: op T recovers S;  SX = S X
+      ZgemmParams g = zgemm_simple(N, m, N, (const cplx*)sp->dS, N, 0, X, N, (int64_t)N * m,
+                                   SX, N, (int64_t)N * m, cnt);
+      BE_TRY(be_zgemm(ctx, BE_OP_T, BE_OP_N, g));
+    }
+    {
+      // the eigensolver reads its input row-major; a column-major buffer holding conj(S_red) =
+      // X^T conj(SX) is S_red when read row-major (S_red is Hermitian)
+      ZgemmParams g = zgemm_simple(m, m, N, X, N, (int64_t)N * m, SX, N, (int64_t)N * m,
+                                   Sred, m, (int64_t)m * m, cnt);
+      BE_TRY(be_zgemm(ctx, BE_OP_T, BE_OP_J, g));
+    }
+    {
+      GridMap fm;
+      memset(&fm, 0, sizeof(fm));
+      fm.ndim = 1; fm.dir = 0; fm.n1 = 1; fm.dims[0] = 1; fm.batch_stride = 1; fm.loops = cnt;
+      BE_TRY(be_eigh_frames(ctx, Sred, fm, 0, cnt, m, m, sig, V, nullptr));
+    }
+    for (int sector = 0; sector < 2; ++sector) {
+      const int ms = sector == 0 ? mlo : mhi;
+      double* out = sector == 0 ? sp->theta_lo : sp->theta_hi;
+      if (ms == 0 || !out) continue;
+      const size_t mark = ctx->arena_used;
+      cplx* F = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * ms * sizeof(cplx));
+      if (!F) return BE_ERR_NOMEM;
+      ZgemmParams g = zgemm_simple(N, ms, m, X, N, (int64_t)N * m, V + (sector ? (int64_t)mlo * m : 0), m,
+                                   (int64_t)m * m, F, N, (int64_t)N * ms, cnt);
+      BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_N, g));
+      cplx* W = nullptr;
+      BE_TRY(be_chain_product(ctx, F, N, ms, nl, n1, d_close, n1 - 1, &W));
+      BE_TRY(be_eigenphases(ctx, W, nl, ms, out + l0 * ms, nullptr));
+      ctx->arena_used = mark;
+    }
+  }
+  return BE_OK;
+}
+
+size_t be_wilson_per_loop_bytes(int N, int m, int n1, int spin) { return per_loop_bytes(N, m, n1, spin != 0); }
+
+static int check_common(be_ctx* ctx, const void* H, const be_grid* g, int n_occ, int dir) {
+  if (!ctx || !H || !g) return BE_ERR_NULL;
+  if (g->ndim < 1 || g->ndim > 3 || g->batch < 1 || g->N < 1) return BE_ERR_SHAPE;
+  if (dir < 0 || dir >= g->ndim) return BE_ERR_SHAPE;
+  if (n_occ < 1 || n_occ > g->N) return BE_ERR_SHAPE;
+  if (!aligned(H, 16)) return BE_ERR_ALIGN;
+  return BE_OK;
+}
+
+extern "C" int be_wilson_loop(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_occ, int dir,
+                              const void* d_close, double* d_theta, double* d_abs, double* d_mingap) {
+  BE_TRY(check_common(ctx, dH_grid, grid, n_occ, dir));
+  if (!d_theta) return BE_ERR_NULL;
+  if ((d_close && !aligned(d_close, 16)) || !aligned(d_theta, 8)) return BE_ERR_ALIGN;
+  GridMap map;
+  BE_TRY(make_map(grid, dir, &map));
+  return wilson_device(ctx, (const cplx*)dH_grid, map, grid->N, n_occ, (const cplx*)d_close,
+                       d_theta, d_abs, d_mingap, nullptr);
+}
+
+extern "C" int be_spin_resolved_wilson(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_occ,
+                                       int dir, const void* dS, int S_is_diag, int m_lo,
+                                       const void* d_close, double* d_theta_lo, double* d_theta_hi,
+                                       double* d_pso) {
+  BE_TRY(check_common(ctx, dH_grid, grid, n_occ, dir));
+  if (!dS) return BE_ERR_NULL;
+  if (m_lo < 0) m_lo = n_occ / 2;
+  if (m_lo > n_occ) return BE_ERR_SHAPE;
+  if (!aligned(dS, S_is_diag ? 8 : 16) || (d_close && !aligned(d_close, 16))) return BE_ERR_ALIGN;
+  GridMap map;
+  BE_TRY(make_map(grid, dir, &map));
+  SpinArgs sp{dS, S_is_diag, m_lo, d_theta_lo, d_theta_hi, d_pso};
+  return wilson_device(ctx, (const cplx*)dH_grid, map, grid->N, n_occ, (const cplx*)d_close,
+                       nullptr, nullptr, nullptr, &sp);
+}
+
+// ---------------------------------------------------------------------------------------------
+extern "C" int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_occ,
+                                int dir1, int dir2, int base, int wb_lo, int wb_hi, double theta_cut,
+                                const void* d_close1, const void* d_close2,
+                                double* d_theta1, double* d_theta_nested) {
+  BE_TRY(check_common(ctx, dH_grid, grid, n_occ, dir1));
+  if (!d_theta_nested) return BE_ERR_NULL;
+  if (grid->ndim < 2 || dir2 < 0 || dir2 >= grid->ndim || dir2 == dir1) return BE_ERR_SHAPE;
+  if (base < 0 || base >= grid->dims[dir1]) return BE_ERR_SHAPE;
+  if (wb_lo < 0 || wb_hi > n_occ || wb_lo >= wb_hi) return BE_ERR_SHAPE;
+  if (n_occ > 2) return BE_ERR_UNSUPPORTED;   // closed-form Wannier-band vectors only (header)
+  const int N = grid->N, m = n_occ, ns = wb_hi - wb_lo;
+  // virtual axis order (other, dir2, dir1) so that loops enumerate [batch][other][i2]
+  GridMap full;
+  BE_TRY(make_map(grid, dir1, &full));
+  GridMap map;
+  memset(&map, 0, sizeof(map));
+  int other = -1;
+  for (int a = 0; a < grid->ndim; ++a) if (a != dir1 && a != dir2) other = a;
+  int k = 0;
+  if (other >= 0) { map.dims[k] = full.dims[other]; map.stride[k] = full.stride[other]; ++k; }
+  map.dims[k] = full.dims[dir2]; map.stride[k] = full.stride[dir2]; ++k;
+  map.dims[k] = full.dims[dir1]; map.stride[k] = full.stride[dir1];
+  map.ndim = k + 1; map.dir = k; map.n1 = full.n1; map.shift = base;
+  map.batch_stride = full.batch_stride; map.loops = full.loops;
+  const int n1 = map.n1, n2 = grid->dims[dir2];
+  const int64_t loops = map.loops, outer2 = loops / n2;
+  const int phi_at = n1 - 1 - base;   // link whose target frame has grid index 0
+
+  const size_t per = (size_t)n1 * (be_eigh_scratch_bytes(1, N, m) + (size_t)N * m * 16 + (size_t)N * 8 + 512)
+                     + (size_t)n1 * m * m * 16 + 8 * (size_t)m * m * 16 + 4096;
+  const size_t persist = (size_t)loops * ((size_t)N * ns * 16 + 256) + (size_t)outer2 * (n2 + 4) * ns * ns * 16 + (8 << 20);
+  int64_t lc = (int64_t)(ctx->ws_limit / per);
+  if (lc < 1) lc = 1;
+  if (lc > loops) lc = loops;
+  BE_TRY(be_arena_reserve(ctx, per * (size_t)lc + persist + (size_t)loops * m * 8 + (4 << 20)));
+  // persistent across chunks: Wannier-band frames and (optional) first-level phases
+  cplx* Wf = (cplx*)be_arena_alloc(ctx, (size_t)loops * N * ns * sizeof(cplx));
+  double* th1 = d_theta1 ? d_theta1 : (double*)be_arena_alloc(ctx, (size_t)loops * m * sizeof(double));
+  if (!Wf || !th1) return BE_ERR_NOMEM;
+  const size_t keep = ctx->arena_used;
+  for (int64_t l0 = 0; l0 < loops; l0 += lc) {
+    const int64_t nl = (loops - l0 < lc) ? loops - l0 : lc;
+    const int64_t cnt = nl * n1;
+    ctx->arena_used = keep;
+    double* E = (double*)be_arena_alloc(ctx, (size_t)cnt * N * sizeof(double));
+    cplx* X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
+    cplx* Vs = (cplx*)be_arena_alloc(ctx, (size_t)nl * m * ns * sizeof(cplx));
+    if (!E || !X || !Vs) return BE_ERR_NOMEM;
+    BE_TRY(be_eigh_frames(ctx, (const cplx*)dH_grid, map, l0, cnt, N, m, E, X, nullptr));
+    cplx* W = nullptr;
+    BE_TRY(be_chain_product(ctx, X, N, m, nl, n1, (const cplx*)d_close1, phi_at, &W));
+    BE_TRY(be_nested_select_small(ctx, W, nl, m, wb_lo, wb_hi, theta_cut, th1 + l0 * m, Vs));
+    // w = U_base V_S  (frame j = 0 of each rolled loop)
+    ZgemmParams g = zgemm_simple(N, ns, m, X, N, (int64_t)n1 * N * m, Vs, m, (int64_t)m * ns,
+                                 Wf + l0 * (int64_t)N * ns, N, (int64_t)N * ns, nl);
+    BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_N, g));
+  }
+  ctx->arena_used = keep;
+  cplx* W2 = nullptr;
+  BE_TRY(be_chain_product(ctx, Wf, N, ns, outer2, n2, (const cplx*)d_close2, n2 - 1, &W2));
+  BE_TRY(be_eigenphases(ctx, W2, outer2, ns, d_theta_nested, nullptr));
+  return BE_OK;
+}
