@@ -71,6 +71,15 @@ int be_set_workspace_limit(be_ctx* ctx, size_t bytes);
 /* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */
 int64_t be_launch_count(const be_ctx* ctx);
 
+/* Optional per-kernel-class profile (bench.py's roofline): when enabled every launch of an
+ * instrumented kernel class is bracketed by a CUDA event pair on the context's stream and its
+ * algorithmic bytes / flops are accumulated.  be_profile_enable resets the counters (it
+ * synchronises the stream); be_profile_get synchronises and returns the summed event time in ms.
+ * Classes 0..be_profile_name(i)==NULL: "hemv", "col", "w", "zgemm", "bisect", "invit", ... */
+int be_profile_enable(be_ctx* ctx, int on);
+const char* be_profile_name(int cls);
+int be_profile_get(be_ctx* ctx, int cls, double* ms, int64_t* launches, double* bytes, double* flops);
+
 /*
  * S1 -- batched Hermitian eigensolve ("exact diagonalization of a discretized
  * Hamiltonian at many points in reciprocal space").

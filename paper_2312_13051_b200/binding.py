@@ -18,6 +18,7 @@ EXPORTS = [
     "be_create", "be_destroy", "be_strerror", "be_workspace_bytes", "be_set_workspace_limit",
     "be_launch_count", "be_eigh_batched", "be_wilson_loop", "be_nested_wilson",
     "be_spin_resolved_wilson", "be_winding", "be_wilson_loop_host", "be_spin_resolved_wilson_host",
+    "be_profile_enable", "be_profile_name", "be_profile_get",
 ]
 
 
@@ -55,6 +56,10 @@ def load_library():
     lib.be_winding.argtypes = [vp, vp, i64, ci, ci, vp]
     lib.be_wilson_loop_host.argtypes = [vp, vp, gp, ci, ci, vp, vp, vp, vp]
     lib.be_spin_resolved_wilson_host.argtypes = [vp, vp, gp, ci, ci, vp, ci, ci, vp, vp, vp, vp]
+    lib.be_profile_enable.argtypes = [vp, ci]
+    lib.be_profile_name.argtypes = [ci]
+    lib.be_profile_name.restype = C.c_char_p
+    lib.be_profile_get.argtypes = [vp, ci, C.POINTER(dbl), C.POINTER(i64), C.POINTER(dbl), C.POINTER(dbl)]
     _lib = lib
     return lib
 
@@ -127,6 +132,23 @@ class Context:
 
     def set_workspace_limit(self, nbytes: int):
         _check(self.lib, self.lib.be_set_workspace_limit(self._h, nbytes))
+
+    def profile_enable(self, on: bool = True):
+        _check(self.lib, self.lib.be_profile_enable(self._h, 1 if on else 0))
+
+    def profile(self) -> dict:
+        """{class: {ms, launches, bytes, flops}} summed since profile_enable."""
+        out = {}
+        i = 0
+        while True:
+            name = self.lib.be_profile_name(i)
+            if not name:
+                break
+            ms, n, by, fl = C.c_double(), C.c_int64(), C.c_double(), C.c_double()
+            _check(self.lib, self.lib.be_profile_get(self._h, i, C.byref(ms), C.byref(n), C.byref(by), C.byref(fl)))
+            out[name.decode()] = {"ms": ms.value, "launches": n.value, "bytes": by.value, "flops": fl.value}
+            i += 1
+        return out
 
     def launch_count(self) -> int:
         return int(self.lib.be_launch_count(self._h))

@@ -15,6 +15,69 @@ int be_chain_product(be_ctx* ctx, const cplx* F, int N, int m, int64_t outer, in
                      const cplx* d_close, int phi_at, cplx** Wout);
 
 // ---------------------------------------------------------------------------------------------
+// optional profile: one CUDA event pair per launch of the instrumented kernel classes
+struct be_prof {
+  bool on = false;
+  std::vector<cudaEvent_t> ev;     // pairs
+  std::vector<int> cls;
+  size_t used = 0;                 // pairs in use
+  double bytes[PK_COUNT] = {0}, flops[PK_COUNT] = {0};
+  int64_t count[PK_COUNT] = {0};
+};
+
+void be_prof_begin(be_ctx* ctx, int cls) {
+  be_prof* p = ctx->prof;
+  if (!p || !p->on) return;
+  if (p->used * 2 >= p->ev.size()) {
+    for (int i = 0; i < 2048; ++i) { cudaEvent_t e; cudaEventCreate(&e); p->ev.push_back(e); }
+    p->cls.resize(p->ev.size() / 2);
+  }
+  p->cls[p->used] = cls;
+  cudaEventRecord(p->ev[2 * p->used], ctx->stream);
+}
+
+void be_prof_end(be_ctx* ctx, int cls, double bytes, double flops) {
+  be_prof* p = ctx->prof;
+  if (!p || !p->on) return;
+  cudaEventRecord(p->ev[2 * p->used + 1], ctx->stream);
+  p->used++;
+  p->bytes[cls] += bytes; p->flops[cls] += flops; p->count[cls]++;
+}
+
+extern "C" int be_profile_enable(be_ctx* ctx, int on) {
+  if (!ctx) return BE_ERR_NULL;
+  if (!ctx->prof) ctx->prof = new (std::nothrow) be_prof;
+  if (!ctx->prof) return BE_ERR_NOMEM;
+  be_prof* p = ctx->prof;
+  BE_CUDA(cudaStreamSynchronize(ctx->stream));
+  p->on = on != 0;
+  p->used = 0;
+  for (int i = 0; i < PK_COUNT; ++i) { p->bytes[i] = p->flops[i] = 0; p->count[i] = 0; }
+  return BE_OK;
+}
+
+extern "C" const char* be_profile_name(int cls) {
+  static const char* names[PK_COUNT] = {"hemv", "col", "w", "zgemm", "bisect", "invit", "cluster_orth",
+                                        "hessenberg", "hqr", "jacobi", "misc"};
+  return (cls >= 0 && cls < PK_COUNT) ? names[cls] : nullptr;
+}
+
+extern "C" int be_profile_get(be_ctx* ctx, int cls, double* ms, int64_t* launches, double* bytes, double* flops) {
+  if (!ctx || !ctx->prof) return BE_ERR_NULL;
+  if (cls < 0 || cls >= PK_COUNT) return BE_ERR_SHAPE;
+  be_prof* p = ctx->prof;
+  BE_CUDA(cudaStreamSynchronize(ctx->stream));
+  double tot = 0;
+  for (size_t i = 0; i < p->used; ++i)
+    if (p->cls[i] == cls) { float t = 0; cudaEventElapsedTime(&t, p->ev[2 * i], p->ev[2 * i + 1]); tot += t; }
+  if (ms) *ms = tot;
+  if (launches) *launches = p->count[cls];
+  if (bytes) *bytes = p->bytes[cls];
+  if (flops) *flops = p->flops[cls];
+  return BE_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
 // arena
 int be_arena_reserve(be_ctx* ctx, size_t bytes) {
   ctx->arena_used = 0;
@@ -62,6 +125,7 @@ extern "C" int be_destroy(be_ctx* ctx) {
   cudaStreamSynchronize(ctx->stream);
   if (ctx->arena) cudaFree(ctx->arena);
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+  if (ctx->prof) { for (cudaEvent_t e : ctx->prof->ev) cudaEventDestroy(e); delete ctx->prof; }
   delete ctx;
   return BE_OK;
 }
@@ -82,7 +146,7 @@ extern "C" const char* be_strerror(int code) {
 
 extern "C" int be_set_workspace_limit(be_ctx* ctx, size_t bytes) {
   if (!ctx) return BE_ERR_NULL;
-  if (bytes < ((size_t)64 << 20)) return BE_ERR_SHAPE;
+  if (bytes < ((size_t)1 << 20)) return BE_ERR_SHAPE;
   ctx->ws_limit = bytes;
   return BE_OK;
 }

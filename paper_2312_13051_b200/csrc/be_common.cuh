@@ -82,7 +82,14 @@ struct be_ctx {
   size_t arena_bytes;
   size_t arena_used;
   int gemm_attr_set;
+  struct be_prof* prof;       // optional per-kernel-class CUDA-event timing (be_profile_enable)
 };
+
+// kernel classes of the profile
+enum { PK_HEMV = 0, PK_COL, PK_W, PK_GEMM, PK_BISECT, PK_INVIT, PK_ORTH, PK_HESS, PK_HQR, PK_JACOBI,
+       PK_MISC, PK_COUNT };
+void be_prof_begin(be_ctx* ctx, int cls);
+void be_prof_end(be_ctx* ctx, int cls, double bytes, double flops);
 
 #define BE_CUDA(x) do { cudaError_t e__ = (x); if (e__ != cudaSuccess) return (int)e__; } while (0)
 #define BE_TRY(x) do { int r__ = (x); if (r__ != BE_OK) return r__; } while (0)

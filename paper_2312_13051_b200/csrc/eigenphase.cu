@@ -280,12 +280,16 @@ int be_eigenvalues_general(be_ctx* ctx, cplx* W, int64_t cnt, int m, cplx* lam, 
   if (m > QR_MAXOWN * nt) return BE_ERR_UNSUPPORTED;
   const size_t sh1 = 2 * (size_t)m * sizeof(cplx);
   if (sh1 > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_hessenberg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh1));
+  be_prof_begin(ctx, PK_HESS);
   k_hessenberg<<<(unsigned)cnt, nt, sh1, st>>>(W, m);
+  be_prof_end(ctx, PK_HESS, (double)cnt * m * m * 32.0, (double)cnt * (40.0 / 3.0) * m * (double)m * m);
   ctx->launches++;
   BE_CUDA(cudaGetLastError());
   const size_t sh2 = (size_t)((m + 1) & ~1) * sizeof(double) + (size_t)m * sizeof(cplx);
   if (sh2 > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_hqr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh2));
+  be_prof_begin(ctx, PK_HQR);
   k_hqr<<<(unsigned)cnt, nt, sh2, st>>>(W, m, lam, fail);
+  be_prof_end(ctx, PK_HQR, (double)cnt * m * m * 32.0, 0.0);
   ctx->launches++;
   return (int)cudaGetLastError();
 }

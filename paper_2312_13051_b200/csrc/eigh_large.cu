@@ -574,13 +574,21 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
       break;
     }
     for (int i = p; i < pend; ++i) {
-      k_col<<<(unsigned)cnt, 256, 0, st>>>(s.Bw, s.Wp, s.d, s.e, s.tau, N, i, p);
-      LAUNCH_CHECK();
       const int n = N - i - 1;
-      const int nJ = (n + HB - 1) / HB;
-      k_hemv<<<(unsigned)(cnt * nJ), 256, 0, st>>>(s.Bw, s.P, s.zpart, N, i, nJ, nJmax);
+      const int kk = i - p;
+      be_prof_begin(ctx, PK_COL);
+      k_col<<<(unsigned)cnt, 256, 0, st>>>(s.Bw, s.Wp, s.d, s.e, s.tau, N, i, p);
+      be_prof_end(ctx, PK_COL, (double)cnt * (n + 1) * 16.0 * (2 + 2 * kk), (double)cnt * (n + 1) * 16.0 * kk);
       LAUNCH_CHECK();
+      const int nJ = (n + HB - 1) / HB;
+      be_prof_begin(ctx, PK_HEMV);
+      k_hemv<<<(unsigned)(cnt * nJ), 256, 0, st>>>(s.Bw, s.P, s.zpart, N, i, nJ, nJmax);
+      // algorithmic traffic: the lower triangle once, v in, y out; 8 real flops per complex fma, 2 per element
+      be_prof_end(ctx, PK_HEMV, (double)cnt * (0.5 * n * (n + 1.0) + 2.0 * n) * 16.0, (double)cnt * 8.0 * n * n);
+      LAUNCH_CHECK();
+      be_prof_begin(ctx, PK_W);
       k_w<<<(unsigned)cnt, 256, ysh_bytes, st>>>(s.Bw, s.Wp, s.P, s.zpart, s.tau, N, i, p, nJmax);
+      be_prof_end(ctx, PK_W, (double)cnt * n * 16.0 * (3 + 4 * kk), (double)cnt * n * 32.0 * kk);
       LAUNCH_CHECK();
     }
     const int q = pend, kb = pend - p;
@@ -616,19 +624,29 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
       BE_CUDA(cudaFuncSetAttribute(k_bisect, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
       BE_CUDA(cudaFuncSetAttribute(k_invit, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
     }
+    be_prof_begin(ctx, PK_BISECT);
     k_bisect<<<(unsigned)(cnt * nblk), 128, sh, st>>>(s.d, s.e, E, s.tnorm, N, nblk);
+    be_prof_end(ctx, PK_BISECT, (double)cnt * N * 24.0, 0.0);
     LAUNCH_CHECK();
     if (nv > 0) {
       const int nvb = (nv + 127) / 128;
+      be_prof_begin(ctx, PK_INVIT);
       k_invit<<<(unsigned)(cnt * nvb), 128, sh, st>>>(s.d, s.e, E, s.tnorm, s.fa, s.fb, s.fc, s.fp, s.Z, N, nv, nvb, 0, 3);
+      be_prof_end(ctx, PK_INVIT, (double)cnt * N * nv * 8.0, 0.0);
       LAUNCH_CHECK();
       const size_t shc = (size_t)nv * sizeof(double);
       if (shc > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_cluster_orth, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shc));
+      be_prof_begin(ctx, PK_ORTH);
       k_cluster_orth<<<(unsigned)cnt, 256, shc, st>>>(E, s.tnorm, s.Z, N, nv, 1e-3, info);
+      be_prof_end(ctx, PK_ORTH, 0.0, 0.0);
       LAUNCH_CHECK();
+      be_prof_begin(ctx, PK_INVIT);
       k_invit<<<(unsigned)(cnt * nvb), 128, sh, st>>>(s.d, s.e, E, s.tnorm, s.fa, s.fb, s.fc, s.fp, s.Z, N, nv, nvb, 1, 1);
+      be_prof_end(ctx, PK_INVIT, 0.0, 0.0);
       LAUNCH_CHECK();
+      be_prof_begin(ctx, PK_ORTH);
       k_cluster_orth<<<(unsigned)cnt, 256, shc, st>>>(E, s.tnorm, s.Z, N, nv, 1e-3, info);
+      be_prof_end(ctx, PK_ORTH, 0.0, 0.0);
       LAUNCH_CHECK();
     }
   }

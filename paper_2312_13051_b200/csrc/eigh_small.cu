@@ -124,12 +124,14 @@ int be_eigh_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
                   int nv, double* E, cplx* X, int* info) {
   const unsigned blocks = (unsigned)((cnt + 127) / 128);
   cudaStream_t st = ctx->stream;
+  be_prof_begin(ctx, PK_JACOBI);
   switch (N) {
 #define CASE(n) case n: k_jacobi<n><<<blocks, 128, 0, st>>>(H, map, loop0, cnt, nv, E, X, info); break;
     CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
 #undef CASE
     default: return BE_ERR_UNSUPPORTED;
   }
+  be_prof_end(ctx, PK_JACOBI, (double)cnt * N * (N + (double)nv + 1) * 16.0, 0.0);
   ctx->launches++;
   return (int)cudaGetLastError();
 }

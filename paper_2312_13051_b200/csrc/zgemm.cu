@@ -183,7 +183,14 @@ int launch(be_ctx* ctx, const ZgemmParams& p) {
     BE_CUDA(cudaFuncSetAttribute(zgemm_kernel<OPA, OPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM_BYTES));
     attr_done = true;
   }
+  be_prof_begin(ctx, PK_GEMM);
   zgemm_kernel<OPA, OPB><<<(unsigned)blocks, NTHREADS, SM_BYTES, ctx->stream>>>(p, tilesM, tilesN);
+  {
+    const double tri = p.lower ? 0.5 : 1.0;
+    const double fl = 8.0 * p.M * (double)p.N * p.K * (double)p.batch * tri;
+    const double by = 16.0 * (double)p.batch * ((double)p.M * p.K + (double)p.K * p.N + tri * (double)p.M * p.N * (1.0 + (p.beta.x != 0.0 || p.beta.y != 0.0)));
+    be_prof_end(ctx, PK_GEMM, by, fl);
+  }
   ctx->launches++;
   return (int)cudaGetLastError();
 }

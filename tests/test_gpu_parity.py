@@ -1,0 +1,321 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Tolerances (BASELINE.json north_star, written here):
+  eigenvalues      |dE| <= 1e-10 * ||H||_2
+  WCC phases       <= 1e-8 in units of 2 pi, sorted points on the circle (R7 comparator), on loops
+                   with a spectral gap
+  invariants       equal as integers / half-integers
+Eigenvectors, Wannier-band vectors, PSO eigenvectors and W itself are gauge dependent and are
+checked only through residuals / orthonormality.
+"""
+import math
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import wilson_oracle as wo
+from paper_2312_13051_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+E_TOL = 1e-10
+PH_TOL = 1e-8  # units of 2 pi
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_2312_13051_b200.binding import Context
+    c = Context()
+    yield c
+    c.close()
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def phase_dist(a, b):
+    """max over loops of the R7 circular distance, in units of 2 pi."""
+    return max(wo.circ_sorted_distance(a[i], b[i]) for i in range(a.shape[0])) / (2 * np.pi)
+
+
+def check_eigh(ctx, H, nv):
+    E, U, info = ctx.eigh_batched(dev(H), nv, want_info=True)
+    E, info = E.cpu().numpy(), info.cpu().numpy()
+    U = U.cpu().numpy() if U is not None else None
+    Eo, _ = wo.eigh_batched(H)
+    assert info.max() == 0
+    for c in range(H.shape[0]):
+        nrm = max(np.abs(Eo[c]).max(), 1e-300)
+        assert np.abs(E[c] - Eo[c]).max() <= E_TOL * nrm
+        assert np.all(np.diff(E[c]) >= 0)
+        if nv:
+            N = H.shape[1]
+            assert np.linalg.norm(H[c] @ U[c] - U[c] * E[c][:nv]) <= 1e-11 * nrm * N
+            assert np.linalg.norm(U[c].conj().T @ U[c] - np.eye(nv)) <= 1e-11 * N
+
+
+# ------------------------------------------------------------------------------ S1
+@pytest.mark.parametrize("N", [1, 2, 3, 4, 7, 8])
+def test_eigh_jacobi_path(ctx, N):
+    rng = np.random.default_rng(N)
+    A = rng.standard_normal((37, N, N)) + 1j * rng.standard_normal((37, N, N))
+    check_eigh(ctx, A + A.conj().transpose(0, 2, 1), N)
+
+
+def test_eigh_jacobi_chiral_degenerate_models(ctx):
+    """H3: E = +-eps doubly degenerate (BHZ, BBH) -- the case one-sided Jacobi on H itself misses."""
+    check_eigh(ctx, wl.config1_grid(13, 9).reshape(-1, 4, 4), 4)
+    check_eigh(ctx, wl.config2_grid(11, 6).reshape(-1, 4, 4), 2)
+
+
+@pytest.mark.parametrize("N,nv", [(9, 9), (31, 10), (64, 32), (65, 65), (100, 37), (257, 128)])
+def test_eigh_tridiagonal_path_random(ctx, N, nv):
+    """sizes spanning several 32-panels / 64-blocks and ragged tails"""
+    rng = np.random.default_rng(N)
+    A = rng.standard_normal((3, N, N)) + 1j * rng.standard_normal((3, N, N))
+    check_eigh(ctx, A + A.conj().transpose(0, 2, 1), nv)
+
+
+def test_eigh_degenerate_clean_supercell_and_identity(ctx):
+    """H4: heavily degenerate spectra (clean supercell at t=0), plus diagonal / scaled identity."""
+    pc = wl.bhz_supercell_parts(6)
+    H = np.array([wl.assemble_supercell(pc, 0.0, 0.0), wl.assemble_supercell(pc, 0.5, 0.0),
+                  wl.assemble_supercell(pc, 0.17, 0.4)])
+    check_eigh(ctx, H, 72)
+    D = np.zeros((2, 20, 20), dtype=complex)
+    D[0] = 2.5 * np.eye(20)
+    D[1] = np.diag(np.arange(20) % 3).astype(complex)
+    check_eigh(ctx, D, 20)
+
+
+def test_eigh_config3_and_config5_matrices(ctx):
+    p3 = wl.config3_parts(1)
+    H = np.array([wl.assemble_supercell(p3, i / 33, 5 / 32) for i in (0, 7, 20)])
+    check_eigh(ctx, H, 200)
+    p5 = wl.config5_parts()
+    rng = np.random.default_rng(5)
+    H = np.array([wl.assemble_config5(p5, 2 * np.pi * rng.uniform(0, 1, 3)) for _ in range(40)])
+    check_eigh(ctx, H, 32)
+
+
+def test_eigh_edge_cases(ctx):
+    H = dev(wl.config1_grid(4, 3).reshape(-1, 4, 4))
+    E, U = ctx.eigh_batched(H, 0)            # eigenvalues only
+    assert U is None and E.shape == (12, 4)
+    E0, U0 = ctx.eigh_batched(H[:0], 2)      # empty batch
+    assert E0.shape == (0, 4)
+    # only the upper triangle of the row-major input is read
+    A = wl.assemble_config5(wl.config5_parts(), np.array([0.3, 0.2, 0.1]))[None]
+    Au = A.copy()
+    Au[0][np.tril_indices(64, -1)] = 123.0
+    E1, _ = ctx.eigh_batched(dev(A), 0)
+    E2, _ = ctx.eigh_batched(dev(Au), 0)
+    assert torch.equal(E1, E2)
+
+
+def test_error_codes(ctx):
+    from paper_2312_13051_b200.binding import BerryEasyError
+    H = dev(wl.config1_grid(4, 3)[None])
+    with pytest.raises(BerryEasyError):
+        ctx.wilson_loop(H, 5, 1)          # n_occ > N
+    with pytest.raises(BerryEasyError):
+        ctx.wilson_loop(H, 2, 2)          # dir out of range
+    with pytest.raises(BerryEasyError):
+        ctx.nested_wilson(H, 2, 1, 1)     # dir1 == dir2
+    assert ctx.lib.be_eigh_batched(ctx._h, None, 1, 4, 4, None, None, None) == -1
+
+
+# ------------------------------------------------------------------------------ config 1 (full size)
+def test_config1_full_wilson_and_spin_resolved(ctx):
+    H = wl.config1_grid()[None]                       # [1][101][100][4][4]
+    th, ab, mg = ctx.wilson_loop(dev(H), 2, 1)
+    tho, abo, mgo = wo.wilson_surface(H, 2, 1)
+    th, ab, mg = th.cpu().numpy(), ab.cpu().numpy(), mg.cpu().numpy()
+    assert mgo.min() > 1.9
+    assert np.abs(mg - mgo).max() < 1e-12
+    assert phase_dist(th, tho) <= PH_TOL
+    assert np.abs(np.sort(ab, 1) - np.sort(abo, 1)).max() < 1e-10
+    S = wl.bhz4_spin_z()
+    lo, hi, pso = ctx.spin_resolved_wilson(dev(H), 2, 1, dev(S))
+    loo, hio, psoo = wo.spin_resolved_surface(H, 2, 1, S)
+    assert phase_dist(lo.cpu().numpy(), loo) <= PH_TOL
+    assert phase_dist(hi.cpu().numpy(), hio) <= PH_TOL
+    assert np.abs(pso.cpu().numpy() - psoo).max() < 1e-10
+    # invariants, exact: total winding 0, sectors +-1 (device winding kernel vs oracle)
+    w = ctx.winding(torch.stack([th_.reshape(101, -1) for th_ in (lo, hi)])).cpu().numpy()
+    assert [int(round(x)) for x in w] == [int(round(wo.winding(loo))), int(round(wo.winding(hio)))] == [1, -1]
+    wt = ctx.winding(torch.from_numpy(th).cuda().reshape(1, 101, 2)).cpu().numpy()
+    assert int(round(wt[0])) == int(round(wo.winding(tho))) == 0
+    assert np.abs(w - np.rint(w)).max() < 1e-9
+
+
+def test_qwz_chern_number_device(ctx):
+    H = wl.qwz_grid(100, 100)[None]
+    th, _, _ = ctx.wilson_loop(dev(H), 1, 1)
+    tho, _, _ = wo.wilson_surface(H, 1, 1)
+    assert phase_dist(th.cpu().numpy(), tho) <= PH_TOL
+    w = ctx.winding(th.reshape(1, 100, 1)).cpu().numpy()[0]
+    assert int(round(-w)) == wo.chern_number(tho) == 1
+
+
+def test_loop_direction_and_batch_axes(ctx):
+    """dir = 0 (loops strided in memory), 3 grid axes, batch > 1."""
+    p5 = wl.config5_parts(norb_spatial=8)
+    H = wl.config5_grid(p5, 5, 4, 6, ix=range(5), iy=range(4))      # [5][4][6][16][16]
+    H4 = np.stack([H, H[::-1].copy()])                              # batch 2, ndim 3
+    for d in (0, 1, 2):
+        th, _, _ = ctx.wilson_loop(dev(H4), 8, d)
+        tho, _, _ = wo.wilson_surface(H4, 8, d)
+        assert phase_dist(th.cpu().numpy(), tho) <= PH_TOL
+
+
+def test_closing_phase_position_gauge(ctx):
+    for v, w_ in ((1.0, 0.5), (0.5, 1.0)):
+        H, phi = wl.ssh_loop(v, w_, 50, position_gauge=True)
+        th, _, _ = ctx.wilson_loop(dev(H[None]), 1, 0, close=dev(phi))
+        tho, _, _ = wo.wilson_loop(H, 1, close=phi)
+        assert abs(wo.wrap_pi(th.cpu().numpy()[0, 0] - tho[0])) / (2 * np.pi) <= PH_TOL
+    # multi-band: supercell in the position gauge along x with Phi = exp(-i 2 pi x / L)
+    L, n1 = 3, 7
+    parts = wl.bhz_supercell_parts(L)
+    xs = np.repeat(np.arange(L), L * 4).astype(float)
+    Hl = []
+    for i in range(n1):
+        D = np.exp(1j * 2 * np.pi * (i / n1) * xs / L)
+        Hl.append((np.conj(D)[:, None] * wl.assemble_supercell(parts, i / n1, 0.37)) * D[None, :])
+    Hl = np.array(Hl)
+    phi = np.exp(-1j * 2 * np.pi * xs / L)
+    th, _, _ = ctx.wilson_loop(dev(Hl[None]), 18, 0, close=dev(phi))
+    tho, _, _ = wo.wilson_loop(Hl, 18, close=phi)
+    assert phase_dist(th.cpu().numpy(), tho[None]) <= PH_TOL
+
+
+def test_degenerate_loops_single_point_and_full_filling(ctx):
+    H = wl.config1_grid(1, 3)[None]                   # N1 = 1: W = U^dagger U = 1
+    th, ab, mg = ctx.wilson_loop(dev(H), 2, 1)
+    assert np.abs(th.cpu().numpy()).max() < 1e-12 and np.abs(ab.cpu().numpy() - 1).max() < 1e-12
+    H = wl.config1_grid(9, 2)[None]                   # n_occ = N: every link unitary, mingap = +inf
+    th, ab, mg = ctx.wilson_loop(dev(H), 4, 1)
+    tho, abo, _ = wo.wilson_surface(H, 4, 1)
+    assert phase_dist(th.cpu().numpy(), tho) <= PH_TOL
+    assert np.abs(ab.cpu().numpy() - 1).max() < 1e-12 and np.all(np.isinf(mg.cpu().numpy()))
+
+
+# ------------------------------------------------------------------------------ config 2 (full size)
+def test_config2_full_nested_polarization(ctx):
+    H = wl.config2_grid()                              # [100][100][4][4]
+    th1, thn = ctx.nested_wilson(dev(H[None]), 2, 1, 0)
+    th1o, thno = wo.nested_wilson(H, 2)
+    assert phase_dist(th1.cpu().numpy()[0], th1o) <= PH_TOL
+    thn = thn.cpu().numpy()[0]
+    assert wo.circ_sorted_distance(thn, thno) / (2 * np.pi) <= PH_TOL
+    assert wo.nested_polarization(thn) == wo.nested_polarization(thno) == 0.5
+
+
+@pytest.mark.parametrize("gamma,p", [(0.5, 0.5), (1.5, 0.0)])
+def test_nested_variants(ctx, gamma, p):
+    H = wl.config2_grid(30, 24, gamma=gamma)
+    for base, band in ((0, 1), (7, 0)):
+        th1, thn = ctx.nested_wilson(dev(H[None]), 2, 1, 0, base=base, wb_lo=band, wb_hi=band + 1)
+        th1o, thno = wo.nested_wilson(H, 2, base=base, wb_lo=band, wb_hi=band + 1)
+        assert phase_dist(th1.cpu().numpy()[0], th1o) <= PH_TOL
+        assert wo.circ_sorted_distance(thn.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
+        assert wo.nested_polarization(thn.cpu().numpy()[0]) == p
+    # both Wannier bands: nested phases of the full occupied space
+    th1, thn = ctx.nested_wilson(dev(H[None]), 2, 1, 0, wb_lo=0, wb_hi=2)
+    _, thno = wo.nested_wilson(H, 2, wb_lo=0, wb_hi=2)
+    assert wo.circ_sorted_distance(thn.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
+    # dir1 = 0, dir2 = 1 on the transposed grid gives the same numbers
+    Ht = np.ascontiguousarray(H.transpose(1, 0, 2, 3))
+    _, thn_t = ctx.nested_wilson(dev(Ht[None]), 2, 0, 1)
+    _, thno = wo.nested_wilson(H, 2)
+    assert wo.circ_sorted_distance(thn_t.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
+
+
+# ------------------------------------------------------------------------------ config 3 (reduced)
+def test_config3_reduced_disordered_supercell(ctx):
+    """N = 400, n_occ = 200, 2 realizations x 2 t2 x 33 t1 (full loop length, full matrix size)."""
+    parts = [wl.config3_parts(r) for r in (0, 5)]
+    H = wl.supercell_grid(parts, 33, 32, t2_indices=[0, 13])
+    th, ab, mg = ctx.wilson_loop(dev(H), 200, 1)
+    tho, abo, mgo = wo.wilson_surface(H, 200, 1)
+    assert mgo.min() > 0.1
+    assert np.abs(mg.cpu().numpy() - mgo).max() < 1e-10 * 4
+    assert phase_dist(th.cpu().numpy(), tho) <= PH_TOL
+    assert np.abs(np.sort(ab.cpu().numpy(), 1) - np.sort(abo, 1)).max() < 1e-9
+
+
+# ------------------------------------------------------------------------------ config 4 (reduced)
+def test_config4_reduced_spin_resolved_supercell(ctx):
+    """L = 8 (N = 256, sectors of 64) full loop length, z impurities ([H,S]=0) and x impurities."""
+    for axis in ("z", "x"):
+        parts = wl.config4_parts(8, axis=axis)
+        H = wl.supercell_grid([parts], 25, 24, t2_indices=[0, 11])
+        S = wl.supercell_spin_z(8)
+        lo, hi, pso = ctx.spin_resolved_wilson(dev(H), 128, 1, dev(S))
+        loo, hio, psoo = wo.spin_resolved_surface(H, 128, 1, S)
+        assert np.abs(pso.cpu().numpy() - psoo).max() < 1e-10
+        assert phase_dist(lo.cpu().numpy(), loo) <= PH_TOL
+        assert phase_dist(hi.cpu().numpy(), hio) <= PH_TOL
+        if axis == "z":
+            assert np.abs(np.abs(psoo) - 1).max() < 1e-10
+    # dense spin operator gives the same answer as the diagonal one
+    lo2, hi2, _ = ctx.spin_resolved_wilson(dev(H), 128, 1, dev(np.diag(S).astype(complex)))
+    assert phase_dist(lo2.cpu().numpy(), loo) <= PH_TOL
+    # uneven split (shape contract only)
+    lo3, hi3, _ = ctx.spin_resolved_wilson(dev(H), 128, 1, dev(S), m_lo=60)
+    assert lo3.shape == (2, 60) and hi3.shape == (2, 68)   # split inside a PSO cluster: values not unique
+
+
+def test_config4_full_matrix_size_one_short_loop(ctx):
+    """N = 1600, n_occ = 800 -> 2 x 400: 4 loop points (oracle ~10 s)."""
+    parts = wl.config4_parts(20)
+    H = wl.supercell_grid([parts], 4, 24, t2_indices=[3])
+    S = wl.supercell_spin_z(20)
+    lo, hi, pso = ctx.spin_resolved_wilson(dev(H), 800, 1, dev(S))
+    loo, hio, psoo = wo.spin_resolved_surface(H, 800, 1, S)
+    assert np.abs(pso.cpu().numpy() - psoo).max() < 1e-10
+    assert phase_dist(lo.cpu().numpy(), loo) <= PH_TOL
+    assert phase_dist(hi.cpu().numpy(), hio) <= PH_TOL
+
+
+# ------------------------------------------------------------------------------ config 5 (reduced)
+def test_config5_reduced_wannier_like(ctx):
+    p5 = wl.config5_parts()
+    H = wl.config5_grid(p5, 64, 64, 65, ix=[0, 17], iy=[3, 31, 60])   # 6 loops x 65 points
+    th, ab, mg = ctx.wilson_loop(dev(H), 32, 2)
+    tho, abo, mgo = wo.wilson_surface(H, 32, 2)
+    assert mgo.min() >= 0.2
+    assert phase_dist(th.cpu().numpy(), tho) <= PH_TOL
+    # device grid assembly used by bench.py reproduces the host grid
+    Ht = wl.config5_grid_torch(p5, 64, 64, 65, "cuda", ix=[0, 17], iy=[3, 31, 60])
+    assert np.abs(Ht.cpu().numpy() - H).max() < 1e-12
+
+
+# ------------------------------------------------------------------------------ host-buffer variants
+def test_host_variants_match_device(ctx):
+    parts = wl.config4_parts(4, axis="x")
+    H = wl.supercell_grid([parts], 6, 5)
+    S = wl.supercell_spin_z(4)
+    Hh = torch.from_numpy(H).pin_memory()
+    ctx.set_workspace_limit(1 << 20)         # force several chunks and the double-buffered stream
+    try:
+        lo, hi, pso = ctx.spin_resolved_wilson_host(Hh, 32, 1, torch.from_numpy(S))
+        th, ab, mg = ctx.wilson_loop_host(Hh, 32, 1)
+    finally:
+        ctx.set_workspace_limit(64 << 30)
+    lod, hid, psod = ctx.spin_resolved_wilson(dev(H), 32, 1, dev(S))
+    thd, abd, mgd = ctx.wilson_loop(dev(H), 32, 1)
+    assert torch.equal(lo, lod.cpu()) and torch.equal(hi, hid.cpu()) and torch.equal(pso, psod.cpu())
+    assert torch.equal(th, thd.cpu()) and torch.equal(mg, mgd.cpu())
+    tho, _, _ = wo.wilson_surface(H, 32, 1)
+    assert phase_dist(th.numpy(), tho) <= PH_TOL
+
+
+def test_launch_counter_counts_kernels(ctx):
+    n0 = ctx.launch_count()
+    ctx.wilson_loop(dev(wl.config1_grid(6, 2)[None]), 2, 1)
+    assert ctx.launch_count() > n0
