@@ -193,8 +193,10 @@ extern "C" size_t be_workspace_bytes(const be_grid* g, int n_occ, int op) {
 // ---------------------------------------------------------------------------------------------
 extern "C" int be_eigh_batched(be_ctx* ctx, const void* dH, int64_t count, int N, int n_vec,
                                double* dE, void* dU, int* d_info) {
-  if (!ctx || !dH || !dE) return BE_ERR_NULL;
+  if (!ctx) return BE_ERR_NULL;
   if (count < 0 || N < 1 || n_vec < 0 || n_vec > N) return BE_ERR_SHAPE;
+  if (count == 0) return BE_OK;
+  if (!dH || !dE) return BE_ERR_NULL;
   if (!aligned(dH, 16) || !aligned(dE, 8) || (dU && !aligned(dU, 16))) return BE_ERR_ALIGN;
   if (count == 0) return BE_OK;
   const int nv = dU ? n_vec : 0;

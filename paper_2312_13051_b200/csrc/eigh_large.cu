@@ -25,6 +25,9 @@ namespace {
 constexpr int NB = 32;    // panel width (tridiagonalization and WY blocks)
 constexpr int HB = 64;    // block-column width of the symmetric matrix-vector kernel
 constexpr int HSTRIPE = 256;
+constexpr double SPLIT_TOL = 32.0;     // |e_i| <= max(SPLIT_TOL, N) * eps * ||T|| splits the tridiagonal matrix
+                                       // (the backward error of the reduction itself is O(N eps ||T||))
+constexpr double CLUSTER_TOL = 3e-4;   // eigenvalues closer than this (relative to ||T||) are re-orthogonalized
 
 // ------------------------------------------------------------------------------------------
 __global__ void k_gather(const cplx* __restrict__ H, cplx* __restrict__ Bw, GridMap map,
@@ -214,7 +217,8 @@ __global__ void __launch_bounds__(256) k_w(const cplx* __restrict__ Bw, cplx* __
 // Sturm-count bisection: one thread per eigenvalue index, d and e^2 in shared memory.
 __global__ void __launch_bounds__(128) k_bisect(const double* __restrict__ dd, const double* __restrict__ ee,
                                                 double* __restrict__ lam, double* __restrict__ tnorm,
-                                                int N, int nblk) {
+                                                double* __restrict__ blo, double* __restrict__ bhi,
+                                                int* __restrict__ bcl, int N, int nblk) {
   extern __shared__ double sh[];   // d[N], e2[N]
   __shared__ double rmin[4], rmax[4], remax[4];
   double* d = sh; double* e2 = sh + N;
@@ -244,13 +248,24 @@ __global__ void __launch_bounds__(128) k_bisect(const double* __restrict__ dd, c
   if (tn == 0.0) tn = DBL_MIN;
   gl -= 2.0 * tn * eps * N + 2.0 * DBL_MIN;
   gu += 2.0 * tn * eps * N + 2.0 * DBL_MIN;
-  const double pivmin = DBL_MIN * fmax(1.0, emax);
+  const double pivmin = DBL_MIN * fmax(1.0, tn * tn);
+  (void)emax;
   const int k = kb * 128 + tid;
   if (kb == 0 && tid == 0) tnorm[c] = tn;
+  // negligible couplings are dropped (T splits into unreduced blocks); k_invit applies the same rule
+  const double split = fmax(SPLIT_TOL, (double)N) * DBL_EPSILON * tn;
+  for (int r = tid; r < N; r += 128) if (e2[r] <= split * split) e2[r] = 0.0;
+  __syncthreads();
   if (k >= N) return;
   double lo = gl, hi = gu;
+  int cnt_lo = 0;
   const double atol = 0.25 * eps * tn;
-  for (int it = 0; it < 128; ++it) {
+  // A fixed depth for every eigenvalue of the matrix: all final intervals are cells of one dyadic
+  // grid, so eigenvalues that cannot be separated share the same cell and k_invit can assign them
+  // to blocks consistently.
+  int depth = (int)ceil(log2((gu - gl) / atol)) + 1;
+  depth = depth < 1 ? 1 : (depth > 120 ? 120 : depth);
+  for (int it = 0; it < depth; ++it) {
     const double mid = 0.5 * (lo + hi);
     if (!(mid > lo && mid < hi)) break;
     int cnt = 0;
@@ -262,10 +277,10 @@ __global__ void __launch_bounds__(128) k_bisect(const double* __restrict__ dd, c
       if (fabs(q) < pivmin) q = -pivmin;
       cnt += (q < 0.0);
     }
-    if (cnt > k) hi = mid; else lo = mid;
-    if (hi - lo <= atol) break;
+    if (cnt > k) hi = mid; else { lo = mid; cnt_lo = cnt; }
   }
   lam[c * N + k] = 0.5 * (lo + hi);
+  blo[c * N + k] = lo; bhi[c * N + k] = hi; bcl[c * N + k] = cnt_lo;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -282,25 +297,63 @@ __global__ void __launch_bounds__(128) k_invit(const double* __restrict__ dd, co
                                                const double* __restrict__ lam, const double* __restrict__ tnorm,
                                                double* __restrict__ fa, double* __restrict__ fb,
                                                double* __restrict__ fc, unsigned char* __restrict__ fp,
-                                               double* __restrict__ Z, int N, int nv, int nvb,
-                                               int refine, int iters) {
+                                               int* __restrict__ blk, const double* __restrict__ blo,
+                                               const double* __restrict__ bhi, const int* __restrict__ bcl,
+                                               double* __restrict__ Z, int N, int nv,
+                                               int nvb, int refine, int iters) {
   extern __shared__ double sh[];   // d[N], e[N]
   double* d = sh; double* e = sh + N;
   const int64_t c = blockIdx.x / nvb;
   const int vb = blockIdx.x % nvb;
-  for (int r = threadIdx.x; r < N; r += 128) { d[r] = dd[c * N + r]; e[r] = (r < N - 1) ? ee[c * N + r] : 0.0; }
+  const double tn = tnorm[c];
+  const double tol = DBL_EPSILON * tn;
+  // T is split where an off-diagonal entry is negligible: eigenvectors live on one unreduced block,
+  // which makes vectors of exactly degenerate eigenvalues (different blocks) orthogonal for free.
+  for (int r = threadIdx.x; r < N; r += 128) {
+    d[r] = dd[c * N + r];
+    double er = (r < N - 1) ? ee[c * N + r] : 0.0;
+    { const double sp = fmax(SPLIT_TOL, (double)N) * DBL_EPSILON * tn; if (er * er <= sp * sp) er = 0.0; }   // as in k_bisect
+    e[r] = er;
+  }
   __syncthreads();
   const int v = vb * 128 + threadIdx.x;
   if (v >= nv) return;
-  const double sig = lam[c * N + v];
-  const double tol = DBL_EPSILON * tnorm[c];
+  const double* l = lam + c * N;
+  const double sig = l[v];
   const int64_t base = c * (int64_t)N * nv + v;   // element (row r) at base + r*nv
+  int bs = 0, be = N - 1;
   if (!refine) {
-    double ai = d[0] - sig, bi = e[0];
-    for (int r = 0; r < N - 1; ++r) {
+    // Which unreduced block owns the v-th eigenvalue: bisection ended with count(lo) <= v <
+    // count(hi); the Sturm count of the split matrix is the sum of the block counts (same
+    // arithmetic as k_bisect), so walking the blocks in order and counting their eigenvalues in
+    // (lo, hi] locates instance number v - count(lo) exactly.
+    const double xm = blo[c * N + v], xp = bhi[c * N + v];
+    int rem = v - bcl[c * N + v];
+    const double pivmin = DBL_MIN * fmax(1.0, tn * tn);
+    int cm = 0, cp = 0, start = 0;
+    bool found = false;
+    double qm = 0.0, qp = 0.0;
+    for (int r = 0; r < N; ++r) {
+      if (r == start) { qm = d[r] - xm; qp = d[r] - xp; }
+      else { const double e2 = e[r - 1] * e[r - 1]; qm = d[r] - xm - e2 / qm; qp = d[r] - xp - e2 / qp; }
+      if (fabs(qm) < pivmin) qm = -pivmin;
+      if (fabs(qp) < pivmin) qp = -pivmin;
+      cm += (qm < 0.0); cp += (qp < 0.0);
+      if (r == N - 1 || e[r] == 0.0) {   // end of a block
+        const int inst = cp - cm;
+        if (rem >= 0 && rem < inst) { bs = start; be = r; found = true; break; }
+        rem -= inst;
+        cm = 0; cp = 0; start = r + 1;
+      }
+    }
+    if (!found) { bs = 0; be = N - 1; }
+    // when the fallback spans several blocks the zero couplings are harmless for the pivoted LU
+    blk[(c * nv + v) * 2] = bs; blk[(c * nv + v) * 2 + 1] = be;
+    double ai = d[bs] - sig, bi = e[bs];
+    for (int r = bs; r < be; ++r) {
       const double sub = e[r];
       const double nd = d[r + 1] - sig;
-      const double ns = e[r + 1];               // e[N-1] == 0
+      const double ns = (r + 1 < be) ? e[r + 1] : 0.0;
       const bool swap = fabs(sub) > fabs(ai);
       double piv = swap ? sub : ai;
       if (fabs(piv) < tol) piv = (piv < 0.0) ? -tol : tol;
@@ -315,16 +368,20 @@ __global__ void __launch_bounds__(128) k_invit(const double* __restrict__ dd, co
       ai = an; bi = bn;
     }
     if (fabs(ai) < tol) ai = (ai < 0.0) ? -tol : tol;
-    fa[base + (int64_t)(N - 1) * nv] = 1.0 / ai;
-    fb[base + (int64_t)(N - 1) * nv] = 0.0;
+    fa[base + (int64_t)be * nv] = 1.0 / ai;
+    fb[base + (int64_t)be * nv] = 0.0;
+    for (int r = 0; r < bs; ++r) Z[base + (int64_t)r * nv] = 0.0;
+    for (int r = be + 1; r < N; ++r) Z[base + (int64_t)r * nv] = 0.0;
+  } else {
+    bs = blk[(c * nv + v) * 2]; be = blk[(c * nv + v) * 2 + 1];
   }
   double ssq = 0.0;
   for (int it = 0; it < iters; ++it) {
     // forward elimination with the stored interchanges
     const bool gen = (!refine && it == 0);
     const uint64_t seed = ((uint64_t)(c * 1315423911ull) ^ ((uint64_t)v << 32));
-    double cur = gen ? hash_uniform(seed) : Z[base];
-    for (int r = 0; r < N - 1; ++r) {
+    double cur = gen ? hash_uniform(seed + (uint64_t)bs * 0x632BE59BD9B4E019ull) : Z[base + (int64_t)bs * nv];
+    for (int r = bs; r < be; ++r) {
       const double nxt = gen ? hash_uniform(seed + (uint64_t)(r + 1) * 0x632BE59BD9B4E019ull)
                              : Z[base + (int64_t)(r + 1) * nv];
       const double m = fc[base + (int64_t)r * nv];
@@ -332,38 +389,49 @@ __global__ void __launch_bounds__(128) k_invit(const double* __restrict__ dd, co
       else { Z[base + (int64_t)r * nv] = cur; cur = nxt - m * cur; }
     }
     // back substitution (U has two super-diagonals; the second is e[r+1] on swapped rows)
-    double x1 = cur * fa[base + (int64_t)(N - 1) * nv], x2 = 0.0;
+    double x1 = cur * fa[base + (int64_t)be * nv], x2 = 0.0;
     ssq = x1 * x1;
-    Z[base + (int64_t)(N - 1) * nv] = x1;
-    for (int r = N - 2; r >= 0; --r) {
-      const double d2 = fp[base + (int64_t)r * nv] ? e[r + 1] : 0.0;
+    Z[base + (int64_t)be * nv] = x1;
+    for (int r = be - 1; r >= bs; --r) {
+      const double d2 = (fp[base + (int64_t)r * nv] && r + 1 < be) ? e[r + 1] : 0.0;
       const double x0 = (Z[base + (int64_t)r * nv] - fb[base + (int64_t)r * nv] * x1 - d2 * x2) * fa[base + (int64_t)r * nv];
       Z[base + (int64_t)r * nv] = x0;
       ssq += x0 * x0;
       x2 = x1; x1 = x0;
     }
     if (it + 1 < iters && ssq > 1e200) {   // guard against overflow on the next solve
-      const double s = rsqrt(ssq);
-      for (int r = 0; r < N; ++r) Z[base + (int64_t)r * nv] *= s;
+      const double sc = rsqrt(ssq);
+      for (int r = bs; r <= be; ++r) Z[base + (int64_t)r * nv] *= sc;
     }
   }
-  const double s = (ssq > 0.0) ? 1.0 / sqrt(ssq) : 0.0;
-  for (int r = 0; r < N; ++r) Z[base + (int64_t)r * nv] *= s;
+  const double sc = (ssq > 0.0) ? 1.0 / sqrt(ssq) : 0.0;
+  for (int r = bs; r <= be; ++r) Z[base + (int64_t)r * nv] *= sc;
 }
 
 // ------------------------------------------------------------------------------------------
 // Orthogonalize the vectors of each cluster of close eigenvalues (gap <= ctol * ||T||) by
 // classical Gram-Schmidt applied twice, one CTA per matrix.
 __global__ void __launch_bounds__(256) k_cluster_orth(const double* __restrict__ lam, const double* __restrict__ tnorm,
-                                                      double* __restrict__ Z, int N, int nv, double ctol, int* __restrict__ info) {
-  extern __shared__ double shd[];      // rs[nv]
+                                                      const int* __restrict__ blk, double* __restrict__ Z, int N, int nv,
+                                                      double ctol, int* __restrict__ info) {
+  extern __shared__ double shd[];      // rs[nv] (double), perm[nv] (int)
   __shared__ double red[33];
-  __shared__ int s_start, s_len, s_next;
+  __shared__ int s_start, s_len, s_next, s_r0, s_r1;
+  int* perm = (int*)(shd + nv);
   const int64_t c = blockIdx.x;
+  const int* bk = blk + c * (int64_t)nv * 2;
   const int tid = threadIdx.x;
   double* Zc = Z + c * (int64_t)N * nv;
   const double* l = lam + c * N;
   const double gaptol = ctol * tnorm[c];
+  // order the vectors by (block, eigenvalue index): close eigenvalues of one unreduced block become
+  // neighbours even when eigenvalues of other blocks lie between them
+  for (int v = tid; v < nv; v += 256) {
+    const int b = bk[2 * v];
+    int rank = 0;
+    for (int u = 0; u < nv; ++u) { const int bu = bk[2 * u]; rank += (bu < b) || (bu == b && u < v); }
+    perm[rank] = v;
+  }
   if (tid == 0) s_next = 0;
   __syncthreads();
   while (true) {
@@ -371,27 +439,31 @@ __global__ void __launch_bounds__(256) k_cluster_orth(const double* __restrict__
       int s = s_next, len = 0;
       while (s < nv) {
         int e = s + 1;
-        while (e < nv && l[e] - l[e - 1] <= gaptol) ++e;
+        while (e < nv && bk[2 * perm[e]] == bk[2 * perm[s]] && l[perm[e]] - l[perm[e - 1]] <= gaptol) ++e;
         if (e - s > 1) { len = e - s; break; }
         s = e;
       }
       s_start = s; s_len = len; s_next = s + len;
+      if (len) { s_r0 = bk[2 * perm[s]]; s_r1 = bk[2 * perm[s] + 1] + 1; }
     }
     __syncthreads();
     const int s0 = s_start, len = s_len;
     if (len == 0) break;
+    const int r0 = s_r0, r1 = s_r1;   // the cluster's vectors are supported on rows [r0, r1)
     for (int j = 0; j < len; ++j) {
+      const int cj = perm[s0 + j];
       for (int pass = 0; pass < 2 && j > 0; ++pass) {
-        // r_k = sum_i Z[i][s0+k] Z[i][s0+j], k < j, in chunks of 8
+        // r_k = sum_i Z[i][col k] Z[i][col j], k < j, in chunks of 8
         for (int k0 = 0; k0 < j; k0 += 8) {
           double acc[8];
+          int ck[8];
 #pragma unroll
-          for (int q = 0; q < 8; ++q) acc[q] = 0.0;
-          for (int r = tid; r < N; r += 256) {
-            const double zj = Zc[(int64_t)r * nv + s0 + j];
+          for (int q = 0; q < 8; ++q) { acc[q] = 0.0; ck[q] = (k0 + q < j) ? perm[s0 + k0 + q] : cj; }
+          for (int r = r0 + tid; r < r1; r += 256) {
+            const double zj = Zc[(int64_t)r * nv + cj];
 #pragma unroll
             for (int q = 0; q < 8; ++q)
-              if (k0 + q < j) acc[q] = fma(Zc[(int64_t)r * nv + s0 + k0 + q], zj, acc[q]);
+              if (k0 + q < j) acc[q] = fma(Zc[(int64_t)r * nv + ck[q]], zj, acc[q]);
           }
 #pragma unroll
           for (int q = 0; q < 8; ++q) {
@@ -400,19 +472,19 @@ __global__ void __launch_bounds__(256) k_cluster_orth(const double* __restrict__
           }
         }
         __syncthreads();
-        for (int r = tid; r < N; r += 256) {
-          double zj = Zc[(int64_t)r * nv + s0 + j];
-          for (int k = 0; k < j; ++k) zj = fma(-shd[k], Zc[(int64_t)r * nv + s0 + k], zj);
-          Zc[(int64_t)r * nv + s0 + j] = zj;
+        for (int r = r0 + tid; r < r1; r += 256) {
+          double zj = Zc[(int64_t)r * nv + cj];
+          for (int k = 0; k < j; ++k) zj = fma(-shd[k], Zc[(int64_t)r * nv + perm[s0 + k]], zj);
+          Zc[(int64_t)r * nv + cj] = zj;
         }
         __syncthreads();
       }
       double ss = 0.0;
-      for (int r = tid; r < N; r += 256) { const double z = Zc[(int64_t)r * nv + s0 + j]; ss = fma(z, z, ss); }
+      for (int r = r0 + tid; r < r1; r += 256) { const double z = Zc[(int64_t)r * nv + cj]; ss = fma(z, z, ss); }
       ss = block_sum(ss, red);
       if (j > 0 && ss < 1e-20 && tid == 0 && info) atomicAdd(&info[c], 1);   // dependent start vectors
       const double sc = (ss > 0.0) ? 1.0 / sqrt(ss) : 0.0;
-      for (int r = tid; r < N; r += 256) Zc[(int64_t)r * nv + s0 + j] *= sc;
+      for (int r = r0 + tid; r < r1; r += 256) Zc[(int64_t)r * nv + cj] *= sc;
       __syncthreads();
     }
   }
@@ -510,6 +582,9 @@ struct EighScratch {
   cplx *Bw, *Wp, *P, *zpart, *tau, *Vb, *T, *G, *tauc, *Y, *Y2;
   double *d, *e, *tnorm, *Z, *fa, *fb, *fc;
   unsigned char* fp;
+  int* blk;
+  double *blo, *bhi;
+  int* bcl;
 };
 
 static size_t eigh_large_carve(char* base, int64_t cnt, int N, int nv, EighScratch* s) {
@@ -536,7 +611,11 @@ static size_t eigh_large_carve(char* base, int64_t cnt, int N, int nv, EighScrat
   double* fb = (double*)take(cnt * nvN * sizeof(double));
   double* fc = (double*)take(cnt * nvN * sizeof(double));
   unsigned char* fp = (unsigned char*)take(cnt * nvN);
-  if (s) { *s = EighScratch{Bw, Wp, P, zp, tau, Vb, T, G, tauc, Y, Y2, d, e, tn, Z, fa, fb, fc, fp}; }
+  int* blk = (int*)take(cnt * (size_t)(nv > 0 ? nv : 1) * 2 * sizeof(int));
+  double* blo = (double*)take(cnt * (size_t)N * sizeof(double));
+  double* bhi = (double*)take(cnt * (size_t)N * sizeof(double));
+  int* bcl = (int*)take(cnt * (size_t)N * sizeof(int));
+  if (s) { *s = EighScratch{Bw, Wp, P, zp, tau, Vb, T, G, tauc, Y, Y2, d, e, tn, Z, fa, fb, fc, fp, blk, blo, bhi, bcl}; }
   return off;
 }
 
@@ -625,27 +704,27 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
       BE_CUDA(cudaFuncSetAttribute(k_invit, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
     }
     be_prof_begin(ctx, PK_BISECT);
-    k_bisect<<<(unsigned)(cnt * nblk), 128, sh, st>>>(s.d, s.e, E, s.tnorm, N, nblk);
+    k_bisect<<<(unsigned)(cnt * nblk), 128, sh, st>>>(s.d, s.e, E, s.tnorm, s.blo, s.bhi, s.bcl, N, nblk);
     be_prof_end(ctx, PK_BISECT, (double)cnt * N * 24.0, 0.0);
     LAUNCH_CHECK();
     if (nv > 0) {
       const int nvb = (nv + 127) / 128;
       be_prof_begin(ctx, PK_INVIT);
-      k_invit<<<(unsigned)(cnt * nvb), 128, sh, st>>>(s.d, s.e, E, s.tnorm, s.fa, s.fb, s.fc, s.fp, s.Z, N, nv, nvb, 0, 3);
+      k_invit<<<(unsigned)(cnt * nvb), 128, sh, st>>>(s.d, s.e, E, s.tnorm, s.fa, s.fb, s.fc, s.fp, s.blk, s.blo, s.bhi, s.bcl, s.Z, N, nv, nvb, 0, 3);
       be_prof_end(ctx, PK_INVIT, (double)cnt * N * nv * 8.0, 0.0);
       LAUNCH_CHECK();
-      const size_t shc = (size_t)nv * sizeof(double);
+      const size_t shc = (size_t)nv * (sizeof(double) + sizeof(int));
       if (shc > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_cluster_orth, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shc));
       be_prof_begin(ctx, PK_ORTH);
-      k_cluster_orth<<<(unsigned)cnt, 256, shc, st>>>(E, s.tnorm, s.Z, N, nv, 1e-3, info);
+      k_cluster_orth<<<(unsigned)cnt, 256, shc, st>>>(E, s.tnorm, s.blk, s.Z, N, nv, CLUSTER_TOL, info);
       be_prof_end(ctx, PK_ORTH, 0.0, 0.0);
       LAUNCH_CHECK();
       be_prof_begin(ctx, PK_INVIT);
-      k_invit<<<(unsigned)(cnt * nvb), 128, sh, st>>>(s.d, s.e, E, s.tnorm, s.fa, s.fb, s.fc, s.fp, s.Z, N, nv, nvb, 1, 1);
+      k_invit<<<(unsigned)(cnt * nvb), 128, sh, st>>>(s.d, s.e, E, s.tnorm, s.fa, s.fb, s.fc, s.fp, s.blk, s.blo, s.bhi, s.bcl, s.Z, N, nv, nvb, 1, 1);
       be_prof_end(ctx, PK_INVIT, 0.0, 0.0);
       LAUNCH_CHECK();
       be_prof_begin(ctx, PK_ORTH);
-      k_cluster_orth<<<(unsigned)cnt, 256, shc, st>>>(E, s.tnorm, s.Z, N, nv, 1e-3, info);
+      k_cluster_orth<<<(unsigned)cnt, 256, shc, st>>>(E, s.tnorm, s.blk, s.Z, N, nv, CLUSTER_TOL, info);
       be_prof_end(ctx, PK_ORTH, 0.0, 0.0);
       LAUNCH_CHECK();
     }

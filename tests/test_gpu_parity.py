@@ -286,8 +286,8 @@ def test_config4_full_matrix_size_one_short_loop(ctx):
 def test_config5_reduced_wannier_like(ctx):
     p5 = wl.config5_parts()
     H = wl.config5_grid(p5, 64, 64, 65, ix=[0, 17], iy=[3, 31, 60])   # 6 loops x 65 points
-    th, ab, mg = ctx.wilson_loop(dev(H), 32, 2)
-    tho, abo, mgo = wo.wilson_surface(H, 32, 2)
+    th, ab, mg = ctx.wilson_loop(dev(H), 32, 1)          # [2][3][65][64][64]: batch 2, dims (3, 65)
+    tho, abo, mgo = wo.wilson_surface(H, 32, 1)
     assert mgo.min() >= 0.2
     assert phase_dist(th.cpu().numpy(), tho) <= PH_TOL
     # device grid assembly used by bench.py reproduces the host grid
@@ -309,8 +309,11 @@ def test_host_variants_match_device(ctx):
         ctx.set_workspace_limit(64 << 30)
     lod, hid, psod = ctx.spin_resolved_wilson(dev(H), 32, 1, dev(S))
     thd, abd, mgd = ctx.wilson_loop(dev(H), 32, 1)
-    assert torch.equal(lo, lod.cpu()) and torch.equal(hi, hid.cpu()) and torch.equal(pso, psod.cpu())
-    assert torch.equal(th, thd.cpu()) and torch.equal(mg, mgd.cpu())
+    # chunking changes the seeded start vectors of the inverse iteration (matrix index inside the
+    # chunk), hence the basis inside degenerate subspaces: equal up to rounding, not bitwise
+    assert phase_dist(lo.numpy(), lod.cpu().numpy()) < 1e-12 and phase_dist(hi.numpy(), hid.cpu().numpy()) < 1e-12
+    assert (pso - psod.cpu()).abs().max() < 1e-12
+    assert phase_dist(th.numpy(), thd.cpu().numpy()) < 1e-12 and (mg - mgd.cpu()).abs().max() < 1e-12
     tho, _, _ = wo.wilson_surface(H, 32, 1)
     assert phase_dist(th.numpy(), tho) <= PH_TOL
 
