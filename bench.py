@@ -137,7 +137,7 @@ class Workload:
         elif c == 5:
             H = wl.config5_grid(wl.config5_parts(), 64, 64, 65, ix=[0], iy=range(48))
             tb = time.perf_counter()
-            wo.wilson_surface(H, self.m, 2)
+            wo.wilson_surface(H, self.m, 1)
             desc, k = "48 loops x 65 k-points (kx=0)", 48 * 65
         elif c == 1:
             H = wl.config1_grid()[None]

@@ -64,7 +64,7 @@ const char* be_strerror(int code);
  * 0 = eigh, 1 = wilson loop, 2 = nested, 3 = spin resolved). */
 size_t be_workspace_bytes(const be_grid* grid, int n_occ, int op);
 
-/* Cap on the scratch used for per-chunk work buffers (default 48 GiB).  Work is processed in
+/* Cap on the scratch used for per-chunk work buffers (default 64 GiB).  Work is processed in
  * chunks of whole loops sized to stay under the cap. */
 int be_set_workspace_limit(be_ctx* ctx, size_t bytes);
 
@@ -142,6 +142,20 @@ int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int 
 int be_spin_resolved_wilson(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_occ,
                             int dir, const void* dS, int S_is_diag, int m_lo, const void* d_close,
                             double* d_theta_lo, double* d_theta_hi, double* d_pso);
+
+/*
+ * S2/S3 building block -- batched complex128 GEMM on the FP64 tensor cores (DMMA), column-major:
+ *     C[b] = alpha * op(A[b]) * op(B[b]) + beta * C[b],   b = 0..batch-1,  X[b] = X + b * strideX
+ * op: 0 = N, 1 = T, 2 = C (conjugate transpose), 3 = J (conjugate).  Supported pairs: NN, NC, CN, NT,
+ * TN, JN, NJ, CC, TJ (others: BE_ERR_UNSUPPORTED).  This is the contraction behind the link overlaps
+ * M_j = U_j^dagger U_{j+1} (op C,N) and the ordered product (op N,N).
+ * alpha, beta: pointers to 2 doubles (re, im) on the HOST.  lower != 0: only tiles on or below the
+ * diagonal are computed.  All matrix pointers are device pointers, strides in complex elements.
+ */
+int be_zgemm_batched(be_ctx* ctx, int opA, int opB, int M, int N, int K,
+                     const double* alpha, const void* dA, int lda, int64_t strideA,
+                     const void* dB, int ldb, int64_t strideB,
+                     const double* beta, void* dC, int ldc, int64_t strideC, int64_t batch, int lower);
 
 /*
  * S7 -- winding of Theta_i = sum_n theta_n over a closed transverse cycle (Eq. 6):

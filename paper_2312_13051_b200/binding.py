@@ -18,7 +18,7 @@ EXPORTS = [
     "be_create", "be_destroy", "be_strerror", "be_workspace_bytes", "be_set_workspace_limit",
     "be_launch_count", "be_eigh_batched", "be_wilson_loop", "be_nested_wilson",
     "be_spin_resolved_wilson", "be_winding", "be_wilson_loop_host", "be_spin_resolved_wilson_host",
-    "be_profile_enable", "be_profile_name", "be_profile_get",
+    "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched",
 ]
 
 
@@ -56,6 +56,8 @@ def load_library():
     lib.be_winding.argtypes = [vp, vp, i64, ci, ci, vp]
     lib.be_wilson_loop_host.argtypes = [vp, vp, gp, ci, ci, vp, vp, vp, vp]
     lib.be_spin_resolved_wilson_host.argtypes = [vp, vp, gp, ci, ci, vp, ci, ci, vp, vp, vp, vp]
+    lib.be_zgemm_batched.argtypes = [vp, ci, ci, ci, ci, ci, C.POINTER(dbl), vp, ci, i64, vp, ci, i64,
+                                     C.POINTER(dbl), vp, ci, i64, i64, ci]
     lib.be_profile_enable.argtypes = [vp, ci]
     lib.be_profile_name.argtypes = [ci]
     lib.be_profile_name.restype = C.c_char_p
@@ -228,6 +230,18 @@ class Context:
                                                    wb_lo, wb_hi, cut, _ptr(close1), _ptr(close2),
                                                    _ptr(th1), _ptr(thn)))
         return th1, thn
+
+    # ------------------------------------------------------------------ be_zgemm_batched
+    def zgemm_batched(self, opA, opB, A, B, C_out, M, N, K, lda, ldb, ldc, strideA, strideB, strideC, batch,
+                      alpha=1.0 + 0j, beta=0.0 + 0j, lower=False):
+        """Raw column-major batched GEMM on device tensors (complex128).  ops: 'N','T','C','J'."""
+        ops = {"N": 0, "T": 1, "C": 2, "J": 3}
+        al = (C.c_double * 2)(alpha.real, alpha.imag)
+        be = (C.c_double * 2)(beta.real, beta.imag)
+        _check(self.lib, self.lib.be_zgemm_batched(self._h, ops[opA], ops[opB], M, N, K, al, _ptr(A), lda, strideA,
+                                                   _ptr(B), ldb, strideB, be, _ptr(C_out), ldc, strideC, batch,
+                                                   1 if lower else 0))
+        return C_out
 
     # ------------------------------------------------------------------ be_winding
     def winding(self, theta):

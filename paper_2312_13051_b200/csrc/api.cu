@@ -230,3 +230,16 @@ extern "C" int be_winding(be_ctx* ctx, const double* d_theta, int64_t n_cycles, 
   if (n_cycles == 0) return BE_OK;
   return be_winding_impl(ctx, d_theta, n_cycles, n_points, m, d_wind);
 }
+
+extern "C" int be_zgemm_batched(be_ctx* ctx, int opA, int opB, int M, int N, int K,
+                                const double* alpha, const void* dA, int lda, int64_t strideA,
+                                const void* dB, int ldb, int64_t strideB,
+                                const double* beta, void* dC, int ldc, int64_t strideC, int64_t batch, int lower) {
+  if (!ctx || !dA || !dB || !dC || !alpha || !beta) return BE_ERR_NULL;
+  if (M < 0 || N < 0 || K < 0 || batch < 0 || lda < 1 || ldb < 1 || ldc < 1) return BE_ERR_SHAPE;
+  if (!aligned(dA, 16) || !aligned(dB, 16) || !aligned(dC, 16)) return BE_ERR_ALIGN;
+  ZgemmParams p = zgemm_simple(M, N, K, (const cplx*)dA, lda, strideA, (const cplx*)dB, ldb, strideB,
+                               (cplx*)dC, ldc, strideC, batch);
+  p.alpha = mkc(alpha[0], alpha[1]); p.beta = mkc(beta[0], beta[1]); p.lower = lower ? 1 : 0;
+  return be_zgemm(ctx, opA, opB, p);
+}

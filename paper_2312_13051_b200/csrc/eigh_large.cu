@@ -22,8 +22,9 @@
 
 namespace {
 
-constexpr int NB = 32;    // panel width (tridiagonalization and WY blocks)
-constexpr int HB = 64;    // block-column width of the symmetric matrix-vector kernel
+constexpr int NB = 32;    // panel width of the tridiagonalization
+constexpr int NBT = 128;  // width of the compact-WY blocks of the back-transform (4 panels)
+constexpr int HB = 32;    // block-column width of the symmetric matrix-vector kernel
 constexpr int HSTRIPE = 256;
 constexpr double SPLIT_TOL = 32.0;     // |e_i| <= max(SPLIT_TOL, N) * eps * ||T|| splits the tridiagonal matrix
                                        // (the backward error of the reduction itself is O(N eps ||T||))
@@ -91,11 +92,15 @@ __global__ void __launch_bounds__(256) k_col(cplx* __restrict__ Bw, const cplx* 
 
 // ------------------------------------------------------------------------------------------
 // y = B22 v with B22 = B[i+1:, i+1:] Hermitian, lower triangle stored; v = B[i+1:, i].
-// CTA = (matrix, block column J of HB columns); warp w owns 8 columns, lane = row inside a tile.
-// Each element B[r][c], r > c, is loaded once and contributes to y[r] (row part, written per
-// block column to P) and to y[c] (column part, accumulated in registers, written to zpart).
-__global__ void __launch_bounds__(256) k_hemv(const cplx* __restrict__ Bw, cplx* __restrict__ P,
-                                              cplx* __restrict__ zpart, int N, int i, int nJ, int nJmax) {
+// CTA = (matrix, block column J of HB = 32 columns); warp w owns 4 columns, lane = row inside a
+// 32-row tile.  Each element B[r][c], r > c, is loaded once and contributes to y[r] (row part,
+// reduced over the 8 warps through shared memory and written per block column to P) and to y[c]
+// (column part, accumulated in registers over the whole column, written to zpart).
+// The kernel is HBM bound (1 flop/byte): loads are issued in batches of 16 independent 16-byte
+// loads per thread (4 row tiles x 4 columns) and 3 CTAs are resident per SM to keep enough bytes
+// in flight.
+__global__ void __launch_bounds__(256, 3) k_hemv(const cplx* __restrict__ Bw, cplx* __restrict__ P,
+                                                 cplx* __restrict__ zpart, int N, int i, int nJ, int nJmax) {
   __shared__ cplx ysm[8][HSTRIPE];
   const int64_t c = blockIdx.x / nJ;
   const int J = blockIdx.x % nJ;
@@ -103,48 +108,63 @@ __global__ void __launch_bounds__(256) k_hemv(const cplx* __restrict__ Bw, cplx*
   const cplx* __restrict__ v = B + (int64_t)i * N;   // v[r], r >= i+1 (global row index)
   const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
   const int c0 = i + 1 + J * HB;
-  const int cb = c0 + 8 * w;
-  cplx vc[8], accz[8];
+  const int cb = c0 + 4 * w;
+  cplx vc[4], accz[4];
+  const cplx* colp[4];
 #pragma unroll
-  for (int q = 0; q < 8; ++q) {
+  for (int q = 0; q < 4; ++q) {
     accz[q] = mkc(0.0, 0.0);
-    vc[q] = (cb + q < N) ? v[cb + q] : mkc(0.0, 0.0);
+    const int col = (cb + q < N) ? cb + q : N - 1;
+    vc[q] = (cb + q < N) ? v[cb + q] : mkc(0.0, 0.0);   // zero weight for columns past the edge
+    colp[q] = B + (int64_t)col * N;
   }
   cplx* Prow = P + (c * nJmax + J) * (int64_t)N;
   for (int rb = c0; rb < N; rb += HSTRIPE) {
-#pragma unroll 2
-    for (int t = 0; t < HSTRIPE / 32; ++t) {
-      const int r = rb + 32 * t + lane;
-      cplx yr = mkc(0.0, 0.0);
-      if (r < N) {
-        const cplx vr = v[r];
-        if (rb + 32 * t >= c0 + HB) {   // whole tile strictly below the diagonal block
 #pragma unroll
-          for (int q = 0; q < 8; ++q) {
-            if (cb + q < N) {
-              const cplx a = B[r + (int64_t)(cb + q) * N];
-              cfma(yr, a, vc[q]);
-              cfmac(accz[q], a, vr);
-            }
-          }
-        } else {
+    for (int half = 0; half < 2; ++half) {
+      const int r0 = rb + 128 * half;
+      if (r0 >= c0 + HB && r0 + 128 <= N) {
+        // fast path: 4 full tiles strictly below the diagonal block
+        cplx a[4][4], vr[4];
 #pragma unroll
-          for (int q = 0; q < 8; ++q) {
-            const int col = cb + q;
-            if (col < N) {
-              if (r > col) {
-                const cplx a = B[r + (int64_t)col * N];
-                cfma(yr, a, vc[q]);
-                cfmac(accz[q], a, vr);
-              } else if (r == col) {
-                const double a = B[r + (int64_t)col * N].x;
-                yr.x = fma(a, vc[q].x, yr.x); yr.y = fma(a, vc[q].y, yr.y);
+        for (int t = 0; t < 4; ++t) {
+          const int r = r0 + 32 * t + lane;
+          vr[t] = v[r];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) a[t][q] = colp[q][r];
+        }
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+          cplx yr = mkc(0.0, 0.0);
+#pragma unroll
+          for (int q = 0; q < 4; ++q) { cfma(yr, a[t][q], vc[q]); cfmac(accz[q], a[t][q], vr[t]); }
+          ysm[w][128 * half + 32 * t + lane] = yr;
+        }
+      } else {
+#pragma unroll 1
+        for (int t = 0; t < 4; ++t) {
+          const int r = r0 + 32 * t + lane;
+          cplx yr = mkc(0.0, 0.0);
+          if (r < N) {
+            const cplx vr = v[r];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              const int col = cb + q;
+              if (col < N) {
+                if (r > col) {
+                  const cplx a = colp[q][r];
+                  cfma(yr, a, vc[q]);
+                  cfmac(accz[q], a, vr);
+                } else if (r == col) {
+                  const double a = colp[q][r].x;
+                  yr.x = fma(a, vc[q].x, yr.x); yr.y = fma(a, vc[q].y, yr.y);
+                }
               }
             }
           }
+          ysm[w][128 * half + 32 * t + lane] = yr;
         }
       }
-      ysm[w][32 * t + lane] = yr;
     }
     __syncthreads();
     {
@@ -159,7 +179,7 @@ __global__ void __launch_bounds__(256) k_hemv(const cplx* __restrict__ Bw, cplx*
     __syncthreads();
   }
 #pragma unroll
-  for (int q = 0; q < 8; ++q) {
+  for (int q = 0; q < 4; ++q) {
     const cplx z = warp_sum(accz[q]);
     if (lane == 0 && cb + q < N) zpart[c * N + cb + q] = z;
   }
@@ -514,7 +534,7 @@ __global__ void k_extract_v(const cplx* __restrict__ Bw, const cplx* __restrict_
                             cplx* __restrict__ tauc, int N, int p, int kb) {
   const int64_t c = blockIdx.x;
   const cplx* B = Bw + c * (int64_t)N * N;
-  cplx* V = Vb + c * (int64_t)N * NB;
+  cplx* V = Vb + c * (int64_t)N * NBT;
   const int rows = N - p - 1;
   for (int idx = threadIdx.x; idx < rows * kb; idx += blockDim.x) {
     const int cc = idx / rows, rr = idx % rows;
@@ -525,31 +545,48 @@ __global__ void k_extract_v(const cplx* __restrict__ Bw, const cplx* __restrict_
     else v = cconj(B[r + (int64_t)(p + cc) * N]);
     V[rr + (int64_t)cc * N] = v;
   }
-  if (threadIdx.x < kb) tauc[c * NB + threadIdx.x] = cconj(tau[c * N + p + threadIdx.x]);
+  if (threadIdx.x < kb) tauc[c * NBT + threadIdx.x] = cconj(tau[c * N + p + threadIdx.x]);
 }
 
 // zlarft (forward, columnwise) from G = V^H V: T(j,j) = tau_j, T(0:j, j) = -tau_j T(0:j,0:j) G(0:j, j).
-// One warp per matrix; T column-major kb x kb with leading dimension NB.
-__global__ void k_larft(const cplx* __restrict__ G, const cplx* __restrict__ tauc, cplx* __restrict__ T, int kb) {
-  __shared__ cplx Ts[NB][NB + 1];
+// One CTA of NBT threads per matrix (thread = row of T); T column-major, leading dimension NBT,
+// built in place in global memory (L1/L2 resident, 256 KB).
+__global__ void __launch_bounds__(NBT) k_larft(const cplx* __restrict__ G, const cplx* __restrict__ tauc,
+                                               cplx* __restrict__ T, int kb) {
   const int64_t c = blockIdx.x;
-  const int lane = threadIdx.x;
-  const cplx* g = G + c * NB * NB;
-  for (int j = 0; j < NB; ++j) Ts[lane][j] = mkc(0.0, 0.0);
-  __syncwarp();
+  const int row = threadIdx.x;
+  const cplx* g = G + c * NBT * NBT;
+  cplx* t = T + c * NBT * NBT;
+  for (int j = 0; j < NBT; ++j) t[row + j * NBT] = mkc(0.0, 0.0);
+  __syncthreads();
   for (int j = 0; j < kb; ++j) {
-    const cplx tj = tauc[c * NB + j];
-    cplx acc = mkc(0.0, 0.0);
-    if (lane < j) {
-      for (int q = lane; q < j; ++q) cfma(acc, Ts[lane][q], g[q + j * NB]);
-      acc = cmul(mkc(-tj.x, -tj.y), acc);
+    const cplx tj = tauc[c * NBT + j];
+    if (row < j) {
+      cplx acc = mkc(0.0, 0.0);
+      for (int q = row; q < j; ++q) cfma(acc, t[row + q * NBT], g[q + j * NBT]);   // own row only
+      t[row + j * NBT] = cmul(mkc(-tj.x, -tj.y), acc);
+    } else if (row == j) {
+      t[j + j * NBT] = tj;
     }
-    __syncwarp();
-    if (lane < j) Ts[lane][j] = acc;
-    if (lane == j) Ts[j][j] = tj;
-    __syncwarp();
   }
-  for (int j = 0; j < NB; ++j) T[c * NB * NB + lane + j * NB] = Ts[lane][j];
+}
+
+// her2k operands for one panel: XA = [V | W], XB = [W | V] restricted to rows q..N-1 (ld N), so that
+// B22 -= XA XB^H is a single rank-2kb update (C read and written once).
+__global__ void k_pack_vw(const cplx* __restrict__ Bw, const cplx* __restrict__ Wp, cplx* __restrict__ Vb,
+                          int N, int p, int q, int kb) {
+  const int64_t c = blockIdx.x;
+  const cplx* B = Bw + c * (int64_t)N * N;
+  const cplx* W = Wp + c * (int64_t)N * NB;
+  cplx* XA = Vb + c * (int64_t)N * NBT;
+  cplx* XB = XA + (int64_t)N * 2 * NB;
+  const int rows = N - q;
+  for (int idx = threadIdx.x; idx < rows * kb; idx += blockDim.x) {
+    const int cc = idx / rows, r = q + idx % rows;
+    const cplx v = B[r + (int64_t)(p + cc) * N], w = W[r + (int64_t)cc * N];
+    XA[(r - q) + (int64_t)cc * N] = v;        XA[(r - q) + (int64_t)(kb + cc) * N] = w;
+    XB[(r - q) + (int64_t)cc * N] = w;        XB[(r - q) + (int64_t)(kb + cc) * N] = v;
+  }
 }
 
 __global__ void k_set_info(int* info, int64_t cnt) {
@@ -597,12 +634,12 @@ static size_t eigh_large_carve(char* base, int64_t cnt, int N, int nv, EighScrat
   cplx* P = (cplx*)take(cnt * (size_t)nJmax * N * sizeof(cplx));
   cplx* zp = (cplx*)take(cnt * (size_t)N * sizeof(cplx));
   cplx* tau = (cplx*)take(cnt * (size_t)N * sizeof(cplx));
-  cplx* Vb = (cplx*)take(cnt * (size_t)N * NB * sizeof(cplx));
-  cplx* T = (cplx*)take(cnt * (size_t)NB * NB * sizeof(cplx));
-  cplx* G = (cplx*)take(cnt * (size_t)NB * NB * sizeof(cplx));
-  cplx* tauc = (cplx*)take(cnt * (size_t)NB * sizeof(cplx));
-  cplx* Y = (cplx*)take(cnt * (size_t)NB * (nv > 0 ? nv : 1) * sizeof(cplx));
-  cplx* Y2 = (cplx*)take(cnt * (size_t)NB * (nv > 0 ? nv : 1) * sizeof(cplx));
+  cplx* Vb = (cplx*)take(cnt * (size_t)N * NBT * sizeof(cplx));
+  cplx* T = (cplx*)take(cnt * (size_t)NBT * NBT * sizeof(cplx));
+  cplx* G = (cplx*)take(cnt * (size_t)NBT * NBT * sizeof(cplx));
+  cplx* tauc = (cplx*)take(cnt * (size_t)NBT * sizeof(cplx));
+  cplx* Y = (cplx*)take(cnt * (size_t)NBT * (nv > 0 ? nv : 1) * sizeof(cplx));
+  cplx* Y2 = (cplx*)take(cnt * (size_t)NBT * (nv > 0 ? nv : 1) * sizeof(cplx));
   double* d = (double*)take(cnt * (size_t)N * sizeof(double));
   double* e = (double*)take(cnt * (size_t)N * sizeof(double));
   double* tn = (double*)take(cnt * sizeof(double));
@@ -672,21 +709,15 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
     }
     const int q = pend, kb = pend - p;
     if (q < N) {
-      if (q == N - 1 && pend == N - 1) {
-        // trailing 1x1 block: handled by the final k_col below through the panel update path
-      }
       const int n2 = N - q;
-      // B[q:, q:] -= V W^H ; -= W V^H  (lower tiles)
-      ZgemmParams g = zgemm_simple(n2, n2, kb, s.Bw + q + (int64_t)p * N, N, (int64_t)N * N,
-                                   s.Wp + q, N, (int64_t)N * NB, s.Bw + q + (int64_t)q * N, N,
-                                   (int64_t)N * N, cnt);
+      // B[q:, q:] -= [V W] [W V]^H  (lower tiles): one rank-2kb update
+      k_pack_vw<<<(unsigned)cnt, 256, 0, st>>>(s.Bw, s.Wp, s.Vb, N, p, q, kb);
+      LAUNCH_CHECK();
+      ZgemmParams g = zgemm_simple(n2, n2, 2 * kb, s.Vb, N, (int64_t)N * NBT,
+                                   s.Vb + (int64_t)N * 2 * NB, N, (int64_t)N * NBT,
+                                   s.Bw + q + (int64_t)q * N, N, (int64_t)N * N, cnt);
       g.alpha = mkc(-1.0, 0.0); g.beta = mkc(1.0, 0.0); g.lower = 1;
       BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_C, g));
-      ZgemmParams g2 = zgemm_simple(n2, n2, kb, s.Wp + q, N, (int64_t)N * NB,
-                                    s.Bw + q + (int64_t)p * N, N, (int64_t)N * N,
-                                    s.Bw + q + (int64_t)q * N, N, (int64_t)N * N, cnt);
-      g2.alpha = mkc(-1.0, 0.0); g2.beta = mkc(1.0, 0.0); g2.lower = 1;
-      BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_C, g2));
     }
     if (pend == N - 1) {   // last diagonal element (no pending panel: it was just applied)
       k_col<<<(unsigned)cnt, 256, 0, st>>>(s.Bw, s.Wp, s.d, s.e, s.tau, N, N - 1, N - 1);
@@ -737,30 +768,30 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
     k_z2x<<<(unsigned)(cnt * tr * tv), 256, 0, st>>>(s.Z, X, N, nv, tr, tv);
     LAUNCH_CHECK();
   }
-  int plast = ((N - 2) / NB) * NB;
-  for (int p = plast; p >= 0; p -= NB) {
-    const int pend = (p + NB < N - 1) ? p + NB : N - 1;
+  int plast = ((N - 2) / NBT) * NBT;
+  for (int p = plast; p >= 0; p -= NBT) {
+    const int pend = (p + NBT < N - 1) ? p + NBT : N - 1;
     const int kb = pend - p;
     if (kb <= 0) continue;
     const int rows = N - p - 1;
     k_extract_v<<<(unsigned)cnt, 256, 0, st>>>(s.Bw, s.tau, s.Vb, s.tauc, N, p, kb);
     LAUNCH_CHECK();
     // G = V^H V
-    ZgemmParams gg = zgemm_simple(kb, kb, rows, s.Vb, N, (int64_t)N * NB, s.Vb, N, (int64_t)N * NB,
-                                  s.G, NB, NB * NB, cnt);
+    ZgemmParams gg = zgemm_simple(kb, kb, rows, s.Vb, N, (int64_t)N * NBT, s.Vb, N, (int64_t)N * NBT,
+                                  s.G, NBT, NBT * NBT, cnt);
     BE_TRY(be_zgemm(ctx, BE_OP_C, BE_OP_N, gg));
-    k_larft<<<(unsigned)cnt, 32, 0, st>>>(s.G, s.tauc, s.T, kb);
+    k_larft<<<(unsigned)cnt, NBT, 0, st>>>(s.G, s.tauc, s.T, kb);
     LAUNCH_CHECK();
     // Y = V^H X[p+1:, :]
-    ZgemmParams gy = zgemm_simple(kb, nv, rows, s.Vb, N, (int64_t)N * NB, X + p + 1, N, (int64_t)N * nv,
-                                  s.Y, NB, (int64_t)NB * nv, cnt);
+    ZgemmParams gy = zgemm_simple(kb, nv, rows, s.Vb, N, (int64_t)N * NBT, X + p + 1, N, (int64_t)N * nv,
+                                  s.Y, NBT, (int64_t)NBT * nv, cnt);
     BE_TRY(be_zgemm(ctx, BE_OP_C, BE_OP_N, gy));
     // Y2 = T Y
-    ZgemmParams gt = zgemm_simple(kb, nv, kb, s.T, NB, NB * NB, s.Y, NB, (int64_t)NB * nv,
-                                  s.Y2, NB, (int64_t)NB * nv, cnt);
+    ZgemmParams gt = zgemm_simple(kb, nv, kb, s.T, NBT, NBT * NBT, s.Y, NBT, (int64_t)NBT * nv,
+                                  s.Y2, NBT, (int64_t)NBT * nv, cnt);
     BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_N, gt));
     // X[p+1:, :] -= V Y2
-    ZgemmParams gx = zgemm_simple(rows, nv, kb, s.Vb, N, (int64_t)N * NB, s.Y2, NB, (int64_t)NB * nv,
+    ZgemmParams gx = zgemm_simple(rows, nv, kb, s.Vb, N, (int64_t)N * NBT, s.Y2, NBT, (int64_t)NBT * nv,
                                   X + p + 1, N, (int64_t)N * nv, cnt);
     gx.alpha = mkc(-1.0, 0.0); gx.beta = mkc(1.0, 0.0);
     BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_N, gx));

@@ -24,7 +24,7 @@ def test_library_builds_and_exports_every_declared_symbol():
     path = build.build()
     lib = ctypes.CDLL(path)
     names = _header_functions()
-    assert len(names) >= 16
+    assert len(names) >= 17
     for n in names:
         assert hasattr(lib, n), f"{n} declared in the header but not exported"
     assert set(binding.EXPORTS) == set(names)
