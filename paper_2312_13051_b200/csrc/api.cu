@@ -12,7 +12,7 @@ int be_winding_impl(be_ctx* ctx, const double* theta, int64_t n_cycles, int n_po
 int be_nested_select_small(be_ctx* ctx, const cplx* W, int64_t cnt, int m, int wb_lo, int wb_hi,
                            double cut, double* theta1, cplx* Vs);
 int be_chain_product(be_ctx* ctx, const cplx* F, int N, int m, int64_t outer, int n1,
-                     const cplx* d_close, int phi_at, cplx** Wout);
+                     const cplx* d_close, int phi_at, cplx* Wdst, cplx** Wout);
 
 // ---------------------------------------------------------------------------------------------
 // optional profile: one CUDA event pair per launch of the instrumented kernel classes
@@ -160,11 +160,11 @@ size_t be_eigh_scratch_bytes(int64_t cnt, int N, int nv) {
 }
 
 int be_eigh_frames(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt,
-                   int N, int nv, double* E, cplx* X, int* info) {
+                   int N, int nv, int ne, double* E, cplx* X, int* info) {
   if (cnt <= 0) return BE_OK;
   if (N <= 8) return be_eigh_small(ctx, H, map, loop0, cnt, N, nv, E, X, info);
   const size_t mark = ctx->arena_used;
-  const int r = be_eigh_large(ctx, H, map, loop0, cnt, N, nv, E, X, info);
+  const int r = be_eigh_large(ctx, H, map, loop0, cnt, N, nv, ne, E, X, info);
   ctx->arena_used = mark;   // stage scratch is dead once its kernels are enqueued (stream order)
   return r;
 }
@@ -216,7 +216,7 @@ extern "C" int be_eigh_batched(be_ctx* ctx, const void* dH, int64_t count, int N
       X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * nv * sizeof(cplx));
       if (!X) return BE_ERR_NOMEM;
     }
-    BE_TRY(be_eigh_frames(ctx, (const cplx*)dH, map, c0, cnt, N, nv, dE + c0 * N, X,
+    BE_TRY(be_eigh_frames(ctx, (const cplx*)dH, map, c0, cnt, N, nv, N, dE + c0 * N, X,
                           d_info ? d_info + c0 : nullptr));
     if (nv > 0) BE_TRY(be_frames_to_public(ctx, X, (cplx*)dU + c0 * (int64_t)N * nv, cnt, N, nv));
   }

@@ -9,7 +9,7 @@ int be_scale_rows(be_ctx* ctx, const cplx* X, const double* S, cplx* SX, int N, 
 int be_nested_select_small(be_ctx* ctx, const cplx* W, int64_t cnt, int m, int wb_lo, int wb_hi,
                            double cut, double* theta1, cplx* Vs);
 int be_chain_product(be_ctx* ctx, const cplx* F, int N, int m, int64_t outer, int n1,
-                     const cplx* d_close, int phi_at, cplx** Wout);
+                     const cplx* d_close, int phi_at, cplx* Wdst, cplx** Wout);
 
 static inline bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
 
@@ -63,21 +63,34 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   if (lc > loops) lc = loops;
   const int64_t nchunks = (loops + lc - 1) / lc;
   lc = (loops + nchunks - 1) / nchunks;
-  BE_TRY(be_arena_reserve(ctx, per * (size_t)lc + (4 << 20)));
   const int mlo = sp ? sp->m_lo : 0, mhi = sp ? m - sp->m_lo : 0;
+  // The Wilson matrices of ALL loops outlive the chunks: their eigenphase solve (S4) is a
+  // latency-bound kernel with one CTA per matrix, so it runs once over every loop at the end
+  // instead of once per chunk with a fraction of the SMs busy.
+  const int msec[2] = {sp ? mlo : m, sp ? mhi : 0};
+  size_t persist = 0;
+  for (int s = 0; s < 2; ++s)
+    persist += be_align256((size_t)loops * msec[s] * msec[s] * sizeof(cplx)) + be_eigenphases_scratch_bytes(loops, msec[s]) + 1024;
+  BE_TRY(be_arena_reserve(ctx, per * (size_t)lc + persist + (4 << 20)));
+  cplx* Wall[2] = {nullptr, nullptr};
+  for (int s = 0; s < 2; ++s)
+    if (msec[s] > 0) {
+      Wall[s] = (cplx*)be_arena_alloc(ctx, (size_t)loops * msec[s] * msec[s] * sizeof(cplx));
+      if (!Wall[s]) return BE_ERR_NOMEM;
+    }
+  const size_t keep = ctx->arena_used;
   for (int64_t l0 = 0; l0 < loops; l0 += lc) {
     const int64_t nl = (loops - l0 < lc) ? loops - l0 : lc;
     const int64_t cnt = nl * n1;
-    ctx->arena_used = 0;
+    ctx->arena_used = keep;
     double* E = (double*)be_arena_alloc(ctx, (size_t)cnt * N * sizeof(double));
     cplx* X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
     if (!E || !X) return BE_ERR_NOMEM;
-    BE_TRY(be_eigh_frames(ctx, H, map, l0, cnt, N, m, E, X, nullptr));
+    BE_TRY(be_eigh_frames(ctx, H, map, l0, cnt, N, m, m + 1, E, X, nullptr));
     if (d_mingap) BE_TRY(be_mingap(ctx, E, N, m, n1, nl, d_mingap + l0));
     if (!sp) {
       cplx* W = nullptr;
-      BE_TRY(be_chain_product(ctx, X, N, m, nl, n1, d_close, n1 - 1, &W));
-      BE_TRY(be_eigenphases(ctx, W, nl, m, d_theta + l0 * m, d_abs ? d_abs + l0 * m : nullptr));
+      BE_TRY(be_chain_product(ctx, X, N, m, nl, n1, d_close, n1 - 1, Wall[0] + l0 * (int64_t)m * m, &W));
       continue;
     }
     // ---- spin-resolved: S_red = U^H S U, diagonalize, rotate into sectors
@@ -106,7 +119,7 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
       GridMap fm;
       memset(&fm, 0, sizeof(fm));
       fm.ndim = 1; fm.dir = 0; fm.n1 = 1; fm.dims[0] = 1; fm.batch_stride = 1; fm.loops = cnt;
-      BE_TRY(be_eigh_frames(ctx, Sred, fm, 0, cnt, m, m, sig, V, nullptr));
+      BE_TRY(be_eigh_frames(ctx, Sred, fm, 0, cnt, m, m, m, sig, V, nullptr));
     }
     for (int sector = 0; sector < 2; ++sector) {
       const int ms = sector == 0 ? mlo : mhi;
@@ -119,9 +132,19 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
                                    (int64_t)m * m, F, N, (int64_t)N * ms, cnt);
       BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_N, g));
       cplx* W = nullptr;
-      BE_TRY(be_chain_product(ctx, F, N, ms, nl, n1, d_close, n1 - 1, &W));
-      BE_TRY(be_eigenphases(ctx, W, nl, ms, out + l0 * ms, nullptr));
+      BE_TRY(be_chain_product(ctx, F, N, ms, nl, n1, d_close, n1 - 1, Wall[sector] + l0 * (int64_t)ms * ms, &W));
       ctx->arena_used = mark;
+    }
+  }
+  // ---- S4 for every loop at once
+  ctx->arena_used = keep;
+  if (!sp) {
+    BE_TRY(be_eigenphases(ctx, Wall[0], loops, m, d_theta, d_abs));
+  } else {
+    for (int sector = 0; sector < 2; ++sector) {
+      double* out = sector == 0 ? sp->theta_lo : sp->theta_hi;
+      if (msec[sector] == 0 || !out) continue;
+      BE_TRY(be_eigenphases(ctx, Wall[sector], loops, msec[sector], out, nullptr));
     }
   }
   return BE_OK;
@@ -214,9 +237,9 @@ extern "C" int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid*
     cplx* X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
     cplx* Vs = (cplx*)be_arena_alloc(ctx, (size_t)nl * m * ns * sizeof(cplx));
     if (!E || !X || !Vs) return BE_ERR_NOMEM;
-    BE_TRY(be_eigh_frames(ctx, (const cplx*)dH_grid, map, l0, cnt, N, m, E, X, nullptr));
+    BE_TRY(be_eigh_frames(ctx, (const cplx*)dH_grid, map, l0, cnt, N, m, m + 1, E, X, nullptr));
     cplx* W = nullptr;
-    BE_TRY(be_chain_product(ctx, X, N, m, nl, n1, (const cplx*)d_close1, phi_at, &W));
+    BE_TRY(be_chain_product(ctx, X, N, m, nl, n1, (const cplx*)d_close1, phi_at, nullptr, &W));
     BE_TRY(be_nested_select_small(ctx, W, nl, m, wb_lo, wb_hi, theta_cut, th1 + l0 * m, Vs));
     // w = U_base V_S  (frame j = 0 of each rolled loop)
     ZgemmParams g = zgemm_simple(N, ns, m, X, N, (int64_t)n1 * N * m, Vs, m, (int64_t)m * ns,
@@ -225,7 +248,7 @@ extern "C" int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid*
   }
   ctx->arena_used = keep;
   cplx* W2 = nullptr;
-  BE_TRY(be_chain_product(ctx, Wf, N, ns, outer2, n2, (const cplx*)d_close2, n2 - 1, &W2));
+  BE_TRY(be_chain_product(ctx, Wf, N, ns, outer2, n2, (const cplx*)d_close2, n2 - 1, nullptr, &W2));
   BE_TRY(be_eigenphases(ctx, W2, outer2, ns, d_theta_nested, nullptr));
   return BE_OK;
 }

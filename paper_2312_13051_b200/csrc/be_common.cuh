@@ -161,8 +161,9 @@ __host__ __device__ inline int64_t gridmap_index(const GridMap& g, int64_t loop,
 //   matrix c = (loop0 + c / map.n1, c % map.n1).  Outputs:
 //   E [cnt][N] ascending;  X [cnt][nv][N] column-major frames (X[c][v*N + r] = U[r][v]);
 //   info [cnt] or NULL.  Scratch comes from the context arena (caller reserved it).
+//   ne: only E[c][0..ne-1] are computed (ne >= nv; N = all); the rest of the row is left untouched.
 int be_eigh_frames(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt,
-                   int N, int nv, double* E, cplx* X, int* info);
+                   int N, int nv, int ne, double* E, cplx* X, int* info);
 size_t be_eigh_scratch_bytes(int64_t cnt, int N, int nv);
 
 // eigenphases of ``cnt`` general complex m x m matrices W (column-major, stride m*m, destroyed):
@@ -174,6 +175,6 @@ int be_eigenvalues_general(be_ctx* ctx, cplx* W, int64_t cnt, int m, cplx* lam, 
 int be_eigh_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N,
                   int nv, double* E, cplx* X, int* info);
 int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N,
-                  int nv, double* E, cplx* X, int* info);
+                  int nv, int ne, double* E, cplx* X, int* info);
 size_t be_eigh_large_scratch_bytes(int64_t cnt, int N, int nv);
 int be_frames_to_public(be_ctx* ctx, const cplx* X, cplx* U, int64_t cnt, int N, int nv);

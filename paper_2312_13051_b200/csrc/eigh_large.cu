@@ -25,10 +25,13 @@ namespace {
 constexpr int NB = 32;    // panel width of the tridiagonalization
 constexpr int NBT = 128;  // width of the compact-WY blocks of the back-transform (4 panels)
 constexpr int HB = 32;    // block-column width of the symmetric matrix-vector kernel
-constexpr int HSTRIPE = 256;
 constexpr double SPLIT_TOL = 32.0;     // |e_i| <= max(SPLIT_TOL, N) * eps * ||T|| splits the tridiagonal matrix
                                        // (the backward error of the reduction itself is O(N eps ||T||))
-constexpr double CLUSTER_TOL = 3e-4;   // eigenvalues closer than this (relative to ||T||) are re-orthogonalized
+constexpr double CLUSTER_TOL = 2e-5;   // eigenvalues closer than this (relative to ||T||) are re-orthogonalized:
+                                       // inverse-iteration vectors of eigenvalues a gap g apart are orthogonal to
+                                       // ~eps ||T|| / g, i.e. <= 1e-11 outside clusters (LAPACK's 1e-3 buys eps-level
+                                       // orthogonality the 1e-8 phase tolerance does not need, at the price of
+                                       // clusters of 50-90 vectors on the N = 1600 supercell)
 
 // ------------------------------------------------------------------------------------------
 __global__ void k_gather(const cplx* __restrict__ H, cplx* __restrict__ Bw, GridMap map,
@@ -92,96 +95,151 @@ __global__ void __launch_bounds__(256) k_col(cplx* __restrict__ Bw, const cplx* 
 
 // ------------------------------------------------------------------------------------------
 // y = B22 v with B22 = B[i+1:, i+1:] Hermitian, lower triangle stored; v = B[i+1:, i].
-// CTA = (matrix, block column J of HB = 32 columns); warp w owns 4 columns, lane = row inside a
-// 32-row tile.  Each element B[r][c], r > c, is loaded once and contributes to y[r] (row part,
-// reduced over the 8 warps through shared memory and written per block column to P) and to y[c]
-// (column part, accumulated in registers over the whole column, written to zpart).
-// The kernel is HBM bound (1 flop/byte): loads are issued in batches of 16 independent 16-byte
-// loads per thread (4 row tiles x 4 columns) and 3 CTAs are resident per SM to keep enough bytes
-// in flight.
-__global__ void __launch_bounds__(256, 3) k_hemv(const cplx* __restrict__ Bw, cplx* __restrict__ P,
-                                                 cplx* __restrict__ zpart, int N, int i, int nJ, int nJmax) {
-  __shared__ cplx ysm[8][HSTRIPE];
+//
+// The kernel is HBM bound (1 flop/byte): every element B[r][c], r > c, is read exactly once and used
+// twice, for y[r] (row part) and for y[c] (column part).  CTA = (matrix, block column J of HB = 32
+// columns).  A producer warp streams the block column through shared memory in stages of
+// HROWS = 64 rows with TMA bulk copies (cp.async.bulk, one per column segment plus one for the
+// matching piece of v, completion on an mbarrier), HSTAGES deep, so the bytes in flight do not
+// depend on registers or on the progress of the arithmetic.  256 consumer threads: thread =
+// (row lr of the stage, group cg of 8 columns).  Row part: summed over the 4 column groups through
+// shared memory and written per block column to P (k_w adds the block columns up: no atomics, the
+// result is bitwise reproducible).  Column part: 8 accumulators per thread kept in registers over
+// the whole block column, reduced once at the end and written to zpart.
+constexpr int HROWS = 64;
+constexpr int HSTAGES = 3;
+constexpr int HEMV_THREADS = 256 + 32;
+constexpr int HSTAGE_ELEMS = (HB + 1) * HROWS;                 // 32 columns + the v segment
+constexpr size_t HEMV_SMEM = (size_t)HSTAGES * HSTAGE_ELEMS * sizeof(cplx) + 2 * 4 * HROWS * sizeof(cplx)
+                             + 2 * HSTAGES * sizeof(unsigned long long) + 64;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(void* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(void* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity) {
+  asm volatile(
+      "{\n .reg .pred p;\n WAIT_LOOP:\n"
+      " mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      " @p bra WAIT_DONE;\n bra WAIT_LOOP;\n WAIT_DONE:\n}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, uint32_t bytes, void* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+__global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict__ Bw, cplx* __restrict__ P,
+                                                          cplx* __restrict__ zpart, int N, int i, int nJ, int nJmax) {
+  extern __shared__ __align__(128) unsigned char hsm[];
+  cplx* stage = (cplx*)hsm;                                           // [HSTAGES][HB + 1][HROWS]
+  cplx* ysm = stage + (size_t)HSTAGES * HSTAGE_ELEMS;                 // [2][4][HROWS]
+  unsigned long long* full = (unsigned long long*)(ysm + 2 * 4 * HROWS);
+  unsigned long long* empty = full + HSTAGES;
   const int64_t c = blockIdx.x / nJ;
   const int J = blockIdx.x % nJ;
   const cplx* __restrict__ B = Bw + c * (int64_t)N * N;
   const cplx* __restrict__ v = B + (int64_t)i * N;   // v[r], r >= i+1 (global row index)
-  const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+  const int tid = threadIdx.x;
   const int c0 = i + 1 + J * HB;
-  const int cb = c0 + 4 * w;
-  cplx vc[4], accz[4];
-  const cplx* colp[4];
+  const int ncols = (N - c0 < HB) ? N - c0 : HB;
+  const int nst = (N - c0 + HROWS - 1) / HROWS;
+  if (tid == 0) {
+    for (int s = 0; s < HSTAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (tid >= 256) {
+    // ---- producer warp: lane = column of the block column (lane 0 also copies the v segment)
+    const int lane = tid - 256;
+    for (int s = 0; s < nst; ++s) {
+      const int slot = s % HSTAGES;
+      if (s >= HSTAGES) mbar_wait(&empty[slot], ((s / HSTAGES) - 1) & 1);
+      const int r0 = c0 + s * HROWS;
+      const int nr = (N - r0 < HROWS) ? N - r0 : HROWS;
+      const uint32_t seg = (uint32_t)nr * sizeof(cplx);
+      cplx* dst = stage + (size_t)slot * HSTAGE_ELEMS;
+      if (lane == 0) {
+        mbar_expect_tx(&full[slot], seg * (uint32_t)(ncols + 1));
+        tma_bulk_g2s(dst + HB * HROWS, v + r0, seg, &full[slot]);
+      }
+      __syncwarp();
+      if (lane < ncols) tma_bulk_g2s(dst + lane * HROWS, B + (int64_t)(c0 + lane) * N + r0, seg, &full[slot]);
+    }
+    return;
+  }
+
+  // ---- consumers
+  const int lr = tid & (HROWS - 1), cg = tid >> 6, lane = tid & 31, warp = tid >> 5;
+  int nq = ncols - cg * 8;
+  nq = nq < 0 ? 0 : (nq > 8 ? 8 : nq);
+  cplx vc[8], accz[8];
 #pragma unroll
-  for (int q = 0; q < 4; ++q) {
+  for (int q = 0; q < 8; ++q) {
     accz[q] = mkc(0.0, 0.0);
-    const int col = (cb + q < N) ? cb + q : N - 1;
-    vc[q] = (cb + q < N) ? v[cb + q] : mkc(0.0, 0.0);   // zero weight for columns past the edge
-    colp[q] = B + (int64_t)col * N;
+    vc[q] = (q < nq) ? v[c0 + cg * 8 + q] : mkc(0.0, 0.0);
   }
   cplx* Prow = P + (c * nJmax + J) * (int64_t)N;
-  for (int rb = c0; rb < N; rb += HSTRIPE) {
+  for (int s = 0; s < nst; ++s) {
+    const int slot = s % HSTAGES;
+    const cplx* st = stage + (size_t)slot * HSTAGE_ELEMS;
+    const int r = c0 + s * HROWS + lr;
+    mbar_wait(&full[slot], (s / HSTAGES) & 1);
+    cplx yr = mkc(0.0, 0.0);
+    if (r < N) {
+      const cplx vr = st[HB * HROWS + lr];
+      if (s > 0) {
+        if (nq == 8) {
+          cplx a[8];
 #pragma unroll
-    for (int half = 0; half < 2; ++half) {
-      const int r0 = rb + 128 * half;
-      if (r0 >= c0 + HB && r0 + 128 <= N) {
-        // fast path: 4 full tiles strictly below the diagonal block
-        cplx a[4][4], vr[4];
+          for (int q = 0; q < 8; ++q) a[q] = st[(cg * 8 + q) * HROWS + lr];
 #pragma unroll
-        for (int t = 0; t < 4; ++t) {
-          const int r = r0 + 32 * t + lane;
-          vr[t] = v[r];
+          for (int q = 0; q < 8; ++q) { cfma(yr, a[q], vc[q]); cfmac(accz[q], a[q], vr); }
+        } else {
 #pragma unroll
-          for (int q = 0; q < 4; ++q) a[t][q] = colp[q][r];
-        }
-#pragma unroll
-        for (int t = 0; t < 4; ++t) {
-          cplx yr = mkc(0.0, 0.0);
-#pragma unroll
-          for (int q = 0; q < 4; ++q) { cfma(yr, a[t][q], vc[q]); cfmac(accz[q], a[t][q], vr[t]); }
-          ysm[w][128 * half + 32 * t + lane] = yr;
+          for (int q = 0; q < 8; ++q)
+            if (q < nq) { const cplx a = st[(cg * 8 + q) * HROWS + lr]; cfma(yr, a, vc[q]); cfmac(accz[q], a, vr); }
         }
       } else {
-#pragma unroll 1
-        for (int t = 0; t < 4; ++t) {
-          const int r = r0 + 32 * t + lane;
-          cplx yr = mkc(0.0, 0.0);
-          if (r < N) {
-            const cplx vr = v[r];
+        // first stage: holds the diagonal block (upper triangle is not part of the matrix)
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-              const int col = cb + q;
-              if (col < N) {
-                if (r > col) {
-                  const cplx a = colp[q][r];
-                  cfma(yr, a, vc[q]);
-                  cfmac(accz[q], a, vr);
-                } else if (r == col) {
-                  const double a = colp[q][r].x;
-                  yr.x = fma(a, vc[q].x, yr.x); yr.y = fma(a, vc[q].y, yr.y);
-                }
-              }
-            }
+        for (int q = 0; q < 8; ++q)
+          if (q < nq) {
+            const int col = c0 + cg * 8 + q;
+            const cplx a = st[(cg * 8 + q) * HROWS + lr];
+            if (r > col) { cfma(yr, a, vc[q]); cfmac(accz[q], a, vr); }
+            else if (r == col) { yr.x = fma(a.x, vc[q].x, yr.x); yr.y = fma(a.x, vc[q].y, yr.y); }
           }
-          ysm[w][128 * half + 32 * t + lane] = yr;
-        }
       }
     }
-    __syncthreads();
-    {
-      const int r = rb + tid;
-      if (r < N) {
-        cplx s = ysm[0][tid];
-#pragma unroll
-        for (int ww = 1; ww < 8; ++ww) s = cadd(s, ysm[ww][tid]);
-        Prow[r] = s;
-      }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[slot]);          // this warp is done with the stage
+    cplx* yb = ysm + (s & 1) * 4 * HROWS;
+    yb[cg * HROWS + lr] = yr;
+    asm volatile("bar.sync 1, 256;" ::: "memory");     // consumers only
+    if (tid < HROWS && r < N) {
+      cplx t = cadd(cadd(yb[tid], yb[HROWS + tid]), cadd(yb[2 * HROWS + tid], yb[3 * HROWS + tid]));
+      Prow[r] = t;
     }
-    __syncthreads();
   }
+  // column part: reduce over the 64 rows (2 warps per column group)
+  asm volatile("bar.sync 1, 256;" ::: "memory");
+  cplx* zsm = ysm;   // [8 warps][8]
 #pragma unroll
-  for (int q = 0; q < 4; ++q) {
+  for (int q = 0; q < 8; ++q) {
     const cplx z = warp_sum(accz[q]);
-    if (lane == 0 && cb + q < N) zpart[c * N + cb + q] = z;
+    if (lane == 0) zsm[warp * 8 + q] = z;
+  }
+  asm volatile("bar.sync 1, 256;" ::: "memory");
+  if (tid < HB && tid < ncols) {
+    const int g = tid >> 3, q = tid & 7;
+    zpart[c * N + c0 + tid] = cadd(zsm[(2 * g) * 8 + q], zsm[(2 * g + 1) * 8 + q]);
   }
 }
 
@@ -238,7 +296,7 @@ __global__ void __launch_bounds__(256) k_w(const cplx* __restrict__ Bw, cplx* __
 __global__ void __launch_bounds__(128) k_bisect(const double* __restrict__ dd, const double* __restrict__ ee,
                                                 double* __restrict__ lam, double* __restrict__ tnorm,
                                                 double* __restrict__ blo, double* __restrict__ bhi,
-                                                int* __restrict__ bcl, int N, int nblk) {
+                                                int* __restrict__ bcl, int N, int nblk, int ne) {
   extern __shared__ double sh[];   // d[N], e2[N]
   __shared__ double rmin[4], rmax[4], remax[4];
   double* d = sh; double* e2 = sh + N;
@@ -276,7 +334,7 @@ __global__ void __launch_bounds__(128) k_bisect(const double* __restrict__ dd, c
   const double split = fmax(SPLIT_TOL, (double)N) * DBL_EPSILON * tn;
   for (int r = tid; r < N; r += 128) if (e2[r] <= split * split) e2[r] = 0.0;
   __syncthreads();
-  if (k >= N) return;
+  if (k >= ne) return;   // only the ne lowest eigenvalues are wanted
   double lo = gl, hi = gu;
   int cnt_lo = 0;
   const double atol = 0.25 * eps * tn;
@@ -661,7 +719,9 @@ size_t be_eigh_large_scratch_bytes(int64_t cnt, int N, int nv) { return eigh_lar
 #define LAUNCH_CHECK() do { ctx->launches++; cudaError_t e__ = cudaGetLastError(); if (e__ != cudaSuccess) return (int)e__; } while (0)
 
 int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N,
-                  int nv, double* E, cplx* X, int* info) {
+                  int nv, int ne, double* E, cplx* X, int* info) {
+  if (ne < nv) ne = nv;
+  if (ne > N) ne = N;
   const size_t need = be_eigh_large_scratch_bytes(cnt, N, nv);
   char* base = (char*)be_arena_alloc(ctx, need);
   if (!base) return BE_ERR_NOMEM;
@@ -680,6 +740,7 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
   const size_t ysh_bytes = (size_t)N * sizeof(cplx);
   if (ysh_bytes > 200 * 1024) return BE_ERR_UNSUPPORTED;
   if (ysh_bytes > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_w, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ysh_bytes));
+  BE_CUDA(cudaFuncSetAttribute(k_hemv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HEMV_SMEM));
 
   // ---- S1a: blocked tridiagonalization
   for (int p = 0; p < N; p += NB) {
@@ -698,7 +759,7 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
       LAUNCH_CHECK();
       const int nJ = (n + HB - 1) / HB;
       be_prof_begin(ctx, PK_HEMV);
-      k_hemv<<<(unsigned)(cnt * nJ), 256, 0, st>>>(s.Bw, s.P, s.zpart, N, i, nJ, nJmax);
+      k_hemv<<<(unsigned)(cnt * nJ), HEMV_THREADS, HEMV_SMEM, st>>>(s.Bw, s.P, s.zpart, N, i, nJ, nJmax);
       // algorithmic traffic: the lower triangle once, v in, y out; 8 real flops per complex fma, 2 per element
       be_prof_end(ctx, PK_HEMV, (double)cnt * (0.5 * n * (n + 1.0) + 2.0 * n) * 16.0, (double)cnt * 8.0 * n * n);
       LAUNCH_CHECK();
@@ -728,14 +789,14 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
 
   // ---- S1b: tridiagonal eigenproblem
   {
-    const int nblk = (N + 127) / 128;
+    const int nblk = (ne + 127) / 128;
     const size_t sh = 2 * (size_t)N * sizeof(double);
     if (sh > 48 * 1024) {
       BE_CUDA(cudaFuncSetAttribute(k_bisect, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
       BE_CUDA(cudaFuncSetAttribute(k_invit, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
     }
     be_prof_begin(ctx, PK_BISECT);
-    k_bisect<<<(unsigned)(cnt * nblk), 128, sh, st>>>(s.d, s.e, E, s.tnorm, s.blo, s.bhi, s.bcl, N, nblk);
+    k_bisect<<<(unsigned)(cnt * nblk), 128, sh, st>>>(s.d, s.e, E, s.tnorm, s.blo, s.bhi, s.bcl, N, nblk, ne);
     be_prof_end(ctx, PK_BISECT, (double)cnt * N * 24.0, 0.0);
     LAUNCH_CHECK();
     if (nv > 0) {

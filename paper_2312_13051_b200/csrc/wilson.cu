@@ -157,9 +157,10 @@ int be_nested_select_small(be_ctx* ctx, const cplx* W, int64_t cnt, int m, int w
 
 // Chain of one chunk: frames F [outer][inner][m][N] (column-major N x m each, ld N) ->
 // links M_j = F_j^H F_{j+1} (ring, Phi on the link at inner index phi_at) -> ordered product
-// W = M_0 M_1 ... M_{n1-1} per outer.  Returns W (column-major m x m, stride m*m) in *Wout.
+// W = M_0 M_1 ... M_{n1-1} per outer.  Returns W (column-major m x m, stride m*m) in *Wout; when
+// Wdst is not NULL the final product is written there (a buffer that outlives the chunk).
 int be_chain_product(be_ctx* ctx, const cplx* F, int N, int m, int64_t outer, int n1,
-                     const cplx* d_close, int phi_at, cplx** Wout) {
+                     const cplx* d_close, int phi_at, cplx* Wdst, cplx** Wout) {
   const int64_t mm = (int64_t)m * m;
   cplx* M = (cplx*)be_arena_alloc(ctx, (size_t)outer * n1 * mm * sizeof(cplx));
   cplx* W0 = (cplx*)be_arena_alloc(ctx, (size_t)outer * mm * sizeof(cplx));
@@ -175,15 +176,16 @@ int be_chain_product(be_ctx* ctx, const cplx* F, int N, int m, int64_t outer, in
   g.alpha = mkc(1.0, 0.0); g.beta = mkc(0.0, 0.0); g.lower = 0;
   BE_TRY(be_zgemm(ctx, BE_OP_C, BE_OP_N, g));
   if (n1 == 1) {
-    BE_CUDA(cudaMemcpyAsync(W0, M, (size_t)outer * mm * sizeof(cplx), cudaMemcpyDeviceToDevice, ctx->stream));
-    *Wout = W0;
+    cplx* dst = Wdst ? Wdst : W0;
+    BE_CUDA(cudaMemcpyAsync(dst, M, (size_t)outer * mm * sizeof(cplx), cudaMemcpyDeviceToDevice, ctx->stream));
+    *Wout = dst;
     return BE_OK;
   }
   const cplx* cur = M;            // running product, stride curs
   int64_t curs = (int64_t)n1 * mm;
   cplx* bufs[2] = {W0, W1};
   for (int j = 1; j < n1; ++j) {
-    cplx* dst = bufs[j & 1];
+    cplx* dst = (j == n1 - 1 && Wdst) ? Wdst : bufs[j & 1];
     ZgemmParams p = zgemm_simple(m, m, m, cur, m, curs, M + (int64_t)j * mm, m, (int64_t)n1 * mm,
                                  dst, m, mm, outer);
     BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_N, p));

@@ -134,14 +134,21 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
         br[nb] = s[2 * SM_PLANE + k * LDS + n];
         bim[nb] = s[3 * SM_PLANE + k * LDS + n];
       }
+      // four real products; consecutive DMMAs never touch the same accumulator (no back-to-back
+      // dependency on the 16-deep accumulator set)
+#pragma unroll
+      for (int mb = 0; mb < 4; ++mb)
+#pragma unroll
+        for (int nb = 0; nb < 2; ++nb) {
+          dmma(accr[mb][nb][0], accr[mb][nb][1], ar[mb], br[nb]);
+          dmma(acci[mb][nb][0], acci[mb][nb][1], ar[mb], bim[nb]);
+        }
 #pragma unroll
       for (int mb = 0; mb < 4; ++mb) {
         const double nai = -aim[mb];
 #pragma unroll
         for (int nb = 0; nb < 2; ++nb) {
-          dmma(accr[mb][nb][0], accr[mb][nb][1], ar[mb], br[nb]);
           dmma(accr[mb][nb][0], accr[mb][nb][1], nai, bim[nb]);
-          dmma(acci[mb][nb][0], acci[mb][nb][1], ar[mb], bim[nb]);
           dmma(acci[mb][nb][0], acci[mb][nb][1], aim[mb], br[nb]);
         }
       }
