@@ -4,9 +4,9 @@
 // All matrices of a chunk advance in lock step, one kernel launch per algorithmic step over the
 // whole batch, so every launch is a wide streaming kernel:
 //   S1a  blocked Householder tridiagonalization  B = Q T Q^H  (panel width NB = 32)
-//          k_col   : apply the pending panel updates to column i, generate the reflector
+//          k_colw  : finish w_i (panel corrections, tau, -1/2 tau (w^H v) v) and, in the same sweep
+//                    over the panels, apply the pending updates to column i+1 and generate its reflector
 //          k_hemv  : y = B22 v on the lower triangle only (each element read once, used twice)
-//          k_w     : finish w_i (panel corrections, tau, -1/2 tau (w^H v) v)
 //          rank-2k : B22 -= V W^H + W V^H                   -> DMMA ZGEMM (zgemm.cu), lower tiles
 //   S1b  real symmetric tridiagonal eigenproblem
 //          k_bisect: all eigenvalues by Sturm-count bisection, one thread per eigenvalue
@@ -47,53 +47,6 @@ __global__ void k_gather(const cplx* __restrict__ H, cplx* __restrict__ Bw, Grid
 }
 
 // ------------------------------------------------------------------------------------------
-// column i: B[i:, i] -= V[i:, :k] conj(W[i, :k]) + W[i:, :k] conj(V[i, :k]); then zlarfg.
-__global__ void __launch_bounds__(256) k_col(cplx* __restrict__ Bw, const cplx* __restrict__ Wp,
-                                             double* __restrict__ dd, double* __restrict__ ee,
-                                             cplx* __restrict__ tau, int N, int i, int p) {
-  __shared__ cplx cw[NB], cv[NB];
-  __shared__ double red[33];
-  __shared__ cplx sh_alpha;
-  const int64_t c = blockIdx.x;
-  cplx* B = Bw + c * (int64_t)N * N;
-  const cplx* W = Wp + c * (int64_t)N * NB;
-  const int k = i - p, tid = threadIdx.x;
-  if (tid < k) {
-    cw[tid] = cconj(W[i + (int64_t)tid * N]);
-    cv[tid] = cconj(B[i + (int64_t)(p + tid) * N]);
-  }
-  __syncthreads();
-  double ss = 0.0;
-  for (int r = i + tid; r < N; r += 256) {
-    cplx acc = B[r + (int64_t)i * N];
-    for (int cc = 0; cc < k; ++cc) {
-      cfms(acc, B[r + (int64_t)(p + cc) * N], cw[cc]);
-      cfms(acc, W[r + (int64_t)cc * N], cv[cc]);
-    }
-    if (r == i) { acc.y = 0.0; dd[c * N + i] = acc.x; }
-    else if (r == i + 1) sh_alpha = acc;
-    else ss += cabs2(acc);
-    B[r + (int64_t)i * N] = acc;
-  }
-  if (i >= N - 1) return;
-  const double xn2 = block_sum(ss, red);
-  const cplx alpha = sh_alpha;
-  double beta; cplx t, scale;
-  if (xn2 == 0.0 && alpha.y == 0.0) {
-    beta = alpha.x; t = mkc(0.0, 0.0); scale = mkc(0.0, 0.0);
-  } else {
-    beta = -copysign(sqrt(cabs2(alpha) + xn2), alpha.x);
-    t = mkc((beta - alpha.x) / beta, -alpha.y / beta);
-    scale = cdiv(mkc(1.0, 0.0), mkc(alpha.x - beta, alpha.y));
-  }
-  for (int r = i + tid; r < N; r += 256) {
-    if (r == i + 1) B[r + (int64_t)i * N] = mkc(1.0, 0.0);
-    else if (r >= i + 2) B[r + (int64_t)i * N] = cmul(B[r + (int64_t)i * N], scale);
-  }
-  if (tid == 0) { ee[c * N + i] = beta; tau[c * N + i] = t; }
-}
-
-// ------------------------------------------------------------------------------------------
 // y = B22 v with B22 = B[i+1:, i+1:] Hermitian, lower triangle stored; v = B[i+1:, i].
 //
 // The kernel is HBM bound (1 flop/byte): every element B[r][c], r > c, is read exactly once and used
@@ -103,7 +56,7 @@ __global__ void __launch_bounds__(256) k_col(cplx* __restrict__ Bw, const cplx* 
 // matching piece of v, completion on an mbarrier), HSTAGES deep, so the bytes in flight do not
 // depend on registers or on the progress of the arithmetic.  256 consumer threads: thread =
 // (row lr of the stage, group cg of 8 columns).  Row part: summed over the 4 column groups through
-// shared memory and written per block column to P (k_w adds the block columns up: no atomics, the
+// shared memory and written per block column to P (k_colw adds the block columns up: no atomics, the
 // result is bitwise reproducible).  Column part: 8 accumulators per thread kept in registers over
 // the whole block column, reduced once at the end and written to zpart.
 constexpr int HROWS = 64;
@@ -134,15 +87,43 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, uint32_
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+constexpr int HDOT = 8;   // dot CTAs per matrix
 __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict__ Bw, cplx* __restrict__ P,
-                                                          cplx* __restrict__ zpart, int N, int i, int nJ, int nJmax) {
+                                                          cplx* __restrict__ zpart, int N, int i, int nJ, int nJmax,
+                                                          const cplx* __restrict__ Wp, cplx* __restrict__ pqg,
+                                                          int p, int ndot) {
+  if ((int)blockIdx.x < ndot) {
+    // ---- dot CTAs (scheduled first, overlapped with the streaming CTAs): the 2k products
+    //      pq[q] = W[:, q]^H v (q < k), V[:, q-k]^H v (q >= k) that k_colw needs for w_i
+    const int64_t c = blockIdx.x / HDOT;
+    const int part = blockIdx.x % HDOT;
+    const cplx* __restrict__ B = Bw + c * (int64_t)N * N;
+    const cplx* __restrict__ W = Wp + c * (int64_t)N * NB;
+    const cplx* __restrict__ v = B + (int64_t)i * N;
+    const int k = i - p, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int q = part * (HEMV_THREADS / 32) + warp; q < 2 * k; q += HDOT * (HEMV_THREADS / 32)) {
+      const cplx* ptr = (q < k) ? (W + (int64_t)q * N) : (B + (int64_t)(p + q - k) * N);
+      cplx a0 = mkc(0.0, 0.0), a1 = a0, a2 = a0, a3 = a0;
+      int r = i + 1 + lane;
+      for (; r + 96 < N; r += 128) {
+        const cplx x0 = ptr[r], x1 = ptr[r + 32], x2 = ptr[r + 64], x3 = ptr[r + 96];
+        const cplx v0 = v[r], v1 = v[r + 32], v2 = v[r + 64], v3 = v[r + 96];
+        cfmac(a0, x0, v0); cfmac(a1, x1, v1); cfmac(a2, x2, v2); cfmac(a3, x3, v3);
+      }
+      for (; r < N; r += 32) cfmac(a0, ptr[r], v[r]);
+      const cplx acc = warp_sum(cadd(cadd(a0, a1), cadd(a2, a3)));
+      if (lane == 0) pqg[c * (2 * NB) + q] = acc;
+    }
+    return;
+  }
+  const int bid = blockIdx.x - ndot;
   extern __shared__ __align__(128) unsigned char hsm[];
   cplx* stage = (cplx*)hsm;                                           // [HSTAGES][HB + 1][HROWS]
   cplx* ysm = stage + (size_t)HSTAGES * HSTAGE_ELEMS;                 // [2][4][HROWS]
   unsigned long long* full = (unsigned long long*)(ysm + 2 * 4 * HROWS);
   unsigned long long* empty = full + HSTAGES;
-  const int64_t c = blockIdx.x / nJ;
-  const int J = blockIdx.x % nJ;
+  const int64_t c = bid / nJ;
+  const int J = bid % nJ;
   const cplx* __restrict__ B = Bw + c * (int64_t)N * N;
   const cplx* __restrict__ v = B + (int64_t)i * N;   // v[r], r >= i+1 (global row index)
   const int tid = threadIdx.x;
@@ -244,51 +225,128 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
 }
 
 // ------------------------------------------------------------------------------------------
-// w = tau (y - V (W^H v) - W (V^H v)); w += -1/2 tau (w^H v) v; stored as column k of the W panel.
-__global__ void __launch_bounds__(256) k_w(const cplx* __restrict__ Bw, cplx* __restrict__ Wp,
-                                           const cplx* __restrict__ P, const cplx* __restrict__ zpart,
-                                           const cplx* __restrict__ tau, int N, int i, int p, int nJmax) {
-  extern __shared__ cplx ysh[];   // N entries, indexed by global row
-  __shared__ cplx pq[2 * NB];
-  __shared__ cplx red[33];
+// Fused panel step, one CTA per matrix.
+//   do_w  : finish w_i = tau (y - V (W^H v) - W (V^H v)), w_i += -1/2 tau (w_i^H v) v, stored as column
+//           k = i - p of the W panel.  y = zpart + sum_J P[J] (k_hemv), the 2k dot products W^H v,
+//           V^H v come from the dot CTAs of the same k_hemv launch (pqg).
+//   do_col: column ic (= i + 1 with do_w, = i without) gets the pending panel updates
+//           B[ic:, ic] -= V[ic:, :kc] conj(W[ic, :kc]) + W[ic:, :kc] conj(V[ic, :kc]) and its reflector
+//           is generated (zlarfg): d[ic], e[ic], tau[ic], v stored in place with a unit head.
+// With both flags the V and W panels are read ONCE: the column update of ic is accumulated in the
+// same sweep that corrects y, the term of the new reflector i is added from shared memory.
+constexpr int CW_THREADS = 512;
+__global__ void __launch_bounds__(CW_THREADS) k_colw(cplx* __restrict__ Bw, cplx* __restrict__ Wp,
+                                                     const cplx* __restrict__ P, const cplx* __restrict__ zpart,
+                                                     const cplx* __restrict__ pqg, double* __restrict__ dd,
+                                                     double* __restrict__ ee, cplx* __restrict__ tau,
+                                                     int N, int i, int p, int nJmax, int do_w, int do_col) {
+  extern __shared__ cplx ysh[];   // w[N] (indexed by global row), then a2[N]
+  __shared__ cplx pq[2 * NB], cw2[NB], cv2[NB];
+  __shared__ cplx redc[33];
+  __shared__ double redd[33];
+  __shared__ cplx sh_alpha;
+  cplx* a2s = ysh + N;
   const int64_t c = blockIdx.x;
-  const cplx* __restrict__ B = Bw + c * (int64_t)N * N;
+  cplx* __restrict__ B = Bw + c * (int64_t)N * N;
   cplx* __restrict__ W = Wp + c * (int64_t)N * NB;
-  const cplx* __restrict__ v = B + (int64_t)i * N;
-  const int k = i - p, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  for (int r = i + 1 + tid; r < N; r += 256) {
-    cplx y = zpart[c * N + r];
-    const int Jr = (r - (i + 1)) / HB;
-    for (int J = 0; J <= Jr; ++J) y = cadd(y, P[(c * nJmax + J) * (int64_t)N + r]);
-    ysh[r] = y;
-  }
-  for (int col = warp; col < 2 * k; col += 8) {
-    const cplx* ptr = (col < k) ? (W + (int64_t)col * N) : (B + (int64_t)(p + col - k) * N);
-    cplx acc = mkc(0.0, 0.0);
-    for (int r = i + 1 + lane; r < N; r += 32) cfmac(acc, ptr[r], v[r]);
-    acc = warp_sum(acc);
-    if (lane == 0) pq[col] = acc;
-  }
-  __syncthreads();
-  const cplx t = tau[c * N + i];
-  cplx dot = mkc(0.0, 0.0);
-  for (int r = i + 1 + tid; r < N; r += 256) {
-    cplx y = ysh[r];
-    for (int cc = 0; cc < k; ++cc) {
-      cfms(y, B[r + (int64_t)(p + cc) * N], pq[cc]);
-      cfms(y, W[r + (int64_t)cc * N], pq[k + cc]);
+  const int tid = threadIdx.x;
+  const int ic = do_w ? i + 1 : i;
+  if (do_w) {
+    const cplx* __restrict__ v = B + (int64_t)i * N;
+    const int k = i - p;
+    if (tid < 2 * k) pq[tid] = pqg[c * (2 * NB) + tid];
+    if (do_col && tid < k) {
+      cw2[tid] = cconj(W[ic + (int64_t)tid * N]);
+      cv2[tid] = cconj(B[ic + (int64_t)(p + tid) * N]);
     }
-    const cplx wv = cmul(t, y);
-    ysh[r] = wv;
-    cfmac(dot, wv, v[r]);
+    __syncthreads();
+    const cplx t = tau[c * N + i];
+    cplx dot = mkc(0.0, 0.0);
+    for (int r = i + 1 + tid; r < N; r += CW_THREADS) {
+      cplx y = zpart[c * N + r];
+      const int Jr = (r - (i + 1)) / HB;
+      cplx a2 = do_col ? B[r + (int64_t)ic * N] : mkc(0.0, 0.0);
+      {
+        const cplx* Pr = P + c * nJmax * (int64_t)N + r;
+        int J = 0;
+        for (; J + 4 <= Jr + 1; J += 4) {   // independent loads first: the sweep is latency bound
+          const cplx p0 = Pr[(int64_t)J * N], p1 = Pr[(int64_t)(J + 1) * N], p2 = Pr[(int64_t)(J + 2) * N],
+                     p3 = Pr[(int64_t)(J + 3) * N];
+          y = cadd(cadd(y, cadd(p0, p1)), cadd(p2, p3));
+        }
+        for (; J <= Jr; ++J) y = cadd(y, Pr[(int64_t)J * N]);
+      }
+      int cc = 0;
+      for (; cc + 4 <= k; cc += 4) {
+        cplx bv[4], wv[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { bv[u] = B[r + (int64_t)(p + cc + u) * N]; wv[u] = W[r + (int64_t)(cc + u) * N]; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          cfms(y, bv[u], pq[cc + u]);
+          cfms(y, wv[u], pq[k + cc + u]);
+          if (do_col) { cfms(a2, bv[u], cw2[cc + u]); cfms(a2, wv[u], cv2[cc + u]); }
+        }
+      }
+      for (; cc < k; ++cc) {
+        const cplx bv = B[r + (int64_t)(p + cc) * N], wv = W[r + (int64_t)cc * N];
+        cfms(y, bv, pq[cc]);
+        cfms(y, wv, pq[k + cc]);
+        if (do_col) { cfms(a2, bv, cw2[cc]); cfms(a2, wv, cv2[cc]); }
+      }
+      const cplx wv = cmul(t, y);
+      ysh[r] = wv;
+      a2s[r] = a2;
+      cfmac(dot, wv, v[r]);
+    }
+    dot = block_sum(dot, redc);
+    const cplx al = cmul(mkc(-0.5 * t.x, -0.5 * t.y), dot);
+    for (int r = i + 1 + tid; r < N; r += CW_THREADS) {
+      cplx wv = ysh[r];
+      cfma(wv, al, v[r]);
+      W[r + (int64_t)k * N] = wv;
+      ysh[r] = wv;
+    }
+    __syncthreads();
+    if (!do_col) return;
+    // term of reflector i itself: V[r][k] = v[r] (v[ic] = 1), W[r][k] = w[r]
+    const cplx cwi = cconj(ysh[ic]);
+    for (int r = ic + tid; r < N; r += CW_THREADS) {
+      cplx a2 = a2s[r];
+      cfms(a2, v[r], cwi);
+      a2 = csub(a2, ysh[r]);
+      a2s[r] = a2;
+    }
+  } else {
+    for (int r = ic + tid; r < N; r += CW_THREADS) a2s[r] = B[r + (int64_t)ic * N];
   }
-  dot = block_sum(dot, red);
-  const cplx a2 = cmul(mkc(-0.5 * t.x, -0.5 * t.y), dot);
-  for (int r = i + 1 + tid; r < N; r += 256) {
-    cplx wv = ysh[r];
-    cfma(wv, a2, v[r]);
-    W[r + (int64_t)k * N] = wv;
+  // ---- zlarfg on column ic (each thread re-reads only the rows it wrote)
+  double ss = 0.0;
+  for (int r = ic + tid; r < N; r += CW_THREADS) {
+    const cplx a2 = a2s[r];
+    if (r == ic) dd[c * N + ic] = a2.x;
+    else if (r == ic + 1) sh_alpha = a2;
+    else ss += cabs2(a2);
   }
+  if (ic >= N - 1) return;
+  const double xn2 = block_sum(ss, redd);
+  const cplx alpha = sh_alpha;
+  double beta; cplx t, scale;
+  if (xn2 == 0.0 && alpha.y == 0.0) {
+    beta = alpha.x; t = mkc(0.0, 0.0); scale = mkc(0.0, 0.0);
+  } else {
+    beta = -copysign(sqrt(cabs2(alpha) + xn2), alpha.x);
+    t = mkc((beta - alpha.x) / beta, -alpha.y / beta);
+    scale = cdiv(mkc(1.0, 0.0), mkc(alpha.x - beta, alpha.y));
+  }
+  for (int r = ic + tid; r < N; r += CW_THREADS) {
+    cplx a2 = a2s[r];
+    if (r == ic) a2.y = 0.0;
+    else if (r == ic + 1) a2 = mkc(1.0, 0.0);
+    else a2 = cmul(a2, scale);
+    B[r + (int64_t)ic * N] = a2;
+  }
+  if (tid == 0) { ee[c * N + ic] = beta; tau[c * N + ic] = t; }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -674,7 +732,7 @@ __global__ void k_x2u(const cplx* __restrict__ X, cplx* __restrict__ U, int N, i
 
 // scratch layout for ``cnt`` matrices
 struct EighScratch {
-  cplx *Bw, *Wp, *P, *zpart, *tau, *Vb, *T, *G, *tauc, *Y, *Y2;
+  cplx *Bw, *Wp, *P, *zpart, *tau, *Vb, *T, *G, *tauc, *Y, *Y2, *pq;
   double *d, *e, *tnorm, *Z, *fa, *fb, *fc;
   unsigned char* fp;
   int* blk;
@@ -698,6 +756,7 @@ static size_t eigh_large_carve(char* base, int64_t cnt, int N, int nv, EighScrat
   cplx* tauc = (cplx*)take(cnt * (size_t)NBT * sizeof(cplx));
   cplx* Y = (cplx*)take(cnt * (size_t)NBT * (nv > 0 ? nv : 1) * sizeof(cplx));
   cplx* Y2 = (cplx*)take(cnt * (size_t)NBT * (nv > 0 ? nv : 1) * sizeof(cplx));
+  cplx* pq = (cplx*)take(cnt * (size_t)2 * NB * sizeof(cplx));
   double* d = (double*)take(cnt * (size_t)N * sizeof(double));
   double* e = (double*)take(cnt * (size_t)N * sizeof(double));
   double* tn = (double*)take(cnt * sizeof(double));
@@ -710,7 +769,7 @@ static size_t eigh_large_carve(char* base, int64_t cnt, int N, int nv, EighScrat
   double* blo = (double*)take(cnt * (size_t)N * sizeof(double));
   double* bhi = (double*)take(cnt * (size_t)N * sizeof(double));
   int* bcl = (int*)take(cnt * (size_t)N * sizeof(int));
-  if (s) { *s = EighScratch{Bw, Wp, P, zp, tau, Vb, T, G, tauc, Y, Y2, d, e, tn, Z, fa, fb, fc, fp, blk, blo, bhi, bcl}; }
+  if (s) { *s = EighScratch{Bw, Wp, P, zp, tau, Vb, T, G, tauc, Y, Y2, pq, d, e, tn, Z, fa, fb, fc, fp, blk, blo, bhi, bcl}; }
   return off;
 }
 
@@ -737,35 +796,37 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
     k_gather<<<(unsigned)(cnt * nchunk), 256, 0, st>>>(H, s.Bw, map, loop0, N, nchunk);
     LAUNCH_CHECK();
   }
-  const size_t ysh_bytes = (size_t)N * sizeof(cplx);
+  const size_t ysh_bytes = 2 * (size_t)N * sizeof(cplx);
   if (ysh_bytes > 200 * 1024) return BE_ERR_UNSUPPORTED;
-  if (ysh_bytes > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_w, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ysh_bytes));
+  if (ysh_bytes > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_colw, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ysh_bytes));
   BE_CUDA(cudaFuncSetAttribute(k_hemv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HEMV_SMEM));
+  auto colw = [&](int i, int p, int do_w, int do_col) {
+    const int n = N - i - 1, kk = i - p;
+    be_prof_begin(ctx, PK_COL);
+    k_colw<<<(unsigned)cnt, CW_THREADS, ysh_bytes, st>>>(s.Bw, s.Wp, s.P, s.zpart, s.pq, s.d, s.e, s.tau, N, i, p,
+                                                         nJmax, do_w, do_col);
+    // panels V, W read once (2 kk columns), y partials, v, w out, column in / out
+    be_prof_end(ctx, PK_COL, (double)cnt * (n + 1) * 16.0 * (2.0 * kk + 6.0 + 0.5 * ((n + HB - 1) / HB)),
+                (double)cnt * (n + 1) * 32.0 * kk);
+  };
 
   // ---- S1a: blocked tridiagonalization
   for (int p = 0; p < N; p += NB) {
     const int pend = (p + NB < N - 1) ? p + NB : N - 1;   // reflector columns p .. pend-1
-    if (p >= N - 1) {   // only the last diagonal entry remains
-      k_col<<<(unsigned)cnt, 256, 0, st>>>(s.Bw, s.Wp, s.d, s.e, s.tau, N, N - 1, p);
-      LAUNCH_CHECK();
-      break;
-    }
+    colw(p, p, 0, 1);   // reflector of column p (or, when p == N-1, just the last diagonal entry)
+    LAUNCH_CHECK();
+    if (p >= N - 1) break;
     for (int i = p; i < pend; ++i) {
       const int n = N - i - 1;
-      const int kk = i - p;
-      be_prof_begin(ctx, PK_COL);
-      k_col<<<(unsigned)cnt, 256, 0, st>>>(s.Bw, s.Wp, s.d, s.e, s.tau, N, i, p);
-      be_prof_end(ctx, PK_COL, (double)cnt * (n + 1) * 16.0 * (2 + 2 * kk), (double)cnt * (n + 1) * 16.0 * kk);
-      LAUNCH_CHECK();
       const int nJ = (n + HB - 1) / HB;
+      const int ndot = (i > p) ? (int)cnt * HDOT : 0;
       be_prof_begin(ctx, PK_HEMV);
-      k_hemv<<<(unsigned)(cnt * nJ), HEMV_THREADS, HEMV_SMEM, st>>>(s.Bw, s.P, s.zpart, N, i, nJ, nJmax);
+      k_hemv<<<(unsigned)(cnt * nJ + ndot), HEMV_THREADS, HEMV_SMEM, st>>>(s.Bw, s.P, s.zpart, N, i, nJ, nJmax, s.Wp,
+                                                                            s.pq, p, ndot);
       // algorithmic traffic: the lower triangle once, v in, y out; 8 real flops per complex fma, 2 per element
       be_prof_end(ctx, PK_HEMV, (double)cnt * (0.5 * n * (n + 1.0) + 2.0 * n) * 16.0, (double)cnt * 8.0 * n * n);
       LAUNCH_CHECK();
-      be_prof_begin(ctx, PK_W);
-      k_w<<<(unsigned)cnt, 256, ysh_bytes, st>>>(s.Bw, s.Wp, s.P, s.zpart, s.tau, N, i, p, nJmax);
-      be_prof_end(ctx, PK_W, (double)cnt * n * 16.0 * (3 + 4 * kk), (double)cnt * n * 32.0 * kk);
+      colw(i, p, 1, (i + 1 < pend) ? 1 : 0);   // w_i, and the reflector of column i+1 inside the panel
       LAUNCH_CHECK();
     }
     const int q = pend, kb = pend - p;
@@ -781,7 +842,7 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
       BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_C, g));
     }
     if (pend == N - 1) {   // last diagonal element (no pending panel: it was just applied)
-      k_col<<<(unsigned)cnt, 256, 0, st>>>(s.Bw, s.Wp, s.d, s.e, s.tau, N, N - 1, N - 1);
+      colw(N - 1, N - 1, 0, 1);
       LAUNCH_CHECK();
       break;
     }

@@ -20,7 +20,8 @@ namespace {
 
 constexpr int TM = 64, TN = 64, TK = 16, LDS = 68;  // LDS % 16 == 4: conflict-free fragment loads
 constexpr int NTHREADS = 256;
-constexpr int SM_PLANE = TK * LDS;                   // doubles per plane
+constexpr int LDK = 20;                              // k-contiguous operands: [mn][k], LDK % 16 == 4
+constexpr int SM_PLANE = TM * LDK;                   // doubles per plane (>= TK * LDS)
 constexpr int SM_STAGE = 4 * SM_PLANE;               // A_re, A_im, B_re, B_im
 constexpr size_t SM_BYTES = 2 * SM_STAGE * sizeof(double);
 
@@ -29,7 +30,7 @@ __device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b)
                : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
-template <int OPA, int OPB>
+template <int OPA, int OPB, bool PHI>
 __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p, int tilesM, int tilesN) {
   extern __shared__ double smem[];
   const int tid = threadIdx.x;
@@ -47,7 +48,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
   if (p.ringB) { biB = bi + 1; if (biB == p.inner) biB = 0; wrap = (bi == p.phi_at); }
   const cplx* __restrict__ B = p.B + bo * p.sBo + (int64_t)biB * p.sBi;
   cplx* __restrict__ C = p.C + bo * p.sCo + (int64_t)bi * p.sCi;
-  const cplx* __restrict__ phi = (wrap && p.phiB) ? p.phiB : nullptr;
+  const cplx* __restrict__ phi = (PHI && wrap && p.phiB) ? p.phiB : nullptr;
 
   const int m0 = tm * TM, n0 = tn * TN;
   const int M = p.M, N = p.N, K = p.K;
@@ -62,26 +63,26 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
   if (!transB) { bk = tid & 15; bn = tid >> 4; bqn = 16; bqk = 0; }
   else         { bn = tid & 63; bk = tid >> 6; bqn = 0; bqk = 4; }
 
-  cplx ra[4], rb[4];
+  cplx ra[4], rb[4], rphi[4];
   auto gload = [&](int k0) {
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       const int i = m0 + ai + q * aqi, k = k0 + ak + q * aqk;
       cplx v = mkc(0.0, 0.0);
       if (i < M && k < K) v = transA ? A[(int64_t)k + (int64_t)i * p.lda] : A[(int64_t)i + (int64_t)k * p.lda];
-      if (conjA) v.y = -v.y;
       ra[q] = v;
     }
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       const int n = n0 + bn + q * bqn, k = k0 + bk + q * bqk;
       cplx v = mkc(0.0, 0.0);
+      cplx f = mkc(1.0, 0.0);
       if (n < N && k < K) {
         v = transB ? B[(int64_t)n + (int64_t)k * p.ldb] : B[(int64_t)k + (int64_t)n * p.ldb];
-        if (phi) v = cmul(phi[k], v);
+        if (PHI && phi) f = phi[k];
       }
-      if (conjB) v.y = -v.y;
-      rb[q] = v;
+      rb[q] = v;          // no arithmetic on loaded values here: the loads stay in flight during the
+      if (PHI) rphi[q] = f;   // multiplication of the current tile; sign flips / phases are applied in sstore
     }
   };
   auto sstore = [&](int stage) {
@@ -89,14 +90,18 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       const int i = ai + q * aqi, k = ak + q * aqk;
-      s[k * LDS + i] = ra[q].x;
-      s[SM_PLANE + k * LDS + i] = ra[q].y;
+      const int o = transA ? i * LDK + k : k * LDS + i;   // conflict-free for the store and the fragment loads
+      s[o] = ra[q].x;
+      s[SM_PLANE + o] = conjA ? -ra[q].y : ra[q].y;
     }
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       const int n = bn + q * bqn, k = bk + q * bqk;
-      s[2 * SM_PLANE + k * LDS + n] = rb[q].x;
-      s[3 * SM_PLANE + k * LDS + n] = rb[q].y;
+      cplx v = rb[q];
+      if (PHI) v = cmul(rphi[q], v);
+      const int o = transB ? k * LDS + n : n * LDK + k;
+      s[2 * SM_PLANE + o] = v.x;
+      s[3 * SM_PLANE + o] = conjB ? -v.y : v.y;
     }
   };
 
@@ -125,14 +130,16 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
 #pragma unroll
       for (int mb = 0; mb < 4; ++mb) {
         const int i = wm * 32 + mb * 8 + g;
-        ar[mb] = s[k * LDS + i];
-        aim[mb] = s[SM_PLANE + k * LDS + i];
+        const int o = transA ? i * LDK + k : k * LDS + i;
+        ar[mb] = s[o];
+        aim[mb] = s[SM_PLANE + o];
       }
 #pragma unroll
       for (int nb = 0; nb < 2; ++nb) {
         const int n = wn * 16 + nb * 8 + g;
-        br[nb] = s[2 * SM_PLANE + k * LDS + n];
-        bim[nb] = s[3 * SM_PLANE + k * LDS + n];
+        const int o = transB ? k * LDS + n : n * LDK + k;
+        br[nb] = s[2 * SM_PLANE + o];
+        bim[nb] = s[3 * SM_PLANE + o];
       }
       // four real products; consecutive DMMAs never touch the same accumulator (no back-to-back
       // dependency on the 16-deep accumulator set)
@@ -160,26 +167,44 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
   }
 
   const bool has_beta = (p.beta.x != 0.0 || p.beta.y != 0.0);
+  // epilogue in two halves of 8 elements: all loads of C first (independent, in flight together),
+  // then the stores -- a load/store per element in program order would serialize 16 round trips
 #pragma unroll
-  for (int mb = 0; mb < 4; ++mb) {
-    const int row = m0 + wm * 32 + mb * 8 + g;
-    if (row >= M) continue;
+  for (int half = 0; half < 2; ++half) {
+    cplx cold[2][2][2];
+    if (has_beta) {
 #pragma unroll
-    for (int nb = 0; nb < 2; ++nb) {
+      for (int m2 = 0; m2 < 2; ++m2) {
+        const int mb = half * 2 + m2;
+        const int row = m0 + wm * 32 + mb * 8 + g;
 #pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        const int col = n0 + wn * 16 + nb * 8 + 2 * tg + e;
-        if (col >= N) continue;
-        cplx v = cmul(p.alpha, mkc(accr[mb][nb][e], acci[mb][nb][e]));
-        cplx* dst = C + (int64_t)row + (int64_t)col * p.ldc;
-        if (has_beta) v = cadd(v, cmul(p.beta, *dst));
-        *dst = v;
+        for (int nb = 0; nb < 2; ++nb)
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const int col = n0 + wn * 16 + nb * 8 + 2 * tg + e;
+            cold[m2][nb][e] = (row < M && col < N) ? C[(int64_t)row + (int64_t)col * p.ldc] : mkc(0.0, 0.0);
+          }
       }
+    }
+#pragma unroll
+    for (int m2 = 0; m2 < 2; ++m2) {
+      const int mb = half * 2 + m2;
+      const int row = m0 + wm * 32 + mb * 8 + g;
+#pragma unroll
+      for (int nb = 0; nb < 2; ++nb)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int col = n0 + wn * 16 + nb * 8 + 2 * tg + e;
+          if (row >= M || col >= N) continue;
+          cplx v = cmul(p.alpha, mkc(accr[mb][nb][e], acci[mb][nb][e]));
+          if (has_beta) v = cadd(v, cmul(p.beta, cold[m2][nb][e]));
+          C[(int64_t)row + (int64_t)col * p.ldc] = v;
+        }
     }
   }
 }
 
-template <int OPA, int OPB>
+template <int OPA, int OPB, bool PHI>
 int launch(be_ctx* ctx, const ZgemmParams& p) {
   const int tilesM = (p.M + TM - 1) / TM, tilesN = (p.N + TN - 1) / TN;
   const int64_t blocks = p.batch * tilesM * tilesN;
@@ -187,11 +212,11 @@ int launch(be_ctx* ctx, const ZgemmParams& p) {
   if (blocks > 0x7fffffffLL) return BE_ERR_SHAPE;
   static bool attr_done = false;  // per instantiation; idempotent
   if (!attr_done) {
-    BE_CUDA(cudaFuncSetAttribute(zgemm_kernel<OPA, OPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM_BYTES));
+    BE_CUDA(cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, PHI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM_BYTES));
     attr_done = true;
   }
   be_prof_begin(ctx, PK_GEMM);
-  zgemm_kernel<OPA, OPB><<<(unsigned)blocks, NTHREADS, SM_BYTES, ctx->stream>>>(p, tilesM, tilesN);
+  zgemm_kernel<OPA, OPB, PHI><<<(unsigned)blocks, NTHREADS, SM_BYTES, ctx->stream>>>(p, tilesM, tilesN);
   {
     const double tri = p.lower ? 0.5 : 1.0;
     const double fl = 8.0 * p.M * (double)p.N * p.K * (double)p.batch * tri;
@@ -206,8 +231,9 @@ int launch(be_ctx* ctx, const ZgemmParams& p) {
 
 int be_zgemm(be_ctx* ctx, int opA, int opB, const ZgemmParams& p) {
   if (p.M <= 0 || p.N <= 0 || p.batch <= 0) return BE_OK;
-  if (p.phiB && opB != BE_OP_N) return BE_ERR_UNSUPPORTED;
-#define CASE(a, b) if (opA == a && opB == b) return launch<a, b>(ctx, p);
+  if (p.phiB && (opA != BE_OP_C || opB != BE_OP_N || !p.ringB)) return BE_ERR_UNSUPPORTED;   // closing phase: link GEMM only
+  if (p.phiB && p.ringB) return launch<BE_OP_C, BE_OP_N, true>(ctx, p);
+#define CASE(a, b) if (opA == a && opB == b) return launch<a, b, false>(ctx, p);
   CASE(BE_OP_N, BE_OP_N) CASE(BE_OP_N, BE_OP_C) CASE(BE_OP_C, BE_OP_N) CASE(BE_OP_N, BE_OP_T)
   CASE(BE_OP_T, BE_OP_N) CASE(BE_OP_J, BE_OP_N) CASE(BE_OP_N, BE_OP_J) CASE(BE_OP_C, BE_OP_C) CASE(BE_OP_T, BE_OP_J)
 #undef CASE
