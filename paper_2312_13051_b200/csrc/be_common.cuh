@@ -177,4 +177,7 @@ int be_eigh_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
 int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N,
                   int nv, int ne, double* E, cplx* X, int* info);
 size_t be_eigh_large_scratch_bytes(int64_t cnt, int N, int nv);
+size_t be_cluster_orth_scratch_bytes(int64_t cnt, int N, int nv);
+int be_cluster_orth(be_ctx* ctx, const double* lam, const double* tnorm, const int* blk, double* Z, int64_t cnt, int N,
+                    int nv, double ctol, int* info, void* scratch, int find, int rounds);
 int be_frames_to_public(be_ctx* ctx, const cplx* X, cplx* U, int64_t cnt, int N, int nv);
