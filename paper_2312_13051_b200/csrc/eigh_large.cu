@@ -88,48 +88,29 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, uint32_
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-constexpr int HDOT = 8;   // dot CTAs per matrix
+// Block columns J >= nJ are "panel blocks": 32 columns of the [W | V] panels streamed through the
+// same pipeline with only their column part kept, pq[q] = W[:, q]^H v (q < k), V[:, q-k]^H v (q >= k),
+// the 2k products k_colw needs for w_i.
 __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict__ Bw, cplx* __restrict__ P,
                                                           cplx* __restrict__ zpart, int N, int i, int nJ, int nJmax,
                                                           const cplx* __restrict__ Wp, cplx* __restrict__ pqg,
-                                                          int p, int ndot) {
-  if ((int)blockIdx.x < ndot) {
-    // ---- dot CTAs (scheduled first, overlapped with the streaming CTAs): the 2k products
-    //      pq[q] = W[:, q]^H v (q < k), V[:, q-k]^H v (q >= k) that k_colw needs for w_i
-    const int64_t c = blockIdx.x / HDOT;
-    const int part = blockIdx.x % HDOT;
-    const cplx* __restrict__ B = Bw + c * (int64_t)N * N;
-    const cplx* __restrict__ W = Wp + c * (int64_t)N * NB;
-    const cplx* __restrict__ v = B + (int64_t)i * N;
-    const int k = i - p, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int q = part * (HEMV_THREADS / 32) + warp; q < 2 * k; q += HDOT * (HEMV_THREADS / 32)) {
-      const cplx* ptr = (q < k) ? (W + (int64_t)q * N) : (B + (int64_t)(p + q - k) * N);
-      cplx a0 = mkc(0.0, 0.0), a1 = a0, a2 = a0, a3 = a0;
-      int r = i + 1 + lane;
-      for (; r + 96 < N; r += 128) {
-        const cplx x0 = ptr[r], x1 = ptr[r + 32], x2 = ptr[r + 64], x3 = ptr[r + 96];
-        const cplx v0 = v[r], v1 = v[r + 32], v2 = v[r + 64], v3 = v[r + 96];
-        cfmac(a0, x0, v0); cfmac(a1, x1, v1); cfmac(a2, x2, v2); cfmac(a3, x3, v3);
-      }
-      for (; r < N; r += 32) cfmac(a0, ptr[r], v[r]);
-      const cplx acc = warp_sum(cadd(cadd(a0, a1), cadd(a2, a3)));
-      if (lane == 0) pqg[c * (2 * NB) + q] = acc;
-    }
-    return;
-  }
-  const int bid = blockIdx.x - ndot;
+                                                          int p, int npb) {
   extern __shared__ __align__(128) unsigned char hsm[];
   cplx* stage = (cplx*)hsm;                                           // [HSTAGES][HB + 1][HROWS]
   cplx* ysm = stage + (size_t)HSTAGES * HSTAGE_ELEMS;                 // [2][4][HROWS]
   unsigned long long* full = (unsigned long long*)(ysm + 2 * 4 * HROWS);
   unsigned long long* empty = full + HSTAGES;
-  const int64_t c = bid / nJ;
-  const int J = bid % nJ;
+  const int64_t c = blockIdx.x / (nJ + npb);
+  const int J = blockIdx.x % (nJ + npb);
+  const bool panel = J >= nJ;
+  const int k = i - p;
   const cplx* __restrict__ B = Bw + c * (int64_t)N * N;
+  const cplx* __restrict__ W = Wp + c * (int64_t)N * NB;
   const cplx* __restrict__ v = B + (int64_t)i * N;   // v[r], r >= i+1 (global row index)
   const int tid = threadIdx.x;
-  const int c0 = i + 1 + J * HB;
-  const int ncols = (N - c0 < HB) ? N - c0 : HB;
+  const int q0 = panel ? (J - nJ) * HB : 0;          // first panel column of a panel block
+  const int c0 = panel ? i + 1 : i + 1 + J * HB;     // first row streamed (and first column of a matrix block)
+  const int ncols = panel ? ((2 * k - q0 < HB) ? 2 * k - q0 : HB) : ((N - c0 < HB) ? N - c0 : HB);
   const int nst = (N - c0 + HROWS - 1) / HROWS;
   if (tid == 0) {
     for (int s = 0; s < HSTAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
@@ -152,7 +133,11 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
         tma_bulk_g2s(dst + HB * HROWS, v + r0, seg, &full[slot]);
       }
       __syncwarp();
-      if (lane < ncols) tma_bulk_g2s(dst + lane * HROWS, B + (int64_t)(c0 + lane) * N + r0, seg, &full[slot]);
+      if (lane < ncols) {
+        const int q = q0 + lane;
+        const cplx* src = !panel ? B + (int64_t)(c0 + lane) * N : (q < k ? W + (int64_t)q * N : B + (int64_t)(p + q - k) * N);
+        tma_bulk_g2s(dst + lane * HROWS, src + r0, seg, &full[slot]);
+      }
     }
     return;
   }
@@ -165,7 +150,7 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
 #pragma unroll
   for (int q = 0; q < 8; ++q) {
     accz[q] = mkc(0.0, 0.0);
-    vc[q] = (q < nq) ? v[c0 + cg * 8 + q] : mkc(0.0, 0.0);
+    vc[q] = (q < nq && !panel) ? v[c0 + cg * 8 + q] : mkc(0.0, 0.0);
   }
   cplx* Prow = P + (c * nJmax + J) * (int64_t)N;
   for (int s = 0; s < nst; ++s) {
@@ -176,7 +161,11 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
     cplx yr = mkc(0.0, 0.0);
     if (r < N) {
       const cplx vr = st[HB * HROWS + lr];
-      if (s > 0) {
+      if (panel) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+          if (q < nq) cfmac(accz[q], st[(cg * 8 + q) * HROWS + lr], vr);
+      } else if (s > 0) {
         if (nq == 8) {
           cplx a[8];
 #pragma unroll
@@ -202,6 +191,7 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(&empty[slot]);          // this warp is done with the stage
+    if (panel) continue;                               // no row part
     cplx* yb = ysm + (s & 1) * 4 * HROWS;
     yb[cg * HROWS + lr] = yr;
     asm volatile("bar.sync 1, 256;" ::: "memory");     // consumers only
@@ -221,7 +211,9 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
   asm volatile("bar.sync 1, 256;" ::: "memory");
   if (tid < HB && tid < ncols) {
     const int g = tid >> 3, q = tid & 7;
-    zpart[c * N + c0 + tid] = cadd(zsm[(2 * g) * 8 + q], zsm[(2 * g + 1) * 8 + q]);
+    const cplx z = cadd(zsm[(2 * g) * 8 + q], zsm[(2 * g + 1) * 8 + q]);
+    if (panel) pqg[c * (2 * NB) + q0 + tid] = z;
+    else zpart[c * N + c0 + tid] = z;
   }
 }
 
@@ -740,10 +732,10 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
     for (int i = p; i < pend; ++i) {
       const int n = N - i - 1;
       const int nJ = (n + HB - 1) / HB;
-      const int ndot = (i > p) ? (int)cnt * HDOT : 0;
+      const int npb = (2 * (i - p) + HB - 1) / HB;   // panel blocks: the 2k dot products for k_colw
       be_prof_begin(ctx, PK_HEMV);
-      k_hemv<<<(unsigned)(cnt * nJ + ndot), HEMV_THREADS, HEMV_SMEM, st>>>(s.Bw, s.P, s.zpart, N, i, nJ, nJmax, s.Wp,
-                                                                            s.pq, p, ndot);
+      k_hemv<<<(unsigned)(cnt * (nJ + npb)), HEMV_THREADS, HEMV_SMEM, st>>>(s.Bw, s.P, s.zpart, N, i, nJ, nJmax, s.Wp,
+                                                                             s.pq, p, npb);
       // algorithmic traffic: the lower triangle once, v in, y out; 8 real flops per complex fma, 2 per element
       be_prof_end(ctx, PK_HEMV, (double)cnt * (0.5 * n * (n + 1.0) + 2.0 * n) * 16.0, (double)cnt * 8.0 * n * n);
       LAUNCH_CHECK();
