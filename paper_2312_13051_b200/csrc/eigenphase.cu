@@ -43,13 +43,18 @@ __global__ void k_eig_small(const cplx* __restrict__ W, int64_t cnt, int m, cplx
 }
 
 // ------------------------------------------------------------------------------------------
-__global__ void k_hessenberg(cplx* __restrict__ W, int m) {
-  extern __shared__ cplx vsh[];   // v[m], y[m]
+// Householder reduction to upper Hessenberg form, one CTA of 1024 threads per matrix (there are few
+// Wilson matrices -- 48 at the bench workload -- so the per-matrix latency is what counts).
+//   left  update: warp per pair of columns (dot over rows with lanes, then axpy)
+//   right update: thread = (row i, column slice s of 2); partial y = H v per slice through shared memory
+template <int HESS_THREADS>
+__global__ void __launch_bounds__(HESS_THREADS) k_hessenberg(cplx* __restrict__ W, int m) {
+  extern __shared__ cplx vsh[];   // v[m], y[2][m]
   __shared__ double redd[33];
   __shared__ cplx sh_alpha;
   cplx* v = vsh; cplx* y = vsh + m;
   cplx* H = W + blockIdx.x * (int64_t)m * m;
-  const int tid = threadIdx.x, nt = blockDim.x, warp = tid >> 5, lane = tid & 31, nw = nt >> 5;
+  const int tid = threadIdx.x, nt = HESS_THREADS, warp = tid >> 5, lane = tid & 31, nw = nt >> 5;
   for (int k = 0; k < m - 2; ++k) {
     double ss = 0.0;
     for (int r = k + 1 + tid; r < m; r += nt) {
@@ -67,22 +72,36 @@ __global__ void k_hessenberg(cplx* __restrict__ W, int m) {
       else { v[r] = cmul(H[r + (int64_t)k * m], scale); H[r + (int64_t)k * m] = mkc(0.0, 0.0); }
     }
     __syncthreads();
-    // left: H[k+1:, j] -= conj(tau) v (v^H H[k+1:, j]),  j > k      (warp per column)
+    // left: H[k+1:, j] -= conj(tau) v (v^H H[k+1:, j]),  j > k
     const cplx ctau = cconj(tau);
-    for (int j = k + 1 + warp; j < m; j += nw) {
-      cplx* col = H + (int64_t)j * m;
-      cplx dot = mkc(0.0, 0.0);
-      for (int r = k + 1 + lane; r < m; r += 32) cfmac(dot, v[r], col[r]);
-      dot = cmul(ctau, warp_sum(dot));
-      for (int r = k + 1 + lane; r < m; r += 32) cfms(col[r], v[r], dot);
+    for (int j = k + 1 + 2 * warp; j < m; j += 2 * nw) {
+      cplx* c0 = H + (int64_t)j * m;
+      const bool two = j + 1 < m;
+      cplx* c1 = two ? c0 + m : c0;
+      cplx d0 = mkc(0.0, 0.0), d1 = mkc(0.0, 0.0);
+      for (int r = k + 1 + lane; r < m; r += 32) { const cplx vr = v[r]; cfmac(d0, vr, c0[r]); cfmac(d1, vr, c1[r]); }
+      d0 = cmul(ctau, warp_sum(d0)); d1 = cmul(ctau, warp_sum(d1));
+      for (int r = k + 1 + lane; r < m; r += 32) {
+        const cplx vr = v[r];
+        cfms(c0[r], vr, d0);
+        if (two) cfms(c1[r], vr, d1);
+      }
     }
     __syncthreads();
-    // right: H[:, k+1:] -= tau (H[:, k+1:] v) v^H                    (thread per row)
-    for (int i = tid; i < m; i += nt) {
-      cplx acc = mkc(0.0, 0.0);
-      for (int j = k + 1; j < m; ++j) cfma(acc, H[i + (int64_t)j * m], v[j]);
-      acc = cmul(tau, acc);
-      for (int j = k + 1; j < m; ++j) {
+    // right: H[:, k+1:] -= tau (H[:, k+1:] v) v^H
+    constexpr int RS = HESS_THREADS / 2;
+    const int sl = tid / RS;   // column slice 0 / 1
+    for (int i = tid % RS; i < m; i += RS) {
+      cplx a0 = mkc(0.0, 0.0), a1 = mkc(0.0, 0.0);
+      int j = k + 1 + sl;
+      for (; j + 2 < m; j += 4) { cfma(a0, H[i + (int64_t)j * m], v[j]); cfma(a1, H[i + (int64_t)(j + 2) * m], v[j + 2]); }
+      if (j < m) cfma(a0, H[i + (int64_t)j * m], v[j]);
+      y[sl * m + i] = cadd(a0, a1);
+    }
+    __syncthreads();
+    for (int i = tid % RS; i < m; i += RS) {
+      const cplx acc = cmul(tau, cadd(y[i], y[m + i]));
+      for (int j = k + 1 + sl; j < m; j += 2) {
         cplx h = H[i + (int64_t)j * m];
         cfms(h, acc, cconj(v[j]));
         H[i + (int64_t)j * m] = h;
@@ -90,7 +109,6 @@ __global__ void k_hessenberg(cplx* __restrict__ W, int m) {
     }
     __syncthreads();
   }
-  (void)y;
 }
 
 // Givens: c real, s complex with [c s; -conj(s) c] [a; b] = [r; 0]
@@ -278,10 +296,16 @@ int be_eigenvalues_general(be_ctx* ctx, cplx* W, int64_t cnt, int m, cplx* lam, 
   int nt = ((m + 31) / 32) * 32;
   if (nt > 256) nt = 256;
   if (m > QR_MAXOWN * nt) return BE_ERR_UNSUPPORTED;
-  const size_t sh1 = 2 * (size_t)m * sizeof(cplx);
-  if (sh1 > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_hessenberg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh1));
+  const size_t sh1 = 3 * (size_t)m * sizeof(cplx);
   be_prof_begin(ctx, PK_HESS);
-  k_hessenberg<<<(unsigned)cnt, nt, sh1, st>>>(W, m);
+  if (m <= 48) {
+    k_hessenberg<64><<<(unsigned)cnt, 64, sh1, st>>>(W, m);
+  } else if (m <= 160) {
+    k_hessenberg<256><<<(unsigned)cnt, 256, sh1, st>>>(W, m);
+  } else {
+    if (sh1 > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_hessenberg<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh1));
+    k_hessenberg<1024><<<(unsigned)cnt, 1024, sh1, st>>>(W, m);
+  }
   be_prof_end(ctx, PK_HESS, (double)cnt * m * m * 32.0, (double)cnt * (40.0 / 3.0) * m * (double)m * m);
   ctx->launches++;
   BE_CUDA(cudaGetLastError());
