@@ -91,6 +91,10 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, uint32_
 // Block columns J >= nJ are "panel blocks": 32 columns of the [W | V] panels streamed through the
 // same pipeline with only their column part kept, pq[q] = W[:, q]^H v (q < k), V[:, q-k]^H v (q >= k),
 // the 2k products k_colw needs for w_i.
+// A CTA owns TWO block columns, J and nJ-1-J (long + short: every CTA streams about the same number
+// of stages, and the pipeline prologue / epilogue is paid once per pair); the stage counter runs on
+// across the pair, so the producer prefetches the second block column while the consumers reduce
+// the column part of the first.  Panel blocks come first in the grid (they are the longest).
 __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict__ Bw, cplx* __restrict__ P,
                                                           cplx* __restrict__ zpart, int N, int i, int nJ, int nJmax,
                                                           const cplx* __restrict__ Wp, cplx* __restrict__ pqg,
@@ -100,18 +104,22 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
   cplx* ysm = stage + (size_t)HSTAGES * HSTAGE_ELEMS;                 // [2][4][HROWS]
   unsigned long long* full = (unsigned long long*)(ysm + 2 * 4 * HROWS);
   unsigned long long* empty = full + HSTAGES;
-  const int64_t c = blockIdx.x / (nJ + npb);
-  const int J = blockIdx.x % (nJ + npb);
-  const bool panel = J >= nJ;
+  const int npair = (nJ + 1) / 2;
+  const int64_t c = blockIdx.x / (npair + npb);
+  const int u = blockIdx.x % (npair + npb);
+  const bool panel = u < npb;
   const int k = i - p;
   const cplx* __restrict__ B = Bw + c * (int64_t)N * N;
   const cplx* __restrict__ W = Wp + c * (int64_t)N * NB;
   const cplx* __restrict__ v = B + (int64_t)i * N;   // v[r], r >= i+1 (global row index)
   const int tid = threadIdx.x;
-  const int q0 = panel ? (J - nJ) * HB : 0;          // first panel column of a panel block
-  const int c0 = panel ? i + 1 : i + 1 + J * HB;     // first row streamed (and first column of a matrix block)
-  const int ncols = panel ? ((2 * k - q0 < HB) ? 2 * k - q0 : HB) : ((N - c0 < HB) ? N - c0 : HB);
-  const int nst = (N - c0 + HROWS - 1) / HROWS;
+  // the (up to) two work items of this CTA
+  int Jw[2], nwork;
+  if (panel) { Jw[0] = u; Jw[1] = 0; nwork = 1; }
+  else {
+    Jw[0] = u - npb; Jw[1] = nJ - 1 - Jw[0];
+    nwork = (Jw[1] > Jw[0]) ? 2 : 1;
+  }
   if (tid == 0) {
     for (int s = 0; s < HSTAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -121,22 +129,30 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
   if (tid >= 256) {
     // ---- producer warp: lane = column of the block column (lane 0 also copies the v segment)
     const int lane = tid - 256;
-    for (int s = 0; s < nst; ++s) {
-      const int slot = s % HSTAGES;
-      if (s >= HSTAGES) mbar_wait(&empty[slot], ((s / HSTAGES) - 1) & 1);
-      const int r0 = c0 + s * HROWS;
-      const int nr = (N - r0 < HROWS) ? N - r0 : HROWS;
-      const uint32_t seg = (uint32_t)nr * sizeof(cplx);
-      cplx* dst = stage + (size_t)slot * HSTAGE_ELEMS;
-      if (lane == 0) {
-        mbar_expect_tx(&full[slot], seg * (uint32_t)(ncols + 1));
-        tma_bulk_g2s(dst + HB * HROWS, v + r0, seg, &full[slot]);
-      }
-      __syncwarp();
+    int gs = 0;
+    for (int wi = 0; wi < nwork; ++wi) {
+      const int q0 = panel ? Jw[wi] * HB : 0;
+      const int c0 = panel ? i + 1 : i + 1 + Jw[wi] * HB;
+      const int ncols = panel ? ((2 * k - q0 < HB) ? 2 * k - q0 : HB) : ((N - c0 < HB) ? N - c0 : HB);
+      const int nst = (N - c0 + HROWS - 1) / HROWS;
+      const cplx* src = nullptr;
       if (lane < ncols) {
         const int q = q0 + lane;
-        const cplx* src = !panel ? B + (int64_t)(c0 + lane) * N : (q < k ? W + (int64_t)q * N : B + (int64_t)(p + q - k) * N);
-        tma_bulk_g2s(dst + lane * HROWS, src + r0, seg, &full[slot]);
+        src = !panel ? B + (int64_t)(c0 + lane) * N : (q < k ? W + (int64_t)q * N : B + (int64_t)(p + q - k) * N);
+      }
+      for (int s = 0; s < nst; ++s, ++gs) {
+        const int slot = gs % HSTAGES;
+        if (gs >= HSTAGES) mbar_wait(&empty[slot], ((gs / HSTAGES) - 1) & 1);
+        const int r0 = c0 + s * HROWS;
+        const int nr = (N - r0 < HROWS) ? N - r0 : HROWS;
+        const uint32_t seg = (uint32_t)nr * sizeof(cplx);
+        cplx* dst = stage + (size_t)slot * HSTAGE_ELEMS;
+        if (lane == 0) {
+          mbar_expect_tx(&full[slot], seg * (uint32_t)(ncols + 1));
+          tma_bulk_g2s(dst + HB * HROWS, v + r0, seg, &full[slot]);
+        }
+        __syncwarp();
+        if (src) tma_bulk_g2s(dst + lane * HROWS, src + r0, seg, &full[slot]);
       }
     }
     return;
@@ -144,76 +160,84 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
 
   // ---- consumers
   const int lr = tid & (HROWS - 1), cg = tid >> 6, lane = tid & 31, warp = tid >> 5;
-  int nq = ncols - cg * 8;
-  nq = nq < 0 ? 0 : (nq > 8 ? 8 : nq);
-  cplx vc[8], accz[8];
+  int gs = 0;
+  for (int wi = 0; wi < nwork; ++wi) {
+    const int q0 = panel ? Jw[wi] * HB : 0;
+    const int c0 = panel ? i + 1 : i + 1 + Jw[wi] * HB;
+    const int ncols = panel ? ((2 * k - q0 < HB) ? 2 * k - q0 : HB) : ((N - c0 < HB) ? N - c0 : HB);
+    const int nst = (N - c0 + HROWS - 1) / HROWS;
+    int nq = ncols - cg * 8;
+    nq = nq < 0 ? 0 : (nq > 8 ? 8 : nq);
+    cplx vc[8], accz[8];
 #pragma unroll
-  for (int q = 0; q < 8; ++q) {
-    accz[q] = mkc(0.0, 0.0);
-    vc[q] = (q < nq && !panel) ? v[c0 + cg * 8 + q] : mkc(0.0, 0.0);
-  }
-  cplx* Prow = P + (c * nJmax + J) * (int64_t)N;
-  for (int s = 0; s < nst; ++s) {
-    const int slot = s % HSTAGES;
-    const cplx* st = stage + (size_t)slot * HSTAGE_ELEMS;
-    const int r = c0 + s * HROWS + lr;
-    mbar_wait(&full[slot], (s / HSTAGES) & 1);
-    cplx yr = mkc(0.0, 0.0);
-    if (r < N) {
-      const cplx vr = st[HB * HROWS + lr];
-      if (panel) {
-#pragma unroll
-        for (int q = 0; q < 8; ++q)
-          if (q < nq) cfmac(accz[q], st[(cg * 8 + q) * HROWS + lr], vr);
-      } else if (s > 0) {
-        if (nq == 8) {
-          cplx a[8];
-#pragma unroll
-          for (int q = 0; q < 8; ++q) a[q] = st[(cg * 8 + q) * HROWS + lr];
-#pragma unroll
-          for (int q = 0; q < 8; ++q) { cfma(yr, a[q], vc[q]); cfmac(accz[q], a[q], vr); }
-        } else {
+    for (int q = 0; q < 8; ++q) {
+      accz[q] = mkc(0.0, 0.0);
+      vc[q] = (q < nq && !panel) ? v[c0 + cg * 8 + q] : mkc(0.0, 0.0);
+    }
+    cplx* Prow = P + (c * nJmax + Jw[wi]) * (int64_t)N;
+    for (int s = 0; s < nst; ++s, ++gs) {
+      const int slot = gs % HSTAGES;
+      const cplx* st = stage + (size_t)slot * HSTAGE_ELEMS;
+      const int r = c0 + s * HROWS + lr;
+      mbar_wait(&full[slot], (gs / HSTAGES) & 1);
+      cplx yr = mkc(0.0, 0.0);
+      if (r < N) {
+        const cplx vr = st[HB * HROWS + lr];
+        if (panel) {
 #pragma unroll
           for (int q = 0; q < 8; ++q)
-            if (q < nq) { const cplx a = st[(cg * 8 + q) * HROWS + lr]; cfma(yr, a, vc[q]); cfmac(accz[q], a, vr); }
-        }
-      } else {
-        // first stage: holds the diagonal block (upper triangle is not part of the matrix)
+            if (q < nq) cfmac(accz[q], st[(cg * 8 + q) * HROWS + lr], vr);
+        } else if (s > 0) {
+          if (nq == 8) {
+            cplx a[8];
 #pragma unroll
-        for (int q = 0; q < 8; ++q)
-          if (q < nq) {
-            const int col = c0 + cg * 8 + q;
-            const cplx a = st[(cg * 8 + q) * HROWS + lr];
-            if (r > col) { cfma(yr, a, vc[q]); cfmac(accz[q], a, vr); }
-            else if (r == col) { yr.x = fma(a.x, vc[q].x, yr.x); yr.y = fma(a.x, vc[q].y, yr.y); }
+            for (int q = 0; q < 8; ++q) a[q] = st[(cg * 8 + q) * HROWS + lr];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) { cfma(yr, a[q], vc[q]); cfmac(accz[q], a[q], vr); }
+          } else {
+#pragma unroll
+            for (int q = 0; q < 8; ++q)
+              if (q < nq) { const cplx a = st[(cg * 8 + q) * HROWS + lr]; cfma(yr, a, vc[q]); cfmac(accz[q], a, vr); }
           }
+        } else {
+          // first stage: holds the diagonal block (upper triangle is not part of the matrix)
+#pragma unroll
+          for (int q = 0; q < 8; ++q)
+            if (q < nq) {
+              const int col = c0 + cg * 8 + q;
+              const cplx a = st[(cg * 8 + q) * HROWS + lr];
+              if (r > col) { cfma(yr, a, vc[q]); cfmac(accz[q], a, vr); }
+              else if (r == col) { yr.x = fma(a.x, vc[q].x, yr.x); yr.y = fma(a.x, vc[q].y, yr.y); }
+            }
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[slot]);          // this warp is done with the stage
+      if (panel) continue;                               // no row part
+      cplx* yb = ysm + (gs & 1) * 4 * HROWS;
+      yb[cg * HROWS + lr] = yr;
+      asm volatile("bar.sync 1, 256;" ::: "memory");     // consumers only
+      if (tid < HROWS && r < N) {
+        cplx t = cadd(cadd(yb[tid], yb[HROWS + tid]), cadd(yb[2 * HROWS + tid], yb[3 * HROWS + tid]));
+        Prow[r] = t;
       }
     }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(&empty[slot]);          // this warp is done with the stage
-    if (panel) continue;                               // no row part
-    cplx* yb = ysm + (s & 1) * 4 * HROWS;
-    yb[cg * HROWS + lr] = yr;
-    asm volatile("bar.sync 1, 256;" ::: "memory");     // consumers only
-    if (tid < HROWS && r < N) {
-      cplx t = cadd(cadd(yb[tid], yb[HROWS + tid]), cadd(yb[2 * HROWS + tid], yb[3 * HROWS + tid]));
-      Prow[r] = t;
-    }
-  }
-  // column part: reduce over the 64 rows (2 warps per column group)
-  asm volatile("bar.sync 1, 256;" ::: "memory");
-  cplx* zsm = ysm;   // [8 warps][8]
+    // column part: reduce over the 64 rows (2 warps per column group)
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    cplx* zsm = ysm;   // [8 warps][8]
 #pragma unroll
-  for (int q = 0; q < 8; ++q) {
-    const cplx z = warp_sum(accz[q]);
-    if (lane == 0) zsm[warp * 8 + q] = z;
-  }
-  asm volatile("bar.sync 1, 256;" ::: "memory");
-  if (tid < HB && tid < ncols) {
-    const int g = tid >> 3, q = tid & 7;
-    const cplx z = cadd(zsm[(2 * g) * 8 + q], zsm[(2 * g + 1) * 8 + q]);
-    if (panel) pqg[c * (2 * NB) + q0 + tid] = z;
-    else zpart[c * N + c0 + tid] = z;
+    for (int q = 0; q < 8; ++q) {
+      const cplx z = warp_sum(accz[q]);
+      if (lane == 0) zsm[warp * 8 + q] = z;
+    }
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    if (tid < HB && tid < ncols) {
+      const int g = tid >> 3, q = tid & 7;
+      const cplx z = cadd(zsm[(2 * g) * 8 + q], zsm[(2 * g + 1) * 8 + q]);
+      if (panel) pqg[c * (2 * NB) + q0 + tid] = z;
+      else zpart[c * N + c0 + tid] = z;
+    }
+    asm volatile("bar.sync 1, 256;" ::: "memory");     // zsm is ysm: done before the next block column writes it
   }
 }
 
@@ -734,7 +758,7 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
       const int nJ = (n + HB - 1) / HB;
       const int npb = (2 * (i - p) + HB - 1) / HB;   // panel blocks: the 2k dot products for k_colw
       be_prof_begin(ctx, PK_HEMV);
-      k_hemv<<<(unsigned)(cnt * (nJ + npb)), HEMV_THREADS, HEMV_SMEM, st>>>(s.Bw, s.P, s.zpart, N, i, nJ, nJmax, s.Wp,
+      k_hemv<<<(unsigned)(cnt * ((nJ + 1) / 2 + npb)), HEMV_THREADS, HEMV_SMEM, st>>>(s.Bw, s.P, s.zpart, N, i, nJ, nJmax, s.Wp,
                                                                              s.pq, p, npb);
       // algorithmic traffic: the lower triangle once, v in, y out; 8 real flops per complex fma, 2 per element
       be_prof_end(ctx, PK_HEMV, (double)cnt * (0.5 * n * (n + 1.0) + 2.0 * n) * 16.0, (double)cnt * 8.0 * n * n);
@@ -779,7 +803,7 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
       // (subspace iteration inside a cluster): several solves in a row with the SAME shift collapse
       // the vectors of a numerically degenerate cluster onto its few nearest eigen-directions
       // (measured: cond 6e10 for the 400-fold +-1 of the projected spin operator).
-      for (int it = 0; it < 4; ++it) {
+      for (int it = 0; it < 3; ++it) {
         be_prof_begin(ctx, PK_INVIT);
         k_invit<<<(unsigned)(cnt * nvb), 128, sh, st>>>(s.d, s.e, E, s.tnorm, s.fa, s.fb, s.fc, s.fp, s.blk, s.blo, s.bhi,
                                                         s.bcl, s.Z, N, nv, nvb, it > 0 ? 1 : 0, 1);
