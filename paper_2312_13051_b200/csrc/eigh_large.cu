@@ -599,26 +599,45 @@ __global__ void k_extract_v(const cplx* __restrict__ Bw, const cplx* __restrict_
   if (threadIdx.x < kb) tauc[c * NBT + threadIdx.x] = cconj(tau[c * N + p + threadIdx.x]);
 }
 
-// zlarft (forward, columnwise) from G = V^H V: T(j,j) = tau_j, T(0:j, j) = -tau_j T(0:j,0:j) G(0:j, j).
-// One CTA of NBT threads per matrix (thread = row of T); T column-major, leading dimension NBT,
-// built in place in global memory (L1/L2 resident, 256 KB).
-__global__ void __launch_bounds__(NBT) k_larft(const cplx* __restrict__ G, const cplx* __restrict__ tauc,
-                                               cplx* __restrict__ T, int kb) {
+// zlarft (forward, columnwise) from G = V^H V by recursive doubling: for a block [T11 T12; 0 T22]
+// of two finished halves, T12 = -T11 G12 T22.  Starting from T_jj = tau_j the block size doubles
+// log2(NBT) times; every level is two small matrix products done by all 1024 threads (element per
+// thread), instead of NBT dependent column solves by NBT threads.  T, G column-major, ld NBT;
+// tmp holds T11 G12.  Rows / columns >= kb are zero (G is not defined there).
+__global__ void __launch_bounds__(1024) k_larft(const cplx* __restrict__ G, const cplx* __restrict__ tauc,
+                                                cplx* __restrict__ T, cplx* __restrict__ tmp, int kb) {
   const int64_t c = blockIdx.x;
-  const int row = threadIdx.x;
   const cplx* g = G + c * NBT * NBT;
   cplx* t = T + c * NBT * NBT;
-  for (int j = 0; j < NBT; ++j) t[row + j * NBT] = mkc(0.0, 0.0);
+  cplx* w = tmp + c * NBT * NBT;
+  const int tid = threadIdx.x;
+  for (int idx = tid; idx < NBT * NBT; idx += 1024) {
+    const int r = idx % NBT, cc = idx / NBT;
+    t[idx] = (r == cc && r < kb) ? tauc[c * NBT + r] : mkc(0.0, 0.0);
+  }
   __syncthreads();
-  for (int j = 0; j < kb; ++j) {
-    const cplx tj = tauc[c * NBT + j];
-    if (row < j) {
+  for (int sz = 1; sz < NBT; sz <<= 1) {
+    // tmp[r][cc] = sum_q T11[r][q] G[q][cc]: r, q in the first half (q >= r), cc in the second half
+    const int per = sz * sz, pairs = NBT / (2 * sz);
+    for (int idx = tid; idx < per * pairs; idx += 1024) {
+      const int b0 = (idx / per) * 2 * sz, e = idx % per;
+      const int r = b0 + e % sz, cc = b0 + sz + e / sz;
       cplx acc = mkc(0.0, 0.0);
-      for (int q = row; q < j; ++q) cfma(acc, t[row + q * NBT], g[q + j * NBT]);   // own row only
-      t[row + j * NBT] = cmul(mkc(-tj.x, -tj.y), acc);
-    } else if (row == j) {
-      t[j + j * NBT] = tj;
+      if (cc < kb)
+        for (int q = r; q < b0 + sz; ++q) cfma(acc, t[r + q * NBT], g[q + cc * NBT]);
+      w[r + cc * NBT] = acc;
     }
+    __syncthreads();
+    // T12[r][cc] = -sum_q tmp[r][q] T22[q][cc]: q, cc in the second half (q <= cc)
+    for (int idx = tid; idx < per * pairs; idx += 1024) {
+      const int b0 = (idx / per) * 2 * sz, e = idx % per;
+      const int r = b0 + e % sz, cc = b0 + sz + e / sz;
+      cplx acc = mkc(0.0, 0.0);
+      if (cc < kb)
+        for (int q = b0 + sz; q <= cc; ++q) cfma(acc, w[r + q * NBT], t[q + cc * NBT]);
+      t[r + cc * NBT] = mkc(-acc.x, -acc.y);
+    }
+    __syncthreads();
   }
 }
 
@@ -667,7 +686,7 @@ __global__ void k_x2u(const cplx* __restrict__ X, cplx* __restrict__ U, int N, i
 
 // scratch layout for ``cnt`` matrices
 struct EighScratch {
-  cplx *Bw, *Wp, *P, *zpart, *tau, *Vb, *T, *G, *tauc, *Y, *Y2, *pq;
+  cplx *Bw, *Wp, *P, *zpart, *tau, *Vb, *T, *G, *tauc, *Y, *Y2, *pq, *Ttmp;
   double *d, *e, *tnorm, *Z, *fa, *fb, *fc;
   unsigned char* fp;
   int* blk;
@@ -693,6 +712,7 @@ static size_t eigh_large_carve(char* base, int64_t cnt, int N, int nv, EighScrat
   cplx* Y = (cplx*)take(cnt * (size_t)NBT * (nv > 0 ? nv : 1) * sizeof(cplx));
   cplx* Y2 = (cplx*)take(cnt * (size_t)NBT * (nv > 0 ? nv : 1) * sizeof(cplx));
   cplx* pq = (cplx*)take(cnt * (size_t)2 * NB * sizeof(cplx));
+  cplx* Ttmp = (cplx*)take(cnt * (size_t)NBT * NBT * sizeof(cplx));
   double* d = (double*)take(cnt * (size_t)N * sizeof(double));
   double* e = (double*)take(cnt * (size_t)N * sizeof(double));
   double* tn = (double*)take(cnt * sizeof(double));
@@ -706,7 +726,7 @@ static size_t eigh_large_carve(char* base, int64_t cnt, int N, int nv, EighScrat
   double* bhi = (double*)take(cnt * (size_t)N * sizeof(double));
   int* bcl = (int*)take(cnt * (size_t)N * sizeof(int));
   void* orth = take(be_cluster_orth_scratch_bytes(cnt, N, nv));
-  if (s) { *s = EighScratch{Bw, Wp, P, zp, tau, Vb, T, G, tauc, Y, Y2, pq, d, e, tn, Z, fa, fb, fc, fp, blk, blo, bhi, bcl, orth}; }
+  if (s) { *s = EighScratch{Bw, Wp, P, zp, tau, Vb, T, G, tauc, Y, Y2, pq, Ttmp, d, e, tn, Z, fa, fb, fc, fp, blk, blo, bhi, bcl, orth}; }
   return off;
 }
 
@@ -833,7 +853,7 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
     ZgemmParams gg = zgemm_simple(kb, kb, rows, s.Vb, N, (int64_t)N * NBT, s.Vb, N, (int64_t)N * NBT,
                                   s.G, NBT, NBT * NBT, cnt);
     BE_TRY(be_zgemm(ctx, BE_OP_C, BE_OP_N, gg));
-    k_larft<<<(unsigned)cnt, NBT, 0, st>>>(s.G, s.tauc, s.T, kb);
+    k_larft<<<(unsigned)cnt, 1024, 0, st>>>(s.G, s.tauc, s.T, s.Ttmp, kb);
     LAUNCH_CHECK();
     // Y = V^H X[p+1:, :]
     ZgemmParams gy = zgemm_simple(kb, nv, rows, s.Vb, N, (int64_t)N * NBT, X + p + 1, N, (int64_t)N * nv,
