@@ -117,13 +117,14 @@ __device__ __forceinline__ void givens(cplx a, cplx b, double& c, cplx& s) {
   if (nb2 == 0.0) { c = 1.0; s = mkc(0.0, 0.0); return; }
   const double na2 = cabs2(a);
   if (na2 == 0.0) { c = 0.0; const double nb = sqrt(nb2); s = mkc(b.x / nb, -b.y / nb); return; }
-  const double na = sqrt(na2), nrm = sqrt(na2 + nb2);
-  c = na / nrm;
-  const cplx ph = mkc(a.x / na, a.y / na);          // a / |a|
-  s = cscale(1.0 / nrm, cmulc(b, ph));              // (a/|a|) conj(b) / nrm
+  // the rotation sits on the sequential chain of the sweep: two reciprocal square roots instead of
+  // two square roots and three divisions
+  const double ia = rsqrt(na2), ir = rsqrt(na2 + nb2);
+  c = na2 * ia * ir;                                  // |a| / sqrt(|a|^2 + |b|^2)
+  s = cscale(ia * ir, cmulc(b, a));                   // (a / |a|) conj(b) / sqrt(|a|^2 + |b|^2)
 }
 
-constexpr int QR_MAXOWN = 8;   // columns / rows owned per thread: m <= 8 * blockDim
+constexpr int QR_MAXOWN = 4;   // columns / rows owned per thread: m <= 4 * blockDim
 
 // Explicit single-shift QR on the upper Hessenberg matrix H (column-major m x m), eigenvalues only.
 __global__ void k_hqr(cplx* __restrict__ W, int m, cplx* __restrict__ lam, int* __restrict__ fail) {
@@ -136,6 +137,7 @@ __global__ void k_hqr(cplx* __restrict__ W, int m, cplx* __restrict__ lam, int* 
   cplx* H = W + blockIdx.x * (int64_t)m * m;
   cplx* out = lam + blockIdx.x * (int64_t)m;
   const int tid = threadIdx.x, nt = blockDim.x;
+  const int nl = (m + QR_MAXOWN - 1) / QR_MAXOWN <= 64 ? (nt < 64 ? nt : 64) : (nt < 128 ? nt : (m <= QR_MAXOWN * 128 ? 128 : nt));
   const double eps = DBL_EPSILON;
   int hi = m - 1, its = 0, nfail = 0;
   while (hi >= 0) {
@@ -186,63 +188,94 @@ __global__ void k_hqr(cplx* __restrict__ W, int m, cplx* __restrict__ lam, int* 
       continue;
     }
     const cplx sig = s_sig;
-    // ---- left phase: R = Q^H (H - sig I); thread owns columns j = l + tid + q*nt
-    cplx carry[QR_MAXOWN];
+    // ---- left phase: R = Q^H (H - sig I).  Thread t < nl owns the QR_MAXOWN CONSECUTIVE columns
+    // l + 4t .. l + 4t + 3.  The rotations form a sequential chain (G_s needs column s after G_{s-1});
+    // with consecutive columns per thread the owner of a round generates its 4 rotations back to back
+    // from registers and publishes them together: one barrier per 4 rotations instead of one per
+    // rotation.  Only nl <= 128 threads take part (the barrier spans 4 warps).
+    if (tid < nl) {
+      const int j0 = l + QR_MAXOWN * tid;
+      cplx carry[QR_MAXOWN];
 #pragma unroll
-    for (int q = 0; q < QR_MAXOWN; ++q) {
-      const int j = l + tid + q * nt;
-      if (j <= hi) {
-        cplx x = H[l + (int64_t)j * m];
-        if (j == l) x = csub(x, sig);
-        carry[q] = x;
+      for (int u = 0; u < QR_MAXOWN; ++u) {
+        const int j = j0 + u;
+        carry[u] = mkc(0.0, 0.0);
+        if (j <= hi) { carry[u] = H[l + (int64_t)j * m]; if (j == l) carry[u] = csub(carry[u], sig); }
       }
-    }
-    for (int s = l; s < hi; ++s) {
-      {
-        const int rel = s - l;
-        if (rel % nt == tid) {
-          const int q = rel / nt;
-          cplx a = mkc(0.0, 0.0);
+      const int nrounds = (hi - l + QR_MAXOWN - 1) / QR_MAXOWN;
+      for (int r = 0; r < nrounds; ++r) {            // every thread runs every round: the barrier is warp-aligned
+        const int sb = l + QR_MAXOWN * r;            // rotations sb .. sb+3 (those < hi)
+        // rows sb+1 .. sb+4 of the owned columns (H - sig I); rows ahead of the sweep are not written by it
+        cplx Y[QR_MAXOWN][QR_MAXOWN];   // [rotation v][column u]
 #pragma unroll
-          for (int qq = 0; qq < QR_MAXOWN; ++qq) if (qq == q) a = carry[qq];
-          const cplx b = H[(s + 1) + (int64_t)s * m];
-          double c_; cplx s_;
-          givens(a, b, c_, s_);
-          cs[rel] = c_; sn[rel] = s_;
+        for (int v = 0; v < QR_MAXOWN; ++v)
+#pragma unroll
+          for (int u = 0; u < QR_MAXOWN; ++u) {
+            const int row = sb + 1 + v, j = j0 + u;
+            cplx y = mkc(0.0, 0.0);
+            if (r <= tid && row <= hi && j <= hi && j + 1 >= row) { y = H[row + (int64_t)j * m]; if (row == j) y = csub(y, sig); }
+            Y[v][u] = y;
+          }
+        if (r == tid) {
+          // owner: generate G_s from the own column s = j0 + v, apply it to the own columns right away
+#pragma unroll
+          for (int v = 0; v < QR_MAXOWN; ++v) {
+            const int sidx = sb + v;
+            if (sidx < hi) {
+              double c_; cplx s_;
+              givens(carry[v], Y[v][v], c_, s_);
+              cs[sidx - l] = c_; sn[sidx - l] = s_;
+#pragma unroll
+              for (int u = 0; u < QR_MAXOWN; ++u)
+                if (u >= v && j0 + u <= hi) {
+                  const cplx x = carry[u], yv = Y[v][u];
+                  cplx top = cscale(c_, x); cfma(top, s_, yv);
+                  cplx bot = cscale(c_, yv); cfms(bot, cconj(s_), x);
+                  H[sidx + (int64_t)(j0 + u) * m] = top;
+                  carry[u] = bot;
+                }
+            }
+          }
+        }
+        asm volatile("bar.sync 1, %0;" ::"r"(nl) : "memory");   // rotations of round r are published
+        if (r < tid) {
+#pragma unroll
+          for (int v = 0; v < QR_MAXOWN; ++v) {
+            const int sidx = sb + v;
+            if (sidx < hi) {
+              const double c_ = cs[sidx - l];
+              const cplx s_ = sn[sidx - l];
+#pragma unroll
+              for (int u = 0; u < QR_MAXOWN; ++u)
+                if (j0 + u <= hi) {
+                  const cplx x = carry[u], yv = Y[v][u];
+                  cplx top = cscale(c_, x); cfma(top, s_, yv);
+                  cplx bot = cscale(c_, yv); cfms(bot, cconj(s_), x);
+                  H[sidx + (int64_t)(j0 + u) * m] = top;
+                  carry[u] = bot;
+                }
+            }
+          }
         }
       }
-      __syncthreads();
-      const double c_ = cs[s - l];
-      const cplx s_ = sn[s - l];
 #pragma unroll
-      for (int q = 0; q < QR_MAXOWN; ++q) {
-        const int j = l + tid + q * nt;
-        if (j >= s && j <= hi) {
-          const cplx x = carry[q];
-          cplx yv = H[(s + 1) + (int64_t)j * m];
-          if (j == s + 1) yv = csub(yv, sig);
-          // new row s: c x + s y ; new row s+1: -conj(s) x + c y
-          cplx top = cscale(c_, x); cfma(top, s_, yv);
-          cplx bot = cscale(c_, yv); cfms(bot, cconj(s_), x);
-          H[s + (int64_t)j * m] = top;
-          carry[q] = bot;
-        }
-      }
-    }
-#pragma unroll
-    for (int q = 0; q < QR_MAXOWN; ++q) {
-      const int j = l + tid + q * nt;
-      if (j == hi) H[hi + (int64_t)hi * m] = carry[q];
+      for (int u = 0; u < QR_MAXOWN; ++u)
+        if (j0 + u == hi) H[hi + (int64_t)hi * m] = carry[u];
     }
     __syncthreads();
     // ---- right phase: H = R Q + sig I; thread owns rows i = l + tid + q*nt, walks along the row
     for (int i = l + tid; i <= hi; i += nt) {
       const int sstart = (i - 1 > l) ? i - 1 : l;
       cplx x = (sstart == i - 1) ? mkc(0.0, 0.0) : H[i + (int64_t)sstart * m];   // R[i][i-1] = 0
+      // the row is walked left to right; its elements are prefetched two columns ahead
+      cplx y0 = (sstart + 1 <= hi) ? H[i + (int64_t)(sstart + 1) * m] : mkc(0.0, 0.0);
+      cplx y1 = (sstart + 2 <= hi) ? H[i + (int64_t)(sstart + 2) * m] : mkc(0.0, 0.0);
       for (int s = sstart; s < hi; ++s) {
         const double c_ = cs[s - l];
         const cplx s_ = sn[s - l];
-        const cplx yv = H[i + (int64_t)(s + 1) * m];
+        const cplx yv = y0;
+        y0 = y1;
+        if (s + 3 <= hi) y1 = H[i + (int64_t)(s + 3) * m];
         // col s: c x + conj(s) y ; col s+1: -s x + c y
         cplx ns = cscale(c_, x); cfma(ns, cconj(s_), yv);
         cplx n1 = cscale(c_, yv); cfms(n1, s_, x);
@@ -294,7 +327,7 @@ int be_eigenvalues_general(be_ctx* ctx, cplx* W, int64_t cnt, int m, cplx* lam, 
     return (int)cudaGetLastError();
   }
   int nt = ((m + 31) / 32) * 32;
-  if (nt > 256) nt = 256;
+  if (nt > 256) nt = (m > QR_MAXOWN * 256) ? 512 : 256;
   if (m > QR_MAXOWN * nt) return BE_ERR_UNSUPPORTED;
   const size_t sh1 = 3 * (size_t)m * sizeof(cplx);
   be_prof_begin(ctx, PK_HESS);
