@@ -113,6 +113,7 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
       // X^T conj(SX) is S_red when read row-major (S_red is Hermitian)
       ZgemmParams g = zgemm_simple(m, m, N, X, N, (int64_t)N * m, SX, N, (int64_t)N * m,
                                    Sred, m, (int64_t)m * m, cnt);
+      g.lower = 1;   // the eigensolver reads only the lower triangle of the column-major buffer
       BE_TRY(be_zgemm(ctx, BE_OP_T, BE_OP_J, g));
     }
     {

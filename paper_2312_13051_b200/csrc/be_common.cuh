@@ -116,6 +116,10 @@ struct ZgemmParams {
   int phi_at;         // inner index of the link that crosses the zone boundary (default inner-1)
   cplx alpha, beta;
   int lower;          // 1: skip tiles strictly above the diagonal (C lower triangle, tile granular)
+  // optional second K segment: for k >= ksplit the operands are read from A2 / B2 at k - ksplit (same
+  // leading dimensions, own outer strides); ksplit = 0: single segment.  Used by the rank-2k update
+  // A22 -= [V W] [W V]^H without packing the panels.
+  const cplx* A2; const cplx* B2; int64_t sA2o, sB2o; int ksplit;
 };
 int be_zgemm(be_ctx* ctx, int opA, int opB, const ZgemmParams& p);
 static inline ZgemmParams zgemm_simple(int M, int N, int K, const cplx* A, int lda, int64_t sA,
@@ -129,6 +133,7 @@ static inline ZgemmParams zgemm_simple(int M, int N, int K, const cplx* A, int l
   p.inner = 1; p.batch = batch;
   p.ringB = 0; p.phiB = nullptr; p.phi_at = -1;
   p.alpha = mkc(1.0, 0.0); p.beta = mkc(0.0, 0.0); p.lower = 0;
+  p.A2 = nullptr; p.B2 = nullptr; p.sA2o = p.sB2o = 0; p.ksplit = 0;
   return p;
 }
 

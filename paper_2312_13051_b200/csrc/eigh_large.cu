@@ -641,24 +641,6 @@ __global__ void __launch_bounds__(1024) k_larft(const cplx* __restrict__ G, cons
   }
 }
 
-// her2k operands for one panel: XA = [V | W], XB = [W | V] restricted to rows q..N-1 (ld N), so that
-// B22 -= XA XB^H is a single rank-2kb update (C read and written once).
-__global__ void k_pack_vw(const cplx* __restrict__ Bw, const cplx* __restrict__ Wp, cplx* __restrict__ Vb,
-                          int N, int p, int q, int kb) {
-  const int64_t c = blockIdx.x;
-  const cplx* B = Bw + c * (int64_t)N * N;
-  const cplx* W = Wp + c * (int64_t)N * NB;
-  cplx* XA = Vb + c * (int64_t)N * NBT;
-  cplx* XB = XA + (int64_t)N * 2 * NB;
-  const int rows = N - q;
-  for (int idx = threadIdx.x; idx < rows * kb; idx += blockDim.x) {
-    const int cc = idx / rows, r = q + idx % rows;
-    const cplx v = B[r + (int64_t)(p + cc) * N], w = W[r + (int64_t)cc * N];
-    XA[(r - q) + (int64_t)cc * N] = v;        XA[(r - q) + (int64_t)(kb + cc) * N] = w;
-    XB[(r - q) + (int64_t)cc * N] = w;        XB[(r - q) + (int64_t)(kb + cc) * N] = v;
-  }
-}
-
 __global__ void k_set_info(int* info, int64_t cnt) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i < cnt) info[i] = 0;
@@ -789,12 +771,13 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
     const int q = pend, kb = pend - p;
     if (q < N) {
       const int n2 = N - q;
-      // B[q:, q:] -= [V W] [W V]^H  (lower tiles): one rank-2kb update
-      k_pack_vw<<<(unsigned)cnt, 256, 0, st>>>(s.Bw, s.Wp, s.Vb, N, p, q, kb);
-      LAUNCH_CHECK();
-      ZgemmParams g = zgemm_simple(n2, n2, 2 * kb, s.Vb, N, (int64_t)N * NBT,
-                                   s.Vb + (int64_t)N * 2 * NB, N, (int64_t)N * NBT,
+      // B[q:, q:] -= [V W] [W V]^H  (lower tiles): one rank-2kb update, the two K segments read in place
+      ZgemmParams g = zgemm_simple(n2, n2, 2 * kb, s.Bw + q + (int64_t)p * N, N, (int64_t)N * N,
+                                   s.Wp + q, N, (int64_t)N * NB,
                                    s.Bw + q + (int64_t)q * N, N, (int64_t)N * N, cnt);
+      g.A2 = s.Wp + q; g.sA2o = (int64_t)N * NB;
+      g.B2 = s.Bw + q + (int64_t)p * N; g.sB2o = (int64_t)N * N;
+      g.ksplit = kb;
       g.alpha = mkc(-1.0, 0.0); g.beta = mkc(1.0, 0.0); g.lower = 1;
       BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_C, g));
     }

@@ -174,6 +174,7 @@ int be_chain_product(be_ctx* ctx, const cplx* F, int N, int m, int64_t outer, in
   g.inner = n1; g.batch = outer * n1;
   g.ringB = 1; g.phiB = d_close; g.phi_at = phi_at;
   g.alpha = mkc(1.0, 0.0); g.beta = mkc(0.0, 0.0); g.lower = 0;
+  g.A2 = nullptr; g.B2 = nullptr; g.sA2o = g.sB2o = 0; g.ksplit = 0;
   BE_TRY(be_zgemm(ctx, BE_OP_C, BE_OP_N, g));
   if (n1 == 1) {
     cplx* dst = Wdst ? Wdst : W0;

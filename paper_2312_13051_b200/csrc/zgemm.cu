@@ -30,16 +30,22 @@ __device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b)
                : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
-template <int OPA, int OPB, bool PHI>
+template <int OPA, int OPB, bool PHI, bool SPLIT>
 __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p, int tilesM, int tilesN) {
   extern __shared__ double smem[];
   const int tid = threadIdx.x;
-  const int64_t tiles = (int64_t)tilesM * tilesN;
+  // lower: only the tilesM (tilesM + 1) / 2 tiles on or below the diagonal are launched
+  const int64_t tiles = p.lower ? (int64_t)tilesM * (tilesM + 1) / 2 : (int64_t)tilesM * tilesN;
   const int64_t bidx = blockIdx.x;
   const int64_t b = bidx / tiles;
   const int t = (int)(bidx - b * tiles);
-  const int tm = t % tilesM, tn = t / tilesM;
-  if (p.lower && tn > tm) return;
+  int tm, tn;
+  if (p.lower) {
+    tm = (int)((sqrt(8.0 * t + 1.0) - 1.0) * 0.5);
+    while ((tm + 1) * (tm + 2) / 2 <= t) ++tm;
+    while (tm * (tm + 1) / 2 > t) --tm;
+    tn = t - tm * (tm + 1) / 2;
+  } else { tm = t % tilesM; tn = t / tilesM; }
   const int64_t bo = b / p.inner;
   const int bi = (int)(b - bo * p.inner);
   const cplx* __restrict__ A = p.A + bo * p.sAo + (int64_t)bi * p.sAi;
@@ -49,6 +55,9 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
   const cplx* __restrict__ B = p.B + bo * p.sBo + (int64_t)biB * p.sBi;
   cplx* __restrict__ C = p.C + bo * p.sCo + (int64_t)bi * p.sCi;
   const cplx* __restrict__ phi = (PHI && wrap && p.phiB) ? p.phiB : nullptr;
+  const int ksplit = SPLIT ? p.ksplit : 0;
+  const cplx* __restrict__ A2 = SPLIT ? p.A2 + bo * p.sA2o : nullptr;
+  const cplx* __restrict__ B2 = SPLIT ? p.B2 + bo * p.sB2o : nullptr;
 
   const int m0 = tm * TM, n0 = tn * TN;
   const int M = p.M, N = p.N, K = p.K;
@@ -69,7 +78,11 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
     for (int q = 0; q < 4; ++q) {
       const int i = m0 + ai + q * aqi, k = k0 + ak + q * aqk;
       cplx v = mkc(0.0, 0.0);
-      if (i < M && k < K) v = transA ? A[(int64_t)k + (int64_t)i * p.lda] : A[(int64_t)i + (int64_t)k * p.lda];
+      if (i < M && k < K) {
+        const cplx* Ap = A; int kk = k;
+        if (SPLIT && k >= ksplit) { Ap = A2; kk = k - ksplit; }
+        v = transA ? Ap[(int64_t)kk + (int64_t)i * p.lda] : Ap[(int64_t)i + (int64_t)kk * p.lda];
+      }
       ra[q] = v;
     }
 #pragma unroll
@@ -78,7 +91,9 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
       cplx v = mkc(0.0, 0.0);
       cplx f = mkc(1.0, 0.0);
       if (n < N && k < K) {
-        v = transB ? B[(int64_t)n + (int64_t)k * p.ldb] : B[(int64_t)k + (int64_t)n * p.ldb];
+        const cplx* Bp = B; int kk = k;
+        if (SPLIT && k >= ksplit) { Bp = B2; kk = k - ksplit; }
+        v = transB ? Bp[(int64_t)n + (int64_t)kk * p.ldb] : Bp[(int64_t)kk + (int64_t)n * p.ldb];
         if (PHI && phi) f = phi[k];
       }
       rb[q] = v;          // no arithmetic on loaded values here: the loads stay in flight during the
@@ -115,6 +130,21 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
 #pragma unroll
     for (int c = 0; c < 2; ++c) { accr[a][c][0] = accr[a][c][1] = 0.0; acci[a][c][0] = acci[a][c][1] = 0.0; }
 
+  const bool has_beta = (p.beta.x != 0.0 || p.beta.y != 0.0);
+  auto cload = [&](int half, cplx (&dst)[2][2][2]) {
+#pragma unroll
+    for (int m2 = 0; m2 < 2; ++m2) {
+      const int mb = half * 2 + m2;
+      const int row = m0 + wm * 32 + mb * 8 + g;
+#pragma unroll
+      for (int nb = 0; nb < 2; ++nb)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int col = n0 + wn * 16 + nb * 8 + 2 * tg + e;
+          dst[m2][nb][e] = (row < M && col < N) ? C[(int64_t)row + (int64_t)col * p.ldc] : mkc(0.0, 0.0);
+        }
+    }
+  };
   const int KT = (K + TK - 1) / TK;
   gload(0);
   sstore(0);
@@ -166,25 +196,13 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
     }
   }
 
-  const bool has_beta = (p.beta.x != 0.0 || p.beta.y != 0.0);
-  // epilogue in two halves of 8 elements: all loads of C first (independent, in flight together),
-  // then the stores -- a load/store per element in program order would serialize 16 round trips
+  // epilogue in two halves of 8 elements: all loads of C first (independent, in flight together), then the stores -- a load/store per element
+  // in program order would serialize 16 round trips
 #pragma unroll
   for (int half = 0; half < 2; ++half) {
     cplx cold[2][2][2];
     if (has_beta) {
-#pragma unroll
-      for (int m2 = 0; m2 < 2; ++m2) {
-        const int mb = half * 2 + m2;
-        const int row = m0 + wm * 32 + mb * 8 + g;
-#pragma unroll
-        for (int nb = 0; nb < 2; ++nb)
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            const int col = n0 + wn * 16 + nb * 8 + 2 * tg + e;
-            cold[m2][nb][e] = (row < M && col < N) ? C[(int64_t)row + (int64_t)col * p.ldc] : mkc(0.0, 0.0);
-          }
-      }
+      cload(half, cold);
     }
 #pragma unroll
     for (int m2 = 0; m2 < 2; ++m2) {
@@ -204,19 +222,20 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
   }
 }
 
-template <int OPA, int OPB, bool PHI>
+template <int OPA, int OPB, bool PHI, bool SPLIT>
 int launch(be_ctx* ctx, const ZgemmParams& p) {
   const int tilesM = (p.M + TM - 1) / TM, tilesN = (p.N + TN - 1) / TN;
-  const int64_t blocks = p.batch * tilesM * tilesN;
+  if (p.lower && p.M != p.N) return BE_ERR_SHAPE;
+  const int64_t blocks = p.batch * (p.lower ? (int64_t)tilesM * (tilesM + 1) / 2 : (int64_t)tilesM * tilesN);
   if (blocks <= 0) return BE_OK;
   if (blocks > 0x7fffffffLL) return BE_ERR_SHAPE;
   static bool attr_done = false;  // per instantiation; idempotent
   if (!attr_done) {
-    BE_CUDA(cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, PHI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM_BYTES));
+    BE_CUDA(cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, PHI, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM_BYTES));
     attr_done = true;
   }
   be_prof_begin(ctx, PK_GEMM);
-  zgemm_kernel<OPA, OPB, PHI><<<(unsigned)blocks, NTHREADS, SM_BYTES, ctx->stream>>>(p, tilesM, tilesN);
+  zgemm_kernel<OPA, OPB, PHI, SPLIT><<<(unsigned)blocks, NTHREADS, SM_BYTES, ctx->stream>>>(p, tilesM, tilesN);
   {
     const double tri = p.lower ? 0.5 : 1.0;
     const double fl = 8.0 * p.M * (double)p.N * p.K * (double)p.batch * tri;
@@ -232,8 +251,12 @@ int launch(be_ctx* ctx, const ZgemmParams& p) {
 int be_zgemm(be_ctx* ctx, int opA, int opB, const ZgemmParams& p) {
   if (p.M <= 0 || p.N <= 0 || p.batch <= 0) return BE_OK;
   if (p.phiB && (opA != BE_OP_C || opB != BE_OP_N || !p.ringB)) return BE_ERR_UNSUPPORTED;   // closing phase: link GEMM only
-  if (p.phiB && p.ringB) return launch<BE_OP_C, BE_OP_N, true>(ctx, p);
-#define CASE(a, b) if (opA == a && opB == b) return launch<a, b, false>(ctx, p);
+  if (p.phiB && p.ringB) return launch<BE_OP_C, BE_OP_N, true, false>(ctx, p);
+  if (p.ksplit > 0) {   // two K segments: the rank-2k update only
+    if (opA != BE_OP_N || opB != BE_OP_C || !p.A2 || !p.B2) return BE_ERR_UNSUPPORTED;
+    return launch<BE_OP_N, BE_OP_C, false, true>(ctx, p);
+  }
+#define CASE(a, b) if (opA == a && opB == b) return launch<a, b, false, false>(ctx, p);
   CASE(BE_OP_N, BE_OP_N) CASE(BE_OP_N, BE_OP_C) CASE(BE_OP_C, BE_OP_N) CASE(BE_OP_N, BE_OP_T)
   CASE(BE_OP_T, BE_OP_N) CASE(BE_OP_J, BE_OP_N) CASE(BE_OP_N, BE_OP_J) CASE(BE_OP_C, BE_OP_C) CASE(BE_OP_T, BE_OP_J)
 #undef CASE
