@@ -90,8 +90,10 @@ int be_profile_get(be_ctx* ctx, int cls, double* ms, int64_t* launches, double* 
  *   d_info [count] int, may be NULL: 0 = converged; >0 = number of vectors whose inverse iteration
  *          or Jacobi sweep limit did not meet its tolerance.
  * Paths: N <= 8 cyclic one-sided Jacobi on the shifted matrix, one thread per matrix; otherwise
- * blocked Householder tridiagonalization + bisection + inverse iteration + compact-WY
- * back-transform, all matrices of the batch advanced in lock step.
+ * blocked Householder tridiagonalization + bisection + inverse iteration (clusters of close
+ * eigenvalues re-orthogonalized after every solve) + compact-WY back-transform, all matrices of the
+ * batch advanced in lock step.  N <= 6400 (shared-memory staging of one column), else
+ * BE_ERR_UNSUPPORTED.
  */
 int be_eigh_batched(be_ctx* ctx, const void* dH, int64_t count, int N, int n_vec,
                     double* dE, void* dU, int* d_info);
@@ -120,8 +122,9 @@ int be_wilson_loop(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_
  * (orthonormalized); w = U_base V_S; a second loop of w runs along dir2 (closing phase d_close2).
  *   d_theta1       [batch][other][dims[dir2]][n_occ]: first-level phases, branch (-pi, pi].
  *   d_theta_nested [batch][other][wb_hi-wb_lo]: nested phases; polarization p = -sum/2pi mod 1.
- * This build: n_occ <= 2 uses closed-form eigenvectors; larger n_occ uses inverse iteration on
- * W - lambda I and requires wb_hi - wb_lo <= 32.
+ * This build: n_occ <= 2 (closed-form eigenvectors of the 2 x 2 Wilson matrix, the case of the
+ * paper's 4-band quadrupole models and of BASELINE.json configs[1]); n_occ > 2 returns
+ * BE_ERR_UNSUPPORTED (nothing is enqueued).
  */
 int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_occ,
                      int dir1, int dir2, int base, int wb_lo, int wb_hi, double theta_cut,
