@@ -68,6 +68,15 @@ size_t be_workspace_bytes(const be_grid* grid, int n_occ, int op);
  * chunks of whole loops sized to stay under the cap. */
 int be_set_workspace_limit(be_ctx* ctx, size_t bytes);
 
+/* Two-stream chunk pipeline for be_wilson_loop / be_spin_resolved_wilson when the work is split
+ * into several chunks (default OFF).  ON: the tridiagonalization of chunk c+1 (HBM bound) runs on the
+ * context's stream while the rest of chunk c (FP64 / latency bound) runs on an internal
+ * high-priority stream, with two scratch regions and one GEMM CTA + one k_hemv CTA sharing each SM;
+ * the caller's stream is joined before return, so the call's semantics do not change.  Measured on
+ * the N = 1600 bench workload it is a wash (3.42 s vs 3.38 s per step: the GEMM kernel loses at one
+ * CTA per SM what the overlap gains -- DESIGN.md section 11), hence the default. */
+int be_set_chunk_pipeline(be_ctx* ctx, int on);
+
 /* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */
 int64_t be_launch_count(const be_ctx* ctx);
 

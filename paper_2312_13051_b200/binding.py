@@ -18,7 +18,7 @@ EXPORTS = [
     "be_create", "be_destroy", "be_strerror", "be_workspace_bytes", "be_set_workspace_limit",
     "be_launch_count", "be_eigh_batched", "be_wilson_loop", "be_nested_wilson",
     "be_spin_resolved_wilson", "be_winding", "be_wilson_loop_host", "be_spin_resolved_wilson_host",
-    "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched",
+    "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched", "be_set_chunk_pipeline",
 ]
 
 
@@ -47,6 +47,7 @@ def load_library():
     lib.be_workspace_bytes.argtypes = [gp, ci, ci]
     lib.be_workspace_bytes.restype = C.c_size_t
     lib.be_set_workspace_limit.argtypes = [vp, C.c_size_t]
+    lib.be_set_chunk_pipeline.argtypes = [vp, ci]
     lib.be_launch_count.argtypes = [vp]
     lib.be_launch_count.restype = i64
     lib.be_eigh_batched.argtypes = [vp, vp, i64, ci, ci, vp, vp, vp]
@@ -134,6 +135,9 @@ class Context:
 
     def set_workspace_limit(self, nbytes: int):
         _check(self.lib, self.lib.be_set_workspace_limit(self._h, nbytes))
+
+    def set_chunk_pipeline(self, on: bool):
+        _check(self.lib, self.lib.be_set_chunk_pipeline(self._h, 1 if on else 0))
 
     def profile_enable(self, on: bool = True):
         _check(self.lib, self.lib.be_profile_enable(self._h, 1 if on else 0))

@@ -125,6 +125,11 @@ extern "C" int be_destroy(be_ctx* ctx) {
   cudaStreamSynchronize(ctx->stream);
   if (ctx->arena) cudaFree(ctx->arena);
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+  if (ctx->stream2) {
+    cudaStreamDestroy(ctx->stream2);
+    cudaEventDestroy(ctx->ev_split); cudaEventDestroy(ctx->ev_join);
+    cudaEventDestroy(ctx->ev_region[0]); cudaEventDestroy(ctx->ev_region[1]);
+  }
   if (ctx->prof) { for (cudaEvent_t e : ctx->prof->ev) cudaEventDestroy(e); delete ctx->prof; }
   delete ctx;
   return BE_OK;
@@ -148,6 +153,12 @@ extern "C" int be_set_workspace_limit(be_ctx* ctx, size_t bytes) {
   if (!ctx) return BE_ERR_NULL;
   if (bytes < ((size_t)1 << 20)) return BE_ERR_SHAPE;
   ctx->ws_limit = bytes;
+  return BE_OK;
+}
+
+extern "C" int be_set_chunk_pipeline(be_ctx* ctx, int on) {
+  if (!ctx) return BE_ERR_NULL;
+  ctx->chunk_pipeline = on ? 1 : 0;
   return BE_OK;
 }
 

@@ -51,6 +51,22 @@ static size_t per_loop_bytes(int N, int m, int n1, bool spin) {
   return b;
 }
 
+static int wilson_chunk(be_ctx* ctx, const cplx* H, const GridMap& map, int N, int m, int n1, int64_t l0, int64_t nl,
+                        int64_t cnt, const cplx* d_close, double* d_mingap, const SpinArgs* sp, int mlo, int mhi,
+                        cplx* const* Wall);
+
+static int pipeline_init(be_ctx* ctx) {
+  if (ctx->stream2) return BE_OK;
+  int least = 0, greatest = 0;
+  BE_CUDA(cudaDeviceGetStreamPriorityRange(&least, &greatest));
+  BE_CUDA(cudaStreamCreateWithPriority(&ctx->stream2, cudaStreamNonBlocking, greatest));
+  BE_CUDA(cudaEventCreateWithFlags(&ctx->ev_split, cudaEventDisableTiming));
+  BE_CUDA(cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming));
+  BE_CUDA(cudaEventCreateWithFlags(&ctx->ev_region[0], cudaEventDisableTiming));
+  BE_CUDA(cudaEventCreateWithFlags(&ctx->ev_region[1], cudaEventDisableTiming));
+  return BE_OK;
+}
+
 // One pass over all loops of ``map`` (device H).  Plain loop when ``sp`` is NULL.
 static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, int m,
                          const cplx* d_close, double* d_theta, double* d_abs, double* d_mingap,
@@ -71,7 +87,16 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   size_t persist = 0;
   for (int s = 0; s < 2; ++s)
     persist += be_align256((size_t)loops * msec[s] * msec[s] * sizeof(cplx)) + be_eigenphases_scratch_bytes(loops, msec[s]) + 1024;
-  BE_TRY(be_arena_reserve(ctx, per * (size_t)lc + persist + (4 << 20)));
+  // Chunk pipeline (more than one chunk): two scratch regions used alternately, the
+  // tridiagonalization of chunk c+1 on the caller's stream overlaps the rest of chunk c on stream2.
+  const size_t region = be_align256(per * (size_t)lc);
+  bool pipe = nchunks > 1 && ctx->chunk_pipeline;
+  if (pipe) {
+    BE_TRY(pipeline_init(ctx));
+    if (be_arena_reserve(ctx, 2 * region + persist + (4 << 20)) != BE_OK) pipe = false;   // not enough memory: serial
+  }
+  if (!pipe) BE_TRY(be_arena_reserve(ctx, region + persist + (4 << 20)));
+  cudaStream_t S1 = ctx->stream;
   cplx* Wall[2] = {nullptr, nullptr};
   for (int s = 0; s < 2; ++s)
     if (msec[s] > 0) {
@@ -82,7 +107,47 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   for (int64_t l0 = 0; l0 < loops; l0 += lc) {
     const int64_t nl = (loops - l0 < lc) ? loops - l0 : lc;
     const int64_t cnt = nl * n1;
-    ctx->arena_used = keep;
+    const int64_t ci = l0 / lc;
+    ctx->arena_used = keep + (pipe ? (size_t)(ci & 1) * region : 0);
+    if (pipe) {
+      ctx->stream = S1;
+      if (ci >= 2) BE_CUDA(cudaStreamWaitEvent(S1, ctx->ev_region[ci & 1], 0));   // region free again
+      ctx->split_after_tridiag = 1;
+      ctx->gemm_pad = (l0 + lc < loops && N > 8) ? 1 : 0;   // a next chunk will stream its matrices next to these GEMMs
+    }
+    const int rc = wilson_chunk(ctx, H, map, N, m, n1, l0, nl, cnt, d_close, d_mingap, sp, mlo, mhi, Wall);
+    if (pipe) {
+      ctx->split_after_tridiag = 0;
+      if (rc == BE_OK) cudaEventRecord(ctx->ev_region[ci & 1], ctx->stream);
+    }
+    if (rc != BE_OK) { ctx->stream = S1; ctx->gemm_pad = 0; return rc; }
+  }
+  // ---- S4 for every loop at once
+  ctx->arena_used = keep;
+  int rc = BE_OK;
+  if (!sp) {
+    rc = be_eigenphases(ctx, Wall[0], loops, m, d_theta, d_abs);
+  } else {
+    for (int sector = 0; sector < 2 && rc == BE_OK; ++sector) {
+      double* out = sector == 0 ? sp->theta_lo : sp->theta_hi;
+      if (msec[sector] == 0 || !out) continue;
+      rc = be_eigenphases(ctx, Wall[sector], loops, msec[sector], out, nullptr);
+    }
+  }
+  if (pipe) {   // join: the caller's stream waits for everything enqueued on stream2
+    cudaEventRecord(ctx->ev_join, ctx->stream);
+    cudaStreamWaitEvent(S1, ctx->ev_join, 0);
+    ctx->stream = S1;
+    ctx->gemm_pad = 0;
+  }
+  return rc;
+}
+
+// One chunk of nl whole loops (cnt = nl * n1 matrices): S1, then S6 (if sp), S2, S3 into Wall.
+static int wilson_chunk(be_ctx* ctx, const cplx* H, const GridMap& map, int N, int m, int n1, int64_t l0, int64_t nl,
+                        int64_t cnt, const cplx* d_close, double* d_mingap, const SpinArgs* sp, int mlo, int mhi,
+                        cplx* const* Wall) {
+  {
     double* E = (double*)be_arena_alloc(ctx, (size_t)cnt * N * sizeof(double));
     cplx* X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
     if (!E || !X) return BE_ERR_NOMEM;
@@ -91,7 +156,7 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
     if (!sp) {
       cplx* W = nullptr;
       BE_TRY(be_chain_product(ctx, X, N, m, nl, n1, d_close, n1 - 1, Wall[0] + l0 * (int64_t)m * m, &W));
-      continue;
+      return BE_OK;
     }
     // ---- spin-resolved: S_red = U^H S U, diagonalize, rotate into sectors
     cplx* SX = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
@@ -135,17 +200,6 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
       cplx* W = nullptr;
       BE_TRY(be_chain_product(ctx, F, N, ms, nl, n1, d_close, n1 - 1, Wall[sector] + l0 * (int64_t)ms * ms, &W));
       ctx->arena_used = mark;
-    }
-  }
-  // ---- S4 for every loop at once
-  ctx->arena_used = keep;
-  if (!sp) {
-    BE_TRY(be_eigenphases(ctx, Wall[0], loops, m, d_theta, d_abs));
-  } else {
-    for (int sector = 0; sector < 2; ++sector) {
-      double* out = sector == 0 ? sp->theta_lo : sp->theta_hi;
-      if (msec[sector] == 0 || !out) continue;
-      BE_TRY(be_eigenphases(ctx, Wall[sector], loops, msec[sector], out, nullptr));
     }
   }
   return BE_OK;

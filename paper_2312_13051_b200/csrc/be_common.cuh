@@ -82,6 +82,15 @@ struct be_ctx {
   size_t arena_bytes;
   size_t arena_used;
   int gemm_attr_set;
+  // two-stream chunk pipeline (be_wilson_loop / be_spin_resolved_wilson with more than one chunk):
+  // the tridiagonalization of chunk c+1 (HBM bound) runs on ``stream`` while everything else of
+  // chunk c (FP64 / latency bound) runs on the high-priority ``stream2``
+  cudaStream_t stream2;
+  cudaEvent_t ev_split, ev_region[2], ev_join;
+  int chunk_pipeline;         // be_set_chunk_pipeline (default 0)
+  int split_after_tridiag;    // consumed by be_eigh_large: switch to stream2 after S1a
+  int gemm_pad;               // zgemm launches with padded shared memory: at most one GEMM CTA per SM,
+                              // leaving room for one k_hemv CTA of the other stream
   struct be_prof* prof;       // optional per-kernel-class CUDA-event timing (be_profile_enable)
 };
 

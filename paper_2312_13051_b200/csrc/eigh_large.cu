@@ -65,7 +65,7 @@ constexpr int HSTAGES = 3;
 constexpr int HEMV_THREADS = 256 + 32;
 constexpr int HSTAGE_ELEMS = (HB + 1) * HROWS;                 // 32 columns + the v segment
 constexpr size_t HEMV_SMEM = (size_t)HSTAGES * HSTAGE_ELEMS * sizeof(cplx) + 2 * 4 * HROWS * sizeof(cplx)
-                             + 2 * HSTAGES * sizeof(unsigned long long) + 64;
+                             + 2 * HSTAGES * sizeof(unsigned long long) + 8 * sizeof(int) + 64;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(void* bar, int count) {
@@ -91,35 +91,27 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, uint32_
 // Block columns J >= nJ are "panel blocks": 32 columns of the [W | V] panels streamed through the
 // same pipeline with only their column part kept, pq[q] = W[:, q]^H v (q < k), V[:, q-k]^H v (q >= k),
 // the 2k products k_colw needs for w_i.
-// A CTA owns TWO block columns, J and nJ-1-J (long + short: every CTA streams about the same number
-// of stages, and the pipeline prologue / epilogue is paid once per pair); the stage counter runs on
-// across the pair, so the producer prefetches the second block column while the consumers reduce
-// the column part of the first.  Panel blocks come first in the grid (they are the longest).
+// The kernel is PERSISTENT: 2 CTAs per SM fetch work items (matrix, block column) from a global
+// counter until none is left (panel blocks and long block columns come first in the item order).
+// The producer warp runs ahead of the consumers across item boundaries -- the stage counter never
+// restarts -- so the prologue / epilogue of one item is covered by the stream of the next and a
+// single resident CTA keeps its share of HBM busy (which is what lets the FP64-bound GEMMs of the
+// previous chunk share the SM in the chunk pipeline).  Item numbers travel from the producer to the
+// consumers through a small ring in shared memory, ordered by the stages' mbarriers.
+constexpr int HRING = 8;
 __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict__ Bw, cplx* __restrict__ P,
                                                           cplx* __restrict__ zpart, int N, int i, int nJ, int nJmax,
                                                           const cplx* __restrict__ Wp, cplx* __restrict__ pqg,
-                                                          int p, int npb) {
+                                                          int p, int npb, int* __restrict__ counter, int total) {
   extern __shared__ __align__(128) unsigned char hsm[];
   cplx* stage = (cplx*)hsm;                                           // [HSTAGES][HB + 1][HROWS]
   cplx* ysm = stage + (size_t)HSTAGES * HSTAGE_ELEMS;                 // [2][4][HROWS]
   unsigned long long* full = (unsigned long long*)(ysm + 2 * 4 * HROWS);
   unsigned long long* empty = full + HSTAGES;
-  const int npair = (nJ + 1) / 2;
-  const int64_t c = blockIdx.x / (npair + npb);
-  const int u = blockIdx.x % (npair + npb);
-  const bool panel = u < npb;
+  volatile int* ring = (volatile int*)(empty + HSTAGES);              // [HRING] item numbers, -1 = end
+  const int per = nJ + npb;                                           // items per matrix
   const int k = i - p;
-  const cplx* __restrict__ B = Bw + c * (int64_t)N * N;
-  const cplx* __restrict__ W = Wp + c * (int64_t)N * NB;
-  const cplx* __restrict__ v = B + (int64_t)i * N;   // v[r], r >= i+1 (global row index)
   const int tid = threadIdx.x;
-  // the (up to) two work items of this CTA
-  int Jw[2], nwork;
-  if (panel) { Jw[0] = u; Jw[1] = 0; nwork = 1; }
-  else {
-    Jw[0] = u - npb; Jw[1] = nJ - 1 - Jw[0];
-    nwork = (Jw[1] > Jw[0]) ? 2 : 1;
-  }
   if (tid == 0) {
     for (int s = 0; s < HSTAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -130,9 +122,26 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
     // ---- producer warp: lane = column of the block column (lane 0 also copies the v segment)
     const int lane = tid - 256;
     int gs = 0;
-    for (int wi = 0; wi < nwork; ++wi) {
-      const int q0 = panel ? Jw[wi] * HB : 0;
-      const int c0 = panel ? i + 1 : i + 1 + Jw[wi] * HB;
+    for (int seq = 0;; ++seq) {
+      int item = 0;
+      if (lane == 0) item = atomicAdd(counter, 1);
+      item = __shfl_sync(0xffffffffu, item, 0);
+      if (item >= total) {
+        // end of work: one empty stage carries the stop mark
+        const int slot = gs % HSTAGES;
+        if (gs >= HSTAGES) mbar_wait(&empty[slot], ((gs / HSTAGES) - 1) & 1);
+        if (lane == 0) { ring[seq % HRING] = -1; mbar_arrive(&full[slot]); }
+        break;
+      }
+      const int64_t c = item / per;
+      const int u = item % per;
+      const bool panel = u < npb;
+      const int J = panel ? u : u - npb;
+      const cplx* __restrict__ B = Bw + c * (int64_t)N * N;
+      const cplx* __restrict__ W = Wp + c * (int64_t)N * NB;
+      const cplx* __restrict__ v = B + (int64_t)i * N;
+      const int q0 = panel ? J * HB : 0;
+      const int c0 = panel ? i + 1 : i + 1 + J * HB;
       const int ncols = panel ? ((2 * k - q0 < HB) ? 2 * k - q0 : HB) : ((N - c0 < HB) ? N - c0 : HB);
       const int nst = (N - c0 + HROWS - 1) / HROWS;
       const cplx* src = nullptr;
@@ -148,6 +157,7 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
         const uint32_t seg = (uint32_t)nr * sizeof(cplx);
         cplx* dst = stage + (size_t)slot * HSTAGE_ELEMS;
         if (lane == 0) {
+          if (s == 0) ring[seq % HRING] = item;      // published by the release of the arrive below
           mbar_expect_tx(&full[slot], seg * (uint32_t)(ncols + 1));
           tma_bulk_g2s(dst + HB * HROWS, v + r0, seg, &full[slot]);
         }
@@ -161,9 +171,17 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
   // ---- consumers
   const int lr = tid & (HROWS - 1), cg = tid >> 6, lane = tid & 31, warp = tid >> 5;
   int gs = 0;
-  for (int wi = 0; wi < nwork; ++wi) {
-    const int q0 = panel ? Jw[wi] * HB : 0;
-    const int c0 = panel ? i + 1 : i + 1 + Jw[wi] * HB;
+  for (int seq = 0;; ++seq) {
+    mbar_wait(&full[gs % HSTAGES], (gs / HSTAGES) & 1);   // first stage of the item (or the stop mark)
+    const int item = ring[seq % HRING];
+    if (item < 0) break;
+    const int64_t c = item / per;
+    const int u = item % per;
+    const bool panel = u < npb;
+    const int J = panel ? u : u - npb;
+    const cplx* __restrict__ v = Bw + c * (int64_t)N * N + (int64_t)i * N;
+    const int q0 = panel ? J * HB : 0;
+    const int c0 = panel ? i + 1 : i + 1 + J * HB;
     const int ncols = panel ? ((2 * k - q0 < HB) ? 2 * k - q0 : HB) : ((N - c0 < HB) ? N - c0 : HB);
     const int nst = (N - c0 + HROWS - 1) / HROWS;
     int nq = ncols - cg * 8;
@@ -174,12 +192,12 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
       accz[q] = mkc(0.0, 0.0);
       vc[q] = (q < nq && !panel) ? v[c0 + cg * 8 + q] : mkc(0.0, 0.0);
     }
-    cplx* Prow = P + (c * nJmax + Jw[wi]) * (int64_t)N;
+    cplx* Prow = P + (c * nJmax + J) * (int64_t)N;
     for (int s = 0; s < nst; ++s, ++gs) {
       const int slot = gs % HSTAGES;
       const cplx* st = stage + (size_t)slot * HSTAGE_ELEMS;
       const int r = c0 + s * HROWS + lr;
-      mbar_wait(&full[slot], (gs / HSTAGES) & 1);
+      if (s > 0) mbar_wait(&full[slot], (gs / HSTAGES) & 1);
       cplx yr = mkc(0.0, 0.0);
       if (r < N) {
         const cplx vr = st[HB * HROWS + lr];
@@ -237,7 +255,7 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
       if (panel) pqg[c * (2 * NB) + q0 + tid] = z;
       else zpart[c * N + c0 + tid] = z;
     }
-    asm volatile("bar.sync 1, 256;" ::: "memory");     // zsm is ysm: done before the next block column writes it
+    asm volatile("bar.sync 1, 256;" ::: "memory");     // zsm is ysm: done before the next item writes it
   }
 }
 
@@ -675,6 +693,7 @@ struct EighScratch {
   double *blo, *bhi;
   int* bcl;
   void* orth;
+  int* hcount;
 };
 
 static size_t eigh_large_carve(char* base, int64_t cnt, int N, int nv, EighScratch* s) {
@@ -708,7 +727,8 @@ static size_t eigh_large_carve(char* base, int64_t cnt, int N, int nv, EighScrat
   double* bhi = (double*)take(cnt * (size_t)N * sizeof(double));
   int* bcl = (int*)take(cnt * (size_t)N * sizeof(int));
   void* orth = take(be_cluster_orth_scratch_bytes(cnt, N, nv));
-  if (s) { *s = EighScratch{Bw, Wp, P, zp, tau, Vb, T, G, tauc, Y, Y2, pq, Ttmp, d, e, tn, Z, fa, fb, fc, fp, blk, blo, bhi, bcl, orth}; }
+  int* hcount = (int*)take((size_t)N * sizeof(int));
+  if (s) { *s = EighScratch{Bw, Wp, P, zp, tau, Vb, T, G, tauc, Y, Y2, pq, Ttmp, d, e, tn, Z, fa, fb, fc, fp, blk, blo, bhi, bcl, orth, hcount}; }
   return off;
 }
 
@@ -750,6 +770,7 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
   };
 
   // ---- S1a: blocked tridiagonalization
+  BE_CUDA(cudaMemsetAsync(s.hcount, 0, (size_t)N * sizeof(int), st));   // work counters of the persistent k_hemv, one per column
   for (int p = 0; p < N; p += NB) {
     const int pend = (p + NB < N - 1) ? p + NB : N - 1;   // reflector columns p .. pend-1
     colw(p, p, 0, 1);   // reflector of column p (or, when p == N-1, just the last diagonal entry)
@@ -760,8 +781,12 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
       const int nJ = (n + HB - 1) / HB;
       const int npb = (2 * (i - p) + HB - 1) / HB;   // panel blocks: the 2k dot products for k_colw
       be_prof_begin(ctx, PK_HEMV);
-      k_hemv<<<(unsigned)(cnt * ((nJ + 1) / 2 + npb)), HEMV_THREADS, HEMV_SMEM, st>>>(s.Bw, s.P, s.zpart, N, i, nJ, nJmax, s.Wp,
-                                                                             s.pq, p, npb);
+      {
+        const int64_t total = cnt * (int64_t)(nJ + npb);
+        const int64_t grid = total < 2 * (int64_t)ctx->sm_count ? total : 2 * (int64_t)ctx->sm_count;
+        k_hemv<<<(unsigned)grid, HEMV_THREADS, HEMV_SMEM, st>>>(s.Bw, s.P, s.zpart, N, i, nJ, nJmax, s.Wp, s.pq, p, npb,
+                                                                 s.hcount + i, (int)total);
+      }
       // algorithmic traffic: the lower triangle once, v in, y out; 8 real flops per complex fma, 2 per element
       be_prof_end(ctx, PK_HEMV, (double)cnt * (0.5 * n * (n + 1.0) + 2.0 * n) * 16.0, (double)cnt * 8.0 * n * n);
       LAUNCH_CHECK();
@@ -786,6 +811,16 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
       LAUNCH_CHECK();
       break;
     }
+  }
+
+  if (ctx->split_after_tridiag) {
+    // chunk pipeline: the rest of this chunk continues on the second stream, the caller's next
+    // chunk starts its tridiagonalization on the first one
+    ctx->split_after_tridiag = 0;
+    BE_CUDA(cudaEventRecord(ctx->ev_split, st));
+    BE_CUDA(cudaStreamWaitEvent(ctx->stream2, ctx->ev_split, 0));
+    ctx->stream = ctx->stream2;
+    st = ctx->stream2;
   }
 
   // ---- S1b: tridiagonal eigenproblem

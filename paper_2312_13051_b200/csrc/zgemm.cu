@@ -24,6 +24,10 @@ constexpr int LDK = 20;                              // k-contiguous operands: [
 constexpr int SM_PLANE = TM * LDK;                   // doubles per plane (>= TK * LDS)
 constexpr int SM_STAGE = 4 * SM_PLANE;               // A_re, A_im, B_re, B_im
 constexpr size_t SM_BYTES = 2 * SM_STAGE * sizeof(double);
+// Padded request of the chunk pipeline (be_ctx::gemm_pad): 2 x (SM_PAD + 1 KB) exceeds the 228 KB of an
+// SM, so at most ONE GEMM CTA is resident per SM, and SM_PAD + one k_hemv CTA (107 KB + 1 KB) still fits:
+// the FP64-bound GEMM of one chunk and the HBM-bound k_hemv of the next share every SM.
+constexpr size_t SM_PAD = 118 * 1024;
 
 __device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -231,11 +235,11 @@ int launch(be_ctx* ctx, const ZgemmParams& p) {
   if (blocks > 0x7fffffffLL) return BE_ERR_SHAPE;
   static bool attr_done = false;  // per instantiation; idempotent
   if (!attr_done) {
-    BE_CUDA(cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, PHI, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM_BYTES));
+    BE_CUDA(cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, PHI, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM_PAD));
     attr_done = true;
   }
   be_prof_begin(ctx, PK_GEMM);
-  zgemm_kernel<OPA, OPB, PHI, SPLIT><<<(unsigned)blocks, NTHREADS, SM_BYTES, ctx->stream>>>(p, tilesM, tilesN);
+  zgemm_kernel<OPA, OPB, PHI, SPLIT><<<(unsigned)blocks, NTHREADS, (ctx->gemm_pad && ctx->stream == ctx->stream2) ? SM_PAD : SM_BYTES, ctx->stream>>>(p, tilesM, tilesN);
   {
     const double tri = p.lower ? 0.5 : 1.0;
     const double fl = 8.0 * p.M * (double)p.N * p.K * (double)p.batch * tri;

@@ -318,6 +318,36 @@ def test_host_variants_match_device(ctx):
     assert phase_dist(th.numpy(), tho) <= PH_TOL
 
 
+def test_chunk_pipeline_matches_single_chunk_and_oracle(ctx):
+    """A small workspace cap splits the loops into >= 3 chunks: the two-stream chunk pipeline
+    (tridiagonalization of chunk c+1 next to the rest of chunk c, two scratch regions) must give
+    the results of the single-chunk run (to rounding: the start vectors of inverse iteration are
+    seeded by the index inside the chunk) and match the oracle."""
+    parts = wl.config3_parts(2, L=4)                       # N = 64
+    H = wl.supercell_grid([parts], 9, 5)                   # 5 loops of 9 points
+    Hd = dev(H)
+    th1, ab1, mg1 = ctx.wilson_loop(Hd, 32, 1)
+    S = wl.supercell_spin_z(4)
+    lo1, hi1, pso1 = ctx.spin_resolved_wilson(Hd, 32, 1, dev(S))
+    try:
+        ctx.set_workspace_limit(5 << 20)                   # one loop per chunk -> 5 chunks
+        ctx.set_chunk_pipeline(True)
+        th2, ab2, mg2 = ctx.wilson_loop(Hd, 32, 1)
+        lo2, hi2, pso2 = ctx.spin_resolved_wilson(Hd, 32, 1, dev(S))
+        torch.cuda.synchronize()
+    finally:
+        ctx.set_workspace_limit(64 << 30)
+        ctx.set_chunk_pipeline(False)
+    assert phase_dist(th1.cpu().numpy(), th2.cpu().numpy()) <= 1e-11
+    assert (mg1 - mg2).abs().max().item() <= 1e-12 and (pso1 - pso2).abs().max().item() <= 1e-12
+    assert phase_dist(lo1.cpu().numpy(), lo2.cpu().numpy()) <= 1e-11
+    assert phase_dist(hi1.cpu().numpy(), hi2.cpu().numpy()) <= 1e-11
+    tho, _, _ = wo.wilson_surface(H, 32, 1)
+    assert phase_dist(th2.cpu().numpy(), tho) <= PH_TOL
+    loo, hio, _ = wo.spin_resolved_surface(H, 32, 1, S)
+    assert phase_dist(lo2.cpu().numpy(), loo) <= PH_TOL and phase_dist(hi2.cpu().numpy(), hio) <= PH_TOL
+
+
 def test_launch_counter_counts_kernels(ctx):
     n0 = ctx.launch_count()
     ctx.wilson_loop(dev(wl.config1_grid(6, 2)[None]), 2, 1)
