@@ -122,10 +122,12 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
     // ---- producer warp: lane = column of the block column (lane 0 also copies the v segment)
     const int lane = tid - 256;
     int gs = 0;
+    int next = 0;
+    if (lane == 0) next = atomicAdd(counter, 1);
     for (int seq = 0;; ++seq) {
-      int item = 0;
-      if (lane == 0) item = atomicAdd(counter, 1);
-      item = __shfl_sync(0xffffffffu, item, 0);
+      // the item after this one is fetched now: the atomic's round trip hides behind the copies
+      const int item = __shfl_sync(0xffffffffu, next, 0);
+      if (lane == 0 && item < total) next = atomicAdd(counter, 1);
       if (item >= total) {
         // end of work: one empty stage carries the stop mark
         const int slot = gs % HSTAGES;
@@ -750,7 +752,10 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
   const int nJmax = (N + HB - 1) / HB;
 
   if (info) { k_set_info<<<(unsigned)((cnt + 255) / 256), 256, 0, st>>>(info, cnt); LAUNCH_CHECK(); }
-  {
+  const bool on_chip = N <= TS_MAXN;   // whole matrix in one CTA's shared memory (tridiag_small.cu)
+  if (on_chip) {
+    BE_TRY(be_tridiag_small(ctx, H, map, loop0, cnt, N, s.Bw, s.d, s.e, s.tau));
+  } else {
     const int nchunk = (int)(((int64_t)N * N + 2047) / 2048);
     k_gather<<<(unsigned)(cnt * nchunk), 256, 0, st>>>(H, s.Bw, map, loop0, N, nchunk);
     LAUNCH_CHECK();
@@ -771,7 +776,7 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
 
   // ---- S1a: blocked tridiagonalization
   BE_CUDA(cudaMemsetAsync(s.hcount, 0, (size_t)N * sizeof(int), st));   // work counters of the persistent k_hemv, one per column
-  for (int p = 0; p < N; p += NB) {
+  for (int p = 0; p < N && !on_chip; p += NB) {
     const int pend = (p + NB < N - 1) ? p + NB : N - 1;   // reflector columns p .. pend-1
     colw(p, p, 0, 1);   // reflector of column p (or, when p == N-1, just the last diagonal entry)
     LAUNCH_CHECK();
