@@ -65,7 +65,7 @@ constexpr int HSTAGES = 3;
 constexpr int HEMV_THREADS = 256 + 32;
 constexpr int HSTAGE_ELEMS = (HB + 1) * HROWS;                 // 32 columns + the v segment
 constexpr size_t HEMV_SMEM = (size_t)HSTAGES * HSTAGE_ELEMS * sizeof(cplx) + 2 * 4 * HROWS * sizeof(cplx)
-                             + 2 * HSTAGES * sizeof(unsigned long long) + 8 * sizeof(int) + 64;
+                             + 2 * HSTAGES * sizeof(unsigned long long) + 8 * sizeof(int) + 64 + 2 * 64 * sizeof(cplx);
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(void* bar, int count) {
@@ -109,6 +109,7 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
   unsigned long long* full = (unsigned long long*)(ysm + 2 * 4 * HROWS);
   unsigned long long* empty = full + HSTAGES;
   volatile int* ring = (volatile int*)(empty + HSTAGES);              // [HRING] item numbers, -1 = end
+  cplx* zsm0 = (cplx*)(hsm + HEMV_SMEM - 2 * 64 * sizeof(cplx));      // [2][8 warps][8]
   const int per = nJ + npb;                                           // items per matrix
   const int k = i - p;
   const int tid = threadIdx.x;
@@ -181,7 +182,6 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
     const int u = item % per;
     const bool panel = u < npb;
     const int J = panel ? u : u - npb;
-    const cplx* __restrict__ v = Bw + c * (int64_t)N * N + (int64_t)i * N;
     const int q0 = panel ? J * HB : 0;
     const int c0 = panel ? i + 1 : i + 1 + J * HB;
     const int ncols = panel ? ((2 * k - q0 < HB) ? 2 * k - q0 : HB) : ((N - c0 < HB) ? N - c0 : HB);
@@ -189,10 +189,14 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
     int nq = ncols - cg * 8;
     nq = nq < 0 ? 0 : (nq > 8 ? 8 : nq);
     cplx vc[8], accz[8];
+    {
+      // v at the block column's own columns = the head of the first stage's v segment (rows c0 ..)
+      const cplx* v0 = stage + (size_t)(gs % HSTAGES) * HSTAGE_ELEMS + HB * HROWS;
 #pragma unroll
-    for (int q = 0; q < 8; ++q) {
-      accz[q] = mkc(0.0, 0.0);
-      vc[q] = (q < nq && !panel) ? v[c0 + cg * 8 + q] : mkc(0.0, 0.0);
+      for (int q = 0; q < 8; ++q) {
+        accz[q] = mkc(0.0, 0.0);
+        vc[q] = (q < nq && !panel) ? v0[cg * 8 + q] : mkc(0.0, 0.0);
+      }
     }
     cplx* Prow = P + (c * nJmax + J) * (int64_t)N;
     for (int s = 0; s < nst; ++s, ++gs) {
@@ -242,13 +246,30 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
         Prow[r] = t;
       }
     }
-    // column part: reduce over the 64 rows (2 warps per column group)
-    asm volatile("bar.sync 1, 256;" ::: "memory");
-    cplx* zsm = ysm;   // [8 warps][8]
+    // column part: reduce over the 64 rows (2 warps per column group); zsm is double buffered by item
+    cplx* zsm = zsm0 + (seq & 1) * 64;   // [8 warps][8]
+    {
+      // 8 sums over the 32 lanes with 9 exchanges per component (halving the live values at every
+      // step) instead of 8 x 5: lane bits 4, 3, 2 end up selecting which of the 8 sums the lane holds
+      cplx b4[4], b2[2], b1;
+      const bool u16 = lane & 16, u8 = lane & 8, u4 = lane & 4;
 #pragma unroll
-    for (int q = 0; q < 8; ++q) {
-      const cplx z = warp_sum(accz[q]);
-      if (lane == 0) zsm[warp * 8 + q] = z;
+      for (int j = 0; j < 4; ++j) {
+        const cplx snd = u16 ? accz[j] : accz[j + 4], kp = u16 ? accz[j + 4] : accz[j];
+        b4[j] = mkc(kp.x + __shfl_xor_sync(0xffffffffu, snd.x, 16), kp.y + __shfl_xor_sync(0xffffffffu, snd.y, 16));
+      }
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const cplx snd = u8 ? b4[j] : b4[j + 2], kp = u8 ? b4[j + 2] : b4[j];
+        b2[j] = mkc(kp.x + __shfl_xor_sync(0xffffffffu, snd.x, 8), kp.y + __shfl_xor_sync(0xffffffffu, snd.y, 8));
+      }
+      {
+        const cplx snd = u4 ? b2[0] : b2[1], kp = u4 ? b2[1] : b2[0];
+        b1 = mkc(kp.x + __shfl_xor_sync(0xffffffffu, snd.x, 4), kp.y + __shfl_xor_sync(0xffffffffu, snd.y, 4));
+      }
+      b1.x += __shfl_xor_sync(0xffffffffu, b1.x, 2); b1.y += __shfl_xor_sync(0xffffffffu, b1.y, 2);
+      b1.x += __shfl_xor_sync(0xffffffffu, b1.x, 1); b1.y += __shfl_xor_sync(0xffffffffu, b1.y, 1);
+      if ((lane & 3) == 0) zsm[warp * 8 + (u16 ? 4 : 0) + (u8 ? 2 : 0) + (u4 ? 1 : 0)] = b1;
     }
     asm volatile("bar.sync 1, 256;" ::: "memory");
     if (tid < HB && tid < ncols) {
@@ -257,7 +278,6 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
       if (panel) pqg[c * (2 * NB) + q0 + tid] = z;
       else zpart[c * N + c0 + tid] = z;
     }
-    asm volatile("bar.sync 1, 256;" ::: "memory");     // zsm is ysm: done before the next item writes it
   }
 }
 

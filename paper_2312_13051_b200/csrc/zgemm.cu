@@ -25,9 +25,9 @@ constexpr int SM_PLANE = TM * LDK;                   // doubles per plane (>= TK
 constexpr int SM_STAGE = 4 * SM_PLANE;               // A_re, A_im, B_re, B_im
 constexpr size_t SM_BYTES = 2 * SM_STAGE * sizeof(double);
 // Padded request of the chunk pipeline (be_ctx::gemm_pad): 2 x (SM_PAD + 1 KB) exceeds the 228 KB of an
-// SM, so at most ONE GEMM CTA is resident per SM, and SM_PAD + one k_hemv CTA (107 KB + 1 KB) still fits:
+// SM, so at most ONE GEMM CTA is resident per SM, and SM_PAD + one k_hemv CTA (109 KB + 1 KB) still fits:
 // the FP64-bound GEMM of one chunk and the HBM-bound k_hemv of the next share every SM.
-constexpr size_t SM_PAD = 118 * 1024;
+constexpr size_t SM_PAD = 116 * 1024;
 
 __device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
