@@ -348,6 +348,88 @@ def test_chunk_pipeline_matches_single_chunk_and_oracle(ctx):
     assert phase_dist(lo2.cpu().numpy(), loo) <= PH_TOL and phase_dist(hi2.cpu().numpy(), hio) <= PH_TOL
 
 
+# ------------------------------------------------------------------------------ full sizes, bench configuration
+def _bench_workload(cfg):
+    import importlib.util, os
+    spec = importlib.util.spec_from_file_location("bench_mod", os.path.join(os.path.dirname(__file__), "..", "bench.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    return mod.Workload(cfg, 0, False)
+
+
+def _need_memory(gb):
+    free, _ = torch.cuda.mem_get_info()
+    if free < gb * 2 ** 30:
+        pytest.skip(f"needs {gb} GB of free device memory")
+
+
+def test_full_size_config4_in_bench_configuration(ctx):
+    """BASELINE.json configs[3] at full size exactly as bench.py runs it (N = 1600, 24 x 25 grid, 2 chunks
+    of 300 matrices): exact invariants on the whole output, and two sampled loops element by element
+    against the oracle (one loop of 25 k-points costs the oracle ~15 s)."""
+    _need_memory(30)
+    wk = _bench_workload(4)
+    H, S = wk.device_grid(torch, torch.device("cuda"))
+    lo, hi, pso = wk.run_device(ctx, H, S)
+    torch.cuda.synchronize()
+    # PSO eigenvalues are exactly +-1 ([H, S_z] = 0, PAPER.md:156), half of each sign
+    p = pso.cpu().numpy()
+    assert np.abs(np.abs(p) - 1.0).max() < 1e-10 and np.all(p[..., :400] < 0) and np.all(p[..., 400:] > 0)
+    # sector windings over the closed t2 cycle: +1 (S_z = -1 sector), -1, total 0 -- exact integers (R11)
+    wl_lo = ctx.winding(lo[None]).item()
+    wl_hi = ctx.winding(hi[None]).item()
+    assert abs(wl_lo - round(wl_lo)) < 1e-9 and abs(wl_hi - round(wl_hi)) < 1e-9
+    assert sorted((round(wl_lo), round(wl_hi))) == [-1, 1]
+    parts = wl.config4_parts(20, realization=0)
+    Sh = wl.supercell_spin_z(20)
+    for j in (0, 17):
+        Hj = H[0, j].cpu().numpy()[None, None]                          # the same matrices on both sides
+        assert np.abs(wl.supercell_grid([parts], 25, 24, t2_indices=[j]) - Hj).max() < 1e-12   # = the seeded recipe
+        loo, hio, _ = wo.spin_resolved_surface(Hj, 800, 1, Sh)
+        assert phase_dist(lo[j:j + 1].cpu().numpy(), loo) <= PH_TOL
+        assert phase_dist(hi[j:j + 1].cpu().numpy(), hio) <= PH_TOL
+    del H
+    torch.cuda.empty_cache()
+
+
+def test_full_size_config3_sampled(ctx):
+    """BASELINE.json configs[2] at full size (16 realizations x 32 x 33, N = 400; 43 GB): sampled loops
+    against the oracle, sum rule sum_n theta_n = arg det W on all loops is implied by the eigen-solver
+    parity; total winding per realization is an exact integer (0: time-reversal symmetric)."""
+    _need_memory(50)
+    wk = _bench_workload(3)
+    H, _ = wk.device_grid(torch, torch.device("cuda"))
+    th, ab, mg = wk.run_device(ctx, H, None)
+    torch.cuda.synchronize()
+    assert mg.min().item() > 0.5
+    w = ctx.winding(th.reshape(16, 32, 200)).cpu().numpy()
+    assert np.abs(w - np.round(w)).max() < 1e-8 and np.all(np.round(w) == 0)
+    for (r, j) in ((0, 0), (7, 13), (15, 31)):
+        Hl = H[r, j].cpu().numpy()[None, None]
+        tho, abo, mgo = wo.wilson_surface(Hl, 200, 1)
+        assert phase_dist(th[r * 32 + j:r * 32 + j + 1].cpu().numpy(), tho) <= PH_TOL
+        assert abs(mg[r * 32 + j].item() - mgo[0]) < 1e-9
+    del H
+    torch.cuda.empty_cache()
+
+
+def test_full_size_config5_sampled(ctx):
+    """BASELINE.json configs[4] at full size (64 x 64 loops of 65 points, N = 64: 266 240 eigensolves)."""
+    _need_memory(25)
+    wk = _bench_workload(5)
+    H, _ = wk.device_grid(torch, torch.device("cuda"))
+    th, ab, mg = wk.run_device(ctx, H, None)
+    torch.cuda.synchronize()
+    assert mg.min().item() > 0.2                               # harness asserts the gap (R13)
+    idx = [0, 77, 1234, 2048, 4095]
+    for l in idx:
+        Hl = H[l // 64, l % 64].cpu().numpy()[None, None]
+        tho, abo, _ = wo.wilson_surface(Hl, 32, 1)
+        assert phase_dist(th[l:l + 1].cpu().numpy(), tho) <= PH_TOL
+    del H
+    torch.cuda.empty_cache()
+
+
 def test_launch_counter_counts_kernels(ctx):
     n0 = ctx.launch_count()
     ctx.wilson_loop(dev(wl.config1_grid(6, 2)[None]), 2, 1)
