@@ -131,9 +131,12 @@ int be_wilson_loop(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_
  * (orthonormalized); w = U_base V_S; a second loop of w runs along dir2 (closing phase d_close2).
  *   d_theta1       [batch][other][dims[dir2]][n_occ]: first-level phases, branch (-pi, pi].
  *   d_theta_nested [batch][other][wb_hi-wb_lo]: nested phases; polarization p = -sum/2pi mod 1.
- * This build: n_occ <= 2 (closed-form eigenvectors of the 2 x 2 Wilson matrix, the case of the
- * paper's 4-band quadrupole models and of BASELINE.json configs[1]); n_occ > 2 returns
- * BE_ERR_UNSUPPORTED (nothing is enqueued).
+ * n_occ <= 2: closed-form eigenvectors of the 2 x 2 Wilson matrix (the paper's 4-band quadrupole
+ * models, BASELINE.json configs[1]).  n_occ > 2: all eigenvalues of W by Hessenberg-QR, the selected
+ * ones refined to eigenvectors by inverse iteration on W - lambda I (partially pivoted LU per band,
+ * every solve followed by the orthonormalization, so degenerate Wannier bands span their cluster);
+ * wb_hi - wb_lo <= 64, else BE_ERR_UNSUPPORTED.  The result is defined when the selected bands are
+ * separated from the others by a Wannier gap (R9).
  */
 int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_occ,
                      int dir1, int dir2, int base, int wb_lo, int wb_hi, double theta_cut,

@@ -253,7 +253,7 @@ extern "C" int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid*
   if (grid->ndim < 2 || dir2 < 0 || dir2 >= grid->ndim || dir2 == dir1) return BE_ERR_SHAPE;
   if (base < 0 || base >= grid->dims[dir1]) return BE_ERR_SHAPE;
   if (wb_lo < 0 || wb_hi > n_occ || wb_lo >= wb_hi) return BE_ERR_SHAPE;
-  if (n_occ > 2) return BE_ERR_UNSUPPORTED;   // closed-form Wannier-band vectors only (header)
+  if (n_occ > 2 && wb_hi - wb_lo > 64) return BE_ERR_UNSUPPORTED;   // inverse-iteration path: at most 64 Wannier bands (header)
   const int N = grid->N, m = n_occ, ns = wb_hi - wb_lo;
   // virtual axis order (other, dir2, dir1) so that loops enumerate [batch][other][i2]
   GridMap full;
@@ -273,7 +273,8 @@ extern "C" int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid*
   const int phi_at = n1 - 1 - base;   // link whose target frame has grid index 0
 
   const size_t per = (size_t)n1 * (be_eigh_scratch_bytes(1, N, m) + (size_t)N * m * 16 + (size_t)N * 8 + 512)
-                     + (size_t)n1 * m * m * 16 + 8 * (size_t)m * m * 16 + 4096;
+                     + (size_t)n1 * m * m * 16 + 8 * (size_t)m * m * 16 + 4096
+                     + (m > 2 ? be_nested_general_scratch_bytes(1, m, ns) + be_eigenphases_scratch_bytes(1, m) : 0);
   const size_t persist = (size_t)loops * ((size_t)N * ns * 16 + 256) + (size_t)outer2 * (n2 + 4) * ns * ns * 16 + (8 << 20);
   int64_t lc = (int64_t)(ctx->ws_limit / per);
   if (lc < 1) lc = 1;
@@ -295,7 +296,8 @@ extern "C" int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid*
     BE_TRY(be_eigh_frames(ctx, (const cplx*)dH_grid, map, l0, cnt, N, m, m + 1, E, X, nullptr));
     cplx* W = nullptr;
     BE_TRY(be_chain_product(ctx, X, N, m, nl, n1, (const cplx*)d_close1, phi_at, nullptr, &W));
-    BE_TRY(be_nested_select_small(ctx, W, nl, m, wb_lo, wb_hi, theta_cut, th1 + l0 * m, Vs));
+    if (m <= 2) BE_TRY(be_nested_select_small(ctx, W, nl, m, wb_lo, wb_hi, theta_cut, th1 + l0 * m, Vs));
+    else BE_TRY(be_nested_select_general(ctx, W, nl, m, wb_lo, wb_hi, theta_cut, th1 + l0 * m, Vs));
     // w = U_base V_S  (frame j = 0 of each rolled loop)
     ZgemmParams g = zgemm_simple(N, ns, m, X, N, (int64_t)n1 * N * m, Vs, m, (int64_t)m * ns,
                                  Wf + l0 * (int64_t)N * ns, N, (int64_t)N * ns, nl);

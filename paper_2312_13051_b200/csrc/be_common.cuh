@@ -185,6 +185,10 @@ size_t be_eigh_scratch_bytes(int64_t cnt, int N, int nv);
 int be_eigenphases(be_ctx* ctx, cplx* W, int64_t cnt, int m, double* theta, double* absl);
 size_t be_eigenphases_scratch_bytes(int64_t cnt, int m);
 int be_eigenvalues_general(be_ctx* ctx, cplx* W, int64_t cnt, int m, cplx* lam, int* fail);
+int be_sort_phases(be_ctx* ctx, const cplx* lam, int64_t cnt, int m, double* theta, double* absl);
+size_t be_nested_general_scratch_bytes(int64_t nl, int m, int ns);
+int be_nested_select_general(be_ctx* ctx, cplx* W, int64_t nl, int m, int wb_lo, int wb_hi, double cut,
+                             double* theta1, cplx* Vs);
 
 int be_eigh_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N,
                   int nv, double* E, cplx* X, int* info);

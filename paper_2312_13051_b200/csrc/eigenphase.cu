@@ -357,6 +357,10 @@ int be_eigenphases(be_ctx* ctx, cplx* W, int64_t cnt, int m, double* theta, doub
   int* fail = (int*)be_arena_alloc(ctx, (size_t)cnt * sizeof(int));
   if (!lam || !fail) return BE_ERR_NOMEM;
   BE_TRY(be_eigenvalues_general(ctx, W, cnt, m, lam, fail));
+  return be_sort_phases(ctx, lam, cnt, m, theta, absl);
+}
+
+int be_sort_phases(be_ctx* ctx, const cplx* lam, int64_t cnt, int m, double* theta, double* absl) {
   int nt = ((m + 31) / 32) * 32;
   if (nt > 256) nt = 256;
   const size_t sh = (size_t)m * sizeof(double);

@@ -235,6 +235,68 @@ def test_nested_variants(ctx, gamma, p):
     assert wo.circ_sorted_distance(thn_t.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
 
 
+def _coupled_bbh_grid(n1, n2, eps=0.05, seed=3):
+    """Two BBH copies (gamma = 0.5, 0.6) weakly coupled: N = 8, n_occ = 4, Wannier gap ~0.8."""
+    rng = np.random.default_rng(seed)
+    C = rng.standard_normal((4, 4)) + 1j * rng.standard_normal((4, 4))
+    H = np.zeros((n2, n1, 8, 8), complex)
+    for j in range(n2):
+        for i in range(n1):
+            kx, ky = 2 * np.pi * i / n1, 2 * np.pi * j / n2
+            H[j, i, :4, :4] = wl.bbh(kx, ky, 0.5, 1.0)
+            H[j, i, 4:, 4:] = wl.bbh(kx, ky, 0.6, 1.0)
+            H[j, i, :4, 4:] = eps * C
+            H[j, i, 4:, :4] = eps * C.conj().T
+    return H
+
+
+def _random_gapped_grid(n1, n2, N=7, m=3, seed=0):
+    rng = np.random.default_rng(seed)
+    A = rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))
+    A0 = np.diag([-2.0] * m + [2.0] * (N - m)) + 0.15 * (A + A.conj().T)
+    T = [0.25 * (rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))) for _ in range(2)]
+    H = np.zeros((n2, n1, N, N), complex)
+    for j in range(n2):
+        for i in range(n1):
+            kx, ky = 2 * np.pi * i / n1, 2 * np.pi * j / n2
+            H[j, i] = (A0 + T[0] * np.exp(1j * kx) + T[0].conj().T * np.exp(-1j * kx)
+                       + T[1] * np.exp(1j * ky) + T[1].conj().T * np.exp(-1j * ky))
+    return H
+
+
+def test_nested_general_n_occ_above_two(ctx):
+    """S5 beyond the closed-form 2 x 2 case: Wannier-band vectors by inverse iteration on W - lambda I."""
+    H = _coupled_bbh_grid(24, 20)
+    th1o, thno = wo.nested_wilson(H, 4, wb_lo=0, wb_hi=2)
+    assert (th1o[:, 2] - th1o[:, 1]).min() > 0.5                      # Wannier gap between the selected pair and the rest
+    th1, thn = ctx.nested_wilson(dev(H[None]), 4, 1, 0, wb_lo=0, wb_hi=2)
+    assert phase_dist(th1.cpu().numpy()[0], th1o) <= PH_TOL
+    assert wo.circ_sorted_distance(thn.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
+    # upper pair, other base point
+    th1o, thno = wo.nested_wilson(H, 4, base=5, wb_lo=2, wb_hi=4)
+    th1, thn = ctx.nested_wilson(dev(H[None]), 4, 1, 0, base=5, wb_lo=2, wb_hi=4)
+    assert phase_dist(th1.cpu().numpy()[0], th1o) <= PH_TOL
+    assert wo.circ_sorted_distance(thn.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
+    # odd sizes, a single non-degenerate middle band
+    H = _random_gapped_grid(20, 16)
+    th1o, thno = wo.nested_wilson(H, 3, wb_lo=1, wb_hi=2)
+    assert min((th1o[:, 1] - th1o[:, 0]).min(), (th1o[:, 2] - th1o[:, 1]).min()) > 0.05
+    th1, thn = ctx.nested_wilson(dev(H[None]), 3, 1, 0, wb_lo=1, wb_hi=2)
+    assert phase_dist(th1.cpu().numpy()[0], th1o) <= PH_TOL
+    assert wo.circ_sorted_distance(thn.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
+    # all bands selected: the nested loop of the whole occupied space = plain loop along dir2 at fixed base
+    th1, thn = ctx.nested_wilson(dev(H[None]), 3, 1, 0, wb_lo=0, wb_hi=3)
+    _, thno = wo.nested_wilson(H, 3, wb_lo=0, wb_hi=3)
+    assert wo.circ_sorted_distance(thn.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
+    # larger occupied space (disordered BHZ supercell, N = 64, n_occ = 32), all 32 Wannier bands: the
+    # Hessenberg-QR + LU path at a size spanning several tiles; the span is the whole occupied space
+    H = wl.supercell_grid([wl.config3_parts(1, L=4)], 9, 6)[0]
+    th1o, thno = wo.nested_wilson(H, 32, wb_lo=0, wb_hi=32)
+    th1, thn = ctx.nested_wilson(dev(H[None]), 32, 1, 0, wb_lo=0, wb_hi=32)
+    assert phase_dist(th1.cpu().numpy()[0], th1o) <= PH_TOL
+    assert wo.circ_sorted_distance(thn.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
+
+
 # ------------------------------------------------------------------------------ config 3 (reduced)
 def test_config3_reduced_disordered_supercell(ctx):
     """N = 400, n_occ = 200, 2 realizations x 2 t2 x 33 t1 (full loop length, full matrix size)."""
