@@ -181,6 +181,23 @@ int be_winding(be_ctx* ctx, const double* d_theta, int64_t n_cycles, int n_point
                double* d_wind);
 
 /*
+ * Step before the path (the Bloch / supercell Hamiltonian at a
+ * wave vector, with boundary phases, is what the paper gets from PyBinding): H_grid assembled on the
+ * device from real-space blocks,
+ *     H[k] = sum_R coef[k][R] * A[R],     coef[k][R] = exp(2 pi i  t_k . R)   (t = reduced coordinates),
+ * as ONE complex GEMM (N^2 x nR) x (nR x count) on the FP64 tensor cores.
+ *   be_bloch_coefficients: d_t [count][nd] double reduced coordinates (nd = 1..3), h_R [nR][nd] int
+ *          lattice vectors on the HOST, d_coef [count][nR] complex128 out.
+ *   be_assemble_bloch: dA [nR][N][N] complex128 row-major blocks (the caller lists A_R and, for R != 0,
+ *          A_{-R} = A_R^dagger explicitly; twisted boundaries: the blocks of the wrapping hops with
+ *          R = +-e_x, +-e_y), d_coef as above (any complex coefficients are accepted), dH [count][N][N]
+ *          out.  Hermiticity of the result is the caller's (the blocks') responsibility.
+ */
+int be_bloch_coefficients(be_ctx* ctx, const double* d_t, const int* h_R, int nd, int nR, int64_t count,
+                          void* d_coef);
+int be_assemble_bloch(be_ctx* ctx, const void* dA, const void* d_coef, int64_t count, int N, int nR, void* dH);
+
+/*
  * Host-buffer variants (end-to-end path): h* pointers are host memory (pinned recommended).  The
  * grid is streamed to the device in chunks of whole loops, overlapped with compute on an internal
  * copy stream; results are copied back before return.  Semantics as the device calls above.

@@ -18,7 +18,7 @@ EXPORTS = [
     "be_create", "be_destroy", "be_strerror", "be_workspace_bytes", "be_set_workspace_limit",
     "be_launch_count", "be_eigh_batched", "be_wilson_loop", "be_nested_wilson",
     "be_spin_resolved_wilson", "be_winding", "be_wilson_loop_host", "be_spin_resolved_wilson_host",
-    "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched", "be_set_chunk_pipeline",
+    "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched", "be_set_chunk_pipeline", "be_bloch_coefficients", "be_assemble_bloch",
 ]
 
 
@@ -48,6 +48,8 @@ def load_library():
     lib.be_workspace_bytes.restype = C.c_size_t
     lib.be_set_workspace_limit.argtypes = [vp, C.c_size_t]
     lib.be_set_chunk_pipeline.argtypes = [vp, ci]
+    lib.be_bloch_coefficients.argtypes = [vp, vp, C.POINTER(ci), ci, ci, i64, vp]
+    lib.be_assemble_bloch.argtypes = [vp, vp, vp, i64, ci, ci, vp]
     lib.be_launch_count.argtypes = [vp]
     lib.be_launch_count.restype = i64
     lib.be_eigh_batched.argtypes = [vp, vp, i64, ci, ci, vp, vp, vp]
@@ -246,6 +248,24 @@ class Context:
                                                    _ptr(B), ldb, strideB, be, _ptr(C_out), ldc, strideC, batch,
                                                    1 if lower else 0))
         return C_out
+
+    # ------------------------------------------------------------------ H(k) assembly (NEXT-1)
+    def assemble_bloch(self, A, t, R):
+        """A [nR][N][N] complex128 blocks (device), t [count][nd] float64 reduced coordinates (device),
+        R [nR][nd] ints (host list / array) -> H [count][N][N] = sum_R exp(2 pi i t.R) A_R."""
+        _dev(A, torch.complex128, "A")
+        _dev(t, torch.float64, "t")
+        nR, N = A.shape[0], A.shape[-1]
+        count, nd = t.shape
+        Rl = [int(x) for row in R for x in row]
+        if len(Rl) != nR * nd:
+            raise ValueError("R must be [nR][nd]")
+        hR = (C.c_int * len(Rl))(*Rl)
+        coef = torch.empty((count, nR), dtype=torch.complex128, device=A.device)
+        _check(self.lib, self.lib.be_bloch_coefficients(self._h, _ptr(t), hR, nd, nR, count, _ptr(coef)))
+        H = torch.empty((count, N, N), dtype=torch.complex128, device=A.device)
+        _check(self.lib, self.lib.be_assemble_bloch(self._h, _ptr(A), _ptr(coef), count, N, nR, _ptr(H)))
+        return H
 
     # ------------------------------------------------------------------ be_winding
     def winding(self, theta):

@@ -254,3 +254,50 @@ extern "C" int be_zgemm_batched(be_ctx* ctx, int opA, int opB, int M, int N, int
   p.alpha = mkc(alpha[0], alpha[1]); p.beta = mkc(beta[0], beta[1]); p.lower = lower ? 1 : 0;
   return be_zgemm(ctx, opA, opB, p);
 }
+
+// ---------------------------------------------------------------------------------------------
+// NEXT-1: H(k) assembly as a GEMM
+namespace {
+__global__ void k_bloch_coef(const double* __restrict__ t, const int* __restrict__ R, int nd, int nR, int64_t count,
+                             cplx* __restrict__ coef) {
+  const int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (idx >= count * nR) return;
+  const int64_t k = idx / nR;
+  const int r = (int)(idx % nR);
+  double x = 0.0;
+  for (int a = 0; a < nd; ++a) x += t[k * nd + a] * (double)R[r * nd + a];
+  double s, c;
+  sincospi(2.0 * x, &s, &c);
+  coef[idx] = mkc(c, s);
+}
+}  // namespace
+
+extern "C" int be_bloch_coefficients(be_ctx* ctx, const double* d_t, const int* h_R, int nd, int nR, int64_t count,
+                                     void* d_coef) {
+  if (!ctx || !d_t || !h_R || !d_coef) return BE_ERR_NULL;
+  if (nd < 1 || nd > 3 || nR < 1 || count < 0) return BE_ERR_SHAPE;
+  if (!aligned(d_t, 8) || !aligned(d_coef, 16)) return BE_ERR_ALIGN;
+  if (count == 0) return BE_OK;
+  BE_TRY(be_arena_reserve(ctx, (size_t)nR * nd * sizeof(int) + 4096));
+  int* dR = (int*)be_arena_alloc(ctx, (size_t)nR * nd * sizeof(int));
+  if (!dR) return BE_ERR_NOMEM;
+  // small pageable copy: staged by the runtime before the call returns
+  BE_CUDA(cudaMemcpyAsync(dR, h_R, (size_t)nR * nd * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
+  const int64_t tot = count * nR;
+  k_bloch_coef<<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(d_t, dR, nd, nR, count, (cplx*)d_coef);
+  ctx->launches++;
+  return (int)cudaGetLastError();
+}
+
+extern "C" int be_assemble_bloch(be_ctx* ctx, const void* dA, const void* d_coef, int64_t count, int N, int nR,
+                                 void* dH) {
+  if (!ctx || !dA || !d_coef || !dH) return BE_ERR_NULL;
+  if (N < 1 || nR < 1 || count < 0 || (int64_t)N * N > 0x7fffffffLL || count > 0x7fffffffLL) return BE_ERR_SHAPE;
+  if (!aligned(dA, 16) || !aligned(d_coef, 16) || !aligned(dH, 16)) return BE_ERR_ALIGN;
+  if (count == 0) return BE_OK;
+  // column-major views: A' = dA as (N^2 x nR), B = d_coef as (nR x count), C = dH as (N^2 x count)
+  const int M = N * N;
+  ZgemmParams g = zgemm_simple(M, (int)count, nR, (const cplx*)dA, M, 0, (const cplx*)d_coef, nR, 0,
+                               (cplx*)dH, M, 0, 1);
+  return be_zgemm(ctx, BE_OP_N, BE_OP_N, g);
+}
