@@ -198,6 +198,22 @@ int be_bloch_coefficients(be_ctx* ctx, const double* d_t, const int* h_R, int nd
 int be_assemble_bloch(be_ctx* ctx, const void* dA, const void* d_coef, int64_t count, int N, int nR, void* dH);
 
 /*
+ * Plaquette mode ("integrated Berry flux through one plaquette",
+ * the coupling-matrix method and its spin-resolved generalization): on a periodic 2D grid
+ * (grid->ndim == 2, dims = (ny, nx)) every point is diagonalized ONCE and
+ *     flux[j][i] = arg det( L_x(j,i) L_y(j,i+1) L_x(j+1,i)^dagger L_y(j,i)^dagger )  in (-pi, pi],
+ *     L_x(j,i) = U(j,i)^dagger U(j,i+1),  L_y(j,i) = U(j,i)^dagger U(j+1,i)   (indices cyclic, R4: no
+ * unitarization; the determinant by partially pivoted LU).  sum(flux) / 2 pi is the Chern number in the
+ * orientation of the paper's Eq. 6 flow (Eq. 4: +1).
+ *   dS NULL: d_flux [batch][ny][nx] of the n_occ lowest bands; d_flux_hi, d_pso ignored.
+ *   dS given (S_is_diag / m_lo as in be_spin_resolved_wilson): d_flux = lower PSO sector, d_flux_hi =
+ *   upper sector (may be NULL), d_pso [batch][ny][nx][n_occ] (may be NULL).
+ * The whole grid has to fit the workspace cap (be_set_workspace_limit), else BE_ERR_UNSUPPORTED.
+ */
+int be_plaquette_flux(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_occ, const void* dS,
+                      int S_is_diag, int m_lo, double* d_flux, double* d_flux_hi, double* d_pso);
+
+/*
  * Host-buffer variants (end-to-end path): h* pointers are host memory (pinned recommended).  The
  * grid is streamed to the device in chunks of whole loops, overlapped with compute on an internal
  * copy stream; results are copied back before return.  Semantics as the device calls above.

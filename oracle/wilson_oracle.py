@@ -221,6 +221,48 @@ def nested_wilson(H_plane: np.ndarray, n_occ: int, base: int = 0, wb_lo: int = 0
 
 
 # ---------------------------------------------------------------------------------------------
+# NEXT-2: Berry flux through the plaquettes of a periodic grid ("integrated Berry
+# flux through one plaquette", the coupling-matrix method on a 20 x 20 grid)
+# ---------------------------------------------------------------------------------------------
+def plaquette_flux(H_plane: np.ndarray, n_occ: int, S=None, m_lo: int | None = None):
+    """H_plane [ny][nx][N][N] (periodic in both directions) -> flux [ny][nx] in (-pi, pi]:
+
+        flux[j][i] = arg det( U_ji^+ U_j,i+1 . U_j,i+1^+ U_j+1,i+1 . U_j+1,i+1^+ U_j+1,i . U_j+1,i^+ U_ji ),
+
+    the discretized loop of Eq. 2 around one plaquette, kx step first (links as in
+    ``wilson_matrix``: R2, R3, R4 -- no unitarization; det makes the result gauge invariant).
+    With ``S`` the frames are first rotated into the lower / upper PSO sectors (R10) and
+    (flux_lo, flux_hi) is returned ("spin-resolved generalization of the coupling matrix method").
+    sum(flux) / 2 pi is an integer: the Chern number in the orientation of the paper's Eq. 6 flow (R3).
+    """
+    ny, nx = H_plane.shape[:2]
+
+    def frames_at(j, i):
+        E, V = np.linalg.eigh(H_plane[j, i])
+        U = V[:, :n_occ]
+        if S is None:
+            return (U,)
+        Sm = np.asarray(S)
+        SU = Sm[:, None] * U if Sm.ndim == 1 else Sm @ U
+        sig, Vs = np.linalg.eigh(U.conj().T @ SU)
+        ml = n_occ // 2 if m_lo is None else m_lo
+        return (U @ Vs[:, :ml], U @ Vs[:, ml:])
+
+    F = [[frames_at(j, i) for i in range(nx)] for j in range(ny)]
+    nsec = len(F[0][0])
+    out = [np.empty((ny, nx)) for _ in range(nsec)]
+    for s in range(nsec):
+        for j in range(ny):
+            for i in range(nx):
+                a, b = F[j][i][s], F[j][(i + 1) % nx][s]
+                c, d = F[(j + 1) % ny][(i + 1) % nx][s], F[(j + 1) % ny][i][s]
+                W = (a.conj().T @ b) @ (b.conj().T @ c) @ (c.conj().T @ d) @ (d.conj().T @ a)
+                ph = np.angle(np.linalg.slogdet(W)[0])
+                out[s][j, i] = np.pi if ph <= -np.pi else ph
+    return out[0] if S is None else (out[0], out[1])
+
+
+# ---------------------------------------------------------------------------------------------
 # S7: invariants (PAPER.md:71-73 Eq. 6)
 # ---------------------------------------------------------------------------------------------
 def wrap_pi(x):

@@ -18,7 +18,7 @@ EXPORTS = [
     "be_create", "be_destroy", "be_strerror", "be_workspace_bytes", "be_set_workspace_limit",
     "be_launch_count", "be_eigh_batched", "be_wilson_loop", "be_nested_wilson",
     "be_spin_resolved_wilson", "be_winding", "be_wilson_loop_host", "be_spin_resolved_wilson_host",
-    "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched", "be_set_chunk_pipeline", "be_bloch_coefficients", "be_assemble_bloch",
+    "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched", "be_set_chunk_pipeline", "be_bloch_coefficients", "be_assemble_bloch", "be_plaquette_flux",
 ]
 
 
@@ -50,6 +50,7 @@ def load_library():
     lib.be_set_chunk_pipeline.argtypes = [vp, ci]
     lib.be_bloch_coefficients.argtypes = [vp, vp, C.POINTER(ci), ci, ci, i64, vp]
     lib.be_assemble_bloch.argtypes = [vp, vp, vp, i64, ci, ci, vp]
+    lib.be_plaquette_flux.argtypes = [vp, vp, gp, ci, vp, ci, ci, vp, vp, vp]
     lib.be_launch_count.argtypes = [vp]
     lib.be_launch_count.restype = i64
     lib.be_eigh_batched.argtypes = [vp, vp, i64, ci, ci, vp, vp, vp]
@@ -266,6 +267,28 @@ class Context:
         H = torch.empty((count, N, N), dtype=torch.complex128, device=A.device)
         _check(self.lib, self.lib.be_assemble_bloch(self._h, _ptr(A), _ptr(coef), count, N, nR, _ptr(H)))
         return H
+
+    # ------------------------------------------------------------------ be_plaquette_flux (NEXT-2)
+    def plaquette_flux(self, H_grid, n_occ, S=None, m_lo=-1, want_pso=False):
+        """H_grid [batch][ny][nx][N][N] (device) -> flux [batch][ny][nx]; with S: (flux_lo, flux_hi[, pso])."""
+        _dev(H_grid, torch.complex128, "H_grid")
+        if H_grid.dim() != 5:
+            raise ValueError("H_grid must be [batch][ny][nx][N][N]")
+        g = _grid_of(H_grid, 2)
+        shp = tuple(H_grid.shape[:3])
+        dev = H_grid.device
+        f0 = torch.empty(shp, dtype=torch.float64, device=dev)
+        if S is None:
+            _check(self.lib, self.lib.be_plaquette_flux(self._h, _ptr(H_grid), C.byref(g), n_occ, None, 0, -1,
+                                                        _ptr(f0), None, None))
+            return f0
+        is_diag = 1 if S.dim() == 1 else 0
+        _dev(S, torch.float64 if is_diag else torch.complex128, "S")
+        f1 = torch.empty(shp, dtype=torch.float64, device=dev)
+        pso = torch.empty(shp + (n_occ,), dtype=torch.float64, device=dev) if want_pso else None
+        _check(self.lib, self.lib.be_plaquette_flux(self._h, _ptr(H_grid), C.byref(g), n_occ, _ptr(S), is_diag, m_lo,
+                                                    _ptr(f0), _ptr(f1), _ptr(pso)))
+        return (f0, f1, pso) if want_pso else (f0, f1)
 
     # ------------------------------------------------------------------ be_winding
     def winding(self, theta):

@@ -51,6 +51,39 @@ static size_t per_loop_bytes(int N, int m, int n1, bool spin) {
   return b;
 }
 
+// S6, first half: S_red = U^H S U for cnt frames X, S_red = V Sigma V^H (ascending).
+// pso_out [cnt][m] receives Sigma (or scratch when NULL); *Vout [cnt][m][m] column-major.
+static int pso_eigenvectors(be_ctx* ctx, const cplx* X, int64_t cnt, int N, int m, const SpinArgs* sp,
+                            double* pso_out, cplx** Vout) {
+  cplx* SX = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
+  cplx* Sred = (cplx*)be_arena_alloc(ctx, (size_t)cnt * m * m * sizeof(cplx));
+  cplx* V = (cplx*)be_arena_alloc(ctx, (size_t)cnt * m * m * sizeof(cplx));
+  double* sig = pso_out ? pso_out : (double*)be_arena_alloc(ctx, (size_t)cnt * m * sizeof(double));
+  if (!SX || !Sred || !V || !sig) return BE_ERR_NOMEM;
+  if (sp->S_is_diag) {
+    BE_TRY(be_scale_rows(ctx, X, (const double*)sp->dS, SX, N, cnt * (int64_t)N * m));
+  } else {
+    // row-major S read column-major is S^T: op T recovers S;  SX = S X
+    ZgemmParams g = zgemm_simple(N, m, N, (const cplx*)sp->dS, N, 0, X, N, (int64_t)N * m,
+                                 SX, N, (int64_t)N * m, cnt);
+    BE_TRY(be_zgemm(ctx, BE_OP_T, BE_OP_N, g));
+  }
+  {
+    // the eigensolver reads its input row-major; a column-major buffer holding conj(S_red) =
+    // X^T conj(SX) is S_red when read row-major (S_red is Hermitian)
+    ZgemmParams g = zgemm_simple(m, m, N, X, N, (int64_t)N * m, SX, N, (int64_t)N * m,
+                                 Sred, m, (int64_t)m * m, cnt);
+    g.lower = 1;   // the eigensolver reads only the lower triangle of the column-major buffer
+    BE_TRY(be_zgemm(ctx, BE_OP_T, BE_OP_J, g));
+  }
+  GridMap fm;
+  memset(&fm, 0, sizeof(fm));
+  fm.ndim = 1; fm.dir = 0; fm.n1 = 1; fm.dims[0] = 1; fm.batch_stride = 1; fm.loops = cnt;
+  BE_TRY(be_eigh_frames(ctx, Sred, fm, 0, cnt, m, m, m, sig, V, nullptr));
+  *Vout = V;
+  return BE_OK;
+}
+
 static int wilson_chunk(be_ctx* ctx, const cplx* H, const GridMap& map, int N, int m, int n1, int64_t l0, int64_t nl,
                         int64_t cnt, const cplx* d_close, double* d_mingap, const SpinArgs* sp, int mlo, int mhi,
                         cplx* const* Wall);
@@ -158,35 +191,8 @@ static int wilson_chunk(be_ctx* ctx, const cplx* H, const GridMap& map, int N, i
       BE_TRY(be_chain_product(ctx, X, N, m, nl, n1, d_close, n1 - 1, Wall[0] + l0 * (int64_t)m * m, &W));
       return BE_OK;
     }
-    // ---- spin-resolved: S_red = U^H S U, diagonalize, rotate into sectors
-    cplx* SX = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
-    cplx* Sred = (cplx*)be_arena_alloc(ctx, (size_t)cnt * m * m * sizeof(cplx));
-    cplx* V = (cplx*)be_arena_alloc(ctx, (size_t)cnt * m * m * sizeof(cplx));
-    double* sig = sp->pso ? sp->pso + l0 * (int64_t)n1 * m
-                          : (double*)be_arena_alloc(ctx, (size_t)cnt * m * sizeof(double));
-    if (!SX || !Sred || !V || !sig) return BE_ERR_NOMEM;
-    if (sp->S_is_diag) {
-      BE_TRY(be_scale_rows(ctx, X, (const double*)sp->dS, SX, N, cnt * (int64_t)N * m));
-    } else {
-      // row-major S read column-major is S^T: op T recovers S;  SX = S X
-      ZgemmParams g = zgemm_simple(N, m, N, (const cplx*)sp->dS, N, 0, X, N, (int64_t)N * m,
-                                   SX, N, (int64_t)N * m, cnt);
-      BE_TRY(be_zgemm(ctx, BE_OP_T, BE_OP_N, g));
-    }
-    {
-      // the eigensolver reads its input row-major; a column-major buffer holding conj(S_red) =
-      // X^T conj(SX) is S_red when read row-major (S_red is Hermitian)
-      ZgemmParams g = zgemm_simple(m, m, N, X, N, (int64_t)N * m, SX, N, (int64_t)N * m,
-                                   Sred, m, (int64_t)m * m, cnt);
-      g.lower = 1;   // the eigensolver reads only the lower triangle of the column-major buffer
-      BE_TRY(be_zgemm(ctx, BE_OP_T, BE_OP_J, g));
-    }
-    {
-      GridMap fm;
-      memset(&fm, 0, sizeof(fm));
-      fm.ndim = 1; fm.dir = 0; fm.n1 = 1; fm.dims[0] = 1; fm.batch_stride = 1; fm.loops = cnt;
-      BE_TRY(be_eigh_frames(ctx, Sred, fm, 0, cnt, m, m, m, sig, V, nullptr));
-    }
+    cplx* V = nullptr;
+    BE_TRY(pso_eigenvectors(ctx, X, cnt, N, m, sp, sp->pso ? sp->pso + l0 * (int64_t)n1 * m : nullptr, &V));
     for (int sector = 0; sector < 2; ++sector) {
       const int ms = sector == 0 ? mlo : mhi;
       double* out = sector == 0 ? sp->theta_lo : sp->theta_hi;
@@ -307,5 +313,85 @@ extern "C" int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid*
   cplx* W2 = nullptr;
   BE_TRY(be_chain_product(ctx, Wf, N, ns, outer2, n2, (const cplx*)d_close2, n2 - 1, nullptr, &W2));
   BE_TRY(be_eigenphases(ctx, W2, outer2, ns, d_theta_nested, nullptr));
+  return BE_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// NEXT-2: plaquette Berry fluxes on a periodic 2D grid (include/berryeasy_b200.h)
+static ZgemmParams link_params(const cplx* A, const cplx* B, cplx* C, int M, int Nn, int K, int lda, int ldb,
+                               int64_t sAi, int64_t sAo, int64_t sBi, int64_t sBo, int64_t sCi, int64_t sCo,
+                               int inner, int64_t batch, int ring) {
+  ZgemmParams g = zgemm_simple(M, Nn, K, A, lda, sAo, B, ldb, sBo, C, M, sCo, batch);
+  g.sAi = sAi; g.sBi = sBi; g.sCi = sCi; g.inner = inner; g.ringB = ring; g.phi_at = -1;
+  return g;
+}
+
+// fluxes of one set of frames F [batch][ny][nx][ms][N]
+static int plaquette_of_frames(be_ctx* ctx, const cplx* F, int64_t batch, int ny, int nx, int N, int ms,
+                               double* d_flux) {
+  const int64_t pts = (int64_t)ny * nx, mm = (int64_t)ms * ms, fr = (int64_t)N * ms;
+  cplx* Lx = (cplx*)be_arena_alloc(ctx, (size_t)batch * pts * mm * sizeof(cplx));
+  cplx* Ly = (cplx*)be_arena_alloc(ctx, (size_t)batch * pts * mm * sizeof(cplx));
+  cplx* P1 = (cplx*)be_arena_alloc(ctx, (size_t)batch * pts * mm * sizeof(cplx));
+  cplx* P2 = (cplx*)be_arena_alloc(ctx, (size_t)batch * pts * mm * sizeof(cplx));
+  if (!Lx || !Ly || !P1 || !P2) return BE_ERR_NOMEM;
+  for (int64_t bt = 0; bt < batch; ++bt) {
+    const cplx* Fb = F + bt * pts * fr;
+    cplx *lx = Lx + bt * pts * mm, *ly = Ly + bt * pts * mm, *p1 = P1 + bt * pts * mm, *p2 = P2 + bt * pts * mm;
+    // L_x(j,i) = F(j,i)^H F(j,i+1): ring over i inside every row j
+    BE_TRY(be_zgemm(ctx, BE_OP_C, BE_OP_N, link_params(Fb, Fb, lx, ms, ms, N, N, N, fr, nx * fr, fr, nx * fr, mm, nx * mm, nx, pts, 1)));
+    // L_y(j,i) = F(j,i)^H F(j+1,i): ring over j inside every column i (stored [j][i] like L_x)
+    BE_TRY(be_zgemm(ctx, BE_OP_C, BE_OP_N, link_params(Fb, Fb, ly, ms, ms, N, N, N, nx * fr, fr, nx * fr, fr, nx * mm, mm, ny, pts, 1)));
+    // P1(j,i) = L_x(j,i) L_y(j,i+1)
+    BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_N, link_params(lx, ly, p1, ms, ms, ms, ms, ms, mm, nx * mm, mm, nx * mm, mm, nx * mm, nx, pts, 1)));
+    // P2(j,i) = P1(j,i) L_x(j+1,i)^H
+    BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_C, link_params(p1, lx, p2, ms, ms, ms, ms, ms, nx * mm, mm, nx * mm, mm, nx * mm, mm, ny, pts, 1)));
+    // P1 <- P2(j,i) L_y(j,i)^H: the closed loop around the plaquette
+    BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_C, link_params(p2, ly, p1, ms, ms, ms, ms, ms, mm, nx * mm, mm, nx * mm, mm, nx * mm, nx, pts, 0)));
+  }
+  return be_det_phase(ctx, P1, batch * pts, ms, d_flux);
+}
+
+extern "C" int be_plaquette_flux(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_occ, const void* dS,
+                                 int S_is_diag, int m_lo, double* d_flux, double* d_flux_hi, double* d_pso) {
+  BE_TRY(check_common(ctx, dH_grid, grid, n_occ, 0));
+  if (grid->ndim != 2 || !d_flux) return grid->ndim != 2 ? BE_ERR_SHAPE : BE_ERR_NULL;
+  const int ny = grid->dims[0], nx = grid->dims[1], N = grid->N, m = n_occ;
+  if (dS) {
+    if (m_lo < 0) m_lo = m / 2;
+    if (m_lo > m || !aligned(dS, S_is_diag ? 8 : 16)) return m_lo > m ? BE_ERR_SHAPE : BE_ERR_ALIGN;
+  }
+  GridMap map;
+  BE_TRY(make_map(grid, 1, &map));           // points enumerated [batch][ny][nx]
+  const int64_t cnt = grid->batch * ny * nx;
+  // everything of the grid is live at once (every point is a corner of four plaquettes)
+  const size_t mmax = (size_t)m * m * sizeof(cplx);
+  const size_t need = (size_t)cnt * (be_eigh_scratch_bytes(1, N, m) + 2 * (size_t)N * m * sizeof(cplx) + N * sizeof(double) +
+                                     (dS ? (size_t)N * m * sizeof(cplx) + 3 * mmax + be_eigh_scratch_bytes(1, m, m) : 0) +
+                                     6 * mmax + 4096) + (8 << 20);
+  if (need > ctx->ws_limit) return BE_ERR_UNSUPPORTED;   // the grid has to fit one chunk (header)
+  BE_TRY(be_arena_reserve(ctx, need));
+  double* E = (double*)be_arena_alloc(ctx, (size_t)cnt * N * sizeof(double));
+  cplx* X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
+  if (!E || !X) return BE_ERR_NOMEM;
+  BE_TRY(be_eigh_frames(ctx, (const cplx*)dH_grid, map, 0, cnt, N, m, m + 1, E, X, nullptr));
+  if (!dS) return plaquette_of_frames(ctx, X, grid->batch, ny, nx, N, m, d_flux);
+  SpinArgs sp{dS, S_is_diag, m_lo, nullptr, nullptr, d_pso};
+  cplx* V = nullptr;
+  BE_TRY(pso_eigenvectors(ctx, X, cnt, N, m, &sp, d_pso, &V));
+  const int msz[2] = {m_lo, m - m_lo};
+  double* outs[2] = {d_flux, d_flux_hi};
+  for (int sector = 0; sector < 2; ++sector) {
+    const int ms = msz[sector];
+    if (ms == 0 || !outs[sector]) continue;
+    const size_t mark = ctx->arena_used;
+    cplx* F = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * ms * sizeof(cplx));
+    if (!F) return BE_ERR_NOMEM;
+    ZgemmParams g = zgemm_simple(N, ms, m, X, N, (int64_t)N * m, V + (sector ? (int64_t)m_lo * m : 0), m,
+                                 (int64_t)m * m, F, N, (int64_t)N * ms, cnt);
+    BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_N, g));
+    BE_TRY(plaquette_of_frames(ctx, F, grid->batch, ny, nx, N, ms, outs[sector]));
+    ctx->arena_used = mark;
+  }
   return BE_OK;
 }

@@ -186,6 +186,7 @@ int be_eigenphases(be_ctx* ctx, cplx* W, int64_t cnt, int m, double* theta, doub
 size_t be_eigenphases_scratch_bytes(int64_t cnt, int m);
 int be_eigenvalues_general(be_ctx* ctx, cplx* W, int64_t cnt, int m, cplx* lam, int* fail);
 int be_sort_phases(be_ctx* ctx, const cplx* lam, int64_t cnt, int m, double* theta, double* absl);
+int be_det_phase(be_ctx* ctx, const cplx* W, int64_t cnt, int m, double* phase);
 size_t be_nested_general_scratch_bytes(int64_t nl, int m, int ns);
 int be_nested_select_general(be_ctx* ctx, cplx* W, int64_t nl, int m, int wb_lo, int wb_hi, double cut,
                              double* theta1, cplx* Vs);

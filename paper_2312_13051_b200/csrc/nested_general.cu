@@ -154,6 +154,28 @@ __global__ void __launch_bounds__(256) k_orth_bands(cplx* __restrict__ Vs, int m
   }
 }
 
+// phase[b] = arg det A = sum_k arg U_kk + pi * (number of row interchanges), wrapped to (-pi, pi]
+__global__ void k_det_phase(const cplx* __restrict__ LU, const int* __restrict__ piv, int m, double* __restrict__ phase) {
+  __shared__ double red[33];
+  const int64_t b = blockIdx.x;
+  const cplx* A = LU + b * (int64_t)m * m;
+  const int* pv = piv + b * (int64_t)m;
+  double acc = 0.0;
+  for (int k = threadIdx.x; k < m; k += blockDim.x) {
+    const cplx u = A[k + (int64_t)k * m];
+    acc += atan2(u.y, u.x);
+    if (pv[k] != k) acc += M_PI;
+  }
+  acc = block_sum(acc, red);
+  if (threadIdx.x == 0) {
+    double t = fmod(acc + M_PI, 2.0 * M_PI);
+    if (t < 0.0) t += 2.0 * M_PI;
+    t -= M_PI;
+    if (t <= -M_PI) t = M_PI;
+    phase[b] = t;
+  }
+}
+
 }  // namespace
 
 #define LAUNCH_CHECK() do { ctx->launches++; cudaError_t e__ = cudaGetLastError(); if (e__ != cudaSuccess) return (int)e__; } while (0)
@@ -195,5 +217,19 @@ int be_nested_select_general(be_ctx* ctx, cplx* W, int64_t nl, int m, int wb_lo,
     k_orth_bands<<<(unsigned)nl, 256, 0, st>>>(Vs, m, ns);
     LAUNCH_CHECK();
   }
+  return BE_OK;
+}
+
+// phase [cnt] = arg det of cnt column-major m x m matrices W (not modified), by partially pivoted LU.
+int be_det_phase(be_ctx* ctx, const cplx* W, int64_t cnt, int m, double* phase) {
+  cplx* LU = (cplx*)be_arena_alloc(ctx, (size_t)cnt * m * m * sizeof(cplx));
+  int* piv = (int*)be_arena_alloc(ctx, (size_t)cnt * m * sizeof(int));
+  cplx* zero = (cplx*)be_arena_alloc(ctx, (size_t)cnt * sizeof(cplx));
+  if (!LU || !piv || !zero) return BE_ERR_NOMEM;
+  BE_CUDA(cudaMemsetAsync(zero, 0, (size_t)cnt * sizeof(cplx), ctx->stream));
+  k_lu_shifted<<<(unsigned)cnt, 256, 0, ctx->stream>>>(W, zero, m, 1, LU, piv);
+  LAUNCH_CHECK();
+  k_det_phase<<<(unsigned)cnt, 128, 0, ctx->stream>>>(LU, piv, m, phase);
+  LAUNCH_CHECK();
   return BE_OK;
 }

@@ -515,6 +515,35 @@ def test_assemble_bloch_matches_the_input_recipe(ctx):
     assert np.abs(H - H.conj().transpose(0, 2, 1)).max() < 1e-13
 
 
+def test_plaquette_flux_matches_oracle(ctx):
+    """NEXT-2: plaquette Berry fluxes (coupling-matrix method), plain and spin resolved."""
+    G = wl.qwz_grid(20, 20)                                            # Eq. 4, m = 1
+    f = ctx.plaquette_flux(dev(G[None]), 1).cpu().numpy()[0]
+    fo = wo.plaquette_flux(G, 1)
+    assert np.abs(wo.wrap_pi(f - fo)).max() <= PH_TOL * 2 * np.pi
+    assert round(f.sum() / (2 * np.pi)) == 1                           # C = 1 (PAPER.md:67, 91)
+    H = wl.config1_grid(16, 12)                                        # BHZ, m = 2 -> sectors 1 + 1
+    f = ctx.plaquette_flux(dev(H[None]), 2).cpu().numpy()[0]
+    assert np.abs(wo.wrap_pi(f - wo.plaquette_flux(H, 2))).max() <= PH_TOL * 2 * np.pi
+    flo, fhi, pso = ctx.plaquette_flux(dev(H[None]), 2, dev(wl.bhz4_spin_z()), want_pso=True)
+    floo, fhio = wo.plaquette_flux(H, 2, wl.bhz4_spin_z())
+    assert np.abs(wo.wrap_pi(flo.cpu().numpy()[0] - floo)).max() <= PH_TOL * 2 * np.pi
+    assert np.abs(wo.wrap_pi(fhi.cpu().numpy()[0] - fhio)).max() <= PH_TOL * 2 * np.pi
+    assert (round(flo.sum().item() / (2 * np.pi)), round(fhi.sum().item() / (2 * np.pi))) == (-1, 1)
+    assert np.abs(np.abs(pso.cpu().numpy()) - 1).max() < 1e-12
+    # disordered supercell, two realizations in the batch, ragged grid, tridiagonalization path + LU of 32 x 32
+    parts = [wl.config3_parts(r, L=4) for r in (0, 1)]
+    Hs = wl.supercell_grid(parts, 5, 4)                                # [2][4][5][64][64]
+    f = ctx.plaquette_flux(dev(Hs), 32).cpu().numpy()
+    for r in range(2):
+        assert np.abs(wo.wrap_pi(f[r] - wo.plaquette_flux(Hs[r], 32))).max() <= PH_TOL * 2 * np.pi
+    S = wl.supercell_spin_z(4)
+    flo, fhi = ctx.plaquette_flux(dev(Hs), 32, dev(S))
+    floo, fhio = wo.plaquette_flux(Hs[1], 32, S)
+    assert np.abs(wo.wrap_pi(flo.cpu().numpy()[1] - floo)).max() <= PH_TOL * 2 * np.pi
+    assert np.abs(wo.wrap_pi(fhi.cpu().numpy()[1] - fhio)).max() <= PH_TOL * 2 * np.pi
+
+
 def test_launch_counter_counts_kernels(ctx):
     n0 = ctx.launch_count()
     ctx.wilson_loop(dev(wl.config1_grid(6, 2)[None]), 2, 1)

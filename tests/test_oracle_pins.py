@@ -112,6 +112,37 @@ def test_qwz_chern_matches_berry_curvature_plaquette_sum():
     assert wo.chern_number(th) == int(round(C_curv))
 
 
+def test_plaquette_flux_chern_number_and_stokes():
+    """NEXT-2: plaquette fluxes.  Pins: (i) Eq. 4: sum of the fluxes / 2 pi = C = 1
+    (PAPER.md:67, 91); (ii) closed-form lower-band vectors give the same flux plaquette by plaquette;
+    (iii) Stokes on a row of plaquettes, exact at finite grids because det is Abelian:
+    sum_i flux[j][i] = Theta_j - Theta_{j+1} (mod 2 pi) with Theta = sum_n theta_n of the kx loops;
+    (iv) BHZ: sector Chern numbers -1 / +1 = -winding (R3), total 0."""
+    n = 20
+    G = wl.qwz_grid(n, n)
+    f = wo.plaquette_flux(G, 1)
+    assert abs(f.sum() / (2 * np.pi) - int(GOLD["qwz_eq4_chern"])) < 1e-12
+    ks = 2 * np.pi * np.arange(n) / n
+    u = [[lower_band_vector(qwz_d(kx, ky)) for kx in ks] for ky in ks]        # [ky][kx]
+    for (j, i) in ((0, 0), (3, 17), (19, 19)):
+        a, b = u[j][i], u[j][(i + 1) % n]
+        c, d = u[(j + 1) % n][(i + 1) % n], u[(j + 1) % n][i]
+        ref = np.angle(np.vdot(a, b) * np.vdot(b, c) * np.vdot(c, d) * np.vdot(d, a))
+        assert abs(wo.wrap_pi(f[j, i] - ref)) < 1e-12
+    th, _, _ = wo.wilson_surface(G[None], 1, 1)
+    Th = th.sum(1)
+    assert np.abs(wo.wrap_pi(f.sum(1) - (Th - np.roll(Th, -1)))).max() < 1e-12
+    H = wl.config1_grid(16, 12)
+    th, _, _ = wo.wilson_surface(H[None], 2, 1)
+    Th = th.sum(1)
+    assert np.abs(wo.wrap_pi(wo.plaquette_flux(H, 2).sum(1) - (Th - np.roll(Th, -1)))).max() < 1e-12
+    flo, fhi = wo.plaquette_flux(H, 2, wl.bhz4_spin_z())
+    clo, chi = flo.sum() / (2 * np.pi), fhi.sum() / (2 * np.pi)
+    assert abs(clo + 1) < 1e-12 and abs(chi - 1) < 1e-12
+    lo, hi, _ = wo.spin_resolved_surface(H[None], 2, 1, wl.bhz4_spin_z())
+    assert wo.chern_number(lo) == round(clo) and wo.chern_number(hi) == round(chi)
+
+
 def test_abelian_loop_equals_scalar_product_of_closed_form_vectors():
     """m = 1: W = prod_j <u_j|u_{j+1}> is a scalar; u from the closed form, not from eigh."""
     n1 = 37
