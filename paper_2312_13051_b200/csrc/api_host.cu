@@ -31,18 +31,8 @@ int host_run(be_ctx* ctx, const void* hH, const be_grid* grid, int n_occ, int di
   } else if (!h_a) return BE_ERR_NULL;
   if (!ctx->copy_stream) BE_CUDA(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
 
-  const size_t per = be_wilson_per_loop_bytes(N, m, n1, spin ? 1 : 0);
   const size_t loop_bytes = (size_t)n1 * N * N * sizeof(cplx);
-  // leave room for the two staging buffers next to the work arena
-  int64_t lc = (int64_t)(ctx->ws_limit / (per + 2 * loop_bytes));
-  if (lc < 1) lc = 1;
-  if (lc > loops) lc = loops;
-  const int64_t nchunks = (loops + lc - 1) / lc;
-  lc = (loops + nchunks - 1) / nchunks;
-
-  DevBuf stage[2], dS, dclose, da, db, dc;
-  BE_TRY(stage[0].alloc(loop_bytes * lc));
-  if (nchunks > 1) BE_TRY(stage[1].alloc(loop_bytes * lc));
+  DevBuf dS, dclose, da, db, dc;
   const int mlo = spin ? m_lo : 0, mhi = spin ? m - m_lo : 0;
   if (spin) {
     const size_t sb = S_is_diag ? (size_t)N * sizeof(double) : (size_t)N * N * sizeof(cplx);
@@ -60,41 +50,21 @@ int host_run(be_ctx* ctx, const void* hH, const be_grid* grid, int n_occ, int di
     BE_TRY(dclose.alloc((size_t)N * sizeof(cplx)));
     BE_CUDA(cudaMemcpyAsync(dclose.p, h_close, (size_t)N * sizeof(cplx), cudaMemcpyHostToDevice, ctx->stream));
   }
-  cudaEvent_t copied[2], freed[2];
+  // The chunking, the scratch arena and the single eigenphase solve at the end are those of the device
+  // entry points; the chunks' matrices come through two staging buffers filled on the copy stream.
+  HostStage hs;
+  memset(&hs, 0, sizeof(hs));
+  hs.hH = (const char*)hH;
+  hs.loop_bytes = loop_bytes;
   for (int i = 0; i < 2; ++i) {
-    BE_CUDA(cudaEventCreateWithFlags(&copied[i], cudaEventDisableTiming));
-    BE_CUDA(cudaEventCreateWithFlags(&freed[i], cudaEventDisableTiming));
+    BE_CUDA(cudaEventCreateWithFlags(&hs.copied[i], cudaEventDisableTiming));
+    BE_CUDA(cudaEventCreateWithFlags(&hs.freed[i], cudaEventDisableTiming));
   }
-  int rc = BE_OK;
-  auto issue_copy = [&](int64_t ci) -> int {
-    const int b = (int)(ci & 1);
-    const int64_t l0 = ci * lc, nl = (loops - l0 < lc) ? loops - l0 : lc;
-    if (ci >= 2) BE_CUDA(cudaStreamWaitEvent(ctx->copy_stream, freed[b], 0));
-    BE_CUDA(cudaMemcpyAsync(stage[b].p, (const char*)hH + (size_t)l0 * loop_bytes, (size_t)nl * loop_bytes,
-                            cudaMemcpyHostToDevice, ctx->copy_stream));
-    BE_CUDA(cudaEventRecord(copied[b], ctx->copy_stream));
-    return BE_OK;
-  };
-  rc = issue_copy(0);
-  for (int64_t ci = 0; ci < nchunks && rc == BE_OK; ++ci) {
-    const int b = (int)(ci & 1);
-    const int64_t l0 = ci * lc, nl = (loops - l0 < lc) ? loops - l0 : lc;
-    if (ci + 1 < nchunks) { rc = issue_copy(ci + 1); if (rc != BE_OK) break; }
-    rc = (int)cudaStreamWaitEvent(ctx->stream, copied[b], 0);
-    if (rc != BE_OK) break;
-    be_grid g;
-    g.ndim = 1; g.batch = nl; g.dims[0] = n1; g.dims[1] = g.dims[2] = 1; g.N = N;
-    if (spin)
-      rc = be_spin_resolved_wilson(ctx, stage[b].p, &g, m, 0, dS.p, S_is_diag, m_lo, dclose.p,
-                                   da.p ? (double*)da.p + l0 * mlo : nullptr,
-                                   db.p && h_b ? (double*)db.p + l0 * mhi : nullptr,
-                                   dc.p && h_c ? (double*)dc.p + l0 * (int64_t)n1 * m : nullptr);
-    else
-      rc = be_wilson_loop(ctx, stage[b].p, &g, m, 0, dclose.p, (double*)da.p + l0 * m,
-                          h_b ? (double*)db.p + l0 * m : nullptr, h_c ? (double*)dc.p + l0 : nullptr);
-    if (rc != BE_OK) break;
-    rc = (int)cudaEventRecord(freed[b], ctx->stream);
-  }
+  int rc = be_wilson_host_device(ctx, &hs, loops, n1, N, m, dclose.p,
+                                 spin ? nullptr : (double*)da.p, spin ? nullptr : (double*)db.p,
+                                 spin ? nullptr : (double*)dc.p, dS.p, S_is_diag, m_lo,
+                                 spin ? (double*)da.p : nullptr, spin ? (double*)db.p : nullptr,
+                                 spin ? (double*)dc.p : nullptr, spin ? 1 : 0);
   if (rc == BE_OK) {
     cudaStream_t st = ctx->stream;
     if (spin) {
@@ -110,7 +80,10 @@ int host_run(be_ctx* ctx, const void* hH, const be_grid* grid, int n_occ, int di
   cudaStreamSynchronize(ctx->copy_stream);
   const cudaError_t se = cudaStreamSynchronize(ctx->stream);
   if (rc == BE_OK && se != cudaSuccess) rc = (int)se;
-  for (int i = 0; i < 2; ++i) { cudaEventDestroy(copied[i]); cudaEventDestroy(freed[i]); }
+  for (int i = 0; i < 2; ++i) {
+    cudaEventDestroy(hs.copied[i]); cudaEventDestroy(hs.freed[i]);
+    if (hs.stage[i]) cudaFree(hs.stage[i]);
+  }
   return rc;
 }
 

@@ -84,9 +84,9 @@ static int pso_eigenvectors(be_ctx* ctx, const cplx* X, int64_t cnt, int N, int 
   return BE_OK;
 }
 
-static int wilson_chunk(be_ctx* ctx, const cplx* H, const GridMap& map, int N, int m, int n1, int64_t l0, int64_t nl,
-                        int64_t cnt, const cplx* d_close, double* d_mingap, const SpinArgs* sp, int mlo, int mhi,
-                        cplx* const* Wall);
+static int wilson_chunk(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t gl0, int N, int m, int n1, int64_t l0,
+                        int64_t nl, int64_t cnt, const cplx* d_close, double* d_mingap, const SpinArgs* sp, int mlo,
+                        int mhi, cplx* const* Wall);
 
 static int pipeline_init(be_ctx* ctx) {
   if (ctx->stream2) return BE_OK;
@@ -103,7 +103,7 @@ static int pipeline_init(be_ctx* ctx) {
 // One pass over all loops of ``map`` (device H).  Plain loop when ``sp`` is NULL.
 static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, int m,
                          const cplx* d_close, double* d_theta, double* d_abs, double* d_mingap,
-                         const SpinArgs* sp) {
+                         const SpinArgs* sp, HostStage* hs = nullptr) {
   const int n1 = map.n1;
   const int64_t loops = map.loops;
   const size_t per = per_loop_bytes(N, m, n1, sp != nullptr);
@@ -123,7 +123,25 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   // Chunk pipeline (more than one chunk): two scratch regions used alternately, the
   // tridiagonalization of chunk c+1 on the caller's stream overlaps the rest of chunk c on stream2.
   const size_t region = be_align256(per * (size_t)lc);
-  bool pipe = nchunks > 1 && ctx->chunk_pipeline;
+  bool pipe = nchunks > 1 && ctx->chunk_pipeline && !hs;
+  // host-resident grid: staging buffers for lc loops each, next to the work arena
+  GridMap smap;
+  auto issue_copy = [&](int64_t ci) -> int {
+    const int b = (int)(ci & 1);
+    const int64_t c0 = ci * lc, cn = (loops - c0 < lc) ? loops - c0 : lc;
+    if (ci >= 2) BE_CUDA(cudaStreamWaitEvent(ctx->copy_stream, hs->freed[b], 0));
+    BE_CUDA(cudaMemcpyAsync(hs->stage[b], hs->hH + (size_t)c0 * hs->loop_bytes, (size_t)cn * hs->loop_bytes,
+                            cudaMemcpyHostToDevice, ctx->copy_stream));
+    BE_CUDA(cudaEventRecord(hs->copied[b], ctx->copy_stream));
+    return BE_OK;
+  };
+  if (hs) {
+    for (int b = 0; b < (nchunks > 1 ? 2 : 1); ++b)
+      if (cudaMalloc(&hs->stage[b], (size_t)lc * hs->loop_bytes) != cudaSuccess) { cudaGetLastError(); return BE_ERR_NOMEM; }
+    memset(&smap, 0, sizeof(smap));
+    smap.ndim = 1; smap.dir = 0; smap.n1 = n1; smap.dims[0] = n1; smap.stride[0] = 1; smap.batch_stride = n1; smap.loops = lc;
+    BE_TRY(issue_copy(0));
+  }
   if (pipe) {
     BE_TRY(pipeline_init(ctx));
     if (be_arena_reserve(ctx, 2 * region + persist + (4 << 20)) != BE_OK) pipe = false;   // not enough memory: serial
@@ -148,7 +166,15 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
       ctx->split_after_tridiag = 1;
       ctx->gemm_pad = (l0 + lc < loops && N > 8) ? 1 : 0;   // a next chunk will stream its matrices next to these GEMMs
     }
-    const int rc = wilson_chunk(ctx, H, map, N, m, n1, l0, nl, cnt, d_close, d_mingap, sp, mlo, mhi, Wall);
+    const cplx* Hc = H;
+    if (hs) {
+      if (ci + 1 < nchunks) BE_TRY(issue_copy(ci + 1));
+      BE_CUDA(cudaStreamWaitEvent(ctx->stream, hs->copied[ci & 1], 0));
+      Hc = (const cplx*)hs->stage[ci & 1];
+    }
+    const int rc = wilson_chunk(ctx, Hc, hs ? smap : map, hs ? 0 : l0, N, m, n1, l0, nl, cnt, d_close, d_mingap, sp, mlo,
+                                mhi, Wall);
+    if (hs && rc == BE_OK) cudaEventRecord(hs->freed[ci & 1], ctx->stream);
     if (pipe) {
       ctx->split_after_tridiag = 0;
       if (rc == BE_OK) cudaEventRecord(ctx->ev_region[ci & 1], ctx->stream);
@@ -177,14 +203,15 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
 }
 
 // One chunk of nl whole loops (cnt = nl * n1 matrices): S1, then S6 (if sp), S2, S3 into Wall.
-static int wilson_chunk(be_ctx* ctx, const cplx* H, const GridMap& map, int N, int m, int n1, int64_t l0, int64_t nl,
-                        int64_t cnt, const cplx* d_close, double* d_mingap, const SpinArgs* sp, int mlo, int mhi,
-                        cplx* const* Wall) {
+// gl0: first loop of the chunk inside (H, map); l0: first loop of the chunk in the outputs.
+static int wilson_chunk(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t gl0, int N, int m, int n1, int64_t l0,
+                        int64_t nl, int64_t cnt, const cplx* d_close, double* d_mingap, const SpinArgs* sp, int mlo,
+                        int mhi, cplx* const* Wall) {
   {
     double* E = (double*)be_arena_alloc(ctx, (size_t)cnt * N * sizeof(double));
     cplx* X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
     if (!E || !X) return BE_ERR_NOMEM;
-    BE_TRY(be_eigh_frames(ctx, H, map, l0, cnt, N, m, m + 1, E, X, nullptr));
+    BE_TRY(be_eigh_frames(ctx, H, map, gl0, cnt, N, m, m + 1, E, X, nullptr));
     if (d_mingap) BE_TRY(be_mingap(ctx, E, N, m, n1, nl, d_mingap + l0));
     if (!sp) {
       cplx* W = nullptr;
@@ -394,4 +421,16 @@ extern "C" int be_plaquette_flux(be_ctx* ctx, const void* dH_grid, const be_grid
     ctx->arena_used = mark;
   }
   return BE_OK;
+}
+
+// host-resident grid (api_host.cu): same chunking, deferred eigenphases and scratch as the device path
+int be_wilson_host_device(be_ctx* ctx, HostStage* hs, int64_t loops, int n1, int N, int m, const void* d_close,
+                          double* d_theta, double* d_abs, double* d_mingap, const void* dS, int S_is_diag, int m_lo,
+                          double* d_theta_lo, double* d_theta_hi, double* d_pso, int spin) {
+  GridMap map;
+  memset(&map, 0, sizeof(map));
+  map.ndim = 1; map.dir = 0; map.n1 = n1; map.dims[0] = n1; map.stride[0] = 1; map.batch_stride = n1; map.loops = loops;
+  if (!spin) return wilson_device(ctx, nullptr, map, N, m, (const cplx*)d_close, d_theta, d_abs, d_mingap, nullptr, hs);
+  SpinArgs sp{dS, S_is_diag, m_lo, d_theta_lo, d_theta_hi, d_pso};
+  return wilson_device(ctx, nullptr, map, N, m, (const cplx*)d_close, nullptr, nullptr, nullptr, &sp, hs);
 }

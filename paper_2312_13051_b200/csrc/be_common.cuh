@@ -169,6 +169,18 @@ __host__ __device__ inline int64_t gridmap_index(const GridMap& g, int64_t loop,
 }
 
 // ---------------------------------------------------------------------------------------------
+// Host-resident H_grid streamed chunk by chunk (be_*_host): two device staging buffers filled on the
+// copy stream while the previous chunk computes.  Loops must be contiguous (dir == last axis).
+struct HostStage {
+  const char* hH;          // host grid
+  size_t loop_bytes;       // n1 * N * N * 16
+  void* stage[2];          // device staging buffers, lc loops each (filled by be_wilson_host_device)
+  cudaEvent_t copied[2], freed[2];
+};
+int be_wilson_host_device(be_ctx* ctx, HostStage* hs, int64_t loops, int n1, int N, int m, const void* d_close,
+                          double* d_theta, double* d_abs, double* d_mingap, const void* dS, int S_is_diag, int m_lo,
+                          double* d_theta_lo, double* d_theta_hi, double* d_pso, int spin);
+
 // Stage entry points (host functions enqueueing kernels on ctx->stream)
 
 // Frames-producing eigensolve for ``cnt`` matrices gathered from H via (loop0.., map):
