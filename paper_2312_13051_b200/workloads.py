@@ -255,6 +255,32 @@ def supercell_grid_torch(parts_list, n1: int, n2: int, device, t2_indices=None):
 
 
 # --------------------------------------------------------------------------------------------
+# Eq. 9: chiral higher-order topological insulator, second validation model
+# --------------------------------------------------------------------------------------------
+def chiral_hoti(kx: float, ky: float, kz: float, delta0: float = 1.0) -> np.ndarray:
+    """H(k)/t = sin kx s1 x t1 + sin ky s1 x t2 + sin kz s1 x t3 + (cos kx + cos ky + cos kz - 1.5) s3 x t0
+    + Delta0 (cos kx - cos ky) s2 x t0, with A x B = np.kron(A, B) (R12: first factor slow)."""
+    return (np.sin(kx) * np.kron(sx, sx) + np.sin(ky) * np.kron(sx, sy) + np.sin(kz) * np.kron(sx, sz)
+            + (np.cos(kx) + np.cos(ky) + np.cos(kz) - 1.5) * np.kron(sz, s0)
+            + delta0 * (np.cos(kx) - np.cos(ky)) * np.kron(sy, s0))
+
+
+def chiral_hoti_spin() -> np.ndarray:
+    """s = sigma_3 x tau_3 = diag(1, -1, -1, 1), as a real diagonal."""
+    return np.real(np.diag(np.kron(sz, sz))).copy()
+
+
+def chiral_hoti_grid(n1: int, n2: int, kzs, delta0: float = 1.0) -> np.ndarray:
+    """[len(kzs)][n2 ky][n1 kx][4][4]; kz given in reduced units t3 (kz = 2 pi t3), loops run along kx."""
+    H = np.empty((len(kzs), n2, n1, 4, 4), dtype=np.complex128)
+    for a, t3 in enumerate(kzs):
+        for j in range(n2):
+            for i in range(n1):
+                H[a, j, i] = chiral_hoti(2 * np.pi * i / n1, 2 * np.pi * j / n2, 2 * np.pi * t3, delta0)
+    return H
+
+
+# --------------------------------------------------------------------------------------------
 # config 5: synthetic Wannier-like 64-orbital cubic model
 # --------------------------------------------------------------------------------------------
 def config5_half_space_vectors():

@@ -544,6 +544,29 @@ def test_plaquette_flux_matches_oracle(ctx):
     assert np.abs(wo.wrap_pi(fhi.cpu().numpy()[1] - fhio)).max() <= PH_TOL * 2 * np.pi
 
 
+def test_chiral_hoti_eq9_on_device(ctx):
+    """NEXT-4: the paper's second worked example (Eq. 9) through the C ABI: nested loops for 20 k_z slices
+    in one batched call, spin-resolved surface at k_z = 0; invariants exact, phases against the oracle."""
+    kzs = [j / 20 for j in range(20)]
+    Hz = wl.chiral_hoti_grid(24, 24, kzs, 1.0)                              # [20][24][24][4][4]
+    th1, thn = ctx.nested_wilson(dev(Hz), 2, 1, 0)                          # batch = k_z
+    thn = thn.cpu().numpy()
+    for a in (0, 3, 11, 19):
+        th1o, thno = wo.nested_wilson(Hz[a], 2)
+        assert phase_dist(th1.cpu().numpy()[a], th1o) <= PH_TOL
+        assert wo.circ_sorted_distance(thn[a], thno) / (2 * np.pi) <= PH_TOL
+    w = ctx.winding(dev(thn[None])).item()
+    assert abs(w - round(w)) < 1e-9 and abs(round(w)) == 1                   # gapless nested spectrum (PAPER.md:150)
+    H = wl.chiral_hoti_grid(32, 32, [0.0], 1.0)
+    S = wl.chiral_hoti_spin()
+    lo, hi, pso = ctx.spin_resolved_wilson(dev(H), 2, 1, dev(S))
+    loo, hio, psoo = wo.spin_resolved_surface(H, 2, 1, S)
+    assert phase_dist(lo.cpu().numpy(), loo) <= PH_TOL and phase_dist(hi.cpu().numpy(), hio) <= PH_TOL
+    assert np.abs(pso.cpu().numpy() - psoo).max() < 1e-12
+    wlo, whi = ctx.winding(lo[None]).item(), ctx.winding(hi[None]).item()
+    assert sorted((round(wlo), round(whi))) == [-1, 1]                       # |C_s| = 1 (PAPER.md:164)
+
+
 def test_launch_counter_counts_kernels(ctx):
     n0 = ctx.launch_count()
     ctx.wilson_loop(dev(wl.config1_grid(6, 2)[None]), 2, 1)

@@ -366,6 +366,34 @@ def test_bbh_nested_polarization(gamma, key):
     assert np.allclose(nu[:, 0], -nu[:, 1], atol=1e-10)
 
 
+def test_chiral_hoti_eq9_validation_model():
+    """NEXT-4, Eq. 9: (a) Delta_0 = 1, k_z = 0: the WCC spectrum is gapped (PAPER.md:142,
+    Fig. 4(a)) although (b) |C_s| = 1 with s = sigma_3 x tau_3 = diag(1,-1,-1,1) and a PSO whose
+    eigenvalues left +-1 but stay gapped; (c) Delta_0 = 0, k_z = 0 is the BHZ-like QSH
+    plane with a gapless (connected) WCC spectrum; (d) the nested Wilson loop along k_y of
+    the lower Wannier band is gapless as a function of k_z: it winds once (Fig. 4(b))."""
+    n = 32
+    S = wl.chiral_hoti_spin()
+    assert np.array_equal(S, np.array([1.0, -1.0, -1.0, 1.0]))            # op = np.diag([1,-1,-1,1]), PAPER.md:170
+    H = wl.chiral_hoti_grid(n, n, [0.0], 1.0)
+    th, _, mg = wo.wilson_surface(H, 2, 1)
+    assert mg.min() > 1.0
+    assert np.abs(th).min() > 0.3 and np.abs(th).max() < np.pi - 0.3        # (a) gaps around 0 and pi for all k_y
+    assert wo.chern_number(th) == 0
+    lo, hi, pso = wo.spin_resolved_surface(H, 2, 1, S)
+    assert abs(wo.chern_number(lo)) == abs(wo.chern_number(hi)) == int(GOLD["hoti_abs_spin_chern"])   # (b)
+    assert wo.chern_number(lo) + wo.chern_number(hi) == 0
+    assert np.abs(np.abs(pso) - 1).max() > 1e-3 and (pso[..., 1] - pso[..., 0]).min() > 0.4
+    H0 = wl.chiral_hoti_grid(n, 96, [0.0], 0.0)
+    th0, _, _ = wo.wilson_surface(H0, 2, 1)
+    pts = np.sort(np.mod(th0.ravel(), 2 * np.pi))
+    assert np.diff(np.concatenate([pts, [pts[0] + 2 * np.pi]])).max() < 0.5   # (c) no empty arc: connected spectrum
+    kzs = [j / 20 for j in range(20)]
+    Hz = wl.chiral_hoti_grid(24, 24, kzs, 1.0)
+    nested = np.array([wo.nested_wilson(Hz[a], 2)[1] for a in range(20)])   # [20][1]
+    assert abs(wo.chern_number(nested)) == int(GOLD["hoti_nested_abs_winding"])   # (d)
+
+
 def test_nested_first_level_matches_plain_surface():
     H = wl.config2_grid(24, 20)
     th1, _ = wo.nested_wilson(H, 2)
