@@ -19,6 +19,7 @@
 // B is reduced on its lower triangle; eigenvectors of H are the conjugates of those of B, which
 // is obtained for free by back-transforming with conjugated reflectors (Z is real).
 #include "be_common.cuh"
+#include "tma.cuh"
 #include <float.h>
 
 namespace {
@@ -67,30 +68,6 @@ constexpr int HSTAGE_ELEMS = (HB + 1) * HROWS;                 // 32 columns + t
 constexpr size_t HEMV_SMEM = (size_t)HSTAGES * HSTAGE_ELEMS * sizeof(cplx) + 2 * 4 * HROWS * sizeof(cplx)
                              + 2 * HSTAGES * sizeof(unsigned long long) + 8 * sizeof(int) + 64 + 2 * 64 * sizeof(cplx);
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(void* bar, int count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(void* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(void* bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity) {
-  asm volatile(
-      "{\n .reg .pred p;\n WAIT_LOOP:\n"
-      " mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      " @p bra WAIT_DONE;\n bra WAIT_LOOP;\n WAIT_DONE:\n}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, uint32_t bytes, void* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-
-// Block columns J >= nJ are "panel blocks": 32 columns of the [W | V] panels streamed through the
-// same pipeline with only their column part kept, pq[q] = W[:, q]^H v (q < k), V[:, q-k]^H v (q >= k),
-// the 2k products k_colw needs for w_i.
 // The kernel is PERSISTENT: 2 CTAs per SM fetch work items (matrix, block column) from a global
 // counter until none is left (panel blocks and long block columns come first in the item order).
 // The producer warp runs ahead of the consumers across item boundaries -- the stage counter never
