@@ -627,26 +627,28 @@ __global__ void __launch_bounds__(1024) k_larft(const cplx* __restrict__ G, cons
   const cplx* g = G + c * NBT * NBT;
   cplx* t = T + c * NBT * NBT;
   cplx* w = tmp + c * NBT * NBT;
-  const int tid = threadIdx.x;
-  for (int idx = tid; idx < NBT * NBT; idx += 1024) {
-    const int r = idx % NBT, cc = idx / NBT;
-    t[idx] = (r == cc && r < kb) ? tauc[c * NBT + r] : mkc(0.0, 0.0);
+  const int tid = threadIdx.x, nt = blockDim.x;
+  int kbp = 1;
+  while (kbp < kb) kbp <<= 1;               // only the leading kbp x kbp part is built (kb <= kbp <= NBT)
+  for (int idx = tid; idx < kbp * kbp; idx += nt) {
+    const int r = idx % kbp, cc = idx / kbp;
+    t[r + cc * NBT] = (r == cc && r < kb) ? tauc[c * NBT + r] : mkc(0.0, 0.0);
   }
   __syncthreads();
-  for (int sz = 1; sz < NBT; sz <<= 1) {
+  for (int sz = 1; sz < kbp; sz <<= 1) {
     // tmp[r][cc] = sum_q T11[r][q] G[q][cc]: r, q in the first half (q >= r), cc in the second half
-    const int per = sz * sz, pairs = NBT / (2 * sz);
-    for (int idx = tid; idx < per * pairs; idx += 1024) {
+    const int per = sz * sz, pairs = kbp / (2 * sz);
+    for (int idx = tid; idx < per * pairs; idx += nt) {
       const int b0 = (idx / per) * 2 * sz, e = idx % per;
       const int r = b0 + e % sz, cc = b0 + sz + e / sz;
       cplx acc = mkc(0.0, 0.0);
       if (cc < kb)
-        for (int q = r; q < b0 + sz; ++q) cfma(acc, t[r + q * NBT], g[q + cc * NBT]);
+        for (int q = r; q < b0 + sz && q < kb; ++q) cfma(acc, t[r + q * NBT], g[q + cc * NBT]);   // G is defined for q < kb only
       w[r + cc * NBT] = acc;
     }
     __syncthreads();
     // T12[r][cc] = -sum_q tmp[r][q] T22[q][cc]: q, cc in the second half (q <= cc)
-    for (int idx = tid; idx < per * pairs; idx += 1024) {
+    for (int idx = tid; idx < per * pairs; idx += nt) {
       const int b0 = (idx / per) * 2 * sz, e = idx % per;
       const int r = b0 + e % sz, cc = b0 + sz + e / sz;
       cplx acc = mkc(0.0, 0.0);
@@ -873,7 +875,7 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
     ZgemmParams gg = zgemm_simple(kb, kb, rows, s.Vb, N, (int64_t)N * NBT, s.Vb, N, (int64_t)N * NBT,
                                   s.G, NBT, NBT * NBT, cnt);
     BE_TRY(be_zgemm(ctx, BE_OP_C, BE_OP_N, gg));
-    k_larft<<<(unsigned)cnt, 1024, 0, st>>>(s.G, s.tauc, s.T, s.Ttmp, kb);
+    k_larft<<<(unsigned)cnt, kb <= 64 ? 256 : 1024, 0, st>>>(s.G, s.tauc, s.T, s.Ttmp, kb);
     LAUNCH_CHECK();
     // Y = V^H X[p+1:, :]
     ZgemmParams gy = zgemm_simple(kb, nv, rows, s.Vb, N, (int64_t)N * NBT, X + p + 1, N, (int64_t)N * nv,

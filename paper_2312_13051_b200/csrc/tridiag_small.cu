@@ -11,13 +11,36 @@ namespace {
 
 constexpr int TS_THREADS = 256;
 
+// Block-wide sum with ONE barrier: per-warp partials go to one of two alternating buffers (the next use
+// of the same buffer is two reductions, hence at least one barrier, later), every thread adds the 8 partials.
+__device__ __forceinline__ double block_sum1(double v, double* buf, int& par) {
+  v = warp_sum(v);
+  if ((threadIdx.x & 31) == 0) buf[par * 8 + (threadIdx.x >> 5)] = v;
+  __syncthreads();
+  double t = buf[par * 8];
+#pragma unroll
+  for (int w = 1; w < TS_THREADS / 32; ++w) t += buf[par * 8 + w];
+  par ^= 1;
+  return t;
+}
+__device__ __forceinline__ cplx block_sum1(cplx v, cplx* buf, int& par) {
+  v = warp_sum(v);
+  if ((threadIdx.x & 31) == 0) buf[par * 8 + (threadIdx.x >> 5)] = v;
+  __syncthreads();
+  cplx t = buf[par * 8];
+#pragma unroll
+  for (int w = 1; w < TS_THREADS / 32; ++w) t = cadd(t, buf[par * 8 + w]);
+  par ^= 1;
+  return t;
+}
+
 __global__ void __launch_bounds__(TS_THREADS) k_tridiag_smem(const cplx* __restrict__ H, GridMap map, int64_t loop0,
                                                              cplx* __restrict__ Bw, double* __restrict__ dd,
                                                              double* __restrict__ ee, cplx* __restrict__ tau, int N) {
   extern __shared__ cplx tsm[];             // A [N][ld] column-major (ld = N + 1: conflict-free column walks), w [N]
-  __shared__ double redd[33];
-  __shared__ cplx redc[33];
-  __shared__ cplx sh_alpha;
+  __shared__ double redd[16];
+  __shared__ cplx redc[16];
+  int pard = 0, parc = 0;
   const int ld = N + 1;
   cplx* A = tsm;
   cplx* w = tsm + (size_t)N * ld;
@@ -39,9 +62,8 @@ __global__ void __launch_bounds__(TS_THREADS) k_tridiag_smem(const cplx* __restr
     // ---- zlarfg
     double ss = 0.0;
     for (int r = 1 + tid; r < n; r += TS_THREADS) ss += cabs2(x[r]);
-    if (tid == 0) sh_alpha = x[0];
-    const double xn2 = block_sum(ss, redd);
-    const cplx alpha = sh_alpha;
+    const cplx alpha = x[0];                 // not modified before the next barrier
+    const double xn2 = block_sum1(ss, redd, pard);
     double beta; cplx t;
     if (xn2 == 0.0 && alpha.y == 0.0) {
       beta = alpha.x; t = mkc(0.0, 0.0);
@@ -77,7 +99,7 @@ __global__ void __launch_bounds__(TS_THREADS) k_tridiag_smem(const cplx* __restr
     // ---- w += -1/2 tau (w^H v) v
     cplx dot = mkc(0.0, 0.0);
     for (int r = tid; r < n; r += TS_THREADS) cfmac(dot, w[r], x[r]);
-    dot = block_sum(dot, redc);
+    dot = block_sum1(dot, redc, parc);
     const cplx al = cmul(mkc(-0.5 * t.x, -0.5 * t.y), dot);
     for (int r = tid; r < n; r += TS_THREADS) { cplx wr = w[r]; cfma(wr, al, x[r]); w[r] = wr; }
     __syncthreads();
