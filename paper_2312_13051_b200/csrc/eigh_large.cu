@@ -775,8 +775,11 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
 
   // ---- S1a: blocked tridiagonalization
   BE_CUDA(cudaMemsetAsync(s.hcount, 0, (size_t)N * sizeof(int), st));   // work counters of the persistent k_hemv, one per column
-  for (int p = 0; p < N && !on_chip; p += NB) {
-    const int pend = (p + NB < N - 1) ? p + NB : N - 1;   // reflector columns p .. pend-1
+  // panel width: the panel work (k_colw and the panel block columns of k_hemv) grows with nb / n, the
+  // rank-2k GEMM likes a deep K = 2 nb: 16 for mid-size matrices, NB = 32 for large ones
+  const int nb = (N <= 640) ? NB / 2 : NB;
+  for (int p = 0; p < N && !on_chip; p += nb) {
+    const int pend = (p + nb < N - 1) ? p + nb : N - 1;   // reflector columns p .. pend-1
     colw(p, p, 0, 1);   // reflector of column p (or, when p == N-1, just the last diagonal entry)
     LAUNCH_CHECK();
     if (p >= N - 1) break;
