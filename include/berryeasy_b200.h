@@ -84,7 +84,9 @@ int64_t be_launch_count(const be_ctx* ctx);
  * instrumented kernel class is bracketed by a CUDA event pair on the context's stream and its
  * algorithmic bytes / flops are accumulated.  be_profile_enable resets the counters (it
  * synchronises the stream); be_profile_get synchronises and returns the summed event time in ms.
- * Classes 0..be_profile_name(i)==NULL: "hemv", "col", "w", "zgemm", "bisect", "invit", ... */
+ * Classes 0..be_profile_name(i)==NULL: "hemv" (k_hemv, or the on-chip
+ * tridiagonalization for N <= 104), "colw", "zgemm", "bisect", "invit", "cluster_orth", "hessenberg", "hqr",
+ * "jacobi", "misc". */
 int be_profile_enable(be_ctx* ctx, int on);
 const char* be_profile_name(int cls);
 int be_profile_get(be_ctx* ctx, int cls, double* ms, int64_t* launches, double* bytes, double* flops);

@@ -57,7 +57,7 @@ extern "C" int be_profile_enable(be_ctx* ctx, int on) {
 }
 
 extern "C" const char* be_profile_name(int cls) {
-  static const char* names[PK_COUNT] = {"hemv", "col", "w", "zgemm", "bisect", "invit", "cluster_orth",
+  static const char* names[PK_COUNT] = {"hemv", "colw", "zgemm", "bisect", "invit", "cluster_orth",
                                         "hessenberg", "hqr", "jacobi", "misc"};
   return (cls >= 0 && cls < PK_COUNT) ? names[cls] : nullptr;
 }

@@ -95,7 +95,7 @@ struct be_ctx {
 };
 
 // kernel classes of the profile
-enum { PK_HEMV = 0, PK_COL, PK_W, PK_GEMM, PK_BISECT, PK_INVIT, PK_ORTH, PK_HESS, PK_HQR, PK_JACOBI,
+enum { PK_HEMV = 0, PK_COL, PK_GEMM, PK_BISECT, PK_INVIT, PK_ORTH, PK_HESS, PK_HQR, PK_JACOBI,
        PK_MISC, PK_COUNT };
 void be_prof_begin(be_ctx* ctx, int cls);
 void be_prof_end(be_ctx* ctx, int cls, double bytes, double flops);
