@@ -119,7 +119,8 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   const int msec[2] = {sp ? mlo : m, sp ? mhi : 0};
   size_t persist = 0;
   for (int s = 0; s < 2; ++s)
-    persist += be_align256((size_t)loops * msec[s] * msec[s] * sizeof(cplx)) + be_eigenphases_scratch_bytes(loops, msec[s]) + 1024;
+    persist += be_align256((size_t)loops * msec[s] * msec[s] * sizeof(cplx)) + be_eigenphases_scratch_bytes(2 * loops, msec[s]) +
+               be_align256(2 * (size_t)loops * msec[s] * sizeof(double)) + 1024;
   // Chunk pipeline (more than one chunk): two scratch regions used alternately, the
   // tridiagonalization of chunk c+1 on the caller's stream overlaps the rest of chunk c on stream2.
   const size_t region = be_align256(per * (size_t)lc);
@@ -149,11 +150,19 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   if (!pipe) BE_TRY(be_arena_reserve(ctx, region + persist + (4 << 20)));
   cudaStream_t S1 = ctx->stream;
   cplx* Wall[2] = {nullptr, nullptr};
-  for (int s = 0; s < 2; ++s)
-    if (msec[s] > 0) {
-      Wall[s] = (cplx*)be_arena_alloc(ctx, (size_t)loops * msec[s] * msec[s] * sizeof(cplx));
-      if (!Wall[s]) return BE_ERR_NOMEM;
-    }
+  // equal sectors: one contiguous buffer, so that both sectors' Wilson matrices are solved in ONE batch
+  const bool joint = sp && msec[0] == msec[1] && msec[0] > 0 && sp->theta_lo && sp->theta_hi;
+  if (joint) {
+    Wall[0] = (cplx*)be_arena_alloc(ctx, 2 * (size_t)loops * msec[0] * msec[0] * sizeof(cplx));
+    if (!Wall[0]) return BE_ERR_NOMEM;
+    Wall[1] = Wall[0] + (size_t)loops * msec[0] * msec[0];
+  } else {
+    for (int s = 0; s < 2; ++s)
+      if (msec[s] > 0) {
+        Wall[s] = (cplx*)be_arena_alloc(ctx, (size_t)loops * msec[s] * msec[s] * sizeof(cplx));
+        if (!Wall[s]) return BE_ERR_NOMEM;
+      }
+  }
   const size_t keep = ctx->arena_used;
   for (int64_t l0 = 0; l0 < loops; l0 += lc) {
     const int64_t nl = (loops - l0 < lc) ? loops - l0 : lc;
@@ -186,6 +195,14 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   int rc = BE_OK;
   if (!sp) {
     rc = be_eigenphases(ctx, Wall[0], loops, m, d_theta, d_abs);
+  } else if (joint) {
+    // the solve is latency bound per matrix: 2 x loops matrices in one launch cost what loops do
+    const size_t nb = (size_t)loops * msec[0] * sizeof(double);
+    double* th = (double*)be_arena_alloc(ctx, 2 * nb);
+    if (!th) rc = BE_ERR_NOMEM;
+    if (rc == BE_OK) rc = be_eigenphases(ctx, Wall[0], 2 * loops, msec[0], th, nullptr);
+    if (rc == BE_OK) rc = (int)cudaMemcpyAsync(sp->theta_lo, th, nb, cudaMemcpyDeviceToDevice, ctx->stream);
+    if (rc == BE_OK) rc = (int)cudaMemcpyAsync(sp->theta_hi, (char*)th + nb, nb, cudaMemcpyDeviceToDevice, ctx->stream);
   } else {
     for (int sector = 0; sector < 2 && rc == BE_OK; ++sector) {
       double* out = sector == 0 ? sp->theta_lo : sp->theta_hi;
