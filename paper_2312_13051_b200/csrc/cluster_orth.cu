@@ -264,7 +264,8 @@ __global__ void __launch_bounds__(256) k_cgram(const double* __restrict__ Z, int
 // ------------------------------------------------------------------------------------------
 // Per big cluster: G = R^T R (Cholesky-Crout, row by row, in place in the upper triangle), then
 // X = R^-1 in place (column by column).  One CTA per cluster; G stays in L2.
-__global__ void __launch_bounds__(256) k_chol_inv(int nv, int maxbig, ClusterBufs cb, int* __restrict__ info) {
+constexpr int CHT = 512;   // threads of k_chol_inv
+__global__ void __launch_bounds__(CHT) k_chol_inv(int nv, int maxbig, ClusterBufs cb, int* __restrict__ info) {
   extern __shared__ double colk[];   // L doubles
   __shared__ int s_fail;
   const int64_t c = blockIdx.x / maxbig;
@@ -275,9 +276,9 @@ __global__ void __launch_bounds__(256) k_chol_inv(int nv, int maxbig, ClusterBuf
   const int tid = threadIdx.x;
   if (tid == 0) s_fail = 0;
   for (int k = 0; k < L; ++k) {
-    for (int p = tid; p < k; p += 256) colk[p] = G[(int64_t)p * L + k];   // R[0:k, k]
+    for (int p = tid; p < k; p += CHT) colk[p] = G[(int64_t)p * L + k];   // R[0:k, k]
     __syncthreads();
-    for (int j = k + tid; j < L; j += 256) {
+    for (int j = k + tid; j < L; j += CHT) {
       double t0 = G[(int64_t)k * L + j], t1 = 0.0;
       int p = 0;
       for (; p + 1 < k; p += 2) {
@@ -292,24 +293,24 @@ __global__ void __launch_bounds__(256) k_chol_inv(int nv, int maxbig, ClusterBuf
     if (!(d > 1e-13)) { d = 1.0; if (tid == 0) s_fail = 1; }   // vectors are normalized: G[k][k] started at 1
     const double rs = 1.0 / sqrt(d);
     __syncthreads();
-    for (int j = k + tid; j < L; j += 256) {
+    for (int j = k + tid; j < L; j += CHT) {
       const double t = G[(int64_t)k * L + j];
       G[(int64_t)k * L + j] = (j == k) ? d * rs : t * rs;
     }
     __syncthreads();
   }
   if (s_fail) {   // numerically dependent vectors: leave the cluster as it is (identity), flag the matrix
-    for (int idx = tid; idx < L * L; idx += 256) G[idx] = (idx / L == idx % L) ? 1.0 : 0.0;
+    for (int idx = tid; idx < L * L; idx += CHT) G[idx] = (idx / L == idx % L) ? 1.0 : 0.0;
     if (tid == 0 && info) atomicAdd(&info[c], 1);
     return;
   }
   // X = R^-1, upper triangular, column j: X[j][j] = 1 / R[j][j], X[i][j] = -(sum_{k=i}^{j-1} X[i][k] R[k][j]) X[j][j]
   for (int j = 0; j < L; ++j) {
-    for (int k = tid; k < j; k += 256) colk[k] = G[(int64_t)k * L + j];
+    for (int k = tid; k < j; k += CHT) colk[k] = G[(int64_t)k * L + j];
     __syncthreads();
     const double xjj = 1.0 / G[(int64_t)j * L + j];
     __syncthreads();
-    for (int i = tid; i <= j; i += 256) {
+    for (int i = tid; i <= j; i += CHT) {
       if (i == j) { G[(int64_t)j * L + j] = xjj; continue; }
       double t0 = 0.0, t1 = 0.0;
       const double* xi = G + (int64_t)i * L;
@@ -450,7 +451,7 @@ int be_cluster_orth(be_ctx* ctx, const double* lam, const double* tnorm, const i
   for (int it = 0; it < rounds; ++it) {
     k_cgram<<<(unsigned)(cnt * tmaxg), 256, 0, st>>>(Z, N, nv, mb, tmaxg, cb);
     LAUNCH_CHECK();
-    k_chol_inv<<<(unsigned)(cnt * mb), 256, sh, st>>>(nv, mb, cb, info);
+    k_chol_inv<<<(unsigned)(cnt * mb), CHT, sh, st>>>(nv, mb, cb, info);
     LAUNCH_CHECK();
     k_cupdate<<<(unsigned)(cnt * tmaxu), 256, 0, st>>>(Z, N, nv, mb, tmaxu, cb);
     LAUNCH_CHECK();

@@ -854,7 +854,10 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
                                                         s.bcl, s.Z, N, nv, nvb, it > 0 ? 1 : 0, 1);
         be_prof_end(ctx, PK_INVIT, (double)cnt * N * nv * 8.0, 0.0);
         LAUNCH_CHECK();
-        BE_TRY(be_cluster_orth(ctx, E, s.tnorm, s.blk, s.Z, cnt, N, nv, CLUSTER_TOL, info, s.orth, it == 0, 2));
+        // Cholesky-QR passes: 2 after the first solve (random starts: cond up to ~1e5) and after the last
+        // one (final orthogonality at eps); 1 in between (one solve applied to an orthonormal basis keeps
+        // cond below ~5e2, and the next solve re-mixes the cluster anyway)
+        BE_TRY(be_cluster_orth(ctx, E, s.tnorm, s.blk, s.Z, cnt, N, nv, CLUSTER_TOL, info, s.orth, it == 0, it == 1 ? 1 : 2));
       }
     }
   }
