@@ -200,6 +200,21 @@ int be_bloch_coefficients(be_ctx* ctx, const double* d_t, const int* h_R, int nd
 int be_assemble_bloch(be_ctx* ctx, const void* dA, const void* d_coef, int64_t count, int N, int nR, void* dH);
 
 /*
+ * The same step FUSED in front of S1: be_wilson_loop / be_spin_resolved_wilson on a grid that is never
+ * materialised.  H at grid point (i_0, .., i_{ndim-1}) of batch entry b is
+ *     H = sum_R exp(2 pi i sum_a (i_a / dims[a]) R[a]) * A[b][R],
+ * generated chunk by chunk straight into the eigensolver's work copy (no 17-43 GB H_grid, no read of it).
+ *   dA  [batch][nR][N][N] complex128 row-major blocks (every batch entry -- disorder realization -- has
+ *       its own set; list A_R and A_{-R} = A_R^dagger both), h_R [nR][ndim] int lattice vectors on the HOST.
+ * All other arguments, outputs and conventions as in be_wilson_loop / be_spin_resolved_wilson.
+ */
+int be_wilson_loop_bloch(be_ctx* ctx, const void* dA, const int* h_R, int nR, const be_grid* grid, int n_occ,
+                         int dir, const void* d_close, double* d_theta, double* d_abs, double* d_mingap);
+int be_spin_resolved_wilson_bloch(be_ctx* ctx, const void* dA, const int* h_R, int nR, const be_grid* grid,
+                                  int n_occ, int dir, const void* dS, int S_is_diag, int m_lo, const void* d_close,
+                                  double* d_theta_lo, double* d_theta_hi, double* d_pso);
+
+/*
  * Plaquette mode ("integrated Berry flux through one plaquette",
  * the coupling-matrix method and its spin-resolved generalization): on a periodic 2D grid
  * (grid->ndim == 2, dims = (ny, nx)) every point is diagonalized ONCE and

@@ -18,7 +18,8 @@ EXPORTS = [
     "be_create", "be_destroy", "be_strerror", "be_workspace_bytes", "be_set_workspace_limit",
     "be_launch_count", "be_eigh_batched", "be_wilson_loop", "be_nested_wilson",
     "be_spin_resolved_wilson", "be_winding", "be_wilson_loop_host", "be_spin_resolved_wilson_host",
-    "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched", "be_set_chunk_pipeline", "be_bloch_coefficients", "be_assemble_bloch", "be_plaquette_flux",
+    "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched", "be_set_chunk_pipeline", "be_bloch_coefficients", "be_assemble_bloch", "be_plaquette_flux", "be_wilson_loop_bloch",
+    "be_spin_resolved_wilson_bloch",
 ]
 
 
@@ -51,6 +52,8 @@ def load_library():
     lib.be_bloch_coefficients.argtypes = [vp, vp, C.POINTER(ci), ci, ci, i64, vp]
     lib.be_assemble_bloch.argtypes = [vp, vp, vp, i64, ci, ci, vp]
     lib.be_plaquette_flux.argtypes = [vp, vp, gp, ci, vp, ci, ci, vp, vp, vp]
+    lib.be_wilson_loop_bloch.argtypes = [vp, vp, C.POINTER(ci), ci, gp, ci, ci, vp, vp, vp, vp]
+    lib.be_spin_resolved_wilson_bloch.argtypes = [vp, vp, C.POINTER(ci), ci, gp, ci, ci, vp, ci, ci, vp, vp, vp, vp]
     lib.be_launch_count.argtypes = [vp]
     lib.be_launch_count.restype = i64
     lib.be_eigh_batched.argtypes = [vp, vp, i64, ci, ci, vp, vp, vp]
@@ -267,6 +270,63 @@ class Context:
         H = torch.empty((count, N, N), dtype=torch.complex128, device=A.device)
         _check(self.lib, self.lib.be_assemble_bloch(self._h, _ptr(A), _ptr(coef), count, N, nR, _ptr(H)))
         return H
+
+    # ------------------------------------------------------------------ fused H(k) generation (NEXT-1)
+    def _bloch_grid(self, A, dims):
+        if A.dim() != 4:
+            raise ValueError("A must be [batch][nR][N][N]")
+        g = BeGrid()
+        g.ndim = len(dims)
+        g.batch = A.shape[0]
+        for a in range(3):
+            g.dims[a] = dims[a] if a < len(dims) else 1
+        g.N = A.shape[-1]
+        return g
+
+    def wilson_loop_bloch(self, A, R, dims, n_occ, direction, close=None):
+        """A [batch][nR][N][N] blocks (device), R [nR][ndim] ints, dims = grid points per axis: the loops of
+        be_wilson_loop on the grid H = sum_R exp(2 pi i (i/dims).R) A_R, generated on the fly."""
+        _dev(A, torch.complex128, "A")
+        g = self._bloch_grid(A, dims)
+        nR = A.shape[1]
+        Rl = [int(x) for row in R for x in row]
+        if len(Rl) != nR * len(dims):
+            raise ValueError("R must be [nR][ndim]")
+        hR = (C.c_int * len(Rl))(*Rl)
+        loops = A.shape[0]
+        for a, d in enumerate(dims):
+            if a != direction:
+                loops *= d
+        dev = A.device
+        theta = torch.empty((loops, n_occ), dtype=torch.float64, device=dev)
+        ab = torch.empty((loops, n_occ), dtype=torch.float64, device=dev)
+        mg = torch.empty((loops,), dtype=torch.float64, device=dev)
+        _check(self.lib, self.lib.be_wilson_loop_bloch(self._h, _ptr(A), hR, nR, C.byref(g), n_occ, direction,
+                                                       _ptr(close), _ptr(theta), _ptr(ab), _ptr(mg)))
+        return theta, ab, mg
+
+    def spin_resolved_wilson_bloch(self, A, R, dims, n_occ, direction, S, m_lo=-1, close=None):
+        _dev(A, torch.complex128, "A")
+        g = self._bloch_grid(A, dims)
+        nR = A.shape[1]
+        Rl = [int(x) for row in R for x in row]
+        hR = (C.c_int * len(Rl))(*Rl)
+        loops = A.shape[0]
+        for a, d in enumerate(dims):
+            if a != direction:
+                loops *= d
+        n1 = dims[direction]
+        is_diag = 1 if S.dim() == 1 else 0
+        _dev(S, torch.float64 if is_diag else torch.complex128, "S")
+        mlo = n_occ // 2 if m_lo < 0 else m_lo
+        dev = A.device
+        lo = torch.empty((loops, mlo), dtype=torch.float64, device=dev)
+        hi = torch.empty((loops, n_occ - mlo), dtype=torch.float64, device=dev)
+        pso = torch.empty((loops, n1, n_occ), dtype=torch.float64, device=dev)
+        _check(self.lib, self.lib.be_spin_resolved_wilson_bloch(self._h, _ptr(A), hR, nR, C.byref(g), n_occ, direction,
+                                                                _ptr(S), is_diag, m_lo, _ptr(close), _ptr(lo),
+                                                                _ptr(hi), _ptr(pso)))
+        return lo, hi, pso
 
     # ------------------------------------------------------------------ be_plaquette_flux (NEXT-2)
     def plaquette_flux(self, H_grid, n_occ, S=None, m_lo=-1, want_pso=False):

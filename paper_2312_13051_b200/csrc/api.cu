@@ -125,6 +125,7 @@ extern "C" int be_destroy(be_ctx* ctx) {
   cudaStreamSynchronize(ctx->stream);
   if (ctx->arena) cudaFree(ctx->arena);
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+  if (ctx->dR_buf) cudaFree(ctx->dR_buf);
   if (ctx->stream2) {
     cudaStreamDestroy(ctx->stream2);
     cudaEventDestroy(ctx->ev_split); cudaEventDestroy(ctx->ev_join);
@@ -166,15 +167,33 @@ extern "C" int64_t be_launch_count(const be_ctx* ctx) { return ctx ? ctx->launch
 
 // ---------------------------------------------------------------------------------------------
 size_t be_eigh_scratch_bytes(int64_t cnt, int N, int nv) {
-  if (N <= 8) return 256;
+  if (N <= 8) return 256 + (size_t)cnt * N * N * sizeof(cplx);   // (+ the assembled chunk of a *_bloch call)
+  if (N <= TS_MAXN) return be_eigh_large_scratch_bytes(cnt, N, nv) + (size_t)cnt * N * N * sizeof(cplx) + 4096;
   return be_eigh_large_scratch_bytes(cnt, N, nv) + 4096;
 }
 
 int be_eigh_frames(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt,
                    int N, int nv, int ne, double* E, cplx* X, int* info) {
   if (cnt <= 0) return BE_OK;
-  if (N <= 8) return be_eigh_small(ctx, H, map, loop0, cnt, N, nv, E, X, info);
   const size_t mark = ctx->arena_used;
+  if (ctx->bloch && N <= TS_MAXN) {
+    // small matrices: assemble the chunk into a scratch grid, then solve it as a flat batch (the large
+    // path assembles straight into its work copy inside be_eigh_large)
+    const BlochSrc* bs = ctx->bloch;
+    cplx* T = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * N * sizeof(cplx));
+    if (!T) return BE_ERR_NOMEM;
+    BE_TRY(be_bloch_assemble_chunk(ctx, bs, loop0, cnt, N, T));
+    ctx->bloch = nullptr;
+    GridMap fm;
+    memset(&fm, 0, sizeof(fm));
+    fm.ndim = 1; fm.dir = 0; fm.n1 = 1; fm.dims[0] = 1; fm.batch_stride = 1; fm.loops = cnt;
+    const int r = (N <= 8) ? be_eigh_small(ctx, T, fm, 0, cnt, N, nv, E, X, info)
+                           : be_eigh_large(ctx, T, fm, 0, cnt, N, nv, ne, E, X, info);
+    ctx->bloch = bs;
+    ctx->arena_used = mark;
+    return r;
+  }
+  if (N <= 8) return be_eigh_small(ctx, H, map, loop0, cnt, N, nv, E, X, info);
   const int r = be_eigh_large(ctx, H, map, loop0, cnt, N, nv, ne, E, X, info);
   ctx->arena_used = mark;   // stage scratch is dead once its kernels are enqueued (stream order)
   return r;
@@ -300,4 +319,55 @@ extern "C" int be_assemble_bloch(be_ctx* ctx, const void* dA, const void* d_coef
   ZgemmParams g = zgemm_simple(M, (int)count, nR, (const cplx*)dA, M, 0, (const cplx*)d_coef, nR, 0,
                                (cplx*)dH, M, 0, 1);
   return be_zgemm(ctx, BE_OP_N, BE_OP_N, g);
+}
+
+// ---------------------------------------------------------------------------------------------
+// chunk-wise H(k) generation for the *_bloch entry points
+namespace {
+__global__ void k_bloch_coef_chunk(const int* __restrict__ R, int nR, GridMap map, int64_t loop0, int64_t cnt,
+                                   cplx* __restrict__ coef) {
+  const int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (idx >= cnt * nR) return;
+  const int64_t c = idx / nR;
+  const int r = (int)(idx % nR);
+  int64_t rest = loop0 + c / map.n1;
+  int j = (int)(c % map.n1) + map.shift;
+  if (j >= map.n1) j -= map.n1;
+  double x = (double)j / map.n1 * (double)R[r * map.ndim + map.dir];
+  for (int a = map.ndim - 1; a >= 0; --a) {
+    if (a == map.dir) continue;
+    const int64_t i = rest % map.dims[a];
+    rest /= map.dims[a];
+    x += (double)i / map.dims[a] * (double)R[r * map.ndim + a];
+  }
+  double s, co;
+  sincospi(2.0 * x, &s, &co);
+  coef[idx] = mkc(co, s);
+}
+}  // namespace
+
+int be_bloch_assemble_chunk(be_ctx* ctx, const BlochSrc* bs, int64_t loop0, int64_t cnt, int N, cplx* out) {
+  const size_t mark = ctx->arena_used;
+  cplx* coef = (cplx*)be_arena_alloc(ctx, (size_t)cnt * bs->nR * sizeof(cplx));
+  if (!coef) return BE_ERR_NOMEM;
+  const int64_t tot = cnt * bs->nR;
+  k_bloch_coef_chunk<<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(bs->dR, bs->nR, bs->map, loop0, cnt, coef);
+  ctx->launches++;
+  BE_CUDA(cudaGetLastError());
+  // one GEMM per realization present in the chunk (loops are enumerated batch-major)
+  const int n1 = bs->map.n1;
+  const int M = N * N;
+  int64_t c0 = 0;
+  while (c0 < cnt) {
+    const int64_t loop = loop0 + c0 / n1;
+    const int64_t bt = loop / bs->loops_per_batch;
+    int64_t c1 = ((bt + 1) * bs->loops_per_batch - loop0) * n1;   // first matrix of the next realization
+    if (c1 > cnt) c1 = cnt;
+    ZgemmParams g = zgemm_simple(M, (int)(c1 - c0), bs->nR, bs->A + bt * (int64_t)bs->nR * M, M, 0,
+                                 coef + c0 * bs->nR, bs->nR, 0, out + c0 * (int64_t)M, M, 0, 1);
+    BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_N, g));
+    c0 = c1;
+  }
+  ctx->arena_used = mark;   // coef is dead once the GEMMs are enqueued
+  return BE_OK;
 }

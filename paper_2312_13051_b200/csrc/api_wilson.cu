@@ -103,7 +103,7 @@ static int pipeline_init(be_ctx* ctx) {
 // One pass over all loops of ``map`` (device H).  Plain loop when ``sp`` is NULL.
 static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, int m,
                          const cplx* d_close, double* d_theta, double* d_abs, double* d_mingap,
-                         const SpinArgs* sp, HostStage* hs = nullptr) {
+                         const SpinArgs* sp, HostStage* hs = nullptr, const BlochSrc* bs = nullptr) {
   const int n1 = map.n1;
   const int64_t loops = map.loops;
   const size_t per = per_loop_bytes(N, m, n1, sp != nullptr);
@@ -181,8 +181,10 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
       BE_CUDA(cudaStreamWaitEvent(ctx->stream, hs->copied[ci & 1], 0));
       Hc = (const cplx*)hs->stage[ci & 1];
     }
+    ctx->bloch = bs;   // consumed (and cleared) by the H eigensolve of the chunk
     const int rc = wilson_chunk(ctx, Hc, hs ? smap : map, hs ? 0 : l0, N, m, n1, l0, nl, cnt, d_close, d_mingap, sp, mlo,
                                 mhi, Wall);
+    ctx->bloch = nullptr;
     if (hs && rc == BE_OK) cudaEventRecord(hs->freed[ci & 1], ctx->stream);
     if (pipe) {
       ctx->split_after_tridiag = 0;
@@ -228,7 +230,11 @@ static int wilson_chunk(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t 
     double* E = (double*)be_arena_alloc(ctx, (size_t)cnt * N * sizeof(double));
     cplx* X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
     if (!E || !X) return BE_ERR_NOMEM;
-    BE_TRY(be_eigh_frames(ctx, H, map, gl0, cnt, N, m, m + 1, E, X, nullptr));
+    {
+      const int r = be_eigh_frames(ctx, H, map, gl0, cnt, N, m, m + 1, E, X, nullptr);
+      ctx->bloch = nullptr;   // only H(k) is generated; the PSO solve below reads S_red from memory
+      BE_TRY(r);
+    }
     if (d_mingap) BE_TRY(be_mingap(ctx, E, N, m, n1, nl, d_mingap + l0));
     if (!sp) {
       cplx* W = nullptr;
@@ -450,4 +456,51 @@ int be_wilson_host_device(be_ctx* ctx, HostStage* hs, int64_t loops, int n1, int
   if (!spin) return wilson_device(ctx, nullptr, map, N, m, (const cplx*)d_close, d_theta, d_abs, d_mingap, nullptr, hs);
   SpinArgs sp{dS, S_is_diag, m_lo, d_theta_lo, d_theta_hi, d_pso};
   return wilson_device(ctx, nullptr, map, N, m, (const cplx*)d_close, nullptr, nullptr, nullptr, &sp, hs);
+}
+
+// ---------------------------------------------------------------------------------------------
+// NEXT-1 fused in front of S1: the loops of a grid whose H(k) is generated chunk by chunk from real-space
+// blocks (no H_grid in memory).
+static int bloch_source(be_ctx* ctx, const void* dA, const int* h_R, int nR, const be_grid* grid, int dir,
+                        BlochSrc* bs) {
+  if (!dA || !h_R) return BE_ERR_NULL;
+  if (nR < 1) return BE_ERR_SHAPE;
+  if (!aligned(dA, 16)) return BE_ERR_ALIGN;
+  BE_TRY(make_map(grid, dir, &bs->map));
+  const size_t need = (size_t)nR * grid->ndim * sizeof(int);
+  if (need > ctx->dR_cap) {
+    if (ctx->dR_buf) { BE_CUDA(cudaStreamSynchronize(ctx->stream)); cudaFree(ctx->dR_buf); ctx->dR_buf = nullptr; ctx->dR_cap = 0; }
+    if (cudaMalloc((void**)&ctx->dR_buf, need) != cudaSuccess) { cudaGetLastError(); return BE_ERR_NOMEM; }
+    ctx->dR_cap = need;
+  }
+  BE_CUDA(cudaMemcpyAsync(ctx->dR_buf, h_R, need, cudaMemcpyHostToDevice, ctx->stream));
+  bs->A = (const cplx*)dA; bs->dR = ctx->dR_buf; bs->nR = nR;
+  bs->loops_per_batch = bs->map.loops / grid->batch;
+  return BE_OK;
+}
+
+extern "C" int be_wilson_loop_bloch(be_ctx* ctx, const void* dA, const int* h_R, int nR, const be_grid* grid,
+                                    int n_occ, int dir, const void* d_close, double* d_theta, double* d_abs,
+                                    double* d_mingap) {
+  BE_TRY(check_common(ctx, dA, grid, n_occ, dir));
+  if (!d_theta) return BE_ERR_NULL;
+  BlochSrc bs;
+  BE_TRY(bloch_source(ctx, dA, h_R, nR, grid, dir, &bs));
+  return wilson_device(ctx, nullptr, bs.map, grid->N, n_occ, (const cplx*)d_close, d_theta, d_abs, d_mingap, nullptr,
+                       nullptr, &bs);
+}
+
+extern "C" int be_spin_resolved_wilson_bloch(be_ctx* ctx, const void* dA, const int* h_R, int nR, const be_grid* grid,
+                                             int n_occ, int dir, const void* dS, int S_is_diag, int m_lo,
+                                             const void* d_close, double* d_theta_lo, double* d_theta_hi,
+                                             double* d_pso) {
+  BE_TRY(check_common(ctx, dA, grid, n_occ, dir));
+  if (!dS) return BE_ERR_NULL;
+  if (m_lo < 0) m_lo = n_occ / 2;
+  if (m_lo > n_occ) return BE_ERR_SHAPE;
+  BlochSrc bs;
+  BE_TRY(bloch_source(ctx, dA, h_R, nR, grid, dir, &bs));
+  SpinArgs sp{dS, S_is_diag, m_lo, d_theta_lo, d_theta_hi, d_pso};
+  return wilson_device(ctx, nullptr, bs.map, grid->N, n_occ, (const cplx*)d_close, nullptr, nullptr, nullptr, &sp,
+                       nullptr, &bs);
 }

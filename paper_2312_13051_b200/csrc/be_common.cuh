@@ -87,6 +87,8 @@ struct be_ctx {
   // chunk c (FP64 / latency bound) runs on the high-priority ``stream2``
   cudaStream_t stream2;
   cudaEvent_t ev_split, ev_region[2], ev_join;
+  int* dR_buf; size_t dR_cap;      // device copy of the lattice vectors of a *_bloch call
+  const struct BlochSrc* bloch;   // set while the H eigensolve of a *_bloch call runs: H(k) is assembled, not read
   int chunk_pipeline;         // be_set_chunk_pipeline (default 0)
   int split_after_tridiag;    // consumed by be_eigh_large: switch to stream2 after S1a
   int gemm_pad;               // zgemm launches with padded shared memory: at most one GEMM CTA per SM,
@@ -169,6 +171,17 @@ __host__ __device__ inline int64_t gridmap_index(const GridMap& g, int64_t loop,
 }
 
 // ---------------------------------------------------------------------------------------------
+// H(k) generated on the fly (be_*_bloch): H[k] = sum_R exp(2 pi i t_k . R) A_R, t = grid index / dims.
+struct BlochSrc {
+  const cplx* A;        // [batch][nR][N][N]
+  const int* dR;        // device [nR][ndim]
+  int nR;
+  GridMap map;          // decodes (loop, j) into grid indices (the same enumeration as H_grid)
+  int64_t loops_per_batch;
+};
+// matrices c = 0..cnt-1 of the chunk starting at loop0, written to out [cnt][N][N]; coef: scratch [cnt][nR]
+int be_bloch_assemble_chunk(be_ctx* ctx, const BlochSrc* bs, int64_t loop0, int64_t cnt, int N, cplx* out);
+
 // Host-resident H_grid streamed chunk by chunk (be_*_host): two device staging buffers filled on the
 // copy stream while the previous chunk computes.  Loops must be contiguous (dir == last axis).
 struct HostStage {

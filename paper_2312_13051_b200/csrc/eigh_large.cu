@@ -754,6 +754,8 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
   const bool on_chip = N <= TS_MAXN;   // whole matrix in one CTA's shared memory (tridiag_small.cu)
   if (on_chip) {
     BE_TRY(be_tridiag_small(ctx, H, map, loop0, cnt, N, s.Bw, s.d, s.e, s.tau));
+  } else if (ctx->bloch) {
+    BE_TRY(be_bloch_assemble_chunk(ctx, ctx->bloch, loop0, cnt, N, s.Bw));   // H(k) generated into the work copy
   } else {
     const int nchunk = (int)(((int64_t)N * N + 2047) / 2048);
     k_gather<<<(unsigned)(cnt * nchunk), 256, 0, st>>>(H, s.Bw, map, loop0, N, nchunk);

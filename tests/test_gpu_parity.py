@@ -567,6 +567,50 @@ def test_chiral_hoti_eq9_on_device(ctx):
     assert sorted((round(wlo), round(whi))) == [-1, 1]                       # |C_s| = 1
 
 
+def test_fused_bloch_generation_matches_materialised_grid(ctx):
+    """NEXT-1 fused in front of S1: loops on a grid that is generated chunk by chunk from real-space blocks
+    equal the loops on the materialised H_grid (same seeded recipe), and the oracle."""
+    # two disorder realizations of the twisted 6 x 6 supercell (N = 144: blocked path), grid 3 x 9
+    parts = [wl.config3_parts(r, L=6) for r in (0, 1)]
+    A = np.stack([np.stack([Hb, Bx, Bx.conj().T, By, By.conj().T]) for (Hb, Bx, By) in parts])   # [2][5][N][N]
+    R = [[0, 0], [0, 1], [0, -1], [1, 0], [-1, 0]]            # grid axes (t2, t1): Bx goes with the t1 axis
+    H = wl.supercell_grid(parts, 9, 3)                          # [2][3][9][144][144]
+    th, ab, mg = ctx.wilson_loop(dev(H), 72, 1)
+    try:
+        ctx.set_workspace_limit(40 << 20)                       # several chunks, chunks spanning realizations
+        thb, abb, mgb = ctx.wilson_loop_bloch(dev(A), R, (3, 9), 72, 1)
+        S = wl.supercell_spin_z(6)
+        lob, hib, psob = ctx.spin_resolved_wilson_bloch(dev(A), R, (3, 9), 72, 1, dev(S))
+        torch.cuda.synchronize()
+    finally:
+        ctx.set_workspace_limit(64 << 30)
+    assert phase_dist(thb.cpu().numpy(), th.cpu().numpy()) <= 1e-10
+    assert (mgb - mg).abs().max().item() < 1e-11
+    tho, _, _ = wo.wilson_surface(H, 72, 1)
+    assert phase_dist(thb.cpu().numpy(), tho) <= PH_TOL
+    loo, hio, _ = wo.spin_resolved_surface(H, 72, 1, S)
+    assert phase_dist(lob.cpu().numpy(), loo) <= PH_TOL and phase_dist(hib.cpu().numpy(), hio) <= PH_TOL
+    # small matrices (Jacobi path): config 1 from its three hopping blocks
+    T0 = np.kron(wl.sz, wl.s0).astype(complex)                                   # on-site m = 1
+    Tx = np.kron(wl.sx, wl.sz) / 2j - np.kron(wl.sz, wl.s0) / 2
+    Ty = np.kron(wl.sy, wl.s0) / 2j - np.kron(wl.sz, wl.s0) / 2
+    A1 = np.stack([T0, Tx, Tx.conj().T, Ty, Ty.conj().T])[None]
+    R1 = [[0, 0], [0, 1], [0, -1], [1, 0], [-1, 0]]                              # axes (ky, kx)
+    H1 = wl.config1_grid(20, 11)
+    th1, _, _ = ctx.wilson_loop_bloch(dev(A1), R1, (11, 20), 2, 1)
+    th1o, _, _ = wo.wilson_surface(H1[None], 2, 1)
+    assert phase_dist(th1.cpu().numpy(), th1o) <= PH_TOL
+    # on-chip path (N = 64): config 5 blocks, loops along kz
+    H0, Rs, HR = wl.config5_parts()
+    A5 = np.concatenate([H0[None], HR, HR.conj().transpose(0, 2, 1)])[None]
+    R5 = [[0, 0, 0]] + [list(map(int, r)) for r in Rs] + [list(map(int, -r)) for r in Rs]
+    th5, _, _ = ctx.wilson_loop_bloch(dev(A5), R5, (2, 3, 13), 32, 2)
+    H5 = np.array([[[wl.assemble_config5((H0, Rs, HR), 2 * np.pi * np.array([i / 2, j / 3, l / 13])) for l in range(13)]
+                    for j in range(3)] for i in range(2)])
+    th5o, _, _ = wo.wilson_surface(H5[None], 32, 2)
+    assert phase_dist(th5.cpu().numpy(), th5o) <= PH_TOL
+
+
 def test_launch_counter_counts_kernels(ctx):
     n0 = ctx.launch_count()
     ctx.wilson_loop(dev(wl.config1_grid(6, 2)[None]), 2, 1)
