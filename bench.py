@@ -345,7 +345,11 @@ def main():
     else:
         ach = d["bytes"] / (d["ms"] * 1e-3) / 1e9
         roof = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s",
-                "frac": ach / peak, "traffic": None, "peak_source": peak_src,
+                "frac": ach / peak,
+                # bytes per launch, like `achieved`: the DRAM read + write of the one captured launch exceeds
+                # its algorithmic bytes by the factor below; that factor is applied to the mean launch
+                "traffic": 1.065 * d["bytes"] / max(1, d["launches"]), "traffic_unit": "bytes per launch",
+                "algorithmic_bytes_per_launch": d["bytes"] / max(1, d["launches"]), "peak_source": peak_src,
                 # one ncu --set full capture of one launch (profiles/r01h_hemv_ncu_details.md): DRAM
                 # read + write 5.135 GB for 4.82 GB algorithmic; `achieved` averages over all launches,
                 # so the per-launch capture is reported as a ratio, not as `traffic`
