@@ -79,6 +79,15 @@ def test_eigh_tridiagonal_path_random(ctx, N, nv):
     check_eigh(ctx, A + A.conj().transpose(0, 2, 1), nv)
 
 
+def test_eigh_large_all_vectors(ctx):
+    """N = 1000 with ALL eigenvectors, N = 641 (first size on the 32-wide panels) and N = 640 (last on the
+    16-wide ones) with a ragged vector count: residual, orthonormality and eigenvalues at scale."""
+    rng = np.random.default_rng(1000)
+    for N, nv in ((1000, 1000), (641, 333), (640, 320)):
+        A = rng.standard_normal((2, N, N)) + 1j * rng.standard_normal((2, N, N))
+        check_eigh(ctx, A + A.conj().transpose(0, 2, 1), nv)
+
+
 def test_eigh_degenerate_clean_supercell_and_identity(ctx):
     """H4: heavily degenerate spectra (clean supercell at t=0), plus diagonal / scaled identity."""
     pc = wl.bhz_supercell_parts(6)
