@@ -443,7 +443,7 @@ __global__ void __launch_bounds__(128) k_bisect(const double* __restrict__ dd, c
     if (fabs(q) < pivmin) q = -pivmin;
     cnt += (q < 0.0);
     for (int r = 1; r < N; ++r) {
-      q = d[r] - mid - e2[r - 1] / q;
+      q = d[r] - mid - e2[r - 1] * __drcp_rn(q);   // same expression in k_invit's block search (counts must agree)
       if (fabs(q) < pivmin) q = -pivmin;
       cnt += (q < 0.0);
     }
@@ -505,7 +505,7 @@ __global__ void __launch_bounds__(128) k_invit(const double* __restrict__ dd, co
     double qm = 0.0, qp = 0.0;
     for (int r = 0; r < N; ++r) {
       if (r == start) { qm = d[r] - xm; qp = d[r] - xp; }
-      else { const double e2 = e[r - 1] * e[r - 1]; qm = d[r] - xm - e2 / qm; qp = d[r] - xp - e2 / qp; }
+      else { const double e2 = e[r - 1] * e[r - 1]; qm = d[r] - xm - e2 * __drcp_rn(qm); qp = d[r] - xp - e2 * __drcp_rn(qp); }
       if (fabs(qm) < pivmin) qm = -pivmin;
       if (fabs(qp) < pivmin) qp = -pivmin;
       cm += (qm < 0.0); cp += (qp < 0.0);
