@@ -7,6 +7,7 @@
 // Output sorted ascending on the branch (-pi, pi] (R7) by a rank sort.
 #include "be_common.cuh"
 #include <float.h>
+#include <cooperative_groups.h>
 
 namespace {
 
@@ -108,6 +109,88 @@ __global__ void __launch_bounds__(HESS_THREADS) k_hessenberg(cplx* __restrict__ 
       }
     }
     __syncthreads();
+  }
+}
+
+// The same reduction with a thread-block CLUSTER per matrix (few Wilson matrices, many idle SMs: 48
+// matrices on 148 SMs at the bench workload): the CTAs of a cluster split the columns of the left update
+// and the rows of the right update; the reflector is computed redundantly by every CTA, so the only
+// communication is the cluster barrier that orders the global-memory updates (3 per column).
+__global__ void __launch_bounds__(1024) k_hessenberg_cluster(cplx* __restrict__ W, int m) {
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  const int CS = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
+  extern __shared__ cplx vsh[];   // v[m], y[4][rows_per]
+  __shared__ double redd[33];
+  cplx* v = vsh; cplx* y = vsh + m;
+  cplx* H = W + (blockIdx.x / CS) * (int64_t)m * m;
+  const int tid = threadIdx.x, nt = 1024, warp = tid >> 5, lane = tid & 31, nw = nt >> 5;
+  const int rows_per = (m + CS - 1) / CS;
+  const int i0 = rank * rows_per, i1 = (i0 + rows_per < m) ? i0 + rows_per : m;
+  for (int k = 0; k < m - 2; ++k) {
+    // column k into shared memory (every CTA), norm of its tail
+    double ss = 0.0;
+    for (int r = k + 1 + tid; r < m; r += nt) {
+      const cplx x = H[r + (int64_t)k * m];
+      v[r] = x;
+      if (r > k + 1) ss += cabs2(x);
+    }
+    const double xn2 = block_sum(ss, redd);
+    const cplx alpha = v[k + 1];
+    cluster.sync();                                   // everybody has read column k
+    if (xn2 == 0.0 && alpha.y == 0.0) continue;       // (uniform over the cluster)
+    const double beta = -copysign(sqrt(cabs2(alpha) + xn2), alpha.x);
+    const cplx tau = mkc((beta - alpha.x) / beta, -alpha.y / beta);
+    const cplx scale = cdiv(mkc(1.0, 0.0), mkc(alpha.x - beta, alpha.y));
+    __syncthreads();                                  // alpha read before v[k+1] is overwritten
+    for (int r = k + 1 + tid; r < m; r += nt) {
+      const cplx x = v[r];
+      v[r] = (r == k + 1) ? mkc(1.0, 0.0) : cmul(x, scale);
+      if (rank == 0) H[r + (int64_t)k * m] = (r == k + 1) ? mkc(beta, 0.0) : mkc(0.0, 0.0);
+    }
+    __syncthreads();
+    // left: H[k+1:, j] -= conj(tau) v (v^H H[k+1:, j]),  j > k; column pairs dealt round robin over the cluster
+    const cplx ctau = cconj(tau);
+    for (int j = k + 1 + 2 * (warp + nw * rank); j < m; j += 2 * nw * CS) {
+      cplx* c0 = H + (int64_t)j * m;
+      const bool two = j + 1 < m;
+      cplx* c1 = two ? c0 + m : c0;
+      cplx d0 = mkc(0.0, 0.0), d1 = mkc(0.0, 0.0);
+      for (int r = k + 1 + lane; r < m; r += 32) { const cplx vr = v[r]; cfmac(d0, vr, c0[r]); cfmac(d1, vr, c1[r]); }
+      d0 = cmul(ctau, warp_sum(d0)); d1 = cmul(ctau, warp_sum(d1));
+      for (int r = k + 1 + lane; r < m; r += 32) {
+        const cplx vr = v[r];
+        cfms(c0[r], vr, d0);
+        if (two) cfms(c1[r], vr, d1);
+      }
+    }
+    cluster.sync();                                   // all columns updated before rows are combined
+    // right: H[i0:i1, k+1:] -= tau (H[i0:i1, k+1:] v) v^H; thread = (row, column slice of 4)
+    const int sl = tid >> 8;
+    for (int ib = i0; ib < i1; ib += 256) {
+      const int i = ib + (tid & 255);
+      if (i < i1) {
+        cplx a0 = mkc(0.0, 0.0), a1 = mkc(0.0, 0.0);
+        int j = k + 1 + sl;
+        for (; j + 4 < m; j += 8) { cfma(a0, H[i + (int64_t)j * m], v[j]); cfma(a1, H[i + (int64_t)(j + 4) * m], v[j + 4]); }
+        if (j < m) cfma(a0, H[i + (int64_t)j * m], v[j]);
+        y[sl * rows_per + (i - i0)] = cadd(a0, a1);
+      }
+    }
+    __syncthreads();
+    for (int ib = i0; ib < i1; ib += 256) {
+      const int i = ib + (tid & 255);
+      if (i < i1) {
+        const int li = i - i0;
+        const cplx acc = cmul(tau, cadd(cadd(y[li], y[rows_per + li]), cadd(y[2 * rows_per + li], y[3 * rows_per + li])));
+        for (int j = k + 1 + sl; j < m; j += 4) {
+          cplx h = H[i + (int64_t)j * m];
+          cfms(h, acc, cconj(v[j]));
+          H[i + (int64_t)j * m] = h;
+        }
+      }
+    }
+    cluster.sync();                                   // rows updated before the next column is read
   }
 }
 
@@ -336,8 +419,24 @@ int be_eigenvalues_general(be_ctx* ctx, cplx* W, int64_t cnt, int m, cplx* lam, 
   } else if (m <= 160) {
     k_hessenberg<256><<<(unsigned)cnt, 256, sh1, st>>>(W, m);
   } else {
-    if (sh1 > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_hessenberg<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh1));
-    k_hessenberg<1024><<<(unsigned)cnt, 1024, sh1, st>>>(W, m);
+    // few large matrices: a cluster of CTAs per matrix as long as the clusters fit the machine in one wave
+    int cs = 1;
+    for (int c = 2; c <= 4; ++c) if (cnt * c <= ctx->sm_count) cs = c;
+    if (cs > 1) {
+      const size_t shc = ((size_t)m + 4 * (size_t)((m + cs - 1) / cs)) * sizeof(cplx);
+      if (shc > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_hessenberg_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shc));
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)(cnt * cs)); cfg.blockDim = dim3(1024); cfg.dynamicSmemBytes = shc; cfg.stream = st;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      if (cudaLaunchKernelEx(&cfg, k_hessenberg_cluster, W, m) != cudaSuccess) { cudaGetLastError(); cs = 1; }   // cluster shape refused
+    }
+    if (cs == 1) {
+      if (sh1 > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_hessenberg<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh1));
+      k_hessenberg<1024><<<(unsigned)cnt, 1024, sh1, st>>>(W, m);
+    }
   }
   be_prof_end(ctx, PK_HESS, (double)cnt * m * m * 32.0, (double)cnt * (40.0 / 3.0) * m * (double)m * m);
   ctx->launches++;
