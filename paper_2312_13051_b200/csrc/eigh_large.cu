@@ -476,7 +476,8 @@ __global__ void __launch_bounds__(128) k_invit(const double* __restrict__ dd, co
   const int64_t c = blockIdx.x / nvb;
   const int vb = blockIdx.x % nvb;
   const double tn = tnorm[c];
-  const double tol = DBL_EPSILON * tn;
+  // pivot floor; the absolute part keeps the squared norm of a solve finite for a matrix that is exactly zero
+  const double tol = fmax(DBL_EPSILON * tn, 1e-145);
   // T is split where an off-diagonal entry is negligible: eigenvectors live on one unreduced block,
   // which makes vectors of exactly degenerate eigenvalues (different blocks) orthogonal for free.
   for (int r = threadIdx.x; r < N; r += 128) {

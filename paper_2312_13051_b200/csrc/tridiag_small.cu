@@ -1,5 +1,7 @@
 // S1a for matrices that fit shared memory (8 < N <= TS_MAXN): unblocked Householder
-// tridiagonalization (zhetd2, lower) with the whole matrix resident in one CTA's shared memory.
+// tridiagonalization (zhetd2, lower) with the lower triangle of the matrix resident in one CTA's shared
+// memory, packed by columns (35 KB for N = 64, four CTAs per SM with 64 registers per thread; ncu: the
+// kernel is bound by shared-memory wavefronts, 67 % of the LSU peak).
 // This is the regime of the many-band Wannier-like workload (BASELINE.json configs[4]: 266 240
 // matrices of 64 x 64): the lock-step path launches two kernels per column and streams every matrix
 // through HBM N times; here a matrix is read once, reduced on chip, and its reflectors are written
@@ -11,121 +13,137 @@ namespace {
 
 constexpr int TS_THREADS = 256;
 
-// Block-wide sum with ONE barrier: per-warp partials go to one of two alternating buffers (the next use
-// of the same buffer is two reductions, hence at least one barrier, later), every thread adds the 8 partials.
-__device__ __forceinline__ double block_sum1(double v, double* buf, int& par) {
-  v = warp_sum(v);
-  if ((threadIdx.x & 31) == 0) buf[par * 8 + (threadIdx.x >> 5)] = v;
-  __syncthreads();
-  double t = buf[par * 8];
+// packed lower triangle, column by column: element (r, c), r >= c
+__device__ __forceinline__ int pk(int r, int c, int N) { return c * N - (c * (c - 1)) / 2 + (r - c); }
+
+// Per column i (n = N - i - 1, x = column i below the diagonal), four barriers:
+//   warp 0: zlarfg scalars, reflector v = s x~ to HBM, x~[0] = alpha - beta in place | hemv by all:
+//   y = tau s A22 x~ | warp 0: w~ = conj(s) (y - 1/2 tau s^2 (y^H x~) x~) | update by all:
+//   A22 -= x~ w~^H + w~ x~^H.  The reflector is not scaled in place: with x~ = x except x~[0] =
+//   alpha - beta one has v = s x~, s = 1 / (alpha - beta), so s only multiplies per-row scalars.
+// The inner loops walk the packed triangle with running offsets (two integer adds per element).
+template <int LGP>
+__device__ __forceinline__ void hemv_rows(const cplx* __restrict__ A, const cplx* __restrict__ x, cplx* __restrict__ yb,
+                                          cplx ts, int N, int i, int n, int tid) {
+  constexpr int P = 1 << LGP;
+  const int part = tid & (P - 1);
+  constexpr int RPW = 32 >> LGP;                        // rows per warp (an aligned block): warp-uniform trip count
+  for (int r = tid >> LGP; r < ((n + RPW - 1) & ~(RPW - 1)); r += TS_THREADS >> LGP) {
+    cplx acc = mkc(0.0, 0.0);
+    if (r < n) {
+      int cc = part;
+      int o = pk(i + 1 + r, i + 1 + part, N);           // (r, cc) of the trailing block, cc <= r: along row r
+      int step = P * (n - 1 - part) - P * (P - 1) / 2;
+      for (; cc <= r; cc += P) { cfma(acc, A[o], x[cc]); o += step; step -= P * P; }
+      int o2 = pk(i + 1 + cc, i + 1 + r, N);            // (cc, r), cc > r: down column r, conjugated
+      for (; cc < n; cc += P) { cfmac(acc, A[o2], x[cc]); o2 += P; }
+    }
 #pragma unroll
-  for (int w = 1; w < TS_THREADS / 32; ++w) t += buf[par * 8 + w];
-  par ^= 1;
-  return t;
-}
-__device__ __forceinline__ cplx block_sum1(cplx v, cplx* buf, int& par) {
-  v = warp_sum(v);
-  if ((threadIdx.x & 31) == 0) buf[par * 8 + (threadIdx.x >> 5)] = v;
-  __syncthreads();
-  cplx t = buf[par * 8];
-#pragma unroll
-  for (int w = 1; w < TS_THREADS / 32; ++w) t = cadd(t, buf[par * 8 + w]);
-  par ^= 1;
-  return t;
+    for (int m = 1; m < P; m <<= 1) {
+      acc.x += __shfl_xor_sync(0xffffffffu, acc.x, m);
+      acc.y += __shfl_xor_sync(0xffffffffu, acc.y, m);
+    }
+    if (part == 0 && r < n) yb[r] = cmul(ts, acc);
+  }
 }
 
-__global__ void __launch_bounds__(TS_THREADS) k_tridiag_smem(const cplx* __restrict__ H, GridMap map, int64_t loop0,
-                                                             cplx* __restrict__ Bw, double* __restrict__ dd,
-                                                             double* __restrict__ ee, cplx* __restrict__ tau, int N) {
-  extern __shared__ cplx tsm[];             // A [N][ld] column-major (ld = N + 1: conflict-free column walks), w [N]
-  __shared__ double redd[16];
-  __shared__ cplx redc[16];
-  int pard = 0, parc = 0;
-  const int ld = N + 1;
+__global__ void __launch_bounds__(TS_THREADS, 4) k_tridiag_smem(const cplx* __restrict__ H, GridMap map, int64_t loop0,
+                                                                cplx* __restrict__ Bw, double* __restrict__ dd,
+                                                                double* __restrict__ ee, cplx* __restrict__ tau, int N) {
+  extern __shared__ cplx tsm[];             // A: lower triangle packed by columns (pk), y [N], w~ [N]
+  __shared__ cplx sc[3];                    // tau s, -1/2 tau s^2, s
   cplx* A = tsm;
-  cplx* w = tsm + (size_t)N * ld;
+  cplx* yb = tsm + (size_t)N * (N + 1) / 2;
+  cplx* wb = yb + N;
   const int64_t c = blockIdx.x;
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31;
   {
     // the row-major Hermitian input read as a column-major array is B = conj(H) (eigh_large.cu)
     const int64_t src = gridmap_index(map, loop0 + c / map.n1, (int)(c % map.n1));
     const cplx* h = H + src * (int64_t)N * N;
     for (int idx = tid; idx < N * N; idx += TS_THREADS) {
       const int r = idx % N, cc = idx / N;
-      A[r + cc * ld] = h[idx];
+      if (r >= cc) A[pk(r, cc, N)] = h[idx];
     }
   }
+  cplx* Bc = Bw + c * (int64_t)N * N;
   __syncthreads();
   for (int i = 0; i < N - 1; ++i) {
     const int n = N - i - 1;                // order of the trailing block A22 = A[i+1:, i+1:]
-    cplx* x = A + (i + 1) + i * ld;         // column i below the diagonal, length n
-    // ---- zlarfg
-    double ss = 0.0;
-    for (int r = 1 + tid; r < n; r += TS_THREADS) ss += cabs2(x[r]);
-    const cplx alpha = x[0];                 // not modified before the next barrier
-    const double xn2 = block_sum1(ss, redd, pard);
-    double beta; cplx t;
-    if (xn2 == 0.0 && alpha.y == 0.0) {
-      beta = alpha.x; t = mkc(0.0, 0.0);
-    } else {
-      beta = -copysign(sqrt(cabs2(alpha) + xn2), alpha.x);
-      t = mkc((beta - alpha.x) / beta, -alpha.y / beta);
-      const cplx scale = cdiv(mkc(1.0, 0.0), mkc(alpha.x - beta, alpha.y));
-      for (int r = 1 + tid; r < n; r += TS_THREADS) x[r] = cmul(x[r], scale);
-    }
-    if (tid == 0) {
-      x[0] = mkc(1.0, 0.0);
-      dd[c * N + i] = A[i + i * ld].x;
-      ee[c * N + i] = beta;
-      tau[c * N + i] = t;
-    }
-    __syncthreads();
-    if (t.x == 0.0 && t.y == 0.0) continue;   // H_i = 1 (uniform over the CTA)
-    // ---- y = tau A22 v on the lower triangle: thread = (row, quarter of the columns)
-    const cplx* A22 = A + (i + 1) + (i + 1) * ld;
-    for (int r0 = 0; r0 < n; r0 += TS_THREADS / 4) {
-      const int r = r0 + (tid >> 2), part = tid & 3;
-      cplx acc = mkc(0.0, 0.0);
-      if (r < n)
-        for (int cc = part; cc < n; cc += 4) {
-          if (cc <= r) cfma(acc, A22[r + cc * ld], x[cc]);
-          else cfmac(acc, A22[cc + r * ld], x[cc]);
-        }
-      acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 1); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 1);
-      acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 2); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 2);
-      if (r < n && part == 0) w[r] = cmul(t, acc);
+    cplx* x = A + pk(i + 1, i, N);          // column i below the diagonal, length n (contiguous)
+    if (tid < 32) {
+      // ---- zlarfg (warp 0)
+      const cplx alpha = x[0];
+      double ss = 0.0;
+      for (int j = 1 + lane; j < n; j += 32) ss += cabs2(x[j]);
+      ss = warp_sum(ss);
+      cplx t = mkc(0.0, 0.0), scale = t, amb = t;
+      double beta = alpha.x;
+      if (ss != 0.0 || alpha.y != 0.0) {
+        // in-line reciprocal square root / reciprocals; no rescaling against over/underflow of the
+        // squared norm: |H| far from 1e+-150
+        const double s2 = cabs2(alpha) + ss;
+        const double rs = rsqrt(s2);
+        double nrm = s2 * rs;
+        nrm = fma(0.5 * rs, fma(-nrm, nrm, s2), nrm);
+        beta = -copysign(nrm, alpha.x);
+        const double rb = __drcp_rn(beta);
+        t = mkc((beta - alpha.x) * rb, -alpha.y * rb);
+        amb = mkc(alpha.x - beta, alpha.y);          // real parts of the same sign: no cancellation
+        const double q = __drcp_rn(amb.x * amb.x + amb.y * amb.y);
+        scale = mkc(amb.x * q, -amb.y * q);
+      }
+      for (int j = 1 + lane; j < n; j += 32) Bc[(i + 1 + j) + (int64_t)i * N] = cmul(scale, x[j]);   // reflector i
+      if (lane == 0) {
+        const cplx ts = cmul(t, scale);
+        sc[0] = ts;
+        sc[1] = cmul(mkc(-0.5 * ts.x, -0.5 * ts.y), scale);
+        sc[2] = scale;
+        dd[c * N + i] = A[pk(i, i, N)].x;
+        ee[c * N + i] = beta;
+        tau[c * N + i] = t;
+        x[0] = amb;
+      }
     }
     __syncthreads();
-    // ---- w += -1/2 tau (w^H v) v
-    cplx dot = mkc(0.0, 0.0);
-    for (int r = tid; r < n; r += TS_THREADS) cfmac(dot, w[r], x[r]);
-    dot = block_sum1(dot, redc, parc);
-    const cplx al = cmul(mkc(-0.5 * t.x, -0.5 * t.y), dot);
-    for (int r = tid; r < n; r += TS_THREADS) { cplx wr = w[r]; cfma(wr, al, x[r]); w[r] = wr; }
+    // ---- y = tau s A22 x~ on the lower triangle: thread = (row, one of P column classes)
+    {
+      const cplx ts = sc[0];
+      if (n > 32) hemv_rows<2>(A, x, yb, ts, N, i, n, tid);
+      else if (n > 16) hemv_rows<3>(A, x, yb, ts, N, i, n, tid);
+      else if (n > 8) hemv_rows<4>(A, x, yb, ts, N, i, n, tid);
+      else hemv_rows<5>(A, x, yb, ts, N, i, n, tid);
+    }
     __syncthreads();
-    // ---- A22 -= v w^H + w v^H (lower triangle): thread = (row, quarter of the columns)
-    cplx* A22w = A + (i + 1) + (i + 1) * ld;
-    for (int r0 = 0; r0 < n; r0 += 64) {
-      const int r = r0 + (tid & 63);
-      if (r < n) {
-        const cplx vr = x[r], wr = w[r];
-        for (int cc = tid >> 6; cc <= r; cc += 4) {
-          cplx a = A22w[r + cc * ld];
-          cfms(a, vr, cconj(w[cc]));
+    if (tid < 32) {
+      // ---- w~ = conj(s) (y - 1/2 tau s^2 (y^H x~) x~)   (warp 0)
+      cplx dot = mkc(0.0, 0.0);
+      for (int j = lane; j < n; j += 32) cfmac(dot, yb[j], x[j]);
+      dot = warp_sum(dot);
+      const cplx al = cmul(sc[1], dot), cs = cconj(sc[2]);
+      for (int j = lane; j < n; j += 32) { cplx wj = yb[j]; cfma(wj, al, x[j]); wb[j] = cmul(cs, wj); }
+    }
+    __syncthreads();
+    // ---- A22 -= x~ w~^H + w~ x~^H (lower triangle): thread = (row, one of Q column classes)
+    {
+      const int lgr = n > 32 ? 6 : 5;
+      const int q = tid >> lgr, Q = TS_THREADS >> lgr;
+      for (int r = tid & ((1 << lgr) - 1); r < n; r += 1 << lgr) {
+        const cplx xr = x[r], wr = wb[r];
+        int o = pk(i + 1 + r, i + 1 + q, N);
+        int step = Q * (n - 1 - q) - Q * (Q - 1) / 2;
+        for (int cc = q; cc <= r; cc += Q) {
+          cplx a = A[o];
+          cfms(a, xr, cconj(wb[cc]));
           cfms(a, wr, cconj(x[cc]));
-          A22w[r + cc * ld] = a;
+          A[o] = a;
+          o += step; step -= Q * Q;
         }
       }
     }
     __syncthreads();
   }
-  if (tid == 0) dd[c * N + N - 1] = A[(N - 1) + (N - 1) * ld].x;
-  // reflectors (and the rest of the work copy) for the back-transform
-  cplx* Bc = Bw + c * (int64_t)N * N;
-  for (int idx = tid; idx < N * N; idx += TS_THREADS) {
-    const int r = idx % N, cc = idx / N;
-    Bc[idx] = A[r + cc * ld];
-  }
+  if (tid == 0) dd[c * N + N - 1] = A[pk(N - 1, N - 1, N)].x;
 }
 
 }  // namespace
@@ -133,7 +151,7 @@ __global__ void __launch_bounds__(TS_THREADS) k_tridiag_smem(const cplx* __restr
 int be_tridiag_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N, cplx* Bw,
                      double* d, double* e, cplx* tau) {
   if (N > TS_MAXN) return BE_ERR_UNSUPPORTED;
-  const size_t sh = ((size_t)N * (N + 1) + N) * sizeof(cplx);
+  const size_t sh = ((size_t)N * (N + 1) / 2 + 2 * N) * sizeof(cplx);
   if (sh > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_tridiag_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
   be_prof_begin(ctx, PK_HEMV);
   k_tridiag_smem<<<(unsigned)cnt, TS_THREADS, sh, ctx->stream>>>(H, map, loop0, Bw, d, e, tau, N);

@@ -49,7 +49,7 @@ def check_eigh(ctx, H, nv):
     assert info.max() == 0
     for c in range(H.shape[0]):
         nrm = max(np.abs(Eo[c]).max(), 1e-300)
-        assert np.abs(E[c] - Eo[c]).max() <= E_TOL * nrm
+        assert np.abs(E[c] - Eo[c]).max() <= E_TOL * nrm + 1e-300   # bisection resolves 0 to the smallest normal number
         assert np.all(np.diff(E[c]) >= 0)
         if nv:
             N = H.shape[1]
@@ -71,7 +71,7 @@ def test_eigh_jacobi_chiral_degenerate_models(ctx):
     check_eigh(ctx, wl.config2_grid(11, 6).reshape(-1, 4, 4), 2)
 
 
-@pytest.mark.parametrize("N,nv", [(9, 9), (31, 10), (64, 32), (65, 65), (100, 37), (257, 128)])
+@pytest.mark.parametrize("N,nv", [(9, 9), (17, 17), (31, 10), (33, 33), (64, 32), (65, 65), (100, 37), (104, 104), (257, 128)])
 def test_eigh_tridiagonal_path_random(ctx, N, nv):
     """sizes spanning several 32-panels / 64-blocks and ragged tails"""
     rng = np.random.default_rng(N)
@@ -98,6 +98,16 @@ def test_eigh_degenerate_clean_supercell_and_identity(ctx):
     D[0] = 2.5 * np.eye(20)
     D[1] = np.diag(np.arange(20) % 3).astype(complex)
     check_eigh(ctx, D, 20)
+    # the on-chip reduction forms its reflectors with in-line reciprocals: zero columns (tau = 0), an
+    # all-zero matrix, and entries far from 1
+    Z = np.zeros((4, 64, 64), dtype=complex)
+    Z[1] = np.diag(np.linspace(-1, 1, 64))
+    Z[1][5, 40] = Z[1][40, 5] = 0.25          # one coupled pair in an otherwise diagonal matrix
+    rng = np.random.default_rng(64)
+    A = rng.standard_normal((64, 64)) + 1j * rng.standard_normal((64, 64))
+    Z[2] = 1e6 * (A + A.conj().T)
+    Z[3] = 1e-6 * (A + A.conj().T)
+    check_eigh(ctx, Z, 64)
 
 
 def test_eigh_config3_and_config5_matrices(ctx):
