@@ -90,6 +90,38 @@ def eigenphases(W: np.ndarray):
     return th[order], np.abs(lam)[order]
 
 
+def window_frames(H_loop: np.ndarray, band_lo: int, band_hi: int):
+    """NEXT-3 (PAPER.md:79 ``bands`` "the list of band indices"): frames of the bands
+    [band_lo, band_hi) in ascending-energy order, U_j = V_j[:, band_lo:band_hi].
+
+    Returns (frames, mingap) with mingap = min over the loop of the gaps at BOTH edges of the window,
+    E[band_lo] - E[band_lo-1] (if band_lo > 0) and E[band_hi] - E[band_hi-1] (if band_hi < N)."""
+    frames = []
+    mingap = np.inf
+    for j in range(H_loop.shape[0]):
+        E, V = np.linalg.eigh(H_loop[j])
+        frames.append(V[:, band_lo:band_hi])
+        if band_lo > 0:
+            mingap = min(mingap, E[band_lo] - E[band_lo - 1])
+        if band_hi < E.shape[0]:
+            mingap = min(mingap, E[band_hi] - E[band_hi - 1])
+    return frames, mingap
+
+
+def wilson_surface_window(H_grid: np.ndarray, band_lo: int, band_hi: int, direction: int, close=None):
+    """``wilson_surface`` for the band window [band_lo, band_hi) instead of the lowest n_occ bands."""
+    grid_ndim = H_grid.ndim - 3
+    L = _loops_view(H_grid, grid_ndim, direction)
+    m = band_hi - band_lo
+    th = np.empty((L.shape[0], m))
+    ab = np.empty((L.shape[0], m))
+    mg = np.empty(L.shape[0])
+    for b in range(L.shape[0]):
+        frames, mg[b] = window_frames(L[b], band_lo, band_hi)
+        th[b], ab[b] = eigenphases(wilson_matrix(frames, close))
+    return th, ab, mg
+
+
 def wilson_loop(H_loop: np.ndarray, n_occ: int, close=None):
     """One loop: H_loop [N1][N][N] -> (theta [n_occ], |lambda| [n_occ], mingap)."""
     frames, mingap = occupied_frames(H_loop, n_occ)

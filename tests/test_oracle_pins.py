@@ -85,6 +85,34 @@ def test_qwz_chern_number_is_one_paper_value():
     assert wo.chern_number(th0) == 0
 
 
+def test_band_windows_upper_band_completeness_and_edge_gaps():
+    """NEXT-3 band windows [lo, hi) (PAPER.md:79 ``bands``): (i) the Chern numbers of all bands sum to
+    zero, so Eq. 4's upper band carries -C of the printed lower-band value; (ii) its loops equal the
+    scalar products of the closed-form upper eigenvectors; (iii) the window of ALL bands has W = 1
+    (completeness of the eigenbasis, periodic gauge); (iv) the gap flag looks at both window edges."""
+    H = wl.qwz_grid(60, 60)
+    th_up, _, mg = wo.wilson_surface_window(H[None], 1, 2, direction=1)
+    assert wo.chern_number(th_up) == -int(GOLD["qwz_eq4_chern"])
+    assert mg.min() > 0.9
+    n1 = 60
+    for i2 in (0, 7, 31):
+        ky = 2 * np.pi * i2 / 60
+        vecs = [lower_band_vector(-qwz_d(2 * np.pi * j / n1, ky)) for j in range(n1)]   # upper band of d.sigma
+        w = 1.0 + 0j
+        for j in range(n1):
+            w *= np.vdot(vecs[j], vecs[(j + 1) % n1])
+        assert abs(np.angle(np.exp(1j * (th_up[i2, 0] - np.angle(w))))) < 1e-12
+    Hb = wl.config1_grid(12, 5)[None]
+    th_all, ab_all, mg_all = wo.wilson_surface_window(Hb, 0, 4, direction=1)
+    assert np.abs(th_all).max() < 1e-12 and np.abs(ab_all - 1).max() < 1e-12
+    assert np.all(np.isinf(mg_all))                       # no edge inside the spectrum
+    th_lo, _, mg_lo = wo.wilson_surface_window(Hb, 0, 2, direction=1)
+    th_ref, _, mg_ref = wo.wilson_surface(Hb, 2, direction=1)
+    assert np.array_equal(th_lo, th_ref) and np.array_equal(mg_lo, mg_ref)
+    _, _, mg_mid = wo.wilson_surface_window(Hb, 1, 3, direction=1)
+    assert mg_mid.max() < 1e-12                           # BHZ bands are two-fold degenerate: both edges closed
+
+
 def test_qwz_chern_matches_berry_curvature_plaquette_sum():
     """Independent route (Eq. 5, PAPER.md:69 with A = i<u|d_k u>, Eq. 1): lattice field strength
     from closed-form eigenvectors, summed over plaquettes.  <u_k|u_{k+dk}> ~ 1 - i A dk, so the
