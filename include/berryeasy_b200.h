@@ -146,6 +146,22 @@ int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int 
                      double* d_theta1, double* d_theta_nested);
 
 /*
+ * band windows (``bands``, "the list of band indices"): the loop
+ * of the bands [band_lo, band_hi) in ascending-energy order instead of the lowest n_occ (band_lo = 0,
+ * band_hi = n_occ is be_wilson_loop).  The lowest band_hi eigenvectors are computed at every k and the
+ * window's columns are looped; outputs have m = band_hi - band_lo columns.
+ *   d_mingap [loops]: min over the loop of the gaps at BOTH edges of the window, E[band_lo]-E[band_lo-1]
+ *            (band_lo > 0) and E[band_hi]-E[band_hi-1] (band_hi < N); +inf without an inner edge.
+ * 0 <= band_lo < band_hi <= N, else BE_ERR_SHAPE.  All other arguments as in be_wilson_loop /
+ * be_spin_resolved_wilson (m_lo = -1 means m / 2; d_pso [loops][N1][m]).
+ */
+int be_wilson_loop_window(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int band_lo, int band_hi,
+                          int dir, const void* d_close, double* d_theta, double* d_abs, double* d_mingap);
+int be_spin_resolved_wilson_window(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int band_lo,
+                                   int band_hi, int dir, const void* dS, int S_is_diag, int m_lo,
+                                   const void* d_close, double* d_theta_lo, double* d_theta_hi, double* d_pso);
+
+/*
  * S6 -- spin-resolved Wilson loop (``WSpinSurf``): at every k the reduced
  * projected spin operator U^dagger S U (the non-zero block of P S P) is
  * diagonalized, S_red = V Sigma V^dagger (ascending); the occupied frame is rotated into the

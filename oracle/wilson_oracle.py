@@ -167,18 +167,21 @@ def projected_spin(U: np.ndarray, S: np.ndarray):
     return U.conj().T @ SU
 
 
-def spin_resolved_loop(H_loop: np.ndarray, n_occ: int, S, m_lo: int | None = None, close=None):
+def spin_resolved_loop(H_loop: np.ndarray, n_occ: int, S, m_lo: int | None = None, close=None, band_lo: int = 0):
     """Wilson loop of the negative (lower) and positive (upper) eigenstates of the
     PSO.  R10: the split is by count m_lo (default n_occ/2) on ascending PSO eigenvalues; the
     closing link uses Phi U_0 V_0^sigma.
 
-    Returns (theta_lo [m_lo], theta_hi [n_occ-m_lo], pso [N1][n_occ], abs_lo, abs_hi, mingap).
+    ``band_lo`` > 0 (NEXT-3): the bands [band_lo, n_occ) instead of the lowest n_occ, m = n_occ - band_lo.
+
+    Returns (theta_lo [m_lo], theta_hi [m-m_lo], pso [N1][m], abs_lo, abs_hi, mingap).
     """
+    m = n_occ - band_lo
     if m_lo is None or m_lo < 0:
-        m_lo = n_occ // 2
-    frames, mingap = occupied_frames(H_loop, n_occ)
+        m_lo = m // 2
+    frames, mingap = window_frames(H_loop, band_lo, n_occ) if band_lo else occupied_frames(H_loop, n_occ)
     lo, hi = [], []
-    pso = np.empty((len(frames), n_occ))
+    pso = np.empty((len(frames), m))
     for j, U in enumerate(frames):
         sig, V = np.linalg.eigh(projected_spin(U, S))
         pso[j] = sig
@@ -189,18 +192,19 @@ def spin_resolved_loop(H_loop: np.ndarray, n_occ: int, S, m_lo: int | None = Non
     return th_lo, th_hi, pso, ab_lo, ab_hi, mingap
 
 
-def spin_resolved_surface(H_grid, n_occ, direction, S, m_lo=None, close=None):
+def spin_resolved_surface(H_grid, n_occ, direction, S, m_lo=None, close=None, band_lo: int = 0):
     """``WSpinSurf``: spin_resolved_loop for every transverse point / batch entry."""
+    m = n_occ - band_lo
     if m_lo is None or m_lo < 0:
-        m_lo = n_occ // 2
+        m_lo = m // 2
     grid_ndim = H_grid.ndim - 3
     L = _loops_view(H_grid, grid_ndim, direction)
     B, n1 = L.shape[0], L.shape[1]
     th_lo = np.empty((B, m_lo))
-    th_hi = np.empty((B, n_occ - m_lo))
-    pso = np.empty((B, n1, n_occ))
+    th_hi = np.empty((B, m - m_lo))
+    pso = np.empty((B, n1, m))
     for b in range(B):
-        th_lo[b], th_hi[b], pso[b], _, _, _ = spin_resolved_loop(L[b], n_occ, S, m_lo, close)
+        th_lo[b], th_hi[b], pso[b], _, _, _ = spin_resolved_loop(L[b], n_occ, S, m_lo, close, band_lo)
     return th_lo, th_hi, pso
 
 

@@ -19,7 +19,7 @@ EXPORTS = [
     "be_launch_count", "be_eigh_batched", "be_wilson_loop", "be_nested_wilson",
     "be_spin_resolved_wilson", "be_winding", "be_wilson_loop_host", "be_spin_resolved_wilson_host",
     "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched", "be_set_chunk_pipeline", "be_bloch_coefficients", "be_assemble_bloch", "be_plaquette_flux", "be_wilson_loop_bloch",
-    "be_spin_resolved_wilson_bloch",
+    "be_spin_resolved_wilson_bloch", "be_wilson_loop_window", "be_spin_resolved_wilson_window",
 ]
 
 
@@ -58,6 +58,8 @@ def load_library():
     lib.be_launch_count.restype = i64
     lib.be_eigh_batched.argtypes = [vp, vp, i64, ci, ci, vp, vp, vp]
     lib.be_wilson_loop.argtypes = [vp, vp, gp, ci, ci, vp, vp, vp, vp]
+    lib.be_wilson_loop_window.argtypes = [vp, vp, gp, ci, ci, ci, vp, vp, vp, vp]
+    lib.be_spin_resolved_wilson_window.argtypes = [vp, vp, gp, ci, ci, ci, vp, ci, ci, vp, vp, vp, vp]
     lib.be_nested_wilson.argtypes = [vp, vp, gp, ci, ci, ci, ci, ci, ci, dbl, vp, vp, vp, vp]
     lib.be_spin_resolved_wilson.argtypes = [vp, vp, gp, ci, ci, vp, ci, ci, vp, vp, vp, vp]
     lib.be_winding.argtypes = [vp, vp, i64, ci, ci, vp]
@@ -178,8 +180,12 @@ class Context:
         return (E, U, info) if want_info else (E, U)
 
     # ------------------------------------------------------------------ be_wilson_loop
-    def wilson_loop(self, H_grid, n_occ, direction, close=None, want_abs=True, want_mingap=True):
-        """H_grid [batch][dims...][N][N] -> theta [loops][n_occ], |lambda| or None, mingap or None."""
+    def wilson_loop(self, H_grid, n_occ, direction, close=None, want_abs=True, want_mingap=True, band_lo=0):
+        """H_grid [batch][dims...][N][N] -> theta [loops][m], |lambda| or None, mingap or None.
+
+        Bands [band_lo, n_occ) in ascending-energy order (be_wilson_loop_window when band_lo > 0)."""
+        if band_lo:
+            return self._wilson_loop_window(H_grid, band_lo, n_occ, direction, close, want_abs, want_mingap)
         _dev(H_grid, torch.complex128, "H_grid")
         nd = H_grid.dim() - 3
         g = _grid_of(H_grid, nd)
@@ -196,6 +202,48 @@ class Context:
         _check(self.lib, self.lib.be_wilson_loop(self._h, _ptr(H_grid), C.byref(g), n_occ, direction,
                                                  _ptr(close), _ptr(theta), _ptr(ab), _ptr(mg)))
         return theta, ab, mg
+
+    def _wilson_loop_window(self, H_grid, band_lo, band_hi, direction, close, want_abs, want_mingap):
+        _dev(H_grid, torch.complex128, "H_grid")
+        nd = H_grid.dim() - 3
+        g = _grid_of(H_grid, nd)
+        loops = H_grid.shape[0]
+        for a in range(nd):
+            if a != direction:
+                loops *= H_grid.shape[1 + a]
+        dev = H_grid.device
+        m = max(band_hi - band_lo, 0)
+        theta = torch.empty((loops, m), dtype=torch.float64, device=dev)
+        ab = torch.empty((loops, m), dtype=torch.float64, device=dev) if want_abs else None
+        mg = torch.empty((loops,), dtype=torch.float64, device=dev) if want_mingap else None
+        if close is not None:
+            _dev(close, torch.complex128, "close")
+        _check(self.lib, self.lib.be_wilson_loop_window(self._h, _ptr(H_grid), C.byref(g), band_lo, band_hi, direction,
+                                                        _ptr(close), _ptr(theta), _ptr(ab), _ptr(mg)))
+        return theta, ab, mg
+
+    def spin_resolved_wilson_window(self, H_grid, band_lo, band_hi, direction, S, m_lo=-1, close=None, want_pso=True):
+        """be_spin_resolved_wilson_window: the spin-resolved loop of the bands [band_lo, band_hi)."""
+        _dev(H_grid, torch.complex128, "H_grid")
+        nd = H_grid.dim() - 3
+        g = _grid_of(H_grid, nd)
+        loops = H_grid.shape[0]
+        for a in range(nd):
+            if a != direction:
+                loops *= H_grid.shape[1 + a]
+        n1 = H_grid.shape[1 + direction]
+        is_diag = 1 if S.dim() == 1 else 0
+        _dev(S, torch.float64 if is_diag else torch.complex128, "S")
+        m = max(band_hi - band_lo, 0)
+        mlo = m // 2 if m_lo < 0 else m_lo
+        dev = H_grid.device
+        lo = torch.empty((loops, mlo), dtype=torch.float64, device=dev)
+        hi = torch.empty((loops, max(m - mlo, 0)), dtype=torch.float64, device=dev)
+        pso = torch.empty((loops, n1, m), dtype=torch.float64, device=dev) if want_pso else None
+        _check(self.lib, self.lib.be_spin_resolved_wilson_window(self._h, _ptr(H_grid), C.byref(g), band_lo, band_hi,
+                                                                 direction, _ptr(S), is_diag, m_lo, _ptr(close),
+                                                                 _ptr(lo), _ptr(hi), _ptr(pso)))
+        return lo, hi, pso
 
     # ------------------------------------------------------------------ be_spin_resolved_wilson
     def spin_resolved_wilson(self, H_grid, n_occ, direction, S, m_lo=-1, close=None, want_pso=True):

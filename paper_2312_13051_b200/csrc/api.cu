@@ -6,7 +6,7 @@
 #include <string.h>
 
 // stage entry points defined in wilson.cu
-int be_mingap(be_ctx* ctx, const double* E, int N, int m, int n1, int64_t loops, double* out);
+int be_mingap(be_ctx* ctx, const double* E, int N, int lo, int hi, int n1, int64_t loops, double* out);
 int be_scale_rows(be_ctx* ctx, const cplx* X, const double* S, cplx* SX, int N, int64_t total);
 int be_winding_impl(be_ctx* ctx, const double* theta, int64_t n_cycles, int n_points, int m, double* wind);
 int be_nested_select_small(be_ctx* ctx, const cplx* W, int64_t cnt, int m, int wb_lo, int wb_hi,

@@ -4,7 +4,7 @@
 #include <string.h>
 #include <vector>
 
-int be_mingap(be_ctx* ctx, const double* E, int N, int m, int n1, int64_t loops, double* out);
+int be_mingap(be_ctx* ctx, const double* E, int N, int lo, int hi, int n1, int64_t loops, double* out);
 int be_scale_rows(be_ctx* ctx, const cplx* X, const double* S, cplx* SX, int N, int64_t total);
 int be_nested_select_small(be_ctx* ctx, const cplx* W, int64_t cnt, int m, int wb_lo, int wb_hi,
                            double cut, double* theta1, cplx* Vs);
@@ -37,9 +37,11 @@ struct SpinArgs {
 };
 
 // bytes of scratch one loop needs (upper bound), plain or spin-resolved
-static size_t per_loop_bytes(int N, int m, int n1, bool spin) {
+static size_t per_loop_bytes(int N, int m, int n1, bool spin, int lo = 0) {
   const size_t fr = (size_t)N * m * sizeof(cplx);
-  size_t b = (size_t)n1 * (be_eigh_scratch_bytes(1, N, m) + fr + (size_t)N * sizeof(double) + 512);
+  // a band window [lo, lo + m) needs the lowest lo + m vectors, then a compact copy of its m columns
+  size_t b = (size_t)n1 * (be_eigh_scratch_bytes(1, N, lo + m) + (size_t)N * (lo + m) * sizeof(cplx) + (lo ? fr : 0) +
+                           (size_t)N * sizeof(double) + 512);
   const size_t mm = (size_t)m * m * sizeof(cplx);
   b += (size_t)n1 * mm + 4 * mm + (size_t)m * 64 + 4096;           // links, products, eigenvalues
   if (spin) {
@@ -106,7 +108,7 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
                          const SpinArgs* sp, HostStage* hs = nullptr, const BlochSrc* bs = nullptr) {
   const int n1 = map.n1;
   const int64_t loops = map.loops;
-  const size_t per = per_loop_bytes(N, m, n1, sp != nullptr);
+  const size_t per = per_loop_bytes(N, m, n1, sp != nullptr, ctx->band_lo);
   int64_t lc = (int64_t)(ctx->ws_limit / per);
   if (lc < 1) lc = 1;
   if (lc > loops) lc = loops;
@@ -227,15 +229,24 @@ static int wilson_chunk(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t 
                         int64_t nl, int64_t cnt, const cplx* d_close, double* d_mingap, const SpinArgs* sp, int mlo,
                         int mhi, cplx* const* Wall) {
   {
+    const int lo = ctx->band_lo, hi = lo + m;   // band window [lo, hi): the lowest hi vectors are computed
     double* E = (double*)be_arena_alloc(ctx, (size_t)cnt * N * sizeof(double));
-    cplx* X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
+    cplx* X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * hi * sizeof(cplx));
     if (!E || !X) return BE_ERR_NOMEM;
     {
-      const int r = be_eigh_frames(ctx, H, map, gl0, cnt, N, m, m + 1, E, X, nullptr);
+      const int r = be_eigh_frames(ctx, H, map, gl0, cnt, N, hi, hi + 1, E, X, nullptr);
       ctx->bloch = nullptr;   // only H(k) is generated; the PSO solve below reads S_red from memory
       BE_TRY(r);
     }
-    if (d_mingap) BE_TRY(be_mingap(ctx, E, N, m, n1, nl, d_mingap + l0));
+    if (d_mingap) BE_TRY(be_mingap(ctx, E, N, lo, hi, n1, nl, d_mingap + l0));
+    if (lo > 0) {
+      // frames are column-major N x hi per k-point: columns lo .. hi-1 are one contiguous run per frame
+      cplx* F = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
+      if (!F) return BE_ERR_NOMEM;
+      BE_CUDA(cudaMemcpy2DAsync(F, (size_t)N * m * sizeof(cplx), X + (size_t)lo * N, (size_t)N * hi * sizeof(cplx),
+                                (size_t)N * m * sizeof(cplx), (size_t)cnt, cudaMemcpyDeviceToDevice, ctx->stream));
+      X = F;
+    }
     if (!sp) {
       cplx* W = nullptr;
       BE_TRY(be_chain_product(ctx, X, N, m, nl, n1, d_close, n1 - 1, Wall[0] + l0 * (int64_t)m * m, &W));
@@ -281,6 +292,42 @@ extern "C" int be_wilson_loop(be_ctx* ctx, const void* dH_grid, const be_grid* g
   BE_TRY(make_map(grid, dir, &map));
   return wilson_device(ctx, (const cplx*)dH_grid, map, grid->N, n_occ, (const cplx*)d_close,
                        d_theta, d_abs, d_mingap, nullptr);
+}
+
+extern "C" int be_wilson_loop_window(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int band_lo, int band_hi,
+                                     int dir, const void* d_close, double* d_theta, double* d_abs, double* d_mingap) {
+  if (band_lo < 0 || band_hi <= band_lo) return BE_ERR_SHAPE;
+  BE_TRY(check_common(ctx, dH_grid, grid, band_hi, dir));
+  if (!d_theta) return BE_ERR_NULL;
+  if ((d_close && !aligned(d_close, 16)) || !aligned(d_theta, 8)) return BE_ERR_ALIGN;
+  GridMap map;
+  BE_TRY(make_map(grid, dir, &map));
+  ctx->band_lo = band_lo;
+  const int rc = wilson_device(ctx, (const cplx*)dH_grid, map, grid->N, band_hi - band_lo, (const cplx*)d_close,
+                               d_theta, d_abs, d_mingap, nullptr);
+  ctx->band_lo = 0;
+  return rc;
+}
+
+extern "C" int be_spin_resolved_wilson_window(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int band_lo,
+                                              int band_hi, int dir, const void* dS, int S_is_diag, int m_lo,
+                                              const void* d_close, double* d_theta_lo, double* d_theta_hi,
+                                              double* d_pso) {
+  if (band_lo < 0 || band_hi <= band_lo) return BE_ERR_SHAPE;
+  BE_TRY(check_common(ctx, dH_grid, grid, band_hi, dir));
+  if (!dS) return BE_ERR_NULL;
+  const int m = band_hi - band_lo;
+  if (m_lo < 0) m_lo = m / 2;
+  if (m_lo > m) return BE_ERR_SHAPE;
+  if (!aligned(dS, S_is_diag ? 8 : 16) || (d_close && !aligned(d_close, 16))) return BE_ERR_ALIGN;
+  GridMap map;
+  BE_TRY(make_map(grid, dir, &map));
+  SpinArgs sp{dS, S_is_diag, m_lo, d_theta_lo, d_theta_hi, d_pso};
+  ctx->band_lo = band_lo;
+  const int rc = wilson_device(ctx, (const cplx*)dH_grid, map, grid->N, m, (const cplx*)d_close,
+                               nullptr, nullptr, nullptr, &sp);
+  ctx->band_lo = 0;
+  return rc;
 }
 
 extern "C" int be_spin_resolved_wilson(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_occ,

@@ -90,6 +90,7 @@ struct be_ctx {
   int* dR_buf; size_t dR_cap;      // device copy of the lattice vectors of a *_bloch call
   const struct BlochSrc* bloch;   // set while the H eigensolve of a *_bloch call runs: H(k) is assembled, not read
   int chunk_pipeline;         // be_set_chunk_pipeline (default 0)
+  int band_lo;                // band window [band_lo, band_lo + m) of the running Wilson call (0 = lowest m bands)
   int split_after_tridiag;    // consumed by be_eigh_large: switch to stream2 after S1a
   int gemm_pad;               // zgemm launches with padded shared memory: at most one GEMM CTA per SM,
                               // leaving room for one k_hemv CTA of the other stream

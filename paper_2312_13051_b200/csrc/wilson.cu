@@ -6,17 +6,18 @@
 
 namespace {
 
-// min over the loop of E[m] - E[m-1] (R8); +inf when m == N.
-__global__ void k_mingap(const double* __restrict__ E, int N, int m, int n1, int64_t loops,
+// min over the loop of the gaps at the edges of the band window [lo, hi): E[hi] - E[hi-1] (R8) and,
+// for lo > 0, E[lo] - E[lo-1]; +inf when the window has no edge inside the spectrum.
+__global__ void k_mingap(const double* __restrict__ E, int N, int lo, int hi, int n1, int64_t loops,
                          double* __restrict__ out) {
   const int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (l >= loops) return;
   double g = INFINITY;
-  if (m < N)
-    for (int j = 0; j < n1; ++j) {
-      const double* e = E + (l * n1 + j) * (int64_t)N;
-      g = fmin(g, e[m] - e[m - 1]);
-    }
+  for (int j = 0; j < n1; ++j) {
+    const double* e = E + (l * n1 + j) * (int64_t)N;
+    if (hi < N) g = fmin(g, e[hi] - e[hi - 1]);
+    if (lo > 0) g = fmin(g, e[lo] - e[lo - 1]);
+  }
   out[l] = g;
 }
 
@@ -130,8 +131,8 @@ __global__ void k_nested_select_small(const cplx* __restrict__ W, int64_t cnt, i
 
 #define LAUNCH_CHECK() do { ctx->launches++; cudaError_t e__ = cudaGetLastError(); if (e__ != cudaSuccess) return (int)e__; } while (0)
 
-int be_mingap(be_ctx* ctx, const double* E, int N, int m, int n1, int64_t loops, double* out) {
-  k_mingap<<<(unsigned)((loops + 127) / 128), 128, 0, ctx->stream>>>(E, N, m, n1, loops, out);
+int be_mingap(be_ctx* ctx, const double* E, int N, int lo, int hi, int n1, int64_t loops, double* out) {
+  k_mingap<<<(unsigned)((loops + 127) / 128), 128, 0, ctx->stream>>>(E, N, lo, hi, n1, loops, out);
   LAUNCH_CHECK();
   return BE_OK;
 }

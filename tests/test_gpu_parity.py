@@ -630,6 +630,53 @@ def test_fused_bloch_generation_matches_materialised_grid(ctx):
     assert phase_dist(th5.cpu().numpy(), th5o) <= PH_TOL
 
 
+def test_band_windows_match_oracle(ctx):
+    """NEXT-3: be_wilson_loop_window / be_spin_resolved_wilson_window on the Jacobi, on-chip and blocked
+    eigensolver paths: phases, both-edge gap flag, the paper's upper-band Chern number, completeness."""
+    from paper_2312_13051_b200.binding import BerryEasyError
+    # Eq. 4, upper band: C = -1
+    H = wl.qwz_grid(40, 40)[None]
+    th, ab, mg = ctx.wilson_loop(dev(H), 2, 1, band_lo=1)
+    tho, abo, mgo = wo.wilson_surface_window(H, 1, 2, 1)
+    assert phase_dist(th.cpu().numpy(), tho) <= PH_TOL
+    assert np.abs(mg.cpu().numpy() - mgo).max() < 1e-12
+    assert wo.chern_number(th.cpu().numpy()) == -1
+    # BHZ: unoccupied pair; all four bands (W = 1, no inner edge); the degenerate middle window is flagged
+    Hb = wl.config1_grid(30, 7)[None]
+    th, ab, mg = ctx.wilson_loop(dev(Hb), 4, 1, band_lo=2)
+    tho, abo, mgo = wo.wilson_surface_window(Hb, 2, 4, 1)
+    assert phase_dist(th.cpu().numpy(), tho) <= PH_TOL and np.abs(mg.cpu().numpy() - mgo).max() < 1e-12
+    th, ab, mg = ctx.wilson_loop(dev(Hb), 4, 1, band_lo=0)
+    assert np.abs(th.cpu().numpy()).max() < 1e-10 and np.all(np.isinf(mg.cpu().numpy()))
+    _, _, mg = ctx.wilson_loop(dev(Hb), 3, 1, band_lo=1)
+    assert mg.cpu().numpy().max() < 1e-10
+    S = wl.bhz4_spin_z()
+    lo, hi, pso = ctx.spin_resolved_wilson_window(dev(Hb), 2, 4, 1, dev(S))
+    loo, hio, psoo = wo.spin_resolved_surface(Hb, 4, 1, S, band_lo=2)
+    assert phase_dist(lo.cpu().numpy(), loo) <= PH_TOL and phase_dist(hi.cpu().numpy(), hio) <= PH_TOL
+    assert np.abs(pso.cpu().numpy() - psoo).max() < 1e-10
+    # on-chip path (N = 64): a window across the gap
+    p5 = wl.config5_parts()
+    H5 = wl.config5_grid(p5, 64, 64, 13, ix=[3], iy=[5, 40])
+    th, ab, mg = ctx.wilson_loop(dev(H5), 40, 1, band_lo=24)      # [1][2][13][64][64]: batch 1, dims (2, 13)
+    tho, abo, mgo = wo.wilson_surface_window(H5, 24, 40, 1)
+    assert mgo.min() > 1e-4
+    assert phase_dist(th.cpu().numpy(), tho) <= PH_TOL and np.abs(mg.cpu().numpy() - mgo).max() < 1e-10
+    # blocked path: the same recipe with 56 spatial orbitals (N = 112), window [40, 70) across the gap.  (A
+    # window edge inside the DISORDERED bands of config 3 is no parity case: the oracle's own phases move by
+    # 0.4 rad under a 1e-12 perturbation there, |lambda| down to 1e-16.)
+    p7 = wl.config5_parts(norb_spatial=56)
+    H7 = wl.config5_grid(p7, 64, 64, 17, ix=[3], iy=[5, 40])
+    th, ab, mg = ctx.wilson_loop(dev(H7), 70, 1, band_lo=40)
+    tho, abo, mgo = wo.wilson_surface_window(H7, 40, 70, 1)
+    assert mgo.min() > 1e-2 and np.abs(mg.cpu().numpy() - mgo).max() < 1e-10
+    assert phase_dist(th.cpu().numpy(), tho) <= PH_TOL
+    with pytest.raises(BerryEasyError):
+        ctx.wilson_loop(dev(Hb), 2, 1, band_lo=2)      # empty window
+    with pytest.raises(BerryEasyError):
+        ctx.wilson_loop(dev(Hb), 5, 1, band_lo=1)      # band_hi > N
+
+
 def test_launch_counter_counts_kernels(ctx):
     n0 = ctx.launch_count()
     ctx.wilson_loop(dev(wl.config1_grid(6, 2)[None]), 2, 1)

@@ -351,6 +351,11 @@ def test_bhz_spin_resolved_windings_and_block_reduction():
     assert abs(wo.winding(th) - GOLD["bhz_total_winding"]) < 1e-10
     # R11: lower sector (S_z = -1) winds +1 => C_down = -1, C_up = +1, C_s = +1 (paper sign)
     assert round(w_lo) == 1 and round(w_hi) == -1
+    # band window [2, 4) (NEXT-3): within each spin block the two bands carry opposite Chern numbers,
+    # so the unoccupied pair winds the other way, sector by sector
+    ulo, uhi, upso = wo.spin_resolved_surface(H[None], 4, 1, S, band_lo=2)
+    assert np.allclose(np.abs(upso), GOLD["pso_abs_eigenvalue_no_soc"], atol=1e-12)
+    assert round(wo.winding(ulo)) == -1 and round(wo.winding(uhi)) == 1
     # block reduction: spin-down block (indices 1,3) is -sin kx sx + sin ky sy + M sz etc.
     for j in (0, 5, 17):
         ky = 2 * np.pi * j / n2
