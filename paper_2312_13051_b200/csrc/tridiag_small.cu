@@ -47,7 +47,7 @@ __device__ __forceinline__ void hemv_rows(const cplx* __restrict__ A, const cplx
   }
 }
 
-__global__ void __launch_bounds__(TS_THREADS, 4) k_tridiag_smem(const cplx* __restrict__ H, GridMap map, int64_t loop0,
+__global__ void __launch_bounds__(TS_THREADS, 5) k_tridiag_smem(const cplx* __restrict__ H, GridMap map, int64_t loop0,
                                                                 cplx* __restrict__ Bw, double* __restrict__ dd,
                                                                 double* __restrict__ ee, cplx* __restrict__ tau, int N) {
   extern __shared__ cplx tsm[];             // A: lower triangle packed by columns (pk), y [N], w~ [N]
@@ -153,6 +153,8 @@ int be_tridiag_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loo
   if (N > TS_MAXN) return BE_ERR_UNSUPPORTED;
   const size_t sh = ((size_t)N * (N + 1) / 2 + 2 * N) * sizeof(cplx);
   if (sh > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_tridiag_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
+  // six CTAs of 35 KB per SM need the full shared-memory carve-out
+  BE_CUDA(cudaFuncSetAttribute(k_tridiag_smem, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
   be_prof_begin(ctx, PK_HEMV);
   k_tridiag_smem<<<(unsigned)cnt, TS_THREADS, sh, ctx->stream>>>(H, map, loop0, Bw, d, e, tau, N);
   be_prof_end(ctx, PK_HEMV, (double)cnt * N * N * 32.0, (double)cnt * (16.0 / 3.0) * N * (double)N * N);
