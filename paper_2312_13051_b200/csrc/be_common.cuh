@@ -225,6 +225,8 @@ size_t be_eigh_large_scratch_bytes(int64_t cnt, int N, int nv);
 constexpr int TS_MAXN = 104;   // largest matrix reduced entirely in shared memory (tridiag_small.cu)
 int be_tridiag_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N, cplx* Bw,
                      double* d, double* e, cplx* tau);
+int be_backtransform_small(be_ctx* ctx, const cplx* Bw, const cplx* tau, const double* Z, cplx* X, int64_t cnt, int N,
+                           int nv);
 size_t be_cluster_orth_scratch_bytes(int64_t cnt, int N, int nv);
 int be_cluster_orth(be_ctx* ctx, const double* lam, const double* tnorm, const int* blk, double* Z, int64_t cnt, int N,
                     int nv, double ctol, int* info, void* scratch, int find, int rounds);

@@ -866,7 +866,8 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
   }
   if (nv == 0) return BE_OK;
 
-  // ---- S1c: back-transform X = conj(Q) Z with compact-WY blocks, last block first
+  // ---- S1c: back-transform X = conj(Q) Z: on chip for small matrices, else compact-WY blocks, last block first
+  if (on_chip) return be_backtransform_small(ctx, s.Bw, s.tau, s.Z, X, cnt, N, nv);
   {
     const int tr = (N + 31) / 32, tv = (nv + 31) / 32;
     k_z2x<<<(unsigned)(cnt * tr * tv), 256, 0, st>>>(s.Z, X, N, nv, tr, tv);

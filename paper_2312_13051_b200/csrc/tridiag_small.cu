@@ -146,6 +146,73 @@ __global__ void __launch_bounds__(TS_THREADS, 5) k_tridiag_smem(const cplx* __re
   if (tid == 0) dd[c * N + N - 1] = A[pk(N - 1, N - 1, N)].x;
 }
 
+
+// ---- S1c for the same sizes: X = conj(Q) Z, Q = H_0 H_1 ... H_{N-2}, reflector by reflector with the
+// eigenvector columns in REGISTERS.  Eight threads share one column (thread = rows part, part + 8, ...), a
+// warp holds four columns; the only communication is the 8-lane butterfly of v^T x, so there is no block
+// barrier after the reflectors have been staged (strict lower triangle packed by columns, unit entries
+// stored).  Replaces, for N <= TS_MAXN, the compact-WY chain (V extraction, V^H V, T, three GEMMs), whose
+// 64 x 64 operands made it HBM bound at ~1 MB of traffic per matrix.
+//   The work matrix is B = conj(H) (see above), so eigenvectors of H are conj(Q) Z:
+//   x[i+1:] -= conj(tau_i) conj(v_i) (v_i^T x[i+1:]),  i = N-2 .. 0,  x real on entry.
+template <int RPT>
+__global__ void __launch_bounds__(256, RPT <= 8 ? 3 : 2) k_backtransform_small(const cplx* __restrict__ Bw, const cplx* __restrict__ tau,
+                                                                const double* __restrict__ Z, cplx* __restrict__ X,
+                                                                int N, int nv) {
+  extern __shared__ cplx bsm[];             // V packed: column i holds rows i+1 .. N-1 at i (N-1) - i (i-1)/2
+  cplx* vs = bsm;
+  cplx* tc = bsm + (size_t)N * (N - 1) / 2;   // conj(tau) [N]
+  const int64_t c = blockIdx.x;
+  const int tid = threadIdx.x, part = tid & 7;
+  const int j = blockIdx.y * 32 + (tid >> 3);
+  const cplx* Bc = Bw + c * (int64_t)N * N;
+  for (int idx = tid; idx < N * N; idx += 256) {
+    const int r = idx % N, i = idx / N;
+    if (r > i && i < N - 1) vs[i * (N - 1) - (i * (i - 1)) / 2 + (r - i - 1)] = (r == i + 1) ? mkc(1.0, 0.0) : Bc[idx];
+  }
+  for (int i = tid; i < N - 1; i += 256) tc[i] = cconj(tau[c * N + i]);
+  cplx z[RPT];
+#pragma unroll
+  for (int k = 0; k < RPT; ++k) {
+    const int r = part + 8 * k;
+    z[k] = (r < N && j < nv) ? mkc(Z[c * (int64_t)N * nv + (int64_t)r * nv + j], 0.0) : mkc(0.0, 0.0);
+  }
+  __syncthreads();
+  for (int i = N - 2; i >= 0; --i) {
+    const cplx* v = vs + i * (N - 1) - (i * (i - 1)) / 2 - (i + 1);   // v[r], r = i+1 .. N-1
+    cplx d0 = mkc(0.0, 0.0), d1 = mkc(0.0, 0.0);
+#pragma unroll
+    for (int k = 0; k < RPT; ++k) {
+      if (8 * k + 7 > i) {
+        const int r = part + 8 * k;
+        if (r > i && r < N) { if (k & 1) cfma(d1, v[r], z[k]); else cfma(d0, v[r], z[k]); }
+      }
+    }
+    d0 = cadd(d0, d1);
+#pragma unroll
+    for (int m = 1; m < 8; m <<= 1) {
+      d0.x += __shfl_xor_sync(0xffffffffu, d0.x, m);
+      d0.y += __shfl_xor_sync(0xffffffffu, d0.y, m);
+    }
+    const cplx g = cmul(tc[i], d0);
+#pragma unroll
+    for (int k = 0; k < RPT; ++k) {
+      if (8 * k + 7 > i) {
+        const int r = part + 8 * k;
+        if (r > i && r < N) cfms(z[k], cconj(v[r]), g);
+      }
+    }
+  }
+  if (j < nv) {
+    cplx* Xc = X + c * (int64_t)N * nv + (int64_t)j * N;
+#pragma unroll
+    for (int k = 0; k < RPT; ++k) {
+      const int r = part + 8 * k;
+      if (r < N) Xc[r] = z[k];
+    }
+  }
+}
+
 }  // namespace
 
 int be_tridiag_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N, cplx* Bw,
@@ -158,6 +225,25 @@ int be_tridiag_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loo
   be_prof_begin(ctx, PK_HEMV);
   k_tridiag_smem<<<(unsigned)cnt, TS_THREADS, sh, ctx->stream>>>(H, map, loop0, Bw, d, e, tau, N);
   be_prof_end(ctx, PK_HEMV, (double)cnt * N * N * 32.0, (double)cnt * (16.0 / 3.0) * N * (double)N * N);
+  ctx->launches++;
+  return (int)cudaGetLastError();
+}
+
+int be_backtransform_small(be_ctx* ctx, const cplx* Bw, const cplx* tau, const double* Z, cplx* X, int64_t cnt, int N,
+                           int nv) {
+  if (N > TS_MAXN) return BE_ERR_UNSUPPORTED;
+  const size_t sh = ((size_t)N * (N - 1) / 2 + N) * sizeof(cplx);
+  const dim3 grid((unsigned)cnt, (unsigned)((nv + 31) / 32));
+  be_prof_begin(ctx, PK_GEMM);
+  if (N <= 64) {
+    if (sh > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_backtransform_small<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
+    BE_CUDA(cudaFuncSetAttribute(k_backtransform_small<8>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    k_backtransform_small<8><<<grid, 256, sh, ctx->stream>>>(Bw, tau, Z, X, N, nv);
+  } else {
+    BE_CUDA(cudaFuncSetAttribute(k_backtransform_small<13>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
+    k_backtransform_small<13><<<grid, 256, sh, ctx->stream>>>(Bw, tau, Z, X, N, nv);
+  }
+  be_prof_end(ctx, PK_GEMM, (double)cnt * (16.0 * N * N + 24.0 * N * nv), (double)cnt * 8.0 * N * (double)N * nv);
   ctx->launches++;
   return (int)cudaGetLastError();
 }
