@@ -453,6 +453,71 @@ __global__ void __launch_bounds__(128) k_bisect(const double* __restrict__ dd, c
   blo[c * N + k] = lo; bhi[c * N + k] = hi; bcl[c * N + k] = cnt_lo;
 }
 
+// The same bisection for few wanted eigenvalues (ne <= 64): a block serves mpb = 128 / ne matrices, so
+// that the warps are full (config 5: ne = 33 left one lane alone in the second warp of every block).
+// Same arithmetic as k_bisect in every step (min / max reductions are exact), hence the same bits.
+__global__ void __launch_bounds__(128) k_bisect_packed(const double* __restrict__ dd, const double* __restrict__ ee,
+                                                       double* __restrict__ lam, double* __restrict__ tnorm,
+                                                       double* __restrict__ blo, double* __restrict__ bhi,
+                                                       int* __restrict__ bcl, int N, int64_t count, int ne, int mpb) {
+  extern __shared__ double sh[];   // per matrix of the block: d[N], |e|[N], e2[N]
+  const int tid = threadIdx.x;
+  const int64_t c0 = (int64_t)blockIdx.x * mpb;
+  for (int idx = tid; idx < mpb * N; idx += 128) {
+    const int mi = idx / N, r = idx % N;
+    const int64_t c = c0 + mi;
+    double di = 0.0, er = 0.0;
+    if (c < count) { di = dd[c * N + r]; er = (r < N - 1) ? fabs(ee[c * N + r]) : 0.0; }
+    sh[mi * 3 * N + r] = di; sh[mi * 3 * N + N + r] = er;
+  }
+  __syncthreads();
+  const int mi = tid / ne, k = tid % ne;
+  const int64_t c = c0 + mi;
+  const bool live = mi < mpb && c < count;
+  const double* d = sh + (live ? mi : 0) * 3 * N;
+  const double* ea = d + N;
+  double* e2 = sh + (live ? mi : 0) * 3 * N + 2 * N;
+  double gl = DBL_MAX, gu = -DBL_MAX;
+  for (int r = 0; r < N; ++r) {
+    const double el = (r > 0) ? ea[r - 1] : 0.0, er = ea[r];
+    gl = fmin(gl, d[r] - el - er); gu = fmax(gu, d[r] + el + er);
+  }
+  const double eps = DBL_EPSILON;
+  double tn = fmax(fabs(gl), fabs(gu));
+  if (tn == 0.0) tn = DBL_MIN;
+  gl -= 2.0 * tn * eps * N + 2.0 * DBL_MIN;
+  gu += 2.0 * tn * eps * N + 2.0 * DBL_MIN;
+  const double pivmin = DBL_MIN * fmax(1.0, tn * tn);
+  const double split = fmax(SPLIT_TOL, (double)N) * DBL_EPSILON * tn;
+  if (live) {
+    if (k == 0) tnorm[c] = tn;
+    for (int r = k; r < N; r += ne) { const double v = ea[r] * ea[r]; e2[r] = (v <= split * split) ? 0.0 : v; }
+  }
+  __syncthreads();
+  if (!live) return;
+  double lo = gl, hi = gu;
+  int cnt_lo = 0;
+  const double atol = 0.25 * eps * tn;
+  int depth = (int)ceil(log2((gu - gl) / atol)) + 1;
+  depth = depth < 1 ? 1 : (depth > 120 ? 120 : depth);
+  for (int it = 0; it < depth; ++it) {
+    const double mid = 0.5 * (lo + hi);
+    if (!(mid > lo && mid < hi)) break;
+    int cnt = 0;
+    double q = d[0] - mid;
+    if (fabs(q) < pivmin) q = -pivmin;
+    cnt += (q < 0.0);
+    for (int r = 1; r < N; ++r) {
+      q = d[r] - mid - e2[r - 1] * __drcp_rn(q);
+      if (fabs(q) < pivmin) q = -pivmin;
+      cnt += (q < 0.0);
+    }
+    if (cnt > k) hi = mid; else { lo = mid; cnt_lo = cnt; }
+  }
+  lam[c * N + k] = 0.5 * (lo + hi);
+  blo[c * N + k] = lo; bhi[c * N + k] = hi; bcl[c * N + k] = cnt_lo;
+}
+
 // ------------------------------------------------------------------------------------------
 // Inverse iteration, one thread per (matrix, vector).  Pivoted LU of T - sigma I (row
 // interchanges between neighbours only), factors kept in global memory laid out [row][vector] so
@@ -842,7 +907,12 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
       BE_CUDA(cudaFuncSetAttribute(k_invit, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
     }
     be_prof_begin(ctx, PK_BISECT);
-    k_bisect<<<(unsigned)(cnt * nblk), 128, sh, st>>>(s.d, s.e, E, s.tnorm, s.blo, s.bhi, s.bcl, N, nblk, ne);
+    const int mpb = ne <= 64 ? 128 / ne : 1;
+    if (mpb > 1 && 3 * (size_t)mpb * N * sizeof(double) <= 48 * 1024)
+      k_bisect_packed<<<(unsigned)((cnt + mpb - 1) / mpb), 128, 3 * (size_t)mpb * N * sizeof(double), st>>>(
+          s.d, s.e, E, s.tnorm, s.blo, s.bhi, s.bcl, N, cnt, ne, mpb);
+    else
+      k_bisect<<<(unsigned)(cnt * nblk), 128, sh, st>>>(s.d, s.e, E, s.tnorm, s.blo, s.bhi, s.bcl, N, nblk, ne);
     be_prof_end(ctx, PK_BISECT, (double)cnt * N * 24.0, 0.0);
     LAUNCH_CHECK();
     if (nv > 0) {
