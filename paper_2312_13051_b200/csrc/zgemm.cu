@@ -18,8 +18,12 @@
 
 namespace {
 
-constexpr int TM = 64, TN = 64, TK = 16, LDS = 68;  // LDS % 16 == 4: conflict-free fragment loads
-constexpr int NTHREADS = 256;
+constexpr bool M3 = true;   // 3-multiplication complex product (see the main loop)
+// 3M keeps three accumulator sets (~190 registers): 64 x 32 tiles on 128 threads, so that two CTAs still
+// share an SM and one CTA's epilogue overlaps the other's main loop
+constexpr int TM = 64, TN = M3 ? 32 : 64, TK = 16, LDS = 68;  // LDS % 16 == 4: conflict-free fragment loads
+constexpr int NTHREADS = M3 ? 128 : 256;
+constexpr int QA = TM * TK / NTHREADS, QB = TN * TK / NTHREADS;   // staged elements per thread
 constexpr int LDK = 20;                              // k-contiguous operands: [mn][k], LDK % 16 == 4
 constexpr int SM_PLANE = TM * LDK;                   // doubles per plane (>= TK * LDS)
 constexpr int SM_STAGE = 4 * SM_PLANE;               // A_re, A_im, B_re, B_im
@@ -39,16 +43,18 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
   extern __shared__ double smem[];
   const int tid = threadIdx.x;
   // lower: only the tilesM (tilesM + 1) / 2 tiles on or below the diagonal are launched
-  const int64_t tiles = p.lower ? (int64_t)tilesM * (tilesM + 1) / 2 : (int64_t)tilesM * tilesN;
+  const int64_t tiles = p.lower ? (int64_t)(TM / TN) * tilesM * (tilesM + 1) / 2 : (int64_t)tilesM * tilesN;
   const int64_t bidx = blockIdx.x;
   const int64_t b = bidx / tiles;
   const int t = (int)(bidx - b * tiles);
   int tm, tn;
   if (p.lower) {
-    tm = (int)((sqrt(8.0 * t + 1.0) - 1.0) * 0.5);
-    while ((tm + 1) * (tm + 2) / 2 <= t) ++tm;
-    while (tm * (tm + 1) / 2 > t) --tm;
-    tn = t - tm * (tm + 1) / 2;
+    // row tm of TM-row tiles holds RT (tm + 1) tiles of TN columns, RT = TM / TN
+    constexpr int RT = TM / TN;
+    tm = (int)((sqrt(8.0 * t / RT + 1.0) - 1.0) * 0.5);
+    while (RT * (tm + 1) * (tm + 2) / 2 <= t) ++tm;
+    while (RT * tm * (tm + 1) / 2 > t) --tm;
+    tn = t - RT * tm * (tm + 1) / 2;
   } else { tm = t % tilesM; tn = t / tilesM; }
   const int64_t bo = b / p.inner;
   const int bi = (int)(b - bo * p.inner);
@@ -69,17 +75,17 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
   const bool transB = (OPB == BE_OP_T || OPB == BE_OP_C), conjB = (OPB == BE_OP_C || OPB == BE_OP_J);
 
   // staging coordinates
-  int ai, ak, aqi, aqk;   // A tile element (i, k) = (ai + q*aqi, ak + q*aqk), q = 0..3
-  if (!transA) { ai = tid & 63; ak = tid >> 6; aqi = 0; aqk = 4; }
-  else         { ak = tid & 15; ai = tid >> 4; aqi = 16; aqk = 0; }
-  int bn, bk, bqn, bqk;
-  if (!transB) { bk = tid & 15; bn = tid >> 4; bqn = 16; bqk = 0; }
-  else         { bn = tid & 63; bk = tid >> 6; bqn = 0; bqk = 4; }
+  int ai, ak, aqi, aqk;   // A tile element (i, k) = (ai + q*aqi, ak + q*aqk), q = 0..QA-1
+  if (!transA) { ai = tid % TM; ak = tid / TM; aqi = 0; aqk = NTHREADS / TM; }
+  else         { ak = tid % TK; ai = tid / TK; aqi = NTHREADS / TK; aqk = 0; }
+  int bn, bk, bqn, bqk;   // B tile element (k, n) = (bk + q*bqk, bn + q*bqn), q = 0..QB-1
+  if (!transB) { bk = tid % TK; bn = tid / TK; bqn = NTHREADS / TK; bqk = 0; }
+  else         { bn = tid % TN; bk = tid / TN; bqn = 0; bqk = NTHREADS / TN; }
 
-  cplx ra[4], rb[4], rphi[4];
+  cplx ra[QA], rb[QB], rphi[QB];
   auto gload = [&](int k0) {
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
+    for (int q = 0; q < QA; ++q) {
       const int i = m0 + ai + q * aqi, k = k0 + ak + q * aqk;
       cplx v = mkc(0.0, 0.0);
       if (i < M && k < K) {
@@ -90,7 +96,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
       ra[q] = v;
     }
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
+    for (int q = 0; q < QB; ++q) {
       const int n = n0 + bn + q * bqn, k = k0 + bk + q * bqk;
       cplx v = mkc(0.0, 0.0);
       cplx f = mkc(1.0, 0.0);
@@ -107,14 +113,14 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
   auto sstore = [&](int stage) {
     double* s = smem + stage * SM_STAGE;
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
+    for (int q = 0; q < QA; ++q) {
       const int i = ai + q * aqi, k = ak + q * aqk;
       const int o = transA ? i * LDK + k : k * LDS + i;   // conflict-free for the store and the fragment loads
       s[o] = ra[q].x;
       s[SM_PLANE + o] = conjA ? -ra[q].y : ra[q].y;
     }
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
+    for (int q = 0; q < QB; ++q) {
       const int n = bn + q * bqn, k = bk + q * bqk;
       cplx v = rb[q];
       if (PHI) v = cmul(rphi[q], v);
@@ -128,11 +134,15 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
   const int wm = warp & 1, wn = warp >> 1;
   const int g = lane >> 2, tg = lane & 3;
 
-  double accr[4][2][2], acci[4][2][2];
+  // 4M: accr = Re, acci = Im.  3M: accr = sum Ar Br, acci = sum Ai Bi, accs = sum (Ar + Ai)(Br + Bi).
+  double accr[4][2][2], acci[4][2][2], accs[M3 ? 4 : 1][2][2];
 #pragma unroll
   for (int a = 0; a < 4; ++a)
 #pragma unroll
-    for (int c = 0; c < 2; ++c) { accr[a][c][0] = accr[a][c][1] = 0.0; acci[a][c][0] = acci[a][c][1] = 0.0; }
+    for (int c = 0; c < 2; ++c) {
+      accr[a][c][0] = accr[a][c][1] = 0.0; acci[a][c][0] = acci[a][c][1] = 0.0;
+      if (M3) accs[a][c][0] = accs[a][c][1] = 0.0;
+    }
 
   const bool has_beta = (p.beta.x != 0.0 || p.beta.y != 0.0);
   auto cload = [&](int half, cplx (&dst)[2][2][2]) {
@@ -174,6 +184,26 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
         const int o = transB ? k * LDS + n : n * LDK + k;
         br[nb] = s[2 * SM_PLANE + o];
         bim[nb] = s[3 * SM_PLANE + o];
+      }
+      if (M3) {
+        // three real products instead of four (Karatsuba): Re = P1 - P2, Im = P3 - P1 - P2 with P1 = Ar Br,
+        // P2 = Ai Bi, P3 = (Ar + Ai)(Br + Bi).  The tensor pipe is the bound of this loop (ncu: math-pipe
+        // throttle is the top stall), so a quarter fewer DMMAs is a quarter less main-loop time; the six
+        // extra additions per k-step are noise.  Error: normwise eps |A||B| on both parts.
+        double sa[4], sb[2];
+#pragma unroll
+        for (int mb = 0; mb < 4; ++mb) sa[mb] = ar[mb] + aim[mb];
+#pragma unroll
+        for (int nb = 0; nb < 2; ++nb) sb[nb] = br[nb] + bim[nb];
+#pragma unroll
+        for (int mb = 0; mb < 4; ++mb)
+#pragma unroll
+          for (int nb = 0; nb < 2; ++nb) {
+            dmma(accr[mb][nb][0], accr[mb][nb][1], ar[mb], br[nb]);
+            dmma(acci[mb][nb][0], acci[mb][nb][1], aim[mb], bim[nb]);
+            dmma(accs[mb][nb][0], accs[mb][nb][1], sa[mb], sb[nb]);
+          }
+        continue;
       }
       // four real products; consecutive DMMAs never touch the same accumulator (no back-to-back
       // dependency on the 16-deep accumulator set)
@@ -218,7 +248,9 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
         for (int e = 0; e < 2; ++e) {
           const int col = n0 + wn * 16 + nb * 8 + 2 * tg + e;
           if (row >= M || col >= N) continue;
-          cplx v = cmul(p.alpha, mkc(accr[mb][nb][e], acci[mb][nb][e]));
+          const cplx ab = M3 ? mkc(accr[mb][nb][e] - acci[mb][nb][e], accs[mb][nb][e] - accr[mb][nb][e] - acci[mb][nb][e])
+                             : mkc(accr[mb][nb][e], acci[mb][nb][e]);
+          cplx v = cmul(p.alpha, ab);
           if (has_beta) v = cadd(v, cmul(p.beta, cold[m2][nb][e]));
           C[(int64_t)row + (int64_t)col * p.ldc] = v;
         }
@@ -230,7 +262,7 @@ template <int OPA, int OPB, bool PHI, bool SPLIT>
 int launch(be_ctx* ctx, const ZgemmParams& p) {
   const int tilesM = (p.M + TM - 1) / TM, tilesN = (p.N + TN - 1) / TN;
   if (p.lower && p.M != p.N) return BE_ERR_SHAPE;
-  const int64_t blocks = p.batch * (p.lower ? (int64_t)tilesM * (tilesM + 1) / 2 : (int64_t)tilesM * tilesN);
+  const int64_t blocks = p.batch * (p.lower ? (int64_t)(TM / TN) * tilesM * (tilesM + 1) / 2 : (int64_t)tilesM * tilesN);
   if (blocks <= 0) return BE_OK;
   if (blocks > 0x7fffffffLL) return BE_ERR_SHAPE;
   static bool attr_done = false;  // per instantiation; idempotent
