@@ -25,8 +25,10 @@ constexpr int TM = 64, TN = M3 ? 32 : 64, TK = 16, LDS = 68;  // LDS % 16 == 4: 
 constexpr int NTHREADS = M3 ? 128 : 256;
 constexpr int QA = TM * TK / NTHREADS, QB = TN * TK / NTHREADS;   // staged elements per thread
 constexpr int LDK = 20;                              // k-contiguous operands: [mn][k], LDK % 16 == 4
-constexpr int SM_PLANE = TM * LDK;                   // doubles per plane (>= TK * LDS)
-constexpr int SM_STAGE = 4 * SM_PLANE;               // A_re, A_im, B_re, B_im
+constexpr int SM_PLANE = TM * LDK;                   // doubles per A plane (>= TK * LDS)
+constexpr int LDSB = TN + 4;                         // B staged [k][n]: LDSB % 16 == 4 as well
+constexpr int SM_PLANEB = TN * LDK > TK * LDSB ? TN * LDK : TK * LDSB;   // doubles per B plane
+constexpr int SM_STAGE = 2 * SM_PLANE + 2 * SM_PLANEB;   // A_re, A_im, B_re, B_im
 constexpr size_t SM_BYTES = 2 * SM_STAGE * sizeof(double);
 // Padded request of the chunk pipeline (be_ctx::gemm_pad): 2 x (SM_PAD + 1 KB) exceeds the 228 KB of an
 // SM, so at most ONE GEMM CTA is resident per SM, and SM_PAD + one k_hemv CTA (109 KB + 1 KB) still fits:
@@ -124,9 +126,9 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
       const int n = bn + q * bqn, k = bk + q * bqk;
       cplx v = rb[q];
       if (PHI) v = cmul(rphi[q], v);
-      const int o = transB ? k * LDS + n : n * LDK + k;
+      const int o = transB ? k * LDSB + n : n * LDK + k;
       s[2 * SM_PLANE + o] = v.x;
-      s[3 * SM_PLANE + o] = conjB ? -v.y : v.y;
+      s[2 * SM_PLANE + SM_PLANEB + o] = conjB ? -v.y : v.y;
     }
   };
 
@@ -181,9 +183,9 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
 #pragma unroll
       for (int nb = 0; nb < 2; ++nb) {
         const int n = wn * 16 + nb * 8 + g;
-        const int o = transB ? k * LDS + n : n * LDK + k;
+        const int o = transB ? k * LDSB + n : n * LDK + k;
         br[nb] = s[2 * SM_PLANE + o];
-        bim[nb] = s[3 * SM_PLANE + o];
+        bim[nb] = s[2 * SM_PLANE + SM_PLANEB + o];
       }
       if (M3) {
         // three real products instead of four (Karatsuba): Re = P1 - P2, Im = P3 - P1 - P2 with P1 = Ar Br,
