@@ -224,7 +224,7 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
 size_t be_eigh_large_scratch_bytes(int64_t cnt, int N, int nv);
 constexpr int TS_MAXN = 104;   // largest matrix reduced entirely in shared memory (tridiag_small.cu)
 int be_tridiag_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N, cplx* Bw,
-                     double* d, double* e, cplx* tau);
+                     double* d, double* e, cplx* tau, int p0 = 0);
 int be_backtransform_small(be_ctx* ctx, const cplx* Bw, const cplx* tau, const double* Z, cplx* X, int64_t cnt, int N,
                            int nv);
 size_t be_cluster_orth_scratch_bytes(int64_t cnt, int N, int nv);

@@ -847,6 +847,12 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
   // rank-2k GEMM likes a deep K = 2 nb: 16 for mid-size matrices, NB = 32 for large ones
   const int nb = (N <= 640) ? NB / 2 : NB;
   for (int p = 0; p < N && !on_chip; p += nb) {
+    if (p > 0 && N - p <= TS_MAXN) {
+      // the trailing block is up to date at a panel boundary and fits one CTA's shared memory: its ~100
+      // columns are too short to feed two launches each (k_hemv bottoms out at ~50 us per launch)
+      BE_TRY(be_tridiag_small(ctx, nullptr, map, loop0, cnt, N, s.Bw, s.d, s.e, s.tau, p));
+      break;
+    }
     const int pend = (p + nb < N - 1) ? p + nb : N - 1;   // reflector columns p .. pend-1
     colw(p, p, 0, 1);   // reflector of column p (or, when p == N-1, just the last diagonal entry)
     LAUNCH_CHECK();

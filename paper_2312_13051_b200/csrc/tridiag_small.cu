@@ -49,7 +49,12 @@ __device__ __forceinline__ void hemv_rows(const cplx* __restrict__ A, const cplx
 
 __global__ void __launch_bounds__(TS_THREADS, 5) k_tridiag_smem(const cplx* __restrict__ H, GridMap map, int64_t loop0,
                                                                 cplx* __restrict__ Bw, double* __restrict__ dd,
-                                                                double* __restrict__ ee, cplx* __restrict__ tau, int N) {
+                                                                double* __restrict__ ee, cplx* __restrict__ tau, int ldn,
+                                                                int p0) {
+  // The matrix reduced here has order N = ldn - p0: the whole input (p0 = 0, read from H), or the trailing
+  // block [p0:, p0:] of the blocked path's work copy Bw (H == nullptr), whose last columns are too short
+  // to feed a launch per column.  Outputs go to rows / columns p0 + .. of the ldn-strided arrays.
+  const int N = ldn - p0;
   extern __shared__ cplx tsm[];             // A: lower triangle packed by columns (pk), y [N], w~ [N]
   __shared__ cplx sc[3];                    // tau s, -1/2 tau s^2, s
   cplx* A = tsm;
@@ -57,7 +62,8 @@ __global__ void __launch_bounds__(TS_THREADS, 5) k_tridiag_smem(const cplx* __re
   cplx* wb = yb + N;
   const int64_t c = blockIdx.x;
   const int tid = threadIdx.x, lane = tid & 31;
-  {
+  cplx* Bc = Bw + c * (int64_t)ldn * ldn + p0 + (int64_t)p0 * ldn;   // element (r, cc) of the block at r + cc * ldn
+  if (H) {
     // the row-major Hermitian input read as a column-major array is B = conj(H) (eigh_large.cu)
     const int64_t src = gridmap_index(map, loop0 + c / map.n1, (int)(c % map.n1));
     const cplx* h = H + src * (int64_t)N * N;
@@ -65,8 +71,13 @@ __global__ void __launch_bounds__(TS_THREADS, 5) k_tridiag_smem(const cplx* __re
       const int r = idx % N, cc = idx / N;
       if (r >= cc) A[pk(r, cc, N)] = h[idx];
     }
+  } else {
+    for (int idx = tid; idx < N * N; idx += TS_THREADS) {
+      const int r = idx % N, cc = idx / N;
+      if (r >= cc) A[pk(r, cc, N)] = Bc[r + (int64_t)cc * ldn];
+    }
   }
-  cplx* Bc = Bw + c * (int64_t)N * N;
+  dd += c * (int64_t)ldn + p0; ee += c * (int64_t)ldn + p0; tau += c * (int64_t)ldn + p0;
   __syncthreads();
   for (int i = 0; i < N - 1; ++i) {
     const int n = N - i - 1;                // order of the trailing block A22 = A[i+1:, i+1:]
@@ -93,15 +104,15 @@ __global__ void __launch_bounds__(TS_THREADS, 5) k_tridiag_smem(const cplx* __re
         const double q = __drcp_rn(amb.x * amb.x + amb.y * amb.y);
         scale = mkc(amb.x * q, -amb.y * q);
       }
-      for (int j = 1 + lane; j < n; j += 32) Bc[(i + 1 + j) + (int64_t)i * N] = cmul(scale, x[j]);   // reflector i
+      for (int j = 1 + lane; j < n; j += 32) Bc[(i + 1 + j) + (int64_t)i * ldn] = cmul(scale, x[j]);   // reflector i
       if (lane == 0) {
         const cplx ts = cmul(t, scale);
         sc[0] = ts;
         sc[1] = cmul(mkc(-0.5 * ts.x, -0.5 * ts.y), scale);
         sc[2] = scale;
-        dd[c * N + i] = A[pk(i, i, N)].x;
-        ee[c * N + i] = beta;
-        tau[c * N + i] = t;
+        dd[i] = A[pk(i, i, N)].x;
+        ee[i] = beta;
+        tau[i] = t;
         x[0] = amb;
       }
     }
@@ -143,7 +154,7 @@ __global__ void __launch_bounds__(TS_THREADS, 5) k_tridiag_smem(const cplx* __re
     }
     __syncthreads();
   }
-  if (tid == 0) dd[c * N + N - 1] = A[pk(N - 1, N - 1, N)].x;
+  if (tid == 0) dd[N - 1] = A[pk(N - 1, N - 1, N)].x;
 }
 
 
@@ -216,15 +227,16 @@ __global__ void __launch_bounds__(256, RPT <= 8 ? 3 : 2) k_backtransform_small(c
 }  // namespace
 
 int be_tridiag_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N, cplx* Bw,
-                     double* d, double* e, cplx* tau) {
-  if (N > TS_MAXN) return BE_ERR_UNSUPPORTED;
-  const size_t sh = ((size_t)N * (N + 1) / 2 + 2 * N) * sizeof(cplx);
+                     double* d, double* e, cplx* tau, int p0) {
+  const int ns = N - p0;   // order of the matrix reduced on chip (H == nullptr: trailing block of Bw)
+  if (ns > TS_MAXN || ns < 1 || (H && p0 != 0)) return BE_ERR_UNSUPPORTED;
+  const size_t sh = ((size_t)ns * (ns + 1) / 2 + 2 * ns) * sizeof(cplx);
   if (sh > 48 * 1024) BE_CUDA(cudaFuncSetAttribute(k_tridiag_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh));
   // six CTAs of 35 KB per SM need the full shared-memory carve-out
   BE_CUDA(cudaFuncSetAttribute(k_tridiag_smem, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
   be_prof_begin(ctx, PK_HEMV);
-  k_tridiag_smem<<<(unsigned)cnt, TS_THREADS, sh, ctx->stream>>>(H, map, loop0, Bw, d, e, tau, N);
-  be_prof_end(ctx, PK_HEMV, (double)cnt * N * N * 32.0, (double)cnt * (16.0 / 3.0) * N * (double)N * N);
+  k_tridiag_smem<<<(unsigned)cnt, TS_THREADS, sh, ctx->stream>>>(H, map, loop0, Bw, d, e, tau, N, p0);
+  be_prof_end(ctx, PK_HEMV, (double)cnt * ns * ns * 32.0, (double)cnt * (16.0 / 3.0) * ns * (double)ns * ns);
   ctx->launches++;
   return (int)cudaGetLastError();
 }
