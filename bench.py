@@ -115,13 +115,13 @@ class Workload:
         return ctx.wilson_loop_host(Hh, self.m, Hh.dim() - 4)
 
     # bounded oracle sample: whole loops cut to ``pts`` points of the same matrices
-    def oracle_sample(self, budget_s: float = 20.0):
+    def oracle_sample(self, pts4: int = 25):
         from oracle import wilson_oracle as wo
         from paper_2312_13051_b200 import workloads as wl
         c = self.cfg
         t0 = time.perf_counter()
         if c == 4:
-            pts = 4
+            pts = pts4          # 25 = one whole loop, ~13 s on the GPU box's 16 cores
             parts = wl.config4_parts(self.L, realization=self.rank)
             H = wl.supercell_grid([parts], pts, 24, t2_indices=[0])
             S = wl.supercell_spin_z(self.L)
@@ -215,11 +215,14 @@ def reference_arm(args, wk: Workload, rank: int):
         return
     os.environ.setdefault("OMP_NUM_THREADS", str(os.cpu_count()))
     cores = os.cpu_count()
-    for _ in range(max(0, min(args.warmup, 1))):
-        wk.oracle_sample()
+    nwarm = max(0, min(args.warmup, 1))
+    # bounded sample per step: the whole run stays within a few minutes whatever --steps says
+    pts4 = max(4, min(25, 100 // max(1, args.steps + nwarm)))
+    for _ in range(nwarm):
+        wk.oracle_sample(pts4)
     vals, dts = [], []
     for _ in range(args.steps):
-        v, desc, dt, _ = wk.oracle_sample()
+        v, desc, dt, _ = wk.oracle_sample(pts4)
         vals.append(v); dts.append(dt)
     tot_k = sum(v * d for v, d in zip(vals, dts))
     value = tot_k / sum(dts)
