@@ -260,6 +260,188 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_kernel(const ZgemmParams p,
   }
 }
 
+
+// ---------------------------------------------------------------------------------------------------------
+// cp.async variant (no closing phase): the operands stay INTERLEAVED (re, im) in shared memory, one 16-byte
+// cp.async per complex element straight from global memory (no staging registers, zero fill at the edges via
+// src-size 0), one 16-byte fragment load per operand element.  Transposition is a choice of shared-memory
+// layout ([k][mn] with LD % 8 == 2 or [mn][k] with LDK % 8 == 4: both conflict free for the 16-byte fragment
+// loads, 8 lanes per wavefront); conjugation is folded into the 3-multiplication algebra
+// (Ai -> sA Ai, Bi -> sB Bi: P3 = (Ar + sA Ai)(Br + sB Bi), Re = P1 - sA sB P2, Im = P3 - P1 - sA sB P2 with the
+// raw P2 = Ai Bi).  Without the 48 staging registers the kernel fits 168 registers: three CTAs per SM.
+constexpr int ALD = TM + 2, BLD = TN + 2;
+constexpr int AS_A = (TM * LDK > TK * ALD) ? TM * LDK : TK * ALD;
+constexpr int AS_B = (TN * LDK > TK * BLD) ? TN * LDK : TK * BLD;
+constexpr int AS_STAGE = AS_A + AS_B;                       // complex elements per stage
+constexpr size_t AS_BYTES = 2 * AS_STAGE * sizeof(cplx);
+
+__device__ __forceinline__ void cp_async16(const cplx* smem_dst, const cplx* gsrc, bool pred) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  const int sz = pred ? 16 : 0;
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" :: "r"(d), "l"(gsrc), "r"(sz) : "memory");
+}
+
+template <int OPA, int OPB, bool SPLIT>
+__global__ void __launch_bounds__(NTHREADS, 3) zgemm_async_kernel(const ZgemmParams p, int tilesM, int tilesN) {
+  extern __shared__ __align__(16) double smem[];
+  cplx* sm = reinterpret_cast<cplx*>(smem);
+  const int tid = threadIdx.x;
+  const int64_t tiles = p.lower ? (int64_t)(TM / TN) * tilesM * (tilesM + 1) / 2 : (int64_t)tilesM * tilesN;
+  const int64_t bidx = blockIdx.x;
+  const int64_t b = bidx / tiles;
+  const int t = (int)(bidx - b * tiles);
+  int tm, tn;
+  if (p.lower) {
+    constexpr int RT = TM / TN;
+    tm = (int)((sqrt(8.0 * t / RT + 1.0) - 1.0) * 0.5);
+    while (RT * (tm + 1) * (tm + 2) / 2 <= t) ++tm;
+    while (RT * tm * (tm + 1) / 2 > t) --tm;
+    tn = t - RT * tm * (tm + 1) / 2;
+  } else { tm = t % tilesM; tn = t / tilesM; }
+  const int64_t bo = b / p.inner;
+  const int bi = (int)(b - bo * p.inner);
+  const cplx* __restrict__ A = p.A + bo * p.sAo + (int64_t)bi * p.sAi;
+  int biB = bi;
+  if (p.ringB) { biB = bi + 1; if (biB == p.inner) biB = 0; }
+  const cplx* __restrict__ B = p.B + bo * p.sBo + (int64_t)biB * p.sBi;
+  cplx* __restrict__ C = p.C + bo * p.sCo + (int64_t)bi * p.sCi;
+  const int ksplit = SPLIT ? p.ksplit : 0;
+  const cplx* __restrict__ A2 = SPLIT ? p.A2 + bo * p.sA2o : nullptr;
+  const cplx* __restrict__ B2 = SPLIT ? p.B2 + bo * p.sB2o : nullptr;
+
+  const int m0 = tm * TM, n0 = tn * TN;
+  const int M = p.M, N = p.N, K = p.K;
+  constexpr bool transA = (OPA == BE_OP_T || OPA == BE_OP_C), conjA = (OPA == BE_OP_C || OPA == BE_OP_J);
+  constexpr bool transB = (OPB == BE_OP_T || OPB == BE_OP_C), conjB = (OPB == BE_OP_C || OPB == BE_OP_J);
+
+  int ai, ak, aqi, aqk;
+  if (!transA) { ai = tid % TM; ak = tid / TM; aqi = 0; aqk = NTHREADS / TM; }
+  else         { ak = tid % TK; ai = tid / TK; aqi = NTHREADS / TK; aqk = 0; }
+  int bn, bk, bqn, bqk;
+  if (!transB) { bk = tid % TK; bn = tid / TK; bqn = NTHREADS / TK; bqk = 0; }
+  else         { bn = tid % TN; bk = tid / TN; bqn = 0; bqk = NTHREADS / TN; }
+
+  auto aload = [&](int k0, int stage) {
+    cplx* sa_ = sm + stage * AS_STAGE;
+    cplx* sb_ = sa_ + AS_A;
+#pragma unroll
+    for (int q = 0; q < QA; ++q) {
+      const int il = ai + q * aqi, kl = ak + q * aqk;
+      const int i = m0 + il, k = k0 + kl;
+      const bool ok = (i < M && k < K);
+      const cplx* Ap = A; int kk = k;
+      if (SPLIT && k >= ksplit) { Ap = A2; kk = k - ksplit; }
+      const cplx* src = ok ? (transA ? Ap + (int64_t)kk + (int64_t)i * p.lda : Ap + (int64_t)i + (int64_t)kk * p.lda) : A;
+      cp_async16(sa_ + (transA ? il * LDK + kl : kl * ALD + il), src, ok);
+    }
+#pragma unroll
+    for (int q = 0; q < QB; ++q) {
+      const int nl = bn + q * bqn, kl = bk + q * bqk;
+      const int n = n0 + nl, k = k0 + kl;
+      const bool ok = (n < N && k < K);
+      const cplx* Bp = B; int kk = k;
+      if (SPLIT && k >= ksplit) { Bp = B2; kk = k - ksplit; }
+      const cplx* src = ok ? (transB ? Bp + (int64_t)n + (int64_t)kk * p.ldb : Bp + (int64_t)kk + (int64_t)n * p.ldb) : B;
+      cp_async16(sb_ + (transB ? kl * BLD + nl : nl * LDK + kl), src, ok);
+    }
+    asm volatile("cp.async.commit_group;\n" ::: "memory");
+  };
+
+  const int warp = tid >> 5, lane = tid & 31;
+  const int wm = warp & 1, wn = warp >> 1;
+  const int g = lane >> 2, tg = lane & 3;
+
+  double accr[4][2][2], acci[4][2][2], accs[4][2][2];
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      accr[a][c][0] = accr[a][c][1] = 0.0; acci[a][c][0] = acci[a][c][1] = 0.0; accs[a][c][0] = accs[a][c][1] = 0.0;
+    }
+
+  const int KT = (K + TK - 1) / TK;
+  aload(0, 0);
+  for (int kt = 0; kt < KT; ++kt) {
+    const int cur = kt & 1;
+    asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+    __syncthreads();                 // tile kt visible to all; everyone is done with tile kt-1 (the other stage)
+    if (kt + 1 < KT) aload((kt + 1) * TK, cur ^ 1);
+    const cplx* sA_ = sm + cur * AS_STAGE;
+    const cplx* sB_ = sA_ + AS_A;
+#pragma unroll
+    for (int ks = 0; ks < 4; ++ks) {
+      const int k = ks * 4 + tg;
+      cplx a[4], bb[2];
+#pragma unroll
+      for (int mb = 0; mb < 4; ++mb) {
+        const int i = wm * 32 + mb * 8 + g;
+        a[mb] = sA_[transA ? i * LDK + k : k * ALD + i];
+      }
+#pragma unroll
+      for (int nb = 0; nb < 2; ++nb) {
+        const int n = wn * 16 + nb * 8 + g;
+        bb[nb] = sB_[transB ? k * BLD + n : n * LDK + k];
+      }
+      double sa[4], sb[2];
+#pragma unroll
+      for (int mb = 0; mb < 4; ++mb) sa[mb] = conjA ? a[mb].x - a[mb].y : a[mb].x + a[mb].y;
+#pragma unroll
+      for (int nb = 0; nb < 2; ++nb) sb[nb] = conjB ? bb[nb].x - bb[nb].y : bb[nb].x + bb[nb].y;
+#pragma unroll
+      for (int mb = 0; mb < 4; ++mb)
+#pragma unroll
+        for (int nb = 0; nb < 2; ++nb) {
+          dmma(accr[mb][nb][0], accr[mb][nb][1], a[mb].x, bb[nb].x);
+          dmma(acci[mb][nb][0], acci[mb][nb][1], a[mb].y, bb[nb].y);
+          dmma(accs[mb][nb][0], accs[mb][nb][1], sa[mb], sb[nb]);
+        }
+    }
+  }
+
+  const bool has_beta = (p.beta.x != 0.0 || p.beta.y != 0.0);
+  constexpr double ss = (conjA != conjB) ? -1.0 : 1.0;   // sA sB
+#pragma unroll
+  for (int half = 0; half < 2; ++half) {
+    cplx cold[2][2][2];
+    if (has_beta) {
+#pragma unroll
+      for (int m2 = 0; m2 < 2; ++m2) {
+        const int row = m0 + wm * 32 + (half * 2 + m2) * 8 + g;
+#pragma unroll
+        for (int nb = 0; nb < 2; ++nb)
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const int col = n0 + wn * 16 + nb * 8 + 2 * tg + e;
+            cold[m2][nb][e] = (row < M && col < N) ? C[(int64_t)row + (int64_t)col * p.ldc] : mkc(0.0, 0.0);
+          }
+      }
+    }
+#pragma unroll
+    for (int m2 = 0; m2 < 2; ++m2) {
+      const int mb = half * 2 + m2;
+      const int row = m0 + wm * 32 + mb * 8 + g;
+#pragma unroll
+      for (int nb = 0; nb < 2; ++nb)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int col = n0 + wn * 16 + nb * 8 + 2 * tg + e;
+          if (row >= M || col >= N) continue;
+          const double p2 = ss * acci[mb][nb][e];
+          const cplx ab = mkc(accr[mb][nb][e] - p2, accs[mb][nb][e] - accr[mb][nb][e] - p2);
+          cplx v = cmul(p.alpha, ab);
+          if (has_beta) v = cadd(v, cmul(p.beta, cold[m2][nb][e]));
+          C[(int64_t)row + (int64_t)col * p.ldc] = v;
+        }
+    }
+  }
+}
+
+static int gemm_async_mode() {   // BE_GEMM_ASYNC=0 selects the register-staged kernel everywhere
+  static int mode = -1;
+  if (mode < 0) { const char* e = getenv("BE_GEMM_ASYNC"); mode = (e && e[0] == '0') ? 0 : 1; }
+  return mode;
+}
+
 template <int OPA, int OPB, bool PHI, bool SPLIT>
 int launch(be_ctx* ctx, const ZgemmParams& p) {
   const int tilesM = (p.M + TM - 1) / TM, tilesN = (p.N + TN - 1) / TN;
@@ -273,7 +455,21 @@ int launch(be_ctx* ctx, const ZgemmParams& p) {
     attr_done = true;
   }
   be_prof_begin(ctx, PK_GEMM);
-  zgemm_kernel<OPA, OPB, PHI, SPLIT><<<(unsigned)blocks, NTHREADS, (ctx->gemm_pad && ctx->stream == ctx->stream2) ? SM_PAD : SM_BYTES, ctx->stream>>>(p, tilesM, tilesN);
+  if constexpr (!PHI) {
+    if (M3 && gemm_async_mode() && !ctx->gemm_pad) {
+      static bool attr2_done = false;
+      if (!attr2_done) {
+        BE_CUDA(cudaFuncSetAttribute(zgemm_async_kernel<OPA, OPB, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AS_BYTES));
+        BE_CUDA(cudaFuncSetAttribute(zgemm_async_kernel<OPA, OPB, SPLIT>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        attr2_done = true;
+      }
+      zgemm_async_kernel<OPA, OPB, SPLIT><<<(unsigned)blocks, NTHREADS, AS_BYTES, ctx->stream>>>(p, tilesM, tilesN);
+    } else {
+      zgemm_kernel<OPA, OPB, PHI, SPLIT><<<(unsigned)blocks, NTHREADS, (ctx->gemm_pad && ctx->stream == ctx->stream2) ? SM_PAD : SM_BYTES, ctx->stream>>>(p, tilesM, tilesN);
+    }
+  } else {
+    zgemm_kernel<OPA, OPB, PHI, SPLIT><<<(unsigned)blocks, NTHREADS, (ctx->gemm_pad && ctx->stream == ctx->stream2) ? SM_PAD : SM_BYTES, ctx->stream>>>(p, tilesM, tilesN);
+  }
   {
     const double tri = p.lower ? 0.5 : 1.0;
     const double fl = 8.0 * p.M * (double)p.N * p.K * (double)p.batch * tri;

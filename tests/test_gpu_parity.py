@@ -681,3 +681,58 @@ def test_launch_counter_counts_kernels(ctx):
     n0 = ctx.launch_count()
     ctx.wilson_loop(dev(wl.config1_grid(6, 2)[None]), 2, 1)
     assert ctx.launch_count() > n0
+
+
+# ------------------------------------------------------------------------------ S2/S3 building block
+@pytest.mark.parametrize("opA,opB", [("N", "N"), ("N", "C"), ("C", "N"), ("N", "T"), ("T", "N"), ("J", "N"),
+                                     ("N", "J"), ("C", "C"), ("T", "J")])
+def test_zgemm_batched_op_pairs_ragged_against_plain_matmul(ctx, opA, opB):
+    """be_zgemm_batched = alpha op(A) op(B) + beta C (the contraction of Eq. 2's links and of the ordered
+    product) against numpy's matmul, on sizes that span several 64 x 32 x 16 tiles with
+    ragged tails in M, N and K, with padding in the leading dimensions."""
+    rng = np.random.default_rng(7)
+    op = {"N": lambda X: X, "T": lambda X: X.transpose(0, 2, 1), "C": lambda X: X.conj().transpose(0, 2, 1),
+          "J": lambda X: X.conj()}
+    for (M, N, K, batch) in [(150, 77, 45, 3), (64, 32, 16, 2), (1, 1, 1, 1), (70, 33, 130, 2)]:
+        shA = (K, M) if opA in "TC" else (M, K)
+        shB = (N, K) if opB in "TC" else (K, N)
+        A = rng.standard_normal((batch,) + shA) + 1j * rng.standard_normal((batch,) + shA)
+        B = rng.standard_normal((batch,) + shB) + 1j * rng.standard_normal((batch,) + shB)
+        C0 = rng.standard_normal((batch, M, N)) + 1j * rng.standard_normal((batch, M, N))
+        alpha, beta = 0.7 - 0.3j, -0.2 + 1.1j
+        want = alpha * (op[opA](A) @ op[opB](B)) + beta * C0
+        # column-major storage with padded leading dimensions: X[b] is stored as its transpose, row-major
+        def colmajor(X, pad):
+            b, r, c = X.shape
+            buf = np.zeros((b, c, r + pad), dtype=np.complex128)
+            buf[:, :, :r] = X.transpose(0, 2, 1)
+            return buf
+        Ad, Bd, Cd = dev(colmajor(A, 3)), dev(colmajor(B, 1)), dev(colmajor(C0, 2))
+        lda, ldb, ldc = shA[0] + 3, shB[0] + 1, M + 2
+        ctx.zgemm_batched(opA, opB, Ad, Bd, Cd, M, N, K, lda, ldb, ldc, shA[1] * lda, shB[1] * ldb, N * ldc, batch,
+                          alpha=alpha, beta=beta)
+        torch.cuda.synchronize()
+        got = Cd.cpu().numpy()[:, :, :M].transpose(0, 2, 1)
+        scale = np.abs(A).max() * np.abs(B).max() * K + np.abs(C0).max()
+        assert np.abs(got - want).max() <= 1e-14 * scale * 4, (opA, opB, M, N, K)
+        assert np.all(Cd.cpu().numpy()[:, :, M:] == 0)     # the padding rows are never written
+
+
+def test_zgemm_lower_touches_only_tiles_on_or_below_the_diagonal(ctx):
+    rng = np.random.default_rng(8)
+    n, k, batch = 200, 64, 2
+    V = rng.standard_normal((batch, n, k)) + 1j * rng.standard_normal((batch, n, k))
+    C0 = rng.standard_normal((batch, n, n)) + 1j * rng.standard_normal((batch, n, n))
+    Vd = dev(V.transpose(0, 2, 1))          # column-major [n][k]
+    Cd = dev(C0.transpose(0, 2, 1))
+    ctx.zgemm_batched("N", "C", Vd, Vd, Cd, n, n, k, n, n, n, n * k, n * k, n * n, batch, alpha=-1.0 + 0j, beta=1.0 + 0j,
+                      lower=True)
+    torch.cuda.synchronize()
+    got = Cd.cpu().numpy().transpose(0, 2, 1)
+    want = C0 - V @ V.conj().transpose(0, 2, 1)
+    low = np.tril(np.ones((n, n), dtype=bool))
+    assert np.abs(got - want)[:, low].max() <= 1e-12
+    # strictly above the 64 x 32 tile staircase nothing was written
+    r, c = np.indices((n, n))
+    untouched = (c // 32) > (2 * (r // 64) + 1)
+    assert np.all(got[:, untouched] == C0[:, untouched])
