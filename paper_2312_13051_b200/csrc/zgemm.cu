@@ -360,7 +360,18 @@ __global__ void __launch_bounds__(NTHREADS, 3) zgemm_async_kernel(const ZgemmPar
     }
 
   const int KT = (K + TK - 1) / TK;
+  const bool has_beta = (p.beta.x != 0.0 || p.beta.y != 0.0);
   aload(0, 0);
+  if (has_beta) {
+    // read-modify-write (the rank-2k update has only K / TK = 4 k-tiles per C tile): pull the C tile, 32 columns
+    // of 1 KB, into L2 now so that the epilogue's loads do not wait on DRAM
+#pragma unroll
+    for (int q = 0; q < TM * TN * 16 / 128 / NTHREADS; ++q) {
+      const int line = tid + q * NTHREADS;
+      const int col = n0 + line / (TM / 8), row = m0 + (line % (TM / 8)) * 8;
+      if (row < M && col < N) asm volatile("prefetch.global.L2 [%0];\n" :: "l"(C + (int64_t)row + (int64_t)col * p.ldc));
+    }
+  }
   for (int kt = 0; kt < KT; ++kt) {
     const int cur = kt & 1;
     asm volatile("cp.async.wait_group 0;\n" ::: "memory");
@@ -398,7 +409,6 @@ __global__ void __launch_bounds__(NTHREADS, 3) zgemm_async_kernel(const ZgemmPar
     }
   }
 
-  const bool has_beta = (p.beta.x != 0.0 || p.beta.y != 0.0);
   constexpr double ss = (conjA != conjB) ? -1.0 : 1.0;   // sA sB
 #pragma unroll
   for (int half = 0; half < 2; ++half) {
