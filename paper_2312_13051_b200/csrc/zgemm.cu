@@ -11,9 +11,13 @@
 // update of the blocked tridiagonalization, the compact-WY back-transform, U^dagger S U and the
 // sector rotations of the spin-resolved loop.
 //
-// Tile: 64 x 64 x 16 per CTA, 256 threads = 8 warps as 2 (M) x 4 (N), warp tile 32 x 16 =
-// 4 x 2 DMMA blocks, 32 DMMAs per 12 shared loads per k4 step.  Double-buffered shared memory,
-// global loads of tile t+1 are in flight while tile t is multiplied.
+// Two kernels share the tile shape (64 x 32 x 16 per CTA, 128 threads = 4 warps as 2 (M) x 2 (N), warp tile
+// 32 x 16 = 4 x 2 DMMA blocks, three real DMMAs per complex block):
+//   zgemm_async_kernel -- the default: interleaved operands brought in by 16-byte cp.async, 16-byte fragment
+//                         loads, 152-160 registers, three CTAs per SM;
+//   zgemm_kernel       -- register-staged loader that de-interleaves re/im (and applies the closing phase
+//                         Phi) on the way into shared memory: the closing-phase link GEMM, the chunk pipeline
+//                         and BE_GEMM_ASYNC=0.
 #include "be_common.cuh"
 
 namespace {
