@@ -58,7 +58,7 @@ extern "C" int be_profile_enable(be_ctx* ctx, int on) {
 
 extern "C" const char* be_profile_name(int cls) {
   static const char* names[PK_COUNT] = {"hemv", "colw", "zgemm", "bisect", "invit", "cluster_orth",
-                                        "hessenberg", "hqr", "jacobi", "misc"};
+                                        "hessenberg", "hqr", "jacobi", "misc", "fused", "panel", "chase", "q2"};
   return (cls >= 0 && cls < PK_COUNT) ? names[cls] : nullptr;
 }
 
@@ -160,6 +160,13 @@ extern "C" int be_set_workspace_limit(be_ctx* ctx, size_t bytes) {
 extern "C" int be_set_chunk_pipeline(be_ctx* ctx, int on) {
   if (!ctx) return BE_ERR_NULL;
   ctx->chunk_pipeline = on ? 1 : 0;
+  return BE_OK;
+}
+
+extern "C" int be_set_eigh_algorithm(be_ctx* ctx, int algo) {
+  if (!ctx) return BE_ERR_NULL;
+  if (algo < 0 || algo > 1) return BE_ERR_SHAPE;
+  ctx->eigh_algo = algo;
   return BE_OK;
 }
 

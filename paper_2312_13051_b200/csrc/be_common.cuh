@@ -95,11 +95,12 @@ struct be_ctx {
   int gemm_pad;               // zgemm launches with padded shared memory: at most one GEMM CTA per SM,
                               // leaving room for one k_hemv CTA of the other stream
   struct be_prof* prof;       // optional per-kernel-class CUDA-event timing (be_profile_enable)
+  int eigh_algo;              // be_set_eigh_algorithm: 0 one-stage tridiagonalization, 1 two-stage (band) where supported
 };
 
 // kernel classes of the profile
 enum { PK_HEMV = 0, PK_COL, PK_GEMM, PK_BISECT, PK_INVIT, PK_ORTH, PK_HESS, PK_HQR, PK_JACOBI,
-       PK_MISC, PK_COUNT };
+       PK_MISC, PK_FUSED, PK_PANEL, PK_CHASE, PK_Q2, PK_COUNT };
 void be_prof_begin(be_ctx* ctx, int cls);
 void be_prof_end(be_ctx* ctx, int cls, double bytes, double flops);
 
@@ -222,6 +223,12 @@ int be_eigh_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
 int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N,
                   int nv, int ne, double* E, cplx* X, int* info);
 size_t be_eigh_large_scratch_bytes(int64_t cnt, int N, int nv);
+// two-stage reduction (eigh_band.cu): dense -> band of width BE_BAND_KB -> tridiagonal
+constexpr int BE_BAND_KB = 8;
+constexpr int BE_BAND_MINN = 128, BE_BAND_MAXN = 2048;
+size_t be_band_scratch_bytes(int64_t cnt, int N);
+int be_band_reduce(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double* e, cplx* tau, void* scratch);
+int be_band_q2(be_ctx* ctx, const cplx* Bw, cplx* X, int64_t cnt, int N, int nv);
 constexpr int TS_MAXN = 104;   // largest matrix reduced entirely in shared memory (tridiag_small.cu)
 int be_tridiag_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N, cplx* Bw,
                      double* d, double* e, cplx* tau, int p0 = 0);

@@ -1,0 +1,1070 @@
+// S1a, two-stage variant -- Hermitian tridiagonalization without a level-2 pass over the trailing matrix
+// ("exact diagonalization ... at many points in reciprocal space" is where the time goes;
+// SURVEY 7.3 H1 names the two-stage reduction as the fallback when the HEMV half of the one-stage
+// reduction caps the total).
+//
+//   stage 1  dense -> band of width KB = 8:  B = Q1 A_band Q1^H.  Per panel of KB columns
+//              k_panel : one CTA per matrix -- finish W of the previous panel from the partial products,
+//                        bring the next KB columns up to date, Householder QR of the part below the band
+//                        (one block reduction per column), explicit V panel for the streaming kernel
+//              k_fused : ONE streaming pass over the trailing matrix per panel: every 64 x 64 tile is read
+//                        once (TMA bulk copies), gets the pending rank-2KB update of the previous panel
+//                        A -= W V^H + V W^H on the FP64 tensor cores, is written back (bulk store), and is
+//                        multiplied by the new panel's V from both sides of the symmetry (Y = A V) before
+//                        it leaves the SM.  16 flops per byte of HBM traffic instead of the 1 flop per
+//                        byte of a HEMV.
+//   stage 2  band -> real tridiagonal by bulge chasing (k_chase): one CTA per matrix, one warp per sweep,
+//            sweeps pipelined two chase steps apart; the reflectors (length KB) go to the unused upper
+//            triangle of the work matrix.
+//   Q2       X <- conj(Q2) X (k_q2): the N^2 / (2 KB) short reflectors are applied with the eigenvector
+//            entries in registers: a thread owns one column and a sliding window of QG + KB - 1 rows, a
+//            group of QG consecutive sweeps is applied per pass over the column (plain DFMA: on B200 the
+//            DMMA and DFMA peaks are equal, and the diamond-shaped WY form of these reflectors would
+//            cost 2-4x their flops).
+//   Q1       compact-WY GEMMs of the one-stage path (eigh_large.cu) with the reflector heads KB rows
+//            below the diagonal.
+//
+// Memory view as in eigh_large.cu: B = conj(H) column-major, lower triangle referenced; the upper
+// triangle of the diagonal tiles is kept as the mirror image during stage 1 so that a diagonal tile is an
+// ordinary full tile for the multiplication.
+#include "be_common.cuh"
+#include "tma.cuh"
+#include <float.h>
+#include <vector>
+
+namespace {
+
+constexpr int KB = BE_BAND_KB;     // band width
+constexpr int LDP = KB + 1;        // row stride of the explicit panel arrays (odd: conflict-free fragment loads)
+constexpr int TS = 64;             // tile of the streaming kernel
+constexpr int LDT = 67;            // shared-memory column stride of a tile (= 3 mod 8)
+constexpr int LDAB = 2 * KB;       // compact band storage: AB[j][d] = A[j + d][j], d < 2 KB (bulge included)
+
+__device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ cplx shfl_c(cplx v, int src) {
+  return mkc(__shfl_sync(0xffffffffu, v.x, src), __shfl_sync(0xffffffffu, v.y, src));
+}
+__device__ __forceinline__ cplx shfl_xor_c(cplx v, int m) {
+  return mkc(__shfl_xor_sync(0xffffffffu, v.x, m), __shfl_xor_sync(0xffffffffu, v.y, m));
+}
+
+// ------------------------------------------------------------------------------------------
+// The diagonal 64 x 64 tiles get their upper triangle from the lower one (the input contract reads
+// only one triangle of H), and an exactly real diagonal.
+__global__ void k_symdiag(cplx* __restrict__ Bw, int N) {
+  const int c0 = blockIdx.x * TS;
+  cplx* B = Bw + (int64_t)blockIdx.y * N * N;
+  for (int idx = threadIdx.x; idx < TS * TS; idx += blockDim.x) {
+    const int rr = idx % TS, cc = idx / TS;
+    const int r = c0 + rr, col = c0 + cc;
+    if (r >= N) continue;
+    if (rr > cc) B[col + (int64_t)r * N] = cconj(B[r + (int64_t)col * N]);
+    else if (rr == cc) B[r + (int64_t)r * N].y = 0.0;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// Block-wide sum of KB complex values per thread (PT threads); result in res[0..KB).
+constexpr int PT = 512;
+__device__ __forceinline__ void block_sum8(const cplx (&part)[KB], cplx* red, cplx* res) {
+  static_assert(KB == 8, "butterfly written for 8 values");
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const bool u16 = lane & 16, u8 = lane & 8, u4 = lane & 4;
+  cplx b4[4], b2[2], b1;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const cplx snd = u16 ? part[j] : part[j + 4], kp = u16 ? part[j + 4] : part[j];
+    b4[j] = cadd(kp, shfl_xor_c(snd, 16));
+  }
+#pragma unroll
+  for (int j = 0; j < 2; ++j) {
+    const cplx snd = u8 ? b4[j] : b4[j + 2], kp = u8 ? b4[j + 2] : b4[j];
+    b2[j] = cadd(kp, shfl_xor_c(snd, 8));
+  }
+  {
+    const cplx snd = u4 ? b2[0] : b2[1], kp = u4 ? b2[1] : b2[0];
+    b1 = cadd(kp, shfl_xor_c(snd, 4));
+  }
+  b1 = cadd(b1, shfl_xor_c(b1, 2));
+  b1 = cadd(b1, shfl_xor_c(b1, 1));
+  if ((lane & 3) == 0) red[warp * KB + (u16 ? 4 : 0) + (u8 ? 2 : 0) + (u4 ? 1 : 0)] = b1;
+  __syncthreads();
+  if (threadIdx.x < KB) {
+    cplx t = mkc(0.0, 0.0);
+#pragma unroll
+    for (int w = 0; w < PT / 32; ++w) t = cadd(t, red[w * KB + threadIdx.x]);
+    res[threadIdx.x] = t;
+  }
+  __syncthreads();
+}
+
+// Panel step p of the band reduction, one CTA per matrix (thread t owns the rows p KB + t + s PT).
+//   p > 0 : W_{p-1} = Y T - V (1/2 T^H (V^H Y) T),  Y = sum of the partial products of k_fused(p-1);
+//           columns p KB .. p KB + KB - 1 receive the pending update  -= W V^H + V W^H
+//   do_qr : Householder QR of those columns below row j2 = (p + 1) KB: reflectors stored in place (R on and
+//           above the sub-band diagonal), explicit V (unit heads, zeros above) for k_fused, tau, T
+//   !do_qr: the trailing block (at most KB + 1 columns) only receives the update -- end of stage 1.
+// The panel stays on chip during the QR: row slot 0 of every thread in registers, the slots s >= 1 in
+// shared memory ([slot][column][thread]: conflict free), which reuses the staging area of the W phase.
+template <int RPT>
+__global__ void __launch_bounds__(PT, 1) k_panel(cplx* __restrict__ Bw, cplx* __restrict__ Vnew, cplx* __restrict__ Vprev,
+                                                 cplx* __restrict__ Wx, const cplx* __restrict__ P,
+                                                 const cplx* __restrict__ Zc, cplx* __restrict__ T1,
+                                                 cplx* __restrict__ tau1, int N, int Np, int nT, int p, int do_qr) {
+  extern __shared__ __align__(16) cplx psm[];   // W phase: Vsh[PT][KB], Ysh[PT][KB]; QR: panel slots 1 .. RPT-1
+  __shared__ cplx Ts[KB * KB], Cs[KB * KB], Ms[8 * 64], Mf[64], Tn[KB * KB];
+  __shared__ cplx Vtop[(KB + 1) * KB], Wtop[(KB + 1) * KB];
+  __shared__ cplx red[(PT / 32) * KB], res[2][KB], head[2][KB];
+  const int64_t c = blockIdx.x;
+  const int tid = threadIdx.x;
+  cplx* __restrict__ B = Bw + c * (int64_t)N * N;
+  cplx* __restrict__ Vn = Vnew + c * (int64_t)Np * LDP;
+  cplx* __restrict__ Vp = Vprev + c * (int64_t)Np * LDP;
+  cplx* __restrict__ W = Wx + c * (int64_t)Np * LDP;
+  const int jprev = p * KB, j2 = jprev + KB;
+  cplx a0[KB];
+#define PA(s, q) psm[(((s) - 1) * KB + (q)) * PT + tid]
+
+  if (p > 0) {
+    cplx* Vsh = psm;
+    cplx* Ysh = psm + PT * KB;
+    if (tid < 64) Ts[tid] = T1[c * 64 + tid];
+    const int J0 = jprev / TS;
+    const int pid = tid & 63, slice = tid >> 6, mq = pid >> 3, mq2 = pid & 7;
+    cplx macc = mkc(0.0, 0.0);
+    // pass 1: Y = Zc + sum_J P[J] (kept in Wx for pass 2), M = V^H Y
+#pragma unroll 1
+    for (int s = 0; s < RPT; ++s) {
+      if (jprev + s * PT >= N) break;   // uniform
+      const int r = jprev + tid + s * PT;
+      cplx y[KB];
+#pragma unroll
+      for (int q = 0; q < KB; ++q) y[q] = mkc(0.0, 0.0);
+      if (r < N) {
+        const cplx* zc = Zc + (c * Np + r) * (int64_t)KB;
+#pragma unroll
+        for (int q = 0; q < KB; ++q) y[q] = zc[q];
+        const int I = r / TS;
+        for (int J = J0; J <= I; ++J) {
+          const cplx* pp = P + ((c * nT + J) * (int64_t)Np + r) * KB;
+#pragma unroll
+          for (int q = 0; q < KB; ++q) y[q] = cadd(y[q], pp[q]);
+        }
+#pragma unroll
+        for (int q = 0; q < KB; ++q) W[(int64_t)r * LDP + q] = y[q];
+      }
+#pragma unroll
+      for (int q = 0; q < KB; ++q) {
+        Ysh[tid * KB + q] = y[q];
+        Vsh[tid * KB + q] = (r < N) ? Vp[(int64_t)r * LDP + q] : mkc(0.0, 0.0);
+      }
+      __syncthreads();
+      for (int rr = slice * 64; rr < slice * 64 + 64; ++rr) cfmac(macc, Vsh[rr * KB + mq], Ysh[rr * KB + mq2]);
+      __syncthreads();
+    }
+    Ms[slice * 64 + pid] = macc;
+    __syncthreads();
+    if (tid < 64) {
+      cplx t = mkc(0.0, 0.0);
+#pragma unroll
+      for (int sl = 0; sl < 8; ++sl) t = cadd(t, Ms[sl * 64 + tid]);
+      Mf[tid] = t;
+    }
+    __syncthreads();
+    if (tid < 64) {
+      // C = 1/2 T^H M T
+      const int q = tid >> 3, q2 = tid & 7;
+      cplx acc = mkc(0.0, 0.0);
+      for (int b2 = 0; b2 < KB; ++b2) {
+        cplx t = mkc(0.0, 0.0);
+        for (int a2 = 0; a2 < KB; ++a2) cfmac(t, Ts[a2 * KB + q], Mf[a2 * KB + b2]);   // conj(T[a][q]) M[a][b]
+        cfma(acc, t, Ts[b2 * KB + q2]);
+      }
+      Cs[tid] = cscale(0.5, acc);
+    }
+    __syncthreads();
+    // pass 2a: the top rows of W and V (needed by every row of the column update)
+    if (tid < KB + 1) {
+      const int r = jprev + tid;
+#pragma unroll
+      for (int q = 0; q < KB; ++q) { Vtop[tid * KB + q] = mkc(0.0, 0.0); Wtop[tid * KB + q] = mkc(0.0, 0.0); }
+      if (r < N) {
+        cplx y[KB], v[KB];
+#pragma unroll
+        for (int q = 0; q < KB; ++q) { y[q] = W[(int64_t)r * LDP + q]; v[q] = Vp[(int64_t)r * LDP + q]; }
+#pragma unroll
+        for (int q2 = 0; q2 < KB; ++q2) {
+          cplx w = mkc(0.0, 0.0);
+#pragma unroll
+          for (int q = 0; q < KB; ++q) { cfma(w, y[q], Ts[q * KB + q2]); cfms(w, v[q], Cs[q * KB + q2]); }
+          Wtop[tid * KB + q2] = w;
+          Vtop[tid * KB + q2] = v[q2];
+        }
+      }
+    }
+    __syncthreads();
+    // pass 2b: W rows (explicit panel for k_fused: zero above j2) ...
+#pragma unroll 1
+    for (int s = 0; s < RPT; ++s) {
+      const int r = jprev + tid + s * PT;
+      if (r < N) {
+        cplx y[KB], v[KB];
+#pragma unroll
+        for (int q = 0; q < KB; ++q) { y[q] = W[(int64_t)r * LDP + q]; v[q] = Vp[(int64_t)r * LDP + q]; }
+        const bool keep = r >= j2;
+#pragma unroll
+        for (int q2 = 0; q2 < KB; ++q2) {
+          cplx t = mkc(0.0, 0.0);
+#pragma unroll
+          for (int q = 0; q < KB; ++q) { cfma(t, y[q], Ts[q * KB + q2]); cfms(t, v[q], Cs[q * KB + q2]); }
+          W[(int64_t)r * LDP + q2] = keep ? t : mkc(0.0, 0.0);
+        }
+      }
+    }
+    if (!do_qr) {
+      // last step: the trailing block B[jprev:, jprev:] (at most KB + 1 columns) gets the update
+      if (tid < (KB + 1) * (KB + 1)) {
+        const int rr = tid % (KB + 1), cc = tid / (KB + 1);
+        const int r = jprev + rr, col = jprev + cc;
+        if (rr >= cc && r < N) {
+          cplx acc = B[r + (int64_t)col * N];
+#pragma unroll
+          for (int q = 0; q < KB; ++q) {
+            cfms(acc, Wtop[rr * KB + q], cconj(Vtop[cc * KB + q]));
+            cfms(acc, Vtop[rr * KB + q], cconj(Wtop[cc * KB + q]));
+          }
+          if (rr == cc) acc.y = 0.0;
+          B[r + (int64_t)col * N] = acc;
+        }
+      }
+      return;
+    }
+    // ... pass 2c: and the update of the panel columns (each thread re-reads the rows it wrote); the staging
+    // area of pass 1 is dead, the panel slots take its place
+#pragma unroll
+    for (int s = 0; s < RPT; ++s) {
+      const int r = jprev + tid + s * PT;
+      cplx acc8[KB];
+#pragma unroll
+      for (int q = 0; q < KB; ++q) acc8[q] = mkc(0.0, 0.0);
+      if (r < N) {
+        cplx v[KB], w[KB];
+#pragma unroll
+        for (int q = 0; q < KB; ++q) {
+          v[q] = (r < j2) ? Vtop[(r - jprev) * KB + q] : Vp[(int64_t)r * LDP + q];
+          w[q] = (r < j2) ? Wtop[(r - jprev) * KB + q] : W[(int64_t)r * LDP + q];
+        }
+#pragma unroll
+        for (int cc = 0; cc < KB; ++cc) {
+          const int col = jprev + cc;
+          cplx acc = (r >= col) ? B[r + (int64_t)col * N] : mkc(0.0, 0.0);
+#pragma unroll
+          for (int q = 0; q < KB; ++q) {
+            cfms(acc, w[q], cconj(Vtop[cc * KB + q]));
+            cfms(acc, v[q], cconj(Wtop[cc * KB + q]));
+          }
+          acc8[cc] = acc;
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < KB; ++q) { if (s == 0) a0[q] = acc8[q]; else PA(s, q) = acc8[q]; }
+    }
+  } else {
+#pragma unroll
+    for (int s = 0; s < RPT; ++s) {
+      const int r = jprev + tid + s * PT;
+#pragma unroll
+      for (int cc = 0; cc < KB; ++cc) {
+        const cplx t = (r < N && r >= jprev + cc) ? B[r + (int64_t)(jprev + cc) * N] : mkc(0.0, 0.0);
+        if (s == 0) a0[cc] = t; else PA(s, cc) = t;
+      }
+    }
+  }
+
+  // rows jprev .. j2-1 are final band entries (lower part of the diagonal block)
+  if (tid < KB) {
+    const int r = jprev + tid;
+    if (r < N) {
+#pragma unroll
+      for (int cc = 0; cc < KB; ++cc)
+        if (cc <= tid) {
+          cplx t = a0[cc];
+          if (cc == tid) t.y = 0.0;
+          B[r + (int64_t)(jprev + cc) * N] = t;
+        }
+    }
+  }
+  if (tid < 64) Tn[tid] = mkc(0.0, 0.0);
+
+  // ---- Householder QR of the rows >= j2 (local row lr = r - j2; the thread's slot s holds lr = tid - KB + s PT)
+  const int lr0 = tid - KB;
+#pragma unroll 1
+  for (int cc = 0; cc < KB; ++cc) {
+    const int hb = cc & 1;
+    if (tid == KB + cc) {
+#pragma unroll
+      for (int q = 0; q < KB; ++q) head[hb][q] = a0[q];
+    }
+    cplx part[KB];
+#pragma unroll
+    for (int q = 0; q < KB; ++q) part[q] = mkc(0.0, 0.0);
+#pragma unroll
+    for (int s = 0; s < RPT; ++s) {
+      const int lr = lr0 + s * PT;
+      if (lr > cc && j2 + lr < N) {
+        cplx row[KB];
+#pragma unroll
+        for (int q = 0; q < KB; ++q) row[q] = (s == 0) ? a0[q] : PA(s, q);
+        cplx ac = row[0];
+#pragma unroll
+        for (int q = 1; q < KB; ++q) if (q == cc) ac = row[q];
+#pragma unroll
+        for (int q = 0; q < KB; ++q) {
+          if (q >= cc) cfmac(part[q], ac, row[q]);   // conj(a_cc) a_q
+          else cfmac(part[q], row[q], ac);           // conj(v_q) a_cc
+        }
+      }
+    }
+    block_sum8(part, red, res[hb]);
+    const cplx alpha = head[hb][cc];
+    const double xn2 = res[hb][cc].x;
+    cplx tau, scale, betac;
+    if (xn2 == 0.0) {
+      tau = mkc(0.0, 0.0); scale = mkc(0.0, 0.0); betac = alpha;
+    } else {
+      const double beta = -copysign(sqrt(cabs2(alpha) + xn2), alpha.x);
+      tau = mkc((beta - alpha.x) / beta, -alpha.y / beta);
+      scale = cdiv(mkc(1.0, 0.0), mkc(alpha.x - beta, alpha.y));
+      betac = mkc(beta, 0.0);
+    }
+    // f[q] = conj(tau) (head[q] + conj(scale) g[q]),  q > cc
+    cplx f[KB];
+#pragma unroll
+    for (int q = 0; q < KB; ++q) {
+      f[q] = mkc(0.0, 0.0);
+      if (q > cc) {
+        cplx t = head[hb][q];
+        cfmac(t, scale, res[hb][q]);
+        f[q] = cmulc(tau, t);
+      }
+    }
+#pragma unroll
+    for (int s = 0; s < RPT; ++s) {
+      const int lr = lr0 + s * PT;
+      if (lr >= cc && j2 + lr < N) {
+        cplx row[KB];
+#pragma unroll
+        for (int q = 0; q < KB; ++q) row[q] = (s == 0) ? a0[q] : PA(s, q);
+        cplx ac = row[0];
+#pragma unroll
+        for (int q = 1; q < KB; ++q) if (q == cc) ac = row[q];
+        const cplx vv = (lr > cc) ? cmul(ac, scale) : mkc(1.0, 0.0);
+#pragma unroll
+        for (int q = 0; q < KB; ++q) {
+          if (q > cc) cfms(row[q], f[q], vv);
+          else if (q == cc) row[q] = (lr > cc) ? vv : betac;
+        }
+#pragma unroll
+        for (int q = 0; q < KB; ++q) { if (s == 0) a0[q] = row[q]; else PA(s, q) = row[q]; }
+      }
+    }
+    if (tid == 0) {
+      // column cc of T:  T[0:cc, cc] = -tau T[0:cc, 0:cc] z,  z[q] = V_q^H v_cc = conj(v_q[cc]) + scale sum_{lr>cc} conj(v_q) a_cc
+      cplx z[KB];
+#pragma unroll
+      for (int q = 0; q < KB; ++q) {
+        z[q] = mkc(0.0, 0.0);
+        if (q < cc) { z[q] = cconj(head[hb][q]); cfma(z[q], scale, res[hb][q]); }
+      }
+      for (int q = 0; q < cc; ++q) {
+        cplx t = mkc(0.0, 0.0);
+        for (int q2 = q; q2 < cc; ++q2) cfma(t, Tn[q * KB + q2], z[q2]);
+        Tn[q * KB + cc] = cmul(mkc(-tau.x, -tau.y), t);
+      }
+      Tn[cc * KB + cc] = tau;
+      tau1[c * N + jprev + cc] = tau;
+    }
+  }
+  __syncthreads();
+  if (tid < 64) T1[c * 64 + tid] = Tn[tid];
+  // ---- write the panel back: R / v in place, explicit V for k_fused
+#pragma unroll
+  for (int s = 0; s < RPT; ++s) {
+    const int lr = lr0 + s * PT;
+    const int r = j2 + lr;
+    if (lr >= 0 && r < N) {
+#pragma unroll
+      for (int cc = 0; cc < KB; ++cc) {
+        const cplx t = (s == 0) ? a0[cc] : PA(s, cc);
+        B[r + (int64_t)(jprev + cc) * N] = t;
+        Vn[(int64_t)r * LDP + cc] = (lr > cc) ? t : (lr == cc ? mkc(1.0, 0.0) : mkc(0.0, 0.0));
+      }
+    }
+  }
+  if (tid < KB) {
+    const int r = jprev + tid;
+    if (r < Np) {
+#pragma unroll
+      for (int q = 0; q < KB; ++q) {
+        Vn[(int64_t)r * LDP + q] = mkc(0.0, 0.0);
+        Vp[(int64_t)r * LDP + q] = mkc(0.0, 0.0);
+        W[(int64_t)r * LDP + q] = mkc(0.0, 0.0);
+      }
+    }
+  }
+#undef PA
+}
+
+// ------------------------------------------------------------------------------------------
+// The streaming kernel of stage 1.  Work item = (matrix c, block column J); the CTA walks down the tiles
+// (I, J), I = J .. nT-1.  Per tile:
+//   1  A_IJ -= W_I V_J^H + V_I W_J^H          previous panel (K = 2 KB), accumulators start from the tile
+//   2  A_IJ goes back to shared memory and from there to HBM (bulk store)
+//   3  Y_I += A_IJ V+_J                        the accumulators are the A operand (no shared-memory round trip)
+//   4  Y_J += A_IJ^H V+_I   (I != J)           the tile in shared memory is the B operand of (V+_I)^H A_IJ
+// A producer warp runs two tiles ahead (TMA bulk copies, mbarrier complete_tx), issues the bulk stores and
+// fetches items from a global counter (longest block columns first); 8 consumer warps, warp w owns the rows
+// 8w .. 8w+7 of the tile in steps 1-3 and the columns 8w .. 8w+7 in step 4.  Row parts go to P[c][J][r][.]
+// (k_panel adds the block columns: no atomics), the column part stays in registers over the whole item.
+constexpr int FUSED_THREADS = 288;
+constexpr size_t F_OFF_VPI = (size_t)2 * TS * LDT * sizeof(cplx);
+constexpr size_t F_OFF_J = F_OFF_VPI + (size_t)2 * TS * LDP * sizeof(cplx);
+constexpr size_t F_OFF_BAR = F_OFF_J + (size_t)2 * 3 * TS * LDP * sizeof(cplx);
+constexpr size_t FUSED_SMEM = F_OFF_BAR + 6 * sizeof(unsigned long long) + 4 * sizeof(int4) + 16;
+
+__device__ __forceinline__ void bulk_s2g(void* gdst, const void* ssrc, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+__global__ void __launch_bounds__(FUSED_THREADS, 1)
+k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __restrict__ Vprev,
+        const cplx* __restrict__ Wx, cplx* __restrict__ P, cplx* __restrict__ Zc, int N, int Np, int nT, int J0,
+        int cnt, int has_upd, int* __restrict__ counter, int total) {
+  extern __shared__ __align__(128) unsigned char fsm[];
+  cplx* At = (cplx*)fsm;                                   // [2][TS cols][LDT]
+  cplx* VpI = (cplx*)(fsm + F_OFF_VPI);                    // [2][TS][LDP]
+  cplx* Jp = (cplx*)(fsm + F_OFF_J);                       // [2][3][TS][LDP]: V- (prev), W- (prev), V+ (new) rows of J
+  unsigned long long* full = (unsigned long long*)(fsm + F_OFF_BAR);
+  unsigned long long* empty = full + 2;
+  unsigned long long* stready = full + 4;
+  volatile int4* desc = (volatile int4*)(full + 6);        // ring of 4 tile descriptors {c, J, I, flags}
+  volatile int* published = (volatile int*)(desc + 4);
+  const int tid = threadIdx.x;
+  if (tid == 0) {
+    for (int s = 0; s < 2; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); mbar_init(&stready[s], 1); }
+    *published = 0;
+    mbar_fence_init();
+  }
+  // stale tile data is multiplied by exact zeros of the panels (rows / columns beyond N): keep it finite
+  for (int idx = tid; idx < 2 * TS * LDT; idx += FUSED_THREADS) At[idx] = mkc(0.0, 0.0);
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  __syncthreads();
+  constexpr uint32_t PANEL_BYTES = TS * LDP * sizeof(cplx);
+
+  if (tid >= 256) {
+    // ------------------------------- producer warp
+    const int lane = tid - 256;
+    int gt = 0, itemseq = 0;
+    int next = 0;
+    if (lane == 0) next = atomicAdd(counter, 1);
+    int pc = 0, pJ = 0, pI = 0;          // previous tile (its store is issued one tile later)
+    bool have_prev = false;
+    for (;;) {
+      const int item = __shfl_sync(0xffffffffu, next, 0);
+      if (lane == 0 && item < total) next = atomicAdd(counter, 1);
+      if (item >= total) break;
+      const int jj = item / cnt;
+      const int c = item - jj * cnt;
+      const int J = J0 + jj;
+      for (int I = J; I < nT; ++I, ++gt) {
+        const int s = gt & 1;
+        if (gt >= 2) { mbar_wait(&empty[s], ((gt >> 1) - 1) & 1); bulk_wait_read0(); }
+        const int r0 = I * TS, c0 = J * TS;
+        const int nr = (N - r0 < TS) ? N - r0 : TS;
+        const int nc = (N - c0 < TS) ? N - c0 : TS;
+        const bool first = (I == J);
+        if (lane == 0) {
+          int4 d; d.x = c; d.y = J; d.z = I; d.w = (first ? 1 : 0) | (I == nT - 1 ? 2 : 0);
+          desc[gt & 3].x = d.x; desc[gt & 3].y = d.y; desc[gt & 3].z = d.z; desc[gt & 3].w = d.w;
+          __threadfence_block();
+          *published = gt + 1;
+          mbar_expect_tx(&full[s], (uint32_t)nc * nr * sizeof(cplx) + PANEL_BYTES + (first ? 3 * PANEL_BYTES : 0));
+        }
+        __syncwarp();
+        const cplx* B = Bw + (int64_t)c * N * N;
+        cplx* at = At + (size_t)s * TS * LDT;
+        for (int col = lane; col < nc; col += 32)
+          tma_bulk_g2s(at + col * LDT, B + r0 + (int64_t)(c0 + col) * N, (uint32_t)nr * sizeof(cplx), &full[s]);
+        if (lane == 0)
+          tma_bulk_g2s(VpI + (size_t)s * TS * LDP, Vnew + ((int64_t)c * Np + r0) * LDP, PANEL_BYTES, &full[s]);
+        if (first && lane >= 1 && lane <= 3) {
+          const cplx* src = (lane == 1 ? Vprev : (lane == 2 ? Wx : Vnew)) + ((int64_t)c * Np + c0) * LDP;
+          tma_bulk_g2s(Jp + ((size_t)(itemseq & 1) * 3 + (lane - 1)) * TS * LDP, src, PANEL_BYTES, &full[s]);
+        }
+        // the updated previous tile goes back to HBM as soon as the consumers have written it to shared memory
+        if (has_upd && have_prev) {
+          const int ps = (gt - 1) & 1;
+          mbar_wait(&stready[ps], ((gt - 1) >> 1) & 1);
+          const int pr0 = pI * TS, pc0 = pJ * TS;
+          const int pnr = (N - pr0 < TS) ? N - pr0 : TS;
+          const int pnc = (N - pc0 < TS) ? N - pc0 : TS;
+          cplx* Bp = Bw + (int64_t)pc * N * N;
+          const cplx* pat = At + (size_t)ps * TS * LDT;
+          for (int col = lane; col < pnc; col += 32)
+            bulk_s2g(Bp + pr0 + (int64_t)(pc0 + col) * N, pat + col * LDT, (uint32_t)pnr * sizeof(cplx));
+          bulk_commit();
+        }
+        pc = c; pJ = J; pI = I; have_prev = true;
+      }
+      ++itemseq;
+    }
+    if (has_upd && have_prev) {
+      const int ps = (gt - 1) & 1;
+      mbar_wait(&stready[ps], ((gt - 1) >> 1) & 1);
+      const int pr0 = pI * TS, pc0 = pJ * TS;
+      const int pnr = (N - pr0 < TS) ? N - pr0 : TS;
+      const int pnc = (N - pc0 < TS) ? N - pc0 : TS;
+      cplx* Bp = Bw + (int64_t)pc * N * N;
+      const cplx* pat = At + (size_t)ps * TS * LDT;
+      for (int col = lane; col < pnc; col += 32)
+        bulk_s2g(Bp + pr0 + (int64_t)(pc0 + col) * N, pat + col * LDT, (uint32_t)pnr * sizeof(cplx));
+      bulk_commit();
+    }
+    // stop mark
+    {
+      const int s = gt & 1;
+      if (gt >= 2) mbar_wait(&empty[s], ((gt >> 1) - 1) & 1);
+      if (lane == 0) {
+        desc[gt & 3].x = -1;
+        __threadfence_block();
+        *published = gt + 1;
+        mbar_arrive(&full[s]);
+      }
+    }
+    bulk_wait0();
+    return;
+  }
+
+  // ------------------------------- consumers
+  const int lane = tid & 31, w = tid >> 5, g = lane >> 2, q = lane & 3;
+  double z0r[2] = {0.0, 0.0}, z0i[2] = {0.0, 0.0}, z1r[2] = {0.0, 0.0}, z1i[2] = {0.0, 0.0};   // column part (two chains)
+  int jb = 1;
+  cplx Lw[2], Lv[2];          // fragments of [W- V-] rows of the tile, k = 2q, 2q+1
+  int Lfor = -1;              // tile number these fragments were fetched for
+  for (int gt = 0;; ++gt) {
+    const int s = gt & 1;
+    mbar_wait(&full[s], (gt >> 1) & 1);
+    const int c = desc[gt & 3].x;
+    if (c < 0) break;
+    const int J = desc[gt & 3].y, I = desc[gt & 3].z, fl = desc[gt & 3].w;
+    if (fl & 1) jb ^= 1;
+    const cplx* at = At + (size_t)s * TS * LDT;
+    const cplx* vpi = VpI + (size_t)s * TS * LDP;
+    const cplx* VmJ = Jp + ((size_t)jb * 3 + 0) * TS * LDP;
+    const cplx* WmJ = Jp + ((size_t)jb * 3 + 1) * TS * LDP;
+    const cplx* VpJ = Jp + ((size_t)jb * 3 + 2) * TS * LDP;
+    const int rI = I * TS + 8 * w + g;    // < Np always
+    cplx lw0, lw1, lv0, lv1;
+    if (has_upd) {
+      if (Lfor != gt) {
+        const cplx* wr = Wx + ((int64_t)c * Np + rI) * LDP + 2 * q;
+        const cplx* vr = Vprev + ((int64_t)c * Np + rI) * LDP + 2 * q;
+        Lw[0] = wr[0]; Lw[1] = wr[1]; Lv[0] = vr[0]; Lv[1] = vr[1];
+      }
+      lw0 = Lw[0]; lw1 = Lw[1]; lv0 = Lv[0]; lv1 = Lv[1];
+      // fragments of the next tile, if the producer has already announced it
+      if (*published > gt + 1) {
+        const int nc2 = desc[(gt + 1) & 3].x, nI = desc[(gt + 1) & 3].z;
+        if (nc2 >= 0) {
+          const int nr2 = nI * TS + 8 * w + g;
+          const cplx* wr = Wx + ((int64_t)nc2 * Np + nr2) * LDP + 2 * q;
+          const cplx* vr = Vprev + ((int64_t)nc2 * Np + nr2) * LDP + 2 * q;
+          Lw[0] = wr[0]; Lw[1] = wr[1]; Lv[0] = vr[0]; Lv[1] = vr[1];
+          Lfor = gt + 1;
+        }
+      }
+    }
+    // accumulators <- tile: thread holds A[8w+g][8nb + 2q + j]
+    double ar[8][2], ai[8][2];
+#pragma unroll
+    for (int nb = 0; nb < 8; ++nb)
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const cplx t = at[(8 * nb + 2 * q + j) * LDT + 8 * w + g];
+        ar[nb][j] = t.x; ai[nb][j] = t.y;
+      }
+    if (has_upd) {
+      // step 1: C -= L R^H, L = [W_I V_I], R = [V_J W_J]:  Re -= Lr Rr + Li Ri,  Im -= Li Rr - Lr Ri
+      const double l_r[4] = {lw0.x, lw1.x, lv0.x, lv1.x};
+      const double l_i[4] = {lw0.y, lw1.y, lv0.y, lv1.y};
+#pragma unroll
+      for (int nb = 0; nb < 8; ++nb) {
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks) {
+          const cplx rj = (ks < 2 ? VmJ : WmJ)[(8 * nb + g) * LDP + 2 * q + (ks & 1)];
+          dmma(ar[nb][0], ar[nb][1], -l_r[ks], rj.x);
+          dmma(ar[nb][0], ar[nb][1], -l_i[ks], rj.y);
+          dmma(ai[nb][0], ai[nb][1], -l_i[ks], rj.x);
+          dmma(ai[nb][0], ai[nb][1], l_r[ks], rj.y);
+        }
+      }
+      // step 2: back to shared memory (same positions), then the bulk store by the producer
+      cplx* atw = At + (size_t)s * TS * LDT;
+#pragma unroll
+      for (int nb = 0; nb < 8; ++nb)
+#pragma unroll
+        for (int j = 0; j < 2; ++j) atw[(8 * nb + 2 * q + j) * LDT + 8 * w + g] = mkc(ar[nb][j], ai[nb][j]);
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      if (tid == 0) mbar_arrive(&stready[s]);
+    }
+    // step 3: Y_I[8w+g][n] += sum_col A[.][col] V+_J[col][n]; k index q <-> column 8nb + 2q + j
+    {
+      double yr[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, yi[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+#pragma unroll
+      for (int nb = 0; nb < 8; ++nb)
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          const cplx b = VpJ[(8 * nb + 2 * q + j) * LDP + g];
+          const int ch = nb & 1;
+          dmma(yr[ch][0], yr[ch][1], ar[nb][j], b.x);
+          dmma(yr[ch][0], yr[ch][1], -ai[nb][j], b.y);
+          dmma(yi[ch][0], yi[ch][1], ar[nb][j], b.y);
+          dmma(yi[ch][0], yi[ch][1], ai[nb][j], b.x);
+        }
+      cplx* pr = P + (((int64_t)c * nT + J) * Np + rI) * KB + 2 * q;
+      pr[0] = mkc(yr[0][0] + yr[1][0], yi[0][0] + yi[1][0]);
+      pr[1] = mkc(yr[0][1] + yr[1][1], yi[0][1] + yi[1][1]);
+    }
+    // step 4: Z[m][col] += sum_row conj(V+_I[row][m]) A[row][col], col = 8w + n;  Y_J[col][m] = conj(Z[m][col])
+    if (I != J) {
+#pragma unroll
+      for (int blk = 0; blk < 8; ++blk)
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          const int row = 8 * blk + 2 * q + j;
+          const cplx v = vpi[row * LDP + g];
+          const cplx b = at[(8 * w + g) * LDT + row];
+          if (blk & 1) {
+            dmma(z1r[0], z1r[1], v.x, b.x); dmma(z1r[0], z1r[1], v.y, b.y);
+            dmma(z1i[0], z1i[1], v.x, b.y); dmma(z1i[0], z1i[1], -v.y, b.x);
+          } else {
+            dmma(z0r[0], z0r[1], v.x, b.x); dmma(z0r[0], z0r[1], v.y, b.y);
+            dmma(z0i[0], z0i[1], v.x, b.y); dmma(z0i[0], z0i[1], -v.y, b.x);
+          }
+        }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[s]);
+    if (fl & 2) {
+      // end of the item: column part of block column J
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const int col = J * TS + 8 * w + 2 * q + j;
+        Zc[((int64_t)c * Np + col) * KB + g] = mkc(z0r[j] + z1r[j], -(z0i[j] + z1i[j]));
+        z0r[j] = z0i[j] = z1r[j] = z1i[j] = 0.0;
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// Compact band storage for the chase: AB[c][j][d] = A[j + d][j], d = 0 .. 2 KB - 1 (the fill of the
+// bulges reaches 2 KB - 1 below the diagonal), zero where nothing is stored.
+__global__ void k_band_extract(const cplx* __restrict__ Bw, cplx* __restrict__ AB, int N) {
+  const int64_t c = blockIdx.y;
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= N * LDAB) return;
+  const int j = idx / LDAB, d = idx % LDAB;
+  cplx v = mkc(0.0, 0.0);
+  if (d <= KB && j + d < N) v = Bw[c * (int64_t)N * N + (j + d) + (int64_t)j * N];
+  if (d == 0) v.y = 0.0;
+  AB[c * (int64_t)N * LDAB + idx] = v;
+}
+
+// Bulge chasing, one CTA per matrix, one warp per sweep; sweep i runs its chase steps k = 0, 1, ..
+// (reflector on rows i + 1 + k KB ..) one per time step, starting at start[i] (host schedule: sweep i + 1
+// stays two steps behind sweep i, a warp takes the sweeps w, w + G, ..).  Step (i, k):
+//   k > 0: E = A[R_k, R_{k-1}] <- E H_{k-1};  H_k from E[:, 0];  E <- H_k^H E
+//   k = 0: H_0 from A[R_0, i]
+//   D = A[R_k, R_k] <- H_k^H D H_k
+// Lane (rr = lane & 7, cg = lane >> 3) holds rows rr, columns cg and cg + 4 of a KB x KB block.  The
+// reflector (tau in the head slot) is stored in the upper triangle of the work matrix: V2(i, rho) at
+// Bw[i + rho N], rho = row the entry acts on.
+__global__ void __launch_bounds__(512) k_chase(cplx* __restrict__ ABw, cplx* __restrict__ Bw, double* __restrict__ dd,
+                                               double* __restrict__ ee, const int* __restrict__ start, int N, int tend) {
+  static_assert(KB == 8, "lane mapping written for KB = 8");
+  const int64_t c = blockIdx.x;
+  cplx* __restrict__ ab = ABw + c * (int64_t)N * LDAB;
+  cplx* __restrict__ Bc = Bw + c * (int64_t)N * N;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, G = blockDim.x >> 5;
+  const int rr = lane & 7, cg = lane >> 3;
+  int i = warp;
+  int st_i = (i < N - 1) ? start[i] : 0;
+  cplx vprev = mkc(0.0, 0.0), tauprev = mkc(0.0, 0.0);
+  for (int t = 0; t < tend; ++t) {
+    while (i < N - 1 && t - st_i >= (N - 1 - i + KB - 1) / KB) {
+      i += G;
+      st_i = (i < N - 1) ? start[i] : 0;
+    }
+    const int k = t - st_i;
+    if (i < N - 1 && k >= 0) {
+      const int st = i + 1 + k * KB;
+      const int len = (N - st < KB) ? N - st : KB;
+      // ---- loads (independent: one L2 round trip)
+      cplx e0 = mkc(0.0, 0.0), e1 = mkc(0.0, 0.0), d0 = mkc(0.0, 0.0), d1 = mkc(0.0, 0.0), x = mkc(0.0, 0.0);
+      if (k > 0 && rr < len) {
+        e0 = __ldcg(&ab[(int64_t)(st - KB + cg) * LDAB + KB + rr - cg]);
+        e1 = __ldcg(&ab[(int64_t)(st - KB + cg + 4) * LDAB + KB + rr - cg - 4]);
+      }
+      if (rr < len) {
+        if (cg < len) d0 = (rr >= cg) ? __ldcg(&ab[(int64_t)(st + cg) * LDAB + rr - cg])
+                                      : cconj(__ldcg(&ab[(int64_t)(st + rr) * LDAB + cg - rr]));
+        if (cg + 4 < len) d1 = (rr >= cg + 4) ? __ldcg(&ab[(int64_t)(st + cg + 4) * LDAB + rr - cg - 4])
+                                              : cconj(__ldcg(&ab[(int64_t)(st + rr) * LDAB + cg + 4 - rr]));
+      }
+      if (k == 0 && cg == 0 && rr < len) x = __ldcg(&ab[(int64_t)i * LDAB + 1 + rr]);
+      if (k > 0) {
+        // E <- E H_{k-1}
+        const cplx vp0 = shfl_c(vprev, cg), vp1 = shfl_c(vprev, cg + 4);
+        cplx wv = cmul(e0, vp0);
+        cfma(wv, e1, vp1);
+        wv = cadd(wv, shfl_xor_c(wv, 8));
+        wv = cadd(wv, shfl_xor_c(wv, 16));
+        const cplx tw = cmul(tauprev, wv);
+        cfms(e0, tw, cconj(vp0));
+        cfms(e1, tw, cconj(vp1));
+        x = e0;   // meaningful on the lanes cg == 0
+      }
+      // ---- reflector from x (lanes 0..7 hold x[rr])
+      const cplx xr = shfl_c(x, rr);
+      const cplx alpha = shfl_c(x, 0);
+      double xn2 = (rr >= 1 && rr < len) ? cabs2(xr) : 0.0;
+      xn2 += __shfl_xor_sync(0xffffffffu, xn2, 1);
+      xn2 += __shfl_xor_sync(0xffffffffu, xn2, 2);
+      xn2 += __shfl_xor_sync(0xffffffffu, xn2, 4);
+      double beta; cplx tau, scale;
+      if (xn2 == 0.0 && alpha.y == 0.0) {
+        beta = alpha.x; tau = mkc(0.0, 0.0); scale = mkc(0.0, 0.0);
+      } else {
+        beta = -copysign(sqrt(cabs2(alpha) + xn2), alpha.x);
+        tau = mkc((beta - alpha.x) / beta, -alpha.y / beta);
+        scale = cdiv(mkc(1.0, 0.0), mkc(alpha.x - beta, alpha.y));
+      }
+      const cplx v = (rr == 0) ? mkc(1.0, 0.0) : (rr < len ? cmul(xr, scale) : mkc(0.0, 0.0));
+      if (cg == 0 && rr < len) Bc[i + (int64_t)(st + rr) * N] = (rr == 0) ? tau : v;
+      if (k == 0) {
+        if (cg == 0 && rr < len) ab[(int64_t)i * LDAB + 1 + rr] = (rr == 0) ? mkc(beta, 0.0) : mkc(0.0, 0.0);
+        if (lane == 0) { ee[c * N + i] = beta; dd[c * N + i] = __ldcg(&ab[(int64_t)i * LDAB]).x; }
+      } else {
+        // E <- H^H E (column 0 becomes beta e_1)
+        cplx z0 = cmulc(v, e0), z1 = cmulc(v, e1);
+#pragma unroll
+        for (int o = 1; o < 8; o <<= 1) { z0 = cadd(z0, shfl_xor_c(z0, o)); z1 = cadd(z1, shfl_xor_c(z1, o)); }
+        const cplx ct = cconj(tau);
+        if (cg == 0) e0 = (rr == 0) ? mkc(beta, 0.0) : mkc(0.0, 0.0);
+        else cfms(e0, cmul(ct, v), z0);
+        cfms(e1, cmul(ct, v), z1);
+        if (rr < len) {
+          ab[(int64_t)(st - KB + cg) * LDAB + KB + rr - cg] = e0;
+          ab[(int64_t)(st - KB + cg + 4) * LDAB + KB + rr - cg - 4] = e1;
+        }
+      }
+      // ---- D <- H^H D H = D - w v^H - v w^H,  w = tau p - 1/2 |tau|^2 (v^H p) v,  p = D v
+      {
+        const cplx vc0 = shfl_c(v, cg), vc1 = shfl_c(v, cg + 4);
+        cplx pp = cmul(d0, vc0);
+        cfma(pp, d1, vc1);
+        pp = cadd(pp, shfl_xor_c(pp, 8));
+        pp = cadd(pp, shfl_xor_c(pp, 16));
+        double al = v.x * pp.x + v.y * pp.y;   // Re(conj(v) p)
+        al += __shfl_xor_sync(0xffffffffu, al, 1);
+        al += __shfl_xor_sync(0xffffffffu, al, 2);
+        al += __shfl_xor_sync(0xffffffffu, al, 4);
+        cplx wv = cmul(tau, pp);
+        const double hf = 0.5 * cabs2(tau) * al;
+        wv.x -= hf * v.x; wv.y -= hf * v.y;
+        const cplx wc0 = shfl_c(wv, cg), wc1 = shfl_c(wv, cg + 4);
+        cfms(d0, wv, cconj(vc0)); cfms(d0, v, cconj(wc0));
+        cfms(d1, wv, cconj(vc1)); cfms(d1, v, cconj(wc1));
+        if (rr < len) {
+          if (cg < len && rr >= cg) { if (rr == cg) d0.y = 0.0; ab[(int64_t)(st + cg) * LDAB + rr - cg] = d0; }
+          if (cg + 4 < len && rr >= cg + 4) { if (rr == cg + 4) d1.y = 0.0; ab[(int64_t)(st + cg + 4) * LDAB + rr - cg - 4] = d1; }
+        }
+      }
+      vprev = v; tauprev = tau;
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { dd[c * N + N - 1] = __ldcg(&ab[(int64_t)(N - 1) * LDAB]).x; ee[c * N + N - 1] = 0.0; }
+}
+
+// start[i] of the chase schedule (see be_band_reduce): one thread, N steps
+__global__ void k_chase_schedule(int* __restrict__ start, int N, int G) {
+  for (int i = 0; i < N - 1; ++i) {
+    int t0 = (i > 0) ? start[i - 1] + 2 : 0;
+    if (i >= G) {
+      const int prev = i - G;
+      const int fin = start[prev] + (N - 1 - prev + KB - 1) / KB;
+      if (fin > t0) t0 = fin;
+    }
+    start[i] = t0;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// X <- conj(Q2) X,  Q2 = prod_i prod_k H_{i,k}  (sweeps ascending; applied last sweep first).
+// A thread owns one column of X (frames layout: column v of matrix c is contiguous) and a window of
+// QWN = QG + KB rows in registers; a group of QG consecutive sweeps at chase step k acts on the matrix rows
+// i0 + 1 + k KB + u, sweep i0 + s on the window rows u = s .. s + KB - 1, and the window slides down by KB
+// rows per step.  QS such stages form a pipeline inside the CTA: stage j applies the sweeps
+// I0 + (QS - 1 - j) QG .. and hands the KB rows it retires per step to stage j + 1 through shared memory,
+// one step behind -- a pass over the column applies QS QG sweeps, so X is streamed N / (QS QG) times instead
+// of N / QG times with the registers of a QG window.  The reflectors of a step are staged in shared memory
+// (cp.async, double buffered) and read as broadcasts.
+constexpr int QG = 16;
+constexpr int QWN = QG + KB;
+constexpr int QS = 3;
+constexpr int Q2_TSG_MAX = 128;   // threads (columns) per stage (3 x 128 threads: 168 registers each)
+
+__device__ __forceinline__ void cp_async16_z(void* sdst, const void* gsrc, bool pred) {
+  const uint32_t d = smem_u32(sdst);
+  const int sz = pred ? 16 : 0;
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(d), "l"(gsrc), "r"(sz) : "memory");
+}
+
+__global__ void __launch_bounds__(QS * Q2_TSG_MAX, 1) k_q2(const cplx* __restrict__ Bw, cplx* __restrict__ X, int N, int nv,
+                                                          int tsg) {
+  extern __shared__ __align__(16) cplx qsm[];
+  cplx* vs = qsm;                                  // [2][QS][QG * KB]
+  cplx* hand = qsm + 2 * QS * QG * KB;             // [2][QS - 1][KB][tsg]
+  const int64_t c = blockIdx.y;
+  const cplx* __restrict__ Bc = Bw + c * (int64_t)N * N;
+  const int j = threadIdx.x / tsg, tcol = threadIdx.x - j * tsg;
+  const int v = blockIdx.x * tsg + tcol;
+  const bool act = v < nv;
+  cplx* __restrict__ x = X + (c * nv + (act ? v : 0)) * (int64_t)N;
+  const int nsuper = (N - 1 + QS * QG - 1) / (QS * QG);
+  auto stage_v = [&](int buf, int i0, int k) {
+    // slot (u, jj): sweep s = u - jj, entry jj; matrix row rho = i0 + 1 + k KB + u, source Bc[(i0 + s) + rho N]
+    cplx* dst = vs + ((size_t)buf * QS + j) * QG * KB;
+    for (int idx = tcol; idx < (QG + KB - 1) * KB; idx += tsg) {
+      const int u = idx / KB, jj = idx % KB;
+      const int s = u - jj;
+      if (s < 0 || s >= QG) continue;
+      const int i = i0 + s, rho = i0 + 1 + k * KB + u;
+      const bool ok = (i < N - 1) && (rho < N);
+      cp_async16_z(&dst[s * KB + jj], ok ? (Bc + i + (int64_t)rho * N) : Bc, ok);
+    }
+  };
+  for (int sg = nsuper - 1; sg >= 0; --sg) {
+    const int I0 = sg * QS * QG;
+    const int i0 = I0 + (QS - 1 - j) * QG;                               // this stage's sweeps i0 .. i0 + QG - 1
+    const int nk = (i0 + 1 < N) ? (N - i0 - 1 + KB - 1) / KB : 0;        // its chase steps
+    const int nk_up = (i0 + QG + 1 < N) ? (N - i0 - QG - 1 + KB - 1) / KB : 0;   // those of the stage above
+    const int NK = (N - I0 - 1 + KB - 1) / KB + QS - 1;                  // steps of the pipeline
+    __syncthreads();   // the previous pass is complete (its stores are visible, its buffers free)
+    cplx wnd[QWN];
+#pragma unroll
+    for (int u = 0; u < QG; ++u) {
+      const int rho = i0 + 1 + u;
+      wnd[u] = (act && rho < N) ? x[rho] : mkc(0.0, 0.0);
+    }
+#pragma unroll
+    for (int u = QG; u < QWN; ++u) wnd[u] = mkc(0.0, 0.0);
+    if (j == 0 && nk > 0) stage_v(0, i0, 0);
+    asm volatile("cp.async.commit_group;\n" ::: "memory");
+    for (int kap = 0; kap < NK; ++kap) {
+      const int k = kap - j;
+      asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+      __syncthreads();
+      if (k + 1 >= 0 && k + 1 < nk) stage_v((kap + 1) & 1, i0, k + 1);
+      asm volatile("cp.async.commit_group;\n" ::: "memory");
+      if (k < 0 || k >= nk) continue;
+      const int rho0 = i0 + 1 + k * KB;
+      // the KB new rows of this step
+      if (j == 0) {
+#pragma unroll
+        for (int u = 0; u < KB; ++u) {
+          const int rho = rho0 + QG + u;
+          wnd[QG + u] = (act && rho < N) ? x[rho] : mkc(0.0, 0.0);
+        }
+      } else {
+        const cplx* hb = hand + ((size_t)((kap - 1) & 1) * (QS - 1) + (j - 1)) * KB * tsg;
+#pragma unroll
+        for (int u = 0; u < KB; ++u) wnd[QG + u] = (k < nk_up) ? hb[u * tsg + tcol] : mkc(0.0, 0.0);
+      }
+      const cplx* vb = vs + ((size_t)(kap & 1) * QS + j) * QG * KB;
+#pragma unroll
+      for (int s = QG - 1; s >= 0; --s) {
+        // conj(H) = I - conj(tau) conj(v) v^T
+        const cplx tau = vb[s * KB];
+        cplx d0 = wnd[s], d1 = mkc(0.0, 0.0);
+#pragma unroll
+        for (int jj = 1; jj < KB; ++jj) {
+          const cplx vj = vb[s * KB + jj];
+          if (jj & 1) cfma(d1, vj, wnd[s + jj]); else cfma(d0, vj, wnd[s + jj]);
+        }
+        const cplx t = cmulc(tau, cadd(d0, d1));   // conj(tau) * dot
+        wnd[s] = csub(wnd[s], t);
+#pragma unroll
+        for (int jj = 1; jj < KB; ++jj) cfms(wnd[s + jj], t, cconj(vb[s * KB + jj]));
+      }
+      // rows u < KB are final for this stage
+      if (j == QS - 1) {
+        if (act) {
+#pragma unroll
+          for (int u = 0; u < KB; ++u) if (rho0 + u < N) x[rho0 + u] = wnd[u];
+        }
+      } else {
+        cplx* hb = hand + ((size_t)(kap & 1) * (QS - 1) + j) * KB * tsg;
+#pragma unroll
+        for (int u = 0; u < KB; ++u) hb[u * tsg + tcol] = wnd[u];
+      }
+#pragma unroll
+      for (int u = 0; u < QG; ++u) wnd[u] = wnd[u + KB];
+    }
+    asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+  }
+}
+
+struct BandScratch {
+  cplx *Vx0, *Vx1, *Wx, *P, *Zc, *T1, *AB;
+  int* counters;
+  int* start;
+};
+
+size_t band_carve(char* base, int64_t cnt, int N, BandScratch* s) {
+  size_t off = 0;
+  auto take = [&](size_t bytes) { char* p = base ? base + off : nullptr; off += be_align256(bytes); return p; };
+  const int nT = (N + TS - 1) / TS, Np = nT * TS;
+  cplx* v0 = (cplx*)take((size_t)cnt * Np * LDP * sizeof(cplx));
+  cplx* v1 = (cplx*)take((size_t)cnt * Np * LDP * sizeof(cplx));
+  cplx* wx = (cplx*)take((size_t)cnt * Np * LDP * sizeof(cplx));
+  cplx* P = (cplx*)take((size_t)cnt * nT * Np * KB * sizeof(cplx));
+  cplx* zc = (cplx*)take((size_t)cnt * Np * KB * sizeof(cplx));
+  cplx* t1 = (cplx*)take((size_t)cnt * 64 * sizeof(cplx));
+  cplx* ab = (cplx*)take((size_t)cnt * N * LDAB * sizeof(cplx));
+  int* counters = (int*)take((size_t)(N / KB + 2) * sizeof(int));
+  int* start = (int*)take((size_t)N * sizeof(int));
+  if (s) *s = BandScratch{v0, v1, wx, P, zc, t1, ab, counters, start};
+  return off;
+}
+
+}  // namespace
+
+size_t be_band_scratch_bytes(int64_t cnt, int N) { return band_carve(nullptr, cnt, N, nullptr); }
+
+#define LAUNCH_CHECK() do { ctx->launches++; cudaError_t e__ = cudaGetLastError(); if (e__ != cudaSuccess) return (int)e__; } while (0)
+
+// Stage 1 + stage 2 on the work copies Bw [cnt][N][N]: d, e of the real tridiagonal matrix, tau of the
+// stage-1 reflectors (column j: head at row j + KB), stage-1 vectors below the band of Bw, stage-2
+// reflectors in its upper triangle.
+int be_band_reduce(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double* e, cplx* tau, void* scratch) {
+  if (N > BE_BAND_MAXN || N < 2 * KB) return BE_ERR_UNSUPPORTED;
+  if (cnt > 0x7fffffffLL / 64) return BE_ERR_SHAPE;
+  BandScratch s;
+  band_carve((char*)scratch, cnt, N, &s);
+  cudaStream_t st = ctx->stream;
+  const int nT = (N + TS - 1) / TS, Np = nT * TS;
+  // last panel with something to annihilate: rows below j2 = (p + 1) KB number N - j2 >= 2
+  const int plast = (N - 2) / KB - 1;
+  const int RPT = (N + PT - 1) / PT;
+  BE_CUDA(cudaMemsetAsync(s.Vx0, 0, (size_t)cnt * Np * LDP * sizeof(cplx), st));
+  BE_CUDA(cudaMemsetAsync(s.Vx1, 0, (size_t)cnt * Np * LDP * sizeof(cplx), st));
+  BE_CUDA(cudaMemsetAsync(s.Wx, 0, (size_t)cnt * Np * LDP * sizeof(cplx), st));
+  BE_CUDA(cudaMemsetAsync(s.counters, 0, (size_t)(N / KB + 2) * sizeof(int), st));
+  BE_CUDA(cudaMemsetAsync(tau, 0, (size_t)cnt * N * sizeof(cplx), st));
+  k_symdiag<<<dim3((unsigned)nT, (unsigned)cnt), 256, 0, st>>>(Bw, N);
+  LAUNCH_CHECK();
+  const size_t psm = (size_t)(RPT - 1 > 2 ? RPT - 1 : 2) * PT * KB * sizeof(cplx);
+  auto panel = [&](int p, int do_qr) -> int {
+    cplx* vn = (p & 1) ? s.Vx1 : s.Vx0;
+    cplx* vp = (p & 1) ? s.Vx0 : s.Vx1;
+    be_prof_begin(ctx, PK_PANEL);
+    const int n = N - p * KB;
+#define PANEL_CASE(R) case R: \
+      BE_CUDA(cudaFuncSetAttribute(k_panel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm)); \
+      k_panel<R><<<(unsigned)cnt, PT, psm, st>>>(Bw, vn, vp, s.Wx, s.P, s.Zc, s.T1, tau, N, Np, nT, p, do_qr); break;
+    switch (RPT) {
+      PANEL_CASE(1) PANEL_CASE(2) PANEL_CASE(3) PANEL_CASE(4)
+      default: return BE_ERR_UNSUPPORTED;
+    }
+#undef PANEL_CASE
+    be_prof_end(ctx, PK_PANEL, (double)cnt * n * 16.0 * (6.0 * KB + 0.5 * KB * ((n + TS - 1) / TS)), (double)cnt * n * 8.0 * 6 * KB * KB);
+    LAUNCH_CHECK();
+    return BE_OK;
+  };
+  BE_CUDA(cudaFuncSetAttribute(k_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSED_SMEM));
+  for (int p = 0; p <= plast; ++p) {
+    BE_TRY(panel(p, 1));
+    const int j2 = (p + 1) * KB;
+    const int J0 = j2 / TS;
+    const int64_t total = cnt * (int64_t)(nT - J0);
+    const int64_t grid = total < (int64_t)ctx->sm_count ? total : (int64_t)ctx->sm_count;
+    const cplx* vn = (p & 1) ? s.Vx1 : s.Vx0;
+    const cplx* vp = (p & 1) ? s.Vx0 : s.Vx1;
+    be_prof_begin(ctx, PK_FUSED);
+    k_fused<<<(unsigned)grid, FUSED_THREADS, FUSED_SMEM, st>>>(Bw, vn, vp, s.Wx, s.P, s.Zc, N, Np, nT, J0, (int)cnt,
+                                                               p > 0 ? 1 : 0, s.counters + p, (int)total);
+    {
+      // algorithmic traffic: the lower triangle of the trailing matrix read once and (p > 0) written once;
+      // flops: rank-2KB update (8 n^2 KB on the lower half) + the two-sided product (8 n^2 KB)
+      const double n = N - j2;
+      be_prof_end(ctx, PK_FUSED, (double)cnt * 0.5 * n * (n + 1.0) * 16.0 * (p > 0 ? 2.0 : 1.0),
+                  (double)cnt * 8.0 * n * n * KB * (p > 0 ? 2.0 : 1.0));
+    }
+    LAUNCH_CHECK();
+  }
+  BE_TRY(panel(plast + 1, 0));
+  // ---- stage 2
+  k_band_extract<<<dim3((unsigned)((N * LDAB + 255) / 256), (unsigned)cnt), 256, 0, st>>>(Bw, s.AB, N);
+  LAUNCH_CHECK();
+  {
+    // schedule: sweep i starts at start[i]; two steps behind its predecessor, and after the sweep its warp ran before
+    int G = 16;
+    if (cnt > 2 * (int64_t)ctx->sm_count) G = 8;
+    std::vector<int> start(N, 0);
+    int tend = 0;
+    for (int i = 0; i < N - 1; ++i) {
+      int t0 = (i > 0) ? start[i - 1] + 2 : 0;
+      if (i >= G) {
+        const int prev = i - G;
+        const int fin = start[prev] + (N - 1 - prev + KB - 1) / KB;
+        if (fin > t0) t0 = fin;
+      }
+      start[i] = t0;
+      const int fin = t0 + (N - 1 - i + KB - 1) / KB;
+      if (fin > tend) tend = fin;
+    }
+    k_chase_schedule<<<1, 1, 0, st>>>(s.start, N, G);   // the same recurrence on the device (no host copy, no sync)
+    LAUNCH_CHECK();
+    be_prof_begin(ctx, PK_CHASE);
+    k_chase<<<(unsigned)cnt, G * 32, 0, st>>>(s.AB, Bw, d, e, s.start, N, tend);
+    be_prof_end(ctx, PK_CHASE, (double)cnt * N * LDAB * 16.0, (double)cnt * 24.0 * N * (double)N * KB);
+    LAUNCH_CHECK();
+  }
+  return BE_OK;
+}
+
+int be_band_q2(be_ctx* ctx, const cplx* Bw, cplx* X, int64_t cnt, int N, int nv) {
+  if (nv <= 0) return BE_OK;
+  // columns per CTA: a divisor-friendly multiple of 32 (nv = 800 -> 5 CTAs of 160 columns)
+  int nslab = (nv + Q2_TSG_MAX - 1) / Q2_TSG_MAX;
+  int tsg = (((nv + nslab - 1) / nslab) + 31) / 32 * 32;
+  nslab = (nv + tsg - 1) / tsg;
+  const size_t smem = ((size_t)2 * QS * QG * KB + (size_t)2 * (QS - 1) * KB * tsg) * sizeof(cplx);
+  BE_CUDA(cudaFuncSetAttribute(k_q2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  be_prof_begin(ctx, PK_Q2);
+  k_q2<<<dim3((unsigned)nslab, (unsigned)cnt), QS * tsg, smem, ctx->stream>>>(Bw, X, N, nv, tsg);
+  be_prof_end(ctx, PK_Q2, (double)cnt * nv * N * 32.0 * ((N + QS * QG - 1) / (QS * QG)), (double)cnt * 8.0 * N * (double)N * nv);
+  LAUNCH_CHECK();
+  return BE_OK;
+}

@@ -665,14 +665,14 @@ __global__ void k_z2x(const double* __restrict__ Z, cplx* __restrict__ X, int N,
 // Vbuf[(r - p - 1) + cc * N] = conj(V[r][cc]) for the WY block starting at column p (kb columns):
 // zero above the unit diagonal, 1 on it, conj(B[r][p+cc]) below.  Also tauc = conj(tau).
 __global__ void k_extract_v(const cplx* __restrict__ Bw, const cplx* __restrict__ tau, cplx* __restrict__ Vb,
-                            cplx* __restrict__ tauc, int N, int p, int kb) {
+                            cplx* __restrict__ tauc, int N, int p, int kb, int off) {
   const int64_t c = blockIdx.x;
   const cplx* B = Bw + c * (int64_t)N * N;
   cplx* V = Vb + c * (int64_t)N * NBT;
-  const int rows = N - p - 1;
+  const int rows = N - p - off;   // off = 1: tridiagonalization; off = KB: band reduction (heads KB below the diagonal)
   for (int idx = threadIdx.x; idx < rows * kb; idx += blockDim.x) {
     const int cc = idx / rows, rr = idx % rows;
-    const int r = p + 1 + rr;
+    const int r = p + off + rr;
     cplx v;
     if (rr < cc) v = mkc(0.0, 0.0);
     else if (rr == cc) v = mkc(1.0, 0.0);
@@ -761,6 +761,7 @@ struct EighScratch {
   int* bcl;
   void* orth;
   int* hcount;
+  void* band;
 };
 
 static size_t eigh_large_carve(char* base, int64_t cnt, int N, int nv, EighScratch* s) {
@@ -795,7 +796,8 @@ static size_t eigh_large_carve(char* base, int64_t cnt, int N, int nv, EighScrat
   int* bcl = (int*)take(cnt * (size_t)N * sizeof(int));
   void* orth = take(be_cluster_orth_scratch_bytes(cnt, N, nv));
   int* hcount = (int*)take((size_t)N * sizeof(int));
-  if (s) { *s = EighScratch{Bw, Wp, P, zp, tau, Vb, T, G, tauc, Y, Y2, pq, Ttmp, d, e, tn, Z, fa, fb, fc, fp, blk, blo, bhi, bcl, orth, hcount}; }
+  void* band = (N >= BE_BAND_MINN && N <= BE_BAND_MAXN) ? take(be_band_scratch_bytes(cnt, N)) : nullptr;
+  if (s) { *s = EighScratch{Bw, Wp, P, zp, tau, Vb, T, G, tauc, Y, Y2, pq, Ttmp, d, e, tn, Z, fa, fb, fc, fp, blk, blo, bhi, bcl, orth, hcount, band}; }
   return off;
 }
 
@@ -846,7 +848,9 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
   // panel width: the panel work (k_colw and the panel block columns of k_hemv) grows with nb / n, the
   // rank-2k GEMM likes a deep K = 2 nb: 16 for mid-size matrices, NB = 32 for large ones
   const int nb = (N <= 640) ? NB / 2 : NB;
-  for (int p = 0; p < N && !on_chip; p += nb) {
+  const bool two_stage = ctx->eigh_algo == 1 && N >= BE_BAND_MINN && N <= BE_BAND_MAXN;
+  if (two_stage) BE_TRY(be_band_reduce(ctx, s.Bw, cnt, N, s.d, s.e, s.tau, s.band));
+  for (int p = 0; p < N && !on_chip && !two_stage; p += nb) {
     if (p > 0 && N - p <= TS_MAXN) {
       // the trailing block is up to date at a panel boundary and fits one CTA's shared memory: its ~100
       // columns are too short to feed two launches each (k_hemv bottoms out at ~50 us per launch)
@@ -949,13 +953,18 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
     k_z2x<<<(unsigned)(cnt * tr * tv), 256, 0, st>>>(s.Z, X, N, nv, tr, tv);
     LAUNCH_CHECK();
   }
-  int plast = ((N - 2) / NBT) * NBT;
+  // two-stage: first the short reflectors of the bulge chasing, then the band reduction's reflectors, whose
+  // heads sit KB rows below the diagonal (columns 0 .. N - KB - 1)
+  if (two_stage) BE_TRY(be_band_q2(ctx, s.Bw, X, cnt, N, nv));
+  const int off = two_stage ? BE_BAND_KB : 1;
+  const int nref = N - off;
+  int plast = ((nref - 1) / NBT) * NBT;
   for (int p = plast; p >= 0; p -= NBT) {
-    const int pend = (p + NBT < N - 1) ? p + NBT : N - 1;
+    const int pend = (p + NBT < nref) ? p + NBT : nref;
     const int kb = pend - p;
     if (kb <= 0) continue;
-    const int rows = N - p - 1;
-    k_extract_v<<<(unsigned)cnt, 256, 0, st>>>(s.Bw, s.tau, s.Vb, s.tauc, N, p, kb);
+    const int rows = N - p - off;
+    k_extract_v<<<(unsigned)cnt, 256, 0, st>>>(s.Bw, s.tau, s.Vb, s.tauc, N, p, kb, off);
     LAUNCH_CHECK();
     // G = V^H V
     ZgemmParams gg = zgemm_simple(kb, kb, rows, s.Vb, N, (int64_t)N * NBT, s.Vb, N, (int64_t)N * NBT,
@@ -964,7 +973,7 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
     k_larft<<<(unsigned)cnt, kb <= 64 ? 256 : 1024, 0, st>>>(s.G, s.tauc, s.T, s.Ttmp, kb);
     LAUNCH_CHECK();
     // Y = V^H X[p+1:, :]
-    ZgemmParams gy = zgemm_simple(kb, nv, rows, s.Vb, N, (int64_t)N * NBT, X + p + 1, N, (int64_t)N * nv,
+    ZgemmParams gy = zgemm_simple(kb, nv, rows, s.Vb, N, (int64_t)N * NBT, X + p + off, N, (int64_t)N * nv,
                                   s.Y, NBT, (int64_t)NBT * nv, cnt);
     BE_TRY(be_zgemm(ctx, BE_OP_C, BE_OP_N, gy));
     // Y2 = T Y
@@ -973,7 +982,7 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
     BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_N, gt));
     // X[p+1:, :] -= V Y2
     ZgemmParams gx = zgemm_simple(rows, nv, kb, s.Vb, N, (int64_t)N * NBT, s.Y2, NBT, (int64_t)NBT * nv,
-                                  X + p + 1, N, (int64_t)N * nv, cnt);
+                                  X + p + off, N, (int64_t)N * nv, cnt);
     gx.alpha = mkc(-1.0, 0.0); gx.beta = mkc(1.0, 0.0);
     BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_N, gx));
   }
