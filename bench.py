@@ -248,6 +248,8 @@ def main():
     ap.add_argument("--small", action="store_true", help="reduced workload for quick checks (not a bench value)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--eigh-algo", type=int, default=None, choices=[0, 1],
+                    help="tridiagonalization: 0 one-stage, 1 two-stage (default: the library's)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -276,6 +278,8 @@ def main():
         torch.cuda.synchronize()
 
     ctx = Context()
+    if args.eigh_algo is not None:
+        ctx.set_eigh_algorithm(args.eigh_algo)
     H, S = wk.device_grid(torch, device)
     torch.cuda.synchronize()
 

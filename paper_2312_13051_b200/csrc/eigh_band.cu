@@ -35,7 +35,7 @@
 namespace {
 
 constexpr int KB = BE_BAND_KB;     // band width
-constexpr int LDP = KB + 1;        // row stride of the explicit panel arrays (odd: conflict-free fragment loads)
+constexpr int LDR = 65;            // shared-memory stride of a panel column in k_fused (= 1 mod 4: conflict-free fragment loads)
 constexpr int TS = 64;             // tile of the streaming kernel
 constexpr int LDT = 67;            // shared-memory column stride of a tile (= 3 mod 8)
 constexpr int LDAB = 2 * KB;       // compact band storage: AB[j][d] = A[j + d][j], d < 2 KB (bulge included)
@@ -101,76 +101,88 @@ __device__ __forceinline__ void block_sum8(const cplx (&part)[KB], cplx* red, cp
   __syncthreads();
 }
 
+// Explicit panels (V of the new panel, V and W of the previous one) and the partial products are stored
+// column by column: element (row r, panel column q) of matrix c at ((c KB + q) Np + r), Np = rows padded to
+// whole tiles.  Rows above the panel's first row and beyond N hold exact zeros.
+#define PIX(q, r) ((int64_t)(q) * Np + (r))
+
+// Y = A V of panel p-1 from the partial products of k_fused (row parts per block column J <= I, column part
+// Zc), one CTA per (row tile I, matrix); thread = (row, q).  Y goes to the W array (k_panel turns it into W
+// in place).  Also the tile's share of M = V^H Y, summed by k_panel.
+__global__ void __launch_bounds__(512) k_ysum(const cplx* __restrict__ P, const cplx* __restrict__ Zc,
+                                              const cplx* __restrict__ Vprev, cplx* __restrict__ Wx, cplx* __restrict__ Mpart,
+                                              int N, int Np, int nT, int J0, int jprev) {
+  __shared__ cplx Ysh[TS * KB], Vsh[TS * KB], Msh[8 * 64];
+  const int64_t c = blockIdx.y;
+  const int I = J0 + blockIdx.x;
+  const int tid = threadIdx.x, q = tid >> 6, rl = tid & 63;
+  const int r = I * TS + rl;
+  cplx y = mkc(0.0, 0.0), v = mkc(0.0, 0.0);
+  if (r >= jprev && r < N) {
+    y = Zc[c * KB * (int64_t)Np + PIX(q, r)];
+    const cplx* pp = P + (c * nT + J0) * (int64_t)KB * Np + PIX(q, r);
+    int J = J0;
+    for (; J + 4 <= I + 1; J += 4) {
+      const cplx p0 = pp[0], p1 = pp[(int64_t)KB * Np], p2 = pp[2 * (int64_t)KB * Np], p3 = pp[3 * (int64_t)KB * Np];
+      y = cadd(cadd(y, cadd(p0, p1)), cadd(p2, p3));
+      pp += 4 * (int64_t)KB * Np;
+    }
+    for (; J <= I; ++J) { y = cadd(y, pp[0]); pp += (int64_t)KB * Np; }
+    v = Vprev[c * KB * (int64_t)Np + PIX(q, r)];
+  }
+  Wx[c * KB * (int64_t)Np + PIX(q, r)] = y;
+  Ysh[rl * KB + q] = y;
+  Vsh[rl * KB + q] = v;
+  __syncthreads();
+  {
+    const int pid = tid & 63, slice = tid >> 6, mq = pid >> 3, mq2 = pid & 7;
+    cplx macc = mkc(0.0, 0.0);
+#pragma unroll
+    for (int rr = slice * 8; rr < slice * 8 + 8; ++rr) cfmac(macc, Vsh[rr * KB + mq], Ysh[rr * KB + mq2]);
+    Msh[slice * 64 + pid] = macc;
+  }
+  __syncthreads();
+  if (tid < 64) {
+    cplx t = mkc(0.0, 0.0);
+#pragma unroll
+    for (int sl = 0; sl < 8; ++sl) t = cadd(t, Msh[sl * 64 + tid]);
+    Mpart[(c * nT + I) * 64 + tid] = t;
+  }
+}
+
 // Panel step p of the band reduction, one CTA per matrix (thread t owns the rows p KB + t + s PT).
-//   p > 0 : W_{p-1} = Y T - V (1/2 T^H (V^H Y) T),  Y = sum of the partial products of k_fused(p-1);
+//   p > 0 : W_{p-1} = Y T - V (1/2 T^H (V^H Y) T)  (Y, M = V^H Y from k_ysum);
 //           columns p KB .. p KB + KB - 1 receive the pending update  -= W V^H + V W^H
 //   do_qr : Householder QR of those columns below row j2 = (p + 1) KB: reflectors stored in place (R on and
 //           above the sub-band diagonal), explicit V (unit heads, zeros above) for k_fused, tau, T
 //   !do_qr: the trailing block (at most KB + 1 columns) only receives the update -- end of stage 1.
 // The panel stays on chip during the QR: row slot 0 of every thread in registers, the slots s >= 1 in
-// shared memory ([slot][column][thread]: conflict free), which reuses the staging area of the W phase.
+// shared memory ([slot][column][thread]: conflict free).
 template <int RPT>
 __global__ void __launch_bounds__(PT, 1) k_panel(cplx* __restrict__ Bw, cplx* __restrict__ Vnew, cplx* __restrict__ Vprev,
-                                                 cplx* __restrict__ Wx, const cplx* __restrict__ P,
-                                                 const cplx* __restrict__ Zc, cplx* __restrict__ T1,
-                                                 cplx* __restrict__ tau1, int N, int Np, int nT, int p, int do_qr) {
-  extern __shared__ __align__(16) cplx psm[];   // W phase: Vsh[PT][KB], Ysh[PT][KB]; QR: panel slots 1 .. RPT-1
-  __shared__ cplx Ts[KB * KB], Cs[KB * KB], Ms[8 * 64], Mf[64], Tn[KB * KB];
+                                                 cplx* __restrict__ Wx, const cplx* __restrict__ Mpart,
+                                                 cplx* __restrict__ T1, cplx* __restrict__ tau1, int N, int Np, int nT,
+                                                 int p, int do_qr) {
+  extern __shared__ __align__(16) cplx psm[];   // panel slots 1 .. RPT-1
+  __shared__ cplx Ts[KB * KB], Cs[KB * KB], Mf[64], Tn[KB * KB];
   __shared__ cplx Vtop[(KB + 1) * KB], Wtop[(KB + 1) * KB];
   __shared__ cplx red[(PT / 32) * KB], res[2][KB], head[2][KB];
   const int64_t c = blockIdx.x;
   const int tid = threadIdx.x;
   cplx* __restrict__ B = Bw + c * (int64_t)N * N;
-  cplx* __restrict__ Vn = Vnew + c * (int64_t)Np * LDP;
-  cplx* __restrict__ Vp = Vprev + c * (int64_t)Np * LDP;
-  cplx* __restrict__ W = Wx + c * (int64_t)Np * LDP;
+  cplx* __restrict__ Vn = Vnew + c * KB * (int64_t)Np;
+  cplx* __restrict__ Vp = Vprev + c * KB * (int64_t)Np;
+  cplx* __restrict__ W = Wx + c * KB * (int64_t)Np;
   const int jprev = p * KB, j2 = jprev + KB;
   cplx a0[KB];
 #define PA(s, q) psm[(((s) - 1) * KB + (q)) * PT + tid]
 
   if (p > 0) {
-    cplx* Vsh = psm;
-    cplx* Ysh = psm + PT * KB;
-    if (tid < 64) Ts[tid] = T1[c * 64 + tid];
     const int J0 = jprev / TS;
-    const int pid = tid & 63, slice = tid >> 6, mq = pid >> 3, mq2 = pid & 7;
-    cplx macc = mkc(0.0, 0.0);
-    // pass 1: Y = Zc + sum_J P[J] (kept in Wx for pass 2), M = V^H Y
-#pragma unroll 1
-    for (int s = 0; s < RPT; ++s) {
-      if (jprev + s * PT >= N) break;   // uniform
-      const int r = jprev + tid + s * PT;
-      cplx y[KB];
-#pragma unroll
-      for (int q = 0; q < KB; ++q) y[q] = mkc(0.0, 0.0);
-      if (r < N) {
-        const cplx* zc = Zc + (c * Np + r) * (int64_t)KB;
-#pragma unroll
-        for (int q = 0; q < KB; ++q) y[q] = zc[q];
-        const int I = r / TS;
-        for (int J = J0; J <= I; ++J) {
-          const cplx* pp = P + ((c * nT + J) * (int64_t)Np + r) * KB;
-#pragma unroll
-          for (int q = 0; q < KB; ++q) y[q] = cadd(y[q], pp[q]);
-        }
-#pragma unroll
-        for (int q = 0; q < KB; ++q) W[(int64_t)r * LDP + q] = y[q];
-      }
-#pragma unroll
-      for (int q = 0; q < KB; ++q) {
-        Ysh[tid * KB + q] = y[q];
-        Vsh[tid * KB + q] = (r < N) ? Vp[(int64_t)r * LDP + q] : mkc(0.0, 0.0);
-      }
-      __syncthreads();
-      for (int rr = slice * 64; rr < slice * 64 + 64; ++rr) cfmac(macc, Vsh[rr * KB + mq], Ysh[rr * KB + mq2]);
-      __syncthreads();
-    }
-    Ms[slice * 64 + pid] = macc;
-    __syncthreads();
     if (tid < 64) {
+      Ts[tid] = T1[c * 64 + tid];
       cplx t = mkc(0.0, 0.0);
-#pragma unroll
-      for (int sl = 0; sl < 8; ++sl) t = cadd(t, Ms[sl * 64 + tid]);
+      for (int I = J0; I < nT; ++I) t = cadd(t, Mpart[(c * nT + I) * 64 + tid]);
       Mf[tid] = t;
     }
     __syncthreads();
@@ -186,7 +198,7 @@ __global__ void __launch_bounds__(PT, 1) k_panel(cplx* __restrict__ Bw, cplx* __
       Cs[tid] = cscale(0.5, acc);
     }
     __syncthreads();
-    // pass 2a: the top rows of W and V (needed by every row of the column update)
+    // the top rows of W and V (needed by every row of the column update)
     if (tid < KB + 1) {
       const int r = jprev + tid;
 #pragma unroll
@@ -194,7 +206,7 @@ __global__ void __launch_bounds__(PT, 1) k_panel(cplx* __restrict__ Bw, cplx* __
       if (r < N) {
         cplx y[KB], v[KB];
 #pragma unroll
-        for (int q = 0; q < KB; ++q) { y[q] = W[(int64_t)r * LDP + q]; v[q] = Vp[(int64_t)r * LDP + q]; }
+        for (int q = 0; q < KB; ++q) { y[q] = W[PIX(q, r)]; v[q] = Vp[PIX(q, r)]; }
 #pragma unroll
         for (int q2 = 0; q2 < KB; ++q2) {
           cplx w = mkc(0.0, 0.0);
@@ -206,21 +218,21 @@ __global__ void __launch_bounds__(PT, 1) k_panel(cplx* __restrict__ Bw, cplx* __
       }
     }
     __syncthreads();
-    // pass 2b: W rows (explicit panel for k_fused: zero above j2) ...
+    // W rows in place of Y (explicit panel for k_fused: zero above j2) ...
 #pragma unroll 1
     for (int s = 0; s < RPT; ++s) {
       const int r = jprev + tid + s * PT;
       if (r < N) {
         cplx y[KB], v[KB];
 #pragma unroll
-        for (int q = 0; q < KB; ++q) { y[q] = W[(int64_t)r * LDP + q]; v[q] = Vp[(int64_t)r * LDP + q]; }
+        for (int q = 0; q < KB; ++q) { y[q] = W[PIX(q, r)]; v[q] = Vp[PIX(q, r)]; }
         const bool keep = r >= j2;
 #pragma unroll
         for (int q2 = 0; q2 < KB; ++q2) {
           cplx t = mkc(0.0, 0.0);
 #pragma unroll
           for (int q = 0; q < KB; ++q) { cfma(t, y[q], Ts[q * KB + q2]); cfms(t, v[q], Cs[q * KB + q2]); }
-          W[(int64_t)r * LDP + q2] = keep ? t : mkc(0.0, 0.0);
+          W[PIX(q2, r)] = keep ? t : mkc(0.0, 0.0);
         }
       }
     }
@@ -242,8 +254,7 @@ __global__ void __launch_bounds__(PT, 1) k_panel(cplx* __restrict__ Bw, cplx* __
       }
       return;
     }
-    // ... pass 2c: and the update of the panel columns (each thread re-reads the rows it wrote); the staging
-    // area of pass 1 is dead, the panel slots take its place
+    // ... and the update of the panel columns (each thread re-reads the rows it wrote)
 #pragma unroll
     for (int s = 0; s < RPT; ++s) {
       const int r = jprev + tid + s * PT;
@@ -254,8 +265,8 @@ __global__ void __launch_bounds__(PT, 1) k_panel(cplx* __restrict__ Bw, cplx* __
         cplx v[KB], w[KB];
 #pragma unroll
         for (int q = 0; q < KB; ++q) {
-          v[q] = (r < j2) ? Vtop[(r - jprev) * KB + q] : Vp[(int64_t)r * LDP + q];
-          w[q] = (r < j2) ? Wtop[(r - jprev) * KB + q] : W[(int64_t)r * LDP + q];
+          v[q] = (r < j2) ? Vtop[(r - jprev) * KB + q] : Vp[PIX(q, r)];
+          w[q] = (r < j2) ? Wtop[(r - jprev) * KB + q] : W[PIX(q, r)];
         }
 #pragma unroll
         for (int cc = 0; cc < KB; ++cc) {
@@ -400,7 +411,7 @@ __global__ void __launch_bounds__(PT, 1) k_panel(cplx* __restrict__ Bw, cplx* __
       for (int cc = 0; cc < KB; ++cc) {
         const cplx t = (s == 0) ? a0[cc] : PA(s, cc);
         B[r + (int64_t)(jprev + cc) * N] = t;
-        Vn[(int64_t)r * LDP + cc] = (lr > cc) ? t : (lr == cc ? mkc(1.0, 0.0) : mkc(0.0, 0.0));
+        Vn[PIX(cc, r)] = (lr > cc) ? t : (lr == cc ? mkc(1.0, 0.0) : mkc(0.0, 0.0));
       }
     }
   }
@@ -409,9 +420,9 @@ __global__ void __launch_bounds__(PT, 1) k_panel(cplx* __restrict__ Bw, cplx* __
     if (r < Np) {
 #pragma unroll
       for (int q = 0; q < KB; ++q) {
-        Vn[(int64_t)r * LDP + q] = mkc(0.0, 0.0);
-        Vp[(int64_t)r * LDP + q] = mkc(0.0, 0.0);
-        W[(int64_t)r * LDP + q] = mkc(0.0, 0.0);
+        Vn[PIX(q, r)] = mkc(0.0, 0.0);
+        Vp[PIX(q, r)] = mkc(0.0, 0.0);
+        W[PIX(q, r)] = mkc(0.0, 0.0);
       }
     }
   }
@@ -431,8 +442,8 @@ __global__ void __launch_bounds__(PT, 1) k_panel(cplx* __restrict__ Bw, cplx* __
 // (k_panel adds the block columns: no atomics), the column part stays in registers over the whole item.
 constexpr int FUSED_THREADS = 288;
 constexpr size_t F_OFF_VPI = (size_t)2 * TS * LDT * sizeof(cplx);
-constexpr size_t F_OFF_J = F_OFF_VPI + (size_t)2 * TS * LDP * sizeof(cplx);
-constexpr size_t F_OFF_BAR = F_OFF_J + (size_t)2 * 3 * TS * LDP * sizeof(cplx);
+constexpr size_t F_OFF_J = F_OFF_VPI + (size_t)2 * KB * LDR * sizeof(cplx);
+constexpr size_t F_OFF_BAR = F_OFF_J + (size_t)2 * 3 * KB * LDR * sizeof(cplx);
 constexpr size_t FUSED_SMEM = F_OFF_BAR + 6 * sizeof(unsigned long long) + 4 * sizeof(int4) + 16;
 
 __device__ __forceinline__ void bulk_s2g(void* gdst, const void* ssrc, uint32_t bytes) {
@@ -449,8 +460,8 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
         int cnt, int has_upd, int* __restrict__ counter, int total) {
   extern __shared__ __align__(128) unsigned char fsm[];
   cplx* At = (cplx*)fsm;                                   // [2][TS cols][LDT]
-  cplx* VpI = (cplx*)(fsm + F_OFF_VPI);                    // [2][TS][LDP]
-  cplx* Jp = (cplx*)(fsm + F_OFF_J);                       // [2][3][TS][LDP]: V- (prev), W- (prev), V+ (new) rows of J
+  cplx* VpI = (cplx*)(fsm + F_OFF_VPI);                    // [2][KB][LDR]
+  cplx* Jp = (cplx*)(fsm + F_OFF_J);                       // [2][3][KB][LDR]: V- (prev), W- (prev), V+ (new) rows of J
   unsigned long long* full = (unsigned long long*)(fsm + F_OFF_BAR);
   unsigned long long* empty = full + 2;
   unsigned long long* stready = full + 4;
@@ -466,7 +477,7 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
   for (int idx = tid; idx < 2 * TS * LDT; idx += FUSED_THREADS) At[idx] = mkc(0.0, 0.0);
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   __syncthreads();
-  constexpr uint32_t PANEL_BYTES = TS * LDP * sizeof(cplx);
+  constexpr uint32_t PANEL_BYTES = KB * TS * sizeof(cplx);   // KB column segments of TS rows
 
   if (tid >= 256) {
     // ------------------------------- producer warp
@@ -502,11 +513,12 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
         cplx* at = At + (size_t)s * TS * LDT;
         for (int col = lane; col < nc; col += 32)
           tma_bulk_g2s(at + col * LDT, B + r0 + (int64_t)(c0 + col) * N, (uint32_t)nr * sizeof(cplx), &full[s]);
-        if (lane == 0)
-          tma_bulk_g2s(VpI + (size_t)s * TS * LDP, Vnew + ((int64_t)c * Np + r0) * LDP, PANEL_BYTES, &full[s]);
-        if (first && lane >= 1 && lane <= 3) {
-          const cplx* src = (lane == 1 ? Vprev : (lane == 2 ? Wx : Vnew)) + ((int64_t)c * Np + c0) * LDP;
-          tma_bulk_g2s(Jp + ((size_t)(itemseq & 1) * 3 + (lane - 1)) * TS * LDP, src, PANEL_BYTES, &full[s]);
+        if (lane < KB)
+          tma_bulk_g2s(VpI + ((size_t)s * KB + lane) * LDR, Vnew + (int64_t)c * KB * Np + PIX(lane, r0), TS * sizeof(cplx), &full[s]);
+        if (first && lane >= KB) {
+          const int arr = (lane - KB) / KB, qq = (lane - KB) % KB;
+          const cplx* src = (arr == 0 ? Vprev : (arr == 1 ? Wx : Vnew)) + (int64_t)c * KB * Np + PIX(qq, c0);
+          tma_bulk_g2s(Jp + (((size_t)(itemseq & 1) * 3 + arr) * KB + qq) * LDR, src, TS * sizeof(cplx), &full[s]);
         }
         // the updated previous tile goes back to HBM as soon as the consumers have written it to shared memory
         if (has_upd && have_prev) {
@@ -566,17 +578,17 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
     const int J = desc[gt & 3].y, I = desc[gt & 3].z, fl = desc[gt & 3].w;
     if (fl & 1) jb ^= 1;
     const cplx* at = At + (size_t)s * TS * LDT;
-    const cplx* vpi = VpI + (size_t)s * TS * LDP;
-    const cplx* VmJ = Jp + ((size_t)jb * 3 + 0) * TS * LDP;
-    const cplx* WmJ = Jp + ((size_t)jb * 3 + 1) * TS * LDP;
-    const cplx* VpJ = Jp + ((size_t)jb * 3 + 2) * TS * LDP;
+    const cplx* vpi = VpI + (size_t)s * KB * LDR;
+    const cplx* VmJ = Jp + ((size_t)jb * 3 + 0) * KB * LDR;
+    const cplx* WmJ = Jp + ((size_t)jb * 3 + 1) * KB * LDR;
+    const cplx* VpJ = Jp + ((size_t)jb * 3 + 2) * KB * LDR;
     const int rI = I * TS + 8 * w + g;    // < Np always
     cplx lw0, lw1, lv0, lv1;
     if (has_upd) {
       if (Lfor != gt) {
-        const cplx* wr = Wx + ((int64_t)c * Np + rI) * LDP + 2 * q;
-        const cplx* vr = Vprev + ((int64_t)c * Np + rI) * LDP + 2 * q;
-        Lw[0] = wr[0]; Lw[1] = wr[1]; Lv[0] = vr[0]; Lv[1] = vr[1];
+        const cplx* wr = Wx + (int64_t)c * KB * Np + PIX(2 * q, rI);
+        const cplx* vr = Vprev + (int64_t)c * KB * Np + PIX(2 * q, rI);
+        Lw[0] = wr[0]; Lw[1] = wr[Np]; Lv[0] = vr[0]; Lv[1] = vr[Np];
       }
       lw0 = Lw[0]; lw1 = Lw[1]; lv0 = Lv[0]; lv1 = Lv[1];
       // fragments of the next tile, if the producer has already announced it
@@ -584,9 +596,9 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
         const int nc2 = desc[(gt + 1) & 3].x, nI = desc[(gt + 1) & 3].z;
         if (nc2 >= 0) {
           const int nr2 = nI * TS + 8 * w + g;
-          const cplx* wr = Wx + ((int64_t)nc2 * Np + nr2) * LDP + 2 * q;
-          const cplx* vr = Vprev + ((int64_t)nc2 * Np + nr2) * LDP + 2 * q;
-          Lw[0] = wr[0]; Lw[1] = wr[1]; Lv[0] = vr[0]; Lv[1] = vr[1];
+          const cplx* wr = Wx + (int64_t)nc2 * KB * Np + PIX(2 * q, nr2);
+          const cplx* vr = Vprev + (int64_t)nc2 * KB * Np + PIX(2 * q, nr2);
+          Lw[0] = wr[0]; Lw[1] = wr[Np]; Lv[0] = vr[0]; Lv[1] = vr[Np];
           Lfor = gt + 1;
         }
       }
@@ -608,7 +620,7 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
       for (int nb = 0; nb < 8; ++nb) {
 #pragma unroll
         for (int ks = 0; ks < 4; ++ks) {
-          const cplx rj = (ks < 2 ? VmJ : WmJ)[(8 * nb + g) * LDP + 2 * q + (ks & 1)];
+          const cplx rj = (ks < 2 ? VmJ : WmJ)[(2 * q + (ks & 1)) * LDR + 8 * nb + g];
           dmma(ar[nb][0], ar[nb][1], -l_r[ks], rj.x);
           dmma(ar[nb][0], ar[nb][1], -l_i[ks], rj.y);
           dmma(ai[nb][0], ai[nb][1], -l_i[ks], rj.x);
@@ -632,16 +644,16 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
       for (int nb = 0; nb < 8; ++nb)
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
-          const cplx b = VpJ[(8 * nb + 2 * q + j) * LDP + g];
+          const cplx b = VpJ[g * LDR + 8 * nb + 2 * q + j];
           const int ch = nb & 1;
           dmma(yr[ch][0], yr[ch][1], ar[nb][j], b.x);
           dmma(yr[ch][0], yr[ch][1], -ai[nb][j], b.y);
           dmma(yi[ch][0], yi[ch][1], ar[nb][j], b.y);
           dmma(yi[ch][0], yi[ch][1], ai[nb][j], b.x);
         }
-      cplx* pr = P + (((int64_t)c * nT + J) * Np + rI) * KB + 2 * q;
+      cplx* pr = P + ((int64_t)c * nT + J) * KB * Np + PIX(2 * q, rI);
       pr[0] = mkc(yr[0][0] + yr[1][0], yi[0][0] + yi[1][0]);
-      pr[1] = mkc(yr[0][1] + yr[1][1], yi[0][1] + yi[1][1]);
+      pr[Np] = mkc(yr[0][1] + yr[1][1], yi[0][1] + yi[1][1]);
     }
     // step 4: Z[m][col] += sum_row conj(V+_I[row][m]) A[row][col], col = 8w + n;  Y_J[col][m] = conj(Z[m][col])
     if (I != J) {
@@ -650,7 +662,7 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
           const int row = 8 * blk + 2 * q + j;
-          const cplx v = vpi[row * LDP + g];
+          const cplx v = vpi[g * LDR + row];
           const cplx b = at[(8 * w + g) * LDT + row];
           if (blk & 1) {
             dmma(z1r[0], z1r[1], v.x, b.x); dmma(z1r[0], z1r[1], v.y, b.y);
@@ -668,7 +680,7 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
 #pragma unroll
       for (int j = 0; j < 2; ++j) {
         const int col = J * TS + 8 * w + 2 * q + j;
-        Zc[((int64_t)c * Np + col) * KB + g] = mkc(z0r[j] + z1r[j], -(z0i[j] + z1i[j]));
+        Zc[(int64_t)c * KB * Np + PIX(g, col)] = mkc(z0r[j] + z1r[j], -(z0i[j] + z1i[j]));
         z0r[j] = z0i[j] = z1r[j] = z1i[j] = 0.0;
       }
     }
@@ -827,8 +839,11 @@ __global__ void k_chase_schedule(int* __restrict__ start, int N, int G) {
 // rows per step.  QS such stages form a pipeline inside the CTA: stage j applies the sweeps
 // I0 + (QS - 1 - j) QG .. and hands the KB rows it retires per step to stage j + 1 through shared memory,
 // one step behind -- a pass over the column applies QS QG sweeps, so X is streamed N / (QS QG) times instead
-// of N / QG times with the registers of a QG window.  The reflectors of a step are staged in shared memory
-// (cp.async, double buffered) and read as broadcasts.
+// of N / QG times with the registers of a QG window.  Stage 0 takes its new rows from memory: they are
+// fetched one step ahead with cp.async into the same kind of hand-over buffer, so no stage waits on HBM
+// inside a step.  The reflectors of a step are staged in shared memory (cp.async, double buffered) and
+// read as broadcasts.  (A variant with the real and imaginary parts of a column on two lanes -- half the
+// registers, 15 instead of 12 warps -- executed 1.6x the instructions and was slower: 174 vs 142 ms.)
 constexpr int QG = 16;
 constexpr int QWN = QG + KB;
 constexpr int QS = 3;
@@ -844,7 +859,7 @@ __global__ void __launch_bounds__(QS * Q2_TSG_MAX, 1) k_q2(const cplx* __restric
                                                           int tsg) {
   extern __shared__ __align__(16) cplx qsm[];
   cplx* vs = qsm;                                  // [2][QS][QG * KB]
-  cplx* hand = qsm + 2 * QS * QG * KB;             // [2][QS - 1][KB][tsg]
+  cplx* hand = qsm + 2 * QS * QG * KB;             // [2][QS][KB][tsg]: input rows of stage j (j = 0: from memory)
   const int64_t c = blockIdx.y;
   const cplx* __restrict__ Bc = Bw + c * (int64_t)N * N;
   const int j = threadIdx.x / tsg, tcol = threadIdx.x - j * tsg;
@@ -864,6 +879,16 @@ __global__ void __launch_bounds__(QS * Q2_TSG_MAX, 1) k_q2(const cplx* __restric
       cp_async16_z(&dst[s * KB + jj], ok ? (Bc + i + (int64_t)rho * N) : Bc, ok);
     }
   };
+  // stage 0: the KB rows that enter the window at step k, rho = i0 + 1 + k KB + QG + u
+  auto stage_x = [&](int buf, int i0, int k) {
+    cplx* dst = hand + ((size_t)buf * QS) * KB * tsg;
+#pragma unroll
+    for (int u = 0; u < KB; ++u) {
+      const int rho = i0 + 1 + k * KB + QG + u;
+      const bool ok = act && rho < N;
+      cp_async16_z(&dst[u * tsg + tcol], ok ? (x + rho) : x, ok);
+    }
+  };
   for (int sg = nsuper - 1; sg >= 0; --sg) {
     const int I0 = sg * QS * QG;
     const int i0 = I0 + (QS - 1 - j) * QG;                               // this stage's sweeps i0 .. i0 + QG - 1
@@ -879,27 +904,25 @@ __global__ void __launch_bounds__(QS * Q2_TSG_MAX, 1) k_q2(const cplx* __restric
     }
 #pragma unroll
     for (int u = QG; u < QWN; ++u) wnd[u] = mkc(0.0, 0.0);
-    if (j == 0 && nk > 0) stage_v(0, i0, 0);
+    if (j == 0 && nk > 0) { stage_v(0, i0, 0); stage_x(1, i0, 0); }   // step kap reads hand[(kap - 1) & 1]
     asm volatile("cp.async.commit_group;\n" ::: "memory");
     for (int kap = 0; kap < NK; ++kap) {
       const int k = kap - j;
       asm volatile("cp.async.wait_group 0;\n" ::: "memory");
       __syncthreads();
-      if (k + 1 >= 0 && k + 1 < nk) stage_v((kap + 1) & 1, i0, k + 1);
+      if (k + 1 >= 0 && k + 1 < nk) {
+        stage_v((kap + 1) & 1, i0, k + 1);
+        if (j == 0) stage_x(kap & 1, i0, k + 1);
+      }
       asm volatile("cp.async.commit_group;\n" ::: "memory");
       if (k < 0 || k >= nk) continue;
       const int rho0 = i0 + 1 + k * KB;
       // the KB new rows of this step
-      if (j == 0) {
+      {
+        const cplx* hb = hand + ((size_t)((kap - 1) & 1) * QS + j) * KB * tsg;
+        const bool ok = (j == 0) || (k < nk_up);
 #pragma unroll
-        for (int u = 0; u < KB; ++u) {
-          const int rho = rho0 + QG + u;
-          wnd[QG + u] = (act && rho < N) ? x[rho] : mkc(0.0, 0.0);
-        }
-      } else {
-        const cplx* hb = hand + ((size_t)((kap - 1) & 1) * (QS - 1) + (j - 1)) * KB * tsg;
-#pragma unroll
-        for (int u = 0; u < KB; ++u) wnd[QG + u] = (k < nk_up) ? hb[u * tsg + tcol] : mkc(0.0, 0.0);
+        for (int u = 0; u < KB; ++u) wnd[QG + u] = ok ? hb[u * tsg + tcol] : mkc(0.0, 0.0);
       }
       const cplx* vb = vs + ((size_t)(kap & 1) * QS + j) * QG * KB;
 #pragma unroll
@@ -924,7 +947,7 @@ __global__ void __launch_bounds__(QS * Q2_TSG_MAX, 1) k_q2(const cplx* __restric
           for (int u = 0; u < KB; ++u) if (rho0 + u < N) x[rho0 + u] = wnd[u];
         }
       } else {
-        cplx* hb = hand + ((size_t)(kap & 1) * (QS - 1) + j) * KB * tsg;
+        cplx* hb = hand + ((size_t)(kap & 1) * QS + j + 1) * KB * tsg;
 #pragma unroll
         for (int u = 0; u < KB; ++u) hb[u * tsg + tcol] = wnd[u];
       }
@@ -936,7 +959,7 @@ __global__ void __launch_bounds__(QS * Q2_TSG_MAX, 1) k_q2(const cplx* __restric
 }
 
 struct BandScratch {
-  cplx *Vx0, *Vx1, *Wx, *P, *Zc, *T1, *AB;
+  cplx *Vx0, *Vx1, *Wx, *P, *Zc, *T1, *AB, *Mpart;
   int* counters;
   int* start;
 };
@@ -945,16 +968,17 @@ size_t band_carve(char* base, int64_t cnt, int N, BandScratch* s) {
   size_t off = 0;
   auto take = [&](size_t bytes) { char* p = base ? base + off : nullptr; off += be_align256(bytes); return p; };
   const int nT = (N + TS - 1) / TS, Np = nT * TS;
-  cplx* v0 = (cplx*)take((size_t)cnt * Np * LDP * sizeof(cplx));
-  cplx* v1 = (cplx*)take((size_t)cnt * Np * LDP * sizeof(cplx));
-  cplx* wx = (cplx*)take((size_t)cnt * Np * LDP * sizeof(cplx));
+  cplx* v0 = (cplx*)take((size_t)cnt * Np * KB * sizeof(cplx));
+  cplx* v1 = (cplx*)take((size_t)cnt * Np * KB * sizeof(cplx));
+  cplx* wx = (cplx*)take((size_t)cnt * Np * KB * sizeof(cplx));
   cplx* P = (cplx*)take((size_t)cnt * nT * Np * KB * sizeof(cplx));
   cplx* zc = (cplx*)take((size_t)cnt * Np * KB * sizeof(cplx));
   cplx* t1 = (cplx*)take((size_t)cnt * 64 * sizeof(cplx));
   cplx* ab = (cplx*)take((size_t)cnt * N * LDAB * sizeof(cplx));
+  cplx* mp = (cplx*)take((size_t)cnt * nT * 64 * sizeof(cplx));
   int* counters = (int*)take((size_t)(N / KB + 2) * sizeof(int));
   int* start = (int*)take((size_t)N * sizeof(int));
-  if (s) *s = BandScratch{v0, v1, wx, P, zc, t1, ab, counters, start};
+  if (s) *s = BandScratch{v0, v1, wx, P, zc, t1, ab, mp, counters, start};
   return off;
 }
 
@@ -977,22 +1001,27 @@ int be_band_reduce(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double*
   // last panel with something to annihilate: rows below j2 = (p + 1) KB number N - j2 >= 2
   const int plast = (N - 2) / KB - 1;
   const int RPT = (N + PT - 1) / PT;
-  BE_CUDA(cudaMemsetAsync(s.Vx0, 0, (size_t)cnt * Np * LDP * sizeof(cplx), st));
-  BE_CUDA(cudaMemsetAsync(s.Vx1, 0, (size_t)cnt * Np * LDP * sizeof(cplx), st));
-  BE_CUDA(cudaMemsetAsync(s.Wx, 0, (size_t)cnt * Np * LDP * sizeof(cplx), st));
+  BE_CUDA(cudaMemsetAsync(s.Vx0, 0, (size_t)cnt * Np * KB * sizeof(cplx), st));
+  BE_CUDA(cudaMemsetAsync(s.Vx1, 0, (size_t)cnt * Np * KB * sizeof(cplx), st));
+  BE_CUDA(cudaMemsetAsync(s.Wx, 0, (size_t)cnt * Np * KB * sizeof(cplx), st));
   BE_CUDA(cudaMemsetAsync(s.counters, 0, (size_t)(N / KB + 2) * sizeof(int), st));
   BE_CUDA(cudaMemsetAsync(tau, 0, (size_t)cnt * N * sizeof(cplx), st));
   k_symdiag<<<dim3((unsigned)nT, (unsigned)cnt), 256, 0, st>>>(Bw, N);
   LAUNCH_CHECK();
-  const size_t psm = (size_t)(RPT - 1 > 2 ? RPT - 1 : 2) * PT * KB * sizeof(cplx);
+  const size_t psm = (size_t)(RPT - 1) * PT * KB * sizeof(cplx);
   auto panel = [&](int p, int do_qr) -> int {
     cplx* vn = (p & 1) ? s.Vx1 : s.Vx0;
     cplx* vp = (p & 1) ? s.Vx0 : s.Vx1;
     be_prof_begin(ctx, PK_PANEL);
     const int n = N - p * KB;
+    if (p > 0) {
+      const int J0 = (p * KB) / TS;
+      k_ysum<<<dim3((unsigned)(nT - J0), (unsigned)cnt), 512, 0, st>>>(s.P, s.Zc, vp, s.Wx, s.Mpart, N, Np, nT, J0, p * KB);
+      ctx->launches++;
+    }
 #define PANEL_CASE(R) case R: \
       BE_CUDA(cudaFuncSetAttribute(k_panel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm)); \
-      k_panel<R><<<(unsigned)cnt, PT, psm, st>>>(Bw, vn, vp, s.Wx, s.P, s.Zc, s.T1, tau, N, Np, nT, p, do_qr); break;
+      k_panel<R><<<(unsigned)cnt, PT, psm, st>>>(Bw, vn, vp, s.Wx, s.Mpart, s.T1, tau, N, Np, nT, p, do_qr); break;
     switch (RPT) {
       PANEL_CASE(1) PANEL_CASE(2) PANEL_CASE(3) PANEL_CASE(4)
       default: return BE_ERR_UNSUPPORTED;
@@ -1056,15 +1085,15 @@ int be_band_reduce(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double*
 
 int be_band_q2(be_ctx* ctx, const cplx* Bw, cplx* X, int64_t cnt, int N, int nv) {
   if (nv <= 0) return BE_OK;
-  // columns per CTA: a divisor-friendly multiple of 32 (nv = 800 -> 5 CTAs of 160 columns)
+  // columns per CTA: a divisor-friendly multiple of 32 (nv = 800 -> 7 CTAs of 128 columns)
   int nslab = (nv + Q2_TSG_MAX - 1) / Q2_TSG_MAX;
   int tsg = (((nv + nslab - 1) / nslab) + 31) / 32 * 32;
   nslab = (nv + tsg - 1) / tsg;
-  const size_t smem = ((size_t)2 * QS * QG * KB + (size_t)2 * (QS - 1) * KB * tsg) * sizeof(cplx);
+  const size_t smem = ((size_t)2 * QS * QG * KB + (size_t)2 * QS * KB * tsg) * sizeof(cplx);
   BE_CUDA(cudaFuncSetAttribute(k_q2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   be_prof_begin(ctx, PK_Q2);
   k_q2<<<dim3((unsigned)nslab, (unsigned)cnt), QS * tsg, smem, ctx->stream>>>(Bw, X, N, nv, tsg);
-  be_prof_end(ctx, PK_Q2, (double)cnt * nv * N * 32.0 * ((N + QS * QG - 1) / (QS * QG)), (double)cnt * 8.0 * N * (double)N * nv);
+  be_prof_end(ctx, PK_Q2, (double)cnt * nv * N * 16.0 * ((N + QS * QG - 1) / (QS * QG)), (double)cnt * 8.0 * N * (double)N * nv);
   LAUNCH_CHECK();
   return BE_OK;
 }
