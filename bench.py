@@ -248,7 +248,7 @@ def main():
     ap.add_argument("--small", action="store_true", help="reduced workload for quick checks (not a bench value)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--eigh-algo", type=int, default=None, choices=[0, 1],
+    ap.add_argument("--eigh-algo", type=int, default=None, choices=[0, 1, 2],
                     help="tridiagonalization: 0 one-stage, 1 two-stage (default: the library's)")
     args = ap.parse_args()
 

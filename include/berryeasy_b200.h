@@ -77,15 +77,16 @@ int be_set_workspace_limit(be_ctx* ctx, size_t bytes);
  * CTA per SM what the overlap gains -- DESIGN.md section 11), hence the default. */
 int be_set_chunk_pipeline(be_ctx* ctx, int on);
 
-/* Algorithm of the Hermitian tridiagonalization inside S1 for 256 <= N <= 2048:
+/* Algorithm of the Hermitian tridiagonalization inside S1:
  *   0  one-stage blocked Householder reduction (half of its flops are matrix-vector products streamed
  *      from HBM once per column);
  *   1  two-stage reduction: dense -> band of width 8 in ONE fused tensor-core pass over the trailing
- *      matrix per 8 columns, band -> tridiagonal by bulge chasing on chip, eigenvectors
- *      back-transformed through both stages (the default).
- * Outside that range of N, and for N <= 104 (on-chip paths), the setting is ignored.  Both produce
- * eigenpairs to the same tolerance; selectable per context so that they can be timed on the same input.
- * Returns BE_ERR_SHAPE for any other value. */
+ *      matrix per 8 columns, band -> tridiagonal by bulge chasing, eigenvectors back-transformed
+ *      through both stages, for every 128 <= N <= 2048;
+ *   2  (default) two-stage where it was measured faster (N >= 1024), one-stage below.
+ * Outside 128 <= N <= 2048 the setting is ignored (N <= 104: on-chip paths; N > 2048: one-stage).  Both
+ * produce eigenpairs to the same tolerance; selectable per context so that they can be timed on the
+ * same input.  Returns BE_ERR_SHAPE for any other value. */
 int be_set_eigh_algorithm(be_ctx* ctx, int algo);
 
 /* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */

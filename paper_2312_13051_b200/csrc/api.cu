@@ -116,6 +116,7 @@ extern "C" int be_create(be_ctx** out, void* cuda_stream) {
   if (e != cudaSuccess) { delete c; return (int)e; }
   c->sm_count = prop.multiProcessorCount;
   c->ws_limit = (size_t)64 << 30;
+  c->eigh_algo = 2;
   *out = c;
   return BE_OK;
 }
@@ -165,7 +166,7 @@ extern "C" int be_set_chunk_pipeline(be_ctx* ctx, int on) {
 
 extern "C" int be_set_eigh_algorithm(be_ctx* ctx, int algo) {
   if (!ctx) return BE_ERR_NULL;
-  if (algo < 0 || algo > 1) return BE_ERR_SHAPE;
+  if (algo < 0 || algo > 2) return BE_ERR_SHAPE;
   ctx->eigh_algo = algo;
   return BE_OK;
 }

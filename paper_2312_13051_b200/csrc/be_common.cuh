@@ -225,7 +225,7 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
 size_t be_eigh_large_scratch_bytes(int64_t cnt, int N, int nv);
 // two-stage reduction (eigh_band.cu): dense -> band of width BE_BAND_KB -> tridiagonal
 constexpr int BE_BAND_KB = 8;
-constexpr int BE_BAND_MINN = 128, BE_BAND_MAXN = 2048;
+constexpr int BE_BAND_MINN = 128, BE_BAND_MAXN = 2048, BE_BAND_AUTON = 1024;
 size_t be_band_scratch_bytes(int64_t cnt, int N);
 int be_band_reduce(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double* e, cplx* tau, void* scratch);
 int be_band_q2(be_ctx* ctx, const cplx* Bw, cplx* X, int64_t cnt, int N, int nv);

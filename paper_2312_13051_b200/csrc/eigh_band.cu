@@ -591,17 +591,6 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
         Lw[0] = wr[0]; Lw[1] = wr[Np]; Lv[0] = vr[0]; Lv[1] = vr[Np];
       }
       lw0 = Lw[0]; lw1 = Lw[1]; lv0 = Lv[0]; lv1 = Lv[1];
-      // fragments of the next tile, if the producer has already announced it
-      if (*published > gt + 1) {
-        const int nc2 = desc[(gt + 1) & 3].x, nI = desc[(gt + 1) & 3].z;
-        if (nc2 >= 0) {
-          const int nr2 = nI * TS + 8 * w + g;
-          const cplx* wr = Wx + (int64_t)nc2 * KB * Np + PIX(2 * q, nr2);
-          const cplx* vr = Vprev + (int64_t)nc2 * KB * Np + PIX(2 * q, nr2);
-          Lw[0] = wr[0]; Lw[1] = wr[Np]; Lv[0] = vr[0]; Lv[1] = vr[Np];
-          Lfor = gt + 1;
-        }
-      }
     }
     // accumulators <- tile: thread holds A[8w+g][8nb + 2q + j]
     double ar[8][2], ai[8][2];
@@ -627,15 +616,24 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
           dmma(ai[nb][0], ai[nb][1], l_r[ks], rj.y);
         }
       }
-      // step 2: back to shared memory (same positions), then the bulk store by the producer
+      // step 2: back to shared memory (same positions); the bulk store by the producer follows the barrier below
       cplx* atw = At + (size_t)s * TS * LDT;
 #pragma unroll
       for (int nb = 0; nb < 8; ++nb)
 #pragma unroll
         for (int j = 0; j < 2; ++j) atw[(8 * nb + 2 * q + j) * LDT + 8 * w + g] = mkc(ar[nb][j], ai[nb][j]);
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-      if (tid == 0) mbar_arrive(&stready[s]);
+      // fragments of the next tile (the producer announced it when this tile started: no race by now)
+      if (*published > gt + 1) {
+        const int nc2 = desc[(gt + 1) & 3].x, nI = desc[(gt + 1) & 3].z;
+        if (nc2 >= 0) {
+          const int nr2 = nI * TS + 8 * w + g;
+          const cplx* wr = Wx + (int64_t)nc2 * KB * Np + PIX(2 * q, nr2);
+          const cplx* vr = Vprev + (int64_t)nc2 * KB * Np + PIX(2 * q, nr2);
+          Lw[0] = wr[0]; Lw[1] = wr[Np]; Lv[0] = vr[0]; Lv[1] = vr[Np];
+          Lfor = gt + 1;
+        }
+      }
     }
     // step 3: Y_I[8w+g][n] += sum_col A[.][col] V+_J[col][n]; k index q <-> column 8nb + 2q + j
     {
@@ -654,6 +652,11 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
       cplx* pr = P + ((int64_t)c * nT + J) * KB * Np + PIX(2 * q, rI);
       pr[0] = mkc(yr[0][0] + yr[1][0], yi[0][0] + yi[1][0]);
       pr[Np] = mkc(yr[0][1] + yr[1][1], yi[0][1] + yi[1][1]);
+    }
+    if (has_upd) {
+      // every warp's part of the updated tile is in shared memory: release the bulk store, start step 4
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      if (tid == 0) mbar_arrive(&stready[s]);
     }
     // step 4: Z[m][col] += sum_row conj(V+_I[row][m]) A[row][col], col = 8w + n;  Y_J[col][m] = conj(Z[m][col])
     if (I != J) {

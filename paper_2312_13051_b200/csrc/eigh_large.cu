@@ -848,7 +848,10 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
   // panel width: the panel work (k_colw and the panel block columns of k_hemv) grows with nb / n, the
   // rank-2k GEMM likes a deep K = 2 nb: 16 for mid-size matrices, NB = 32 for large ones
   const int nb = (N <= 640) ? NB / 2 : NB;
-  const bool two_stage = ctx->eigh_algo == 1 && N >= BE_BAND_MINN && N <= BE_BAND_MAXN;
+  // 1: two-stage wherever it is supported; 2 (default): where it is faster -- measured on B200: N = 1600 (half of the
+  // vectors) 905 vs 1035 ms per 300 matrices, N = 800 (all vectors) 215 vs 203 ms, N = 400 even
+  const bool two_stage = N >= BE_BAND_MINN && N <= BE_BAND_MAXN &&
+                         (ctx->eigh_algo == 1 || (ctx->eigh_algo == 2 && N >= BE_BAND_AUTON));
   if (two_stage) BE_TRY(be_band_reduce(ctx, s.Bw, cnt, N, s.d, s.e, s.tau, s.band));
   for (int p = 0; p < N && !on_chip && !two_stage; p += nb) {
     if (p > 0 && N - p <= TS_MAXN) {
