@@ -51,6 +51,24 @@ __device__ __forceinline__ cplx shfl_xor_c(cplx v, int m) {
   return mkc(__shfl_xor_sync(0xffffffffu, v.x, m), __shfl_xor_sync(0xffffffffu, v.y, m));
 }
 
+// Scalars of a Householder reflector H = I - tau v v^H, H^H (alpha; x) = (beta; 0), |x|^2 = xn2 > 0 or Im alpha != 0
+// (zlarfg): beta = -sign(Re alpha) sqrt(|alpha|^2 + xn2), tau = (beta - alpha) / beta, v = x / (alpha - beta).
+// IEEE double division and square root are ~100-instruction dependent chains on the GPU, and these scalars sit on
+// the critical path of every chase step and every panel column: rsqrt + one Newton step and one reciprocal instead.
+__device__ __forceinline__ void larfg_scalars(cplx alpha, double xn2, double& beta, cplx& tau, cplx& scale) {
+  const double s2 = cabs2(alpha) + xn2;
+  const double r = rsqrt(s2);
+  double nb = s2 * r;
+  nb = fma(0.5 * r, fma(-nb, nb, s2), nb);          // |beta| to the last bit or two
+  const bool pos = alpha.x >= 0.0;
+  beta = pos ? -nb : nb;
+  const double ib = pos ? -r : r;                    // 1 / beta (relative error ~1e-16)
+  tau = mkc(fma(-alpha.x, ib, 1.0), -alpha.y * ib);
+  const double dx = alpha.x - beta;                  // no cancellation: beta has the opposite sign
+  const double rd = __drcp_rn(fma(dx, dx, alpha.y * alpha.y));
+  scale = mkc(dx * rd, -alpha.y * rd);
+}
+
 // ------------------------------------------------------------------------------------------
 // The diagonal 64 x 64 tiles get their upper triangle from the lower one (the input contract reads
 // only one triangle of H), and an exactly real diagonal.
@@ -346,9 +364,8 @@ __global__ void __launch_bounds__(PT, 1) k_panel(cplx* __restrict__ Bw, cplx* __
     if (xn2 == 0.0) {
       tau = mkc(0.0, 0.0); scale = mkc(0.0, 0.0); betac = alpha;
     } else {
-      const double beta = -copysign(sqrt(cabs2(alpha) + xn2), alpha.x);
-      tau = mkc((beta - alpha.x) / beta, -alpha.y / beta);
-      scale = cdiv(mkc(1.0, 0.0), mkc(alpha.x - beta, alpha.y));
+      double beta;
+      larfg_scalars(alpha, xn2, beta, tau, scale);
       betac = mkc(beta, 0.0);
     }
     // f[q] = conj(tau) (head[q] + conj(scale) g[q]),  q > cc
@@ -704,48 +721,91 @@ __global__ void k_band_extract(const cplx* __restrict__ Bw, cplx* __restrict__ A
   AB[c * (int64_t)N * LDAB + idx] = v;
 }
 
-// Bulge chasing, one CTA per matrix, one warp per sweep; sweep i runs its chase steps k = 0, 1, ..
-// (reflector on rows i + 1 + k KB ..) one per time step, starting at start[i] (host schedule: sweep i + 1
-// stays two steps behind sweep i, a warp takes the sweeps w, w + G, ..).  Step (i, k):
+// Bulge chasing, one CTA per matrix, one warp per sweep.  The G sweeps i0 .. i0 + G - 1 of a "train" run
+// two chase steps apart (sweep i0 + w does step k = t - 2w at time t), so everything the train touches at
+// time t lies in a window of 15 G + 16 columns of the band, which is kept in a ring buffer in shared memory:
+// per time step 8 columns enter at the front (cp.async, fetched one step ahead) and 8 leave at the back.
+// Step (i, k), reflector on the rows st = i + 1 + k KB ..:
 //   k > 0: E = A[R_k, R_{k-1}] <- E H_{k-1};  H_k from E[:, 0];  E <- H_k^H E
 //   k = 0: H_0 from A[R_0, i]
 //   D = A[R_k, R_k] <- H_k^H D H_k
 // Lane (rr = lane & 7, cg = lane >> 3) holds rows rr, columns cg and cg + 4 of a KB x KB block.  The
 // reflector (tau in the head slot) is stored in the upper triangle of the work matrix: V2(i, rho) at
 // Bw[i + rho N], rho = row the entry acts on.
-__global__ void __launch_bounds__(512) k_chase(cplx* __restrict__ ABw, cplx* __restrict__ Bw, double* __restrict__ dd,
-                                               double* __restrict__ ee, const int* __restrict__ start, int N, int tend) {
+constexpr int CH_RING = 256;     // columns of the ring buffer (>= 15 G + 16 + 8)
+constexpr int CH_GMAX = 15;
+__global__ void __launch_bounds__(CH_GMAX * 32) k_chase(cplx* __restrict__ ABw, cplx* __restrict__ Bw, double* __restrict__ dd,
+                                                       double* __restrict__ ee, int N) {
   static_assert(KB == 8, "lane mapping written for KB = 8");
+  extern __shared__ __align__(16) cplx ring[];   // [CH_RING][LDAB]
   const int64_t c = blockIdx.x;
-  cplx* __restrict__ ab = ABw + c * (int64_t)N * LDAB;
+  cplx* __restrict__ abg = ABw + c * (int64_t)N * LDAB;
   cplx* __restrict__ Bc = Bw + c * (int64_t)N * N;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, G = blockDim.x >> 5;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, G = blockDim.x >> 5;
   const int rr = lane & 7, cg = lane >> 3;
-  int i = warp;
-  int st_i = (i < N - 1) ? start[i] : 0;
-  cplx vprev = mkc(0.0, 0.0), tauprev = mkc(0.0, 0.0);
-  for (int t = 0; t < tend; ++t) {
-    while (i < N - 1 && t - st_i >= (N - 1 - i + KB - 1) / KB) {
-      i += G;
-      st_i = (i < N - 1) ? start[i] : 0;
+#define RG(col, d) ring[((col) & (CH_RING - 1)) * LDAB + (d)]
+  // columns [c0, c1) global -> ring (cp.async, 16 bytes per thread and element)
+  auto load_cols = [&](int c0, int c1) {
+    if (c1 > N) c1 = N;
+    for (int idx = tid; idx < (c1 - c0) * LDAB; idx += blockDim.x) {
+      const int col = c0 + idx / LDAB, d = idx % LDAB;
+      const uint32_t dst = smem_u32(&RG(col, d));
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(abg + (int64_t)col * LDAB + d) : "memory");
     }
-    const int k = t - st_i;
-    if (i < N - 1 && k >= 0) {
+  };
+  auto store_cols = [&](int c0, int c1) {
+    if (c1 > N) c1 = N;
+    for (int idx = tid; idx < (c1 - c0) * LDAB; idx += blockDim.x) {
+      const int col = c0 + idx / LDAB, d = idx % LDAB;
+      abg[(int64_t)col * LDAB + d] = RG(col, d);
+    }
+  };
+  for (int i0 = 0; i0 < N - 1; i0 += G) {
+    const int i = i0 + warp;
+    const int T = (N - 1 - i0 + KB - 1) / KB + 2 * (G - 1);   // time steps of this train
+    int back = i0;                                            // columns < back are in memory
+    int front = (i0 + 9 < N) ? i0 + 9 : N;                    // columns < front are in the ring (or on their way)
+    load_cols(i0, front);
+    asm volatile("cp.async.commit_group;\n" ::: "memory");
+    cplx vprev = mkc(0.0, 0.0), tauprev = mkc(0.0, 0.0);
+    for (int t = 0; t < T; ++t) {
+      asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+      __syncthreads();
+      {
+        // the columns of the next step enter; those the last sweep left two steps ago go back to memory
+        const int nf = (i0 + 8 * (t + 1) + 9 < N) ? i0 + 8 * (t + 1) + 9 : N;
+        if (nf > front) { load_cols(front, nf); front = nf; }
+        asm volatile("cp.async.commit_group;\n" ::: "memory");
+        int nb = i0 + G + 8 * (t - 2 * (G - 1)) - 16;         // st of the last sweep at time t, minus 16
+        if (nb > front) nb = front;
+        if (nb > back) { store_cols(back, nb); back = nb; }
+      }
+      const int k = t - 2 * warp;
+      if (i >= N - 1 || k < 0) continue;
       const int st = i + 1 + k * KB;
+      if (st >= N) continue;
       const int len = (N - st < KB) ? N - st : KB;
-      // ---- loads (independent: one L2 round trip)
       cplx e0 = mkc(0.0, 0.0), e1 = mkc(0.0, 0.0), d0 = mkc(0.0, 0.0), d1 = mkc(0.0, 0.0), x = mkc(0.0, 0.0);
       if (k > 0 && rr < len) {
-        e0 = __ldcg(&ab[(int64_t)(st - KB + cg) * LDAB + KB + rr - cg]);
-        e1 = __ldcg(&ab[(int64_t)(st - KB + cg + 4) * LDAB + KB + rr - cg - 4]);
+        e0 = RG(st - KB + cg, KB + rr - cg);
+        e1 = RG(st - KB + cg + 4, KB + rr - cg - 4);
       }
       if (rr < len) {
-        if (cg < len) d0 = (rr >= cg) ? __ldcg(&ab[(int64_t)(st + cg) * LDAB + rr - cg])
-                                      : cconj(__ldcg(&ab[(int64_t)(st + rr) * LDAB + cg - rr]));
-        if (cg + 4 < len) d1 = (rr >= cg + 4) ? __ldcg(&ab[(int64_t)(st + cg + 4) * LDAB + rr - cg - 4])
-                                              : cconj(__ldcg(&ab[(int64_t)(st + rr) * LDAB + cg + 4 - rr]));
+        // full Hermitian block from the stored lower triangle: one load, conjugated above the diagonal
+        if (cg < len) {
+          const bool lo = rr >= cg;
+          const int cc_ = lo ? st + cg : st + rr, oo_ = lo ? rr - cg : cg - rr;
+          d0 = RG(cc_, oo_);
+          if (!lo) d0.y = -d0.y;
+        }
+        if (cg + 4 < len) {
+          const bool lo = rr >= cg + 4;
+          const int cc_ = lo ? st + cg + 4 : st + rr, oo_ = lo ? rr - cg - 4 : cg + 4 - rr;
+          d1 = RG(cc_, oo_);
+          if (!lo) d1.y = -d1.y;
+        }
       }
-      if (k == 0 && cg == 0 && rr < len) x = __ldcg(&ab[(int64_t)i * LDAB + 1 + rr]);
+      if (k == 0 && cg == 0 && rr < len) x = RG(i, 1 + rr);
       if (k > 0) {
         // E <- E H_{k-1}
         const cplx vp0 = shfl_c(vprev, cg), vp1 = shfl_c(vprev, cg + 4);
@@ -769,15 +829,13 @@ __global__ void __launch_bounds__(512) k_chase(cplx* __restrict__ ABw, cplx* __r
       if (xn2 == 0.0 && alpha.y == 0.0) {
         beta = alpha.x; tau = mkc(0.0, 0.0); scale = mkc(0.0, 0.0);
       } else {
-        beta = -copysign(sqrt(cabs2(alpha) + xn2), alpha.x);
-        tau = mkc((beta - alpha.x) / beta, -alpha.y / beta);
-        scale = cdiv(mkc(1.0, 0.0), mkc(alpha.x - beta, alpha.y));
+        larfg_scalars(alpha, xn2, beta, tau, scale);
       }
       const cplx v = (rr == 0) ? mkc(1.0, 0.0) : (rr < len ? cmul(xr, scale) : mkc(0.0, 0.0));
       if (cg == 0 && rr < len) Bc[i + (int64_t)(st + rr) * N] = (rr == 0) ? tau : v;
       if (k == 0) {
-        if (cg == 0 && rr < len) ab[(int64_t)i * LDAB + 1 + rr] = (rr == 0) ? mkc(beta, 0.0) : mkc(0.0, 0.0);
-        if (lane == 0) { ee[c * N + i] = beta; dd[c * N + i] = __ldcg(&ab[(int64_t)i * LDAB]).x; }
+        if (cg == 0 && rr < len) RG(i, 1 + rr) = (rr == 0) ? mkc(beta, 0.0) : mkc(0.0, 0.0);
+        if (lane == 0) { ee[c * N + i] = beta; dd[c * N + i] = RG(i, 0).x; }
       } else {
         // E <- H^H E (column 0 becomes beta e_1)
         cplx z0 = cmulc(v, e0), z1 = cmulc(v, e1);
@@ -788,8 +846,8 @@ __global__ void __launch_bounds__(512) k_chase(cplx* __restrict__ ABw, cplx* __r
         else cfms(e0, cmul(ct, v), z0);
         cfms(e1, cmul(ct, v), z1);
         if (rr < len) {
-          ab[(int64_t)(st - KB + cg) * LDAB + KB + rr - cg] = e0;
-          ab[(int64_t)(st - KB + cg + 4) * LDAB + KB + rr - cg - 4] = e1;
+          RG(st - KB + cg, KB + rr - cg) = e0;
+          RG(st - KB + cg + 4, KB + rr - cg - 4) = e1;
         }
       }
       // ---- D <- H^H D H = D - w v^H - v w^H,  w = tau p - 1/2 |tau|^2 (v^H p) v,  p = D v
@@ -810,28 +868,19 @@ __global__ void __launch_bounds__(512) k_chase(cplx* __restrict__ ABw, cplx* __r
         cfms(d0, wv, cconj(vc0)); cfms(d0, v, cconj(wc0));
         cfms(d1, wv, cconj(vc1)); cfms(d1, v, cconj(wc1));
         if (rr < len) {
-          if (cg < len && rr >= cg) { if (rr == cg) d0.y = 0.0; ab[(int64_t)(st + cg) * LDAB + rr - cg] = d0; }
-          if (cg + 4 < len && rr >= cg + 4) { if (rr == cg + 4) d1.y = 0.0; ab[(int64_t)(st + cg + 4) * LDAB + rr - cg - 4] = d1; }
+          if (cg < len && rr >= cg) { if (rr == cg) d0.y = 0.0; RG(st + cg, rr - cg) = d0; }
+          if (cg + 4 < len && rr >= cg + 4) { if (rr == cg + 4) d1.y = 0.0; RG(st + cg + 4, rr - cg - 4) = d1; }
         }
       }
       vprev = v; tauprev = tau;
     }
+    asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+    __syncthreads();
+    store_cols(back, front);   // what is left of the window
     __syncthreads();
   }
-  if (threadIdx.x == 0) { dd[c * N + N - 1] = __ldcg(&ab[(int64_t)(N - 1) * LDAB]).x; ee[c * N + N - 1] = 0.0; }
-}
-
-// start[i] of the chase schedule (see be_band_reduce): one thread, N steps
-__global__ void k_chase_schedule(int* __restrict__ start, int N, int G) {
-  for (int i = 0; i < N - 1; ++i) {
-    int t0 = (i > 0) ? start[i - 1] + 2 : 0;
-    if (i >= G) {
-      const int prev = i - G;
-      const int fin = start[prev] + (N - 1 - prev + KB - 1) / KB;
-      if (fin > t0) t0 = fin;
-    }
-    start[i] = t0;
-  }
+  if (tid == 0) { dd[c * N + N - 1] = abg[(int64_t)(N - 1) * LDAB].x; ee[c * N + N - 1] = 0.0; }
+#undef RG
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1060,26 +1109,13 @@ int be_band_reduce(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double*
   k_band_extract<<<dim3((unsigned)((N * LDAB + 255) / 256), (unsigned)cnt), 256, 0, st>>>(Bw, s.AB, N);
   LAUNCH_CHECK();
   {
-    // schedule: sweep i starts at start[i]; two steps behind its predecessor, and after the sweep its warp ran before
-    int G = 16;
-    if (cnt > 2 * (int64_t)ctx->sm_count) G = 8;
-    std::vector<int> start(N, 0);
-    int tend = 0;
-    for (int i = 0; i < N - 1; ++i) {
-      int t0 = (i > 0) ? start[i - 1] + 2 : 0;
-      if (i >= G) {
-        const int prev = i - G;
-        const int fin = start[prev] + (N - 1 - prev + KB - 1) / KB;
-        if (fin > t0) t0 = fin;
-      }
-      start[i] = t0;
-      const int fin = t0 + (N - 1 - i + KB - 1) / KB;
-      if (fin > tend) tend = fin;
-    }
-    k_chase_schedule<<<1, 1, 0, st>>>(s.start, N, G);   // the same recurrence on the device (no host copy, no sync)
-    LAUNCH_CHECK();
+    // warps (sweeps in flight) per matrix: as many as keep the whole chunk resident in one wave (64 KB of
+    // shared memory and <= 64 registers per thread: 3 CTAs of 10 warps per SM, else 2 of 15)
+    int G = CH_GMAX;
+    if (cnt > 2 * (int64_t)ctx->sm_count) G = 10;
+    BE_CUDA(cudaFuncSetAttribute(k_chase, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(CH_RING * LDAB * sizeof(cplx))));
     be_prof_begin(ctx, PK_CHASE);
-    k_chase<<<(unsigned)cnt, G * 32, 0, st>>>(s.AB, Bw, d, e, s.start, N, tend);
+    k_chase<<<(unsigned)cnt, G * 32, CH_RING * LDAB * sizeof(cplx), st>>>(s.AB, Bw, d, e, N);
     be_prof_end(ctx, PK_CHASE, (double)cnt * N * LDAB * 16.0, (double)cnt * 24.0 * N * (double)N * KB);
     LAUNCH_CHECK();
   }
