@@ -248,6 +248,7 @@ def main():
     ap.add_argument("--small", action="store_true", help="reduced workload for quick checks (not a bench value)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--ws-gib", type=float, default=None, help="workspace cap in GiB (default: the library's)")
     ap.add_argument("--eigh-algo", type=int, default=None, choices=[0, 1, 2],
                     help="tridiagonalization: 0 one-stage, 1 two-stage (default: the library's)")
     args = ap.parse_args()
@@ -280,6 +281,8 @@ def main():
     ctx = Context()
     if args.eigh_algo is not None:
         ctx.set_eigh_algorithm(args.eigh_algo)
+    if args.ws_gib is not None:
+        ctx.set_workspace_limit(int(args.ws_gib * 2 ** 30))
     H, S = wk.device_grid(torch, device)
     torch.cuda.synchronize()
 

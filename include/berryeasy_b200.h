@@ -64,8 +64,9 @@ const char* be_strerror(int code);
  * 0 = eigh, 1 = wilson loop, 2 = nested, 3 = spin resolved). */
 size_t be_workspace_bytes(const be_grid* grid, int n_occ, int op);
 
-/* Cap on the scratch used for per-chunk work buffers (default 64 GiB).  Work is processed in
- * chunks of whole loops sized to stay under the cap. */
+/* Cap on the scratch used for per-chunk work buffers (default: 65 % of the device memory, 119 GB on a
+ * B200; the caller's own buffers have to fit beside it).  Work is processed in chunks of whole loops
+ * sized to stay under the cap. */
 int be_set_workspace_limit(be_ctx* ctx, size_t bytes);
 
 /* Two-stream chunk pipeline for be_wilson_loop / be_spin_resolved_wilson when the work is split
