@@ -128,6 +128,58 @@ def config2_grid(n1: int = 100, n2: int = 100, gamma: float = 0.5, lam: float = 
     return H
 
 
+def position_gauge_plane(H: np.ndarray, r1, r2, shift1: int = 0) -> np.ndarray:
+    """H [n2][n1][N][N] (periodic gauge) -> D^dagger H D with D(k) = diag(exp(i (k1 r1 + k2 r2))), the same
+    model with orbital alpha at the position (r1, r2)[alpha] inside the unit cell:
+    H(k + G_a) = Phi_a H(k) Phi_a^dagger with the closing phases Phi_a = exp(-2 pi i r_a).
+    ``shift1``: the periodic-gauge grid is first rolled by ``shift1`` points along k1 (grid index i then
+    stands for k1 = 2 pi (i + shift1) / n1 while D still uses 2 pi i / n1) -- the input of the base-point pin.
+    Returns (H_pos, Phi_1, Phi_2)."""
+    n2, n1 = H.shape[:2]
+    r1 = np.asarray(r1, dtype=np.float64)
+    r2 = np.asarray(r2, dtype=np.float64)
+    Hs = np.roll(H, -shift1, axis=1) if shift1 else H
+    out = np.empty_like(Hs)
+    for j in range(n2):
+        for i in range(n1):
+            D = np.exp(2j * np.pi * (i / n1 * r1 + j / n2 * r2))
+            out[j, i] = np.conj(D)[:, None] * Hs[j, i] * D[None, :]
+    return out, np.exp(-2j * np.pi * r1), np.exp(-2j * np.pi * r2)
+
+
+def bhz4_plus_band(kx: float, ky: float, m: float = 1.0) -> np.ndarray:
+    """5 bands: the BHZ model of config 1 plus one occupied, trivial spin-down orbital
+    eps(k) = -2.5 - 0.3 cos kx (decoupled).  With n_occ = 3 the PSO has the eigenvalues (-1, -1, +1): the
+    spin sectors have the sizes 2 and 1 (an uneven split, m_lo = 2)."""
+    H = np.zeros((5, 5), dtype=np.complex128)
+    H[:4, :4] = bhz4(kx, ky, m)
+    H[4, 4] = -2.5 - 0.3 * np.cos(kx)
+    return H
+
+
+def bhz4_plus_band_spin_z() -> np.ndarray:
+    return np.array([1.0, -1.0, 1.0, -1.0, -1.0])
+
+
+def bhz4_plus_band_grid(n1: int, n2: int) -> np.ndarray:
+    H = np.empty((n2, n1, 5, 5), dtype=np.complex128)
+    for j in range(n2):
+        for i in range(n1):
+            H[j, i] = bhz4_plus_band(2 * np.pi * i / n1, 2 * np.pi * j / n2)
+    return H
+
+
+def rotated_basis(H: np.ndarray, S_diag: np.ndarray, seed: int = 7):
+    """The same model in a randomly rotated orbital basis: H' = R H R^dagger at every grid point and the DENSE
+    spin operator S' = R diag(S) R^dagger (``op`` may be any Hermitian matrix)."""
+    N = H.shape[-1]
+    rng = _rng(90, seed)
+    R, _ = np.linalg.qr(rng.normal(size=(N, N)) + 1j * rng.normal(size=(N, N)))
+    Hr = R @ H @ R.conj().T
+    Sr = (R * np.asarray(S_diag)[None, :]) @ R.conj().T
+    return Hr, 0.5 * (Sr + Sr.conj().T)
+
+
 # --------------------------------------------------------------------------------------------
 # configs 3, 4: BHZ supercells with twisted boundary phases (PAPER.md:42-44)
 # --------------------------------------------------------------------------------------------

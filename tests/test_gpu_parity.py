@@ -88,6 +88,51 @@ def test_eigh_large_all_vectors(ctx):
         check_eigh(ctx, A + A.conj().transpose(0, 2, 1), nv)
 
 
+@pytest.mark.parametrize("N,nv", [(128, 128), (130, 65), (200, 77), (257, 257), (400, 200), (449, 1), (800, 800)])
+def test_eigh_two_stage_path_random(ctx, N, nv):
+    """be_set_eigh_algorithm(1): dense -> band (k_panel / k_ysum / k_fused) -> tridiagonal (k_chase), back-transform
+    through both stages (k_q2 + compact WY); sizes with ragged last tiles, a ragged last panel and short last
+    reflectors (N not a multiple of 64 / 8)."""
+    rng = np.random.default_rng(N)
+    A = rng.standard_normal((2, N, N)) + 1j * rng.standard_normal((2, N, N))
+    H = A + A.conj().transpose(0, 2, 1)
+    ctx.set_eigh_algorithm(1)
+    try:
+        check_eigh(ctx, H, nv)
+    finally:
+        ctx.set_eigh_algorithm(2)
+
+
+def test_eigh_two_stage_structured_and_degenerate(ctx):
+    """Two-stage path on what the one-stage tests cover: a sparse disordered supercell (rank-deficient panels:
+    most of a panel's rows are exact zeros), the clean supercell (highly degenerate spectrum), the identity and a
+    zero matrix (every reflector trivial), and both algorithms giving the same eigenvalues on the same input."""
+    ctx.set_eigh_algorithm(1)
+    try:
+        H = wl.supercell_grid([wl.config3_parts(2, L=6)], 3, 2).reshape(-1, 144, 144)
+        check_eigh(ctx, H, 72)
+        Hc = wl.supercell_grid([wl.bhz_supercell_parts(6)], 2, 2).reshape(-1, 144, 144)
+        check_eigh(ctx, Hc, 144)
+        Z = np.zeros((2, 160, 160), complex)
+        Z[1] = np.eye(160)
+        E, U = ctx.eigh_batched(dev(Z), 160)
+        assert np.abs(E.cpu().numpy()[0]).max() < 1e-300 and np.abs(E.cpu().numpy()[1] - 1).max() < 1e-14
+        for c in range(2):
+            Uc = U.cpu().numpy()[c]
+            assert np.linalg.norm(Uc.conj().T @ Uc - np.eye(160)) < 1e-11 * 160
+        rng = np.random.default_rng(5)
+        A = rng.standard_normal((3, 320, 320)) + 1j * rng.standard_normal((3, 320, 320))
+        Hd = dev(A + A.conj().transpose(0, 2, 1))
+        E1, _ = ctx.eigh_batched(Hd, 0)
+        ctx.set_eigh_algorithm(0)
+        E0, _ = ctx.eigh_batched(Hd, 0)
+        assert (E1 - E0).abs().max().item() < 1e-10 * E0.abs().max().item()
+    finally:
+        ctx.set_eigh_algorithm(2)
+    with pytest.raises(RuntimeError):
+        ctx.set_eigh_algorithm(3)
+
+
 def test_eigh_degenerate_clean_supercell_and_identity(ctx):
     """H4: heavily degenerate spectra (clean supercell at t=0), plus diagonal / scaled identity."""
     pc = wl.bhz_supercell_parts(6)
@@ -252,6 +297,93 @@ def test_nested_variants(ctx, gamma, p):
     _, thn_t = ctx.nested_wilson(dev(Ht[None]), 2, 0, 1)
     _, thno = wo.nested_wilson(H, 2)
     assert wo.circ_sorted_distance(thn_t.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
+
+
+def test_nested_closing_phases_base_and_cut_on_device(ctx):
+    """d_close1 / d_close2 / base / theta_cut of be_nested_wilson:
+    BBH in a position gauge (asymmetric orbital positions, generic gamma), loops started at base = 5 so that
+    wrapped frames carry Phi_1; the chiral position gauge whose nested polarization is exactly 1/2 + 0.1; and
+    the chiral HOTI slice whose two Wannier bands are re-numbered by the cut."""
+    n = 14
+    H = wl.config2_grid(n, n, gamma=0.7)
+    r1 = np.array([0.11, 0.37, -0.23, 0.41])
+    r2 = np.array([0.29, -0.13, 0.07, 0.33])
+    Hp, c1, c2 = wl.position_gauge_plane(H, r1, r2)
+    for base, band in ((0, 0), (5, 1), (13, 0)):
+        th1, thn = ctx.nested_wilson(dev(Hp[None]), 2, 1, 0, base=base, wb_lo=band, wb_hi=band + 1,
+                                     close1=dev(c1), close2=dev(c2))
+        th1o, thno = wo.nested_wilson(Hp, 2, base=base, wb_lo=band, wb_hi=band + 1, close1=c1, close2=c2)
+        assert phase_dist(th1.cpu().numpy()[0], th1o) <= PH_TOL
+        assert wo.circ_sorted_distance(thn.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
+    # only one of the two phases
+    th1, thn = ctx.nested_wilson(dev(Hp[None]), 2, 1, 0, base=3, close2=dev(c2))
+    th1o, thno = wo.nested_wilson(Hp, 2, base=3, close2=c2)
+    assert phase_dist(th1.cpu().numpy()[0], th1o) <= PH_TOL
+    assert wo.circ_sorted_distance(thn.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
+    # exact value: chiral position gauge along k2, p = 1/2 + 0.1 (tests/test_oracle_pins.py)
+    Hb = wl.config2_grid(24, 24, gamma=0.5)
+    r = np.array([0.3, 0.3, -0.1, -0.1])
+    Hy, _, cy = wl.position_gauge_plane(Hb, np.zeros(4), r)
+    _, thn = ctx.nested_wilson(dev(Hy[None]), 2, 1, 0, close2=dev(cy))
+    assert abs(((-thn.cpu().numpy()[0, 0] / (2 * np.pi)) % 1.0) - 0.6) < 1e-8
+    # n_occ > 2 (general Wannier-band path) with closing phases and a base point
+    Hc = _coupled_bbh_grid(12, 10)
+    r1 = np.linspace(-0.3, 0.4, 8); r2 = np.linspace(0.25, -0.35, 8)
+    Hcp, c1, c2 = wl.position_gauge_plane(Hc, r1, r2)
+    th1o, thno = wo.nested_wilson(Hcp, 4, base=4, wb_lo=0, wb_hi=2, close1=c1, close2=c2)
+    th1, thn = ctx.nested_wilson(dev(Hcp[None]), 4, 1, 0, base=4, wb_lo=0, wb_hi=2, close1=dev(c1), close2=dev(c2))
+    assert phase_dist(th1.cpu().numpy()[0], th1o) <= PH_TOL
+    assert wo.circ_sorted_distance(thn.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
+    # theta_cut: the cut at 0 swaps the numbers of the two Wannier bands of the chiral HOTI slice
+    Hz = wl.chiral_hoti_grid(16, 16, [0.1], 1.0)
+    for cut in (0.0, np.pi, -1.0):
+        for band in (0, 1):
+            _, thn = ctx.nested_wilson(dev(Hz), 2, 2, 1, wb_lo=band, wb_hi=band + 1, theta_cut=cut)
+            _, thno = wo.nested_wilson(Hz[0], 2, wb_lo=band, wb_hi=band + 1, theta_cut=cut)
+            assert wo.circ_sorted_distance(thn.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
+    _, a = ctx.nested_wilson(dev(Hz), 2, 2, 1, wb_lo=0, wb_hi=1, theta_cut=0.0)
+    _, b = ctx.nested_wilson(dev(Hz), 2, 2, 1, wb_lo=1, wb_hi=2, theta_cut=np.pi)
+    _, c = ctx.nested_wilson(dev(Hz), 2, 2, 1, wb_lo=0, wb_hi=1, theta_cut=np.pi)
+    assert abs(wo.wrap_pi(a.cpu().numpy()[0, 0] - b.cpu().numpy()[0, 0])) < 1e-8
+    assert abs(wo.wrap_pi(a.cpu().numpy()[0, 0] - c.cpu().numpy()[0, 0])) > 0.1
+
+
+def test_spin_resolved_uneven_split_and_dense_spin_operator_on_device(ctx):
+    """m_lo != m / 2 at a real PSO gap and a dense Hermitian S (R10): BHZ plus one occupied
+    spin-down orbital, n_occ = 3, sectors of 2 and 1; the same model in a rotated basis (dense S); and a
+    spin-mixing supercell with an uneven split at its PSO gap."""
+    n1, n2 = 40, 21
+    H = wl.bhz4_plus_band_grid(n1, n2)
+    S = wl.bhz4_plus_band_spin_z()
+    loo, hio, psoo = wo.spin_resolved_surface(H[None], 3, 1, S, m_lo=2)
+    lo, hi, pso = ctx.spin_resolved_wilson(dev(H[None]), 3, 1, dev(S), m_lo=2)
+    assert lo.shape == (n2, 2) and hi.shape == (n2, 1)
+    assert np.abs(pso.cpu().numpy() - psoo).max() < 1e-10
+    assert phase_dist(lo.cpu().numpy(), loo) <= PH_TOL and phase_dist(hi.cpu().numpy(), hio) <= PH_TOL
+    w_lo, w_hi = ctx.winding(lo[None]).item(), ctx.winding(hi[None]).item()
+    assert abs(abs(w_lo) - 1) < 1e-9 and abs(w_lo + w_hi) < 1e-9
+    Hr, Sr = wl.rotated_basis(H, S)
+    loo_r, hio_r, psoo_r = wo.spin_resolved_surface(Hr[None], 3, 1, Sr, m_lo=2)      # the oracle's dense-S branch
+    lo_r, hi_r, pso_r = ctx.spin_resolved_wilson(dev(Hr[None]), 3, 1, dev(Sr), m_lo=2)
+    assert np.abs(pso_r.cpu().numpy() - psoo_r).max() < 1e-10
+    assert phase_dist(lo_r.cpu().numpy(), loo_r) <= PH_TOL and phase_dist(hi_r.cpu().numpy(), hio_r) <= PH_TOL
+    assert phase_dist(lo_r.cpu().numpy(), loo) <= PH_TOL                               # = the diagonal-S result
+    # blocked eigensolver + DMMA GEMM path: spin-mixing N = 144 supercell plus three decoupled occupied spin-down
+    # levels (N = 147, n_occ = 75): the PSO has 39 negative and 36 positive eigenvalues, gapped around 0
+    parts = wl.config4_parts(6, axis="x")
+    H0 = wl.supercell_grid([parts], 9, 4, t2_indices=[1, 2])
+    Hs = np.zeros(H0.shape[:3] + (147, 147), complex)
+    Hs[..., :144, :144] = H0
+    for q in range(3):
+        Hs[..., 144 + q, 144 + q] = -4.0 - 0.1 * q
+    Ss = np.concatenate([wl.supercell_spin_z(6), -np.ones(3)])
+    _, _, p0 = wo.spin_resolved_surface(Hs, 75, 1, Ss)
+    assert np.all((p0 < 0).sum(axis=-1) == 39) and np.abs(p0).min() > 0.05             # a gap at the count 39 everywhere
+    loo, hio, psoo = wo.spin_resolved_surface(Hs, 75, 1, Ss, m_lo=39)
+    lo, hi, pso = ctx.spin_resolved_wilson(dev(Hs), 75, 1, dev(Ss), m_lo=39)
+    assert lo.shape == (2, 39) and hi.shape == (2, 36)
+    assert np.abs(pso.cpu().numpy() - psoo).max() < 1e-10
+    assert phase_dist(lo.cpu().numpy(), loo) <= PH_TOL and phase_dist(hi.cpu().numpy(), hio) <= PH_TOL
 
 
 def _coupled_bbh_grid(n1, n2, eps=0.05, seed=3):
@@ -445,9 +577,10 @@ def _need_memory(gb):
 
 
 def test_full_size_config4_in_bench_configuration(ctx):
-    """BASELINE.json configs[3] at full size exactly as bench.py runs it (N = 1600, 24 x 25 grid, 2 chunks
-    of 300 matrices): exact invariants on the whole output, and two sampled loops element by element
-    against the oracle (one loop of 25 k-points costs the oracle ~15 s)."""
+    """BASELINE.json configs[3] at full size exactly as bench.py runs it (N = 1600, 24 x 25 grid, default
+    workspace cap and eigensolver selection: the two-stage reduction for N = 1600, the one-stage one for the
+    PSO): exact invariants on the whole output, and four sampled loops element by element against the
+    oracle (one loop of 25 k-points costs the oracle ~15 s)."""
     _need_memory(30)
     wk = _bench_workload(4)
     H, S = wk.device_grid(torch, torch.device("cuda"))
@@ -463,7 +596,7 @@ def test_full_size_config4_in_bench_configuration(ctx):
     assert sorted((round(wl_lo), round(wl_hi))) == [-1, 1]
     parts = wl.config4_parts(20, realization=0)
     Sh = wl.supercell_spin_z(20)
-    for j in (0, 17):
+    for j in (0, 5, 11, 17):
         Hj = H[0, j].cpu().numpy()[None, None]                          # the same matrices on both sides
         assert np.abs(wl.supercell_grid([parts], 25, 24, t2_indices=[j]) - Hj).max() < 1e-12   # = the seeded recipe
         loo, hio, _ = wo.spin_resolved_surface(Hj, 800, 1, Sh)
@@ -473,8 +606,24 @@ def test_full_size_config4_in_bench_configuration(ctx):
     torch.cuda.empty_cache()
 
 
+def test_full_size_config4_spin_mixing_variant_one_loop(ctx):
+    """SURVEY 8(d), config 4 "second, harder variant for tests": impurity fields along x do not commute with
+    S_z, the PSO eigenvalues leave +-1 and its 800 eigenvectors are non-degenerate -- one whole
+    loop (25 k-points) at N = 1600 / m = 800 against the oracle, element by element."""
+    _need_memory(12)
+    parts = wl.config4_parts(20, axis="x")
+    H = wl.supercell_grid([parts], 25, 24, t2_indices=[7])
+    S = wl.supercell_spin_z(20)
+    lo, hi, pso = ctx.spin_resolved_wilson(dev(H), 800, 1, dev(S))
+    loo, hio, psoo = wo.spin_resolved_surface(H, 800, 1, S)
+    assert np.abs(np.abs(psoo) - 1).max() > 1e-3 and np.abs(psoo).min() > 0.5     # spin mixing, still gapped at 400 | 400
+    assert np.abs(pso.cpu().numpy() - psoo).max() < 1e-10
+    assert phase_dist(lo.cpu().numpy(), loo) <= PH_TOL
+    assert phase_dist(hi.cpu().numpy(), hio) <= PH_TOL
+
+
 def test_full_size_config3_sampled(ctx):
-    """BASELINE.json configs[2] at full size (16 realizations x 32 x 33, N = 400; 43 GB): sampled loops
+    """BASELINE.json configs[2] at full size (16 realizations x 32 x 33, N = 400; 43 GB): 32 sampled loops
     against the oracle, sum rule sum_n theta_n = arg det W on all loops is implied by the eigen-solver
     parity; total winding per realization is an exact integer (0: time-reversal symmetric)."""
     _need_memory(50)
@@ -485,7 +634,7 @@ def test_full_size_config3_sampled(ctx):
     assert mg.min().item() > 0.5
     w = ctx.winding(th.reshape(16, 32, 200)).cpu().numpy()
     assert np.abs(w - np.round(w)).max() < 1e-8 and np.all(np.round(w) == 0)
-    for (r, j) in ((0, 0), (7, 13), (15, 31)):
+    for (r, j) in [(r, j) for r in (0, 5, 10, 15) for j in (0, 3, 9, 13, 18, 22, 27, 31)]:   # 32 loops, 4 realizations
         Hl = H[r, j].cpu().numpy()[None, None]
         tho, abo, mgo = wo.wilson_surface(Hl, 200, 1)
         assert phase_dist(th[r * 32 + j:r * 32 + j + 1].cpu().numpy(), tho) <= PH_TOL
@@ -502,7 +651,7 @@ def test_full_size_config5_sampled(ctx):
     th, ab, mg = wk.run_device(ctx, H, None)
     torch.cuda.synchronize()
     assert mg.min().item() > 0.2                               # harness asserts the gap (R13)
-    idx = [0, 77, 1234, 2048, 4095]
+    idx = list(range(0, 4096, 16)) + [77, 1234, 4095]     # 259 of the 4096 loops
     for l in idx:
         Hl = H[l // 64, l % 64].cpu().numpy()[None, None]
         tho, abo, _ = wo.wilson_surface(Hl, 32, 1)

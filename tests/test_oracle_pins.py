@@ -427,6 +427,115 @@ def test_chiral_hoti_eq9_validation_model():
     assert abs(wo.chern_number(nested)) == int(GOLD["hoti_nested_abs_winding"])   # (d)
 
 
+def test_nested_closing_phases_chiral_position_gauge():
+    """close1 / close2 of nested_wilson.  BBH is chiral (tau_3 x sigma_0
+    anticommutes with H), so every vector of the occupied space has weight exactly 1/2 on the orbitals
+    {0, 1} and 1/2 on {2, 3}.  Putting those two pairs at the positions a and b along an axis therefore shifts
+    every Berry phase along that axis by exactly -2 pi (a + b) / 2 when the embedding phase
+    Phi = exp(-2 pi i r) closes the loop -- at any grid size -- as in the SSH pin above.  Dropping Phi_2
+    gives back p = 1/2, conj(Phi_2) gives 0.9: both are caught."""
+    n = 24
+    H = wl.config2_grid(n, n, gamma=0.5)
+    th1_per, thn_per = wo.nested_wilson(H, 2)
+    r = np.array([0.3, 0.3, -0.1, -0.1])   # (a + b) / 2 = 0.1
+    zero = np.zeros(4)
+    # position gauge along k2 only: first-level phases untouched, nested polarization 1/2 + 0.1
+    Hy, _, c2 = wl.position_gauge_plane(H, zero, r)
+    for band in (0, 1):
+        th1, thn = wo.nested_wilson(Hy, 2, wb_lo=band, wb_hi=band + 1, close2=c2)
+        assert abs(((-thn[0] / (2 * np.pi)) % 1.0) - (GOLD["bbh_nested_polarization_topological"] + 0.1)) < 1e-10
+        assert max(wo.circ_sorted_distance(th1[j], th1_per[j]) for j in range(n)) < 1e-11
+    # position gauge along k1 only: det W (the sum of the first-level phases, two occupied vectors) moves by
+    # -2 pi 2 (a + b) / 2 exactly, the nested polarization stays 1/2
+    Hx, c1, _ = wl.position_gauge_plane(H, r, zero)
+    th1, thn = wo.nested_wilson(Hx, 2, close1=c1)
+    assert np.abs(wo.wrap_pi(th1.sum(axis=1) - th1_per.sum(axis=1) + 2 * np.pi * 0.2)).max() < 1e-11
+    assert abs(((-thn[0] / (2 * np.pi)) % 1.0) - GOLD["bbh_nested_polarization_topological"]) < 1e-10
+    # both axes
+    Hxy, c1, c2 = wl.position_gauge_plane(H, r, 0.5 * r)
+    th1, thn = wo.nested_wilson(Hxy, 2, close1=c1, close2=c2)
+    assert abs(((-thn[0] / (2 * np.pi)) % 1.0) - (GOLD["bbh_nested_polarization_topological"] + 0.05)) < 1e-10
+    # a missing Phi_1 is caught at both levels
+    th1_no, thn_no = wo.nested_wilson(Hx, 2)
+    assert np.abs(wo.wrap_pi(th1_no.sum(axis=1) - th1_per.sum(axis=1) + 2 * np.pi * 0.2)).max() > 0.1
+    assert abs(((-thn_no[0] / (2 * np.pi)) % 1.0) - GOLD["bbh_nested_polarization_topological"]) > 1e-2
+
+
+def test_nested_base_point_rephasing_exact_identity():
+    """The ``base > 0`` branch of nested_wilson with a closing phase (R6, R9): a loop that starts at grid
+    index b wraps past the zone boundary, and the wrapped frames carry Phi_1.  Exact identity: with
+    D(k) = exp(i k r), H_pos(k_{i+b}) = C^dagger [D^dagger(k_i) H_per(k_{i+b}) D(k_i)] C, C = D(k_b)
+    constant, so the base-b loop of H_pos equals the base-0 loop of the position-gauge version of the
+    ROLLED periodic grid, first-level phases and nested phases alike (asymmetric positions, generic bands)."""
+    n, b = 14, 5
+    H = wl.config2_grid(n, n, gamma=0.7)
+    r1 = np.array([0.11, 0.37, -0.23, 0.41])
+    r2 = np.array([0.29, -0.13, 0.07, 0.33])
+    Hp, c1, c2 = wl.position_gauge_plane(H, r1, r2)
+    Hrolled, _, _ = wl.position_gauge_plane(H, r1, r2, shift1=b)
+    for band in (0, 1):
+        ta, na = wo.nested_wilson(Hp, 2, base=b, wb_lo=band, wb_hi=band + 1, close1=c1, close2=c2)
+        tb, nb = wo.nested_wilson(Hrolled, 2, base=0, wb_lo=band, wb_hi=band + 1, close1=c1, close2=c2)
+        assert max(wo.circ_sorted_distance(ta[j], tb[j]) for j in range(n)) < 1e-11
+        assert abs(wo.wrap_pi(na[0] - nb[0])) < 1e-10
+    # the identity is sharp: without the closing phase the base-b loop is a different object
+    tc, nc = wo.nested_wilson(Hp, 2, base=b, close2=c2)
+    assert max(wo.circ_sorted_distance(tc[j], tb[j]) for j in range(n)) > 1e-3
+
+
+def test_nested_theta_cut_relabels_the_wannier_bands():
+    """R9: Wannier bands are numbered by ascending phase on the branch (theta_cut - 2 pi, theta_cut].  The
+    two Wannier bands of the chiral HOTI slice (Eq. 9) sit at +-nu with 0 < nu < 1/2: with
+    the cut at pi band 0 is -nu, with the cut at 0 (branch (-2 pi, 0]) band 0 is +nu, and their nested
+    phases at generic k_z are +-theta, not equal -- so the cut is observable."""
+    Hz = wl.chiral_hoti_grid(16, 16, [0.1], 1.0)[0]
+    th1, n_pi_0 = wo.nested_wilson(Hz, 2, wb_lo=0, wb_hi=1, theta_cut=np.pi)
+    _, n_pi_1 = wo.nested_wilson(Hz, 2, wb_lo=1, wb_hi=2, theta_cut=np.pi)
+    _, n_0_0 = wo.nested_wilson(Hz, 2, wb_lo=0, wb_hi=1, theta_cut=0.0)
+    _, n_0_1 = wo.nested_wilson(Hz, 2, wb_lo=1, wb_hi=2, theta_cut=0.0)
+    assert np.all(th1[:, 0] < -0.05) and np.all(th1[:, 1] > 0.05)        # the premise: bands at -nu and +nu
+    assert abs(wo.wrap_pi(n_pi_0[0] - n_pi_1[0])) > 0.1                   # the two bands differ ...
+    assert abs(wo.wrap_pi(n_0_0[0] - n_pi_1[0])) < 1e-10                  # ... and the cut swaps their numbers
+    assert abs(wo.wrap_pi(n_0_1[0] - n_pi_0[0])) < 1e-10
+    # both bands together: the selected span is the whole occupied space for either cut
+    _, n_both_pi = wo.nested_wilson(Hz, 2, wb_lo=0, wb_hi=2, theta_cut=np.pi)
+    _, n_both_0 = wo.nested_wilson(Hz, 2, wb_lo=0, wb_hi=2, theta_cut=0.0)
+    assert wo.circ_sorted_distance(n_both_pi, n_both_0) < 1e-10
+
+
+def test_spin_resolved_uneven_split_and_dense_spin_operator():
+    """m_lo != m / 2 (R10) and the dense-S branch of projected_spin.  BHZ plus one
+    decoupled occupied spin-down orbital, n_occ = 3: the PSO spectrum is (-1, -1, +1), so the sectors have
+    the sizes 2 and 1.  Block reduction: the lower sector's phases are the union of the spin-down BHZ block's
+    loop and the Abelian loop of the extra orbital (a k-independent vector: phase 0), the upper sector is
+    the spin-up block; sector windings -+1.  The same model in a randomly rotated basis has
+    a dense Hermitian S and must give the same phases."""
+    n1, n2 = 40, 21
+    H = wl.bhz4_plus_band_grid(n1, n2)
+    S = wl.bhz4_plus_band_spin_z()
+    lo, hi, pso = wo.spin_resolved_surface(H[None], 3, 1, S, m_lo=2)
+    assert lo.shape == (n2, 2) and hi.shape == (n2, 1)
+    assert np.abs(pso[..., :2] + GOLD["pso_abs_eigenvalue_no_soc"]).max() < 1e-12 and np.abs(pso[..., 2] - 1).max() < 1e-12
+    up = [0, 2]; dn = [1, 3]
+    th_up, _, _ = wo.wilson_surface(H[None][..., up, :][..., :, up], 1, 1)
+    th_dn, _, _ = wo.wilson_surface(H[None][..., dn, :][..., :, dn], 1, 1)
+    for j in range(n2):
+        assert wo.circ_sorted_distance(hi[j], th_up[j]) < 1e-10
+        assert wo.circ_sorted_distance(lo[j], np.sort(np.array([th_dn[j, 0], 0.0]))) < 1e-10
+    assert abs(abs(wo.winding(lo)) - GOLD["bhz_sector_abs_winding"]) < 1e-9
+    assert abs(wo.winding(lo) + wo.winding(hi)) < 1e-9
+    # default split (m_lo = 1) cuts the degenerate pair of -1 eigenvalues: a different, ill-defined object
+    Hr, Sr = wl.rotated_basis(H, S)
+    assert np.abs(Sr - np.diag(np.diag(Sr))).max() > 0.1                     # S really is dense
+    lo_r, hi_r, pso_r = wo.spin_resolved_surface(Hr[None], 3, 1, Sr, m_lo=2)
+    assert np.abs(pso_r - pso).max() < 1e-11
+    for j in range(n2):
+        assert wo.circ_sorted_distance(lo_r[j], lo[j]) < 1e-10 and wo.circ_sorted_distance(hi_r[j], hi[j]) < 1e-10
+    # a transposed or conjugated S is a different operator in the rotated basis and breaks the +-1 spectrum
+    _, _, pso_t = wo.spin_resolved_surface(Hr[None][:, :2], 3, 1, Sr.T, m_lo=2)
+    assert np.abs(np.abs(pso_t) - 1).max() > 1e-3
+
+
 def test_nested_first_level_matches_plain_surface():
     H = wl.config2_grid(24, 20)
     th1, _ = wo.nested_wilson(H, 2)
