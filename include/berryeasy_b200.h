@@ -90,6 +90,12 @@ int be_set_chunk_pipeline(be_ctx* ctx, int on);
  * same input.  Returns BE_ERR_SHAPE for any other value. */
 int be_set_eigh_algorithm(be_ctx* ctx, int algo);
 
+/* FP64 peak probe (measurement aid for bench.py's roofline, not part of the path): runs a chain of
+ * which = 0: DMMA.8x8x4 (mma.sync.m8n8k4.f64), 1: DFMA with reused operands, 2: DFMA with three distinct
+ * register operands per instruction, on every SM of the context's device and stream, and writes the
+ * achieved rate in TFLOP/s to *tflops (host pointer).  Synchronises the stream; ~20 ms. */
+int be_probe_fp64(be_ctx* ctx, int which, double* tflops);
+
 /* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */
 int64_t be_launch_count(const be_ctx* ctx);
 

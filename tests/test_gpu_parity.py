@@ -338,12 +338,12 @@ def test_nested_closing_phases_base_and_cut_on_device(ctx):
     Hz = wl.chiral_hoti_grid(16, 16, [0.1], 1.0)
     for cut in (0.0, np.pi, -1.0):
         for band in (0, 1):
-            _, thn = ctx.nested_wilson(dev(Hz), 2, 2, 1, wb_lo=band, wb_hi=band + 1, theta_cut=cut)
+            _, thn = ctx.nested_wilson(dev(Hz), 2, 1, 0, wb_lo=band, wb_hi=band + 1, theta_cut=cut)
             _, thno = wo.nested_wilson(Hz[0], 2, wb_lo=band, wb_hi=band + 1, theta_cut=cut)
             assert wo.circ_sorted_distance(thn.cpu().numpy()[0], thno) / (2 * np.pi) <= PH_TOL
-    _, a = ctx.nested_wilson(dev(Hz), 2, 2, 1, wb_lo=0, wb_hi=1, theta_cut=0.0)
-    _, b = ctx.nested_wilson(dev(Hz), 2, 2, 1, wb_lo=1, wb_hi=2, theta_cut=np.pi)
-    _, c = ctx.nested_wilson(dev(Hz), 2, 2, 1, wb_lo=0, wb_hi=1, theta_cut=np.pi)
+    _, a = ctx.nested_wilson(dev(Hz), 2, 1, 0, wb_lo=0, wb_hi=1, theta_cut=0.0)
+    _, b = ctx.nested_wilson(dev(Hz), 2, 1, 0, wb_lo=1, wb_hi=2, theta_cut=np.pi)
+    _, c = ctx.nested_wilson(dev(Hz), 2, 1, 0, wb_lo=0, wb_hi=1, theta_cut=np.pi)
     assert abs(wo.wrap_pi(a.cpu().numpy()[0, 0] - b.cpu().numpy()[0, 0])) < 1e-8
     assert abs(wo.wrap_pi(a.cpu().numpy()[0, 0] - c.cpu().numpy()[0, 0])) > 0.1
 
