@@ -124,7 +124,7 @@ class Workload:
         if self.kind == "spin_resolved":
             return ctx.spin_resolved_wilson_host(Hh, self.m, Hh.dim() - 4, Sh)
         if self.kind == "nested":
-            return None
+            return ctx.nested_wilson_host(Hh, self.m, 1, 0)
         return ctx.wilson_loop_host(Hh, self.m, Hh.dim() - 4)
 
     # bounded oracle sample: whole loops of the same matrices
@@ -393,7 +393,7 @@ def main():
 
     # ---- end to end through the host-buffer C-ABI call (H2D of the grid inside the timed region)
     e2e = None
-    if not args.no_e2e and wk.kind != "nested":
+    if not args.no_e2e:
         Hh = torch.empty(H.shape, dtype=H.dtype).pin_memory()
         Hh.copy_(H)
         Sh = S.cpu() if S is not None else None

@@ -64,9 +64,9 @@ const char* be_strerror(int code);
  * 0 = eigh, 1 = wilson loop, 2 = nested, 3 = spin resolved). */
 size_t be_workspace_bytes(const be_grid* grid, int n_occ, int op);
 
-/* Cap on the scratch used for per-chunk work buffers (default: 65 % of the device memory, 119 GB on a
- * B200; the caller's own buffers have to fit beside it).  Work is processed in chunks of whole loops
- * sized to stay under the cap. */
+/* Cap on the scratch used for per-chunk work buffers (default: 70 % of the device memory, 134 GB on a
+ * B200).  Work is processed in chunks of whole loops sized to stay under the cap and under what the device
+ * has free when the call is made (free memory + the scratch the context already holds - 2 GiB). */
 int be_set_workspace_limit(be_ctx* ctx, size_t bytes);
 
 /* Two-stream chunk pipeline for be_wilson_loop / be_spin_resolved_wilson when the work is split
@@ -268,8 +268,11 @@ int be_plaquette_flux(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int
 /*
  * Host-buffer variants (end-to-end path): h* pointers are host memory (pinned recommended).  The
  * grid is streamed to the device in chunks of whole loops, overlapped with compute on an internal
- * copy stream; results are copied back before return.  Semantics as the device calls above.
- * Requires dir == ndim-1 (loops contiguous in memory), else BE_ERR_UNSUPPORTED.
+ * copy stream (growing chunks: 1/8 of the loops, 1/4, then what the workspace cap allows, so that only
+ * the first, small copy is exposed); results are copied back before return.  Semantics as the device
+ * calls above; any loop direction (dir == ndim-1: one contiguous copy per chunk, else one strided copy
+ * per loop).  The two staging buffers are kept in the context between calls.  be_nested_wilson_host
+ * copies the whole grid in one piece (both levels need the whole plane).
  */
 int be_wilson_loop_host(be_ctx* ctx, const void* hH_grid, const be_grid* grid, int n_occ, int dir,
                         const void* h_close, double* h_theta, double* h_abs, double* h_mingap);
@@ -277,6 +280,9 @@ int be_spin_resolved_wilson_host(be_ctx* ctx, const void* hH_grid, const be_grid
                                  int dir, const void* hS, int S_is_diag, int m_lo,
                                  const void* h_close, double* h_theta_lo, double* h_theta_hi,
                                  double* h_pso);
+int be_nested_wilson_host(be_ctx* ctx, const void* hH_grid, const be_grid* grid, int n_occ, int dir1, int dir2,
+                          int base, int wb_lo, int wb_hi, double theta_cut, const void* h_close1,
+                          const void* h_close2, double* h_theta1, double* h_theta_nested);
 
 #ifdef __cplusplus
 }

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libberryeasy_b200.so")
 EXPORTS = [
     "be_create", "be_destroy", "be_strerror", "be_workspace_bytes", "be_set_workspace_limit",
     "be_launch_count", "be_eigh_batched", "be_wilson_loop", "be_nested_wilson",
-    "be_spin_resolved_wilson", "be_winding", "be_wilson_loop_host", "be_spin_resolved_wilson_host",
+    "be_spin_resolved_wilson", "be_winding", "be_wilson_loop_host", "be_spin_resolved_wilson_host", "be_nested_wilson_host",
     "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched", "be_set_chunk_pipeline", "be_set_eigh_algorithm", "be_probe_fp64", "be_bloch_coefficients", "be_assemble_bloch", "be_plaquette_flux", "be_wilson_loop_bloch",
     "be_spin_resolved_wilson_bloch", "be_wilson_loop_window", "be_spin_resolved_wilson_window",
 ]
@@ -67,6 +67,7 @@ def load_library():
     lib.be_winding.argtypes = [vp, vp, i64, ci, ci, vp]
     lib.be_wilson_loop_host.argtypes = [vp, vp, gp, ci, ci, vp, vp, vp, vp]
     lib.be_spin_resolved_wilson_host.argtypes = [vp, vp, gp, ci, ci, vp, ci, ci, vp, vp, vp, vp]
+    lib.be_nested_wilson_host.argtypes = [vp, vp, gp, ci, ci, ci, ci, ci, ci, dbl, vp, vp, vp, vp]
     lib.be_zgemm_batched.argtypes = [vp, ci, ci, ci, ci, ci, C.POINTER(dbl), vp, ci, i64, vp, ci, i64,
                                      C.POINTER(dbl), vp, ci, i64, i64, ci]
     lib.be_profile_enable.argtypes = [vp, ci]
@@ -451,3 +452,22 @@ class Context:
                                                                direction, _ptr(S), is_diag, m_lo, _ptr(close),
                                                                _ptr(lo), _ptr(hi), _ptr(pso)))
         return lo, hi, pso
+
+    def nested_wilson_host(self, H_grid, n_occ, dir1, dir2, base=0, wb_lo=0, wb_hi=1, theta_cut=None,
+                           close1=None, close2=None):
+        import math
+        _host(H_grid, torch.complex128, "H_grid")
+        nd = H_grid.dim() - 3
+        g = _grid_of(H_grid, nd)
+        outer = H_grid.shape[0]
+        for a in range(nd):
+            if a not in (dir1, dir2):
+                outer *= H_grid.shape[1 + a]
+        n2 = H_grid.shape[1 + dir2]
+        th1 = torch.empty((outer, n2, n_occ), dtype=torch.float64).pin_memory()
+        thn = torch.empty((outer, wb_hi - wb_lo), dtype=torch.float64).pin_memory()
+        cut = math.pi if theta_cut is None else float(theta_cut)
+        _check(self.lib, self.lib.be_nested_wilson_host(self._h, _ptr(H_grid), C.byref(g), n_occ, dir1, dir2, base,
+                                                        wb_lo, wb_hi, cut, _ptr(close1), _ptr(close2),
+                                                        _ptr(th1), _ptr(thn)))
+        return th1, thn

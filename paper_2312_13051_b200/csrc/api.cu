@@ -94,6 +94,17 @@ int be_arena_reserve(be_ctx* ctx, size_t bytes) {
   return BE_OK;
 }
 
+// The cap that applies to a call: the configured limit, but never more than what the device can give right now
+// (free memory plus the arena already held, minus a margin for the caller's outputs and the CUDA context).
+size_t be_effective_ws_limit(be_ctx* ctx) {
+  size_t fr = 0, tot = 0;
+  if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) { cudaGetLastError(); return ctx->ws_limit; }
+  const size_t margin = (size_t)2 << 30;
+  size_t avail = fr + ctx->arena_bytes;
+  avail = avail > margin ? avail - margin : avail / 2;
+  return ctx->ws_limit < avail ? ctx->ws_limit : avail;
+}
+
 void* be_arena_alloc(be_ctx* ctx, size_t bytes) {
   const size_t b = be_align256(bytes ? bytes : 1);
   if (ctx->arena_used + b > ctx->arena_bytes) return nullptr;
@@ -115,9 +126,9 @@ extern "C" int be_create(be_ctx** out, void* cuda_stream) {
   e = cudaGetDeviceProperties(&prop, c->device);
   if (e != cudaSuccess) { delete c; return (int)e; }
   c->sm_count = prop.multiProcessorCount;
-  // scratch cap: 65 % of the device memory (119 GB on a B200).  Larger chunks fill the one-CTA-per-matrix kernels'
+  // scratch cap: 70 % of the device memory (134 GB on a B200).  Larger chunks fill the one-CTA-per-matrix kernels'
   // waves better (600 matrices in one chunk instead of 2 x 300: 2481 vs 2561 ms on the bench workload)
-  c->ws_limit = (size_t)(0.65 * (double)prop.totalGlobalMem);
+  c->ws_limit = (size_t)(0.70 * (double)prop.totalGlobalMem);
   if (c->ws_limit < ((size_t)4 << 30)) c->ws_limit = (size_t)4 << 30;
   c->eigh_algo = 2;
   *out = c;
@@ -130,6 +141,7 @@ extern "C" int be_destroy(be_ctx* ctx) {
   if (ctx->arena) cudaFree(ctx->arena);
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
   if (ctx->dR_buf) cudaFree(ctx->dR_buf);
+  for (int i = 0; i < 2; ++i) if (ctx->stage_buf[i]) cudaFree(ctx->stage_buf[i]);
   if (ctx->stream2) {
     cudaStreamDestroy(ctx->stream2);
     cudaEventDestroy(ctx->ev_split); cudaEventDestroy(ctx->ev_join);
@@ -242,7 +254,7 @@ extern "C" int be_eigh_batched(be_ctx* ctx, const void* dH, int64_t count, int N
   if (count == 0) return BE_OK;
   const int nv = dU ? n_vec : 0;
   const size_t per = be_eigh_scratch_bytes(1, N, nv) + (size_t)N * (nv > 0 ? nv : 1) * sizeof(cplx) + 1024;
-  int64_t chunk = (int64_t)(ctx->ws_limit / per);
+  int64_t chunk = (int64_t)(be_effective_ws_limit(ctx) / per);
   if (chunk < 1) chunk = 1;
   if (chunk > count) chunk = count;
   const int64_t nchunks = (count + chunk - 1) / chunk;

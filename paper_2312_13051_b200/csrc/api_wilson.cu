@@ -109,11 +109,41 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   const int n1 = map.n1;
   const int64_t loops = map.loops;
   const size_t per = per_loop_bytes(N, m, n1, sp != nullptr, ctx->band_lo);
-  int64_t lc = (int64_t)(ctx->ws_limit / per);
+  size_t ws = be_effective_ws_limit(ctx);
+  if (hs) {
+    // the two staging buffers of a host grid come out of the same budget (2 x loop_bytes per loop of a chunk)
+    const size_t held = 2 * ctx->stage_cap;
+    ws = (size_t)((double)(ws + held) * (double)per / (double)(per + 2 * hs->loop_bytes));
+  }
+  int64_t lc = (int64_t)(ws / per);
   if (lc < 1) lc = 1;
   if (lc > loops) lc = loops;
-  const int64_t nchunks = (loops + lc - 1) / lc;
-  lc = (loops + nchunks - 1) / nchunks;
+  // Chunk boundaries.  Device grid: equal chunks of at most lc loops.  Host grid: the first copy cannot overlap
+  // anything, so the chunks grow -- 1/8 of the loops, then 1/4, then what the cap allows -- and every later
+  // copy hides behind the (longer) computation of the chunk before it.
+  std::vector<int64_t> cstart;
+  if (!hs) {
+    const int64_t nch = (loops + lc - 1) / lc;
+    lc = (loops + nch - 1) / nch;
+    for (int64_t l0 = 0; l0 < loops; l0 += lc) cstart.push_back(l0);
+  } else {
+    int64_t l0 = 0, step = (loops + 7) / 8;
+    while (l0 < loops) {
+      cstart.push_back(l0);
+      int64_t c = step < lc ? step : lc;
+      if (loops - l0 - c > 0 && loops - l0 - c < c / 2) c = loops - l0;   // no tiny last chunk
+      if (c > lc) c = lc;
+      l0 += c;
+      step *= 2;
+    }
+    lc = 0;
+    for (size_t i = 0; i < cstart.size(); ++i) {
+      const int64_t e = (i + 1 < cstart.size()) ? cstart[i + 1] : loops;
+      if (e - cstart[i] > lc) lc = e - cstart[i];
+    }
+  }
+  cstart.push_back(loops);
+  const int64_t nchunks = (int64_t)cstart.size() - 1;
   const int mlo = sp ? sp->m_lo : 0, mhi = sp ? m - sp->m_lo : 0;
   // The Wilson matrices of ALL loops outlive the chunks: their eigenphase solve (S4) is a
   // latency-bound kernel with one CTA per matrix, so it runs once over every loop at the end
@@ -127,20 +157,40 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   // tridiagonalization of chunk c+1 on the caller's stream overlaps the rest of chunk c on stream2.
   const size_t region = be_align256(per * (size_t)lc);
   bool pipe = nchunks > 1 && ctx->chunk_pipeline && !hs;
-  // host-resident grid: staging buffers for lc loops each, next to the work arena
+  // host-resident grid: two staging buffers (kept in the context between calls) next to the work arena
   GridMap smap;
   auto issue_copy = [&](int64_t ci) -> int {
     const int b = (int)(ci & 1);
-    const int64_t c0 = ci * lc, cn = (loops - c0 < lc) ? loops - c0 : lc;
+    const int64_t c0 = cstart[ci], cn = cstart[ci + 1] - c0;
     if (ci >= 2) BE_CUDA(cudaStreamWaitEvent(ctx->copy_stream, hs->freed[b], 0));
-    BE_CUDA(cudaMemcpyAsync(hs->stage[b], hs->hH + (size_t)c0 * hs->loop_bytes, (size_t)cn * hs->loop_bytes,
-                            cudaMemcpyHostToDevice, ctx->copy_stream));
+    const GridMap& hm = hs->hmap;
+    if (hm.dir == hm.ndim - 1) {
+      // loops are contiguous in the host grid, and so are consecutive loops: one copy per chunk
+      BE_CUDA(cudaMemcpyAsync(hs->stage[b], hs->hH + (size_t)c0 * hs->loop_bytes, (size_t)cn * hs->loop_bytes,
+                              cudaMemcpyHostToDevice, ctx->copy_stream));
+    } else {
+      // a loop is n1 matrices a fixed stride apart: one strided copy per loop
+      for (int64_t l = 0; l < cn; ++l) {
+        const int64_t src = gridmap_index(hm, c0 + l, 0);
+        BE_CUDA(cudaMemcpy2DAsync((char*)hs->stage[b] + (size_t)l * hs->loop_bytes, hs->mat_bytes,
+                                  hs->hH + (size_t)src * hs->mat_bytes, (size_t)hm.stride[hm.dir] * hs->mat_bytes,
+                                  hs->mat_bytes, (size_t)n1, cudaMemcpyHostToDevice, ctx->copy_stream));
+      }
+    }
     BE_CUDA(cudaEventRecord(hs->copied[b], ctx->copy_stream));
     return BE_OK;
   };
   if (hs) {
-    for (int b = 0; b < (nchunks > 1 ? 2 : 1); ++b)
-      if (cudaMalloc(&hs->stage[b], (size_t)lc * hs->loop_bytes) != cudaSuccess) { cudaGetLastError(); return BE_ERR_NOMEM; }
+    const size_t need = (size_t)lc * hs->loop_bytes;
+    if (need > ctx->stage_cap) {
+      BE_CUDA(cudaStreamSynchronize(ctx->stream));
+      for (int b = 0; b < 2; ++b) { if (ctx->stage_buf[b]) cudaFree(ctx->stage_buf[b]); ctx->stage_buf[b] = nullptr; }
+      ctx->stage_cap = 0;
+      for (int b = 0; b < 2; ++b)
+        if (cudaMalloc(&ctx->stage_buf[b], need) != cudaSuccess) { cudaGetLastError(); return BE_ERR_NOMEM; }
+      ctx->stage_cap = need;
+    }
+    hs->stage[0] = ctx->stage_buf[0]; hs->stage[1] = ctx->stage_buf[1];
     memset(&smap, 0, sizeof(smap));
     smap.ndim = 1; smap.dir = 0; smap.n1 = n1; smap.dims[0] = n1; smap.stride[0] = 1; smap.batch_stride = n1; smap.loops = lc;
     BE_TRY(issue_copy(0));
@@ -166,16 +216,15 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
       }
   }
   const size_t keep = ctx->arena_used;
-  for (int64_t l0 = 0; l0 < loops; l0 += lc) {
-    const int64_t nl = (loops - l0 < lc) ? loops - l0 : lc;
+  for (int64_t ci = 0; ci < nchunks; ++ci) {
+    const int64_t l0 = cstart[ci], nl = cstart[ci + 1] - l0;
     const int64_t cnt = nl * n1;
-    const int64_t ci = l0 / lc;
     ctx->arena_used = keep + (pipe ? (size_t)(ci & 1) * region : 0);
     if (pipe) {
       ctx->stream = S1;
       if (ci >= 2) BE_CUDA(cudaStreamWaitEvent(S1, ctx->ev_region[ci & 1], 0));   // region free again
       ctx->split_after_tridiag = 1;
-      ctx->gemm_pad = (l0 + lc < loops && N > 8) ? 1 : 0;   // a next chunk will stream its matrices next to these GEMMs
+      ctx->gemm_pad = (ci + 1 < nchunks && N > 8) ? 1 : 0;   // a next chunk will stream its matrices next to these GEMMs
     }
     const cplx* Hc = H;
     if (hs) {
@@ -379,7 +428,7 @@ extern "C" int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid*
                      + (size_t)n1 * m * m * 16 + 8 * (size_t)m * m * 16 + 4096
                      + (m > 2 ? be_nested_general_scratch_bytes(1, m, ns) + be_eigenphases_scratch_bytes(1, m) : 0);
   const size_t persist = (size_t)loops * ((size_t)N * ns * 16 + 256) + (size_t)outer2 * (n2 + 4) * ns * ns * 16 + (8 << 20);
-  int64_t lc = (int64_t)(ctx->ws_limit / per);
+  int64_t lc = (int64_t)(be_effective_ws_limit(ctx) / per);
   if (lc < 1) lc = 1;
   if (lc > loops) lc = loops;
   BE_TRY(be_arena_reserve(ctx, per * (size_t)lc + persist + (size_t)loops * m * 8 + (4 << 20)));
@@ -466,7 +515,7 @@ extern "C" int be_plaquette_flux(be_ctx* ctx, const void* dH_grid, const be_grid
   const size_t need = (size_t)cnt * (be_eigh_scratch_bytes(1, N, m) + 2 * (size_t)N * m * sizeof(cplx) + N * sizeof(double) +
                                      (dS ? (size_t)N * m * sizeof(cplx) + 3 * mmax + be_eigh_scratch_bytes(1, m, m) : 0) +
                                      6 * mmax + 4096) + (8 << 20);
-  if (need > ctx->ws_limit) return BE_ERR_UNSUPPORTED;   // the grid has to fit one chunk (header)
+  if (need > be_effective_ws_limit(ctx)) return BE_ERR_UNSUPPORTED;   // the grid has to fit one chunk (header)
   BE_TRY(be_arena_reserve(ctx, need));
   double* E = (double*)be_arena_alloc(ctx, (size_t)cnt * N * sizeof(double));
   cplx* X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
@@ -494,9 +543,13 @@ extern "C" int be_plaquette_flux(be_ctx* ctx, const void* dH_grid, const be_grid
 }
 
 // host-resident grid (api_host.cu): same chunking, deferred eigenphases and scratch as the device path
-int be_wilson_host_device(be_ctx* ctx, HostStage* hs, int64_t loops, int n1, int N, int m, const void* d_close,
+int be_wilson_host_device(be_ctx* ctx, HostStage* hs, const be_grid* grid, int dir, int m, const void* d_close,
                           double* d_theta, double* d_abs, double* d_mingap, const void* dS, int S_is_diag, int m_lo,
                           double* d_theta_lo, double* d_theta_hi, double* d_pso, int spin) {
+  BE_TRY(make_map(grid, dir, &hs->hmap));
+  const int n1 = hs->hmap.n1, N = grid->N;
+  const int64_t loops = hs->hmap.loops;
+  // inside a staged chunk the loops are contiguous whatever the direction in the host grid was
   GridMap map;
   memset(&map, 0, sizeof(map));
   map.ndim = 1; map.dir = 0; map.n1 = n1; map.dims[0] = n1; map.stride[0] = 1; map.batch_stride = n1; map.loops = loops;

@@ -95,6 +95,8 @@ struct be_ctx {
   int gemm_pad;               // zgemm launches with padded shared memory: at most one GEMM CTA per SM,
                               // leaving room for one k_hemv CTA of the other stream
   struct be_prof* prof;       // optional per-kernel-class CUDA-event timing (be_profile_enable)
+  void* stage_buf[2];         // host variants: device staging buffers, kept between calls
+  size_t stage_cap;
   int eigh_algo;              // be_set_eigh_algorithm: 0 one-stage tridiagonalization, 1 two-stage (band) where supported
 };
 
@@ -109,7 +111,8 @@ void be_prof_end(be_ctx* ctx, int cls, double bytes, double flops);
 
 // bump allocator on the context arena; pointers stay valid until arena_reset
 int  be_arena_reserve(be_ctx* ctx, size_t bytes);   // ensure capacity (may sync + realloc); resets
-void* be_arena_alloc(be_ctx* ctx, size_t bytes);    // 256-byte aligned; NULL when exhausted
+void* be_arena_alloc(be_ctx* ctx, size_t bytes);
+size_t be_effective_ws_limit(be_ctx* ctx);          // min(configured cap, what the device can give now)    // 256-byte aligned; NULL when exhausted
 static inline size_t be_align256(size_t b) { return (b + 255) & ~(size_t)255; }
 
 // ---------------------------------------------------------------------------------------------
@@ -189,10 +192,12 @@ int be_bloch_assemble_chunk(be_ctx* ctx, const BlochSrc* bs, int64_t loop0, int6
 struct HostStage {
   const char* hH;          // host grid
   size_t loop_bytes;       // n1 * N * N * 16
-  void* stage[2];          // device staging buffers, lc loops each (filled by be_wilson_host_device)
+  size_t mat_bytes;        // N * N * 16
+  GridMap hmap;            // (loop, j) -> matrix index inside the host grid (any loop direction)
+  void* stage[2];          // device staging buffers (cached in the context), the largest chunk each
   cudaEvent_t copied[2], freed[2];
 };
-int be_wilson_host_device(be_ctx* ctx, HostStage* hs, int64_t loops, int n1, int N, int m, const void* d_close,
+int be_wilson_host_device(be_ctx* ctx, HostStage* hs, const be_grid* grid, int dir, int m, const void* d_close,
                           double* d_theta, double* d_abs, double* d_mingap, const void* dS, int S_is_diag, int m_lo,
                           double* d_theta_lo, double* d_theta_hi, double* d_pso, int spin);
 

@@ -519,7 +519,7 @@ def test_host_variants_match_device(ctx):
         lo, hi, pso = ctx.spin_resolved_wilson_host(Hh, 32, 1, torch.from_numpy(S))
         th, ab, mg = ctx.wilson_loop_host(Hh, 32, 1)
     finally:
-        ctx.set_workspace_limit(64 << 30)
+        ctx.set_workspace_limit(110 << 30)
     lod, hid, psod = ctx.spin_resolved_wilson(dev(H), 32, 1, dev(S))
     thd, abd, mgd = ctx.wilson_loop(dev(H), 32, 1)
     # chunking changes the seeded start vectors of the inverse iteration (matrix index inside the
@@ -529,6 +529,24 @@ def test_host_variants_match_device(ctx):
     assert phase_dist(th.numpy(), thd.cpu().numpy()) < 1e-12 and (mg - mgd.cpu()).abs().max() < 1e-12
     tho, _, _ = wo.wilson_surface(H, 32, 1)
     assert phase_dist(th.numpy(), tho) <= PH_TOL
+    # default workspace cap: the host variants still stream the grid in growing chunks (1/8, 1/4, rest)
+    th2, _, _ = ctx.wilson_loop_host(Hh, 32, 1)
+    assert phase_dist(th2.numpy(), tho) <= PH_TOL
+    # loops along the slow grid axis: not contiguous in the host grid (one strided copy per loop)
+    th0, _, mg0 = ctx.wilson_loop_host(Hh, 32, 0)
+    th0o, _, mg0o = wo.wilson_surface(H, 32, 0)
+    assert phase_dist(th0.numpy(), th0o) <= PH_TOL and np.abs(mg0.numpy() - mg0o).max() < 1e-10
+    lo0, hi0, _ = ctx.spin_resolved_wilson_host(Hh, 32, 0, torch.from_numpy(S))
+    lo0o, hi0o, _ = wo.spin_resolved_surface(H, 32, 0, S)
+    assert phase_dist(lo0.numpy(), lo0o) <= PH_TOL and phase_dist(hi0.numpy(), hi0o) <= PH_TOL
+    # nested loop on a host grid, with closing phases and a base point
+    Hb = wl.config2_grid(14, 12, gamma=0.7)
+    Hp, c1, c2 = wl.position_gauge_plane(Hb, np.array([0.11, 0.37, -0.23, 0.41]), np.array([0.29, -0.13, 0.07, 0.33]))
+    t1, tn = ctx.nested_wilson_host(torch.from_numpy(Hp[None]).pin_memory(), 2, 1, 0, base=3, wb_lo=1, wb_hi=2,
+                                    close1=torch.from_numpy(c1), close2=torch.from_numpy(c2))
+    t1o, tno = wo.nested_wilson(Hp, 2, base=3, wb_lo=1, wb_hi=2, close1=c1, close2=c2)
+    assert phase_dist(t1.numpy()[0], t1o) <= PH_TOL
+    assert wo.circ_sorted_distance(tn.numpy()[0], tno) / (2 * np.pi) <= PH_TOL
 
 
 def test_chunk_pipeline_matches_single_chunk_and_oracle(ctx):
