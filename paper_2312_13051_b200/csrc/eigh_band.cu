@@ -583,7 +583,8 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
 
   // ------------------------------- consumers
   const int lane = tid & 31, w = tid >> 5, g = lane >> 2, q = lane & 3;
-  double z0r[2] = {0.0, 0.0}, z0i[2] = {0.0, 0.0}, z1r[2] = {0.0, 0.0}, z1i[2] = {0.0, 0.0};   // column part (two chains)
+  // column part of the item in 3-product form (two chains each)
+  double zs1[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, zs2[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, zs3[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
   int jb = 1;
   cplx Lw[2], Lv[2];          // fragments of [W- V-] rows of the tile, k = 2q, 2q+1
   int Lfor = -1;              // tile number these fragments were fetched for
@@ -652,30 +653,35 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
         }
       }
     }
-    // step 3: Y_I[8w+g][n] += sum_col A[.][col] V+_J[col][n]; k index q <-> column 8nb + 2q + j
+    // step 3: Y_I[8w+g][n] += sum_col A[.][col] V+_J[col][n]; k index q <-> column 8nb + 2q + j.  Three real
+    // products per complex one (Karatsuba): P1 = ar br, P2 = ai bi, P3 = (ar + ai)(br + bi); Re = P1 - P2,
+    // Im = P3 - P1 - P2 -- the operand sums cost one DADD each, a quarter of the DMMAs is saved.
     {
-      double yr[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, yi[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+      double y1[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, y2[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, y3[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
       for (int nb = 0; nb < 8; ++nb)
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
           const cplx b = VpJ[g * LDR + 8 * nb + 2 * q + j];
           const int ch = nb & 1;
-          dmma(yr[ch][0], yr[ch][1], ar[nb][j], b.x);
-          dmma(yr[ch][0], yr[ch][1], -ai[nb][j], b.y);
-          dmma(yi[ch][0], yi[ch][1], ar[nb][j], b.y);
-          dmma(yi[ch][0], yi[ch][1], ai[nb][j], b.x);
+          dmma(y1[ch][0], y1[ch][1], ar[nb][j], b.x);
+          dmma(y2[ch][0], y2[ch][1], ai[nb][j], b.y);
+          dmma(y3[ch][0], y3[ch][1], ar[nb][j] + ai[nb][j], b.x + b.y);
         }
       cplx* pr = P + ((int64_t)c * nT + J) * KB * Np + PIX(2 * q, rI);
-      pr[0] = mkc(yr[0][0] + yr[1][0], yi[0][0] + yi[1][0]);
-      pr[Np] = mkc(yr[0][1] + yr[1][1], yi[0][1] + yi[1][1]);
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const double p1 = y1[0][e] + y1[1][e], p2 = y2[0][e] + y2[1][e], p3 = y3[0][e] + y3[1][e];
+        pr[(int64_t)e * Np] = mkc(p1 - p2, p3 - p1 - p2);
+      }
     }
     if (has_upd) {
       // every warp's part of the updated tile is in shared memory: release the bulk store, start step 4
       asm volatile("bar.sync 1, 256;" ::: "memory");
       if (tid == 0) mbar_arrive(&stready[s]);
     }
-    // step 4: Z[m][col] += sum_row conj(V+_I[row][m]) A[row][col], col = 8w + n;  Y_J[col][m] = conj(Z[m][col])
+    // step 4: Z[m][col] += sum_row conj(V+_I[row][m]) A[row][col], col = 8w + n;  Y_J[col][m] = conj(Z[m][col]).
+    // Karatsuba again: S1 = sum vr br, S2 = sum vi bi, S3 = sum (vr - vi)(br + bi); Re Z = S1 + S2, Im Z = S3 - S1 + S2
     if (I != J) {
 #pragma unroll
       for (int blk = 0; blk < 8; ++blk)
@@ -684,13 +690,10 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
           const int row = 8 * blk + 2 * q + j;
           const cplx v = vpi[g * LDR + row];
           const cplx b = at[(8 * w + g) * LDT + row];
-          if (blk & 1) {
-            dmma(z1r[0], z1r[1], v.x, b.x); dmma(z1r[0], z1r[1], v.y, b.y);
-            dmma(z1i[0], z1i[1], v.x, b.y); dmma(z1i[0], z1i[1], -v.y, b.x);
-          } else {
-            dmma(z0r[0], z0r[1], v.x, b.x); dmma(z0r[0], z0r[1], v.y, b.y);
-            dmma(z0i[0], z0i[1], v.x, b.y); dmma(z0i[0], z0i[1], -v.y, b.x);
-          }
+          const int ch = blk & 1;
+          dmma(zs1[ch][0], zs1[ch][1], v.x, b.x);
+          dmma(zs2[ch][0], zs2[ch][1], v.y, b.y);
+          dmma(zs3[ch][0], zs3[ch][1], v.x - v.y, b.x + b.y);
         }
     }
     __syncwarp();
@@ -700,8 +703,9 @@ k_fused(cplx* __restrict__ Bw, const cplx* __restrict__ Vnew, const cplx* __rest
 #pragma unroll
       for (int j = 0; j < 2; ++j) {
         const int col = J * TS + 8 * w + 2 * q + j;
-        Zc[(int64_t)c * KB * Np + PIX(g, col)] = mkc(z0r[j] + z1r[j], -(z0i[j] + z1i[j]));
-        z0r[j] = z0i[j] = z1r[j] = z1i[j] = 0.0;
+        const double s1 = zs1[0][j] + zs1[1][j], s2 = zs2[0][j] + zs2[1][j], s3 = zs3[0][j] + zs3[1][j];
+        Zc[(int64_t)c * KB * Np + PIX(g, col)] = mkc(s1 + s2, -((s3 - s1) + s2));
+        zs1[0][j] = zs1[1][j] = zs2[0][j] = zs2[1][j] = zs3[0][j] = zs3[1][j] = 0.0;
       }
     }
   }
@@ -989,8 +993,21 @@ __global__ void __launch_bounds__(QS * Q2_TSG_MAX, 1) k_q2(const cplx* __restric
         }
         const cplx t = cmulc(tau, cadd(d0, d1));   // conj(tau) * dot
         wnd[s] = csub(wnd[s], t);
+        // x_j -= t conj(v_j), all products with t.x first, then all with t.y: consecutive DFMAs share an operand
+        // (register-file bandwidth, not the FP64 pipe, limits three-operand DFMA streams on this part)
+        cplx vj[KB];
 #pragma unroll
-        for (int jj = 1; jj < KB; ++jj) cfms(wnd[s + jj], t, cconj(vb[s * KB + jj]));
+        for (int jj = 1; jj < KB; ++jj) vj[jj] = vb[s * KB + jj];
+#pragma unroll
+        for (int jj = 1; jj < KB; ++jj) {
+          wnd[s + jj].x = fma(-t.x, vj[jj].x, wnd[s + jj].x);
+          wnd[s + jj].y = fma(t.x, vj[jj].y, wnd[s + jj].y);
+        }
+#pragma unroll
+        for (int jj = 1; jj < KB; ++jj) {
+          wnd[s + jj].x = fma(-t.y, vj[jj].y, wnd[s + jj].x);
+          wnd[s + jj].y = fma(-t.y, vj[jj].x, wnd[s + jj].y);
+        }
       }
       // rows u < KB are final for this stage
       if (j == QS - 1) {
