@@ -4,9 +4,10 @@
 // reduction caps the total).
 //
 //   stage 1  dense -> band of width KB = 8:  B = Q1 A_band Q1^H.  Per panel of KB columns
-//              k_panel : one CTA per matrix -- finish W of the previous panel from the partial products,
-//                        bring the next KB columns up to date, Householder QR of the part below the band
-//                        (one block reduction per column), explicit V panel for the streaming kernel
+//              k_ysum, k_wupd : wide kernels -- sum the partial products of the previous panel (Y = A V), finish
+//                        W = Y T - V C and bring the next KB columns up to date
+//              k_panel : one CTA per matrix -- Householder QR of those columns below the band (one block
+//                        reduction per column), explicit V panel for the streaming kernel
 //              k_fused : ONE streaming pass over the trailing matrix per panel: every 64 x 64 tile is read
 //                        once (TMA bulk copies), gets the pending rank-2KB update of the previous panel
 //                        A -= W V^H + V W^H on the FP64 tensor cores, is written back (bulk store), and is
@@ -125,8 +126,7 @@ __device__ __forceinline__ void block_sum8(const cplx (&part)[KB], cplx* red, cp
 #define PIX(q, r) ((int64_t)(q) * Np + (r))
 
 // Y = A V of panel p-1 from the partial products of k_fused (row parts per block column J <= I, column part
-// Zc), one CTA per (row tile I, matrix); thread = (row, q).  Y goes to the W array (k_panel turns it into W
-// in place).  Also the tile's share of M = V^H Y, summed by k_panel.
+// Zc), one CTA per (row tile I, matrix); thread = (row, q).  Also the tile's share of M = V^H Y, summed by k_wupd.
 __global__ void __launch_bounds__(512) k_ysum(const cplx* __restrict__ P, const cplx* __restrict__ Zc,
                                               const cplx* __restrict__ Vprev, cplx* __restrict__ Wx, cplx* __restrict__ Mpart,
                                               int N, int Np, int nT, int J0, int jprev) {
@@ -168,22 +168,119 @@ __global__ void __launch_bounds__(512) k_ysum(const cplx* __restrict__ P, const 
   }
 }
 
-// Panel step p of the band reduction, one CTA per matrix (thread t owns the rows p KB + t + s PT).
-//   p > 0 : W_{p-1} = Y T - V (1/2 T^H (V^H Y) T)  (Y, M = V^H Y from k_ysum);
-//           columns p KB .. p KB + KB - 1 receive the pending update  -= W V^H + V W^H
-//   do_qr : Householder QR of those columns below row j2 = (p + 1) KB: reflectors stored in place (R on and
-//           above the sub-band diagonal), explicit V (unit heads, zeros above) for k_fused, tau, T
-//   !do_qr: the trailing block (at most KB + 1 columns) only receives the update -- end of stage 1.
-// The panel stays on chip during the QR: row slot 0 of every thread in registers, the slots s >= 1 in
-// shared memory ([slot][column][thread]: conflict free).
+// Per-matrix scalars of a panel step (p > 0), one small CTA per matrix: M = sum of the tiles' shares of V^H Y,
+// C = 1/2 T^H M T, and the top KB + 1 rows of V and of W = Y T - V C (every row of the column update needs them).
+// Layout of MC [cnt][64 + 2 * 72]: C, Vtop [9][8], Wtop [9][8].
+constexpr int MC_STRIDE = 64 + 2 * (KB + 1) * KB;
+__global__ void __launch_bounds__(96) k_mc(const cplx* __restrict__ Yx, const cplx* __restrict__ Vprev,
+                                           const cplx* __restrict__ Mpart, const cplx* __restrict__ T1,
+                                           cplx* __restrict__ MC, int N, int Np, int nT, int J0, int jprev) {
+  __shared__ cplx Ts[KB * KB], Cs[KB * KB], Mf[64], Yt[(KB + 1) * KB], Vt[(KB + 1) * KB];
+  const int64_t c = blockIdx.x;
+  const int tid = threadIdx.x;
+  const cplx* __restrict__ Y = Yx + c * KB * (int64_t)Np;
+  const cplx* __restrict__ Vp = Vprev + c * KB * (int64_t)Np;
+  if (tid < 64) {
+    Ts[tid] = T1[c * 64 + tid];
+    cplx t0 = mkc(0.0, 0.0), t1 = mkc(0.0, 0.0);
+    int I2 = J0;
+    for (; I2 + 1 < nT; I2 += 2) {   // independent loads
+      t0 = cadd(t0, Mpart[(c * nT + I2) * 64 + tid]);
+      t1 = cadd(t1, Mpart[(c * nT + I2 + 1) * 64 + tid]);
+    }
+    if (I2 < nT) t0 = cadd(t0, Mpart[(c * nT + I2) * 64 + tid]);
+    Mf[tid] = cadd(t0, t1);
+  }
+  if (tid < (KB + 1) * KB) {
+    const int tr = tid / KB, tq = tid % KB;
+    const int rr = jprev + tr;
+    Yt[tid] = (rr < N) ? Y[PIX(tq, rr)] : mkc(0.0, 0.0);
+    Vt[tid] = (rr < N) ? Vp[PIX(tq, rr)] : mkc(0.0, 0.0);
+  }
+  __syncthreads();
+  if (tid < 64) {
+    const int a = tid >> 3, b2 = tid & 7;
+    cplx acc = mkc(0.0, 0.0);
+    for (int k2 = 0; k2 < KB; ++k2) {
+      cplx t = mkc(0.0, 0.0);
+      for (int k1 = 0; k1 < KB; ++k1) cfmac(t, Ts[k1 * KB + a], Mf[k1 * KB + k2]);   // conj(T[k1][a]) M[k1][k2]
+      cfma(acc, t, Ts[k2 * KB + b2]);
+    }
+    Cs[tid] = cscale(0.5, acc);
+    MC[c * MC_STRIDE + tid] = Cs[tid];
+  }
+  __syncthreads();
+  if (tid < (KB + 1) * KB) {
+    const int tr = tid / KB, tq = tid % KB;
+    cplx w = mkc(0.0, 0.0);
+#pragma unroll
+    for (int k1 = 0; k1 < KB; ++k1) { cfma(w, Yt[tr * KB + k1], Ts[k1 * KB + tq]); cfms(w, Vt[tr * KB + k1], Cs[k1 * KB + tq]); }
+    MC[c * MC_STRIDE + 64 + tid] = Vt[tid];
+    MC[c * MC_STRIDE + 64 + (KB + 1) * KB + tid] = w;
+  }
+}
+
+// Second wide kernel of a panel step (p > 0), one CTA per (row tile I, matrix), thread = (row, column):
+//   W_{p-1} = Y T - V C for the rows of the tile  -> Wx (explicit panel for k_fused: zero above j2)
+//   the columns p KB .. of the trailing matrix receive the pending update  -= W V^H + V W^H, in place
+//   (ncol = KB columns; at the end of stage 1 the whole trailing block of at most KB + 1 columns).
+__global__ void __launch_bounds__(512) k_wupd(cplx* __restrict__ Bw, const cplx* __restrict__ Yx, const cplx* __restrict__ Vprev,
+                                              cplx* __restrict__ Wx, const cplx* __restrict__ MC,
+                                              const cplx* __restrict__ T1, int N, int Np, int J0, int jprev, int ncol) {
+  __shared__ cplx Ts[KB * KB], Cs[KB * KB], Vtop[(KB + 1) * KB], Wtop[(KB + 1) * KB];
+  __shared__ cplx Ysh[TS * (KB + 1)], Vsh[TS * (KB + 1)], Wsh[TS * (KB + 1)];
+  const int64_t c = blockIdx.y;
+  const int I = J0 + blockIdx.x;
+  const int tid = threadIdx.x, q = tid >> 6, rl = tid & 63;
+  const int r = I * TS + rl, j2 = jprev + KB;
+  cplx* __restrict__ B = Bw + c * (int64_t)N * N;
+  if (tid < 64) { Ts[tid] = T1[c * 64 + tid]; Cs[tid] = MC[c * MC_STRIDE + tid]; }
+  else if (tid < 64 + (KB + 1) * KB) Vtop[tid - 64] = MC[c * MC_STRIDE + tid];
+  else if (tid < 64 + 2 * (KB + 1) * KB) Wtop[tid - 64 - (KB + 1) * KB] = MC[c * MC_STRIDE + tid];
+  // rows of the tile (coalesced: 64 consecutive rows per column q)
+  Ysh[rl * (KB + 1) + q] = Yx[c * KB * (int64_t)Np + PIX(q, r)];
+  Vsh[rl * (KB + 1) + q] = Vprev[c * KB * (int64_t)Np + PIX(q, r)];
+  // the tile's piece of the columns to update: loaded now, used after the barriers
+  cplx bcol[2];
+#pragma unroll
+  for (int u = 0; u < 2; ++u) {
+    const int cc = q + 8 * u, col = jprev + cc;
+    bcol[u] = (cc < ncol && r >= col && r < N) ? B[r + (int64_t)col * N] : mkc(0.0, 0.0);
+  }
+  __syncthreads();
+  cplx w = mkc(0.0, 0.0);
+#pragma unroll
+  for (int k1 = 0; k1 < KB; ++k1) { cfma(w, Ysh[rl * (KB + 1) + k1], Ts[k1 * KB + q]); cfms(w, Vsh[rl * (KB + 1) + k1], Cs[k1 * KB + q]); }
+  Wsh[rl * (KB + 1) + q] = w;
+  Wx[c * KB * (int64_t)Np + PIX(q, r)] = (r >= j2 && r < N) ? w : mkc(0.0, 0.0);
+  __syncthreads();
+#pragma unroll
+  for (int u = 0; u < 2; ++u) {
+    const int cc = q + 8 * u, col = jprev + cc;
+    if (cc < ncol && r >= col && r < N) {
+      cplx acc = bcol[u];
+#pragma unroll
+      for (int k1 = 0; k1 < KB; ++k1) {
+        cfms(acc, Wsh[rl * (KB + 1) + k1], cconj(Vtop[cc * KB + k1]));
+        cfms(acc, Vsh[rl * (KB + 1) + k1], cconj(Wtop[cc * KB + k1]));
+      }
+      if (r == col) acc.y = 0.0;
+      B[r + (int64_t)col * N] = acc;
+    }
+  }
+}
+
+// QR step of panel p, one CTA per matrix: Householder QR of the columns p KB .. p KB + KB - 1 below row
+// j2 = (p + 1) KB (thread t owns the rows j2 + t + s PT): reflectors stored in place (R on and above the
+// sub-band diagonal), explicit V (unit heads, zeros above) for k_fused, tau, T; one block reduction per column.
+// The panel stays on chip: row slot 0 of every thread in registers, the slots s >= 1 in shared memory
+// ([slot][column][thread]: conflict free).
 template <int RPT>
 __global__ void __launch_bounds__(PT, 1) k_panel(cplx* __restrict__ Bw, cplx* __restrict__ Vnew, cplx* __restrict__ Vprev,
-                                                 cplx* __restrict__ Wx, const cplx* __restrict__ Mpart,
-                                                 cplx* __restrict__ T1, cplx* __restrict__ tau1, int N, int Np, int nT,
-                                                 int p, int do_qr) {
+                                                 cplx* __restrict__ Wx, cplx* __restrict__ T1, cplx* __restrict__ tau1,
+                                                 int N, int Np, int p) {
   extern __shared__ __align__(16) cplx psm[];   // panel slots 1 .. RPT-1
-  __shared__ cplx Ts[KB * KB], Cs[KB * KB], Mf[64], Tn[KB * KB];
-  __shared__ cplx Vtop[(KB + 1) * KB], Wtop[(KB + 1) * KB];
+  __shared__ cplx Tn[KB * KB];
   __shared__ cplx red[(PT / 32) * KB], res[2][KB], head[2][KB];
   const int64_t c = blockIdx.x;
   const int tid = threadIdx.x;
@@ -194,146 +291,23 @@ __global__ void __launch_bounds__(PT, 1) k_panel(cplx* __restrict__ Bw, cplx* __
   const int jprev = p * KB, j2 = jprev + KB;
   cplx a0[KB];
 #define PA(s, q) psm[(((s) - 1) * KB + (q)) * PT + tid]
-
-  if (p > 0) {
-    const int J0 = jprev / TS;
-    if (tid < 64) {
-      Ts[tid] = T1[c * 64 + tid];
-      cplx t = mkc(0.0, 0.0);
-      for (int I = J0; I < nT; ++I) t = cadd(t, Mpart[(c * nT + I) * 64 + tid]);
-      Mf[tid] = t;
-    }
-    __syncthreads();
-    if (tid < 64) {
-      // C = 1/2 T^H M T
-      const int q = tid >> 3, q2 = tid & 7;
-      cplx acc = mkc(0.0, 0.0);
-      for (int b2 = 0; b2 < KB; ++b2) {
-        cplx t = mkc(0.0, 0.0);
-        for (int a2 = 0; a2 < KB; ++a2) cfmac(t, Ts[a2 * KB + q], Mf[a2 * KB + b2]);   // conj(T[a][q]) M[a][b]
-        cfma(acc, t, Ts[b2 * KB + q2]);
-      }
-      Cs[tid] = cscale(0.5, acc);
-    }
-    __syncthreads();
-    // the top rows of W and V (needed by every row of the column update)
-    if (tid < KB + 1) {
-      const int r = jprev + tid;
 #pragma unroll
-      for (int q = 0; q < KB; ++q) { Vtop[tid * KB + q] = mkc(0.0, 0.0); Wtop[tid * KB + q] = mkc(0.0, 0.0); }
-      if (r < N) {
-        cplx y[KB], v[KB];
+  for (int s = 0; s < RPT; ++s) {
+    const int r = j2 + tid + s * PT;
 #pragma unroll
-        for (int q = 0; q < KB; ++q) { y[q] = W[PIX(q, r)]; v[q] = Vp[PIX(q, r)]; }
-#pragma unroll
-        for (int q2 = 0; q2 < KB; ++q2) {
-          cplx w = mkc(0.0, 0.0);
-#pragma unroll
-          for (int q = 0; q < KB; ++q) { cfma(w, y[q], Ts[q * KB + q2]); cfms(w, v[q], Cs[q * KB + q2]); }
-          Wtop[tid * KB + q2] = w;
-          Vtop[tid * KB + q2] = v[q2];
-        }
-      }
-    }
-    __syncthreads();
-    // W rows in place of Y (explicit panel for k_fused: zero above j2) ...
-#pragma unroll 1
-    for (int s = 0; s < RPT; ++s) {
-      const int r = jprev + tid + s * PT;
-      if (r < N) {
-        cplx y[KB], v[KB];
-#pragma unroll
-        for (int q = 0; q < KB; ++q) { y[q] = W[PIX(q, r)]; v[q] = Vp[PIX(q, r)]; }
-        const bool keep = r >= j2;
-#pragma unroll
-        for (int q2 = 0; q2 < KB; ++q2) {
-          cplx t = mkc(0.0, 0.0);
-#pragma unroll
-          for (int q = 0; q < KB; ++q) { cfma(t, y[q], Ts[q * KB + q2]); cfms(t, v[q], Cs[q * KB + q2]); }
-          W[PIX(q2, r)] = keep ? t : mkc(0.0, 0.0);
-        }
-      }
-    }
-    if (!do_qr) {
-      // last step: the trailing block B[jprev:, jprev:] (at most KB + 1 columns) gets the update
-      if (tid < (KB + 1) * (KB + 1)) {
-        const int rr = tid % (KB + 1), cc = tid / (KB + 1);
-        const int r = jprev + rr, col = jprev + cc;
-        if (rr >= cc && r < N) {
-          cplx acc = B[r + (int64_t)col * N];
-#pragma unroll
-          for (int q = 0; q < KB; ++q) {
-            cfms(acc, Wtop[rr * KB + q], cconj(Vtop[cc * KB + q]));
-            cfms(acc, Vtop[rr * KB + q], cconj(Wtop[cc * KB + q]));
-          }
-          if (rr == cc) acc.y = 0.0;
-          B[r + (int64_t)col * N] = acc;
-        }
-      }
-      return;
-    }
-    // ... and the update of the panel columns (each thread re-reads the rows it wrote)
-#pragma unroll
-    for (int s = 0; s < RPT; ++s) {
-      const int r = jprev + tid + s * PT;
-      cplx acc8[KB];
-#pragma unroll
-      for (int q = 0; q < KB; ++q) acc8[q] = mkc(0.0, 0.0);
-      if (r < N) {
-        cplx v[KB], w[KB];
-#pragma unroll
-        for (int q = 0; q < KB; ++q) {
-          v[q] = (r < j2) ? Vtop[(r - jprev) * KB + q] : Vp[PIX(q, r)];
-          w[q] = (r < j2) ? Wtop[(r - jprev) * KB + q] : W[PIX(q, r)];
-        }
-#pragma unroll
-        for (int cc = 0; cc < KB; ++cc) {
-          const int col = jprev + cc;
-          cplx acc = (r >= col) ? B[r + (int64_t)col * N] : mkc(0.0, 0.0);
-#pragma unroll
-          for (int q = 0; q < KB; ++q) {
-            cfms(acc, w[q], cconj(Vtop[cc * KB + q]));
-            cfms(acc, v[q], cconj(Wtop[cc * KB + q]));
-          }
-          acc8[cc] = acc;
-        }
-      }
-#pragma unroll
-      for (int q = 0; q < KB; ++q) { if (s == 0) a0[q] = acc8[q]; else PA(s, q) = acc8[q]; }
-    }
-  } else {
-#pragma unroll
-    for (int s = 0; s < RPT; ++s) {
-      const int r = jprev + tid + s * PT;
-#pragma unroll
-      for (int cc = 0; cc < KB; ++cc) {
-        const cplx t = (r < N && r >= jprev + cc) ? B[r + (int64_t)(jprev + cc) * N] : mkc(0.0, 0.0);
-        if (s == 0) a0[cc] = t; else PA(s, cc) = t;
-      }
-    }
-  }
-
-  // rows jprev .. j2-1 are final band entries (lower part of the diagonal block)
-  if (tid < KB) {
-    const int r = jprev + tid;
-    if (r < N) {
-#pragma unroll
-      for (int cc = 0; cc < KB; ++cc)
-        if (cc <= tid) {
-          cplx t = a0[cc];
-          if (cc == tid) t.y = 0.0;
-          B[r + (int64_t)(jprev + cc) * N] = t;
-        }
+    for (int cc = 0; cc < KB; ++cc) {
+      const cplx t = (r < N) ? B[r + (int64_t)(jprev + cc) * N] : mkc(0.0, 0.0);
+      if (s == 0) a0[cc] = t; else PA(s, cc) = t;
     }
   }
   if (tid < 64) Tn[tid] = mkc(0.0, 0.0);
 
-  // ---- Householder QR of the rows >= j2 (local row lr = r - j2; the thread's slot s holds lr = tid - KB + s PT)
-  const int lr0 = tid - KB;
+  // ---- Householder QR (local row lr = r - j2; the thread's slot s holds lr = tid + s PT)
+  const int lr0 = tid;
 #pragma unroll 1
   for (int cc = 0; cc < KB; ++cc) {
     const int hb = cc & 1;
-    if (tid == KB + cc) {
+    if (tid == cc) {
 #pragma unroll
       for (int q = 0; q < KB; ++q) head[hb][q] = a0[q];
     }
@@ -1028,7 +1002,7 @@ __global__ void __launch_bounds__(QS * Q2_TSG_MAX, 1) k_q2(const cplx* __restric
 }
 
 struct BandScratch {
-  cplx *Vx0, *Vx1, *Wx, *P, *Zc, *T1, *AB, *Mpart;
+  cplx *Vx0, *Vx1, *Wx, *Yx, *P, *Zc, *T1, *AB, *Mpart, *MC;
   int* counters;
   int* start;
 };
@@ -1040,14 +1014,16 @@ size_t band_carve(char* base, int64_t cnt, int N, BandScratch* s) {
   cplx* v0 = (cplx*)take((size_t)cnt * Np * KB * sizeof(cplx));
   cplx* v1 = (cplx*)take((size_t)cnt * Np * KB * sizeof(cplx));
   cplx* wx = (cplx*)take((size_t)cnt * Np * KB * sizeof(cplx));
+  cplx* yx = (cplx*)take((size_t)cnt * Np * KB * sizeof(cplx));
   cplx* P = (cplx*)take((size_t)cnt * nT * Np * KB * sizeof(cplx));
   cplx* zc = (cplx*)take((size_t)cnt * Np * KB * sizeof(cplx));
   cplx* t1 = (cplx*)take((size_t)cnt * 64 * sizeof(cplx));
   cplx* ab = (cplx*)take((size_t)cnt * N * LDAB * sizeof(cplx));
   cplx* mp = (cplx*)take((size_t)cnt * nT * 64 * sizeof(cplx));
+  cplx* mc = (cplx*)take((size_t)cnt * MC_STRIDE * sizeof(cplx));
   int* counters = (int*)take((size_t)(N / KB + 2) * sizeof(int));
   int* start = (int*)take((size_t)N * sizeof(int));
-  if (s) *s = BandScratch{v0, v1, wx, P, zc, t1, ab, mp, counters, start};
+  if (s) *s = BandScratch{v0, v1, wx, yx, P, zc, t1, ab, mp, mc, counters, start};
   return off;
 }
 
@@ -1069,7 +1045,6 @@ int be_band_reduce(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double*
   const int nT = (N + TS - 1) / TS, Np = nT * TS;
   // last panel with something to annihilate: rows below j2 = (p + 1) KB number N - j2 >= 2
   const int plast = (N - 2) / KB - 1;
-  const int RPT = (N + PT - 1) / PT;
   BE_CUDA(cudaMemsetAsync(s.Vx0, 0, (size_t)cnt * Np * KB * sizeof(cplx), st));
   BE_CUDA(cudaMemsetAsync(s.Vx1, 0, (size_t)cnt * Np * KB * sizeof(cplx), st));
   BE_CUDA(cudaMemsetAsync(s.Wx, 0, (size_t)cnt * Np * KB * sizeof(cplx), st));
@@ -1077,25 +1052,35 @@ int be_band_reduce(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double*
   BE_CUDA(cudaMemsetAsync(tau, 0, (size_t)cnt * N * sizeof(cplx), st));
   k_symdiag<<<dim3((unsigned)nT, (unsigned)cnt), 256, 0, st>>>(Bw, N);
   LAUNCH_CHECK();
-  const size_t psm = (size_t)(RPT - 1) * PT * KB * sizeof(cplx);
   auto panel = [&](int p, int do_qr) -> int {
     cplx* vn = (p & 1) ? s.Vx1 : s.Vx0;
     cplx* vp = (p & 1) ? s.Vx0 : s.Vx1;
     be_prof_begin(ctx, PK_PANEL);
     const int n = N - p * KB;
     if (p > 0) {
+      // two wide kernels: Y = sum of the partial products (+ the tiles' shares of V^H Y), then W and the update
+      // of the next panel's columns
       const int J0 = (p * KB) / TS;
-      k_ysum<<<dim3((unsigned)(nT - J0), (unsigned)cnt), 512, 0, st>>>(s.P, s.Zc, vp, s.Wx, s.Mpart, N, Np, nT, J0, p * KB);
+      k_ysum<<<dim3((unsigned)(nT - J0), (unsigned)cnt), 512, 0, st>>>(s.P, s.Zc, vp, s.Yx, s.Mpart, N, Np, nT, J0, p * KB);
+      ctx->launches++;
+      k_mc<<<(unsigned)cnt, 96, 0, st>>>(s.Yx, vp, s.Mpart, s.T1, s.MC, N, Np, nT, J0, p * KB);
+      ctx->launches++;
+      k_wupd<<<dim3((unsigned)(nT - J0), (unsigned)cnt), 512, 0, st>>>(Bw, s.Yx, vp, s.Wx, s.MC, s.T1, N, Np, J0,
+                                                                      p * KB, do_qr ? KB : N - p * KB);
       ctx->launches++;
     }
+    if (do_qr) {
+      const int rpt = (N - (p + 1) * KB + PT - 1) / PT;
+      const size_t psm = (size_t)(rpt - 1) * PT * KB * sizeof(cplx);
 #define PANEL_CASE(R) case R: \
       BE_CUDA(cudaFuncSetAttribute(k_panel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm)); \
-      k_panel<R><<<(unsigned)cnt, PT, psm, st>>>(Bw, vn, vp, s.Wx, s.Mpart, s.T1, tau, N, Np, nT, p, do_qr); break;
-    switch (RPT) {
-      PANEL_CASE(1) PANEL_CASE(2) PANEL_CASE(3) PANEL_CASE(4)
-      default: return BE_ERR_UNSUPPORTED;
-    }
+      k_panel<R><<<(unsigned)cnt, PT, psm, st>>>(Bw, vn, vp, s.Wx, s.T1, tau, N, Np, p); break;
+      switch (rpt) {
+        PANEL_CASE(1) PANEL_CASE(2) PANEL_CASE(3) PANEL_CASE(4)
+        default: return BE_ERR_UNSUPPORTED;
+      }
 #undef PANEL_CASE
+    }
     be_prof_end(ctx, PK_PANEL, (double)cnt * n * 16.0 * (6.0 * KB + 0.5 * KB * ((n + TS - 1) / TS)), (double)cnt * n * 8.0 * 6 * KB * KB);
     LAUNCH_CHECK();
     return BE_OK;
