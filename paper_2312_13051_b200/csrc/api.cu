@@ -45,6 +45,7 @@ void be_prof_end(be_ctx* ctx, int cls, double bytes, double flops) {
 }
 
 extern "C" int be_profile_enable(be_ctx* ctx, int on) {
+  BE_DEVICE_GUARD(ctx);
   if (!ctx) return BE_ERR_NULL;
   if (!ctx->prof) ctx->prof = new (std::nothrow) be_prof;
   if (!ctx->prof) return BE_ERR_NOMEM;
@@ -63,6 +64,7 @@ extern "C" const char* be_profile_name(int cls) {
 }
 
 extern "C" int be_profile_get(be_ctx* ctx, int cls, double* ms, int64_t* launches, double* bytes, double* flops) {
+  BE_DEVICE_GUARD(ctx);
   if (!ctx || !ctx->prof) return BE_ERR_NULL;
   if (cls < 0 || cls >= PK_COUNT) return BE_ERR_SHAPE;
   be_prof* p = ctx->prof;
@@ -136,6 +138,7 @@ extern "C" int be_create(be_ctx** out, void* cuda_stream) {
 }
 
 extern "C" int be_destroy(be_ctx* ctx) {
+  BE_DEVICE_GUARD(ctx);
   if (!ctx) return BE_ERR_NULL;
   cudaStreamSynchronize(ctx->stream);
   if (ctx->arena) cudaFree(ctx->arena);
@@ -167,6 +170,7 @@ extern "C" const char* be_strerror(int code) {
 }
 
 extern "C" int be_set_workspace_limit(be_ctx* ctx, size_t bytes) {
+  BE_DEVICE_GUARD(ctx);
   if (!ctx) return BE_ERR_NULL;
   if (bytes < ((size_t)1 << 20)) return BE_ERR_SHAPE;
   ctx->ws_limit = bytes;
@@ -174,19 +178,22 @@ extern "C" int be_set_workspace_limit(be_ctx* ctx, size_t bytes) {
 }
 
 extern "C" int be_set_chunk_pipeline(be_ctx* ctx, int on) {
+  BE_DEVICE_GUARD(ctx);
   if (!ctx) return BE_ERR_NULL;
   ctx->chunk_pipeline = on ? 1 : 0;
   return BE_OK;
 }
 
 extern "C" int be_set_eigh_algorithm(be_ctx* ctx, int algo) {
+  BE_DEVICE_GUARD(ctx);
   if (!ctx) return BE_ERR_NULL;
   if (algo < 0 || algo > 2) return BE_ERR_SHAPE;
   ctx->eigh_algo = algo;
   return BE_OK;
 }
 
-extern "C" int64_t be_launch_count(const be_ctx* ctx) { return ctx ? ctx->launches : 0; }
+extern "C" int64_t be_launch_count(const be_ctx* ctx) {
+  BE_DEVICE_GUARD(ctx); return ctx ? ctx->launches : 0; }
 
 // ---------------------------------------------------------------------------------------------
 size_t be_eigh_scratch_bytes(int64_t cnt, int N, int nv) {
@@ -246,6 +253,7 @@ extern "C" size_t be_workspace_bytes(const be_grid* g, int n_occ, int op) {
 // ---------------------------------------------------------------------------------------------
 extern "C" int be_eigh_batched(be_ctx* ctx, const void* dH, int64_t count, int N, int n_vec,
                                double* dE, void* dU, int* d_info) {
+  BE_DEVICE_GUARD(ctx);
   if (!ctx) return BE_ERR_NULL;
   if (count < 0 || N < 1 || n_vec < 0 || n_vec > N) return BE_ERR_SHAPE;
   if (count == 0) return BE_OK;
@@ -278,6 +286,7 @@ extern "C" int be_eigh_batched(be_ctx* ctx, const void* dH, int64_t count, int N
 
 extern "C" int be_winding(be_ctx* ctx, const double* d_theta, int64_t n_cycles, int n_points, int m,
                           double* d_wind) {
+  BE_DEVICE_GUARD(ctx);
   if (!ctx || !d_theta || !d_wind) return BE_ERR_NULL;
   if (n_cycles < 0 || n_points < 1 || m < 1) return BE_ERR_SHAPE;
   if (n_cycles == 0) return BE_OK;
@@ -288,6 +297,7 @@ extern "C" int be_zgemm_batched(be_ctx* ctx, int opA, int opB, int M, int N, int
                                 const double* alpha, const void* dA, int lda, int64_t strideA,
                                 const void* dB, int ldb, int64_t strideB,
                                 const double* beta, void* dC, int ldc, int64_t strideC, int64_t batch, int lower) {
+  BE_DEVICE_GUARD(ctx);
   if (!ctx || !dA || !dB || !dC || !alpha || !beta) return BE_ERR_NULL;
   if (M < 0 || N < 0 || K < 0 || batch < 0 || lda < 1 || ldb < 1 || ldc < 1) return BE_ERR_SHAPE;
   if (!aligned(dA, 16) || !aligned(dB, 16) || !aligned(dC, 16)) return BE_ERR_ALIGN;
@@ -316,6 +326,7 @@ __global__ void k_bloch_coef(const double* __restrict__ t, const int* __restrict
 
 extern "C" int be_bloch_coefficients(be_ctx* ctx, const double* d_t, const int* h_R, int nd, int nR, int64_t count,
                                      void* d_coef) {
+  BE_DEVICE_GUARD(ctx);
   if (!ctx || !d_t || !h_R || !d_coef) return BE_ERR_NULL;
   if (nd < 1 || nd > 3 || nR < 1 || count < 0) return BE_ERR_SHAPE;
   if (!aligned(d_t, 8) || !aligned(d_coef, 16)) return BE_ERR_ALIGN;
@@ -333,6 +344,7 @@ extern "C" int be_bloch_coefficients(be_ctx* ctx, const double* d_t, const int* 
 
 extern "C" int be_assemble_bloch(be_ctx* ctx, const void* dA, const void* d_coef, int64_t count, int N, int nR,
                                  void* dH) {
+  BE_DEVICE_GUARD(ctx);
   if (!ctx || !dA || !d_coef || !dH) return BE_ERR_NULL;
   if (N < 1 || nR < 1 || count < 0 || (int64_t)N * N > 0x7fffffffLL || count > 0x7fffffffLL) return BE_ERR_SHAPE;
   if (!aligned(dA, 16) || !aligned(d_coef, 16) || !aligned(dH, 16)) return BE_ERR_ALIGN;

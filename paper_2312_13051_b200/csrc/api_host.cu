@@ -113,6 +113,7 @@ int host_run(be_ctx* ctx, const void* hH, const be_grid* grid, int n_occ, int di
 
 extern "C" int be_wilson_loop_host(be_ctx* ctx, const void* hH_grid, const be_grid* grid, int n_occ, int dir,
                                    const void* h_close, double* h_theta, double* h_abs, double* h_mingap) {
+  BE_DEVICE_GUARD(ctx);
   return host_run(ctx, hH_grid, grid, n_occ, dir, nullptr, 0, 0, false, h_close, h_theta, h_abs, h_mingap);
 }
 
@@ -120,6 +121,7 @@ extern "C" int be_spin_resolved_wilson_host(be_ctx* ctx, const void* hH_grid, co
                                             int dir, const void* hS, int S_is_diag, int m_lo,
                                             const void* h_close, double* h_theta_lo, double* h_theta_hi,
                                             double* h_pso) {
+  BE_DEVICE_GUARD(ctx);
   return host_run(ctx, hH_grid, grid, n_occ, dir, hS, S_is_diag, m_lo, true, h_close, h_theta_lo,
                   h_theta_hi, h_pso);
 }
@@ -129,6 +131,7 @@ extern "C" int be_spin_resolved_wilson_host(be_ctx* ctx, const void* hH_grid, co
 extern "C" int be_nested_wilson_host(be_ctx* ctx, const void* hH_grid, const be_grid* grid, int n_occ, int dir1, int dir2,
                                      int base, int wb_lo, int wb_hi, double theta_cut, const void* h_close1,
                                      const void* h_close2, double* h_theta1, double* h_theta_nested) {
+  BE_DEVICE_GUARD(ctx);
   if (!ctx || !hH_grid || !grid || !h_theta_nested) return BE_ERR_NULL;
   if (grid->ndim < 2 || grid->ndim > 3 || grid->batch < 1 || grid->N < 1) return BE_ERR_SHAPE;
   if (dir1 < 0 || dir1 >= grid->ndim || dir2 < 0 || dir2 >= grid->ndim || dir1 == dir2) return BE_ERR_SHAPE;

@@ -334,6 +334,7 @@ static int check_common(be_ctx* ctx, const void* H, const be_grid* g, int n_occ,
 
 extern "C" int be_wilson_loop(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_occ, int dir,
                               const void* d_close, double* d_theta, double* d_abs, double* d_mingap) {
+  BE_DEVICE_GUARD(ctx);
   BE_TRY(check_common(ctx, dH_grid, grid, n_occ, dir));
   if (!d_theta) return BE_ERR_NULL;
   if ((d_close && !aligned(d_close, 16)) || !aligned(d_theta, 8)) return BE_ERR_ALIGN;
@@ -345,6 +346,7 @@ extern "C" int be_wilson_loop(be_ctx* ctx, const void* dH_grid, const be_grid* g
 
 extern "C" int be_wilson_loop_window(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int band_lo, int band_hi,
                                      int dir, const void* d_close, double* d_theta, double* d_abs, double* d_mingap) {
+  BE_DEVICE_GUARD(ctx);
   if (band_lo < 0 || band_hi <= band_lo) return BE_ERR_SHAPE;
   BE_TRY(check_common(ctx, dH_grid, grid, band_hi, dir));
   if (!d_theta) return BE_ERR_NULL;
@@ -362,6 +364,7 @@ extern "C" int be_spin_resolved_wilson_window(be_ctx* ctx, const void* dH_grid, 
                                               int band_hi, int dir, const void* dS, int S_is_diag, int m_lo,
                                               const void* d_close, double* d_theta_lo, double* d_theta_hi,
                                               double* d_pso) {
+  BE_DEVICE_GUARD(ctx);
   if (band_lo < 0 || band_hi <= band_lo) return BE_ERR_SHAPE;
   BE_TRY(check_common(ctx, dH_grid, grid, band_hi, dir));
   if (!dS) return BE_ERR_NULL;
@@ -383,6 +386,7 @@ extern "C" int be_spin_resolved_wilson(be_ctx* ctx, const void* dH_grid, const b
                                        int dir, const void* dS, int S_is_diag, int m_lo,
                                        const void* d_close, double* d_theta_lo, double* d_theta_hi,
                                        double* d_pso) {
+  BE_DEVICE_GUARD(ctx);
   BE_TRY(check_common(ctx, dH_grid, grid, n_occ, dir));
   if (!dS) return BE_ERR_NULL;
   if (m_lo < 0) m_lo = n_occ / 2;
@@ -400,6 +404,7 @@ extern "C" int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid*
                                 int dir1, int dir2, int base, int wb_lo, int wb_hi, double theta_cut,
                                 const void* d_close1, const void* d_close2,
                                 double* d_theta1, double* d_theta_nested) {
+  BE_DEVICE_GUARD(ctx);
   BE_TRY(check_common(ctx, dH_grid, grid, n_occ, dir1));
   if (!d_theta_nested) return BE_ERR_NULL;
   if (grid->ndim < 2 || dir2 < 0 || dir2 >= grid->ndim || dir2 == dir1) return BE_ERR_SHAPE;
@@ -500,6 +505,7 @@ static int plaquette_of_frames(be_ctx* ctx, const cplx* F, int64_t batch, int ny
 
 extern "C" int be_plaquette_flux(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int n_occ, const void* dS,
                                  int S_is_diag, int m_lo, double* d_flux, double* d_flux_hi, double* d_pso) {
+  BE_DEVICE_GUARD(ctx);
   BE_TRY(check_common(ctx, dH_grid, grid, n_occ, 0));
   if (grid->ndim != 2 || !d_flux) return grid->ndim != 2 ? BE_ERR_SHAPE : BE_ERR_NULL;
   const int ny = grid->dims[0], nx = grid->dims[1], N = grid->N, m = n_occ;
@@ -582,6 +588,7 @@ static int bloch_source(be_ctx* ctx, const void* dA, const int* h_R, int nR, con
 extern "C" int be_wilson_loop_bloch(be_ctx* ctx, const void* dA, const int* h_R, int nR, const be_grid* grid,
                                     int n_occ, int dir, const void* d_close, double* d_theta, double* d_abs,
                                     double* d_mingap) {
+  BE_DEVICE_GUARD(ctx);
   BE_TRY(check_common(ctx, dA, grid, n_occ, dir));
   if (!d_theta) return BE_ERR_NULL;
   BlochSrc bs;
@@ -594,6 +601,7 @@ extern "C" int be_spin_resolved_wilson_bloch(be_ctx* ctx, const void* dA, const 
                                              int n_occ, int dir, const void* dS, int S_is_diag, int m_lo,
                                              const void* d_close, double* d_theta_lo, double* d_theta_hi,
                                              double* d_pso) {
+  BE_DEVICE_GUARD(ctx);
   BE_TRY(check_common(ctx, dA, grid, n_occ, dir));
   if (!dS) return BE_ERR_NULL;
   if (m_lo < 0) m_lo = n_occ / 2;

@@ -106,6 +106,17 @@ enum { PK_HEMV = 0, PK_COL, PK_GEMM, PK_BISECT, PK_INVIT, PK_ORTH, PK_HESS, PK_H
 void be_prof_begin(be_ctx* ctx, int cls);
 void be_prof_end(be_ctx* ctx, int cls, double bytes, double flops);
 
+// Every extern "C" entry point makes the context's device current for its duration (the scratch arena, the
+// internal streams and the function attributes belong to that device) and restores the caller's on return.
+struct be_device_guard {
+  int prev = -1;
+  explicit be_device_guard(const be_ctx* ctx) {
+    if (ctx && cudaGetDevice(&prev) == cudaSuccess && prev != ctx->device) cudaSetDevice(ctx->device); else prev = -1;
+  }
+  ~be_device_guard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define BE_DEVICE_GUARD(ctx) be_device_guard be_guard__(ctx)
+
 #define BE_CUDA(x) do { cudaError_t e__ = (x); if (e__ != cudaSuccess) return (int)e__; } while (0)
 #define BE_TRY(x) do { int r__ = (x); if (r__ != BE_OK) return r__; } while (0)
 

@@ -63,6 +63,7 @@ __global__ void __launch_bounds__(256) k_probe_dfma3(double* out, const double* 
 }  // namespace
 
 extern "C" int be_probe_fp64(be_ctx* ctx, int which, double* tflops) {
+  BE_DEVICE_GUARD(ctx);
   if (!ctx || !tflops) return BE_ERR_NULL;
   if (which < 0 || which > 2) return BE_ERR_SHAPE;
   int prev = 0;

@@ -450,10 +450,9 @@ __global__ void __launch_bounds__(NTHREADS, 3) zgemm_async_kernel(const ZgemmPar
   }
 }
 
-static int gemm_async_mode() {   // BE_GEMM_ASYNC=0 selects the register-staged kernel everywhere
-  static int mode = -1;
-  if (mode < 0) { const char* e = getenv("BE_GEMM_ASYNC"); mode = (e && e[0] == '0') ? 0 : 1; }
-  return mode;
+static int gemm_async_mode() {   // BE_GEMM_ASYNC=0 selects the register-staged kernel everywhere (A/B measurements)
+  const char* e = getenv("BE_GEMM_ASYNC");
+  return (e && e[0] == '0') ? 0 : 1;
 }
 
 template <int OPA, int OPB, bool PHI, bool SPLIT>
@@ -463,25 +462,19 @@ int launch(be_ctx* ctx, const ZgemmParams& p) {
   const int64_t blocks = p.batch * (p.lower ? (int64_t)(TM / TN) * tilesM * (tilesM + 1) / 2 : (int64_t)tilesM * tilesN);
   if (blocks <= 0) return BE_OK;
   if (blocks > 0x7fffffffLL) return BE_ERR_SHAPE;
-  static bool attr_done = false;  // per instantiation; idempotent
-  if (!attr_done) {
-    BE_CUDA(cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, PHI, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM_PAD));
-    attr_done = true;
-  }
+  // function attributes are per device: set on every launch (the context's device is current; no process-wide flag)
   be_prof_begin(ctx, PK_GEMM);
   if constexpr (!PHI) {
     if (M3 && gemm_async_mode() && !ctx->gemm_pad) {
-      static bool attr2_done = false;
-      if (!attr2_done) {
-        BE_CUDA(cudaFuncSetAttribute(zgemm_async_kernel<OPA, OPB, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AS_BYTES));
-        BE_CUDA(cudaFuncSetAttribute(zgemm_async_kernel<OPA, OPB, SPLIT>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-        attr2_done = true;
-      }
+      BE_CUDA(cudaFuncSetAttribute(zgemm_async_kernel<OPA, OPB, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AS_BYTES));
+      BE_CUDA(cudaFuncSetAttribute(zgemm_async_kernel<OPA, OPB, SPLIT>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
       zgemm_async_kernel<OPA, OPB, SPLIT><<<(unsigned)blocks, NTHREADS, AS_BYTES, ctx->stream>>>(p, tilesM, tilesN);
     } else {
+      BE_CUDA(cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, PHI, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM_PAD));
       zgemm_kernel<OPA, OPB, PHI, SPLIT><<<(unsigned)blocks, NTHREADS, (ctx->gemm_pad && ctx->stream == ctx->stream2) ? SM_PAD : SM_BYTES, ctx->stream>>>(p, tilesM, tilesN);
     }
   } else {
+    BE_CUDA(cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, PHI, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM_PAD));
     zgemm_kernel<OPA, OPB, PHI, SPLIT><<<(unsigned)blocks, NTHREADS, (ctx->gemm_pad && ctx->stream == ctx->stream2) ? SM_PAD : SM_BYTES, ctx->stream>>>(p, tilesM, tilesN);
   }
   {
