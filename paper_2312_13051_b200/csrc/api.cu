@@ -98,7 +98,9 @@ int be_arena_reserve(be_ctx* ctx, size_t bytes) {
 
 // The cap that applies to a call: the configured limit, but never more than what the device can give right now
 // (free memory plus the arena already held, minus a margin for the caller's outputs and the CUDA context).
-size_t be_effective_ws_limit(be_ctx* ctx) {
+size_t be_effective_ws_limit(be_ctx* ctx, size_t want) {
+  // cudaMemGetInfo costs ~0.5 ms: not worth asking when the whole request is small or already held
+  if (want <= ctx->arena_bytes || want <= ((size_t)1 << 30)) return ctx->ws_limit;
   size_t fr = 0, tot = 0;
   if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) { cudaGetLastError(); return ctx->ws_limit; }
   const size_t margin = (size_t)2 << 30;
@@ -262,7 +264,7 @@ extern "C" int be_eigh_batched(be_ctx* ctx, const void* dH, int64_t count, int N
   if (count == 0) return BE_OK;
   const int nv = dU ? n_vec : 0;
   const size_t per = be_eigh_scratch_bytes(1, N, nv) + (size_t)N * (nv > 0 ? nv : 1) * sizeof(cplx) + 1024;
-  int64_t chunk = (int64_t)(be_effective_ws_limit(ctx) / per);
+  int64_t chunk = (int64_t)(be_effective_ws_limit(ctx, per * (size_t)count) / per);
   if (chunk < 1) chunk = 1;
   if (chunk > count) chunk = count;
   const int64_t nchunks = (count + chunk - 1) / chunk;

@@ -43,7 +43,7 @@ static size_t per_loop_bytes(int N, int m, int n1, bool spin, int lo = 0) {
   size_t b = (size_t)n1 * (be_eigh_scratch_bytes(1, N, lo + m) + (size_t)N * (lo + m) * sizeof(cplx) + (lo ? fr : 0) +
                            (size_t)N * sizeof(double) + 512);
   const size_t mm = (size_t)m * m * sizeof(cplx);
-  b += (size_t)n1 * mm + 4 * mm + (size_t)m * 64 + 4096;           // links, products, eigenvalues
+  b += (size_t)2 * n1 * mm + 8 * mm + (size_t)m * 64 + 4096;       // links, product tree, eigenvalues
   if (spin) {
     b += (size_t)n1 * (fr /*SX*/ + 2 * mm /*S_red, V*/ + fr /*sector frames*/ + (size_t)m * 8 + 1024);
     const size_t inner = (size_t)n1 * be_eigh_scratch_bytes(1, m, m);
@@ -108,8 +108,15 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
                          const SpinArgs* sp, HostStage* hs = nullptr, const BlochSrc* bs = nullptr) {
   const int n1 = map.n1;
   const int64_t loops = map.loops;
+  // tiny matrices, at most two bands: the whole path in one kernel, a warp per loop (small_loop.cu)
+  if (!hs && !bs && ctx->band_lo == 0 && be_small_loop_applies(N, m, n1) && (!sp || sp->m_lo <= m)) {
+    if (sp) return be_small_loop(ctx, H, nullptr, map, N, m, d_close, n1 - 1, nullptr, nullptr, nullptr, nullptr, nullptr, sp->dS,
+                                 sp->S_is_diag, sp->m_lo, sp->theta_lo, sp->theta_hi, sp->pso);
+    return be_small_loop(ctx, H, nullptr, map, N, m, d_close, n1 - 1, d_theta, d_abs, d_mingap, nullptr, nullptr, nullptr, 0, 0,
+                         nullptr, nullptr, nullptr);
+  }
   const size_t per = per_loop_bytes(N, m, n1, sp != nullptr, ctx->band_lo);
-  size_t ws = be_effective_ws_limit(ctx);
+  size_t ws = be_effective_ws_limit(ctx, per * (size_t)loops + (hs ? 2 * hs->loop_bytes * (size_t)loops : 0));
   if (hs) {
     // the two staging buffers of a host grid come out of the same budget (2 x loop_bytes per loop of a chunk)
     const size_t held = 2 * ctx->stage_cap;
@@ -430,10 +437,10 @@ extern "C" int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid*
   const int phi_at = n1 - 1 - base;   // link whose target frame has grid index 0
 
   const size_t per = (size_t)n1 * (be_eigh_scratch_bytes(1, N, m) + (size_t)N * m * 16 + (size_t)N * 8 + 512)
-                     + (size_t)n1 * m * m * 16 + 8 * (size_t)m * m * 16 + 4096
+                     + (size_t)2 * n1 * m * m * 16 + 8 * (size_t)m * m * 16 + 4096
                      + (m > 2 ? be_nested_general_scratch_bytes(1, m, ns) + be_eigenphases_scratch_bytes(1, m) : 0);
-  const size_t persist = (size_t)loops * ((size_t)N * ns * 16 + 256) + (size_t)outer2 * (n2 + 4) * ns * ns * 16 + (8 << 20);
-  int64_t lc = (int64_t)(be_effective_ws_limit(ctx) / per);
+  const size_t persist = (size_t)loops * ((size_t)N * ns * 16 + 256) + (size_t)outer2 * (2 * n2 + 8) * ns * ns * 16 + (8 << 20);
+  int64_t lc = (int64_t)(be_effective_ws_limit(ctx, per * (size_t)loops) / per);
   if (lc < 1) lc = 1;
   if (lc > loops) lc = loops;
   BE_TRY(be_arena_reserve(ctx, per * (size_t)lc + persist + (size_t)loops * m * 8 + (4 << 20)));
@@ -442,7 +449,20 @@ extern "C" int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid*
   double* th1 = d_theta1 ? d_theta1 : (double*)be_arena_alloc(ctx, (size_t)loops * m * sizeof(double));
   if (!Wf || !th1) return BE_ERR_NOMEM;
   const size_t keep = ctx->arena_used;
-  for (int64_t l0 = 0; l0 < loops; l0 += lc) {
+  const bool fused = be_small_loop_applies(N, m, n1);
+  if (fused) {
+    // first level in one kernel: W of every loop and the frame at the base point, nothing else is written
+    cplx* W = (cplx*)be_arena_alloc(ctx, (size_t)loops * m * m * sizeof(cplx));
+    cplx* X0 = (cplx*)be_arena_alloc(ctx, (size_t)loops * N * m * sizeof(cplx));
+    cplx* Vs = (cplx*)be_arena_alloc(ctx, (size_t)loops * m * ns * sizeof(cplx));
+    if (!W || !X0 || !Vs) return BE_ERR_NOMEM;
+    BE_TRY(be_small_loop(ctx, (const cplx*)dH_grid, nullptr, map, N, m, (const cplx*)d_close1, phi_at, nullptr, nullptr, nullptr, W, X0,
+                         nullptr, 0, 0, nullptr, nullptr, nullptr));
+    BE_TRY(be_nested_select_small(ctx, W, loops, m, wb_lo, wb_hi, theta_cut, th1, Vs));
+    ZgemmParams g = zgemm_simple(N, ns, m, X0, N, (int64_t)N * m, Vs, m, (int64_t)m * ns, Wf, N, (int64_t)N * ns, loops);
+    BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_N, g));
+  }
+  for (int64_t l0 = 0; l0 < loops && !fused; l0 += lc) {
     const int64_t nl = (loops - l0 < lc) ? loops - l0 : lc;
     const int64_t cnt = nl * n1;
     ctx->arena_used = keep;
@@ -461,6 +481,14 @@ extern "C" int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid*
     BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_N, g));
   }
   ctx->arena_used = keep;
+  if (be_small_loop_applies(N, ns, n2)) {
+    // second level on the Wannier-band frames in one kernel as well
+    GridMap m2;
+    memset(&m2, 0, sizeof(m2));
+    m2.ndim = 1; m2.dir = 0; m2.n1 = n2; m2.dims[0] = n2; m2.stride[0] = 1; m2.batch_stride = n2; m2.loops = outer2;
+    return be_small_loop(ctx, nullptr, Wf, m2, N, ns, (const cplx*)d_close2, n2 - 1, d_theta_nested, nullptr, nullptr, nullptr,
+                         nullptr, nullptr, 0, 0, nullptr, nullptr, nullptr);
+  }
   cplx* W2 = nullptr;
   BE_TRY(be_chain_product(ctx, Wf, N, ns, outer2, n2, (const cplx*)d_close2, n2 - 1, nullptr, &W2));
   BE_TRY(be_eigenphases(ctx, W2, outer2, ns, d_theta_nested, nullptr));
@@ -521,7 +549,7 @@ extern "C" int be_plaquette_flux(be_ctx* ctx, const void* dH_grid, const be_grid
   const size_t need = (size_t)cnt * (be_eigh_scratch_bytes(1, N, m) + 2 * (size_t)N * m * sizeof(cplx) + N * sizeof(double) +
                                      (dS ? (size_t)N * m * sizeof(cplx) + 3 * mmax + be_eigh_scratch_bytes(1, m, m) : 0) +
                                      6 * mmax + 4096) + (8 << 20);
-  if (need > be_effective_ws_limit(ctx)) return BE_ERR_UNSUPPORTED;   // the grid has to fit one chunk (header)
+  if (need > be_effective_ws_limit(ctx, need)) return BE_ERR_UNSUPPORTED;   // the grid has to fit one chunk (header)
   BE_TRY(be_arena_reserve(ctx, need));
   double* E = (double*)be_arena_alloc(ctx, (size_t)cnt * N * sizeof(double));
   cplx* X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));

@@ -123,7 +123,7 @@ struct be_device_guard {
 // bump allocator on the context arena; pointers stay valid until arena_reset
 int  be_arena_reserve(be_ctx* ctx, size_t bytes);   // ensure capacity (may sync + realloc); resets
 void* be_arena_alloc(be_ctx* ctx, size_t bytes);
-size_t be_effective_ws_limit(be_ctx* ctx);          // min(configured cap, what the device can give now)    // 256-byte aligned; NULL when exhausted
+size_t be_effective_ws_limit(be_ctx* ctx, size_t want);   // min(configured cap, what the device can give now); want = the uncapped request    // 256-byte aligned; NULL when exhausted
 static inline size_t be_align256(size_t b) { return (b + 255) & ~(size_t)255; }
 
 // ---------------------------------------------------------------------------------------------
@@ -234,6 +234,11 @@ size_t be_nested_general_scratch_bytes(int64_t nl, int m, int ns);
 int be_nested_select_general(be_ctx* ctx, cplx* W, int64_t nl, int m, int wb_lo, int wb_hi, double cut,
                              double* theta1, cplx* Vs);
 
+// fused tiny-N loop (small_loop.cu): N <= 8, m <= 2; plain (theta / abs / mingap / W / first frame) or spin resolved
+bool be_small_loop_applies(int N, int m, int n1);
+int be_small_loop(be_ctx* ctx, const cplx* H, const cplx* frames, const GridMap& map, int N, int m, const cplx* d_close, int phi_at,
+                  double* d_theta, double* d_abs, double* d_mingap, cplx* Wout, cplx* X0, const void* dS, int S_is_diag,
+                  int m_lo, double* d_theta_lo, double* d_theta_hi, double* d_pso);
 int be_eigh_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N,
                   int nv, double* E, cplx* X, int* info);
 int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N,

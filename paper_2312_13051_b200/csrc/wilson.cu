@@ -158,14 +158,18 @@ int be_nested_select_small(be_ctx* ctx, const cplx* W, int64_t cnt, int m, int w
 
 // Chain of one chunk: frames F [outer][inner][m][N] (column-major N x m each, ld N) ->
 // links M_j = F_j^H F_{j+1} (ring, Phi on the link at inner index phi_at) -> ordered product
-// W = M_0 M_1 ... M_{n1-1} per outer.  Returns W (column-major m x m, stride m*m) in *Wout; when
-// Wdst is not NULL the final product is written there (a buffer that outlives the chunk).
+// W = M_0 M_1 ... M_{n1-1} per outer.  The product is a pairwise tree, P_j <- P_2j P_2j+1 level by level
+// (ceil(log2 n1) batched GEMM launches instead of n1 - 1 dependent ones; an odd last factor is carried
+// over): PAPER.md:32, 36-38 fix the ORDER of the factors, which a tree of adjacent pairs keeps.
+// Returns W (column-major m x m, stride m*m) in *Wout; when Wdst is not NULL the final product is written
+// there (a buffer that outlives the chunk).
 int be_chain_product(be_ctx* ctx, const cplx* F, int N, int m, int64_t outer, int n1,
                      const cplx* d_close, int phi_at, cplx* Wdst, cplx** Wout) {
   const int64_t mm = (int64_t)m * m;
+  const int half = (n1 + 1) / 2;
   cplx* M = (cplx*)be_arena_alloc(ctx, (size_t)outer * n1 * mm * sizeof(cplx));
-  cplx* W0 = (cplx*)be_arena_alloc(ctx, (size_t)outer * mm * sizeof(cplx));
-  cplx* W1 = (cplx*)be_arena_alloc(ctx, (size_t)outer * mm * sizeof(cplx));
+  cplx* W0 = (cplx*)be_arena_alloc(ctx, (size_t)outer * half * mm * sizeof(cplx));
+  cplx* W1 = (cplx*)be_arena_alloc(ctx, (size_t)outer * ((half + 1) / 2) * mm * sizeof(cplx));
   if (!M || !W0 || !W1) return BE_ERR_NOMEM;
   ZgemmParams g;
   g.M = m; g.N = m; g.K = N;
@@ -183,15 +187,21 @@ int be_chain_product(be_ctx* ctx, const cplx* F, int N, int m, int64_t outer, in
     *Wout = dst;
     return BE_OK;
   }
-  const cplx* cur = M;            // running product, stride curs
-  int64_t curs = (int64_t)n1 * mm;
+  const cplx* cur = M;            // cnt factors per loop, contiguous: cur[o][j]
+  int cnt = n1, level = 0;
   cplx* bufs[2] = {W0, W1};
-  for (int j = 1; j < n1; ++j) {
-    cplx* dst = (j == n1 - 1 && Wdst) ? Wdst : bufs[j & 1];
-    ZgemmParams p = zgemm_simple(m, m, m, cur, m, curs, M + (int64_t)j * mm, m, (int64_t)n1 * mm,
-                                 dst, m, mm, outer);
+  while (cnt > 1) {
+    const int pairs = cnt / 2, ncnt = pairs + (cnt & 1);
+    cplx* dst = (ncnt == 1 && Wdst) ? Wdst : bufs[level & 1];
+    ZgemmParams p = zgemm_simple(m, m, m, cur, m, (int64_t)cnt * mm, cur + mm, m, (int64_t)cnt * mm,
+                                 dst, m, (int64_t)ncnt * mm, (int64_t)outer * pairs);
+    p.sAi = 2 * mm; p.sBi = 2 * mm; p.sCi = mm; p.inner = pairs;
     BE_TRY(be_zgemm(ctx, BE_OP_N, BE_OP_N, p));
-    cur = dst; curs = mm;
+    if (cnt & 1)   // the unpaired last factor moves up unchanged
+      BE_CUDA(cudaMemcpy2DAsync(dst + (int64_t)pairs * mm, (size_t)ncnt * mm * sizeof(cplx), cur + (int64_t)(cnt - 1) * mm,
+                                (size_t)cnt * mm * sizeof(cplx), (size_t)mm * sizeof(cplx), (size_t)outer,
+                                cudaMemcpyDeviceToDevice, ctx->stream));
+    cur = dst; cnt = ncnt; ++level;
   }
   *Wout = (cplx*)cur;
   return BE_OK;
