@@ -22,7 +22,16 @@
  *    *_host entry points are synchronous: they return after the host outputs are written.
  *  - Errors: return value 0 = BE_OK; negative = argument / shape / alignment error detected on the
  *    host before anything is enqueued; positive = CUDA runtime error (cudaError_t value).
- *    Numerical trouble is never an error return: see d_info / d_mingap.
+ *    Size limits (BE_ERR_UNSUPPORTED, checked before anything is enqueued): N <= 6400 for every entry
+ *    point that diagonalizes H, n_occ (bands of a Wilson matrix) <= 2048.
+ *    Numerical trouble is never an error return: be_eigh_batched reports it per matrix in d_info; the
+ *    Wilson entry points (be_wilson_loop*, be_spin_resolved_wilson*) have no d_info, so the phases of
+ *    every loop (sector) with a flagged eigensolve of H or of the projected spin operator (inverse
+ *    iteration / cluster orthogonalization failure, non-finite eigenvalue) or a Wilson matrix whose QR
+ *    iteration did not converge come back as NaN -- never as plausible numbers.  d_mingap flags loops
+ *    without a spectral gap.
+ *  - Devices: a context belongs to the device that was current in be_create; every entry point makes that
+ *    device current for its duration and restores the caller's.
  *  - Thread safety: one context per host thread; no global state.
  *  - Phases are returned in radians, ascending, on the branch (-pi, pi] (R7).  The library's
  *    W = prod_j U_j^dagger U_{j+1} is the Hermitian conjugate of the paper's product (Eq. 2,

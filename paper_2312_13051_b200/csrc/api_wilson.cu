@@ -6,6 +6,7 @@
 
 int be_mingap(be_ctx* ctx, const double* E, int N, int lo, int hi, int n1, int64_t loops, double* out);
 int be_scale_rows(be_ctx* ctx, const cplx* X, const double* S, cplx* SX, int N, int64_t total);
+int be_flag_loops(be_ctx* ctx, const int* info, const double* E, int ldE, int n1, int64_t nl, int* bad0, int* bad1);
 int be_nested_select_small(be_ctx* ctx, const cplx* W, int64_t cnt, int m, int wb_lo, int wb_hi,
                            double cut, double* theta1, cplx* Vs);
 int be_chain_product(be_ctx* ctx, const cplx* F, int N, int m, int64_t outer, int n1,
@@ -56,7 +57,7 @@ static size_t per_loop_bytes(int N, int m, int n1, bool spin, int lo = 0) {
 // S6, first half: S_red = U^H S U for cnt frames X, S_red = V Sigma V^H (ascending).
 // pso_out [cnt][m] receives Sigma (or scratch when NULL); *Vout [cnt][m][m] column-major.
 static int pso_eigenvectors(be_ctx* ctx, const cplx* X, int64_t cnt, int N, int m, const SpinArgs* sp,
-                            double* pso_out, cplx** Vout) {
+                            double* pso_out, cplx** Vout, int* info, double** sig_out) {
   cplx* SX = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
   cplx* Sred = (cplx*)be_arena_alloc(ctx, (size_t)cnt * m * m * sizeof(cplx));
   cplx* V = (cplx*)be_arena_alloc(ctx, (size_t)cnt * m * m * sizeof(cplx));
@@ -81,14 +82,15 @@ static int pso_eigenvectors(be_ctx* ctx, const cplx* X, int64_t cnt, int N, int 
   GridMap fm;
   memset(&fm, 0, sizeof(fm));
   fm.ndim = 1; fm.dir = 0; fm.n1 = 1; fm.dims[0] = 1; fm.batch_stride = 1; fm.loops = cnt;
-  BE_TRY(be_eigh_frames(ctx, Sred, fm, 0, cnt, m, m, m, sig, V, nullptr));
+  BE_TRY(be_eigh_frames(ctx, Sred, fm, 0, cnt, m, m, m, sig, V, info));
   *Vout = V;
+  if (sig_out) *sig_out = sig;
   return BE_OK;
 }
 
 static int wilson_chunk(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t gl0, int N, int m, int n1, int64_t l0,
                         int64_t nl, int64_t cnt, const cplx* d_close, double* d_mingap, const SpinArgs* sp, int mlo,
-                        int mhi, cplx* const* Wall);
+                        int mhi, cplx* const* Wall, int* bad, int64_t loops);
 
 static int pipeline_init(be_ctx* ctx) {
   if (ctx->stream2) return BE_OK;
@@ -159,7 +161,7 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   size_t persist = 0;
   for (int s = 0; s < 2; ++s)
     persist += be_align256((size_t)loops * msec[s] * msec[s] * sizeof(cplx)) + be_eigenphases_scratch_bytes(2 * loops, msec[s]) +
-               be_align256(2 * (size_t)loops * msec[s] * sizeof(double)) + 1024;
+               be_align256(2 * (size_t)loops * msec[s] * sizeof(double)) + be_align256(2 * (size_t)loops * sizeof(int)) + 1024;
   // Chunk pipeline (more than one chunk): two scratch regions used alternately, the
   // tridiagonalization of chunk c+1 on the caller's stream overlaps the rest of chunk c on stream2.
   const size_t region = be_align256(per * (size_t)lc);
@@ -222,6 +224,9 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
         if (!Wall[s]) return BE_ERR_NOMEM;
       }
   }
+  int* bad = (int*)be_arena_alloc(ctx, 2 * (size_t)loops * sizeof(int));
+  if (!bad) return BE_ERR_NOMEM;
+  BE_CUDA(cudaMemsetAsync(bad, 0, 2 * (size_t)loops * sizeof(int), ctx->stream));
   const size_t keep = ctx->arena_used;
   for (int64_t ci = 0; ci < nchunks; ++ci) {
     const int64_t l0 = cstart[ci], nl = cstart[ci + 1] - l0;
@@ -241,7 +246,7 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
     }
     ctx->bloch = bs;   // consumed (and cleared) by the H eigensolve of the chunk
     const int rc = wilson_chunk(ctx, Hc, hs ? smap : map, hs ? 0 : l0, N, m, n1, l0, nl, cnt, d_close, d_mingap, sp, mlo,
-                                mhi, Wall);
+                                mhi, Wall, bad, loops);
     ctx->bloch = nullptr;
     if (hs && rc == BE_OK) cudaEventRecord(hs->freed[ci & 1], ctx->stream);
     if (pipe) {
@@ -254,20 +259,20 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   ctx->arena_used = keep;
   int rc = BE_OK;
   if (!sp) {
-    rc = be_eigenphases(ctx, Wall[0], loops, m, d_theta, d_abs);
+    rc = be_eigenphases(ctx, Wall[0], loops, m, d_theta, d_abs, bad);
   } else if (joint) {
     // the solve is latency bound per matrix: 2 x loops matrices in one launch cost what loops do
     const size_t nb = (size_t)loops * msec[0] * sizeof(double);
     double* th = (double*)be_arena_alloc(ctx, 2 * nb);
     if (!th) rc = BE_ERR_NOMEM;
-    if (rc == BE_OK) rc = be_eigenphases(ctx, Wall[0], 2 * loops, msec[0], th, nullptr);
+    if (rc == BE_OK) rc = be_eigenphases(ctx, Wall[0], 2 * loops, msec[0], th, nullptr, bad);
     if (rc == BE_OK) rc = (int)cudaMemcpyAsync(sp->theta_lo, th, nb, cudaMemcpyDeviceToDevice, ctx->stream);
     if (rc == BE_OK) rc = (int)cudaMemcpyAsync(sp->theta_hi, (char*)th + nb, nb, cudaMemcpyDeviceToDevice, ctx->stream);
   } else {
     for (int sector = 0; sector < 2 && rc == BE_OK; ++sector) {
       double* out = sector == 0 ? sp->theta_lo : sp->theta_hi;
       if (msec[sector] == 0 || !out) continue;
-      rc = be_eigenphases(ctx, Wall[sector], loops, msec[sector], out, nullptr);
+      rc = be_eigenphases(ctx, Wall[sector], loops, msec[sector], out, nullptr, bad + sector * loops);
     }
   }
   if (pipe) {   // join: the caller's stream waits for everything enqueued on stream2
@@ -283,17 +288,20 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
 // gl0: first loop of the chunk inside (H, map); l0: first loop of the chunk in the outputs.
 static int wilson_chunk(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t gl0, int N, int m, int n1, int64_t l0,
                         int64_t nl, int64_t cnt, const cplx* d_close, double* d_mingap, const SpinArgs* sp, int mlo,
-                        int mhi, cplx* const* Wall) {
+                        int mhi, cplx* const* Wall, int* bad, int64_t loops) {
   {
     const int lo = ctx->band_lo, hi = lo + m;   // band window [lo, hi): the lowest hi vectors are computed
     double* E = (double*)be_arena_alloc(ctx, (size_t)cnt * N * sizeof(double));
     cplx* X = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * hi * sizeof(cplx));
-    if (!E || !X) return BE_ERR_NOMEM;
+    int* info = (int*)be_arena_alloc(ctx, (size_t)cnt * sizeof(int));
+    if (!E || !X || !info) return BE_ERR_NOMEM;
     {
-      const int r = be_eigh_frames(ctx, H, map, gl0, cnt, N, hi, hi + 1, E, X, nullptr);
+      const int r = be_eigh_frames(ctx, H, map, gl0, cnt, N, hi, hi + 1, E, X, info);
       ctx->bloch = nullptr;   // only H(k) is generated; the PSO solve below reads S_red from memory
       BE_TRY(r);
     }
+    // loops with a flagged eigensolve get NaN phases at the end (bad[0 .. loops) lower / plain, [loops ..) upper)
+    BE_TRY(be_flag_loops(ctx, info, E, N, n1, nl, bad + l0, sp ? bad + loops + l0 : nullptr));
     if (d_mingap) BE_TRY(be_mingap(ctx, E, N, lo, hi, n1, nl, d_mingap + l0));
     if (lo > 0) {
       // frames are column-major N x hi per k-point: columns lo .. hi-1 are one contiguous run per frame
@@ -309,7 +317,9 @@ static int wilson_chunk(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t 
       return BE_OK;
     }
     cplx* V = nullptr;
-    BE_TRY(pso_eigenvectors(ctx, X, cnt, N, m, sp, sp->pso ? sp->pso + l0 * (int64_t)n1 * m : nullptr, &V));
+    double* sig = nullptr;
+    BE_TRY(pso_eigenvectors(ctx, X, cnt, N, m, sp, sp->pso ? sp->pso + l0 * (int64_t)n1 * m : nullptr, &V, info, &sig));
+    BE_TRY(be_flag_loops(ctx, info, sig, m, n1, nl, bad + l0, bad + loops + l0));
     for (int sector = 0; sector < 2; ++sector) {
       const int ms = sector == 0 ? mlo : mhi;
       double* out = sector == 0 ? sp->theta_lo : sp->theta_hi;
@@ -336,6 +346,9 @@ static int check_common(be_ctx* ctx, const void* H, const be_grid* g, int n_occ,
   if (dir < 0 || dir >= g->ndim) return BE_ERR_SHAPE;
   if (n_occ < 1 || n_occ > g->N) return BE_ERR_SHAPE;
   if (!aligned(H, 16)) return BE_ERR_ALIGN;
+  // size limits of the kernels, checked before anything is enqueued: the blocked eigensolver keeps two vectors of
+  // length N in shared memory (N <= 6400), the QR iteration of the Wilson matrix owns columns in registers (m <= 2048)
+  if (g->N > BE_MAX_N || n_occ > BE_MAX_M) return BE_ERR_UNSUPPORTED;
   return BE_OK;
 }
 
@@ -558,7 +571,7 @@ extern "C" int be_plaquette_flux(be_ctx* ctx, const void* dH_grid, const be_grid
   if (!dS) return plaquette_of_frames(ctx, X, grid->batch, ny, nx, N, m, d_flux);
   SpinArgs sp{dS, S_is_diag, m_lo, nullptr, nullptr, d_pso};
   cplx* V = nullptr;
-  BE_TRY(pso_eigenvectors(ctx, X, cnt, N, m, &sp, d_pso, &V));
+  BE_TRY(pso_eigenvectors(ctx, X, cnt, N, m, &sp, d_pso, &V, nullptr, nullptr));
   const int msz[2] = {m_lo, m - m_lo};
   double* outs[2] = {d_flux, d_flux_hi};
   for (int sector = 0; sector < 2; ++sector) {

@@ -225,7 +225,7 @@ size_t be_eigh_scratch_bytes(int64_t cnt, int N, int nv);
 
 // eigenphases of ``cnt`` general complex m x m matrices W (column-major, stride m*m, destroyed):
 //   theta [cnt][m] ascending in (-pi, pi], absl [cnt][m] or NULL.
-int be_eigenphases(be_ctx* ctx, cplx* W, int64_t cnt, int m, double* theta, double* absl);
+int be_eigenphases(be_ctx* ctx, cplx* W, int64_t cnt, int m, double* theta, double* absl, const int* bad = nullptr);
 size_t be_eigenphases_scratch_bytes(int64_t cnt, int m);
 int be_eigenvalues_general(be_ctx* ctx, cplx* W, int64_t cnt, int m, cplx* lam, int* fail);
 int be_sort_phases(be_ctx* ctx, const cplx* lam, int64_t cnt, int m, double* theta, double* absl);
@@ -250,6 +250,8 @@ constexpr int BE_BAND_MINN = 128, BE_BAND_MAXN = 2048, BE_BAND_AUTON = 1024;
 size_t be_band_scratch_bytes(int64_t cnt, int N);
 int be_band_reduce(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double* e, cplx* tau, void* scratch);
 int be_band_q2(be_ctx* ctx, const cplx* Bw, cplx* X, int64_t cnt, int N, int nv);
+constexpr int BE_MAX_N = 6400;   // largest matrix order of the blocked eigensolver (be_eigh_batched, every Wilson entry point)
+constexpr int BE_MAX_M = 2048;   // largest Wilson matrix (bands per sector) of the eigenphase solve
 constexpr int TS_MAXN = 104;   // largest matrix reduced entirely in shared memory (tridiag_small.cu)
 int be_tridiag_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0, int64_t cnt, int N, cplx* Bw,
                      double* d, double* e, cplx* tau, int p0 = 0);

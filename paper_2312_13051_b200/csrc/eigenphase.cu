@@ -450,13 +450,30 @@ int be_eigenvalues_general(be_ctx* ctx, cplx* W, int64_t cnt, int m, cplx* lam, 
   return (int)cudaGetLastError();
 }
 
-int be_eigenphases(be_ctx* ctx, cplx* W, int64_t cnt, int m, double* theta, double* absl) {
+// Numerical trouble must not come back as plausible numbers with rc = 0: the phases of a Wilson matrix whose QR
+// iteration gave up (fail), or one of whose eigensolves upstream was flagged (bad: inverse iteration / cluster
+// orthogonalization failures, non-finite eigenvalues), are replaced by NaN.
+__global__ void k_poison(double* __restrict__ theta, double* __restrict__ absl, const int* __restrict__ fail,
+                         const int* __restrict__ bad, int64_t cnt, int m) {
+  const int64_t c = blockIdx.x;
+  if (!(fail[c] || (bad && bad[c]))) return;
+  for (int k = threadIdx.x; k < m; k += blockDim.x) {
+    theta[c * m + k] = nan("");
+    if (absl) absl[c * m + k] = nan("");
+  }
+}
+
+int be_eigenphases(be_ctx* ctx, cplx* W, int64_t cnt, int m, double* theta, double* absl, const int* bad) {
   if (cnt <= 0 || m <= 0) return BE_OK;
   cplx* lam = (cplx*)be_arena_alloc(ctx, (size_t)cnt * m * sizeof(cplx));
   int* fail = (int*)be_arena_alloc(ctx, (size_t)cnt * sizeof(int));
   if (!lam || !fail) return BE_ERR_NOMEM;
+  BE_CUDA(cudaMemsetAsync(fail, 0, (size_t)cnt * sizeof(int), ctx->stream));
   BE_TRY(be_eigenvalues_general(ctx, W, cnt, m, lam, fail));
-  return be_sort_phases(ctx, lam, cnt, m, theta, absl);
+  BE_TRY(be_sort_phases(ctx, lam, cnt, m, theta, absl));
+  k_poison<<<(unsigned)cnt, 64, 0, ctx->stream>>>(theta, absl, fail, bad, cnt, m);
+  ctx->launches++;
+  return (int)cudaGetLastError();
 }
 
 int be_sort_phases(be_ctx* ctx, const cplx* lam, int64_t cnt, int m, double* theta, double* absl) {

@@ -21,6 +21,20 @@ __global__ void k_mingap(const double* __restrict__ E, int N, int lo, int hi, in
   out[l] = g;
 }
 
+// bad[l] |= any eigensolve of loop l was flagged (info != 0) or returned a non-finite lowest eigenvalue
+__global__ void k_flag_loops(const int* __restrict__ info, const double* __restrict__ E, int ldE, int n1, int64_t nl,
+                             int* __restrict__ bad0, int* __restrict__ bad1) {
+  const int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (l >= nl) return;
+  int f = 0;
+  for (int j = 0; j < n1; ++j) {
+    const int64_t c = l * n1 + j;
+    if (info[c]) f = 1;
+    if (E && !isfinite(E[c * ldE])) f = 1;
+  }
+  if (f) { bad0[l] = 1; if (bad1) bad1[l] = 1; }
+}
+
 // SX[c][v][r] = S[r] * X[c][v][r] for a real diagonal S.
 __global__ void k_scale_rows(const cplx* __restrict__ X, const double* __restrict__ S,
                              cplx* __restrict__ SX, int N, int64_t total) {
@@ -133,6 +147,12 @@ __global__ void k_nested_select_small(const cplx* __restrict__ W, int64_t cnt, i
 
 int be_mingap(be_ctx* ctx, const double* E, int N, int lo, int hi, int n1, int64_t loops, double* out) {
   k_mingap<<<(unsigned)((loops + 127) / 128), 128, 0, ctx->stream>>>(E, N, lo, hi, n1, loops, out);
+  LAUNCH_CHECK();
+  return BE_OK;
+}
+
+int be_flag_loops(be_ctx* ctx, const int* info, const double* E, int ldE, int n1, int64_t nl, int* bad0, int* bad1) {
+  k_flag_loops<<<(unsigned)((nl + 127) / 128), 128, 0, ctx->stream>>>(info, E, ldE, n1, nl, bad0, bad1);
   LAUNCH_CHECK();
   return BE_OK;
 }

@@ -180,6 +180,36 @@ def test_eigh_edge_cases(ctx):
     assert torch.equal(E1, E2)
 
 
+def test_numerical_trouble_comes_back_as_nan_not_as_numbers(ctx):
+    """the Wilson entry points have no d_info.  A loop one of whose matrices cannot be diagonalized
+    (here: a NaN entry; the same flag carries inverse-iteration / QR non-convergence) returns NaN phases, the
+    other loops are untouched -- on the Jacobi + general path (N = 9 > 8 forces it), the blocked path and the
+    spin-resolved call."""
+    rng = np.random.default_rng(11)
+    for N, m in ((9, 3), (144, 72)):
+        if N == 9:
+            H = _random_gapped_grid(12, 5, N=9, m=3, seed=4)
+        else:
+            H = wl.supercell_grid([wl.config3_parts(1, L=6)], 7, 5)[0]
+        tho, _, _ = wo.wilson_surface(H[None], m, 1)
+        Hb = H.copy()
+        Hb[2, 3, 0, 1] = np.nan
+        Hb[2, 3, 1, 0] = np.nan
+        th, ab, mg = ctx.wilson_loop(dev(Hb[None]), m, 1)
+        th = th.cpu().numpy()
+        assert np.all(np.isnan(th[2]))
+        good = [0, 1, 3, 4]
+        assert np.all(np.isfinite(th[good])) and phase_dist(th[good], tho[good]) <= PH_TOL
+    H = wl.supercell_grid([wl.config4_parts(6, axis="x")], 7, 4)[0]
+    S = wl.supercell_spin_z(6)
+    Hb = H.copy()
+    Hb[1, 0, 5, 5] = np.inf
+    lo, hi, pso = ctx.spin_resolved_wilson(dev(Hb[None]), 72, 1, dev(S))
+    lo, hi = lo.cpu().numpy(), hi.cpu().numpy()
+    assert np.all(np.isnan(lo[1])) and np.all(np.isnan(hi[1]))
+    assert np.all(np.isfinite(lo[[0, 2, 3]])) and np.all(np.isfinite(hi[[0, 2, 3]]))
+
+
 def test_error_codes(ctx):
     from paper_2312_13051_b200.binding import BerryEasyError
     H = dev(wl.config1_grid(4, 3)[None])
