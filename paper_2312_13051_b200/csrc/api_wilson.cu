@@ -3,6 +3,7 @@
 #include "be_common.cuh"
 #include <string.h>
 #include <vector>
+#include <algorithm>
 
 int be_mingap(be_ctx* ctx, const double* E, int N, int lo, int hi, int n1, int64_t loops, double* out);
 int be_scale_rows(be_ctx* ctx, const cplx* X, const double* S, cplx* SX, int N, int64_t total);
@@ -136,15 +137,35 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
     lc = (loops + nch - 1) / nch;
     for (int64_t l0 = 0; l0 < loops; l0 += lc) cstart.push_back(l0);
   } else {
-    int64_t l0 = 0, step = (loops + 7) / 8;
-    while (l0 < loops) {
-      cstart.push_back(l0);
-      int64_t c = step < lc ? step : lc;
-      if (loops - l0 - c > 0 && loops - l0 - c < c / 2) c = loops - l0;   // no tiny last chunk
-      if (c > lc) c = lc;
-      l0 += c;
-      step *= 2;
+    // Sizes: the one-CTA-per-matrix kernels of the eigensolver (panel QR, bulge chasing) run in waves of sm_count
+    // matrices, so chunks of just under 1, 2, 3, .. waves (5, 8, 11 loops of 25 points on 148 SMs), ascending;
+    // matrices too small for that to matter: 1/8 of the loops, then doubling.
+    std::vector<int64_t> sz;
+    const int64_t w1 = ctx->sm_count / n1;
+    if (N > TS_MAXN && w1 >= 1 && w1 < loops) {
+      int64_t left = loops;
+      for (int k = 1; left > 0; ++k) {
+        int64_t c = (int64_t)k * ctx->sm_count / n1;
+        if (c > lc) c = lc;
+        if (c > left) c = left;
+        sz.push_back(c);
+        left -= c;
+      }
+      std::sort(sz.begin(), sz.end());
+    } else {
+      int64_t left = loops, step = (loops + 7) / 8;
+      while (left > 0) {
+        int64_t c = step < lc ? step : lc;
+        if (left - c > 0 && left - c < c / 2) c = left;   // no tiny last chunk
+        if (c > lc) c = lc;
+        if (c > left) c = left;
+        sz.push_back(c);
+        left -= c;
+        step *= 2;
+      }
     }
+    int64_t l0 = 0;
+    for (size_t i = 0; i < sz.size(); ++i) { cstart.push_back(l0); l0 += sz[i]; }
     lc = 0;
     for (size_t i = 0; i < cstart.size(); ++i) {
       const int64_t e = (i + 1 < cstart.size()) ? cstart[i + 1] : loops;
