@@ -14,9 +14,9 @@
 //                        multiplied by the new panel's V from both sides of the symmetry (Y = A V) before
 //                        it leaves the SM.  16 flops per byte of HBM traffic instead of the 1 flop per
 //                        byte of a HEMV.
-//   stage 2  band -> real tridiagonal by bulge chasing (k_chase): one CTA per matrix, one warp per sweep,
-//            sweeps pipelined two chase steps apart; the reflectors (length KB) go to the unused upper
-//            triangle of the work matrix.
+//   stage 2  band -> real tridiagonal by bulge chasing (k_chase4): one CTA per matrix, eight lanes per sweep,
+//            sweeps pipelined two chase steps apart, the band window in a shared-memory ring; the reflectors
+//            (length KB) go to the unused upper triangle of the work matrix.
 //   Q2       X <- conj(Q2) X (k_q2): the N^2 / (2 KB) short reflectors are applied with the eigenvector
 //            entries in registers: a thread owns one column and a sliding window of QG + KB - 1 rows, a
 //            group of QG consecutive sweeps is applied per pass over the column (plain DFMA: on B200 the
@@ -699,30 +699,40 @@ __global__ void k_band_extract(const cplx* __restrict__ Bw, cplx* __restrict__ A
   AB[c * (int64_t)N * LDAB + idx] = v;
 }
 
-// Bulge chasing, one CTA per matrix, one warp per sweep.  The G sweeps i0 .. i0 + G - 1 of a "train" run
-// two chase steps apart (sweep i0 + w does step k = t - 2w at time t), so everything the train touches at
-// time t lies in a window of 15 G + 16 columns of the band, which is kept in a ring buffer in shared memory:
-// per time step 8 columns enter at the front (cp.async, fetched one step ahead) and 8 leave at the back.
-// Step (i, k), reflector on the rows st = i + 1 + k KB ..:
+// Bulge chasing, one CTA per matrix.  The G sweeps i0 .. i0 + G - 1 of a "train" run two chase steps apart
+// (sweep i0 + s does step k = t - 2s at time t), so everything the train touches at time t lies in a window of
+// 15 G + 16 columns of the band, which is kept in a ring buffer in shared memory: per time step 8 columns enter at
+// the front (cp.async, fetched three steps ahead) and 8 leave at the back.  Step (i, k), reflector on the rows
+// st = i + 1 + k KB ..:
 //   k > 0: E = A[R_k, R_{k-1}] <- E H_{k-1};  H_k from E[:, 0];  E <- H_k^H E
 //   k = 0: H_0 from A[R_0, i]
 //   D = A[R_k, R_k] <- H_k^H D H_k
-// Lane (rr = lane & 7, cg = lane >> 3) holds rows rr, columns cg and cg + 4 of a KB x KB block.  The
-// reflector (tau in the head slot) is stored in the upper triangle of the work matrix: V2(i, rho) at
+// The reflector (tau in the head slot) is stored in the upper triangle of the work matrix: V2(i, rho) at
 // Bw[i + rho N], rho = row the entry acts on.
-constexpr int CH_RING = 256;     // columns of the ring buffer (>= 15 G + 16 + 8)
-constexpr int CH_GMAX = 15;
-__global__ void __launch_bounds__(CH_GMAX * 32) k_chase(cplx* __restrict__ ABw, cplx* __restrict__ Bw, double* __restrict__ dd,
-                                                       double* __restrict__ ee, int N) {
+constexpr int CH_RING = 256;     // columns of the ring buffer (>= 15 G + 16 + 8 * 3)
+
+// FOUR sweeps per warp: a group of 8 lanes owns one chase step, lane r its row r of the two KB x KB blocks (E: 8
+// entries, D: the full Hermitian row, 8 entries).  Row-wise products are lane-local, the column-wise ones (v^H E,
+// v^H p) are 8-lane butterflies; the vectors every lane needs in full (v, w, v^H E) go through a few bytes of
+// shared memory per group.  (A first version with one step per WARP, 2 of the 64 block entries per lane, was
+// issue bound at ~450 instructions per step -- ncu, profiles/r02_chase_ncu_details.md: 56 vs 41 ms per 300
+// matrices of N = 1600.)  G = 4 x warps = 12 sweeps in flight, three CTAs per SM.
+constexpr int CH4_WMAX = 3;      // warps per CTA: 12 sweeps in flight, window 15 * 12 + 25 <= CH_RING
+__global__ void __launch_bounds__(CH4_WMAX * 32) k_chase4(cplx* __restrict__ ABw, cplx* __restrict__ Bw, double* __restrict__ dd,
+                                                         double* __restrict__ ee, int N) {
   static_assert(KB == 8, "lane mapping written for KB = 8");
-  extern __shared__ __align__(16) cplx ring[];   // [CH_RING][LDAB]
+  extern __shared__ __align__(16) cplx ring[];   // [CH_RING][LDAB], then the per-group vectors
   const int64_t c = blockIdx.x;
   cplx* __restrict__ abg = ABw + c * (int64_t)N * LDAB;
   cplx* __restrict__ Bc = Bw + c * (int64_t)N * N;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, G = blockDim.x >> 5;
-  const int rr = lane & 7, cg = lane >> 3;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, G = (blockDim.x >> 5) * 4;
+  const int r = lane & 7, grp = lane >> 3, slot = warp * 4 + grp;
+  cplx* vsm = ring + CH_RING * LDAB + slot * 3 * KB;   // v of the current / previous step
+  cplx* zsm = vsm + KB;                                 // v^H E
+  cplx* wsm = vsm + 2 * KB;                             // w of the two-sided update
+  for (int idx = tid; idx < (int)(blockDim.x >> 5) * 4 * 3 * KB; idx += blockDim.x) ring[CH_RING * LDAB + idx] = mkc(0.0, 0.0);
+  __syncthreads();
 #define RG(col, d) ring[((col) & (CH_RING - 1)) * LDAB + (d)]
-  // columns [c0, c1) global -> ring (cp.async, 16 bytes per thread and element)
   auto load_cols = [&](int c0, int c1) {
     if (c1 > N) c1 = N;
     for (int idx = tid; idx < (c1 - c0) * LDAB; idx += blockDim.x) {
@@ -739,67 +749,64 @@ __global__ void __launch_bounds__(CH_GMAX * 32) k_chase(cplx* __restrict__ ABw, 
     }
   };
   for (int i0 = 0; i0 < N - 1; i0 += G) {
-    const int i = i0 + warp;
-    const int T = (N - 1 - i0 + KB - 1) / KB + 2 * (G - 1);   // time steps of this train
-    int back = i0;                                            // columns < back are in memory
-    int front = (i0 + 9 < N) ? i0 + 9 : N;                    // columns < front are in the ring (or on their way)
+    const int i = i0 + slot;
+    const int T = (N - 1 - i0 + KB - 1) / KB + 2 * (G - 1);
+    int back = i0;
+    // columns enter three time steps before they are needed (an L2 round trip is longer than a step)
+    int front = (i0 + 9 + 16 < N) ? i0 + 9 + 16 : N;
     load_cols(i0, front);
     asm volatile("cp.async.commit_group;\n" ::: "memory");
-    cplx vprev = mkc(0.0, 0.0), tauprev = mkc(0.0, 0.0);
+    asm volatile("cp.async.commit_group;\n" ::: "memory");
+    asm volatile("cp.async.commit_group;\n" ::: "memory");
+    cplx tauprev = mkc(0.0, 0.0);
     for (int t = 0; t < T; ++t) {
-      asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+      asm volatile("cp.async.wait_group 2;\n" ::: "memory");
       __syncthreads();
       {
-        // the columns of the next step enter; those the last sweep left two steps ago go back to memory
-        const int nf = (i0 + 8 * (t + 1) + 9 < N) ? i0 + 8 * (t + 1) + 9 : N;
+        const int nf = (i0 + 8 * (t + 3) + 9 < N) ? i0 + 8 * (t + 3) + 9 : N;
         if (nf > front) { load_cols(front, nf); front = nf; }
         asm volatile("cp.async.commit_group;\n" ::: "memory");
-        int nb = i0 + G + 8 * (t - 2 * (G - 1)) - 16;         // st of the last sweep at time t, minus 16
+        int nb = i0 + G + 8 * (t - 2 * (G - 1)) - 16;
         if (nb > front) nb = front;
         if (nb > back) { store_cols(back, nb); back = nb; }
       }
-      const int k = t - 2 * warp;
-      if (i >= N - 1 || k < 0) continue;
+      const int k = t - 2 * slot;
       const int st = i + 1 + k * KB;
-      if (st >= N) continue;
-      const int len = (N - st < KB) ? N - st : KB;
-      cplx e0 = mkc(0.0, 0.0), e1 = mkc(0.0, 0.0), d0 = mkc(0.0, 0.0), d1 = mkc(0.0, 0.0), x = mkc(0.0, 0.0);
-      if (k > 0 && rr < len) {
-        e0 = RG(st - KB + cg, KB + rr - cg);
-        e1 = RG(st - KB + cg + 4, KB + rr - cg - 4);
-      }
-      if (rr < len) {
-        // full Hermitian block from the stored lower triangle: one load, conjugated above the diagonal
-        if (cg < len) {
-          const bool lo = rr >= cg;
-          const int cc_ = lo ? st + cg : st + rr, oo_ = lo ? rr - cg : cg - rr;
-          d0 = RG(cc_, oo_);
-          if (!lo) d0.y = -d0.y;
-        }
-        if (cg + 4 < len) {
-          const bool lo = rr >= cg + 4;
-          const int cc_ = lo ? st + cg + 4 : st + rr, oo_ = lo ? rr - cg - 4 : cg + 4 - rr;
-          d1 = RG(cc_, oo_);
-          if (!lo) d1.y = -d1.y;
+      const bool act = (i < N - 1) && (k >= 0) && (st < N);
+      // whole warp idle: nothing to do (uniform)
+      if (!__any_sync(0xffffffffu, act)) continue;
+      const int len = act ? ((N - st < KB) ? N - st : KB) : 0;
+      const bool first = (k == 0);
+      const bool rowok = r < len;
+      // ---- loads: row r of E (k > 0) or the entry of column i (k = 0), and the full row r of D
+      cplx e[KB], d[KB];
+#pragma unroll
+      for (int cc = 0; cc < KB; ++cc) {
+        e[cc] = mkc(0.0, 0.0); d[cc] = mkc(0.0, 0.0);
+        if (rowok && !first) e[cc] = RG(st - KB + cc, KB + r - cc);
+        if (rowok && cc < len) {
+          const bool lo = r >= cc;
+          const int c2 = lo ? st + cc : st + r, o2 = lo ? r - cc : cc - r;
+          cplx t2 = RG(c2, o2);
+          if (!lo) t2.y = -t2.y;
+          d[cc] = t2;
         }
       }
-      if (k == 0 && cg == 0 && rr < len) x = RG(i, 1 + rr);
-      if (k > 0) {
-        // E <- E H_{k-1}
-        const cplx vp0 = shfl_c(vprev, cg), vp1 = shfl_c(vprev, cg + 4);
-        cplx wv = cmul(e0, vp0);
-        cfma(wv, e1, vp1);
-        wv = cadd(wv, shfl_xor_c(wv, 8));
-        wv = cadd(wv, shfl_xor_c(wv, 16));
-        const cplx tw = cmul(tauprev, wv);
-        cfms(e0, tw, cconj(vp0));
-        cfms(e1, tw, cconj(vp1));
-        x = e0;   // meaningful on the lanes cg == 0
+      if (rowok && first) e[0] = RG(i, 1 + r);
+      // ---- E <- E H_{k-1}  (v of the previous step is still in vsm; tau = 0 for k = 0)
+      {
+        cplx wv = mkc(0.0, 0.0);
+#pragma unroll
+        for (int cc = 0; cc < KB; ++cc) cfma(wv, e[cc], vsm[cc]);
+        const cplx tw = cmul(first ? mkc(0.0, 0.0) : tauprev, wv);
+#pragma unroll
+        for (int cc = 0; cc < KB; ++cc) cfms(e[cc], tw, cconj(vsm[cc]));
       }
-      // ---- reflector from x (lanes 0..7 hold x[rr])
-      const cplx xr = shfl_c(x, rr);
-      const cplx alpha = shfl_c(x, 0);
-      double xn2 = (rr >= 1 && rr < len) ? cabs2(xr) : 0.0;
+      __syncwarp();
+      // ---- reflector from column 0 of E
+      const cplx x = e[0];
+      const cplx alpha = shfl_c(x, lane & 24);
+      double xn2 = (r >= 1 && rowok) ? cabs2(x) : 0.0;
       xn2 += __shfl_xor_sync(0xffffffffu, xn2, 1);
       xn2 += __shfl_xor_sync(0xffffffffu, xn2, 2);
       xn2 += __shfl_xor_sync(0xffffffffu, xn2, 4);
@@ -809,52 +816,81 @@ __global__ void __launch_bounds__(CH_GMAX * 32) k_chase(cplx* __restrict__ ABw, 
       } else {
         larfg_scalars(alpha, xn2, beta, tau, scale);
       }
-      const cplx v = (rr == 0) ? mkc(1.0, 0.0) : (rr < len ? cmul(xr, scale) : mkc(0.0, 0.0));
-      if (cg == 0 && rr < len) Bc[i + (int64_t)(st + rr) * N] = (rr == 0) ? tau : v;
-      if (k == 0) {
-        if (cg == 0 && rr < len) RG(i, 1 + rr) = (rr == 0) ? mkc(beta, 0.0) : mkc(0.0, 0.0);
-        if (lane == 0) { ee[c * N + i] = beta; dd[c * N + i] = RG(i, 0).x; }
-      } else {
-        // E <- H^H E (column 0 becomes beta e_1)
-        cplx z0 = cmulc(v, e0), z1 = cmulc(v, e1);
+      const cplx v = (r == 0) ? mkc(1.0, 0.0) : (rowok ? cmul(x, scale) : mkc(0.0, 0.0));
+      vsm[r] = v;
+      if (act && rowok) Bc[i + (int64_t)(st + r) * N] = (r == 0) ? tau : v;
+      if (act && first && r == 0) { ee[c * N + i] = beta; dd[c * N + i] = RG(i, 0).x; }
+      // ---- E <- H^H E: z[cc] = sum_r conj(v_r) e_r[cc] by an 8-lane halving butterfly (lane r ends with z[r])
+      {
+        cplx pz[KB];
 #pragma unroll
-        for (int o = 1; o < 8; o <<= 1) { z0 = cadd(z0, shfl_xor_c(z0, o)); z1 = cadd(z1, shfl_xor_c(z1, o)); }
-        const cplx ct = cconj(tau);
-        if (cg == 0) e0 = (rr == 0) ? mkc(beta, 0.0) : mkc(0.0, 0.0);
-        else cfms(e0, cmul(ct, v), z0);
-        cfms(e1, cmul(ct, v), z1);
-        if (rr < len) {
-          RG(st - KB + cg, KB + rr - cg) = e0;
-          RG(st - KB + cg + 4, KB + rr - cg - 4) = e1;
+        for (int cc = 0; cc < KB; ++cc) pz[cc] = cmulc(v, e[cc]);
+        const bool u4 = r & 4, u2 = r & 2, u1 = r & 1;
+        cplx b4[4], b2[2], b1;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const cplx snd = u4 ? pz[j] : pz[j + 4], kp = u4 ? pz[j + 4] : pz[j];
+          b4[j] = cadd(kp, shfl_xor_c(snd, 4));
+        }
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          const cplx snd = u2 ? b4[j] : b4[j + 2], kp = u2 ? b4[j + 2] : b4[j];
+          b2[j] = cadd(kp, shfl_xor_c(snd, 2));
+        }
+        {
+          const cplx snd = u1 ? b2[0] : b2[1], kp = u1 ? b2[1] : b2[0];
+          b1 = cadd(kp, shfl_xor_c(snd, 1));
+        }
+        zsm[r] = b1;   // index (u4 ? 4 : 0) + (u2 ? 2 : 0) + (u1 ? 1 : 0) = r
+      }
+      __syncwarp();
+      cplx vc[KB];
+#pragma unroll
+      for (int cc = 0; cc < KB; ++cc) vc[cc] = vsm[cc];
+      {
+        const cplx ctv = cmul(cconj(tau), v);
+#pragma unroll
+        for (int cc = 1; cc < KB; ++cc) cfms(e[cc], ctv, zsm[cc]);
+        e[0] = (r == 0) ? mkc(beta, 0.0) : mkc(0.0, 0.0);
+      }
+      if (act && rowok) {
+        if (first) RG(i, 1 + r) = e[0];
+        else {
+#pragma unroll
+          for (int cc = 0; cc < KB; ++cc) RG(st - KB + cc, KB + r - cc) = e[cc];
         }
       }
       // ---- D <- H^H D H = D - w v^H - v w^H,  w = tau p - 1/2 |tau|^2 (v^H p) v,  p = D v
       {
-        const cplx vc0 = shfl_c(v, cg), vc1 = shfl_c(v, cg + 4);
-        cplx pp = cmul(d0, vc0);
-        cfma(pp, d1, vc1);
-        pp = cadd(pp, shfl_xor_c(pp, 8));
-        pp = cadd(pp, shfl_xor_c(pp, 16));
-        double al = v.x * pp.x + v.y * pp.y;   // Re(conj(v) p)
+        cplx pp = mkc(0.0, 0.0);
+#pragma unroll
+        for (int cc = 0; cc < KB; ++cc) cfma(pp, d[cc], vc[cc]);
+        double al = v.x * pp.x + v.y * pp.y;
         al += __shfl_xor_sync(0xffffffffu, al, 1);
         al += __shfl_xor_sync(0xffffffffu, al, 2);
         al += __shfl_xor_sync(0xffffffffu, al, 4);
         cplx wv = cmul(tau, pp);
         const double hf = 0.5 * cabs2(tau) * al;
         wv.x -= hf * v.x; wv.y -= hf * v.y;
-        const cplx wc0 = shfl_c(wv, cg), wc1 = shfl_c(wv, cg + 4);
-        cfms(d0, wv, cconj(vc0)); cfms(d0, v, cconj(wc0));
-        cfms(d1, wv, cconj(vc1)); cfms(d1, v, cconj(wc1));
-        if (rr < len) {
-          if (cg < len && rr >= cg) { if (rr == cg) d0.y = 0.0; RG(st + cg, rr - cg) = d0; }
-          if (cg + 4 < len && rr >= cg + 4) { if (rr == cg + 4) d1.y = 0.0; RG(st + cg + 4, rr - cg - 4) = d1; }
+        wsm[r] = wv;
+        __syncwarp();
+#pragma unroll
+        for (int cc = 0; cc < KB; ++cc) {
+          cfms(d[cc], wv, cconj(vc[cc]));
+          cfms(d[cc], v, cconj(wsm[cc]));
+        }
+        if (act && rowok) {
+#pragma unroll
+          for (int cc = 0; cc < KB; ++cc)
+            if (cc <= r && cc < len) { cplx t2 = d[cc]; if (cc == r) t2.y = 0.0; RG(st + cc, r - cc) = t2; }
         }
       }
-      vprev = v; tauprev = tau;
+      tauprev = tau;
+      __syncwarp();
     }
     asm volatile("cp.async.wait_group 0;\n" ::: "memory");
     __syncthreads();
-    store_cols(back, front);   // what is left of the window
+    store_cols(back, front);
     __syncthreads();
   }
   if (tid == 0) { dd[c * N + N - 1] = abg[(int64_t)(N - 1) * LDAB].x; ee[c * N + N - 1] = 0.0; }
@@ -1111,13 +1147,10 @@ int be_band_reduce(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double*
   k_band_extract<<<dim3((unsigned)((N * LDAB + 255) / 256), (unsigned)cnt), 256, 0, st>>>(Bw, s.AB, N);
   LAUNCH_CHECK();
   {
-    // warps (sweeps in flight) per matrix: as many as keep the whole chunk resident in one wave (64 KB of
-    // shared memory and <= 64 registers per thread: 3 CTAs of 10 warps per SM, else 2 of 15)
-    int G = CH_GMAX;
-    if (cnt > 2 * (int64_t)ctx->sm_count) G = 10;
-    BE_CUDA(cudaFuncSetAttribute(k_chase, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(CH_RING * LDAB * sizeof(cplx))));
+    const size_t sm4 = (size_t)(CH_RING * LDAB + CH4_WMAX * 4 * 3 * KB) * sizeof(cplx);
+    BE_CUDA(cudaFuncSetAttribute(k_chase4, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm4));
     be_prof_begin(ctx, PK_CHASE);
-    k_chase<<<(unsigned)cnt, G * 32, CH_RING * LDAB * sizeof(cplx), st>>>(s.AB, Bw, d, e, N);
+    k_chase4<<<(unsigned)cnt, CH4_WMAX * 32, sm4, st>>>(s.AB, Bw, d, e, N);
     be_prof_end(ctx, PK_CHASE, (double)cnt * N * LDAB * 16.0, (double)cnt * 24.0 * N * (double)N * KB);
     LAUNCH_CHECK();
   }
