@@ -421,6 +421,7 @@ def main():
         del H
         r["H"] = None
     torch.cuda.empty_cache()
+    ctx.release_workspace()     # the next workloads' grids (43 GB for config 3) need the memory
 
     # ---- configs 1, 2, 3, 5 (rank 0's numbers; every rank runs them so that the ranks stay in step)
     others = None
@@ -432,6 +433,7 @@ def main():
             r2 = measure(ctx, w2, torch, dist, device, world, max(2, min(args.steps, 3)), 2)
             r2["H"] = None; r2["S"] = None
             torch.cuda.empty_cache()
+            ctx.release_workspace()
             roofs = class_rooflines(r2["prof"], r2["peaks"], hbm_peak, hbm_src)
             dom = max(roofs, key=lambda k: roofs[k]["ms"]) if roofs else None
             tfl = w2.flops / (r2["ms_step"] * 1e-3) / 1e12

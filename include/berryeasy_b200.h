@@ -87,6 +87,11 @@ int be_set_workspace_limit(be_ctx* ctx, size_t bytes);
  * CTA per SM what the overlap gains -- DESIGN.md section 11), hence the default. */
 int be_set_chunk_pipeline(be_ctx* ctx, int on);
 
+/* Frees the scratch the context holds (work arena, host-variant staging buffers); it is re-allocated on
+ * demand by the next call.  Synchronises the context's streams.  For callers that need the device memory
+ * back between calls (the arena of a large call stays allocated otherwise). */
+int be_release_workspace(be_ctx* ctx);
+
 /* Algorithm of the Hermitian tridiagonalization inside S1:
  *   0  one-stage blocked Householder reduction (half of its flops are matrix-vector products streamed
  *      from HBM once per column);

@@ -18,7 +18,7 @@ EXPORTS = [
     "be_create", "be_destroy", "be_strerror", "be_workspace_bytes", "be_set_workspace_limit",
     "be_launch_count", "be_eigh_batched", "be_wilson_loop", "be_nested_wilson",
     "be_spin_resolved_wilson", "be_winding", "be_wilson_loop_host", "be_spin_resolved_wilson_host", "be_nested_wilson_host",
-    "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched", "be_set_chunk_pipeline", "be_set_eigh_algorithm", "be_probe_fp64", "be_bloch_coefficients", "be_assemble_bloch", "be_plaquette_flux", "be_wilson_loop_bloch",
+    "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched", "be_set_chunk_pipeline", "be_set_eigh_algorithm", "be_probe_fp64", "be_release_workspace", "be_bloch_coefficients", "be_assemble_bloch", "be_plaquette_flux", "be_wilson_loop_bloch",
     "be_spin_resolved_wilson_bloch", "be_wilson_loop_window", "be_spin_resolved_wilson_window",
 ]
 
@@ -51,6 +51,7 @@ def load_library():
     lib.be_set_chunk_pipeline.argtypes = [vp, ci]
     lib.be_set_eigh_algorithm.argtypes = [vp, ci]
     lib.be_probe_fp64.argtypes = [vp, ci, C.POINTER(dbl)]
+    lib.be_release_workspace.argtypes = [vp]
     lib.be_bloch_coefficients.argtypes = [vp, vp, C.POINTER(ci), ci, ci, i64, vp]
     lib.be_assemble_bloch.argtypes = [vp, vp, vp, i64, ci, ci, vp]
     lib.be_plaquette_flux.argtypes = [vp, vp, gp, ci, vp, ci, ci, vp, vp, vp]
@@ -153,6 +154,10 @@ class Context:
     def set_eigh_algorithm(self, algo: int):
         """0: one-stage tridiagonalization, 1: two-stage (dense -> band -> tridiagonal) where supported."""
         _check(self.lib, self.lib.be_set_eigh_algorithm(self._h, int(algo)))
+
+    def release_workspace(self):
+        """Give the scratch arena and the staging buffers back to the device (re-allocated on demand)."""
+        _check(self.lib, self.lib.be_release_workspace(self._h))
 
     def probe_fp64(self) -> dict:
         """Measured FP64 rates of this device under the current clocks (TFLOP/s): DMMA chain, DFMA chain with

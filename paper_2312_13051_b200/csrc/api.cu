@@ -194,6 +194,17 @@ extern "C" int be_set_eigh_algorithm(be_ctx* ctx, int algo) {
   return BE_OK;
 }
 
+extern "C" int be_release_workspace(be_ctx* ctx) {
+  BE_DEVICE_GUARD(ctx);
+  if (!ctx) return BE_ERR_NULL;
+  BE_CUDA(cudaStreamSynchronize(ctx->stream));
+  if (ctx->copy_stream) BE_CUDA(cudaStreamSynchronize(ctx->copy_stream));
+  if (ctx->arena) { cudaFree(ctx->arena); ctx->arena = nullptr; ctx->arena_bytes = 0; ctx->arena_used = 0; }
+  for (int i = 0; i < 2; ++i) if (ctx->stage_buf[i]) { cudaFree(ctx->stage_buf[i]); ctx->stage_buf[i] = nullptr; }
+  ctx->stage_cap = 0;
+  return BE_OK;
+}
+
 extern "C" int64_t be_launch_count(const be_ctx* ctx) {
   BE_DEVICE_GUARD(ctx); return ctx ? ctx->launches : 0; }
 

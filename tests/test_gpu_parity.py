@@ -618,7 +618,10 @@ def _bench_workload(cfg):
     return mod.Workload(cfg, 0, False)
 
 
-def _need_memory(gb):
+def _need_memory(gb, ctx=None):
+    if ctx is not None:
+        ctx.release_workspace()          # the arena of an earlier large call stays allocated otherwise
+        torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < gb * 2 ** 30:
         pytest.skip(f"needs {gb} GB of free device memory")
@@ -629,7 +632,7 @@ def test_full_size_config4_in_bench_configuration(ctx):
     workspace cap and eigensolver selection: the two-stage reduction for N = 1600, the one-stage one for the
     PSO): exact invariants on the whole output, and four sampled loops element by element against the
     oracle (one loop of 25 k-points costs the oracle ~15 s)."""
-    _need_memory(30)
+    _need_memory(30, ctx)
     wk = _bench_workload(4)
     H, S = wk.device_grid(torch, torch.device("cuda"))
     lo, hi, pso = wk.run_device(ctx, H, S)
@@ -658,7 +661,7 @@ def test_full_size_config4_spin_mixing_variant_one_loop(ctx):
     """SURVEY 8(d), config 4 "second, harder variant for tests": impurity fields along x do not commute with
     S_z, the PSO eigenvalues leave +-1 and its 800 eigenvectors are non-degenerate -- one whole
     loop (25 k-points) at N = 1600 / m = 800 against the oracle, element by element."""
-    _need_memory(12)
+    _need_memory(12, ctx)
     parts = wl.config4_parts(20, axis="x")
     H = wl.supercell_grid([parts], 25, 24, t2_indices=[7])
     S = wl.supercell_spin_z(20)
@@ -674,7 +677,7 @@ def test_full_size_config3_sampled(ctx):
     """BASELINE.json configs[2] at full size (16 realizations x 32 x 33, N = 400; 43 GB): 32 sampled loops
     against the oracle, sum rule sum_n theta_n = arg det W on all loops is implied by the eigen-solver
     parity; total winding per realization is an exact integer (0: time-reversal symmetric)."""
-    _need_memory(50)
+    _need_memory(50, ctx)
     wk = _bench_workload(3)
     H, _ = wk.device_grid(torch, torch.device("cuda"))
     th, ab, mg = wk.run_device(ctx, H, None)
@@ -693,7 +696,7 @@ def test_full_size_config3_sampled(ctx):
 
 def test_full_size_config5_sampled(ctx):
     """BASELINE.json configs[4] at full size (64 x 64 loops of 65 points, N = 64: 266 240 eigensolves)."""
-    _need_memory(25)
+    _need_memory(25, ctx)
     wk = _bench_workload(5)
     H, _ = wk.device_grid(torch, torch.device("cuda"))
     th, ab, mg = wk.run_device(ctx, H, None)
