@@ -37,7 +37,7 @@ CLASS_BOUND = {"hemv": "hbm", "colw": "hbm", "zgemm": "alu", "fused": "alu", "q2
                "hessenberg": "latency", "hqr": "latency", "jacobi": "hbm", "misc": "hbm"}
 CLASS_KERNEL = {"hemv": "k_hemv", "colw": "k_colw", "zgemm": "zgemm_async_kernel", "fused": "k_fused", "q2": "k_q2",
                 "panel": "k_ysum + k_mc + k_wupd + k_panel", "chase": "k_chase4", "bisect": "k_bisect", "invit": "k_invit",
-                "cluster_orth": "cluster_orth.cu", "hessenberg": "k_hessenberg", "hqr": "k_hqr", "jacobi": "k_jacobi",
+                "cluster_orth": "cluster_orth.cu", "hessenberg": "k_hessenberg", "hqr": "k_hqr", "jacobi": "k_jacobi / k_small_loop",
                 "misc": "k_tridiag_smem"}
 
 
