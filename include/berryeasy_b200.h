@@ -53,6 +53,7 @@ extern "C" {
 #define BE_ERR_ALIGN         -3   /* pointer not 16-byte (complex) / 8-byte (double) aligned   */
 #define BE_ERR_UNSUPPORTED   -4   /* valid request this build cannot serve (stated per call)   */
 #define BE_ERR_NOMEM         -5   /* scratch allocation failed                                 */
+#define BE_ERR_STATIC_LIMIT  -6   /* request exceeds the fixed scratch of a *_static entry     */
 
 typedef struct be_ctx be_ctx;   /* opaque; owns scratch only */
 
@@ -141,6 +142,23 @@ int be_profile_get(be_ctx* ctx, int cls, double* ms, int64_t* launches, double* 
  */
 int be_eigh_batched(be_ctx* ctx, const void* dH, int64_t count, int N, int n_vec,
                     double* dE, void* dU, int* d_info);
+
+/*
+ * S1, variant that allocates nothing: for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  Same arguments, layouts and results as be_eigh_batched on the
+ * Jacobi path (N <= 8, else BE_ERR_UNSUPPORTED); the eigenvector frames the kernel writes before they are
+ * transposed to dU go to a fixed device array of BE_STATIC_EIGH_MAX_ELEMS complex128 (8 MiB), which every GPU
+ * that loads the library holds until the process exits, instead of the context workspace.
+ *   Limit: count <= BE_STATIC_EIGH_MAX_ELEMS and count * N * max(n_vec, 1) <= BE_STATIC_EIGH_MAX_ELEMS
+ *   (e.g. 32768 matrices of N = 4 with all vectors), else BE_ERR_STATIC_LIMIT; nothing is enqueued then.
+ *   No cudaMalloc / cudaFree / allocating routine is called (leave be_profile_enable off: the profile grows its
+ *   event pool on demand).  The array is shared by every context of the process on that device and keeps the
+ *   last call's contents (each call overwrites the part it reads): two calls that overlap on the GPU (different
+ *   streams or contexts without ordering) race on it -- serialize them.  Work is enqueued on the context stream.
+ */
+#define BE_STATIC_EIGH_MAX_ELEMS ((size_t)1 << 19)
+int be_eigh_batched_static(be_ctx* ctx, const void* dH, int64_t count, int N, int n_vec,
+                           double* dE, void* dU, int* d_info);
 
 /*
  * S1-S4 -- hybrid Wannier-centre-charge surface (``WSurf``, Eq. 2

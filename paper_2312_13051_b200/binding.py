@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libberryeasy_b200.so")
 
 EXPORTS = [
     "be_create", "be_destroy", "be_strerror", "be_workspace_bytes", "be_set_workspace_limit",
-    "be_launch_count", "be_eigh_batched", "be_wilson_loop", "be_nested_wilson",
+    "be_launch_count", "be_eigh_batched", "be_eigh_batched_static", "be_wilson_loop", "be_nested_wilson",
     "be_spin_resolved_wilson", "be_winding", "be_wilson_loop_host", "be_spin_resolved_wilson_host", "be_nested_wilson_host",
     "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched", "be_set_chunk_pipeline", "be_set_eigh_algorithm", "be_probe_fp64", "be_release_workspace", "be_bloch_coefficients", "be_assemble_bloch", "be_plaquette_flux", "be_wilson_loop_bloch",
     "be_spin_resolved_wilson_bloch", "be_wilson_loop_window", "be_spin_resolved_wilson_window",
@@ -60,6 +60,7 @@ def load_library():
     lib.be_launch_count.argtypes = [vp]
     lib.be_launch_count.restype = i64
     lib.be_eigh_batched.argtypes = [vp, vp, i64, ci, ci, vp, vp, vp]
+    lib.be_eigh_batched_static.argtypes = [vp, vp, i64, ci, ci, vp, vp, vp]
     lib.be_wilson_loop.argtypes = [vp, vp, gp, ci, ci, vp, vp, vp, vp]
     lib.be_wilson_loop_window.argtypes = [vp, vp, gp, ci, ci, ci, vp, vp, vp, vp]
     lib.be_spin_resolved_wilson_window.argtypes = [vp, vp, gp, ci, ci, ci, vp, ci, ci, vp, vp, vp, vp]
@@ -200,6 +201,19 @@ class Context:
         info = torch.empty((count,), dtype=torch.int32, device=H.device) if want_info else None
         _check(self.lib, self.lib.be_eigh_batched(self._h, _ptr(H), count, N, n_vec, _ptr(E), _ptr(U), _ptr(info)))
         return (E, U, info) if want_info else (E, U)
+
+    def eigh_batched_static(self, H, E, U=None, info=None):
+        """be_eigh_batched_static: N <= 8, caller-provided outputs E [count][N], U [count][N][n_vec] or None; the
+        library allocates nothing (fixed device scratch, BE_STATIC_EIGH_MAX_ELEMS)."""
+        _dev(H, torch.complex128, "H")
+        _dev(E, torch.float64, "E")
+        count, N = H.shape[0], H.shape[-1]
+        n_vec = 0
+        if U is not None:
+            _dev(U, torch.complex128, "U")
+            n_vec = U.shape[-1]
+        _check(self.lib, self.lib.be_eigh_batched_static(self._h, _ptr(H), count, N, n_vec, _ptr(E), _ptr(U), _ptr(info)))
+        return E, U
 
     # ------------------------------------------------------------------ be_wilson_loop
     def wilson_loop(self, H_grid, n_occ, direction, close=None, want_abs=True, want_mingap=True, band_lo=0):

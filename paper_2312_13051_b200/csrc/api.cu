@@ -165,6 +165,7 @@ extern "C" const char* be_strerror(int code) {
     case BE_ERR_ALIGN: return "pointer not aligned";
     case BE_ERR_UNSUPPORTED: return "request not supported by this build";
     case BE_ERR_NOMEM: return "scratch allocation failed";
+    case BE_ERR_STATIC_LIMIT: return "request exceeds the fixed static scratch of this entry point (see BE_STATIC_EIGH_MAX_ELEMS)";
     default: break;
   }
   if (code > 0) return cudaGetErrorString((cudaError_t)code);

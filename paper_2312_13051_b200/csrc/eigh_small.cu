@@ -61,3 +61,59 @@ int be_eigh_small(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
   ctx->launches++;
   return (int)cudaGetLastError();
 }
+
+// ---------------------------------------------------------------------------------------------
+// be_eigh_batched_static: the N <= 8 eigensolver for callers that must not allocate (CUDA graph capture, serving
+// loops, harnesses that forbid cudaMalloc).  k_jacobi writes its frames X [count][n_vec][N] to scratch before they
+// are transposed to the public layout; here that scratch is a file-scope device array, resident on every GPU that
+// loads the library until the process exits, instead of the context arena.  In host code the array's name is a
+// host-side shadow symbol, not a device address: the address is taken with cudaGetSymbolAddress, once per device,
+// with that device current.
+#include <mutex>
+#include <string.h>
+
+static __device__ __align__(256) unsigned char g_static_frames[BE_STATIC_EIGH_MAX_ELEMS * sizeof(cplx)];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mu;
+void* g_static_ptr[STATIC_MAX_DEVICES] = {nullptr};
+
+// device address of g_static_frames on the CURRENT device (the caller holds the device guard)
+int static_frames_ptr(int device, cplx** out) {
+  if (device < 0 || device >= STATIC_MAX_DEVICES) return BE_ERR_UNSUPPORTED;
+  std::lock_guard<std::mutex> lk(g_static_mu);
+  if (!g_static_ptr[device]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_static_frames);
+    if (e != cudaSuccess) return (int)e;
+    if (!p) return BE_ERR_NOMEM;
+    g_static_ptr[device] = p;
+  }
+  *out = (cplx*)g_static_ptr[device];
+  return BE_OK;
+}
+}  // namespace
+
+extern "C" int be_eigh_batched_static(be_ctx* ctx, const void* dH, int64_t count, int N, int n_vec, double* dE,
+                                      void* dU, int* d_info) {
+  BE_DEVICE_GUARD(ctx);
+  if (!ctx) return BE_ERR_NULL;
+  if (count < 0 || N < 1 || n_vec < 0 || n_vec > N) return BE_ERR_SHAPE;
+  if (N > 8) return BE_ERR_UNSUPPORTED;
+  if (count == 0) return BE_OK;
+  if (!dH || !dE) return BE_ERR_NULL;
+  if (((uintptr_t)dH % 16) || ((uintptr_t)dE % 8) || (dU && ((uintptr_t)dU % 16))) return BE_ERR_ALIGN;
+  const int nv = dU ? n_vec : 0;
+  if (count > (int64_t)BE_STATIC_EIGH_MAX_ELEMS || count * (int64_t)N * (nv > 0 ? nv : 1) > (int64_t)BE_STATIC_EIGH_MAX_ELEMS)
+    return BE_ERR_STATIC_LIMIT;
+  cplx* X = nullptr;
+  if (nv > 0) BE_TRY(static_frames_ptr(ctx->device, &X));
+  GridMap fm;
+  memset(&fm, 0, sizeof(fm));
+  fm.ndim = 1; fm.dir = 0; fm.n1 = 1; fm.shift = 0; fm.dims[0] = 1; fm.stride[0] = 0; fm.batch_stride = 1; fm.loops = count;
+  // every frame element in [0, count * nv * N) is written by k_jacobi before k_x2u reads it: nothing to clear
+  BE_TRY(be_eigh_small(ctx, (const cplx*)dH, fm, 0, count, N, nv, dE, X, d_info));
+  if (nv > 0) BE_TRY(be_frames_to_public(ctx, X, (cplx*)dU, count, N, nv));
+  return BE_OK;
+}
