@@ -7,6 +7,9 @@
 
 int be_mingap(be_ctx* ctx, const double* E, int N, int lo, int hi, int n1, int64_t loops, double* out);
 int be_scale_rows(be_ctx* ctx, const cplx* X, const double* S, cplx* SX, int N, int64_t total);
+int be_pack_rows(be_ctx* ctx, const cplx* X, const double* S, const int* sel, double b, cplx* XA, cplx* SXA, int N,
+                 int nsel, int64_t cols);
+int be_add_diag(be_ctx* ctx, cplx* A, int m, int64_t cnt, double b);
 int be_flag_loops(be_ctx* ctx, const int* info, const double* E, int ldE, int n1, int64_t nl, int* bad0, int* bad1);
 int be_nested_select_small(be_ctx* ctx, const cplx* W, int64_t cnt, int m, int wb_lo, int wb_hi,
                            double cut, double* theta1, cplx* Vs);
@@ -36,6 +39,9 @@ static int make_map(const be_grid* g, int dir, GridMap* out) {
 struct SpinArgs {
   const void* dS; int S_is_diag; int m_lo;
   double* theta_lo; double* theta_hi; double* pso;
+  // diagonal S whose most frequent value bval sits on at least half of the rows (set by analyze_diag_S):
+  // sel [nsel] = the other rows, ascending (device)
+  const int* sel; int nsel; double bval;
 };
 
 // bytes of scratch one loop needs (upper bound), plain or spin-resolved
@@ -59,12 +65,18 @@ static size_t per_loop_bytes(int N, int m, int n1, bool spin, int lo = 0) {
 // pso_out [cnt][m] receives Sigma (or scratch when NULL); *Vout [cnt][m][m] column-major.
 static int pso_eigenvectors(be_ctx* ctx, const cplx* X, int64_t cnt, int N, int m, const SpinArgs* sp,
                             double* pso_out, cplx** Vout, int* info, double** sig_out) {
-  cplx* SX = (cplx*)be_arena_alloc(ctx, (size_t)cnt * N * m * sizeof(cplx));
+  const bool packed = sp->S_is_diag && sp->sel != nullptr;
+  const int ks = packed ? sp->nsel : N;    // rows that enter the contraction
+  cplx* SX = (cplx*)be_arena_alloc(ctx, (size_t)cnt * ks * m * sizeof(cplx));
+  cplx* XA = packed ? (cplx*)be_arena_alloc(ctx, (size_t)cnt * ks * m * sizeof(cplx)) : nullptr;
   cplx* Sred = (cplx*)be_arena_alloc(ctx, (size_t)cnt * m * m * sizeof(cplx));
   cplx* V = (cplx*)be_arena_alloc(ctx, (size_t)cnt * m * m * sizeof(cplx));
   double* sig = pso_out ? pso_out : (double*)be_arena_alloc(ctx, (size_t)cnt * m * sizeof(double));
-  if (!SX || !Sred || !V || !sig) return BE_ERR_NOMEM;
-  if (sp->S_is_diag) {
+  if (!SX || !Sred || !V || !sig || (packed && !XA)) return BE_ERR_NOMEM;
+  if (packed) {
+    // U^H S U = b I + U_A^H (S_A - b) U_A (U^H U = I): only the rows with S != b enter the GEMM
+    BE_TRY(be_pack_rows(ctx, X, (const double*)sp->dS, sp->sel, sp->bval, XA, SX, N, ks, cnt * (int64_t)m));
+  } else if (sp->S_is_diag) {
     BE_TRY(be_scale_rows(ctx, X, (const double*)sp->dS, SX, N, cnt * (int64_t)N * m));
   } else {
     // row-major S read column-major is S^T: op T recovers S;  SX = S X
@@ -72,14 +84,17 @@ static int pso_eigenvectors(be_ctx* ctx, const cplx* X, int64_t cnt, int N, int 
                                  SX, N, (int64_t)N * m, cnt);
     BE_TRY(be_zgemm(ctx, BE_OP_T, BE_OP_N, g));
   }
-  {
+  if (ks > 0) {
     // the eigensolver reads its input row-major; a column-major buffer holding conj(S_red) =
     // X^T conj(SX) is S_red when read row-major (S_red is Hermitian)
-    ZgemmParams g = zgemm_simple(m, m, N, X, N, (int64_t)N * m, SX, N, (int64_t)N * m,
+    ZgemmParams g = zgemm_simple(m, m, ks, packed ? XA : X, ks, (int64_t)ks * m, SX, ks, (int64_t)ks * m,
                                  Sred, m, (int64_t)m * m, cnt);
     g.lower = 1;   // the eigensolver reads only the lower triangle of the column-major buffer
     BE_TRY(be_zgemm(ctx, BE_OP_T, BE_OP_J, g));
+  } else {
+    BE_CUDA(cudaMemsetAsync(Sred, 0, (size_t)cnt * m * m * sizeof(cplx), ctx->stream));
   }
+  if (packed) BE_TRY(be_add_diag(ctx, Sred, m, cnt, sp->bval));
   GridMap fm;
   memset(&fm, 0, sizeof(fm));
   fm.ndim = 1; fm.dir = 0; fm.n1 = 1; fm.dims[0] = 1; fm.batch_stride = 1; fm.loops = cnt;
@@ -105,6 +120,34 @@ static int pipeline_init(be_ctx* ctx) {
   return BE_OK;
 }
 
+// Diagonal S: find its most frequent value b; when at least half of the rows carry it, pso_eigenvectors
+// contracts only over the other rows (list written to d_sel).  One small device -> host copy per call.
+static int analyze_diag_S(be_ctx* ctx, SpinArgs* sp, int N, int* d_sel) {
+  std::vector<double> h((size_t)N);
+  BE_CUDA(cudaMemcpyAsync(h.data(), sp->dS, (size_t)N * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+  BE_CUDA(cudaStreamSynchronize(ctx->stream));
+  for (int r = 0; r < N; ++r) if (!(h[r] == h[r])) return BE_OK;   // NaN: leave it to the general path
+  std::vector<double> srt(h);
+  std::sort(srt.begin(), srt.end());
+  double b = srt[0];
+  int best = 0;
+  for (int i = 0; i < N;) {
+    int j = i;
+    while (j < N && srt[j] == srt[i]) ++j;
+    if (j - i > best) { best = j - i; b = srt[i]; }
+    i = j;
+  }
+  if (2 * best < N) return BE_OK;
+  std::vector<int> sel;
+  for (int r = 0; r < N; ++r) if (h[r] != b) sel.push_back(r);
+  if (!sel.empty()) {
+    BE_CUDA(cudaMemcpyAsync(d_sel, sel.data(), sel.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
+    BE_CUDA(cudaStreamSynchronize(ctx->stream));   // sel is a local
+  }
+  sp->sel = d_sel; sp->nsel = (int)sel.size(); sp->bval = b;
+  return BE_OK;
+}
+
 // One pass over all loops of ``map`` (device H).  Plain loop when ``sp`` is NULL.
 static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, int m,
                          const cplx* d_close, double* d_theta, double* d_abs, double* d_mingap,
@@ -118,6 +161,8 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
     return be_small_loop(ctx, H, nullptr, map, N, m, d_close, n1 - 1, d_theta, d_abs, d_mingap, nullptr, nullptr, nullptr, 0, 0,
                          nullptr, nullptr, nullptr);
   }
+  SpinArgs spl;
+  if (sp) { spl = *sp; spl.sel = nullptr; spl.nsel = 0; spl.bval = 0.0; sp = &spl; }
   const size_t per = per_loop_bytes(N, m, n1, sp != nullptr, ctx->band_lo);
   size_t ws = be_effective_ws_limit(ctx, per * (size_t)loops + (hs ? 2 * hs->loop_bytes * (size_t)loops : 0));
   if (hs) {
@@ -183,6 +228,7 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   for (int s = 0; s < 2; ++s)
     persist += be_align256((size_t)loops * msec[s] * msec[s] * sizeof(cplx)) + be_eigenphases_scratch_bytes(2 * loops, msec[s]) +
                be_align256(2 * (size_t)loops * msec[s] * sizeof(double)) + be_align256(2 * (size_t)loops * sizeof(int)) + 1024;
+  persist += be_align256((size_t)N * sizeof(int));
   // Chunk pipeline (more than one chunk): two scratch regions used alternately, the
   // tridiagonalization of chunk c+1 on the caller's stream overlaps the rest of chunk c on stream2.
   const size_t region = be_align256(per * (size_t)lc);
@@ -248,6 +294,11 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   int* bad = (int*)be_arena_alloc(ctx, 2 * (size_t)loops * sizeof(int));
   if (!bad) return BE_ERR_NOMEM;
   BE_CUDA(cudaMemsetAsync(bad, 0, 2 * (size_t)loops * sizeof(int), ctx->stream));
+  if (sp && sp->S_is_diag && N >= 64) {
+    int* d_sel = (int*)be_arena_alloc(ctx, (size_t)N * sizeof(int));
+    if (!d_sel) return BE_ERR_NOMEM;
+    BE_TRY(analyze_diag_S(ctx, &spl, N, d_sel));
+  }
   const size_t keep = ctx->arena_used;
   for (int64_t ci = 0; ci < nchunks; ++ci) {
     const int64_t l0 = cstart[ci], nl = cstart[ci + 1] - l0;

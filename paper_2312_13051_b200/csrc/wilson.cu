@@ -157,6 +157,44 @@ int be_flag_loops(be_ctx* ctx, const int* info, const double* E, int ldE, int n1
   return BE_OK;
 }
 
+// Diagonal S with a dominant value b:  U^H S U = b I + U_A^H (S_A - b) U_A, where A is the set of rows with
+// S[r] != b (U^H U = I).  XA[c][v][i] = X[c][v][sel[i]], SXA = (S[sel[i]] - b) XA; leading dimension nsel.
+__global__ void k_pack_rows(const cplx* __restrict__ X, const double* __restrict__ S, const int* __restrict__ sel,
+                            double b, cplx* __restrict__ XA, cplx* __restrict__ SXA, int N, int nsel, int64_t total) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const int64_t col = i / nsel;
+  const int r = sel[i - col * nsel];
+  const double s = S[r] - b;
+  const cplx x = X[col * N + r];
+  XA[i] = x;
+  SXA[i] = mkc(s * x.x, s * x.y);
+}
+
+__global__ void k_add_diag(cplx* __restrict__ A, int m, int64_t total, double b) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const int64_t c = i / m;
+  const int k = (int)(i - c * m);
+  A[c * (int64_t)m * m + (int64_t)k * m + k].x += b;
+}
+
+int be_pack_rows(be_ctx* ctx, const cplx* X, const double* S, const int* sel, double b, cplx* XA, cplx* SXA, int N,
+                 int nsel, int64_t cols) {
+  const int64_t total = cols * nsel;
+  if (total == 0) return BE_OK;
+  k_pack_rows<<<(unsigned)((total + 255) / 256), 256, 0, ctx->stream>>>(X, S, sel, b, XA, SXA, N, nsel, total);
+  LAUNCH_CHECK();
+  return BE_OK;
+}
+
+int be_add_diag(be_ctx* ctx, cplx* A, int m, int64_t cnt, double b) {
+  const int64_t total = cnt * m;
+  k_add_diag<<<(unsigned)((total + 255) / 256), 256, 0, ctx->stream>>>(A, m, total, b);
+  LAUNCH_CHECK();
+  return BE_OK;
+}
+
 int be_scale_rows(be_ctx* ctx, const cplx* X, const double* S, cplx* SX, int N, int64_t total) {
   k_scale_rows<<<(unsigned)((total + 255) / 256), 256, 0, ctx->stream>>>(X, S, SX, N, total);
   LAUNCH_CHECK();
