@@ -135,6 +135,7 @@ extern "C" int be_create(be_ctx** out, void* cuda_stream) {
   c->ws_limit = (size_t)(0.70 * (double)prop.totalGlobalMem);
   if (c->ws_limit < ((size_t)4 << 30)) c->ws_limit = (size_t)4 << 30;
   c->eigh_algo = 2;
+  c->invit_solves = 3;
   *out = c;
   return BE_OK;
 }

@@ -2,6 +2,7 @@
 // chunking over whole loops and stage sequencing.
 #include "be_common.cuh"
 #include <string.h>
+#include <math.h>
 #include <vector>
 #include <algorithm>
 
@@ -161,6 +162,7 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
     return be_small_loop(ctx, H, nullptr, map, N, m, d_close, n1 - 1, d_theta, d_abs, d_mingap, nullptr, nullptr, nullptr, 0, 0,
                          nullptr, nullptr, nullptr);
   }
+  be_subspace_guard subspace(ctx);   // frames enter only through their span
   SpinArgs spl;
   if (sp) { spl = *sp; spl.sel = nullptr; spl.nsel = 0; spl.bval = 0.0; sp = &spl; }
   const size_t per = per_loop_bytes(N, m, n1, sp != nullptr, ctx->band_lo);
@@ -208,6 +210,16 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
         left -= c;
         step *= 2;
       }
+    }
+    // Large matrices: a loop takes r ~ 5.3 N / 1600 times longer to process than to copy (measured at N = 1600 on
+    // PCIe 5: 99 ms against 18.6 ms), and every extra chunk costs the latency-bound stages another round: TWO
+    // chunks, the first just long enough to hide the copy of the second, c1 = loops / (1 + r) (24 loops of
+    // N = 1600: 4 + 20, 2546 ms against 2604 ms for 5 + 8 + 11 and 2822 ms for one chunk).
+    if (N >= 800 && sz.size() >= 2) {
+      const double r = 5.3 * (double)N / 1600.0;
+      int64_t c1 = (int64_t)ceil((double)loops / (1.0 + r));
+      if (c1 < 1) c1 = 1;
+      if (c1 < loops && loops - c1 <= lc) { sz.clear(); sz.push_back(c1); sz.push_back(loops - c1); }
     }
     int64_t l0 = 0;
     for (size_t i = 0; i < sz.size(); ++i) { cstart.push_back(l0); l0 += sz[i]; }
@@ -498,6 +510,7 @@ extern "C" int be_nested_wilson(be_ctx* ctx, const void* dH_grid, const be_grid*
                                 double* d_theta1, double* d_theta_nested) {
   BE_DEVICE_GUARD(ctx);
   BE_TRY(check_common(ctx, dH_grid, grid, n_occ, dir1));
+  be_subspace_guard subspace(ctx);
   if (!d_theta_nested) return BE_ERR_NULL;
   if (grid->ndim < 2 || dir2 < 0 || dir2 >= grid->ndim || dir2 == dir1) return BE_ERR_SHAPE;
   if (base < 0 || base >= grid->dims[dir1]) return BE_ERR_SHAPE;
@@ -620,6 +633,7 @@ extern "C" int be_plaquette_flux(be_ctx* ctx, const void* dH_grid, const be_grid
                                  int S_is_diag, int m_lo, double* d_flux, double* d_flux_hi, double* d_pso) {
   BE_DEVICE_GUARD(ctx);
   BE_TRY(check_common(ctx, dH_grid, grid, n_occ, 0));
+  be_subspace_guard subspace(ctx);
   if (grid->ndim != 2 || !d_flux) return grid->ndim != 2 ? BE_ERR_SHAPE : BE_ERR_NULL;
   const int ny = grid->dims[0], nx = grid->dims[1], N = grid->N, m = n_occ;
   if (dS) {

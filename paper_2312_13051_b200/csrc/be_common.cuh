@@ -97,6 +97,7 @@ struct be_ctx {
   struct be_prof* prof;       // optional per-kernel-class CUDA-event timing (be_profile_enable)
   void* stage_buf[2];         // host variants: device staging buffers, kept between calls
   size_t stage_cap;
+  int invit_solves;           // inverse-iteration solves per eigenvector: 3 (eigenvectors, be_eigh_batched) or 2 (Wilson paths: only the span matters)
   int eigh_algo;              // be_set_eigh_algorithm: 0 one-stage tridiagonalization, 1 two-stage (band) where supported
 };
 
@@ -116,6 +117,19 @@ struct be_device_guard {
   ~be_device_guard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 #define BE_DEVICE_GUARD(ctx) be_device_guard be_guard__(ctx)
+
+// The Wilson-loop paths use the eigenvectors only through the subspaces they span (the occupied space, the PSO
+// sectors; W changes by a similarity under a change of basis at a k-point), so the third
+// inverse-iteration solve, which only sharpens the individual vectors inside a cluster, is dropped there: after
+// TWO solves (each followed by the cluster orthogonalization) the basis is orthonormal to 2e-13 and lies in the
+// occupied space to 5e-15, the same as after three (N = 400 supercell, 132 matrices; ONE solve from the random
+// start leaves 8e-9 / 3e-11, not enough for |lambda(W)| to 1e-9).  be_eigh_batched, which returns eigenvectors,
+// keeps three solves (subspace iteration inside clusters).
+struct be_subspace_guard {
+  be_ctx* c; int prev;
+  explicit be_subspace_guard(be_ctx* ctx) : c(ctx), prev(ctx->invit_solves) { ctx->invit_solves = 2; }
+  ~be_subspace_guard() { c->invit_solves = prev; }
+};
 
 #define BE_CUDA(x) do { cudaError_t e__ = (x); if (e__ != cudaSuccess) return (int)e__; } while (0)
 #define BE_TRY(x) do { int r__ = (x); if (r__ != BE_OK) return r__; } while (0)

@@ -934,7 +934,8 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
       // (subspace iteration inside a cluster): several solves in a row with the SAME shift collapse
       // the vectors of a numerically degenerate cluster onto its few nearest eigen-directions
       // (measured: cond 6e10 for the 400-fold +-1 of the projected spin operator).
-      for (int it = 0; it < 3; ++it) {
+      const int nsolve = ctx->invit_solves < 1 ? 1 : ctx->invit_solves;
+      for (int it = 0; it < nsolve; ++it) {
         be_prof_begin(ctx, PK_INVIT);
         k_invit<<<(unsigned)(cnt * nvb), 128, sh, st>>>(s.d, s.e, E, s.tnorm, s.fa, s.fb, s.fc, s.fp, s.blk, s.blo, s.bhi,
                                                         s.bcl, s.Z, N, nv, nvb, it > 0 ? 1 : 0, 1);
@@ -943,7 +944,8 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
         // Cholesky-QR passes: 2 after the first solve (random starts: cond up to ~1e5) and after the last
         // one (final orthogonality at eps); 1 in between (one solve applied to an orthonormal basis keeps
         // cond below ~5e2, and the next solve re-mixes the cluster anyway)
-        BE_TRY(be_cluster_orth(ctx, E, s.tnorm, s.blk, s.Z, cnt, N, nv, CLUSTER_TOL, info, s.orth, it == 0, it == 1 ? 1 : 2));
+        BE_TRY(be_cluster_orth(ctx, E, s.tnorm, s.blk, s.Z, cnt, N, nv, CLUSTER_TOL, info, s.orth, it == 0,
+                               (it == 0 || it == nsolve - 1) ? 2 : 1));
       }
     }
   }
