@@ -404,18 +404,21 @@ def main():
         o = wk.run_host(ctx, Hh, Sh)        # warm-up (allocations, page faults)
         barrier()
         t0 = time.perf_counter()
+        copied0 = ctx.host_grid_bytes_copied()
         for _ in range(e2e_steps):
             o = wk.run_host(ctx, Hh, Sh)    # synchronous: returns after the results are on the host
         torch.cuda.synchronize()
+        grid_bytes = (ctx.host_grid_bytes_copied() - copied0) // e2e_steps
         dt = time.perf_counter() - t0
         tt = torch.tensor([dt], dtype=torch.float64, device=device)
         if world > 1:
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         d2h = sum(int(x.numel()) * 8 for x in o if x is not None)
         e2e = {"value": world * wk.kpoints * e2e_steps / float(tt.item()), "unit": "k-points/s",
-               "h2d_bytes_per_step": int(Hh.numel()) * 16 + (int(Sh.numel()) * Sh.element_size() if Sh is not None else 0),
+               "h2d_bytes_per_step": int(grid_bytes) + (int(Sh.numel()) * Sh.element_size() if Sh is not None else 0),
+               "host_grid_bytes": int(Hh.numel()) * 16,
                "d2h_bytes_per_step": d2h, "steps": e2e_steps,
-               "how": "be_*_host C-ABI call on pinned host H_grid; chunked H2D overlapped with compute; wall clock, max over ranks"}
+               "how": "be_*_host C-ABI call on pinned host H_grid; chunked H2D overlapped with compute; h2d_bytes_per_step counts the bytes the library copies (for N >= 256 only the upper triangle of the Hermitian matrices, in 8 row blocks); wall clock, max over ranks"}
         del Hh
     else:
         del H

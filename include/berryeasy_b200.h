@@ -114,6 +114,10 @@ int be_probe_fp64(be_ctx* ctx, int which, double* tflops);
 /* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */
 int64_t be_launch_count(const be_ctx* ctx);
 
+/* Bytes of H_grid the *_host entry points have copied host -> device since the context was created (bench.py's
+ * h2d_bytes_per_step).  Matrices of order >= 256 travel as row blocks of their upper triangle, see the host variants. */
+int64_t be_host_grid_bytes_copied(const be_ctx* ctx);
+
 /* Optional per-kernel-class profile (bench.py's roofline): when enabled every launch of an
  * instrumented kernel class is bracketed by a CUDA event pair on the context's stream and its
  * algorithmic bytes / flops are accumulated.  be_profile_enable resets the counters (it
@@ -300,10 +304,16 @@ int be_plaquette_flux(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int
 /*
  * Host-buffer variants (end-to-end path): h* pointers are host memory (pinned recommended).  The
  * grid is streamed to the device in chunks of whole loops, overlapped with compute on an internal
- * copy stream (growing chunks: 1/8 of the loops, 1/4, then what the workspace cap allows, so that only
- * the first, small copy is exposed); results are copied back before return.  Semantics as the device
- * calls above; any loop direction (dir == ndim-1: one contiguous copy per chunk, else one strided copy
- * per loop).  The two staging buffers are kept in the context between calls.  be_nested_wilson_host
+ * copy stream; results are copied back before return.  Chunks: matrices of order >= 800 in TWO chunks, the
+ * first just long enough to hide the copy of the second (24 loops of N = 1600: 3 + 21); smaller ones in
+ * growing chunks (1/8 of the loops, 1/4, ... or multiples of a wave of SMs), so that only the first, small copy
+ * is exposed.  Semantics as the device calls above; any loop direction.
+ *   Which bytes travel: H(k) is Hermitian and the eigensolver reads only its row-major UPPER triangle
+ *   (diagonal included; the other triangle may hold anything, on the host and on the device).  For
+ *   N >= 256 each matrix is copied as 8 row blocks, block b with the columns from its first row on: 56 % of
+ *   the bytes.  Smaller matrices are copied whole (dir == ndim-1: one contiguous copy per chunk, else one
+ *   strided copy per loop).  be_host_grid_bytes_copied counts what was copied.
+ * The two staging buffers are kept in the context between calls.  be_nested_wilson_host
  * copies the whole grid in one piece (both levels need the whole plane).
  */
 int be_wilson_loop_host(be_ctx* ctx, const void* hH_grid, const be_grid* grid, int n_occ, int dir,

@@ -98,15 +98,19 @@ int be_arena_reserve(be_ctx* ctx, size_t bytes) {
 
 // The cap that applies to a call: the configured limit, but never more than what the device can give right now
 // (free memory plus the arena already held, minus a margin for the caller's outputs and the CUDA context).
-size_t be_effective_ws_limit(be_ctx* ctx, size_t want) {
+// host_grid: the grid is not resident on the device, so the DEFAULT cap (70 % of the memory, which leaves room
+// for a device-resident grid) is raised to 85 %; a cap set by the caller stands.
+size_t be_effective_ws_limit(be_ctx* ctx, size_t want, bool host_grid) {
+  size_t lim = ctx->ws_limit;
+  if (host_grid && !ctx->ws_user) { const size_t l2 = (size_t)(0.85 * (double)ctx->total_mem); if (l2 > lim) lim = l2; }
   // cudaMemGetInfo costs ~0.5 ms: not worth asking when the whole request is small or already held
-  if (want <= ctx->arena_bytes || want <= ((size_t)1 << 30)) return ctx->ws_limit;
+  if (want <= ctx->arena_bytes || want <= ((size_t)1 << 30)) return lim;
   size_t fr = 0, tot = 0;
-  if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) { cudaGetLastError(); return ctx->ws_limit; }
+  if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) { cudaGetLastError(); return lim; }
   const size_t margin = (size_t)2 << 30;
   size_t avail = fr + ctx->arena_bytes;
   avail = avail > margin ? avail - margin : avail / 2;
-  return ctx->ws_limit < avail ? ctx->ws_limit : avail;
+  return lim < avail ? lim : avail;
 }
 
 void* be_arena_alloc(be_ctx* ctx, size_t bytes) {
@@ -133,9 +137,12 @@ extern "C" int be_create(be_ctx** out, void* cuda_stream) {
   // scratch cap: 70 % of the device memory (134 GB on a B200).  Larger chunks fill the one-CTA-per-matrix kernels'
   // waves better (600 matrices in one chunk instead of 2 x 300: 2481 vs 2561 ms on the bench workload)
   c->ws_limit = (size_t)(0.70 * (double)prop.totalGlobalMem);
+  c->total_mem = prop.totalGlobalMem;
+  c->ws_user = 0;
   if (c->ws_limit < ((size_t)4 << 30)) c->ws_limit = (size_t)4 << 30;
   c->eigh_algo = 2;
   c->invit_solves = 3;
+  c->h2d_bytes = 0;
   *out = c;
   return BE_OK;
 }
@@ -178,6 +185,7 @@ extern "C" int be_set_workspace_limit(be_ctx* ctx, size_t bytes) {
   if (!ctx) return BE_ERR_NULL;
   if (bytes < ((size_t)1 << 20)) return BE_ERR_SHAPE;
   ctx->ws_limit = bytes;
+  ctx->ws_user = 1;
   return BE_OK;
 }
 
@@ -203,12 +211,14 @@ extern "C" int be_release_workspace(be_ctx* ctx) {
   if (ctx->copy_stream) BE_CUDA(cudaStreamSynchronize(ctx->copy_stream));
   if (ctx->arena) { cudaFree(ctx->arena); ctx->arena = nullptr; ctx->arena_bytes = 0; ctx->arena_used = 0; }
   for (int i = 0; i < 2; ++i) if (ctx->stage_buf[i]) { cudaFree(ctx->stage_buf[i]); ctx->stage_buf[i] = nullptr; }
-  ctx->stage_cap = 0;
+  ctx->stage_cap[0] = ctx->stage_cap[1] = 0;
   return BE_OK;
 }
 
 extern "C" int64_t be_launch_count(const be_ctx* ctx) {
   BE_DEVICE_GUARD(ctx); return ctx ? ctx->launches : 0; }
+
+extern "C" int64_t be_host_grid_bytes_copied(const be_ctx* ctx) { return ctx ? ctx->h2d_bytes : 0; }
 
 // ---------------------------------------------------------------------------------------------
 size_t be_eigh_scratch_bytes(int64_t cnt, int N, int nv) {

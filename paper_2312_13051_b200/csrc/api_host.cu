@@ -155,6 +155,7 @@ extern "C" int be_nested_wilson_host(be_ctx* ctx, const void* hH_grid, const be_
   if (h_theta1) BE_TRY(dth1.alloc((size_t)loops * n_occ * sizeof(double)));
   cudaStream_t st = ctx->stream;
   BE_CUDA(cudaMemcpyAsync(dH.p, hH_grid, (size_t)pts * N * N * sizeof(cplx), cudaMemcpyHostToDevice, st));
+  ctx->h2d_bytes += (int64_t)pts * N * N * (int64_t)sizeof(cplx);
   if (h_close1) { BE_TRY(dc1.alloc((size_t)N * sizeof(cplx))); BE_CUDA(cudaMemcpyAsync(dc1.p, h_close1, (size_t)N * sizeof(cplx), cudaMemcpyHostToDevice, st)); }
   if (h_close2) { BE_TRY(dc2.alloc((size_t)N * sizeof(cplx))); BE_CUDA(cudaMemcpyAsync(dc2.p, h_close2, (size_t)N * sizeof(cplx), cudaMemcpyHostToDevice, st)); }
   BE_TRY(be_nested_wilson(ctx, dH.p, grid, n_occ, dir1, dir2, base, wb_lo, wb_hi, theta_cut, dc1.p, dc2.p,

@@ -37,6 +37,9 @@ static int make_map(const be_grid* g, int dir, GridMap* out) {
   return BE_OK;
 }
 
+// host grids: matrices of at least this order are copied as row blocks of their upper triangle
+constexpr int HOST_TRI_MINN = 256, HOST_TRI_BLOCKS = 8;
+
 struct SpinArgs {
   const void* dS; int S_is_diag; int m_lo;
   double* theta_lo; double* theta_hi; double* pso;
@@ -166,11 +169,12 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   SpinArgs spl;
   if (sp) { spl = *sp; spl.sel = nullptr; spl.nsel = 0; spl.bval = 0.0; sp = &spl; }
   const size_t per = per_loop_bytes(N, m, n1, sp != nullptr, ctx->band_lo);
-  size_t ws = be_effective_ws_limit(ctx, per * (size_t)loops + (hs ? 2 * hs->loop_bytes * (size_t)loops : 0));
+  size_t ws = be_effective_ws_limit(ctx, per * (size_t)loops + (hs ? 2 * hs->loop_bytes * (size_t)loops : 0), hs != nullptr);
+  size_t ws_total = ws;   // host grid: scratch arena + the two staging buffers
   if (hs) {
     // the two staging buffers of a host grid come out of the same budget (2 x loop_bytes per loop of a chunk)
-    const size_t held = 2 * ctx->stage_cap;
-    ws = (size_t)((double)(ws + held) * (double)per / (double)(per + 2 * hs->loop_bytes));
+    ws_total = ws + ctx->stage_cap[0] + ctx->stage_cap[1];
+    ws = (size_t)((double)ws_total * (double)per / (double)(per + 2 * hs->loop_bytes));
   }
   int64_t lc = (int64_t)(ws / per);
   if (lc < 1) lc = 1;
@@ -216,10 +220,13 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
     // chunks, the first just long enough to hide the copy of the second, c1 = loops / (1 + r) (24 loops of
     // N = 1600: 4 + 20, 2546 ms against 2604 ms for 5 + 8 + 11 and 2822 ms for one chunk).
     if (N >= 800 && sz.size() >= 2) {
-      const double r = 5.3 * (double)N / 1600.0;
+      // (only the upper triangle travels: (HOST_TRI_BLOCKS + 1) / (2 HOST_TRI_BLOCKS) of the bytes)
+      const double r = 5.3 * (double)N / 1600.0 * (2.0 * HOST_TRI_BLOCKS) / (HOST_TRI_BLOCKS + 1.0);
       int64_t c1 = (int64_t)ceil((double)loops / (1.0 + r));
       if (c1 < 1) c1 = 1;
-      if (c1 < loops && loops - c1 <= lc) { sz.clear(); sz.push_back(c1); sz.push_back(loops - c1); }
+      // memory: scratch for the larger chunk, one staging buffer per chunk
+      const size_t need2 = per * (size_t)(loops - c1) + (size_t)loops * hs->loop_bytes + ((size_t)1 << 30);   // + persistent part
+      if (c1 < loops && need2 <= ws_total) { sz.clear(); sz.push_back(c1); sz.push_back(loops - c1); }
     }
     int64_t l0 = 0;
     for (size_t i = 0; i < sz.size(); ++i) { cstart.push_back(l0); l0 += sz[i]; }
@@ -252,10 +259,41 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
     const int64_t c0 = cstart[ci], cn = cstart[ci + 1] - c0;
     if (ci >= 2) BE_CUDA(cudaStreamWaitEvent(ctx->copy_stream, hs->freed[b], 0));
     const GridMap& hm = hs->hmap;
-    if (hm.dir == hm.ndim - 1) {
+    if (N >= HOST_TRI_MINN) {
+      // The eigensolver reads only the row-major UPPER triangle of a Hermitian H (tests: the other triangle may
+      // hold anything): each matrix travels as HOST_TRI_BLOCKS row blocks, block b with the columns from its first
+      // row on -- 56 % of the bytes for 8 blocks.  The rest of the staging buffer keeps stale data.
+      // One 3D copy per row block covers that block of EVERY matrix of a run of equally spaced matrices (a slice =
+      // a matrix): 8 copies per chunk when the loops are contiguous in the host grid, else 8 per loop.  (One 2D
+      // copy per matrix and block -- 4000 calls for 500 matrices -- overflows the stream's queue and blocks the
+      // host thread until most of the copy is done, before it gets to launch the kernels of the chunk in front.)
+      const size_t pitch = (size_t)N * sizeof(cplx);
+      const int h = (N + HOST_TRI_BLOCKS - 1) / HOST_TRI_BLOCKS;
+      const bool contig = hm.dir == hm.ndim - 1;
+      const int64_t runs = contig ? 1 : cn;
+      for (int64_t l = 0; l < runs; ++l) {
+        const int64_t src = gridmap_index(hm, c0 + l, 0);
+        const size_t depth = contig ? (size_t)(cn * n1) : (size_t)n1;
+        const size_t src_rows = contig ? (size_t)N : (size_t)hm.stride[hm.dir] * N;   // rows from one matrix to the next
+        for (int r0 = 0; r0 < N; r0 += h) {
+          const int rows = (N - r0 < h) ? N - r0 : h;
+          cudaMemcpy3DParms q;
+          memset(&q, 0, sizeof(q));
+          q.srcPtr = make_cudaPitchedPtr((void*)(hs->hH + (size_t)src * hs->mat_bytes), pitch, pitch, src_rows);
+          q.dstPtr = make_cudaPitchedPtr((char*)hs->stage[b] + (size_t)l * hs->loop_bytes, pitch, pitch, (size_t)N);
+          q.srcPos = make_cudaPos((size_t)r0 * sizeof(cplx), (size_t)r0, 0);
+          q.dstPos = q.srcPos;
+          q.extent = make_cudaExtent((size_t)(N - r0) * sizeof(cplx), (size_t)rows, depth);
+          q.kind = cudaMemcpyHostToDevice;
+          BE_CUDA(cudaMemcpy3DAsync(&q, ctx->copy_stream));
+          ctx->h2d_bytes += (int64_t)(N - r0) * (int64_t)sizeof(cplx) * rows * (int64_t)depth;
+        }
+      }
+    } else if (hm.dir == hm.ndim - 1) {
       // loops are contiguous in the host grid, and so are consecutive loops: one copy per chunk
       BE_CUDA(cudaMemcpyAsync(hs->stage[b], hs->hH + (size_t)c0 * hs->loop_bytes, (size_t)cn * hs->loop_bytes,
                               cudaMemcpyHostToDevice, ctx->copy_stream));
+      ctx->h2d_bytes += (int64_t)cn * (int64_t)hs->loop_bytes;
     } else {
       // a loop is n1 matrices a fixed stride apart: one strided copy per loop
       for (int64_t l = 0; l < cn; ++l) {
@@ -263,20 +301,26 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
         BE_CUDA(cudaMemcpy2DAsync((char*)hs->stage[b] + (size_t)l * hs->loop_bytes, hs->mat_bytes,
                                   hs->hH + (size_t)src * hs->mat_bytes, (size_t)hm.stride[hm.dir] * hs->mat_bytes,
                                   hs->mat_bytes, (size_t)n1, cudaMemcpyHostToDevice, ctx->copy_stream));
+        ctx->h2d_bytes += (int64_t)hs->loop_bytes;
       }
     }
     BE_CUDA(cudaEventRecord(hs->copied[b], ctx->copy_stream));
     return BE_OK;
   };
   if (hs) {
-    const size_t need = (size_t)lc * hs->loop_bytes;
-    if (need > ctx->stage_cap) {
+    // buffer b serves the chunks b, b + 2, ..: sized for the largest of them
+    size_t need[2] = {0, 0};
+    for (int64_t ci = 0; ci < nchunks; ++ci) {
+      const size_t nb = (size_t)(cstart[ci + 1] - cstart[ci]) * hs->loop_bytes;
+      if (nb > need[ci & 1]) need[ci & 1] = nb;
+    }
+    for (int b = 0; b < 2; ++b) {
+      if (need[b] <= ctx->stage_cap[b]) continue;
       BE_CUDA(cudaStreamSynchronize(ctx->stream));
-      for (int b = 0; b < 2; ++b) { if (ctx->stage_buf[b]) cudaFree(ctx->stage_buf[b]); ctx->stage_buf[b] = nullptr; }
-      ctx->stage_cap = 0;
-      for (int b = 0; b < 2; ++b)
-        if (cudaMalloc(&ctx->stage_buf[b], need) != cudaSuccess) { cudaGetLastError(); return BE_ERR_NOMEM; }
-      ctx->stage_cap = need;
+      if (ctx->stage_buf[b]) cudaFree(ctx->stage_buf[b]);
+      ctx->stage_buf[b] = nullptr; ctx->stage_cap[b] = 0;
+      if (cudaMalloc(&ctx->stage_buf[b], need[b]) != cudaSuccess) { cudaGetLastError(); return BE_ERR_NOMEM; }
+      ctx->stage_cap[b] = need[b];
     }
     hs->stage[0] = ctx->stage_buf[0]; hs->stage[1] = ctx->stage_buf[1];
     memset(&smap, 0, sizeof(smap));

@@ -77,6 +77,7 @@ struct be_ctx {
   int sm_count;
   size_t ws_limit;
   int64_t launches;
+  int64_t h2d_bytes;          // host -> device bytes of H_grid copied by the *_host entry points since creation
   // scratch arena (bump allocated per call, grown on demand)
   char* arena;
   size_t arena_bytes;
@@ -96,7 +97,9 @@ struct be_ctx {
                               // leaving room for one k_hemv CTA of the other stream
   struct be_prof* prof;       // optional per-kernel-class CUDA-event timing (be_profile_enable)
   void* stage_buf[2];         // host variants: device staging buffers, kept between calls
-  size_t stage_cap;
+  size_t stage_cap[2];        // bytes of each (a two-chunk schedule needs a small and a large one)
+  size_t total_mem;           // totalGlobalMem of the device
+  int ws_user;                // be_set_workspace_limit was called: the cap is the caller's, not the default
   int invit_solves;           // inverse-iteration solves per eigenvector: 3 (eigenvectors, be_eigh_batched) or 2 (Wilson paths: only the span matters)
   int eigh_algo;              // be_set_eigh_algorithm: 0 one-stage tridiagonalization, 1 two-stage (band) where supported
 };
@@ -137,7 +140,7 @@ struct be_subspace_guard {
 // bump allocator on the context arena; pointers stay valid until arena_reset
 int  be_arena_reserve(be_ctx* ctx, size_t bytes);   // ensure capacity (may sync + realloc); resets
 void* be_arena_alloc(be_ctx* ctx, size_t bytes);
-size_t be_effective_ws_limit(be_ctx* ctx, size_t want);   // min(configured cap, what the device can give now); want = the uncapped request    // 256-byte aligned; NULL when exhausted
+size_t be_effective_ws_limit(be_ctx* ctx, size_t want, bool host_grid = false);   // min(configured cap, what the device can give now); want = the uncapped request    // 256-byte aligned; NULL when exhausted
 static inline size_t be_align256(size_t b) { return (b + 255) & ~(size_t)255; }
 
 // ---------------------------------------------------------------------------------------------

@@ -579,6 +579,44 @@ def test_host_variants_match_device(ctx):
     assert wo.circ_sorted_distance(tn.numpy()[0], tno) / (2 * np.pi) <= PH_TOL
 
 
+def test_only_the_upper_triangle_of_H_is_read(ctx):
+    """Header contract of the host variants: for N > 104 the eigensolver reads the row-major upper triangle only, so the
+    host variants copy just that (N >= 256, 8 row blocks).  NaN in the other triangle must change nothing, on the
+    device (one- and two-stage solver) and through the triangle-block host copy, both loop directions."""
+    rng = np.random.default_rng(7)
+    for N, algo in ((105, 0), (144, 1), (256, 0), (264, 1)):
+        A = rng.standard_normal((3, N, N)) + 1j * rng.standard_normal((3, N, N))
+        H = (A + A.conj().transpose(0, 2, 1)) / 2
+        Hp = H.copy()
+        il = np.tril_indices(N, -1)
+        Hp[:, il[0], il[1]] = np.nan
+        ctx.set_eigh_algorithm(algo)
+        try:
+            E0, U0 = ctx.eigh_batched(dev(H), N // 2)
+            E1, U1 = ctx.eigh_batched(dev(Hp), N // 2)
+        finally:
+            ctx.set_eigh_algorithm(2)
+        assert torch.equal(E0, E1) and torch.equal(U0, U1)
+    # host grid, N = 256 (L = 8 supercell), lower triangle poisoned on the host
+    parts = wl.config4_parts(8, axis="x")
+    H = wl.supercell_grid([parts], 7, 6, t2_indices=[0, 2, 5])
+    S = wl.supercell_spin_z(8)
+    Hp = H.copy()
+    il = np.tril_indices(256, -1)
+    Hp[..., il[0], il[1]] = np.nan
+    Hh = torch.from_numpy(Hp).pin_memory()
+    before = ctx.host_grid_bytes_copied()
+    lo, hi, pso = ctx.spin_resolved_wilson_host(Hh, 128, 1, torch.from_numpy(S))
+    copied = ctx.host_grid_bytes_copied() - before
+    assert copied == H.shape[0] * H.shape[1] * H.shape[2] * sum((256 - r0) * 32 * 16 for r0 in range(0, 256, 32))
+    loo, hio, psoo = wo.spin_resolved_surface(H, 128, 1, S)
+    assert phase_dist(lo.numpy(), loo) <= PH_TOL and phase_dist(hi.numpy(), hio) <= PH_TOL
+    assert np.abs(pso.numpy().reshape(psoo.shape) - psoo).max() < 1e-10
+    th0, _, _ = ctx.wilson_loop_host(Hh, 128, 0)            # loops along the slow axis
+    th0o, _, _ = wo.wilson_surface(H, 128, 0)
+    assert phase_dist(th0.numpy(), th0o) <= PH_TOL
+
+
 def test_chunk_pipeline_matches_single_chunk_and_oracle(ctx):
     """A small workspace cap splits the loops into >= 3 chunks: the two-stream chunk pipeline
     (tridiagonalization of chunk c+1 next to the rest of chunk c, two scratch regions) must give
