@@ -118,6 +118,11 @@ int64_t be_launch_count(const be_ctx* ctx);
  * h2d_bytes_per_step).  Matrices of order >= 256 travel as row blocks of their upper triangle, see the host variants. */
 int64_t be_host_grid_bytes_copied(const be_ctx* ctx);
 
+/* How the last be_wilson_loop_host / be_spin_resolved_wilson_host call of this context streamed its grid: n > 0 =
+ * n chunks of whole loops, each processed on its own; n < 0 = ONE chunk fed in -n sub-ranges (two-stage eigensolver:
+ * only the dense -> band stage runs per sub-range); 0 = no such call yet. */
+int be_host_schedule(const be_ctx* ctx);
+
 /* Optional per-kernel-class profile (bench.py's roofline): when enabled every launch of an
  * instrumented kernel class is bracketed by a CUDA event pair on the context's stream and its
  * algorithmic bytes / flops are accumulated.  be_profile_enable resets the counters (it

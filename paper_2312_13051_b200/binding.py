@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libberryeasy_b200.so")
 
 EXPORTS = [
     "be_create", "be_destroy", "be_strerror", "be_workspace_bytes", "be_set_workspace_limit",
-    "be_launch_count", "be_host_grid_bytes_copied", "be_eigh_batched", "be_eigh_batched_static", "be_wilson_loop", "be_nested_wilson",
+    "be_launch_count", "be_host_grid_bytes_copied", "be_host_schedule", "be_eigh_batched", "be_eigh_batched_static", "be_wilson_loop", "be_nested_wilson",
     "be_spin_resolved_wilson", "be_winding", "be_wilson_loop_host", "be_spin_resolved_wilson_host", "be_nested_wilson_host",
     "be_profile_enable", "be_profile_name", "be_profile_get", "be_zgemm_batched", "be_set_chunk_pipeline", "be_set_eigh_algorithm", "be_probe_fp64", "be_release_workspace", "be_bloch_coefficients", "be_assemble_bloch", "be_plaquette_flux", "be_wilson_loop_bloch",
     "be_spin_resolved_wilson_bloch", "be_wilson_loop_window", "be_spin_resolved_wilson_window",
@@ -61,6 +61,8 @@ def load_library():
     lib.be_launch_count.restype = i64
     lib.be_host_grid_bytes_copied.argtypes = [vp]
     lib.be_host_grid_bytes_copied.restype = i64
+    lib.be_host_schedule.argtypes = [vp]
+    lib.be_host_schedule.restype = ci
     lib.be_eigh_batched.argtypes = [vp, vp, i64, ci, ci, vp, vp, vp]
     lib.be_eigh_batched_static.argtypes = [vp, vp, i64, ci, ci, vp, vp, vp]
     lib.be_wilson_loop.argtypes = [vp, vp, gp, ci, ci, vp, vp, vp, vp]
@@ -191,6 +193,10 @@ class Context:
 
     def launch_count(self) -> int:
         return int(self.lib.be_launch_count(self._h))
+
+    def host_schedule(self) -> int:
+        """n > 0: the last *_host call ran n chunks; n < 0: one chunk fed in -n sub-ranges (be_host_schedule)."""
+        return int(self.lib.be_host_schedule(self._h))
 
     def host_grid_bytes_copied(self) -> int:
         """Bytes of H_grid the *_host calls of this context have copied to the device so far."""

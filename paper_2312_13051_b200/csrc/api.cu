@@ -219,6 +219,7 @@ extern "C" int64_t be_launch_count(const be_ctx* ctx) {
   BE_DEVICE_GUARD(ctx); return ctx ? ctx->launches : 0; }
 
 extern "C" int64_t be_host_grid_bytes_copied(const be_ctx* ctx) { return ctx ? ctx->h2d_bytes : 0; }
+extern "C" int be_host_schedule(const be_ctx* ctx) { return ctx ? ctx->host_schedule : 0; }
 
 // ---------------------------------------------------------------------------------------------
 size_t be_eigh_scratch_bytes(int64_t cnt, int N, int nv) {

@@ -183,6 +183,7 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   // anything, so the chunks grow -- 1/8 of the loops, then 1/4, then what the cap allows -- and every later
   // copy hides behind the (longer) computation of the chunk before it.
   std::vector<int64_t> cstart;
+  std::vector<int64_t> feed_sub;   // host grid streamed into one chunk: loop boundaries of the sub-ranges
   if (!hs) {
     const int64_t nch = (loops + lc - 1) / lc;
     lc = (loops + nch - 1) / nch;
@@ -228,6 +229,28 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
       const size_t need2 = per * (size_t)(loops - c1) + (size_t)loops * hs->loop_bytes + ((size_t)1 << 30);   // + persistent part
       if (c1 < loops && need2 <= ws_total) { sz.clear(); sz.push_back(c1); sz.push_back(loops - c1); }
     }
+    // Two-stage eigensolver and room for every loop at once: ONE chunk, fed in three sub-ranges (HostFeed).  Only
+    // stage 1 of the eigensolver (dense -> band, a third of the pass, throughput bound) runs per sub-range, while
+    // the next one travels; everything else sees the whole batch, so nothing pays for small batches.  Stage 1 of a
+    // loop takes rho ~ 2.3 N / 1600 times as long as its copy: sub-ranges in the ratio 1 : rho : rho^2
+    // (24 loops of N = 1600: 3 + 7 + 14; exposed: the first 3 loops, 31 ms).
+    const bool two_stage = N >= BE_BAND_MINN && N <= BE_BAND_MAXN && N > TS_MAXN && !bs &&
+                           (ctx->eigh_algo == 1 || (ctx->eigh_algo == 2 && N >= BE_BAND_AUTON));
+    if (two_stage && loops >= 3 && sz.size() >= 2) {
+      double rho = 2.3 * (double)N / 1600.0;
+      rho = rho < 1.2 ? 1.2 : (rho > 3.0 ? 3.0 : rho);
+      int64_t s0 = (int64_t)floor((double)loops / (1.0 + rho + rho * rho) + 0.5);
+      if (s0 < 1) s0 = 1;
+      int64_t s1 = (int64_t)floor((double)s0 * rho + 0.5);
+      if (s1 < 1) s1 = 1;
+      if (s0 + s1 >= loops) { s0 = 1; s1 = 1; }
+      const int64_t s2 = loops - s0 - s1;
+      const size_t stg = (size_t)((s0 > s2 ? s0 : s2) + s1) * hs->loop_bytes;
+      if (per * (size_t)loops + stg + ((size_t)1 << 30) <= ws_total) {
+        feed_sub.push_back(0); feed_sub.push_back(s0); feed_sub.push_back(s0 + s1); feed_sub.push_back(loops);
+        sz.clear(); sz.push_back(loops);
+      }
+    }
     int64_t l0 = 0;
     for (size_t i = 0; i < sz.size(); ++i) { cstart.push_back(l0); l0 += sz[i]; }
     lc = 0;
@@ -256,7 +279,8 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   GridMap smap;
   auto issue_copy = [&](int64_t ci) -> int {
     const int b = (int)(ci & 1);
-    const int64_t c0 = cstart[ci], cn = cstart[ci + 1] - c0;
+    const std::vector<int64_t>& cb = feed_sub.empty() ? cstart : feed_sub;   // chunks, or the sub-ranges of the one chunk
+    const int64_t c0 = cb[ci], cn = cb[ci + 1] - c0;
     if (ci >= 2) BE_CUDA(cudaStreamWaitEvent(ctx->copy_stream, hs->freed[b], 0));
     const GridMap& hm = hs->hmap;
     if (N >= HOST_TRI_MINN) {
@@ -310,8 +334,9 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
   if (hs) {
     // buffer b serves the chunks b, b + 2, ..: sized for the largest of them
     size_t need[2] = {0, 0};
-    for (int64_t ci = 0; ci < nchunks; ++ci) {
-      const size_t nb = (size_t)(cstart[ci + 1] - cstart[ci]) * hs->loop_bytes;
+    const std::vector<int64_t>& cb = feed_sub.empty() ? cstart : feed_sub;
+    for (size_t ci = 0; ci + 1 < cb.size(); ++ci) {
+      const size_t nb = (size_t)(cb[ci + 1] - cb[ci]) * hs->loop_bytes;
       if (nb > need[ci & 1]) need[ci & 1] = nb;
     }
     for (int b = 0; b < 2; ++b) {
@@ -326,6 +351,16 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
     memset(&smap, 0, sizeof(smap));
     smap.ndim = 1; smap.dir = 0; smap.n1 = n1; smap.dims[0] = n1; smap.stride[0] = 1; smap.batch_stride = n1; smap.loops = lc;
     BE_TRY(issue_copy(0));
+    if (!feed_sub.empty()) BE_TRY(issue_copy(1));
+  }
+  HostFeed feed;
+  if (hs) ctx->host_schedule = feed_sub.empty() ? (int)nchunks : -((int)feed_sub.size() - 1);
+  if (!feed_sub.empty()) {
+    feed.nsub = (int)feed_sub.size() - 1;
+    for (size_t i = 0; i < feed_sub.size(); ++i) feed.mstart[i] = feed_sub[i] * n1;
+    for (int b = 0; b < 2; ++b) { feed.buf[b] = hs->stage[b]; feed.copied[b] = hs->copied[b]; feed.freed[b] = hs->freed[b]; }
+    feed.issue = [](void* self, int j) -> int { return (*(decltype(issue_copy)*)self)((int64_t)j); };
+    feed.self = &issue_copy;
   }
   if (pipe) {
     BE_TRY(pipeline_init(ctx));
@@ -367,16 +402,18 @@ static int wilson_device(be_ctx* ctx, const cplx* H, const GridMap& map, int N, 
       ctx->gemm_pad = (ci + 1 < nchunks && N > 8) ? 1 : 0;   // a next chunk will stream its matrices next to these GEMMs
     }
     const cplx* Hc = H;
-    if (hs) {
+    if (hs && feed_sub.empty()) {
       if (ci + 1 < nchunks) BE_TRY(issue_copy(ci + 1));
       BE_CUDA(cudaStreamWaitEvent(ctx->stream, hs->copied[ci & 1], 0));
       Hc = (const cplx*)hs->stage[ci & 1];
     }
     ctx->bloch = bs;   // consumed (and cleared) by the H eigensolve of the chunk
+    ctx->feed = feed_sub.empty() ? nullptr : &feed;   // likewise: the sub-ranges are gathered as they land
     const int rc = wilson_chunk(ctx, Hc, hs ? smap : map, hs ? 0 : l0, N, m, n1, l0, nl, cnt, d_close, d_mingap, sp, mlo,
                                 mhi, Wall, bad, loops);
     ctx->bloch = nullptr;
-    if (hs && rc == BE_OK) cudaEventRecord(hs->freed[ci & 1], ctx->stream);
+    ctx->feed = nullptr;
+    if (hs && feed_sub.empty() && rc == BE_OK) cudaEventRecord(hs->freed[ci & 1], ctx->stream);
     if (pipe) {
       ctx->split_after_tridiag = 0;
       if (rc == BE_OK) cudaEventRecord(ctx->ev_region[ci & 1], ctx->stream);

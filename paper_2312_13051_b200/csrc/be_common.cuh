@@ -70,6 +70,7 @@ __device__ __forceinline__ T block_sum(T v, T* red) {
 }
 
 // ---------------------------------------------------------------------------------------------
+struct HostFeed;
 struct be_ctx {
   cudaStream_t stream;
   cudaStream_t copy_stream;   // host variants only
@@ -77,6 +78,8 @@ struct be_ctx {
   int sm_count;
   size_t ws_limit;
   int64_t launches;
+  HostFeed* feed;             // consumed (and cleared) by the next large eigensolve
+  int host_schedule;          // last *_host call: number of chunks, or -(number of sub-ranges) of the one fed chunk
   int64_t h2d_bytes;          // host -> device bytes of H_grid copied by the *_host entry points since creation
   // scratch arena (bump allocated per call, grown on demand)
   char* arena;
@@ -217,6 +220,18 @@ int be_bloch_assemble_chunk(be_ctx* ctx, const BlochSrc* bs, int64_t loop0, int6
 
 // Host-resident H_grid streamed chunk by chunk (be_*_host): two device staging buffers filled on the
 // copy stream while the previous chunk computes.  Loops must be contiguous (dir == last axis).
+// Host grid streamed INTO one chunk (two-stage eigensolver): the matrices arrive in nsub sub-ranges through two
+// staging buffers; be_eigh_large gathers each as its copy lands and runs stage 1 (dense -> band) on it while the
+// next one travels, then everything else over the whole batch.  issue(self, j) enqueues the copy of sub-range j.
+struct HostFeed {
+  int nsub;
+  int64_t mstart[9];            // matrix index where sub-range j starts (nsub + 1 entries)
+  void* buf[2];
+  cudaEvent_t copied[2], freed[2];
+  int (*issue)(void* self, int j);
+  void* self;
+};
+
 struct HostStage {
   const char* hH;          // host grid
   size_t loop_bytes;       // n1 * N * N * 16
@@ -266,6 +281,8 @@ constexpr int BE_BAND_KB = 8;
 constexpr int BE_BAND_MINN = 128, BE_BAND_MAXN = 2048, BE_BAND_AUTON = 1024;
 size_t be_band_scratch_bytes(int64_t cnt, int N);
 int be_band_reduce(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double* e, cplx* tau, void* scratch);
+int be_band_stage1(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, cplx* tau, void* scratch);
+int be_band_stage2(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double* e, void* scratch);
 int be_band_q2(be_ctx* ctx, const cplx* Bw, cplx* X, int64_t cnt, int N, int nv);
 constexpr int BE_MAX_N = 6400;   // largest matrix order of the blocked eigensolver (be_eigh_batched, every Wilson entry point)
 constexpr int BE_MAX_M = 2048;   // largest Wilson matrix (bands per sector) of the eigenphase solve

@@ -1073,6 +1073,13 @@ size_t be_band_scratch_bytes(int64_t cnt, int N) { return band_carve(nullptr, cn
 // stage-1 reflectors (column j: head at row j + KB), stage-1 vectors below the band of Bw, stage-2
 // reflectors in its upper triangle.
 int be_band_reduce(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double* e, cplx* tau, void* scratch) {
+  BE_TRY(be_band_stage1(ctx, Bw, cnt, N, tau, scratch));
+  return be_band_stage2(ctx, Bw, cnt, N, d, e, scratch);
+}
+
+// Stage 1 (dense -> band) alone.  Everything it leaves behind is in Bw and tau, so it may be run on sub-ranges of
+// a batch one after the other with the same scratch (carved for the sub-range) before ONE stage 2 over the batch.
+int be_band_stage1(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, cplx* tau, void* scratch) {
   if (N > BE_BAND_MAXN || N < 2 * KB) return BE_ERR_UNSUPPORTED;
   if (cnt > 0x7fffffffLL / 64) return BE_ERR_SHAPE;
   BandScratch s;
@@ -1142,8 +1149,15 @@ int be_band_reduce(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double*
     }
     LAUNCH_CHECK();
   }
-  BE_TRY(panel(plast + 1, 0));
-  // ---- stage 2
+  return panel(plast + 1, 0);
+}
+
+// Stage 2 (band -> real tridiagonal by bulge chasing) for the whole batch.
+int be_band_stage2(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double* e, void* scratch) {
+  if (N > BE_BAND_MAXN || N < 2 * KB) return BE_ERR_UNSUPPORTED;
+  BandScratch s;
+  band_carve((char*)scratch, cnt, N, &s);
+  cudaStream_t st = ctx->stream;
   k_band_extract<<<dim3((unsigned)((N * LDAB + 255) / 256), (unsigned)cnt), 256, 0, st>>>(Bw, s.AB, N);
   LAUNCH_CHECK();
   {

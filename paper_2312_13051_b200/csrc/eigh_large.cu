@@ -824,7 +824,7 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
     BE_TRY(be_tridiag_small(ctx, H, map, loop0, cnt, N, s.Bw, s.d, s.e, s.tau));
   } else if (ctx->bloch) {
     BE_TRY(be_bloch_assemble_chunk(ctx, ctx->bloch, loop0, cnt, N, s.Bw));   // H(k) generated into the work copy
-  } else {
+  } else if (!ctx->feed) {
     const int nchunk = (int)(((int64_t)N * N + 2047) / 2048);
     k_gather<<<(unsigned)(cnt * nchunk), 256, 0, st>>>(H, s.Bw, map, loop0, N, nchunk);
     LAUNCH_CHECK();
@@ -852,7 +852,30 @@ int be_eigh_large(be_ctx* ctx, const cplx* H, const GridMap& map, int64_t loop0,
   // vectors) 905 vs 1035 ms per 300 matrices, N = 800 (all vectors) 215 vs 203 ms, N = 400 even
   const bool two_stage = N >= BE_BAND_MINN && N <= BE_BAND_MAXN &&
                          (ctx->eigh_algo == 1 || (ctx->eigh_algo == 2 && N >= BE_BAND_AUTON));
-  if (two_stage) BE_TRY(be_band_reduce(ctx, s.Bw, cnt, N, s.d, s.e, s.tau, s.band));
+  if (ctx->feed) {
+    // host grid streamed into this chunk (HostFeed, be_common.cuh): gather sub-range j when its copy has landed,
+    // hand the staging buffer back, and reduce the sub-range to band form while the next one travels
+    HostFeed* f = ctx->feed;
+    ctx->feed = nullptr;
+    if (!two_stage || f->mstart[f->nsub] != cnt) return BE_ERR_UNSUPPORTED;   // the caller checks both
+    GridMap fm;
+    memset(&fm, 0, sizeof(fm));
+    fm.ndim = 1; fm.dir = 0; fm.n1 = 1; fm.dims[0] = 1; fm.batch_stride = 1;
+    const int nchunk = (int)(((int64_t)N * N + 2047) / 2048);
+    for (int j = 0; j < f->nsub; ++j) {
+      const int64_t c0 = f->mstart[j], cs = f->mstart[j + 1] - c0;
+      fm.loops = cs;
+      BE_CUDA(cudaStreamWaitEvent(st, f->copied[j & 1], 0));
+      k_gather<<<(unsigned)(cs * nchunk), 256, 0, st>>>((const cplx*)f->buf[j & 1], s.Bw + c0 * (int64_t)N * N, fm, 0, N, nchunk);
+      LAUNCH_CHECK();
+      BE_CUDA(cudaEventRecord(f->freed[j & 1], st));
+      if (j + 2 < f->nsub) BE_TRY(f->issue(f->self, j + 2));
+      BE_TRY(be_band_stage1(ctx, s.Bw + c0 * (int64_t)N * N, cs, N, s.tau + c0 * N, s.band));
+    }
+    BE_TRY(be_band_stage2(ctx, s.Bw, cnt, N, s.d, s.e, s.band));
+  } else if (two_stage) {
+    BE_TRY(be_band_reduce(ctx, s.Bw, cnt, N, s.d, s.e, s.tau, s.band));
+  }
   for (int p = 0; p < N && !on_chip && !two_stage; p += nb) {
     if (p > 0 && N - p <= TS_MAXN) {
       // the trailing block is up to date at a panel boundary and fits one CTA's shared memory: its ~100

@@ -617,6 +617,29 @@ def test_only_the_upper_triangle_of_H_is_read(ctx):
     assert phase_dist(th0.numpy(), th0o) <= PH_TOL
 
 
+def test_host_grid_streamed_into_one_chunk(ctx):
+    """N = 1024 (two-stage eigensolver): the host variant feeds ONE chunk in three sub-ranges (1 + 1 + 2 loops), stage 1
+    per sub-range, the rest over the whole batch.  Same phases as the device-resident call and as the oracle (one
+    loop), with the unused triangle poisoned on the host."""
+    _need_memory(6, ctx)
+    parts = wl.config4_parts(16, axis="x")
+    H = wl.supercell_grid([parts], 5, 24, t2_indices=[0, 7, 13, 22])
+    S = wl.supercell_spin_z(16)
+    Hp = H.copy()
+    il = np.tril_indices(1024, -1)
+    Hp[..., il[0], il[1]] = np.nan
+    lo, hi, pso = ctx.spin_resolved_wilson_host(torch.from_numpy(Hp).pin_memory(), 512, 1, torch.from_numpy(S))
+    assert ctx.host_schedule() == -3
+    lod, hid, psod = ctx.spin_resolved_wilson(dev(H), 512, 1, dev(S))
+    assert phase_dist(lo.numpy(), lod.cpu().numpy()) < 1e-10 and phase_dist(hi.numpy(), hid.cpu().numpy()) < 1e-10
+    assert (pso - psod.cpu()).abs().max() < 1e-10
+    loo, hio, _ = wo.spin_resolved_surface(H[:, 2:3], 512, 1, S)
+    assert phase_dist(lo.numpy()[2:3], loo) <= PH_TOL and phase_dist(hi.numpy()[2:3], hio) <= PH_TOL
+    th, _, mg = ctx.wilson_loop_host(torch.from_numpy(Hp).pin_memory(), 512, 1)
+    thd, _, mgd = ctx.wilson_loop(dev(H), 512, 1)
+    assert phase_dist(th.numpy(), thd.cpu().numpy()) < 1e-10 and (mg - mgd.cpu()).abs().max() < 1e-10
+
+
 def test_chunk_pipeline_matches_single_chunk_and_oracle(ctx):
     """A small workspace cap splits the loops into >= 3 chunks: the two-stream chunk pipeline
     (tridiagonalization of chunk c+1 next to the rest of chunk c, two scratch regions) must give
