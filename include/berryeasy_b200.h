@@ -137,7 +137,8 @@ int be_profile_get(be_ctx* ctx, int cls, double* ms, int64_t* launches, double* 
 /*
  * S1 -- batched Hermitian eigensolve ("exact diagonalization of a discretized
  * Hamiltonian at many points in reciprocal space").
- *   dH     [count][N][N] complex128, Hermitian, not modified.
+ *   dH     [count][N][N] complex128, Hermitian, not modified.  Only the row-major upper triangle (diagonal
+ *          included) is read, here and in every call that takes an H_grid.
  *   dE     [count][N] double: all eigenvalues, ascending.
  *   dU     [count][N][n_vec] complex128, may be NULL: U[c][r][v] = component r of the eigenvector of
  *          the v-th lowest eigenvalue; columns orthonormal.  0 <= n_vec <= N.
@@ -309,10 +310,15 @@ int be_plaquette_flux(be_ctx* ctx, const void* dH_grid, const be_grid* grid, int
 /*
  * Host-buffer variants (end-to-end path): h* pointers are host memory (pinned recommended).  The
  * grid is streamed to the device in chunks of whole loops, overlapped with compute on an internal
- * copy stream; results are copied back before return.  Chunks: matrices of order >= 800 in TWO chunks, the
- * first just long enough to hide the copy of the second (24 loops of N = 1600: 3 + 21); smaller ones in
- * growing chunks (1/8 of the loops, 1/4, ... or multiples of a wave of SMs), so that only the first, small copy
- * is exposed.  Semantics as the device calls above; any loop direction.
+ * copy stream; results are copied back before return.  Schedule (be_host_schedule reports it):
+ *   - two-stage eigensolver (N >= 1024, default algorithm) and workspace for all loops at once: ONE chunk, fed in
+ *     three sub-ranges of loops (24 loops of N = 1600: 3 + 7 + 14); only the first stage of the eigensolver runs per
+ *     sub-range, while the next one travels; everything else runs over the whole batch;
+ *   - else N >= 800: TWO chunks, the first just long enough to hide the copy of the second;
+ *   - smaller matrices: growing chunks (1/8 of the loops, 1/4, ... or multiples of a wave of SMs),
+ *   so that only the first, small copy is exposed.  Semantics as the device calls above; any loop direction.
+ *   The default workspace cap is 85 % of the device memory here (the grid is not device resident); a cap set
+ *   with be_set_workspace_limit stands.
  *   Which bytes travel: H(k) is Hermitian and the eigensolver reads only its row-major UPPER triangle
  *   (diagonal included; the other triangle may hold anything, on the host and on the device).  For
  *   N >= 256 each matrix is copied as 8 row blocks, block b with the columns from its first row on: 56 % of

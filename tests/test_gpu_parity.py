@@ -580,11 +580,11 @@ def test_host_variants_match_device(ctx):
 
 
 def test_only_the_upper_triangle_of_H_is_read(ctx):
-    """Header contract of the host variants: for N > 104 the eigensolver reads the row-major upper triangle only, so the
-    host variants copy just that (N >= 256, 8 row blocks).  NaN in the other triangle must change nothing, on the
+    """Header contract: the eigensolver (Jacobi, on-chip, one- and two-stage paths) reads the row-major upper triangle
+    only, so the host variants copy just that (N >= 256, 8 row blocks).  NaN in the other triangle must change nothing, on the
     device (one- and two-stage solver) and through the triangle-block host copy, both loop directions."""
     rng = np.random.default_rng(7)
-    for N, algo in ((105, 0), (144, 1), (256, 0), (264, 1)):
+    for N, algo in ((4, 0), (8, 0), (16, 0), (64, 0), (104, 0), (105, 0), (144, 1), (256, 0), (264, 1)):
         A = rng.standard_normal((3, N, N)) + 1j * rng.standard_normal((3, N, N))
         H = (A + A.conj().transpose(0, 2, 1)) / 2
         Hp = H.copy()
