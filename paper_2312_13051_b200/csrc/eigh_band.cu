@@ -922,14 +922,14 @@ __device__ __forceinline__ void cp_async16_z(void* sdst, const void* gsrc, bool 
 }
 
 __global__ void __launch_bounds__(QS * Q2_TSG_MAX, 1) k_q2(const cplx* __restrict__ Bw, cplx* __restrict__ X, int N, int nv,
-                                                          int tsg) {
+                                                          int tsg, int col0) {
   extern __shared__ __align__(16) cplx qsm[];
   cplx* vs = qsm;                                  // [2][QS][QG * KB]
   cplx* hand = qsm + 2 * QS * QG * KB;             // [2][QS][KB][tsg]: input rows of stage j (j = 0: from memory)
   const int64_t c = blockIdx.y;
   const cplx* __restrict__ Bc = Bw + c * (int64_t)N * N;
   const int j = threadIdx.x / tsg, tcol = threadIdx.x - j * tsg;
-  const int v = blockIdx.x * tsg + tcol;
+  const int v = col0 + blockIdx.x * tsg + tcol;
   const bool act = v < nv;
   cplx* __restrict__ x = X + (c * nv + (act ? v : 0)) * (int64_t)N;
   const int nsuper = (N - 1 + QS * QG - 1) / (QS * QG);
@@ -1173,14 +1173,24 @@ int be_band_stage2(be_ctx* ctx, cplx* Bw, int64_t cnt, int N, double* d, double*
 
 int be_band_q2(be_ctx* ctx, const cplx* Bw, cplx* X, int64_t cnt, int N, int nv) {
   if (nv <= 0) return BE_OK;
-  // columns per CTA: a divisor-friendly multiple of 32 (nv = 800 -> 7 CTAs of 128 columns)
-  int nslab = (nv + Q2_TSG_MAX - 1) / Q2_TSG_MAX;
-  int tsg = (((nv + nslab - 1) / nslab) + 31) / 32 * 32;
-  nslab = (nv + tsg - 1) / tsg;
-  const size_t smem = ((size_t)2 * QS * QG * KB + (size_t)2 * QS * KB * tsg) * sizeof(cplx);
-  BE_CUDA(cudaFuncSetAttribute(k_q2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  // Columns per CTA: whole slabs of Q2_TSG_MAX columns, and the rest (nv = 800: 6 x 128 + 32) in a grid of its own
+  // with narrow CTAs.  A CTA takes the same time whatever share of its warps is active (the 32 leftover columns in a
+  // seventh 128-column slab cost a full slab: 135.6 ms per 148 matrices for nv = 800 .. 896 against 116.3 for 768),
+  // but four 96-thread CTAs fit an SM where one 384-thread CTA does.
+  const int nfull = nv / Q2_TSG_MAX;
+  const int rem = nv - nfull * Q2_TSG_MAX;
+  const int tsg_tail = (rem + 31) / 32 * 32;
   be_prof_begin(ctx, PK_Q2);
-  k_q2<<<dim3((unsigned)nslab, (unsigned)cnt), QS * tsg, smem, ctx->stream>>>(Bw, X, N, nv, tsg);
+  for (int part = 0; part < 2; ++part) {
+    const int tsg = part == 0 ? Q2_TSG_MAX : tsg_tail;
+    const int nslab = part == 0 ? nfull : (rem > 0 ? 1 : 0);
+    if (nslab == 0) continue;
+    const size_t smem = ((size_t)2 * QS * QG * KB + (size_t)2 * QS * KB * tsg) * sizeof(cplx);
+    BE_CUDA(cudaFuncSetAttribute(k_q2, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)(((size_t)2 * QS * QG * KB + (size_t)2 * QS * KB * Q2_TSG_MAX) * sizeof(cplx))));
+    k_q2<<<dim3((unsigned)nslab, (unsigned)cnt), QS * tsg, smem, ctx->stream>>>(Bw, X, N, nv, tsg, part == 0 ? 0 : nfull * Q2_TSG_MAX);
+    if (part == 0 && rem > 0) LAUNCH_CHECK();
+  }
   be_prof_end(ctx, PK_Q2, (double)cnt * nv * N * 16.0 * ((N + QS * QG - 1) / (QS * QG)), (double)cnt * 8.0 * N * (double)N * nv);
   LAUNCH_CHECK();
   return BE_OK;
