@@ -160,6 +160,7 @@ extern "C" int be_destroy(be_ctx* ctx) {
     cudaEventDestroy(ctx->ev_split); cudaEventDestroy(ctx->ev_join);
     cudaEventDestroy(ctx->ev_region[0]); cudaEventDestroy(ctx->ev_region[1]);
   }
+  if (ctx->side_stream) { cudaStreamDestroy(ctx->side_stream); cudaEventDestroy(ctx->ev_side[0]); cudaEventDestroy(ctx->ev_side[1]); }
   if (ctx->prof) { for (cudaEvent_t e : ctx->prof->ev) cudaEventDestroy(e); delete ctx->prof; }
   delete ctx;
   return BE_OK;

@@ -95,6 +95,8 @@ struct be_ctx {
   const struct BlochSrc* bloch;   // set while the H eigensolve of a *_bloch call runs: H(k) is assembled, not read
   int chunk_pipeline;         // be_set_chunk_pipeline (default 0)
   int band_lo;                // band window [band_lo, band_lo + m) of the running Wilson call (0 = lowest m bands)
+  cudaStream_t side_stream;   // k_q2: the grid of narrow CTAs runs here, next to the grid of full slabs
+  cudaEvent_t ev_side[2];
   int split_after_tridiag;    // consumed by be_eigh_large: switch to stream2 after S1a
   int gemm_pad;               // zgemm launches with padded shared memory: at most one GEMM CTA per SM,
                               // leaving room for one k_hemv CTA of the other stream

@@ -1180,16 +1180,34 @@ int be_band_q2(be_ctx* ctx, const cplx* Bw, cplx* X, int64_t cnt, int N, int nv)
   const int nfull = nv / Q2_TSG_MAX;
   const int rem = nv - nfull * Q2_TSG_MAX;
   const int tsg_tail = (rem + 31) / 32 * 32;
+  // The two grids run side by side (the narrow one on ctx->side_stream): a full-slab CTA owns the register file of
+  // its SM, so the narrow CTAs take whole SMs too, four at a time, and the block scheduler packs the two kinds -- no
+  // nearly empty last round of either grid (600 matrices, nv = 800: 24.3 rounds of full slabs + 1.01 of narrow CTAs).
+  const bool both = nfull > 0 && rem > 0;
+  if (both && !ctx->side_stream) {
+    BE_CUDA(cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking));
+    BE_CUDA(cudaEventCreateWithFlags(&ctx->ev_side[0], cudaEventDisableTiming));
+    BE_CUDA(cudaEventCreateWithFlags(&ctx->ev_side[1], cudaEventDisableTiming));
+  }
+  BE_CUDA(cudaFuncSetAttribute(k_q2, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               (int)(((size_t)2 * QS * QG * KB + (size_t)2 * QS * KB * Q2_TSG_MAX) * sizeof(cplx))));
   be_prof_begin(ctx, PK_Q2);
+  if (both) {
+    BE_CUDA(cudaEventRecord(ctx->ev_side[0], ctx->stream));
+    BE_CUDA(cudaStreamWaitEvent(ctx->side_stream, ctx->ev_side[0], 0));
+  }
   for (int part = 0; part < 2; ++part) {
     const int tsg = part == 0 ? Q2_TSG_MAX : tsg_tail;
     const int nslab = part == 0 ? nfull : (rem > 0 ? 1 : 0);
     if (nslab == 0) continue;
     const size_t smem = ((size_t)2 * QS * QG * KB + (size_t)2 * QS * KB * tsg) * sizeof(cplx);
-    BE_CUDA(cudaFuncSetAttribute(k_q2, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)(((size_t)2 * QS * QG * KB + (size_t)2 * QS * KB * Q2_TSG_MAX) * sizeof(cplx))));
-    k_q2<<<dim3((unsigned)nslab, (unsigned)cnt), QS * tsg, smem, ctx->stream>>>(Bw, X, N, nv, tsg, part == 0 ? 0 : nfull * Q2_TSG_MAX);
+    cudaStream_t qs = (part == 1 && both) ? ctx->side_stream : ctx->stream;
+    k_q2<<<dim3((unsigned)nslab, (unsigned)cnt), QS * tsg, smem, qs>>>(Bw, X, N, nv, tsg, part == 0 ? 0 : nfull * Q2_TSG_MAX);
     if (part == 0 && rem > 0) LAUNCH_CHECK();
+  }
+  if (both) {
+    BE_CUDA(cudaEventRecord(ctx->ev_side[1], ctx->side_stream));
+    BE_CUDA(cudaStreamWaitEvent(ctx->stream, ctx->ev_side[1], 0));
   }
   be_prof_end(ctx, PK_Q2, (double)cnt * nv * N * 16.0 * ((N + QS * QG - 1) / (QS * QG)), (double)cnt * 8.0 * N * (double)N * nv);
   LAUNCH_CHECK();
