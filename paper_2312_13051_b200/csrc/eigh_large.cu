@@ -268,8 +268,8 @@ __global__ void __launch_bounds__(HEMV_THREADS, 2) k_hemv(const cplx* __restrict
 //           is generated (zlarfg): d[ic], e[ic], tau[ic], v stored in place with a unit head.
 // With both flags the V and W panels are read ONCE: the column update of ic is accumulated in the
 // same sweep that corrects y, the term of the new reflector i is added from shared memory.
-constexpr int CW_THREADS = 320;   // 3 CTAs per SM: a chunk of 300 matrices is resident in one wave on 148 SMs
-__global__ void __launch_bounds__(CW_THREADS, 3) k_colw(cplx* __restrict__ Bw, cplx* __restrict__ Wp,
+constexpr int CW_THREADS = 192;   // 5 CTAs per SM: a chunk of 600 matrices is resident in one wave on 148 SMs (320 threads, 3 per SM: two rounds, 38.6 ms)
+__global__ void __launch_bounds__(CW_THREADS, 5) k_colw(cplx* __restrict__ Bw, cplx* __restrict__ Wp,
                                                      const cplx* __restrict__ P, const cplx* __restrict__ zpart,
                                                      const cplx* __restrict__ pqg, double* __restrict__ dd,
                                                      double* __restrict__ ee, cplx* __restrict__ tau,
