@@ -462,7 +462,7 @@ int be_cluster_orth(be_ctx* ctx, const double* lam, const double* tnorm, const i
     LAUNCH_CHECK();
   }
   // few matrices: several CTAs per matrix (many: the machine is full anyway, and most CTAs would find nothing to do)
-  const int split = cnt * ORTH_SMALL_SPLIT <= 16 * (int64_t)ctx->sm_count ? ORTH_SMALL_SPLIT : 1;
+  const int split = cnt * ORTH_SMALL_SPLIT <= 32 * (int64_t)ctx->sm_count ? ORTH_SMALL_SPLIT : 1;
   k_orth_small<<<dim3((unsigned)cnt, (unsigned)split), 256, 0, st>>>(blk, Z, N, nv, cb, info);
   LAUNCH_CHECK();
   be_prof_end(ctx, PK_ORTH, 0.0, 0.0);
